@@ -1,0 +1,317 @@
+"""fp64 CPU ORACLE for the 2HOT tree-force path — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package.  It shares no code with paper_1407_2600_b200 (the CUDA path) and never calls it.
+
+Written from SURVEY.md §8(c) (readings O1..O9 of PAPER.md:57-79).  Thin ctypes layer over the plain C
+in this directory; this file holds no arithmetic of the method except the KDK composition `kdk_step`
+(O9), which is three lines of the leapfrog around the C force routines.
+
+Pins (tests/test_oracle_*.py, `-m "not gpu"`): keys (corner cases, bit positions, brute-force
+interleave), sort (numpy stable argsort, adversarial inputs), tree (invariants + spatial brute force),
+moments (M2M == direct P2M, closed forms), b_n/M2P (closed forms, finite differences, convergence
+rate), direct sum (two-body, momentum, uniform/Plummer sphere), tree -> direct as theta -> 0, Ewald
+(alpha independence, 2.837297/L, 4 pi/3 limit, symmetric zero points), far field (Taylor vs direct,
+trace relations, perfect lattice), KDK (time reversal, free drift, Zel'dovich).  Nothing here is
+"parity unpinned".
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+NLEAF = 16
+NCRIT = 64
+WS = 2     # measured: WS = 1 floors the periodic force error at ~3e-3 on near-lattice inputs
+KEY_LEVELS = 21
+FAR_ORDER = 8
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        _lib = C.CDLL(path)
+        _lib.orc_tree_build.restype = C.c_void_p
+        _lib.orc_tree_ncell.restype = C.c_int64
+        _lib.orc_tree_ngroup.restype = C.c_int64
+        _lib.orc_ewald_self.restype = C.c_double
+        _lib.orc_farfield_phi.restype = C.c_double
+        _lib.orc_get_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None else None
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _sink(sink):
+    if sink is None:
+        return None
+    return np.ascontiguousarray(sink, dtype=np.int64)
+
+
+def nparams(p):
+    return (p + 1) * (p + 2) * (p + 3) // 6
+
+
+def midx(a, b, c):
+    l, k = a + b + c, b + c
+    return l * (l + 1) * (l + 2) // 6 + k * (k + 1) // 2 + c
+
+
+def mtable(p):
+    """exponent triples in the interface order (rank ascending, a descending, b descending)"""
+    out = []
+    for l in range(p + 1):
+        for a in range(l, -1, -1):
+            for b in range(l - a, -1, -1):
+                out.append((a, b, l - a - b))
+    return out
+
+
+def threads():
+    return int(lib().orc_get_threads())
+
+
+def set_threads(n):
+    lib().orc_set_threads(C.c_int(int(n)))
+
+
+# ---- O1 / O2 -------------------------------------------------------------------------------------
+def keys(pos, box=1.0, periodic=False):
+    pos = _f32(pos)
+    n = pos.shape[0]
+    key = np.empty(n, dtype=np.uint64)
+    wrapped = np.empty_like(pos)
+    err = lib().orc_keys(C.c_int64(n), _p(pos), C.c_float(box), C.c_int(int(periodic)), _p(key), _p(wrapped))
+    if err:
+        raise ValueError(f"orc_keys error {err}")
+    return key, wrapped
+
+
+def sort(key):
+    key = np.ascontiguousarray(key, dtype=np.uint64)
+    n = key.shape[0]
+    skey = np.empty(n, dtype=np.uint64)
+    order = np.empty(n, dtype=np.uint32)
+    lib().orc_sort(C.c_int64(n), _p(key), _p(skey), _p(order))
+    return skey, order
+
+
+# ---- O3-O6 ---------------------------------------------------------------------------------------
+class OracleTree:
+    def __init__(self, pos, mass, box=1.0, periodic=False, nleaf=NLEAF, ncrit=NCRIT):
+        self.pos = _f32(pos)
+        self.mass = _f32(mass)
+        self.n = self.pos.shape[0]
+        self.box = float(box)
+        self.periodic = bool(periodic)
+        err = C.c_int(0)
+        self._h = lib().orc_tree_build(C.c_int64(self.n), _p(self.pos), _p(self.mass), C.c_float(box),
+                                       C.c_int(int(periodic)), C.c_int(nleaf), C.c_int(ncrit), C.byref(err))
+        if not self._h:
+            raise ValueError(f"orc_tree_build error {err.value}")
+        self._h = C.c_void_p(self._h)
+        self.ncell = int(lib().orc_tree_ncell(self._h))
+        self.ngroup = int(lib().orc_tree_ngroup(self._h))
+        self.p = -1
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().orc_tree_free(self._h)
+            self._h = None
+
+    def sorted(self):
+        skey = np.empty(self.n, dtype=np.uint64)
+        order = np.empty(self.n, dtype=np.uint32)
+        lib().orc_tree_get_sorted(self._h, _p(skey), _p(order))
+        return skey, order
+
+    def wrapped_pos(self):
+        out = np.empty((self.n, 3), dtype=np.float32)
+        lib().orc_tree_get_wrapped(self._h, _p(out))
+        return out
+
+    def cells(self):
+        nc = self.ncell
+        d = dict(hotkey=np.empty(nc, np.uint64), first=np.empty(nc, np.int64), count=np.empty(nc, np.int64),
+                 nchild=np.empty(nc, np.int32), child0=np.empty(nc, np.int64), level=np.empty(nc, np.int32))
+        lib().orc_tree_get_cells(self._h, _p(d["hotkey"]), _p(d["first"]), _p(d["count"]), _p(d["nchild"]),
+                                 _p(d["child0"]), _p(d["level"]))
+        return d
+
+    def groups(self):
+        ng = self.ngroup
+        d = dict(cell=np.empty(ng, np.int64), first=np.empty(ng, np.int64), count=np.empty(ng, np.int64),
+                 bbox=np.empty((ng, 6), np.float32))
+        lib().orc_tree_get_groups(self._h, _p(d["cell"]), _p(d["first"]), _p(d["count"]), _p(d["bbox"]))
+        return d
+
+    def moments(self, p):
+        """fill and return (mass[ncell], com[ncell,3], delta[ncell], M[ncell,NP(p)]) — raw moments"""
+        lib().orc_moments(self._h, C.c_int(p))
+        self.p = p
+        nc, npar = self.ncell, nparams(p)
+        cm = np.empty(nc); com = np.empty((nc, 3)); dl = np.empty(nc); mom = np.empty((nc, npar))
+        lib().orc_tree_get_moments(self._h, _p(cm), _p(com), _p(dl), _p(mom))
+        return cm, com, dl, mom
+
+    def moments_m2m(self, p):
+        if self.p != p:
+            self.moments(p)
+        out = np.empty((self.ncell, nparams(p)))
+        lib().orc_moments_m2m(self._h, C.c_int(p), _p(out))
+        return out
+
+    def accel(self, eps, theta, p, sink=None, ws=WS, want_pot=True):
+        """Tr over the explicit image block only (the far field is added by tree_force)."""
+        if self.p != p:
+            self.moments(p)
+        sink = _sink(sink)
+        ns = self.n if sink is None else sink.shape[0]
+        acc = np.empty((ns, 3)); pot = np.empty(ns) if want_pot else None
+        n_p2p = C.c_int64(0); n_m2p = C.c_int64(0)
+        err = lib().orc_tree_accel(self._h, C.c_double(eps), C.c_double(theta), C.c_int(ws), C.c_int64(ns),
+                                   _p(sink), _p(acc), _p(pot), C.byref(n_p2p), C.byref(n_m2p))
+        if err:
+            raise RuntimeError(f"orc_tree_accel error {err}")
+        return acc, pot, int(n_p2p.value), int(n_m2p.value)
+
+    def list_counts(self, theta, g, ws=WS):
+        a = C.c_int64(0); b = C.c_int64(0); c = C.c_int64(0)
+        lib().orc_group_list_counts(self._h, C.c_double(theta), C.c_int(ws), C.c_int64(g), C.byref(a),
+                                    C.byref(b), C.byref(c))
+        return int(a.value), int(b.value), int(c.value)
+
+
+def tree_force(pos, mass, box, periodic, eps, theta, p, sink=None, tree=None, ws=WS):
+    """The whole oracle path Tr: tree sum over the image block (+ O7 far field when periodic).
+    Returns acc, pot, n_p2p, n_m2p, tree."""
+    if tree is None:
+        tree = OracleTree(pos, mass, box, periodic)
+    acc, pot, n_p2p, n_m2p = tree.accel(eps, theta, p, sink, ws)
+    if periodic:
+        wp = tree.wrapped_pos()
+        lam = farfield_local(wp, mass, box, ws)
+        fa, fp = farfield_eval(lam, box, wp, sink)
+        acc = acc + fa
+        pot = pot + fp
+    return acc, pot, n_p2p, n_m2p, tree
+
+
+def bn(pmax, r, eps2):
+    r = np.ascontiguousarray(r, dtype=np.float64)
+    b = np.empty(nparams(pmax))
+    lib().orc_bn(C.c_int(pmax), _p(r), C.c_double(eps2), _p(b))
+    return b
+
+
+def m2p(p, mom, r, eps2):
+    mom = np.ascontiguousarray(mom, dtype=np.float64)
+    r = np.ascontiguousarray(r, dtype=np.float64)
+    acc = np.zeros(3); pot = C.c_double(0.0)
+    lib().orc_m2p(C.c_int(p), _p(mom), _p(r), C.c_double(eps2), _p(acc), C.byref(pot))
+    return acc, pot.value
+
+
+# ---- D ---------------------------------------------------------------------------------------------
+def direct_iso(pos, mass, eps, sink=None):
+    pos = _f32(pos); mass = _f32(mass); sink = _sink(sink)
+    n = pos.shape[0]; ns = n if sink is None else sink.shape[0]
+    acc = np.empty((ns, 3)); pot = np.empty(ns)
+    lib().orc_direct_iso(C.c_int64(n), _p(pos), _p(mass), C.c_double(eps), C.c_int64(ns), _p(sink), _p(acc), _p(pot))
+    return acc, pot
+
+
+def direct_per(pos, mass, box, eps, sink=None, ws=WS, alpha=None, pairwise=False):
+    pos = _f32(pos); mass = _f32(mass); sink = _sink(sink)
+    n = pos.shape[0]; ns = n if sink is None else sink.shape[0]
+    alpha = 2.0 / box if alpha is None else alpha
+    acc = np.empty((ns, 3)); pot = np.empty(ns)
+    fn = lib().orc_direct_per_pairwise if pairwise else lib().orc_direct_per
+    fn(C.c_int64(n), _p(pos), _p(mass), C.c_double(box), C.c_double(eps), C.c_int(ws), C.c_double(alpha),
+       C.c_int64(ns), _p(sink), _p(acc), _p(pot))
+    return acc, pot
+
+
+def ewald_pair(x, L=1.0, alpha=None, nmax=-1, hmax=-1):
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    alpha = 2.0 / L if alpha is None else alpha
+    psi = C.c_double(0.0); a = np.empty(3)
+    lib().orc_ewald_pair(_p(x), C.c_double(L), C.c_double(alpha), C.c_int(nmax), C.c_int(hmax), C.byref(psi), _p(a))
+    return psi.value, a
+
+
+def ewald_self(L=1.0, alpha=None):
+    alpha = 2.0 / L if alpha is None else alpha
+    return float(lib().orc_ewald_self(C.c_double(L), C.c_double(alpha), C.c_int(-1), C.c_int(-1)))
+
+
+# ---- O7 --------------------------------------------------------------------------------------------
+def farfield_T(L=1.0, ws=WS, order=FAR_ORDER):
+    T = np.empty(nparams(order))
+    lib().orc_farfield_T(C.c_double(L), C.c_int(ws), C.c_int(order), _p(T))
+    return T
+
+
+def farfield_phi(u, L=1.0, ws=WS):
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    a = np.empty(3)
+    phi = lib().orc_farfield_phi(_p(u), C.c_double(L), C.c_int(ws), _p(a))
+    return float(phi), a
+
+
+def farfield_local(pos, mass, L=1.0, ws=WS, order=FAR_ORDER):
+    pos = _f32(pos); mass = _f32(mass)
+    lam = np.empty(nparams(order))
+    lib().orc_farfield_local(C.c_int64(pos.shape[0]), _p(pos), _p(mass), C.c_double(L), C.c_int(ws),
+                             C.c_int(order), _p(lam))
+    return lam
+
+
+def farfield_eval(lam, L, pos, sink=None, order=FAR_ORDER):
+    pos = _f32(pos); sink = _sink(sink)
+    ns = pos.shape[0] if sink is None else sink.shape[0]
+    acc = np.empty((ns, 3)); pot = np.empty(ns)
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    lib().orc_farfield_eval(_p(lam), C.c_int(order), C.c_double(L), C.c_int64(ns), _p(pos), _p(sink), _p(acc), _p(pot))
+    return acc, pot
+
+
+# ---- O9 --------------------------------------------------------------------------------------------
+def kdk_factors(periodic, mtot, box, a, da):
+    k1 = C.c_double(0); d = C.c_double(0); k2 = C.c_double(0)
+    lib().orc_kdk_factors(C.c_int(int(periodic)), C.c_double(mtot), C.c_double(box), C.c_double(a),
+                          C.c_double(da), C.byref(k1), C.byref(d), C.byref(k2))
+    return k1.value, d.value, k2.value
+
+
+def kdk_step(pos, vel, mass, box, periodic, eps, theta, p, a, da, acc=None, force=None):
+    """One KDK step (O9).  State is fp32 (positions/velocities are 32-bit floats); the
+    arithmetic of each update is fp64 and the result is rounded once to fp32.  `acc` is the cached
+    force at `pos` (None: computed first).  `force(pos)` defaults to the oracle tree force Tr.
+    Returns pos', vel', acc' (acc' = force at pos', to be passed to the next step)."""
+    pos = _f32(pos).copy(); vel = _f32(vel).copy(); mass = _f32(mass)
+    if force is None:
+        def force(x):
+            return tree_force(x, mass, box, periodic, eps, theta, p)[0]
+    mtot = float(np.sum(mass.astype(np.float64)))
+    k1, d, k2 = kdk_factors(periodic, mtot, box, a, da)
+    if acc is None:
+        acc = force(pos)
+    vel = (vel.astype(np.float64) + acc * k1).astype(np.float32)
+    pos = (pos.astype(np.float64) + vel.astype(np.float64) * d).astype(np.float32)
+    if periodic:
+        pos = keys(pos, box, True)[1]          # the fp32 wrap of O1
+    acc = force(pos)
+    vel = (vel.astype(np.float64) + acc * k2).astype(np.float32)
+    return pos, vel, acc
