@@ -1,0 +1,127 @@
+/* dsk.h — C ABI of libdsk: B200-native tree gravity, the force path of 2HOT
+ * (arxiv 1407.2600 "Dark Sky Simulations: Early Data Release").
+ *
+ * The operation: the gravitational field of N bodies is evaluated in O(N log N)
+ * by approximating distant groups of bodies with truncated (order-p) multipole expansions held in the
+ * cells of an oct-tree.  Stages: a Morton key per particle -> sort along the
+ * space-filling curve -> oct-tree whose topology the keys define -> multipole moments of every cell
+ * (upward pass) -> per sink group a traversal under a multipole acceptance test that yields the list
+ * of cells to take as multipoles and the list of leaves to take particle by particle -> evaluation
+ * of those lists (m sources x n sinks blocks) -> periodic boundary conditions through a
+ * p = 8 local expansion of the far images -> symplectic leapfrog update.
+ * The exact definitions (key bit layout, tree rule, MAC, expansion, softening, periodic split) are
+ * the readings O1..O9 in DESIGN.md; G = 1.
+ *
+ * Conventions
+ *  - Every array argument is a DEVICE pointer owned by the caller (e.g. a torch tensor's data_ptr())
+ *    unless it says "host".  Layout: pos/vel/acc are AoS float32 [N,3] (the paper's particle record is
+ *    32-bit x,y,z,vx,vy,vz); mass/pot float32 [N].  Outputs are in CALLER order.
+ *  - The library allocates no device memory for its working set: the caller lends one workspace of
+ *    dsk_workspace_bytes() bytes (256-byte aligned) with dsk_bind_workspace(); it must stay valid and
+ *    untouched until dsk_destroy().  (A 4 KiB pinned host page and a few events are owned by the ctx.)
+ *  - All device work is enqueued on the bound CUDA stream (default: the legacy default stream).  Each
+ *    call that can fail on the device ends with ONE small device->host read of a status/counter block
+ *    and a stream synchronise; everything before it is asynchronous.
+ *  - Return value: 0 = DSK_OK, negative = error (below).  No exceptions, no printing, no global state.
+ *    Calls on one context are not thread-safe; different contexts are independent.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns DSK_ECUDA.
+ *
+ * Multi-index order of moment arrays (interface convention): n = (a,b,c), rank l = a+b+c,
+ * index(n) = l(l+1)(l+2)/6 + (b+c)(b+c+1)/2 + c  (ranks ascending; a descending, then b descending),
+ * N_p = (p+1)(p+2)(p+3)/6 entries.
+ */
+#ifndef DSK_H
+#define DSK_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DSK_OK             0
+#define DSK_EINVAL        -1   /* bad argument (N <= 0, p not in {2,4,6,8}, theta not in (0,1], ...)   */
+#define DSK_ENOWORKSPACE  -2   /* no workspace bound, or it is too small / misaligned                  */
+#define DSK_ENOTREE       -3   /* dsk_accel / getters before a successful dsk_build_tree               */
+#define DSK_EOUTOFBOX     -4   /* isolated mode: a position outside [0, box)                           */
+#define DSK_ENONFINITE    -5   /* NaN or Inf position                                                  */
+#define DSK_ELISTOVERFLOW -6   /* traversal stack or interaction-list buffer exhausted                 */
+#define DSK_ECUDA         -7   /* CUDA runtime error (no device, launch failure, ...)                  */
+#define DSK_ECELLOVERFLOW -8   /* more tree cells than the workspace was sized for                     */
+
+typedef struct dsk_ctx dsk_ctx;      /* opaque; created by dsk_create, released by dsk_destroy        */
+
+/* Counters and timings of the last dsk_build_tree / dsk_accel / dsk_kdk_step (host struct).
+ * Interactions are USEFUL ones: sum over groups of n_sink x n_listed (self pairs included in n_p2p).
+ * ms_* are CUDA-event times on the bound stream of the last call that ran that phase. */
+typedef struct dsk_stats {
+    int64_t n, ncell, nleaf_cells, ngroup, nlevel;
+    int64_t n_p2p;            /* particle-particle interactions                                        */
+    int64_t n_m2p;            /* cell-particle interactions                                            */
+    int64_t list_m2p;         /* total M2P list entries (cells) over all groups                        */
+    int64_t list_p2p;         /* total P2P list entries (leaves) over all groups                       */
+    int64_t nbatch;           /* list batches the evaluation was split in                              */
+    float ms_key, ms_sort, ms_build, ms_upward, ms_group, ms_walk, ms_p2p, ms_m2p, ms_far, ms_scatter,
+          ms_kdk;
+} dsk_stats;
+
+/* Create a context for N particles in the cube [0, box)^3.  PAPER.md:61-63; O1-O7.
+ *   periodic : 0 isolated, 1 periodic (explicit (2 WS+1)^3 image block + order-8 far field)
+ *   eps      : Plummer softening length (> 0);  theta : opening angle, 0 < theta <= 1
+ *   p        : expansion order = highest multipole rank kept, one of 2, 4, 6, 8
+ * Host-only work (the lattice tensors of the far field are computed here in fp64). */
+int dsk_create(dsk_ctx **out, int64_t N, float box, int periodic, float eps, float theta, int p);
+int dsk_destroy(dsk_ctx *ctx);
+
+/* Bytes of device workspace this context needs (depends on N and the largest order, p = 8). */
+size_t dsk_workspace_bytes(const dsk_ctx *ctx);
+/* Lend the workspace (device pointer, >= dsk_workspace_bytes(), 256-byte aligned). */
+int dsk_bind_workspace(dsk_ctx *ctx, void *dev_ptr, size_t bytes);
+/* cudaStream_t as void* (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream. */
+int dsk_set_stream(dsk_ctx *ctx, void *cuda_stream);
+/* Change eps / theta / p without rebuilding the tree (moments are recomputed when p changes, lists
+ * when theta changes) — the (theta, p) sweep of BASELINE.json configs[1]. */
+int dsk_set_params(dsk_ctx *ctx, float eps, float theta, int p);
+
+/* Keys -> sort -> octree -> groups -> upward pass (order p) for these positions and masses.
+ * PAPER.md:61 (keys, tree), :57/:75 (moments).  pos dev [N,3], mass dev [N]; not retained. */
+int dsk_build_tree(dsk_ctx *ctx, const float *pos, const float *mass);
+
+/* Walk + evaluate: acc dev [N,3], pot dev [N] or NULL, caller order.  pos/mass must be the arrays the
+ * tree was built from (they are not re-read: the sorted copy made by dsk_build_tree is used).
+ * PAPER.md:69-75 (lists, P2P, multipole interactions), :63 (periodic far field). */
+int dsk_accel(dsk_ctx *ctx, const float *pos, const float *mass, float *acc, float *pot);
+
+/* One kick-drift-kick step of the comoving leapfrog (O9), in place:
+ * vel is the canonical momentum per unit mass a^2 dx/dt; periodic: Einstein-de Sitter factors from
+ * the total mass in the box, positions wrapped to [0,box); isolated: Newtonian with dt = da.
+ * The first call evaluates the force at pos; later calls reuse the force cached by the previous
+ * step (call dsk_kdk_reset after changing pos/vel by hand).  One force evaluation per step. */
+int dsk_kdk_step(dsk_ctx *ctx, float *pos, float *vel, const float *mass, double a, double da);
+int dsk_kdk_reset(dsk_ctx *ctx);
+
+/* ---- introspection (parity tests, reporting) ---------------------------------------------------- */
+/* sorted keys and the permutation: sorted_keys[r] = key(order[r]); dev [N] each (either may be NULL). */
+int dsk_get_keys(dsk_ctx *ctx, uint64_t *sorted_keys, uint32_t *order);
+/* tree topology in canonical (ascending hotkey) order; *ncell is always written (host pointer); the
+ * arrays are dev [ncell] and may be NULL. */
+int dsk_get_tree(dsk_ctx *ctx, int64_t *ncell, uint64_t *hotkey, uint32_t *first, uint32_t *count,
+                 uint8_t *nchild);
+/* per cell (canonical order): com_mass dev [ncell,4] = (com x,y,z, mass); moments dev [ncell,N_p] =
+ * raw (unscaled) Cartesian moments M_n = sum m (y - com)^n of the current order p.  Either may be NULL. */
+int dsk_get_moments(dsk_ctx *ctx, float *com_mass, float *moments);
+/* sink groups in Morton order: *ngroup host; first/count dev [ngroup], bbox dev [ngroup,6] (min, max);
+ * m2p_len/p2p_len dev [ngroup] = list lengths of the last walk (cells / leaves).  Arrays may be NULL. */
+int dsk_get_groups(dsk_ctx *ctx, int64_t *ngroup, uint32_t *first, uint32_t *count, float *bbox,
+                   uint32_t *m2p_len, uint32_t *p2p_len);
+int dsk_get_stats(dsk_ctx *ctx, dsk_stats *out /* host */);
+/* library constants: "NLEAF", "NCRIT", "WS", "KEY_LEVELS", "FAR_ORDER"; host pointer. */
+int dsk_get_param(const char *name, double *value);
+/* far-field lattice tensors T_n (|n| <= 8, 165 doubles, host) of this context; periodic only. */
+int dsk_get_lattice_tensors(dsk_ctx *ctx, double *T /* host [165] */);
+const char *dsk_strerror(int err);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

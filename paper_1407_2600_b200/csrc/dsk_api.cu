@@ -1,0 +1,406 @@
+// dsk_api.cu — the C ABI of include/dsk.h: context, workspace carving, orchestration of the phases
+// K S T G U W F1 F2 F3 X I on the caller's stream, status read-back.  No device allocation after
+// dsk_bind_workspace; one small D2H read + stream synchronise at the end of each compute call.
+#include "dsk_internal.cuh"
+#include <math.h>
+#include <new>
+#include <string.h>
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// carve (or just measure, when base == nullptr) the workspace
+static size_t carve(dsk_ctx *c, char *base)
+{
+    size_t o = 0;
+    const size_t n = (size_t)c->N;
+    auto take = [&](size_t bytes) -> char * {
+        char *p = base ? base + o : nullptr;
+        o += align_up(bytes);
+        return p;
+    };
+    c->ntile = (int)((n + 2047) / 2048);
+    c->ncell_cap = (int64_t)(n * 3 / 4 + 4096);
+    if (c->ncell_cap > (1ll << DSK_CELL_BITS)) c->ncell_cap = 1ll << DSK_CELL_BITS;
+    c->ngroup_cap = (int64_t)(n / 2 + 1024);
+    const size_t nc = (size_t)c->ncell_cap, ng = (size_t)c->ngroup_cap;
+    c->dstate = (dsk_devstate *)take(sizeof(dsk_devstate));
+    c->key_a = (uint64_t *)take(8 * n);
+    c->key_b = (uint64_t *)take(8 * n);
+    c->idx_a = (uint32_t *)take(4 * n);
+    c->idx_b = (uint32_t *)take(4 * n);
+    c->sort_hist = (uint32_t *)take(4 * 256 * (size_t)c->ntile);
+    c->scan_tmp = (uint32_t *)take(4 * 4096);
+    c->spos = (float4 *)take(16 * n);
+    c->sacc = (float4 *)take(16 * n);
+    c->hotkey = (uint64_t *)take(8 * nc);
+    c->cell = (dsk_cellrec *)take(16 * nc);
+    c->parent = (uint32_t *)take(4 * nc);
+    c->nchild_tmp = (uint32_t *)take(4 * nc);
+    c->whdr = (float4 *)take(16 * nc);
+    c->rows = (float *)take(4 * (size_t)dsk_rowlen(DSK_PMAX) * nc);
+    c->gmark = (uint32_t *)take(4 * n);
+    c->gscan = (uint32_t *)take(4 * n);
+    c->gfirst = (uint32_t *)take(4 * ng);
+    c->gcount = (uint32_t *)take(4 * ng);
+    c->gcell = (uint32_t *)take(4 * ng);
+    c->gbox = (float4 *)take(32 * ng);
+    c->g_m2p_len = (uint32_t *)take(4 * ng);
+    c->g_p2p_len = (uint32_t *)take(4 * ng);
+    c->g_p2p_src = (uint32_t *)take(4 * ng);
+    c->g_m2p_off = (uint64_t *)take(8 * (ng + 1));
+    c->g_p2p_off = (uint64_t *)take(8 * (ng + 1));
+    // interaction lists: ~100 / ~12 entries per particle cover theta >= 0.4 in one batch; smaller theta
+    // or very large N run in batches of groups (force.cu)
+    c->list_m2p_cap = n * 100 + (1u << 20);
+    c->list_p2p_cap = n * 12 + (1u << 18);
+    const size_t cap_entries = (size_t)3 << 30;                    // 12 GiB of u32 per list at most
+    if (c->list_m2p_cap > cap_entries) c->list_m2p_cap = cap_entries;
+    if (c->list_p2p_cap > cap_entries / 4) c->list_p2p_cap = cap_entries / 4;
+    c->list_m2p = (uint32_t *)take(4 * c->list_m2p_cap);
+    c->list_p2p = (uint32_t *)take(4 * c->list_p2p_cap);
+    c->kdk_acc = (float *)take(12 * n);
+    c->far_partial = (double *)take(8 * DSK_NFAR * 1024);
+    c->far_M = (double *)take(8 * DSK_NFAR);
+    c->far_T_dev = (double *)take(8 * DSK_NFAR);
+    c->far_lambda = (float *)take(4 * DSK_NFAR);
+    return o;
+}
+
+static int check_params(float eps, float theta, int p)
+{
+    if (!(eps > 0.0f) || !isfinite(eps)) return DSK_EINVAL;
+    if (!(theta > 0.0f && theta <= 1.0f)) return DSK_EINVAL;
+    if (p != 2 && p != 4 && p != 6 && p != 8) return DSK_EINVAL;
+    return DSK_OK;
+}
+
+extern "C" int dsk_create(dsk_ctx **out, int64_t N, float box, int periodic, float eps, float theta, int p)
+{
+    if (!out) return DSK_EINVAL;
+    *out = nullptr;
+    if (N <= 0 || N > 0xfffffff0ll || !(box > 0.0f) || !isfinite(box)) return DSK_EINVAL;
+    if (check_params(eps, theta, p)) return DSK_EINVAL;
+    dsk_ctx *c = new (std::nothrow) dsk_ctx;
+    if (!c) return DSK_ECUDA;
+    memset(c, 0, sizeof(*c));
+    c->N = N; c->box = box; c->periodic = periodic ? 1 : 0; c->eps = eps; c->theta = theta; c->p = p;
+    c->moments_p = -1;
+    c->ws_bytes = 0;
+    carve(c, nullptr);
+    if (c->periodic) dsk_lattice_tensors((double)box, DSK_WS, c->far_T);
+    c->stats.n = N;
+    *out = c;
+    return DSK_OK;
+}
+
+extern "C" int dsk_destroy(dsk_ctx *c)
+{
+    if (!c) return DSK_EINVAL;
+    if (c->hstate) {
+        cudaFreeHost(c->hstate);
+        for (int i = 0; i < 16; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    }
+    delete c;
+    return DSK_OK;
+}
+
+extern "C" size_t dsk_workspace_bytes(const dsk_ctx *c)
+{
+    if (!c) return 0;
+    dsk_ctx tmp = *c;
+    return carve(&tmp, nullptr);
+}
+
+extern "C" int dsk_bind_workspace(dsk_ctx *c, void *dev_ptr, size_t bytes)
+{
+    if (!c) return DSK_EINVAL;
+    if (!dev_ptr || ((uintptr_t)dev_ptr & 255)) return DSK_ENOWORKSPACE;
+    if (bytes < dsk_workspace_bytes(c)) return DSK_ENOWORKSPACE;
+    int dev = 0;
+    DSK_CUDA(cudaGetDevice(&dev));
+    DSK_CUDA(cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, dev));
+    if (!c->hstate) {
+        DSK_CUDA(cudaMallocHost((void **)&c->hstate, 4096));
+        memset(c->hstate, 0, 4096);
+        for (int i = 0; i < 16; i++) DSK_CUDA(cudaEventCreate(&c->ev[i]));
+    }
+    c->ws = (char *)dev_ptr;
+    c->ws_bytes = bytes;
+    carve(c, c->ws);
+    c->have_tree = 0; c->moments_p = -1; c->lists_valid = 0; c->kdk_have_acc = 0;
+    if (c->periodic)
+        DSK_CUDA(cudaMemcpyAsync(c->far_T_dev, c->far_T, sizeof(double) * DSK_NFAR, cudaMemcpyHostToDevice, c->stream));
+    DSK_CUDA(cudaMemsetAsync(c->dstate, 0, sizeof(dsk_devstate), c->stream));
+    DSK_CUDA(cudaStreamSynchronize(c->stream));
+    return DSK_OK;
+}
+
+extern "C" int dsk_set_stream(dsk_ctx *c, void *stream)
+{
+    if (!c) return DSK_EINVAL;
+    c->stream = (cudaStream_t)stream;
+    return DSK_OK;
+}
+
+extern "C" int dsk_set_params(dsk_ctx *c, float eps, float theta, int p)
+{
+    if (!c) return DSK_EINVAL;
+    if (check_params(eps, theta, p)) return DSK_EINVAL;
+    c->eps = eps; c->theta = theta; c->p = p;
+    return DSK_OK;
+}
+
+static int status_to_error(uint32_t st)
+{
+    if (st & ST_NONFINITE) return DSK_ENONFINITE;
+    if (st & ST_OUTOFBOX) return DSK_EOUTOFBOX;
+    if (st & ST_CELLOVF) return DSK_ECELLOVERFLOW;
+    if (st & (ST_STACKOVF | ST_LISTOVF)) return DSK_ELISTOVERFLOW;
+    return DSK_OK;
+}
+
+static int read_state(dsk_ctx *c)
+{
+    DSK_CUDA(cudaMemcpyAsync(c->hstate, c->dstate, sizeof(dsk_devstate), cudaMemcpyDeviceToHost, c->stream));
+    DSK_CUDA(cudaStreamSynchronize(c->stream));
+    DSK_CUDA(cudaGetLastError());
+    return status_to_error(c->hstate->status);
+}
+
+static float ev_ms(cudaEvent_t a, cudaEvent_t b)
+{
+    float ms = 0.0f;
+    if (cudaEventElapsedTime(&ms, a, b) != cudaSuccess) { cudaGetLastError(); return 0.0f; }
+    return ms;
+}
+
+extern "C" int dsk_build_tree(dsk_ctx *c, const float *pos, const float *mass)
+{
+    if (!c || !pos || !mass) return DSK_EINVAL;
+    if (!c->ws) return DSK_ENOWORKSPACE;
+    c->have_tree = 0; c->moments_p = -1; c->lists_valid = 0;
+    DSK_CUDA(cudaMemsetAsync(c->dstate, 0, sizeof(dsk_devstate), c->stream));
+    int e = dsk_run_keysort(c, pos, mass);
+    if (e) return e;
+    e = dsk_run_build(c);
+    if (e) return e;
+    e = read_state(c);                       // ncell, ngroup, level starts, status
+    if (e) return e;
+    c->stats.ncell = c->hstate->ncell; c->stats.ngroup = c->hstate->ngroup;
+    c->stats.nlevel = c->hstate->nlevel; c->stats.nleaf_cells = c->hstate->nleaf_cells;
+    c->have_tree = 1;
+    e = dsk_run_upward(c);
+    if (e) return e;
+    DSK_CUDA(cudaStreamSynchronize(c->stream));
+    c->stats.ms_key = ev_ms(c->ev[0], c->ev[1]);
+    c->stats.ms_sort = ev_ms(c->ev[1], c->ev[2]);
+    c->stats.ms_build = ev_ms(c->ev[2], c->ev[3]);
+    c->stats.ms_group = ev_ms(c->ev[3], c->ev[4]);
+    c->stats.ms_upward = ev_ms(c->ev[5], c->ev[6]);
+    return DSK_OK;
+}
+
+extern "C" int dsk_accel(dsk_ctx *c, const float *pos, const float *mass, float *acc, float *pot)
+{
+    (void)pos; (void)mass;
+    if (!c || !acc) return DSK_EINVAL;
+    if (!c->ws) return DSK_ENOWORKSPACE;
+    if (!c->have_tree) return DSK_ENOTREE;
+    int e;
+    if (c->moments_p != c->p) {
+        e = dsk_run_upward(c);
+        if (e) return e;
+        DSK_CUDA(cudaStreamSynchronize(c->stream));
+        c->stats.ms_upward = ev_ms(c->ev[5], c->ev[6]);
+    }
+    if (!(c->lists_valid && c->lists_theta == c->theta)) {
+        e = dsk_run_walk(c);
+        if (e) return e;
+    }
+    e = dsk_run_force(c, pot != nullptr);
+    if (e) return e;
+    cudaEventRecord(c->ev[12], c->stream);
+    if (c->periodic) {
+        e = dsk_run_farfield(c);
+        if (e) return e;
+    }
+    cudaEventRecord(c->ev[13], c->stream);
+    e = dsk_run_scatter(c, acc, pot);
+    if (e) return e;
+    cudaEventRecord(c->ev[14], c->stream);
+    e = read_state(c);
+    c->stats.ms_far = ev_ms(c->ev[12], c->ev[13]);
+    c->stats.ms_scatter = ev_ms(c->ev[13], c->ev[14]);
+    c->stats.n_p2p = (int64_t)c->hstate->n_p2p; c->stats.n_m2p = (int64_t)c->hstate->n_m2p;
+    c->stats.list_m2p = (int64_t)c->hstate->tot_m2p_list; c->stats.list_p2p = (int64_t)c->hstate->tot_p2p_list;
+    return e;
+}
+
+// Einstein-de Sitter leapfrog factors (O9): H0^2 = (8 pi/3) M_tot / box^3
+static void kdk_factors(const dsk_ctx *c, double mtot, double a, double da, double *k1, double *d, double *k2)
+{
+    if (!c->periodic) { *k1 = 0.5 * da; *d = da; *k2 = 0.5 * da; return; }
+    const double PI = 3.14159265358979323846;
+    const double H0 = sqrt(8.0 * PI / 3.0 * mtot / ((double)c->box * c->box * c->box));
+    const double am = a + 0.5 * da, a1 = a + da;
+    *k1 = 2.0 / H0 * (sqrt(am) - sqrt(a));
+    *k2 = 2.0 / H0 * (sqrt(a1) - sqrt(am));
+    *d = 2.0 / H0 * (1.0 / sqrt(a) - 1.0 / sqrt(a1));
+}
+
+extern "C" int dsk_kdk_reset(dsk_ctx *c)
+{
+    if (!c) return DSK_EINVAL;
+    c->kdk_have_acc = 0;
+    return DSK_OK;
+}
+
+extern "C" int dsk_kdk_step(dsk_ctx *c, float *pos, float *vel, const float *mass, double a, double da)
+{
+    if (!c || !pos || !vel || !mass) return DSK_EINVAL;
+    if (!c->ws) return DSK_ENOWORKSPACE;
+    if (c->periodic && !(a > 0.0 && a + da > 0.0)) return DSK_EINVAL;
+    int e;
+    if (!c->kdk_have_acc) {
+        e = dsk_build_tree(c, pos, mass);
+        if (e) return e;
+        e = dsk_accel(c, pos, mass, c->kdk_acc, nullptr);
+        if (e) return e;
+        c->kdk_have_acc = 1;
+    }
+    // total mass = root monopole of the current tree (row 0 holds the root cell)
+    float mroot = 0.0f;
+    DSK_CUDA(cudaMemcpyAsync(&mroot, c->rows + 8, sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    DSK_CUDA(cudaStreamSynchronize(c->stream));
+    double k1, d, k2;
+    kdk_factors(c, (double)mroot, a, da, &k1, &d, &k2);
+    cudaEventRecord(c->ev[15], c->stream);
+    e = dsk_run_kick(c, vel, c->kdk_acc, (float)k1);
+    if (e) return e;
+    e = dsk_run_drift(c, pos, vel, (float)d);
+    if (e) return e;
+    c->kdk_have_acc = 0;
+    e = dsk_build_tree(c, pos, mass);
+    if (e) return e;
+    e = dsk_accel(c, pos, mass, c->kdk_acc, nullptr);
+    if (e) return e;
+    e = dsk_run_kick(c, vel, c->kdk_acc, (float)k2);
+    if (e) return e;
+    DSK_CUDA(cudaStreamSynchronize(c->stream));
+    c->kdk_have_acc = 1;
+    return DSK_OK;
+}
+
+// ---- introspection -------------------------------------------------------------------------------------
+extern "C" int dsk_get_keys(dsk_ctx *c, uint64_t *sorted_keys, uint32_t *order)
+{
+    if (!c) return DSK_EINVAL;
+    if (!c->have_tree) return DSK_ENOTREE;
+    if (sorted_keys) DSK_CUDA(cudaMemcpyAsync(sorted_keys, c->key_a, 8 * (size_t)c->N, cudaMemcpyDeviceToDevice, c->stream));
+    if (order) DSK_CUDA(cudaMemcpyAsync(order, c->idx_a, 4 * (size_t)c->N, cudaMemcpyDeviceToDevice, c->stream));
+    DSK_CUDA(cudaStreamSynchronize(c->stream));
+    return DSK_OK;
+}
+
+__global__ void k_unpack_cells(const dsk_cellrec *__restrict__ cell, uint32_t n, uint32_t *first, uint32_t *count,
+                               uint8_t *nchild)
+{
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    dsk_cellrec r = cell[i];
+    if (first) first[i] = r.first;
+    if (count) count[i] = r.count;
+    if (nchild) nchild[i] = (uint8_t)(r.meta & 255u);
+}
+
+extern "C" int dsk_get_tree(dsk_ctx *c, int64_t *ncell, uint64_t *hotkey, uint32_t *first, uint32_t *count,
+                            uint8_t *nchild)
+{
+    if (!c || !ncell) return DSK_EINVAL;
+    if (!c->have_tree) return DSK_ENOTREE;
+    const uint32_t n = c->hstate->ncell;
+    *ncell = n;
+    if (hotkey) DSK_CUDA(cudaMemcpyAsync(hotkey, c->hotkey, 8 * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
+    if (first || count || nchild) k_unpack_cells<<<(n + 255) / 256, 256, 0, c->stream>>>(c->cell, n, first, count, nchild);
+    DSK_CUDA(cudaStreamSynchronize(c->stream));
+    return DSK_OK;
+}
+
+extern "C" int dsk_get_moments(dsk_ctx *c, float *com_mass, float *moments)
+{
+    if (!c) return DSK_EINVAL;
+    if (!c->have_tree) return DSK_ENOTREE;
+    if (c->moments_p != c->p) {
+        int e = dsk_run_upward(c);
+        if (e) return e;
+    }
+    return dsk_run_get_moments(c, com_mass, moments);
+}
+
+__global__ void k_unpack_gbox(const float4 *__restrict__ gbox, uint32_t n, float *out)
+{
+    uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= n) return;
+    float4 lo = gbox[2 * (size_t)g], hi = gbox[2 * (size_t)g + 1];
+    float *o = out + 6 * (size_t)g;
+    o[0] = lo.x; o[1] = lo.y; o[2] = lo.z; o[3] = hi.x; o[4] = hi.y; o[5] = hi.z;
+}
+
+extern "C" int dsk_get_groups(dsk_ctx *c, int64_t *ngroup, uint32_t *first, uint32_t *count, float *bbox,
+                              uint32_t *m2p_len, uint32_t *p2p_len)
+{
+    if (!c || !ngroup) return DSK_EINVAL;
+    if (!c->have_tree) return DSK_ENOTREE;
+    const uint32_t n = c->hstate->ngroup;
+    *ngroup = n;
+    cudaStream_t s = c->stream;
+    if (first) DSK_CUDA(cudaMemcpyAsync(first, c->gfirst, 4 * (size_t)n, cudaMemcpyDeviceToDevice, s));
+    if (count) DSK_CUDA(cudaMemcpyAsync(count, c->gcount, 4 * (size_t)n, cudaMemcpyDeviceToDevice, s));
+    if (bbox) k_unpack_gbox<<<(n + 255) / 256, 256, 0, s>>>(c->gbox, n, bbox);
+    if (m2p_len) DSK_CUDA(cudaMemcpyAsync(m2p_len, c->g_m2p_len, 4 * (size_t)n, cudaMemcpyDeviceToDevice, s));
+    if (p2p_len) DSK_CUDA(cudaMemcpyAsync(p2p_len, c->g_p2p_len, 4 * (size_t)n, cudaMemcpyDeviceToDevice, s));
+    DSK_CUDA(cudaStreamSynchronize(s));
+    return DSK_OK;
+}
+
+extern "C" int dsk_get_stats(dsk_ctx *c, dsk_stats *out)
+{
+    if (!c || !out) return DSK_EINVAL;
+    *out = c->stats;
+    return DSK_OK;
+}
+
+extern "C" int dsk_get_param(const char *name, double *v)
+{
+    if (!name || !v) return DSK_EINVAL;
+    if (!strcmp(name, "NLEAF")) *v = DSK_NLEAF;
+    else if (!strcmp(name, "NCRIT")) *v = DSK_NCRIT;
+    else if (!strcmp(name, "WS")) *v = DSK_WS;
+    else if (!strcmp(name, "KEY_LEVELS")) *v = DSK_KEY_LEVELS;
+    else if (!strcmp(name, "FAR_ORDER")) *v = DSK_FAR_ORDER;
+    else return DSK_EINVAL;
+    return DSK_OK;
+}
+
+extern "C" int dsk_get_lattice_tensors(dsk_ctx *c, double *T)
+{
+    if (!c || !T || !c->periodic) return DSK_EINVAL;
+    memcpy(T, c->far_T, sizeof(double) * DSK_NFAR);
+    return DSK_OK;
+}
+
+extern "C" const char *dsk_strerror(int e)
+{
+    switch (e) {
+    case DSK_OK: return "ok";
+    case DSK_EINVAL: return "invalid argument";
+    case DSK_ENOWORKSPACE: return "workspace missing, too small or misaligned";
+    case DSK_ENOTREE: return "no tree built";
+    case DSK_EOUTOFBOX: return "position outside [0, box) in isolated mode";
+    case DSK_ENONFINITE: return "non-finite position";
+    case DSK_ELISTOVERFLOW: return "traversal stack or interaction list overflow";
+    case DSK_ECUDA: return "CUDA error";
+    case DSK_ECELLOVERFLOW: return "more tree cells or groups than the workspace holds";
+    default: return "unknown error";
+    }
+}

@@ -1,0 +1,173 @@
+// dsk_internal.cuh — context, workspace layout and small device helpers shared by the CUDA sources of
+// libdsk (sm_100a).  Nothing here is shared with the oracle.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/dsk.h"
+
+#define DSK_KEY_LEVELS 21
+#define DSK_NLEAF 16
+#define DSK_NCRIT 64
+#define DSK_WS 2              // image block half-width (WS = 1 floors the error at ~3e-3)
+#define DSK_FAR_ORDER 8
+#define DSK_NFAR 165          // C(8+3,3)
+#define DSK_PMAX 8
+#define DSK_IMG_BITS 7        // list entry = image << 25 | cell ... see below
+#define DSK_CELL_BITS 25
+// A list entry packs (image id, cell id).  With WS = 2 there are 125 images (7 bits) which leaves
+// 25 bits = 33.5 M cells per tree; larger trees use WS-image ids only in periodic mode, so isolated
+// runs could use all 32 bits — kept uniform for simplicity (N <= ~1.3e8 at ~0.25 cells/particle).
+
+__host__ __device__ constexpr int dsk_np(int p) { return (p + 1) * (p + 2) * (p + 3) / 6; }
+__host__ __device__ constexpr int dsk_midx(int a, int b, int c)
+{
+    return (a + b + c) * (a + b + c + 1) * (a + b + c + 2) / 6 + (b + c) * (b + c + 1) / 2 + c;
+}
+// moment row (floats): [ctr.x ctr.y ctr.z 1/s | off.x off.y off.z delta | Mhat_0 .. Mhat_{Np-1} | pad]
+// ctr = geometric cell centre (exact), off = com - ctr, Mhat_n = (-1)^|n| M_n / (n! s^|n|)
+__host__ __device__ constexpr int dsk_rowlen(int p) { return ((8 + dsk_np(p)) + 3) / 4 * 4; }
+
+struct dsk_cellrec {          // 16 B, one LDG.128 in the walk
+    uint32_t first, count, child0, meta;   // meta = nchild | level << 8
+};
+
+struct dsk_devstate {         // small device block read back at the end of API calls
+    uint32_t status;          // bit flags: 1 out-of-box, 2 non-finite, 4 cell overflow, 8 stack overflow,
+                              //            16 list overflow
+    uint32_t ncell, ngroup, nlevel;
+    uint32_t lvl_start[DSK_KEY_LEVELS + 3];
+    uint32_t nleaf_cells;
+    unsigned long long tot_m2p_list, tot_p2p_list, tot_p2p_src;   // over all groups
+    unsigned long long n_p2p, n_m2p;                               // useful interactions
+    unsigned long long scratch[4];
+};
+
+enum { ST_OUTOFBOX = 1, ST_NONFINITE = 2, ST_CELLOVF = 4, ST_STACKOVF = 8, ST_LISTOVF = 16 };
+
+struct dsk_ctx {
+    int64_t N;
+    float box;
+    int periodic;
+    float eps, theta;
+    int p;
+    cudaStream_t stream;
+    // workspace
+    char *ws;
+    size_t ws_bytes;
+    // carved arrays
+    uint64_t *key_a, *key_b;
+    uint32_t *idx_a, *idx_b;
+    uint32_t *sort_hist;      // [ntile * 256] per-pass tile histograms (digit-major)
+    uint32_t *scan_tmp;       // block sums for the generic scan
+    float4 *spos;             // sorted (x,y,z,m); periodic: wrapped
+    float4 *sacc;             // sorted (ax,ay,az,pot)
+    uint64_t *hotkey;
+    dsk_cellrec *cell;
+    uint32_t *parent;
+    uint32_t *nchild_tmp;
+    float4 *whdr;             // walk header per cell: com.xyz, delta
+    float *rows;              // [ncell_cap * rowlen(p)]
+    uint32_t *gmark;          // [N] group start markers (cell id + 1)
+    uint32_t *gscan;          // [N]
+    uint32_t *gfirst, *gcount, *gcell;     // [ngroup_cap]
+    float4 *gbox;             // [2 * ngroup_cap]: min.xyz,_ ; max.xyz,_
+    uint32_t *g_m2p_len, *g_p2p_len, *g_p2p_src;   // [ngroup_cap]
+    uint64_t *g_m2p_off, *g_p2p_off;               // [ngroup_cap + 1] exclusive offsets into lists
+    uint32_t *list_m2p, *list_p2p;
+    size_t list_m2p_cap, list_p2p_cap;             // entries
+    float *kdk_acc;           // [N,3] cached force, caller order
+    double *far_partial;      // [nblk * 165]
+    double *far_M;            // [165]
+    float *far_lambda;        // [165]
+    double *far_T_dev;        // [165]
+    dsk_devstate *dstate;     // device
+    dsk_devstate *hstate;     // pinned host
+    // sizes
+    int64_t ncell_cap, ngroup_cap;
+    int ntile;
+    // state
+    int have_tree, moments_p, lists_valid, kdk_have_acc;
+    float lists_theta;
+    double far_T[DSK_NFAR];
+    dsk_stats stats;
+    cudaEvent_t ev[16];
+    int nsm;
+};
+
+#define DSK_CUDA(x)                                 \
+    do {                                            \
+        cudaError_t e__ = (x);                      \
+        if (e__ != cudaSuccess) return DSK_ECUDA;   \
+    } while (0)
+
+// ---- internal entry points (one per source file) -------------------------------------------------
+int dsk_run_keysort(dsk_ctx *c, const float *pos, const float *mass);         // keysort.cu: K, S, gather
+int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot);                      // keysort.cu: X
+void dsk_exclusive_scan_u32(dsk_ctx *c, const uint32_t *in, uint32_t *out, const uint32_t *n_dev,
+                            uint32_t n_max, uint32_t *total_dev);             // keysort.cu
+int dsk_run_build(dsk_ctx *c);                                                // tree.cu: T, G
+int dsk_run_upward(dsk_ctx *c);                                               // upward.cu: U
+int dsk_run_get_moments(dsk_ctx *c, float *com_mass, float *moments);         // upward.cu
+int dsk_run_walk(dsk_ctx *c);                                                 // walk.cu: W
+int dsk_run_force(dsk_ctx *c, int want_pot);                                  // force.cu: F1, F2
+int dsk_run_farfield(dsk_ctx *c);                                             // farfield.cu: F3
+void dsk_lattice_tensors(double L, int ws, double *T);                        // farfield.cu (host)
+int dsk_run_kick(dsk_ctx *c, float *vel, const float *acc, float k);          // kdk.cu
+int dsk_run_drift(dsk_ctx *c, float *pos, const float *vel, float d);         // kdk.cu
+
+// ---- packed f32x2 arithmetic (sm_100a: FFMA2 / FADD2 / FMUL2) ----------------------------------
+// One 64-bit register pair carries two independent fp32 lanes.  Measured on B200: scalar FFMA with
+// three distinct source registers tops out at ~46 TFLOP/s (register-bank limited), FFMA2 reaches the
+// 74 TFLOP/s nominal peak — so the force kernels run two sources per thread in packed form.
+#ifdef __CUDACC__
+struct f2 {
+    unsigned long long v;
+};
+__device__ __forceinline__ f2 f2_make(float lo, float hi)
+{
+    f2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ f2 f2_dup(float x) { return f2_make(x, x); }
+__device__ __forceinline__ float f2_lo(f2 a)
+{
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.v));
+    return lo;
+}
+__device__ __forceinline__ float f2_hi(f2 a)
+{
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.v));
+    return hi;
+}
+__device__ __forceinline__ f2 f2_fma(f2 a, f2 b, f2 c)
+{
+    f2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(a.v), "l"(b.v), "l"(c.v));
+    return r;
+}
+__device__ __forceinline__ f2 f2_mul(f2 a, f2 b)
+{
+    f2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v));
+    return r;
+}
+__device__ __forceinline__ f2 f2_add(f2 a, f2 b)
+{
+    f2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v));
+    return r;
+}
+__device__ __forceinline__ f2 f2_sub(f2 a, f2 b)
+{
+    f2 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v));
+    return r;
+}
+__device__ __forceinline__ f2 f2_rsqrt(f2 a)
+{
+    return f2_make(rsqrtf(f2_lo(a)), rsqrtf(f2_hi(a)));
+}
+#endif

@@ -1,0 +1,283 @@
+// farfield.cu — step F3: periodic far field as an order-8 local expansion about the box centre.
+// DESIGN.md O7 ("periodic boundary conditions using a high-order (p=8) multipole local
+// expansion (Challacombe et al. 1997; Metchnik 2009)").  The (2 WS+1)^3 nearest images are summed by
+// the tree walk; everything else (all farther images + the neutralising background) is the smooth field
+//   Phi_far(u) = psi_Ewald(u) + sum_{|n|_inf <= WS} 1/|u - nL|
+// whose Taylor coefficients T_n (|n| <= 8) are computed once per context on the host in fp64.
+// Per force evaluation: (a) root moments M_k = sum m (x - c)^k, |k| <= 8, fp64 block partials;
+// (b) Lambda_n = sum_k (-1)^|k| C(n+k,k) M_k T_{n+k}; (c) per particle pot += sum Lambda_n X^n,
+// acc_i -= sum n_i Lambda_n X^(n-e_i).
+#include "dsk_internal.cuh"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include <type_traits>
+#include <vector>
+
+#define NF DSK_NFAR
+#define FO DSK_FAR_ORDER
+
+// ---------------------------------------------------------------------------------------------------
+// host: lattice tensors.  Truncated polynomial algebra in three variables (degree <= 8).
+namespace {
+struct Poly {
+    double c[NF];
+    Poly() { memset(c, 0, sizeof(c)); }
+};
+struct Tab {
+    int a[NF], b[NF], c[NF], l[NF];
+    Tab()
+    {
+        for (int L = 0; L <= FO; L++)
+            for (int A = L; A >= 0; A--)
+                for (int B = L - A; B >= 0; B--) {
+                    int C = L - A - B, i = dsk_midx(A, B, C);
+                    a[i] = A; b[i] = B; c[i] = C; l[i] = L;
+                }
+    }
+};
+const Tab &tab()
+{
+    static Tab t;
+    return t;
+}
+Poly mul(const Poly &x, const Poly &y)
+{
+    const Tab &t = tab();
+    Poly r;
+    for (int i = 0; i < NF; i++) {
+        if (x.c[i] == 0.0) continue;
+        for (int j = 0; j < NF && t.l[i] + t.l[j] <= FO; j++)
+            r.c[dsk_midx(t.a[i] + t.a[j], t.b[i] + t.b[j], t.c[i] + t.c[j])] += x.c[i] * y.c[j];
+    }
+    return r;
+}
+// out += sum_k coef[k] * delta^k, k = 0..FO  (delta has no constant term)
+void compose(const double coef[FO + 1], const Poly &delta, Poly &out)
+{
+    Poly pw;
+    pw.c[0] = 1.0;
+    for (int k = 0; k <= FO; k++) {
+        if (k) pw = mul(pw, delta);
+        for (int i = 0; i < NF; i++) out.c[i] += coef[k] * pw.c[i];
+    }
+}
+}   // namespace
+
+void dsk_lattice_tensors(double L, int ws, double *T)
+{
+    const double PI = 3.14159265358979323846, alpha = 2.0 / L, sqpi = sqrt(PI);
+    Poly out;
+    out.c[0] = PI / (alpha * alpha * L * L * L);
+    // real-space images.  s = |u - a|^2 = s0 + delta(u), delta = -2 a.u + |u|^2.
+    // Taylor coefficients in delta of F(s): F^(k)(s0)/k!, with d/ds = -(1/2) * (-(1/r) d/dr).
+    const double rcut = 6.5 / alpha;
+    const int nmax = (int)ceil(rcut / L) + ws + 1;
+    for (int ix = -nmax; ix <= nmax; ix++)
+        for (int iy = -nmax; iy <= nmax; iy++)
+            for (int iz = -nmax; iz <= nmax; iz++) {
+                const bool inblock = abs(ix) <= ws && abs(iy) <= ws && abs(iz) <= ws;
+                const double a[3] = {ix * L, iy * L, iz * L};
+                const double s0 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2];
+                Poly delta;
+                delta.c[dsk_midx(2, 0, 0)] = delta.c[dsk_midx(0, 2, 0)] = delta.c[dsk_midx(0, 0, 2)] = 1.0;
+                delta.c[dsk_midx(1, 0, 0)] = -2 * a[0]; delta.c[dsk_midx(0, 1, 0)] = -2 * a[1];
+                delta.c[dsk_midx(0, 0, 1)] = -2 * a[2];
+                double coef[FO + 1];
+                if (s0 == 0.0) {
+                    // in-block image at the origin: erf(alpha r)/r = 2 alpha/sqrt(pi) sum_k (-alpha^2 s)^k/(k!(2k+1))
+                    double f = 2.0 * alpha / sqpi, kf = 1.0;
+                    for (int k = 0; k <= FO; k++) {
+                        if (k) { f *= -alpha * alpha; kf *= k; }
+                        coef[k] = f / (kf * (2 * k + 1));
+                    }
+                } else {
+                    const double r = sqrt(s0);
+                    if (!inblock && r > rcut + 2 * L) continue;
+                    // E_k = (-(1/r) d/dr)^k [erfc(alpha r)/r],  N_k = (-(1/r) d/dr)^k [1/r] = (2k-1)!!/r^(2k+1)
+                    double E = erfc(alpha * r) / r, N = 1.0 / r, g = exp(-alpha * alpha * s0) / (alpha * sqpi);
+                    double tw = 1.0, sc = 1.0;
+                    for (int k = 0; k <= FO; k++) {
+                        if (k) {
+                            tw *= 2.0 * alpha * alpha;
+                            E = ((2 * k - 1) * E + tw * g) / s0;
+                            N = (2 * k - 1) * N / s0;
+                            sc *= -0.5 / k;
+                        }
+                        coef[k] = sc * (inblock ? (N - E) : -E);     // +erf/r inside the block, -erfc/r outside
+                    }
+                }
+                compose(coef, delta, out);
+            }
+    // reciprocal space: -(1/(pi L)) sum_h h^-2 exp(-pi^2 h^2/(alpha L)^2) cos(w.u), w = 2 pi h / L
+    const Tab &t = tab();
+    double fact[FO + 1];
+    fact[0] = 1.0;
+    for (int i = 1; i <= FO; i++) fact[i] = fact[i - 1] * i;
+    const int hmax = (int)ceil(sqrt(42.0) * alpha * L / PI) + 1;
+    for (int hx = -hmax; hx <= hmax; hx++)
+        for (int hy = -hmax; hy <= hmax; hy++)
+            for (int hz = -hmax; hz <= hmax; hz++) {
+                const int h2 = hx * hx + hy * hy + hz * hz;
+                if (!h2) continue;
+                const double ex = PI * PI * h2 / (alpha * alpha * L * L);
+                if (ex > 42.0) continue;
+                const double amp = -exp(-ex) / (h2 * PI * L);
+                const double w[3] = {2 * PI * hx / L, 2 * PI * hy / L, 2 * PI * hz / L};
+                double pwx[FO + 1], pwy[FO + 1], pwz[FO + 1];
+                pwx[0] = pwy[0] = pwz[0] = 1.0;
+                for (int e = 1; e <= FO; e++) { pwx[e] = pwx[e - 1] * w[0]; pwy[e] = pwy[e - 1] * w[1]; pwz[e] = pwz[e - 1] * w[2]; }
+                for (int i = 0; i < NF; i++) {
+                    if (t.l[i] & 1) continue;
+                    const double sg = ((t.l[i] >> 1) & 1) ? -1.0 : 1.0;
+                    out.c[i] += amp * sg * pwx[t.a[i]] * pwy[t.b[i]] * pwz[t.c[i]] / (fact[t.a[i]] * fact[t.b[i]] * fact[t.c[i]]);
+                }
+            }
+    memcpy(T, out.c, sizeof(double) * NF);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// device
+__constant__ uint8_t f_ea[NF], f_eb[NF], f_ec[NF];
+static bool g_far_tables = false;
+static int far_tables()
+{
+    if (g_far_tables) return DSK_OK;
+    const Tab &t = tab();
+    uint8_t a[NF], b[NF], c[NF];
+    for (int i = 0; i < NF; i++) { a[i] = (uint8_t)t.a[i]; b[i] = (uint8_t)t.b[i]; c[i] = (uint8_t)t.c[i]; }
+    DSK_CUDA(cudaMemcpyToSymbol(f_ea, a, NF));
+    DSK_CUDA(cudaMemcpyToSymbol(f_eb, b, NF));
+    DSK_CUDA(cudaMemcpyToSymbol(f_ec, c, NF));
+    g_far_tables = true;
+    return DSK_OK;
+}
+
+#define FM_THREADS 192
+#define FM_TILE 256
+// (a) block partials of the root moments about the box centre, fp64; thread = multi-index
+__global__ void __launch_bounds__(FM_THREADS) k_far_moments(const float4 *__restrict__ spos, uint32_t n,
+                                                            float half_box, double *__restrict__ partial)
+{
+    __shared__ double4 tile[FM_TILE];
+    const uint32_t chunk = ((n + gridDim.x - 1) / gridDim.x + FM_TILE - 1) / FM_TILE * FM_TILE;
+    const uint64_t lo = (uint64_t)blockIdx.x * chunk, hi = min((uint64_t)n, lo + chunk);
+    const int t = threadIdx.x;
+    const int a = t < NF ? f_ea[t] : 0, b = t < NF ? f_eb[t] : 0, c = t < NF ? f_ec[t] : 0;
+    double acc = 0.0;
+    for (uint64_t i0 = lo; i0 < hi; i0 += FM_TILE) {
+        for (int j = t; j < FM_TILE; j += FM_THREADS) {
+            double4 q = make_double4(0, 0, 0, 0);
+            if (i0 + j < hi) {
+                float4 p = spos[i0 + j];
+                q = make_double4((double)p.x - (double)half_box, (double)p.y - (double)half_box,
+                                 (double)p.z - (double)half_box, (double)p.w);
+            }
+            tile[j] = q;
+        }
+        __syncthreads();
+        if (t < NF) {
+            const int m = (int)min((uint64_t)FM_TILE, hi - i0);
+            for (int j = 0; j < m; j++) {
+                const double4 q = tile[j];
+                double v = q.w;
+                for (int e = 0; e < a; e++) v *= q.x;
+                for (int e = 0; e < b; e++) v *= q.y;
+                for (int e = 0; e < c; e++) v *= q.z;
+                acc += v;
+            }
+        }
+        __syncthreads();
+    }
+    if (t < NF) partial[(size_t)blockIdx.x * NF + t] = acc;
+}
+
+// (b) reduce partials, then Lambda_n = sum_{|k| <= 8-|n|} (-1)^|k| C(n+k,k) M_k T_{n+k}
+__global__ void __launch_bounds__(FM_THREADS) k_far_lambda(const double *__restrict__ partial, int nblk,
+                                                           const double *__restrict__ T, double *__restrict__ M,
+                                                           float *__restrict__ lambda)
+{
+    __shared__ double sM[NF];
+    __shared__ double binom[2 * FO + 1][2 * FO + 1];
+    const int t = threadIdx.x;
+    if (t < NF) {
+        double s = 0.0;
+        for (int b = 0; b < nblk; b++) s += partial[(size_t)b * NF + t];
+        sM[t] = s; M[t] = s;
+    }
+    if (t == 0)
+        for (int i = 0; i <= 2 * FO; i++) {
+            binom[i][0] = 1.0;
+            for (int j = 1; j <= i; j++) binom[i][j] = (j == i) ? 1.0 : binom[i - 1][j - 1] + binom[i - 1][j];
+        }
+    __syncthreads();
+    if (t < NF) {
+        const int a = f_ea[t], b = f_eb[t], c = f_ec[t], l = a + b + c;
+        double s = 0.0;
+        for (int k = 0; k < NF; k++) {
+            const int ka = f_ea[k], kb = f_eb[k], kc = f_ec[k], kl = ka + kb + kc;
+            if (l + kl > FO) break;
+            const double sg = (kl & 1) ? -1.0 : 1.0;
+            s += sg * binom[a + ka][ka] * binom[b + kb][kb] * binom[c + kc][kc] * sM[k] * T[dsk_midx(a + ka, b + kb, c + kc)];
+        }
+        lambda[t] = (float)s;
+    }
+}
+
+template <int I, int N, typename F>
+__device__ __forceinline__ void sfor(F &&f)
+{
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        sfor<I + 1, N>(f);
+    }
+}
+
+// (c) per particle: Horner-free, fully unrolled evaluation of the order-8 polynomial and its gradient
+__global__ void __launch_bounds__(128) k_far_eval(const float4 *__restrict__ spos, uint32_t n, float half_box,
+                                                  const float *__restrict__ lambda, float4 *__restrict__ sacc)
+{
+    __shared__ float sl[NF];
+    for (int i = threadIdx.x; i < NF; i += blockDim.x) sl[i] = lambda[i];
+    __syncthreads();
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 p = spos[i];
+    float px[FO + 1], py[FO + 1], pz[FO + 1];
+    px[0] = py[0] = pz[0] = 1.0f;
+    const float X = p.x - half_box, Y = p.y - half_box, Z = p.z - half_box;
+#pragma unroll
+    for (int e = 1; e <= FO; e++) { px[e] = px[e - 1] * X; py[e] = py[e - 1] * Y; pz[e] = pz[e - 1] * Z; }
+    float pot = 0.0f, gx = 0.0f, gy = 0.0f, gz = 0.0f;
+    sfor<0, FO + 1>([&](auto LL) {
+        constexpr int l = decltype(LL)::value;
+        sfor<0, l + 1>([&](auto KK) {
+            constexpr int k = decltype(KK)::value;          // k = b + c, a = l - k
+            sfor<0, k + 1>([&](auto CC) {
+                constexpr int c = decltype(CC)::value, b = k - c, a = l - k;
+                const float lam = sl[dsk_midx(a, b, c)];
+                const float yz = py[b] * pz[c];
+                pot = fmaf(lam * px[a], yz, pot);
+                if constexpr (a >= 1) gx = fmaf((float)a * lam * px[a - 1], yz, gx);
+                if constexpr (b >= 1) gy = fmaf((float)b * lam * px[a], py[b - 1] * pz[c], gy);
+                if constexpr (c >= 1) gz = fmaf((float)c * lam * px[a], py[b] * pz[c - 1], gz);
+            });
+        });
+    });
+    float4 acc = sacc[i];
+    acc.x -= gx; acc.y -= gy; acc.z -= gz; acc.w += pot;
+    sacc[i] = acc;
+}
+
+int dsk_run_farfield(dsk_ctx *c)
+{
+    int e = far_tables();
+    if (e) return e;
+    const uint32_t n = (uint32_t)c->N;
+    int nblk = c->nsm * 2;
+    if ((int64_t)nblk * FM_TILE > c->N) nblk = (int)((c->N + FM_TILE - 1) / FM_TILE);
+    k_far_moments<<<nblk, FM_THREADS, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_partial);
+    k_far_lambda<<<1, FM_THREADS, 0, c->stream>>>(c->far_partial, nblk, c->far_T_dev, c->far_M, c->far_lambda);
+    k_far_eval<<<(n + 127) / 128, 128, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_lambda, c->sacc);
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
+}

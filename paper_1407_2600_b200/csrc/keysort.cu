@@ -1,0 +1,271 @@
+// keysort.cu — steps K (Morton keys), S (LSD radix sort), the gather into the sorted float4 array,
+// X (scatter back to caller order) and a device-wide exclusive scan used by several phases.
+// DESIGN.md O1/O2 ("assign a Key to each particle, based on Morton ordering";
+// PAPER.md:69 "domain decomposition ... practically identical to a parallel sorting algorithm").
+// All HBM-bound: every global access below is a full-warp contiguous run except the two
+// permutation-driven ones (gather read, scatter write), which move whole 12/16-byte records.
+#include "dsk_internal.cuh"
+
+// ---- K: keys --------------------------------------------------------------------------------------
+// q = floor(fp32(x) * fp32(2^21/box)) with ONE IEEE fp32 multiply (reading A3), clamp to 2^21-1,
+// interleave x (msb of each triple), y, z, placeholder bit 2^63.  Periodic: fp32 wrap first.
+__device__ __forceinline__ float dsk_wrap(float x, float box)
+{
+    float t = __fdiv_rn(x, box);
+    float f = floorf(t);
+    float w = __fsub_rn(x, __fmul_rn(box, f));
+    if (!(w >= 0.0f && w < box)) w = 0.0f;
+    return w;
+}
+
+__device__ __forceinline__ uint64_t dsk_spread3(uint32_t q)
+{   // 21 bits -> every third bit
+    uint64_t x = q & 0x1fffffull;
+    x = (x | x << 32) & 0x1f00000000ffffull;
+    x = (x | x << 16) & 0x1f0000ff0000ffull;
+    x = (x | x << 8) & 0x100f00f00f00f00full;
+    x = (x | x << 4) & 0x10c30c30c30c30c3ull;
+    x = (x | x << 2) & 0x1249249249249249ull;
+    return x;
+}
+
+__global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pos, int64_t n, float box,
+                                              float scale, int periodic, uint64_t *__restrict__ key,
+                                              uint32_t *__restrict__ idx, dsk_devstate *st)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t q[3];
+    uint32_t bad = 0;
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        float x = pos[3 * i + d];
+        if (!isfinite(x)) { bad |= ST_NONFINITE; x = 0.0f; }
+        if (periodic) x = dsk_wrap(x, box);
+        else if (!(x >= 0.0f && x < box)) { bad |= ST_OUTOFBOX; x = 0.0f; }
+        float fl = floorf(__fmul_rn(x, scale));
+        uint32_t qi = (uint32_t)fl;
+        q[d] = qi > 2097151u ? 2097151u : qi;
+    }
+    if (bad) atomicOr(&st->status, bad);
+    key[i] = (1ull << 63) | (dsk_spread3(q[0]) << 2) | (dsk_spread3(q[1]) << 1) | dsk_spread3(q[2]);
+    idx[i] = (uint32_t)i;
+}
+
+// ---- S: LSD radix sort, 8-bit digits ---------------------------------------------------------------
+// Per pass: tile histograms (digit-major matrix) -> exclusive scan -> stable scatter.  A warp owns a
+// contiguous run of SORT_ITEMS*32 keys, so "warp, round, lane" is ascending global index and the
+// per-warp running counters give a stable rank.
+#define SORT_THREADS 256
+#define SORT_ITEMS 8
+#define SORT_TILE (SORT_THREADS * SORT_ITEMS)
+
+__global__ void __launch_bounds__(SORT_THREADS) k_sort_hist(const uint64_t *__restrict__ key, int64_t n,
+                                                            int shift, int ntile,
+                                                            uint32_t *__restrict__ hist)
+{
+    __shared__ uint32_t h[256];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    int64_t base = (int64_t)blockIdx.x * SORT_TILE;
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; i++) {
+        int64_t j = base + i * SORT_THREADS + threadIdx.x;
+        if (j < n) atomicAdd(&h[(key[j] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    hist[(size_t)threadIdx.x * ntile + blockIdx.x] = h[threadIdx.x];
+}
+
+__global__ void __launch_bounds__(SORT_THREADS) k_sort_scatter(
+    const uint64_t *__restrict__ key_in, const uint32_t *__restrict__ idx_in, int64_t n, int shift,
+    int ntile, const uint32_t *__restrict__ hist_scanned, uint64_t *__restrict__ key_out,
+    uint32_t *__restrict__ idx_out)
+{
+    __shared__ uint32_t cnt[SORT_THREADS / 32][256];
+    __shared__ uint32_t goff[256];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < (SORT_THREADS / 32) * 256; i += SORT_THREADS) (&cnt[0][0])[i] = 0;
+    goff[threadIdx.x] = hist_scanned[(size_t)threadIdx.x * ntile + blockIdx.x];
+    __syncthreads();
+    int64_t base = (int64_t)blockIdx.x * SORT_TILE + (int64_t)warp * (SORT_ITEMS * 32);
+    uint64_t k[SORT_ITEMS];
+    uint32_t v[SORT_ITEMS], rank[SORT_ITEMS];
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; i++) {
+        int64_t j = base + i * 32 + lane;
+        bool ok = j < n;
+        k[i] = ok ? key_in[j] : ~0ull;
+        v[i] = ok ? idx_in[j] : 0u;
+    }
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; i++) {
+        uint32_t d = (uint32_t)(k[i] >> shift) & 255u;
+        uint32_t peers = __match_any_sync(0xffffffffu, d);
+        uint32_t before = __popc(peers & ((1u << lane) - 1u));
+        uint32_t old = cnt[warp][d];
+        __syncwarp();
+        if (before == 0) cnt[warp][d] = old + __popc(peers);
+        __syncwarp();
+        rank[i] = old + before;
+    }
+    __syncthreads();
+    {   // exclusive prefix over warps, per digit (thread = digit)
+        uint32_t run = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_THREADS / 32; w++) {
+            uint32_t c = cnt[w][threadIdx.x];
+            cnt[w][threadIdx.x] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; i++) {
+        int64_t j = base + i * 32 + lane;
+        if (j < n) {
+            uint32_t d = (uint32_t)(k[i] >> shift) & 255u;
+            uint32_t dst = goff[d] + cnt[warp][d] + rank[i];
+            key_out[dst] = k[i];
+            idx_out[dst] = v[i];
+        }
+    }
+}
+
+// ---- device-wide exclusive scan (u32), fixed grid, n may live on the device ------------------------
+#define SCAN_THREADS 256
+__device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t *sh)
+{
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    uint32_t t = 0;
+    for (int w = 0; w < SCAN_THREADS / 32; w++) t += sh[w];
+    __syncthreads();
+    return t;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_reduce(const uint32_t *__restrict__ in,
+                                                              const uint32_t *n_dev, uint32_t n_max,
+                                                              uint32_t *__restrict__ bsum)
+{
+    __shared__ uint32_t sh[SCAN_THREADS / 32];
+    uint32_t n = n_dev ? min(*n_dev, n_max) : n_max;
+    uint32_t chunk = ((n + gridDim.x - 1) / gridDim.x + SCAN_THREADS - 1) / SCAN_THREADS * SCAN_THREADS;
+    uint64_t lo = (uint64_t)blockIdx.x * chunk, hi = min((uint64_t)n, lo + chunk);
+    uint32_t s = 0;
+    for (uint64_t i = lo + threadIdx.x; i < hi; i += SCAN_THREADS) s += in[i];
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) bsum[blockIdx.x] = s;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const uint32_t *in, uint32_t *out,   // may alias
+                                                             const uint32_t *n_dev, uint32_t n_max,
+                                                             const uint32_t *__restrict__ bsum,
+                                                             uint32_t *total)
+{
+    __shared__ uint32_t sh[SCAN_THREADS / 32];
+    __shared__ uint32_t wsum[SCAN_THREADS / 32];
+    uint32_t n = n_dev ? min(*n_dev, n_max) : n_max;
+    uint32_t chunk = ((n + gridDim.x - 1) / gridDim.x + SCAN_THREADS - 1) / SCAN_THREADS * SCAN_THREADS;
+    uint64_t lo = (uint64_t)blockIdx.x * chunk, hi = min((uint64_t)n, lo + chunk);
+    uint32_t pre = 0, all = 0;
+    for (uint32_t b = threadIdx.x; b < gridDim.x; b += SCAN_THREADS) {
+        uint32_t v = bsum[b];
+        all += v;
+        if (b < blockIdx.x) pre += v;
+    }
+    pre = block_sum(pre, sh);
+    if (total && blockIdx.x == 0) {
+        all = block_sum(all, sh);
+        if (threadIdx.x == 0) *total = all;
+    }
+    uint32_t carry = pre;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (uint64_t i0 = lo; i0 < hi; i0 += SCAN_THREADS) {
+        uint64_t i = i0 + threadIdx.x;
+        uint32_t v = i < hi ? in[i] : 0u, x = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) wsum[warp] = x;
+        __syncthreads();
+        uint32_t wpre = 0, tot = 0;
+        for (int w = 0; w < SCAN_THREADS / 32; w++) {
+            uint32_t t = wsum[w];
+            if (w < warp) wpre += t;
+            tot += t;
+        }
+        if (i < hi) out[i] = carry + wpre + x - v;
+        carry += tot;
+        __syncthreads();
+    }
+}
+
+void dsk_exclusive_scan_u32(dsk_ctx *c, const uint32_t *in, uint32_t *out, const uint32_t *n_dev,
+                            uint32_t n_max, uint32_t *total_dev)
+{
+    int grid = c->nsm * 4;
+    if ((uint64_t)grid * SCAN_THREADS > (uint64_t)n_max) grid = (int)((n_max + SCAN_THREADS - 1) / SCAN_THREADS);
+    if (grid < 1) grid = 1;
+    k_scan_reduce<<<grid, SCAN_THREADS, 0, c->stream>>>(in, n_dev, n_max, c->scan_tmp);
+    k_scan_apply<<<grid, SCAN_THREADS, 0, c->stream>>>(in, out, n_dev, n_max, c->scan_tmp, total_dev);
+}
+
+// ---- gather / scatter ------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pos, const float *__restrict__ mass,
+                                                const uint32_t *__restrict__ order, int64_t n, float box,
+                                                int periodic, float4 *__restrict__ spos)
+{
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    uint32_t i = order[r];
+    float x = pos[3 * (size_t)i], y = pos[3 * (size_t)i + 1], z = pos[3 * (size_t)i + 2];
+    if (periodic) { x = dsk_wrap(x, box); y = dsk_wrap(y, box); z = dsk_wrap(z, box); }
+    spos[r] = make_float4(x, y, z, mass[i]);
+}
+
+__global__ void __launch_bounds__(256) k_scatter(const float4 *__restrict__ sacc,
+                                                 const uint32_t *__restrict__ order, int64_t n,
+                                                 float *__restrict__ acc, float *__restrict__ pot)
+{
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    uint32_t i = order[r];
+    float4 a = sacc[r];
+    acc[3 * (size_t)i] = a.x; acc[3 * (size_t)i + 1] = a.y; acc[3 * (size_t)i + 2] = a.z;
+    if (pot) pot[i] = a.w;
+}
+
+int dsk_run_keysort(dsk_ctx *c, const float *pos, const float *mass)
+{
+    const int64_t n = c->N;
+    const int nb = (int)((n + 255) / 256);
+    float scale = 2097152.0f / c->box;
+    cudaEventRecord(c->ev[0], c->stream);
+    k_keys<<<nb, 256, 0, c->stream>>>(pos, n, c->box, scale, c->periodic, c->key_a, c->idx_a, c->dstate);
+    cudaEventRecord(c->ev[1], c->stream);
+    uint64_t *ka = c->key_a, *kb = c->key_b;
+    uint32_t *ia = c->idx_a, *ib = c->idx_b;
+    const int ntile = c->ntile;
+    for (int pass = 0; pass < 8; pass++) {
+        int shift = 8 * pass;
+        k_sort_hist<<<ntile, SORT_THREADS, 0, c->stream>>>(ka, n, shift, ntile, c->sort_hist);
+        dsk_exclusive_scan_u32(c, c->sort_hist, c->sort_hist, nullptr, (uint32_t)(256u * (uint32_t)ntile), nullptr);
+        k_sort_scatter<<<ntile, SORT_THREADS, 0, c->stream>>>(ka, ia, n, shift, ntile, c->sort_hist, kb, ib);
+        uint64_t *tk = ka; ka = kb; kb = tk;
+        uint32_t *ti = ia; ia = ib; ib = ti;
+    }
+    // 8 passes: the result is back in (key_a, idx_a)
+    k_gather<<<nb, 256, 0, c->stream>>>(pos, mass, c->idx_a, n, c->box, c->periodic, c->spos);
+    cudaEventRecord(c->ev[2], c->stream);
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
+}
+
+int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot)
+{
+    const int nb = (int)((c->N + 255) / 256);
+    k_scatter<<<nb, 256, 0, c->stream>>>(c->sacc, c->idx_a, c->N, acc, pot);
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
+}

@@ -1,0 +1,176 @@
+// walk.cu — step W: warp-cooperative group tree walk under the opening-angle MAC.
+// DESIGN.md O5 ("this tree is traversed": the sinks of one sink cell share
+// the list of source cells; near the leaves the rest is done with direct interactions).
+//   accept cell c (image shift nL) for group g  iff  d^2 > (s_c/theta + delta_c)^2   (strict)
+//   d = distance from com_c + nL to the AABB of g's members.
+// accepted -> M2P list; rejected leaf -> P2P list; rejected internal -> children are visited.
+// One warp per group, 32 cells tested per step from a LIFO stack in shared memory (depth-first order
+// keeps it short); list entries are compacted with ballots and written as contiguous runs.
+// Run twice: COUNT (list lengths, for the offsets) and FILL.
+#include "dsk_internal.cuh"
+
+#define WW 4                 // warps per block
+#define WSTACK 2048          // stack entries per warp
+
+__device__ __forceinline__ void image_shift(int img, int periodic, float box, float sh[3])
+{
+    if (!periodic) { sh[0] = sh[1] = sh[2] = 0.0f; return; }
+    const int side = 2 * DSK_WS + 1;
+    int iz = img % side - DSK_WS, iy = (img / side) % side - DSK_WS, ix = img / (side * side) - DSK_WS;
+    sh[0] = ix * box; sh[1] = iy * box; sh[2] = iz * box;
+}
+
+template <bool FILL>
+__global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int periodic, float box,
+                                                  float inv_theta,
+                                                  const dsk_cellrec *__restrict__ cell,
+                                                  const float4 *__restrict__ whdr,
+                                                  const float4 *__restrict__ gbox,
+                                                  const uint32_t *__restrict__ gcount,
+                                                  uint32_t *__restrict__ m2p_len, uint32_t *__restrict__ p2p_len,
+                                                  uint32_t *__restrict__ p2p_src,
+                                                  const uint64_t *__restrict__ m2p_off,
+                                                  const uint64_t *__restrict__ p2p_off, uint64_t m2p_base,
+                                                  uint64_t p2p_base, uint32_t *__restrict__ list_m2p,
+                                                  uint32_t *__restrict__ list_p2p, dsk_devstate *st)
+{
+    __shared__ uint32_t stack[WW][WSTACK];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t g = g0 + blockIdx.x * WW + warp;
+    if (g >= g1) return;
+    const float4 blo = gbox[2 * (size_t)g], bhi = gbox[2 * (size_t)g + 1];
+    uint32_t *stk = stack[warp];
+    const int nimg = periodic ? (2 * DSK_WS + 1) * (2 * DSK_WS + 1) * (2 * DSK_WS + 1) : 1;
+    for (int i = lane; i < nimg; i += 32) stk[i] = (uint32_t)i << DSK_CELL_BITS;   // root of every image
+    __syncwarp();
+    int sp = nimg;
+    uint32_t nm = 0, np = 0, nsrc = 0;
+    uint64_t mo = 0, po = 0;
+    if (FILL) { mo = m2p_off[g] - m2p_base; po = p2p_off[g] - p2p_base; }
+    const uint32_t lt = (1u << lane) - 1u;
+    while (sp > 0) {
+        const int take = sp < 32 ? sp : 32;
+        uint32_t e = 0;
+        bool act = lane < take;
+        if (act) e = stk[sp - 1 - lane];
+        sp -= take;
+        __syncwarp();
+        bool accept = false, leaf = false;
+        uint32_t nchild = 0, child0 = 0, cnt = 0;
+        if (act) {
+            const uint32_t c = e & ((1u << DSK_CELL_BITS) - 1u);
+            const int img = (int)(e >> DSK_CELL_BITS);
+            const dsk_cellrec r = cell[c];
+            const float4 h = whdr[c];
+            float sh[3];
+            image_shift(img, periodic, box, sh);
+            const float zx = h.x + sh[0], zy = h.y + sh[1], zz = h.z + sh[2];
+            const float dx = fmaxf(fmaxf(blo.x - zx, zx - bhi.x), 0.0f);
+            const float dy = fmaxf(fmaxf(blo.y - zy, zy - bhi.y), 0.0f);
+            const float dz = fmaxf(fmaxf(blo.z - zz, zz - bhi.z), 0.0f);
+            const float d2 = dx * dx + dy * dy + dz * dz;
+            const int level = (int)(r.meta >> 8);
+            const float s = box * exp2f((float)-level);
+            const float rc = s * inv_theta + h.w;
+            accept = d2 > rc * rc;
+            nchild = r.meta & 255u; child0 = r.child0; cnt = r.count;
+            leaf = !accept && nchild == 0;
+        }
+        const uint32_t bm = __ballot_sync(0xffffffffu, accept);
+        const uint32_t bl = __ballot_sync(0xffffffffu, leaf);
+        if (FILL) {
+            if (accept) list_m2p[mo + nm + __popc(bm & lt)] = e;
+            if (leaf) list_p2p[po + np + __popc(bl & lt)] = e;
+        }
+        nm += __popc(bm); np += __popc(bl);
+        if (leaf) nsrc += cnt;
+        // push the children of rejected internal cells
+        const bool open = act && !accept && nchild != 0;
+        uint32_t push = open ? nchild : 0u, x = push;
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        const uint32_t tot = __shfl_sync(0xffffffffu, x, 31);
+        if (sp + (int)tot > WSTACK) {
+            if (lane == 0) atomicOr(&st->status, ST_STACKOVF);
+            break;
+        }
+        if (open) {
+            uint32_t at = sp + x - push;
+            const uint32_t img = e & ~((1u << DSK_CELL_BITS) - 1u);
+            for (uint32_t k = 0; k < nchild; k++) stk[at + k] = img | (child0 + k);
+        }
+        sp += (int)tot;
+        __syncwarp();
+    }
+    for (int o = 16; o; o >>= 1) nsrc += __shfl_xor_sync(0xffffffffu, nsrc, o);
+    if (lane == 0) {
+        if (!FILL) {
+            m2p_len[g] = nm; p2p_len[g] = np; p2p_src[g] = nsrc;
+        } else {
+            const unsigned long long ns = gcount[g];
+            atomicAdd(&st->n_m2p, ns * nm);
+            atomicAdd(&st->n_p2p, ns * nsrc);
+            atomicAdd(&st->tot_m2p_list, (unsigned long long)nm);
+            atomicAdd(&st->tot_p2p_list, (unsigned long long)np);
+            atomicAdd(&st->tot_p2p_src, (unsigned long long)nsrc);
+        }
+    }
+}
+
+// u32 lengths -> u64 exclusive offsets (single block per 64K-element strip, serial over strips: the
+// group count is small next to N, this is not a hot spot)
+__global__ void __launch_bounds__(1024) k_scan_u64(const uint32_t *__restrict__ len, uint32_t n,
+                                                   uint64_t *__restrict__ off)
+{
+    __shared__ uint64_t wsum[32];
+    __shared__ uint64_t carry_s;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (uint32_t i0 = 0; i0 < n; i0 += 1024) {
+        uint32_t i = i0 + threadIdx.x;
+        uint64_t v = i < n ? len[i] : 0, x = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            uint64_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) wsum[warp] = x;
+        __syncthreads();
+        uint64_t wpre = 0, tot = 0;
+        for (int w = 0; w < 32; w++) { uint64_t t = wsum[w]; if (w < warp) wpre += t; tot += t; }
+        uint64_t carry = carry_s;
+        if (i < n) off[i] = carry + wpre + x - v;
+        __syncthreads();
+        if (threadIdx.x == 0) carry_s = carry + tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) off[n] = carry_s;
+}
+
+// W, COUNT pass + offsets.  The FILL pass is issued per batch by dsk_walk_fill (force.cu drives it).
+int dsk_run_walk(dsk_ctx *c)
+{
+    const uint32_t ng = c->hstate->ngroup;
+    cudaStream_t s = c->stream;
+    const float inv_theta = 1.0f / c->theta;
+    cudaEventRecord(c->ev[7], s);
+    k_walk<false><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic, c->box, inv_theta, c->cell, c->whdr,
+                                                         c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len,
+                                                         c->g_p2p_src, nullptr, nullptr, 0, 0, nullptr, nullptr,
+                                                         c->dstate);
+    k_scan_u64<<<1, 1024, 0, s>>>(c->g_m2p_len, ng, c->g_m2p_off);
+    k_scan_u64<<<1, 1024, 0, s>>>(c->g_p2p_len, ng, c->g_p2p_off);
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
+}
+
+int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base)
+{
+    const float inv_theta = 1.0f / c->theta;
+    k_walk<true><<<(g1 - g0 + WW - 1) / WW, WW * 32, 0, c->stream>>>(
+        g0, g1, c->periodic, c->box, inv_theta, c->cell, c->whdr, c->gbox, c->gcount, c->g_m2p_len,
+        c->g_p2p_len, c->g_p2p_src, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p,
+        c->dstate);
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
+}

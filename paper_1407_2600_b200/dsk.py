@@ -1,0 +1,217 @@
+"""Thin Python binding over the C ABI of libdsk (include/dsk.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the ABI.  PyTorch is used for device memory
+(the workspace and the caller's tensors) and streams.  There is no CPU fallback: if libdsk.so is
+missing or no CUDA device is present, construction fails loudly.
+"""
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdsk.so")
+
+SYMBOLS = [
+    "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
+    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_kdk_step", "dsk_kdk_reset", "dsk_get_keys",
+    "dsk_get_tree", "dsk_get_moments", "dsk_get_groups", "dsk_get_stats", "dsk_get_param",
+    "dsk_get_lattice_tensors", "dsk_strerror",
+]
+
+
+class DskStats(C.Structure):
+    _fields_ = [(k, C.c_int64) for k in ("n", "ncell", "nleaf_cells", "ngroup", "nlevel", "n_p2p", "n_m2p",
+                                         "list_m2p", "list_p2p", "nbatch")] + \
+               [(k, C.c_float) for k in ("ms_key", "ms_sort", "ms_build", "ms_upward", "ms_group", "ms_walk",
+                                         "ms_p2p", "ms_m2p", "ms_far", "ms_scatter", "ms_kdk")]
+
+    def asdict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class DskError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"dsk error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library(path=LIB_PATH):
+    """dlopen libdsk.so and declare the prototypes (no compute call is made)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise ImportError(f"{path} not found: build it with `python -m paper_1407_2600_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(path)
+    vp, i64, f32, i32, f64 = C.c_void_p, C.c_int64, C.c_float, C.c_int, C.c_double
+    lib.dsk_create.argtypes = [C.POINTER(vp), i64, f32, i32, f32, f32, i32]
+    lib.dsk_destroy.argtypes = [vp]
+    lib.dsk_workspace_bytes.argtypes = [vp]
+    lib.dsk_workspace_bytes.restype = C.c_size_t
+    lib.dsk_bind_workspace.argtypes = [vp, vp, C.c_size_t]
+    lib.dsk_set_stream.argtypes = [vp, vp]
+    lib.dsk_set_params.argtypes = [vp, f32, f32, i32]
+    lib.dsk_build_tree.argtypes = [vp, vp, vp]
+    lib.dsk_accel.argtypes = [vp, vp, vp, vp, vp]
+    lib.dsk_kdk_step.argtypes = [vp, vp, vp, vp, f64, f64]
+    lib.dsk_kdk_reset.argtypes = [vp]
+    lib.dsk_get_keys.argtypes = [vp, vp, vp]
+    lib.dsk_get_tree.argtypes = [vp, C.POINTER(i64), vp, vp, vp, vp]
+    lib.dsk_get_moments.argtypes = [vp, vp, vp]
+    lib.dsk_get_groups.argtypes = [vp, C.POINTER(i64), vp, vp, vp, vp, vp]
+    lib.dsk_get_stats.argtypes = [vp, C.POINTER(DskStats)]
+    lib.dsk_get_param.argtypes = [C.c_char_p, C.POINTER(f64)]
+    lib.dsk_get_lattice_tensors.argtypes = [vp, vp]
+    lib.dsk_strerror.argtypes = [i32]
+    lib.dsk_strerror.restype = C.c_char_p
+    for s in SYMBOLS:
+        if s not in ("dsk_workspace_bytes", "dsk_strerror"):
+            getattr(lib, s).restype = i32
+    _lib = lib
+    return lib
+
+
+def get_param(name):
+    v = C.c_double(0)
+    _check(load_library().dsk_get_param(name.encode(), C.byref(v)))
+    return v.value
+
+
+def _check(code):
+    if code != 0:
+        raise DskError(code, load_library().dsk_strerror(code).decode())
+
+
+def nparams(p):
+    return (p + 1) * (p + 2) * (p + 3) // 6
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+def _dev_f32(t, shape=None):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError("expected a contiguous float32 CUDA tensor")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"expected shape {shape}, got {tuple(t.shape)}")
+    return t
+
+
+class Dsk:
+    """One dsk_ctx plus the torch-owned workspace it borrows."""
+
+    def __init__(self, N, box=1.0, periodic=False, eps=1e-3, theta=0.5, p=4, device="cuda:0", stream=None):
+        self.lib = load_library()
+        if not torch.cuda.is_available():
+            raise RuntimeError("dsk needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.device = torch.device(device)
+        self.N, self.box, self.periodic = int(N), float(box), bool(periodic)
+        self.eps, self.theta, self.p = float(eps), float(theta), int(p)
+        h = C.c_void_p(0)
+        _check(self.lib.dsk_create(C.byref(h), self.N, self.box, int(self.periodic), self.eps, self.theta, self.p))
+        self._h = h
+        with torch.cuda.device(self.device):
+            nbytes = self.lib.dsk_workspace_bytes(self._h)
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self.workspace.data_ptr() + 255) & ~255
+            s = stream if stream is not None else torch.cuda.current_stream(self.device)
+            _check(self.lib.dsk_set_stream(self._h, C.c_void_p(s.cuda_stream)))
+            _check(self.lib.dsk_bind_workspace(self._h, C.c_void_p(base), nbytes))
+        self.workspace_bytes = nbytes
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.dsk_destroy(self._h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- the calls of include/dsk.h ------------------------------------------------------------------
+    def set_stream(self, stream):
+        _check(self.lib.dsk_set_stream(self._h, C.c_void_p(stream.cuda_stream)))
+
+    def set_params(self, eps=None, theta=None, p=None):
+        self.eps = self.eps if eps is None else float(eps)
+        self.theta = self.theta if theta is None else float(theta)
+        self.p = self.p if p is None else int(p)
+        _check(self.lib.dsk_set_params(self._h, self.eps, self.theta, self.p))
+
+    def build_tree(self, pos, mass):
+        _dev_f32(pos, (self.N, 3)); _dev_f32(mass, (self.N,))
+        _check(self.lib.dsk_build_tree(self._h, _ptr(pos), _ptr(mass)))
+
+    def accel(self, pos, mass, acc=None, pot=None, want_pot=True):
+        _dev_f32(pos, (self.N, 3)); _dev_f32(mass, (self.N,))
+        if acc is None:
+            acc = torch.empty((self.N, 3), dtype=torch.float32, device=self.device)
+        if pot is None and want_pot:
+            pot = torch.empty(self.N, dtype=torch.float32, device=self.device)
+        _check(self.lib.dsk_accel(self._h, _ptr(pos), _ptr(mass), _ptr(_dev_f32(acc, (self.N, 3))),
+                                  _ptr(pot) if pot is not None else None))
+        return acc, pot
+
+    def kdk_step(self, pos, vel, mass, a, da):
+        _dev_f32(pos, (self.N, 3)); _dev_f32(vel, (self.N, 3)); _dev_f32(mass, (self.N,))
+        _check(self.lib.dsk_kdk_step(self._h, _ptr(pos), _ptr(vel), _ptr(mass), float(a), float(da)))
+
+    def kdk_reset(self):
+        _check(self.lib.dsk_kdk_reset(self._h))
+
+    # ---- introspection -----------------------------------------------------------------------------------
+    def get_keys(self):
+        keys = torch.empty(self.N, dtype=torch.int64, device=self.device)       # bit pattern of uint64
+        order = torch.empty(self.N, dtype=torch.int32, device=self.device)      # bit pattern of uint32
+        _check(self.lib.dsk_get_keys(self._h, _ptr(keys), _ptr(order)))
+        return keys, order
+
+    def get_tree(self):
+        n = C.c_int64(0)
+        _check(self.lib.dsk_get_tree(self._h, C.byref(n), None, None, None, None))
+        nc = n.value
+        hot = torch.empty(nc, dtype=torch.int64, device=self.device)
+        first = torch.empty(nc, dtype=torch.int32, device=self.device)
+        count = torch.empty(nc, dtype=torch.int32, device=self.device)
+        nchild = torch.empty(nc, dtype=torch.uint8, device=self.device)
+        _check(self.lib.dsk_get_tree(self._h, C.byref(n), _ptr(hot), _ptr(first), _ptr(count), _ptr(nchild)))
+        return dict(ncell=nc, hotkey=hot, first=first, count=count, nchild=nchild)
+
+    def get_moments(self):
+        nc = self.get_stats()["ncell"]
+        com_mass = torch.empty((nc, 4), dtype=torch.float32, device=self.device)
+        mom = torch.empty((nc, nparams(self.p)), dtype=torch.float32, device=self.device)
+        _check(self.lib.dsk_get_moments(self._h, _ptr(com_mass), _ptr(mom)))
+        return com_mass, mom
+
+    def get_groups(self):
+        n = C.c_int64(0)
+        _check(self.lib.dsk_get_groups(self._h, C.byref(n), None, None, None, None, None))
+        ng = n.value
+        first = torch.empty(ng, dtype=torch.int32, device=self.device)
+        count = torch.empty(ng, dtype=torch.int32, device=self.device)
+        bbox = torch.empty((ng, 6), dtype=torch.float32, device=self.device)
+        m2p = torch.empty(ng, dtype=torch.int32, device=self.device)
+        p2p = torch.empty(ng, dtype=torch.int32, device=self.device)
+        _check(self.lib.dsk_get_groups(self._h, C.byref(n), _ptr(first), _ptr(count), _ptr(bbox), _ptr(m2p), _ptr(p2p)))
+        return dict(ngroup=ng, first=first, count=count, bbox=bbox, m2p_len=m2p, p2p_len=p2p)
+
+    def get_stats(self):
+        st = DskStats()
+        _check(self.lib.dsk_get_stats(self._h, C.byref(st)))
+        return st.asdict()
+
+    def get_lattice_tensors(self):
+        import numpy as np
+        T = np.empty(165, dtype=np.float64)
+        _check(self.lib.dsk_get_lattice_tensors(self._h, T.ctypes.data_as(C.c_void_p)))
+        return T

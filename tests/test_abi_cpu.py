@@ -1,0 +1,77 @@
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/dsk.h declares, and
+its host-only logic (argument validation, workspace sizing, constants, the fp64 lattice tensors of the
+periodic far field) is right.  No compute call is made (there is no GPU here)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1407_2600_b200 import build, dsk
+    build.build()
+    return dsk.load_library()
+
+
+def test_exports_every_declared_symbol(lib):
+    hdr = open(os.path.join(ROOT, "include", "dsk.h")).read()
+    declared = set(re.findall(r"\b(dsk_[a-z_]+)\s*\(", hdr))
+    assert len(declared) >= 18
+    from paper_1407_2600_b200 import dsk
+    assert declared == set(dsk.SYMBOLS)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_constants_match_oracle_conventions(lib, orc):
+    from paper_1407_2600_b200 import dsk
+    assert dsk.get_param("NLEAF") == orc.NLEAF and dsk.get_param("NCRIT") == orc.NCRIT
+    assert dsk.get_param("WS") == orc.WS and dsk.get_param("KEY_LEVELS") == orc.KEY_LEVELS
+    assert dsk.get_param("FAR_ORDER") == orc.FAR_ORDER
+    with pytest.raises(dsk.DskError):
+        dsk.get_param("NOPE")
+
+
+def test_create_validation_and_workspace(lib):
+    h = C.c_void_p(0)
+    bad = [(0, 1.0, 0, 1e-3, 0.5, 4), (10, -1.0, 0, 1e-3, 0.5, 4), (10, 1.0, 0, 0.0, 0.5, 4),
+           (10, 1.0, 0, 1e-3, 0.0, 4), (10, 1.0, 0, 1e-3, 1.5, 4), (10, 1.0, 0, 1e-3, 0.5, 3),
+           (10, 1.0, 0, 1e-3, 0.5, 10)]
+    for a in bad:
+        assert lib.dsk_create(C.byref(h), *a) == -1
+    assert lib.dsk_create(C.byref(h), 1 << 20, 1.0, 0, 1e-4, 0.5, 4) == 0
+    b1 = lib.dsk_workspace_bytes(h)
+    assert 200e6 < b1 < 4e9                     # ~1.3 kB per particle
+    # calls that need a workspace / tree fail cleanly without touching the device
+    assert lib.dsk_build_tree(h, C.c_void_p(256), C.c_void_p(256)) == -2
+    assert lib.dsk_accel(h, C.c_void_p(256), C.c_void_p(256), C.c_void_p(256), None) == -2
+    assert lib.dsk_bind_workspace(h, C.c_void_p(0), b1) == -2
+    assert lib.dsk_bind_workspace(h, C.c_void_p(257), b1) == -2
+    assert lib.dsk_set_params(h, 1e-4, 0.3, 8) == 0 and lib.dsk_set_params(h, 1e-4, 0.3, 5) == -1
+    assert lib.dsk_destroy(h) == 0
+    assert lib.dsk_strerror(-4).decode().startswith("position outside")
+    h2 = C.c_void_p(0)
+    assert lib.dsk_create(C.byref(h2), 1 << 21, 1.0, 0, 1e-4, 0.5, 4) == 0
+    assert 1.8 < lib.dsk_workspace_bytes(h2) / b1 < 2.2
+    lib.dsk_destroy(h2)
+
+
+def test_lattice_tensors_match_oracle(lib, orc):
+    """the library's own fp64 host computation of T_n (farfield.cu) against the pinned oracle"""
+    for box in (1.0, 2.0):
+        h = C.c_void_p(0)
+        assert lib.dsk_create(C.byref(h), 100, box, 1, 1e-3, 0.5, 4) == 0
+        T = np.empty(165)
+        assert lib.dsk_get_lattice_tensors(h, T.ctypes.data_as(C.c_void_p)) == 0
+        ref = orc.farfield_T(box, orc.WS, 8)
+        assert np.max(np.abs(T - ref)) < 1e-10 * max(1.0, np.abs(ref).max())
+        lib.dsk_destroy(h)
+    h = C.c_void_p(0)
+    lib.dsk_create(C.byref(h), 100, 1.0, 0, 1e-3, 0.5, 4)
+    assert lib.dsk_get_lattice_tensors(h, T.ctypes.data_as(C.c_void_p)) == -1     # isolated: none
+    lib.dsk_destroy(h)
