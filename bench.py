@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the whole tree-force hot path on the configuration BASELINE.json's metric is
+quoted on: configs[1], the isolated Plummer sphere N = 2^20, eps = 1e-4, theta = 0.5, p = 4.
+
+A "step" is one full force evaluation of one batch of N particles: dsk_build_tree (keys, sort, gather,
+octree, groups, upward pass) + dsk_accel (walk, P2P, M2P, scatter), acc and pot in caller order.
+
+    python bench.py --gpus N --steps K --warmup W            (N > 1: launched under torchrun)
+    python bench.py --impl reference ...                     (the CPU oracle, timed as it stands)
+
+Prints ONE JSON line (rank 0).  value = particles whose force was evaluated per second over all ranks
+(replicas: the path does not shard in this build — DESIGN.md "multi-GPU"), timed with CUDA events on the
+stream the kernels run on, L2 flushed between steps, max over ranks.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "particle forces/sec"
+UNIT = "particles/s"
+CFG = 2
+
+
+def workload():
+    from paper_1407_2600_b200 import workloads
+    cfg = dict(workloads.CONFIGS[CFG])
+    pos, mass = workloads.make(CFG)
+    return cfg, pos, mass
+
+
+def config_dict(cfg, n_gpus):
+    return {"workload": "BASELINE.json configs[1]: isolated Plummer sphere, a=0.01 cut 20a, equal masses",
+            "N": cfg["N"], "eps": cfg["eps"], "theta": cfg["theta"], "p": cfg["p"], "periodic": False,
+            "step": "dsk_build_tree + dsk_accel (acc+pot)", "NLEAF": 16, "NCRIT": 64,
+            "l2": "256 MiB buffer written between steps (outside the event pairs); working set ~1 GB > L2",
+            "parallelism": f"replicas x{n_gpus}" if n_gpus > 1 else "single GPU"}
+
+
+# ---- clocks ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index=0):
+        self.gpu = gpu_index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.gpu)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---- multi-rank aggregation (also exercised on CPU with gloo in tests/test_bench_dist_cpu.py) -----------
+def aggregate(dist, ms_local, units_local, device=None):
+    """max of the per-rank times, sum of the per-rank units -> (ms_max, units_total)"""
+    import torch
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(ms_local), float(units_local)
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    u = torch.tensor([float(units_local)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ---- the CPU oracle, timed as it stands -------------------------------------------------------------------
+def oracle_rate(cfg, pos, mass, nsink, seconds_hint=None):
+    """particles/s of the oracle tree Tr on this host: tree build + moments timed in full, the force
+    evaluation on `nsink` sinks and extrapolated to all N (labelled so)."""
+    import oracle
+    from paper_1407_2600_b200 import workloads
+    n = len(pos)
+    t0 = time.perf_counter()
+    tree = oracle.OracleTree(pos, mass, cfg["box"], cfg["periodic"])
+    tree.moments(cfg["p"])
+    t_build = time.perf_counter() - t0
+    # the sample is whole sink groups (every member of ~nsink/18 randomly chosen groups), so the walk
+    # is shared by a group's sinks exactly as in a full evaluation
+    g = tree.groups()
+    _, order = tree.sorted()
+    rng = np.random.Generator(np.random.PCG64(workloads.SEED0 + CFG + 100))
+    picked, tot = [], 0
+    for gi in rng.permutation(tree.ngroup):
+        picked.append(order[g["first"][gi]:g["first"][gi] + g["count"][gi]].astype(np.int64))
+        tot += int(g["count"][gi])
+        if tot >= nsink:
+            break
+    sink = np.concatenate(picked)
+    t0 = time.perf_counter()
+    tree.accel(cfg["eps"], cfg["theta"], cfg["p"], sink, want_pot=True)
+    t_force = time.perf_counter() - t0
+    t_step = t_build + t_force * (n / len(sink))
+    return n / t_step, dict(t_build_s=round(t_build, 3), t_force_sample_s=round(t_force, 3), nsink=int(len(sink)),
+                            cores=oracle.threads())
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg, pos, mass = workload()
+    n = len(pos)
+    nsink = 16384
+    rates, info = [], None
+    for it in range(args.warmup + args.steps):
+        r, info = oracle_rate(cfg, pos, mass, nsink)
+        if it >= args.warmup:
+            rates.append(r)
+    value = float(np.mean(rates))
+    sample = (f"oracle tree Tr (fp64, OpenMP): tree build + moments on all N, forces on a {info['nsink']}-sink "
+              f"sample (whole sink groups) extrapolated to N={n}")
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * n / value, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": config_dict(cfg, 1),
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": info["cores"], "kind": "oracle", "sample": sample},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+# ---- our arm ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1407_2600_b200 import accounting, dsk
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    use_dist = world > 1
+    if use_dist:
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg, pos, mass = workload()
+    n = len(pos)
+    d = dsk.Dsk(n, cfg["box"], cfg["periodic"], cfg["eps"], cfg["theta"], cfg["p"], device=dev)
+    stream = torch.cuda.current_stream(dev)
+    tp, tm = torch.from_numpy(pos).to(dev), torch.from_numpy(mass).to(dev)
+    acc = torch.empty((n, 3), dtype=torch.float32, device=dev)
+    pot = torch.empty(n, dtype=torch.float32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    # pinned host buffers for the end-to-end arm
+    hp, hm = torch.from_numpy(pos).pin_memory(), torch.from_numpy(mass).pin_memory()
+    hacc = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    hpot = torch.empty(n, dtype=torch.float32).pin_memory()
+    tp2, tm2 = torch.empty_like(tp), torch.empty_like(tm)
+
+    def step():
+        d.build_tree(tp, tm)
+        d.accel(tp, tm, acc, pot)
+
+    def step_e2e():
+        tp2.copy_(hp, non_blocking=True); tm2.copy_(hm, non_blocking=True)
+        d.build_tree(tp2, tm2)
+        d.accel(tp2, tm2, acc, pot)
+        hacc.copy_(acc, non_blocking=True); hpot.copy_(pot, non_blocking=True)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if use_dist:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def timed(fn, steps):
+        """sum over steps of the CUDA-event time of each step on the launching stream; L2 flushed between"""
+        tot = 0.0
+        phase = {}
+        for _ in range(steps):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+            e1.synchronize()
+            tot += e0.elapsed_time(e1)
+            st = d.get_stats()
+            for k, v in st.items():
+                if k.startswith("ms_"):
+                    phase[k] = phase.get(k, 0.0) + v
+        return tot, {k: v / steps for k, v in phase.items()}, st
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    ms_total, phase, st = timed(step, args.steps)
+    barrier()
+    clk = clocks.stop() if rank == 0 else None
+    ms_max, units = aggregate(dist if use_dist else None, ms_total, n * args.steps, dev)
+    value = units / (ms_max * 1e-3)
+
+    # end-to-end: pinned host -> device, the same step, device -> pinned host, all inside the event pair
+    for _ in range(2):
+        step_e2e()
+    barrier()
+    ms_e2e, _, _ = timed(step_e2e, args.steps)
+    barrier()
+    ms_e2e_max, units_e = aggregate(dist if use_dist else None, ms_e2e, n * args.steps, dev)
+    e2e_value = units_e / (ms_e2e_max * 1e-3)
+
+    out = None
+    if rank == 0:
+        prop = torch.cuda.get_device_properties(dev)
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+        peak_fp32 = accounting.fp32_peak_flops(prop.multi_processor_count, sm_max)
+        f_m2p = accounting.m2p_flops(cfg["p"], pot=True)
+        f_p2p = accounting.p2p_flops(pot=True)
+        ach_m2p = f_m2p * st["n_m2p"] / (phase["ms_m2p"] * 1e-3)
+        ach_p2p = f_p2p * st["n_p2p"] / (phase["ms_p2p"] * 1e-3) if phase["ms_p2p"] > 0 else 0.0
+        hbm = float(peaks.get("hbm_gbs", 6650.0))
+        bpp = accounting.BYTES_PER_PARTICLE
+        hbm_phases = {}
+        for k, key in (("ms_key", "key"), ("ms_sort", "sort")):
+            if phase.get(k, 0) > 0:
+                b = (bpp[key] + (bpp["gather"] if key == "sort" else 0)) * n
+                hbm_phases[key] = {"GBps": b / (phase[k] * 1e-3) / 1e9, "frac": b / (phase[k] * 1e-3) / 1e9 / hbm}
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "m2p_dram_bytes_per_launch.txt")
+        if os.path.exists(tpath):
+            try:
+                traffic = float(open(tpath).read().split()[0])
+            except Exception:
+                traffic = None
+        # CPU oracle beside it (bounded sample, rank 0, N = 1 only)
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            v, info = oracle_rate(cfg, pos, mass, 16384)
+            cpu = {"value": v, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
+                   "sample": (f"oracle tree Tr fp64 OpenMP: build+moments on all N ({info['t_build_s']} s), forces on "
+                              f"{info['nsink']} of {n} sinks = whole groups ({info['t_force_sample_s']} s) extrapolated to N")}
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+               "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+               "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+               "config": config_dict(cfg, world),
+               "roofline": {"bound": "alu", "kernel": "k_m2p<4,pot,packed>", "achieved": ach_m2p / 1e12,
+                            "peak": peak_fp32 / 1e12, "unit": "TFLOP/s", "frac": ach_m2p / peak_fp32,
+                            "traffic": traffic,
+                            "peak_source": f"nominal FP32: {prop.multi_processor_count} SMs x 128 lanes x 2 x {sm_max:.0f} MHz "
+                                           "(DESIGN.md; FFMA2 microbenchmark measured 74.06 TFLOP/s on this pool)",
+                            "flop_per_interaction": f_m2p, "interactions_per_launch": st["n_m2p"],
+                            "ms_per_launch": phase["ms_m2p"]},
+               "kernels": {"p2p": {"TFLOPs": ach_p2p / 1e12, "frac_fp32_peak": ach_p2p / peak_fp32,
+                                   "pairs_per_s": st["n_p2p"] / (phase["ms_p2p"] * 1e-3) if phase["ms_p2p"] > 0 else None,
+                                   "flop_per_pair": f_p2p},
+                           "m2p": {"interactions_per_s": st["n_m2p"] / (phase["ms_m2p"] * 1e-3)},
+                           "hbm_phases": hbm_phases},
+               "interactions_per_s": (st["n_m2p"] + st["n_p2p"]) * world / (ms_max / args.steps * 1e-3),
+               "phase_ms": {k[3:]: round(v, 4) for k, v in phase.items()},
+               "tree": {"ncell": st["ncell"], "ngroup": st["ngroup"], "nlevel": st["nlevel"],
+                        "n_p2p": st["n_p2p"], "n_m2p": st["n_m2p"], "nbatch": st["nbatch"]},
+               "cpu_baseline": cpu,
+               "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(hp.numel() * 4 + hm.numel() * 4),
+                       "d2h_bytes_per_step": int(hacc.numel() * 4 + hpot.numel() * 4),
+                       "ms_per_step": ms_e2e_max / args.steps},
+               "gpu_launches": int(st["n_launch"]) * args.steps,
+               "clocks": clk}
+    d.close()
+    if use_dist:
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -61,6 +61,7 @@ typedef struct dsk_stats {
     int64_t list_m2p;         /* total M2P list entries (cells) over all groups                        */
     int64_t list_p2p;         /* total P2P list entries (leaves) over all groups                       */
     int64_t nbatch;           /* list batches the evaluation was split in                              */
+    int64_t n_launch;         /* kernels launched since the last dsk_build_tree began (inclusive)      */
     float ms_key, ms_sort, ms_build, ms_upward, ms_group, ms_walk, ms_p2p, ms_m2p, ms_far, ms_scatter,
           ms_kdk;
 } dsk_stats;

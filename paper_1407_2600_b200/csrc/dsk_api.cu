@@ -32,6 +32,7 @@ static size_t carve(dsk_ctx *c, char *base)
     c->scan_tmp = (uint32_t *)take(4 * 4096);
     c->spos = (float4 *)take(16 * n);
     c->sacc = (float4 *)take(16 * n);
+    c->sacc_lo = (float4 *)take(16 * n);
     c->hotkey = (uint64_t *)take(8 * nc);
     c->cell = (dsk_cellrec *)take(16 * nc);
     c->parent = (uint32_t *)take(4 * nc);
@@ -49,10 +50,10 @@ static size_t carve(dsk_ctx *c, char *base)
     c->g_p2p_src = (uint32_t *)take(4 * ng);
     c->g_m2p_off = (uint64_t *)take(8 * (ng + 1));
     c->g_p2p_off = (uint64_t *)take(8 * (ng + 1));
-    // interaction lists: ~100 / ~12 entries per particle cover theta >= 0.4 in one batch; smaller theta
-    // or very large N run in batches of groups (force.cu)
-    c->list_m2p_cap = n * 100 + (1u << 20);
-    c->list_p2p_cap = n * 12 + (1u << 18);
+    // interaction lists: 256 / 32 entries per particle cover theta >= 0.3 in one batch on the paper-like
+    // workloads; anything longer (or very large N) runs in batches of groups (force.cu)
+    c->list_m2p_cap = n * 256 + (1u << 20);
+    c->list_p2p_cap = n * 32 + (1u << 18);
     const size_t cap_entries = (size_t)3 << 30;                    // 12 GiB of u32 per list at most
     if (c->list_m2p_cap > cap_entries) c->list_m2p_cap = cap_entries;
     if (c->list_p2p_cap > cap_entries / 4) c->list_p2p_cap = cap_entries / 4;
@@ -62,7 +63,7 @@ static size_t carve(dsk_ctx *c, char *base)
     c->far_partial = (double *)take(8 * DSK_NFAR * 1024);
     c->far_M = (double *)take(8 * DSK_NFAR);
     c->far_T_dev = (double *)take(8 * DSK_NFAR);
-    c->far_lambda = (float *)take(4 * DSK_NFAR);
+    c->far_lambda = (double *)take(8 * DSK_NFAR);
     return o;
 }
 
@@ -179,6 +180,7 @@ extern "C" int dsk_build_tree(dsk_ctx *c, const float *pos, const float *mass)
     if (!c || !pos || !mass) return DSK_EINVAL;
     if (!c->ws) return DSK_ENOWORKSPACE;
     c->have_tree = 0; c->moments_p = -1; c->lists_valid = 0;
+    c->stats.n_launch = 0;
     DSK_CUDA(cudaMemsetAsync(c->dstate, 0, sizeof(dsk_devstate), c->stream));
     int e = dsk_run_keysort(c, pos, mass);
     if (e) return e;

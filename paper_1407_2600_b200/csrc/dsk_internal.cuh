@@ -60,7 +60,8 @@ struct dsk_ctx {
     uint32_t *sort_hist;      // [ntile * 256] per-pass tile histograms (digit-major)
     uint32_t *scan_tmp;       // block sums for the generic scan
     float4 *spos;             // sorted (x,y,z,m); periodic: wrapped
-    float4 *sacc;             // sorted (ax,ay,az,pot)
+    float4 *sacc;             // sorted (ax,ay,az,pot), high part of the compensated sum
+    float4 *sacc_lo;          // low part (two-float accumulators across tiles, kernels and the far field)
     uint64_t *hotkey;
     dsk_cellrec *cell;
     uint32_t *parent;
@@ -78,7 +79,7 @@ struct dsk_ctx {
     float *kdk_acc;           // [N,3] cached force, caller order
     double *far_partial;      // [nblk * 165]
     double *far_M;            // [165]
-    float *far_lambda;        // [165]
+    double *far_lambda;       // [165]
     double *far_T_dev;        // [165]
     dsk_devstate *dstate;     // device
     dsk_devstate *hstate;     // pinned host
@@ -94,6 +95,7 @@ struct dsk_ctx {
     int nsm;
 };
 
+#define DSK_COUNT(c, k) ((c)->stats.n_launch += (k))
 #define DSK_CUDA(x)                                 \
     do {                                            \
         cudaError_t e__ = (x);                      \
@@ -169,5 +171,16 @@ __device__ __forceinline__ f2 f2_sub(f2 a, f2 b)
 __device__ __forceinline__ f2 f2_rsqrt(f2 a)
 {
     return f2_make(rsqrtf(f2_lo(a)), rsqrtf(f2_hi(a)));
+}
+#endif
+
+#ifdef __CUDACC__
+// two-float accumulation: (hi, lo) += t without losing the rounding error of the addition (TwoSum)
+__device__ __forceinline__ void dsk_fold(float &hi, float &lo, float t)
+{
+    const float s = hi + t;
+    const float bb = s - hi;
+    lo += (hi - (s - bb)) + (t - bb);
+    hi = s;
 }
 #endif

@@ -195,7 +195,7 @@ __global__ void __launch_bounds__(FM_THREADS) k_far_moments(const float4 *__rest
 // (b) reduce partials, then Lambda_n = sum_{|k| <= 8-|n|} (-1)^|k| C(n+k,k) M_k T_{n+k}
 __global__ void __launch_bounds__(FM_THREADS) k_far_lambda(const double *__restrict__ partial, int nblk,
                                                            const double *__restrict__ T, double *__restrict__ M,
-                                                           float *__restrict__ lambda)
+                                                           double *__restrict__ lambda)
 {
     __shared__ double sM[NF];
     __shared__ double binom[2 * FO + 1][2 * FO + 1];
@@ -220,7 +220,7 @@ __global__ void __launch_bounds__(FM_THREADS) k_far_lambda(const double *__restr
             const double sg = (kl & 1) ? -1.0 : 1.0;
             s += sg * binom[a + ka][ka] * binom[b + kb][kb] * binom[c + kc][kc] * sM[k] * T[dsk_midx(a + ka, b + kb, c + kc)];
         }
-        lambda[t] = (float)s;
+        lambda[t] = s;
     }
 }
 
@@ -233,40 +233,48 @@ __device__ __forceinline__ void sfor(F &&f)
     }
 }
 
-// (c) per particle: Horner-free, fully unrolled evaluation of the order-8 polynomial and its gradient
+// (c) per particle: fully unrolled evaluation of the order-8 polynomial and its gradient, in fp64 — the
+// far field cancels an O(1) part of the image-block sum, so it is combined with the two-float tree sum
+// in double and split back into (hi, lo).
 __global__ void __launch_bounds__(128) k_far_eval(const float4 *__restrict__ spos, uint32_t n, float half_box,
-                                                  const float *__restrict__ lambda, float4 *__restrict__ sacc)
+                                                  const double *__restrict__ lambda, float4 *__restrict__ sacc,
+                                                  float4 *__restrict__ sacc_lo)
 {
-    __shared__ float sl[NF];
+    __shared__ double sl[NF];
     for (int i = threadIdx.x; i < NF; i += blockDim.x) sl[i] = lambda[i];
     __syncthreads();
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float4 p = spos[i];
-    float px[FO + 1], py[FO + 1], pz[FO + 1];
-    px[0] = py[0] = pz[0] = 1.0f;
-    const float X = p.x - half_box, Y = p.y - half_box, Z = p.z - half_box;
+    double px[FO + 1], py[FO + 1], pz[FO + 1];
+    px[0] = py[0] = pz[0] = 1.0;
+    const double X = (double)p.x - (double)half_box, Y = (double)p.y - (double)half_box, Z = (double)p.z - (double)half_box;
 #pragma unroll
     for (int e = 1; e <= FO; e++) { px[e] = px[e - 1] * X; py[e] = py[e - 1] * Y; pz[e] = pz[e - 1] * Z; }
-    float pot = 0.0f, gx = 0.0f, gy = 0.0f, gz = 0.0f;
+    double pot = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
     sfor<0, FO + 1>([&](auto LL) {
         constexpr int l = decltype(LL)::value;
         sfor<0, l + 1>([&](auto KK) {
             constexpr int k = decltype(KK)::value;          // k = b + c, a = l - k
             sfor<0, k + 1>([&](auto CC) {
                 constexpr int c = decltype(CC)::value, b = k - c, a = l - k;
-                const float lam = sl[dsk_midx(a, b, c)];
-                const float yz = py[b] * pz[c];
-                pot = fmaf(lam * px[a], yz, pot);
-                if constexpr (a >= 1) gx = fmaf((float)a * lam * px[a - 1], yz, gx);
-                if constexpr (b >= 1) gy = fmaf((float)b * lam * px[a], py[b - 1] * pz[c], gy);
-                if constexpr (c >= 1) gz = fmaf((float)c * lam * px[a], py[b] * pz[c - 1], gz);
+                const double lam = sl[dsk_midx(a, b, c)];
+                const double yz = py[b] * pz[c];
+                pot = fma(lam * px[a], yz, pot);
+                if constexpr (a >= 1) gx = fma((double)a * lam * px[a - 1], yz, gx);
+                if constexpr (b >= 1) gy = fma((double)b * lam * px[a], py[b - 1] * pz[c], gy);
+                if constexpr (c >= 1) gz = fma((double)c * lam * px[a], py[b] * pz[c - 1], gz);
             });
         });
     });
-    float4 acc = sacc[i];
-    acc.x -= gx; acc.y -= gy; acc.z -= gz; acc.w += pot;
-    sacc[i] = acc;
+    const float4 h = sacc[i], l = sacc_lo[i];
+    const double tx = ((double)h.x + (double)l.x) - gx, ty = ((double)h.y + (double)l.y) - gy,
+                 tz = ((double)h.z + (double)l.z) - gz, tw = ((double)h.w + (double)l.w) + pot;
+    float4 oh, ol;
+    oh.x = (float)tx; oh.y = (float)ty; oh.z = (float)tz; oh.w = (float)tw;
+    ol.x = (float)(tx - (double)oh.x); ol.y = (float)(ty - (double)oh.y); ol.z = (float)(tz - (double)oh.z);
+    ol.w = (float)(tw - (double)oh.w);
+    sacc[i] = oh; sacc_lo[i] = ol;
 }
 
 int dsk_run_farfield(dsk_ctx *c)
@@ -278,6 +286,7 @@ int dsk_run_farfield(dsk_ctx *c)
     if ((int64_t)nblk * FM_TILE > c->N) nblk = (int)((c->N + FM_TILE - 1) / FM_TILE);
     k_far_moments<<<nblk, FM_THREADS, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_partial);
     k_far_lambda<<<1, FM_THREADS, 0, c->stream>>>(c->far_partial, nblk, c->far_T_dev, c->far_M, c->far_lambda);
-    k_far_eval<<<(n + 127) / 128, 128, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_lambda, c->sacc);
+    k_far_eval<<<(n + 127) / 128, 128, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_lambda, c->sacc, c->sacc_lo);
+    DSK_COUNT(c, 3);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }

@@ -140,7 +140,8 @@ __global__ void __launch_bounds__(FT) k_m2p(uint32_t g0, int periodic, float box
                                             const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
                                             const uint32_t *__restrict__ gcell, const uint32_t *__restrict__ list,
                                             const uint64_t *__restrict__ off, uint64_t base,
-                                            const uint32_t *__restrict__ len, float4 *__restrict__ sacc)
+                                            const uint32_t *__restrict__ len, float4 *__restrict__ sacc,
+                                            float4 *__restrict__ sacc_lo)
 {
     constexpr int NP = dsk_np(P), ROW = dsk_rowlen(P), TROW = M2P_HDR + NP;
     __shared__ uint32_t s_cell[M2P_TC];
@@ -156,7 +157,10 @@ __global__ void __launch_bounds__(FT) k_m2p(uint32_t g0, int periodic, float box
     const uint32_t n = len[g];
     const uint32_t *lst = list + (off[g] - base);
     using T = typename std::conditional<PACKED, f2, float>::type;
-    T pot = vdup<T>(0.0f), ax = vdup<T>(0.0f), ay = vdup<T>(0.0f), az = vdup<T>(0.0f);
+    // running sums as two-float (hi, lo) pairs, continued from the P2P kernel; each tile is summed from
+    // zero in plain fp32 and folded in with TwoSum, so no addition ever rounds at the size of the total
+    float4 hi = make_float4(0.f, 0.f, 0.f, 0.f), lo = hi;
+    if (t < (int)count) { hi = sacc[first + t]; lo = sacc_lo[first + t]; }
     const T X = vdup<T>(xs), Y = vdup<T>(ys), Z = vdup<T>(zs);
     for (uint32_t b0 = 0; b0 < n; b0 += M2P_TC) {
         const int ntc = (int)min((uint32_t)M2P_TC, n - b0);
@@ -192,21 +196,19 @@ __global__ void __launch_bounds__(FT) k_m2p(uint32_t g0, int periodic, float box
         }
         __syncthreads();
         if (warp_active) {
+            T pot = vdup<T>(0.0f), ax = vdup<T>(0.0f), ay = vdup<T>(0.0f), az = vdup<T>(0.0f);
             if constexpr (PACKED) {
                 const int npair = (ntc + 1) >> 1;
                 for (int k = 0; k < npair; k++) m2p_body<P, T, POT>(X, Y, Z, tile[k], 0, pot, ax, ay, az);
             } else {
                 for (int k = 0; k < ntc; k++) m2p_body<P, T, POT>(X, Y, Z, tile[k >> 1], k & 1, pot, ax, ay, az);
             }
+            dsk_fold(hi.x, lo.x, vsum(ax)); dsk_fold(hi.y, lo.y, vsum(ay)); dsk_fold(hi.z, lo.z, vsum(az));
+            if (POT) dsk_fold(hi.w, lo.w, -vsum(pot));
         }
         __syncthreads();
     }
-    if (t < (int)count) {
-        float4 a = sacc[first + t];
-        a.x += vsum(ax); a.y += vsum(ay); a.z += vsum(az);
-        if (POT) a.w -= vsum(pot);
-        sacc[first + t] = a;
-    }
+    if (t < (int)count) { sacc[first + t] = hi; sacc_lo[first + t] = lo; }
 }
 
 // ---- F1 ----------------------------------------------------------------------------------------------
@@ -217,7 +219,7 @@ __global__ void __launch_bounds__(FT) k_p2p(uint32_t g0, int periodic, float box
                                             const uint32_t *__restrict__ gcount, const uint32_t *__restrict__ gcell,
                                             const uint32_t *__restrict__ list, const uint64_t *__restrict__ off,
                                             uint64_t base, const uint32_t *__restrict__ len,
-                                            float4 *__restrict__ sacc)
+                                            float4 *__restrict__ sacc, float4 *__restrict__ sacc_lo)
 {
     __shared__ uint32_t s_first[FT];
     __shared__ uint32_t s_pref[FT + 1];
@@ -235,7 +237,7 @@ __global__ void __launch_bounds__(FT) k_p2p(uint32_t g0, int periodic, float box
     const bool warp_active = (uint32_t)(t & ~31) < count;
     const uint32_t n = len[g];
     const uint32_t *lst = list + (off[g] - base);
-    f2 ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f), pot = f2_dup(0.0f);
+    float4 hi = make_float4(0.f, 0.f, 0.f, 0.f), lo = hi;     // two-float running sums (see k_m2p)
     for (uint32_t b0 = 0; b0 < n; b0 += FT) {
         // one leaf (segment of sources) per thread; exclusive scan of the segment lengths
         uint32_t cnt = 0;
@@ -285,6 +287,7 @@ __global__ void __launch_bounds__(FT) k_p2p(uint32_t g0, int periodic, float box
             }
             __syncthreads();
             if (warp_active) {
+                f2 ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f), pot = f2_dup(0.0f);
                 const int npair = (int)(npad >> 1);
 #pragma unroll 4
                 for (int k = 0; k < npair; k++) {
@@ -301,16 +304,16 @@ __global__ void __launch_bounds__(FT) k_p2p(uint32_t g0, int periodic, float box
                     ax = f2_fma(dx, mri3, ax); ay = f2_fma(dy, mri3, ay); az = f2_fma(dz, mri3, az);
                     if (POT) pot = f2_sub(pot, mri);
                 }
+                dsk_fold(hi.x, lo.x, vsum(ax)); dsk_fold(hi.y, lo.y, vsum(ay)); dsk_fold(hi.z, lo.z, vsum(az));
+                if (POT) dsk_fold(hi.w, lo.w, vsum(pot));
             }
             __syncthreads();
         }
     }
     if (t < (int)count) {
-        float4 a;
-        a.x = vsum(ax); a.y = vsum(ay); a.z = vsum(az);
         // the sink's own leaf is always in the list: remove its self term -m_i/eps from the potential
-        a.w = POT ? vsum(pot) + me.w * rsqrtf(eps2) : 0.0f;
-        sacc[first + t] = a;
+        if (POT) dsk_fold(hi.w, lo.w, me.w * rsqrtf(eps2));
+        sacc[first + t] = hi; sacc_lo[first + t] = lo;
     }
 }
 
@@ -322,11 +325,11 @@ static void launch_m2p(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t base, int 
     if (want_pot)
         k_m2p<P, true, PACKED><<<g1 - g0, FT, 0, c->stream>>>(g0, c->periodic, c->box, e2, c->rows, c->spos, c->gfirst,
                                                               c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
-                                                              c->g_m2p_len, c->sacc);
+                                                              c->g_m2p_len, c->sacc, c->sacc_lo);
     else
         k_m2p<P, false, PACKED><<<g1 - g0, FT, 0, c->stream>>>(g0, c->periodic, c->box, e2, c->rows, c->spos, c->gfirst,
                                                                c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
-                                                               c->g_m2p_len, c->sacc);
+                                                               c->g_m2p_len, c->sacc, c->sacc_lo);
 }
 
 static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t mb, uint64_t pb, int want_pot, bool fill)
@@ -341,10 +344,10 @@ static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t mb, uint64_
     const int rowlen = dsk_rowlen(c->p);
     if (want_pot)
         k_p2p<true><<<g1 - g0, FT, 0, s>>>(g0, c->periodic, c->box, e2, rowlen, c->rows, c->cell, c->spos, c->gfirst,
-                                           c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc);
+                                           c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     else
         k_p2p<false><<<g1 - g0, FT, 0, s>>>(g0, c->periodic, c->box, e2, rowlen, c->rows, c->cell, c->spos, c->gfirst,
-                                            c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc);
+                                            c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     cudaEventRecord(c->ev[9], s);
     switch (c->p) {
     case 2: launch_m2p<2>(c, g0, g1, mb, want_pot); break;
@@ -354,6 +357,7 @@ static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t mb, uint64_
     default: return DSK_EINVAL;
     }
     cudaEventRecord(c->ev[10], s);
+    DSK_COUNT(c, 2);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
@@ -361,6 +365,7 @@ static void add_ms(cudaEvent_t a, cudaEvent_t b, float *acc)
 {
     float ms = 0.0f;
     if (cudaEventElapsedTime(&ms, a, b) == cudaSuccess) *acc += ms;
+    else cudaGetLastError();      // an event that was never recorded: not an error of the path
 }
 
 // W (fill) + F1 + F2 over all groups, in one batch when the lists fit, else in batches of groups.
@@ -405,8 +410,6 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     cudaMemcpyAsync(hm, c->g_m2p_off, sizeof(uint64_t) * ((size_t)ng + 1), cudaMemcpyDeviceToHost, s);
     cudaMemcpyAsync(hp, c->g_p2p_off, sizeof(uint64_t) * ((size_t)ng + 1), cudaMemcpyDeviceToHost, s);
     if (cudaStreamSynchronize(s) != cudaSuccess) { free(hm); return DSK_ECUDA; }
-    add_ms(c->ev[7], c->ev[8], &c->stats.ms_walk);      // COUNT pass only (ev[8] from a previous call is stale; reset below)
-    c->stats.ms_walk = 0.0f;
     uint32_t g0 = 0;
     int nb = 0, rc = DSK_OK;
     while (g0 < ng) {

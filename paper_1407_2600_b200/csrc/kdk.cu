@@ -28,6 +28,7 @@ int dsk_run_kick(dsk_ctx *c, float *vel, const float *acc, float k)
 {
     int64_t n3 = 3 * c->N;
     k_kick<<<(unsigned)((n3 + 255) / 256), 256, 0, c->stream>>>(vel, acc, n3, k);
+    DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
@@ -35,5 +36,6 @@ int dsk_run_drift(dsk_ctx *c, float *pos, const float *vel, float d)
 {
     int64_t n3 = 3 * c->N;
     k_drift<<<(unsigned)((n3 + 255) / 256), 256, 0, c->stream>>>(pos, vel, n3, d, c->box, c->periodic);
+    DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }

@@ -211,6 +211,7 @@ void dsk_exclusive_scan_u32(dsk_ctx *c, const uint32_t *in, uint32_t *out, const
     if (grid < 1) grid = 1;
     k_scan_reduce<<<grid, SCAN_THREADS, 0, c->stream>>>(in, n_dev, n_max, c->scan_tmp);
     k_scan_apply<<<grid, SCAN_THREADS, 0, c->stream>>>(in, out, n_dev, n_max, c->scan_tmp, total_dev);
+    DSK_COUNT(c, 2);
 }
 
 // ---- gather / scatter ------------------------------------------------------------------------------
@@ -226,7 +227,7 @@ __global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pos, c
     spos[r] = make_float4(x, y, z, mass[i]);
 }
 
-__global__ void __launch_bounds__(256) k_scatter(const float4 *__restrict__ sacc,
+__global__ void __launch_bounds__(256) k_scatter(const float4 *__restrict__ sacc, const float4 *__restrict__ sacc_lo,
                                                  const uint32_t *__restrict__ order, int64_t n,
                                                  float *__restrict__ acc, float *__restrict__ pot)
 {
@@ -234,6 +235,9 @@ __global__ void __launch_bounds__(256) k_scatter(const float4 *__restrict__ sacc
     if (r >= n) return;
     uint32_t i = order[r];
     float4 a = sacc[r];
+    const float4 l = sacc_lo[r];
+    a.x = (float)((double)a.x + (double)l.x); a.y = (float)((double)a.y + (double)l.y);
+    a.z = (float)((double)a.z + (double)l.z); a.w = (float)((double)a.w + (double)l.w);
     acc[3 * (size_t)i] = a.x; acc[3 * (size_t)i + 1] = a.y; acc[3 * (size_t)i + 2] = a.z;
     if (pot) pot[i] = a.w;
 }
@@ -260,12 +264,14 @@ int dsk_run_keysort(dsk_ctx *c, const float *pos, const float *mass)
     // 8 passes: the result is back in (key_a, idx_a)
     k_gather<<<nb, 256, 0, c->stream>>>(pos, mass, c->idx_a, n, c->box, c->periodic, c->spos);
     cudaEventRecord(c->ev[2], c->stream);
+    DSK_COUNT(c, 2 + 2 * 8);        // keys, gather, 8 x (hist, scatter); the scans count themselves
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
 int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot)
 {
     const int nb = (int)((c->N + 255) / 256);
-    k_scatter<<<nb, 256, 0, c->stream>>>(c->sacc, c->idx_a, c->N, acc, pot);
+    k_scatter<<<nb, 256, 0, c->stream>>>(c->sacc, c->sacc_lo, c->idx_a, c->N, acc, pot);
+    DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }

@@ -254,5 +254,6 @@ int dsk_run_build(dsk_ctx *c)
     const int64_t nwarp_blocks = (c->ngroup_cap * 32 + TB - 1) / TB;
     k_group_bbox<<<(unsigned)nwarp_blocks, TB, 0, s>>>(c->spos, c->gfirst, c->gcount, c->gbox, n, c->dstate);
     cudaEventRecord(c->ev[4], s);
+    DSK_COUNT(c, 1 + 2 * (DSK_KEY_LEVELS + 1) + 4);   // init, count+emit per level, mark/flag/emit/bbox
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }

@@ -199,6 +199,7 @@ static void launch_upward(dsk_ctx *c, const uint32_t *lvl_start, int nlevel)
         if (!n) continue;
         k_upward<P><<<(n + UW - 1) / UW, UW * 32, 0, c->stream>>>(beg, n, l, c->box, c->cell, c->hotkey,
                                                                   c->spos, c->rows, c->whdr);
+        DSK_COUNT(c, 1);
     }
 }
 

@@ -162,6 +162,7 @@ int dsk_run_walk(dsk_ctx *c)
                                                          c->dstate);
     k_scan_u64<<<1, 1024, 0, s>>>(c->g_m2p_len, ng, c->g_m2p_off);
     k_scan_u64<<<1, 1024, 0, s>>>(c->g_p2p_len, ng, c->g_p2p_off);
+    DSK_COUNT(c, 3);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
@@ -172,5 +173,6 @@ int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint6
         g0, g1, c->periodic, c->box, inv_theta, c->cell, c->whdr, c->gbox, c->gcount, c->g_m2p_len,
         c->g_p2p_len, c->g_p2p_src, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p,
         c->dstate);
+    DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }

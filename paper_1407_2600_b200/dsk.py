@@ -22,7 +22,7 @@ SYMBOLS = [
 
 class DskStats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("n", "ncell", "nleaf_cells", "ngroup", "nlevel", "n_p2p", "n_m2p",
-                                         "list_m2p", "list_p2p", "nbatch")] + \
+                                         "list_m2p", "list_p2p", "nbatch", "n_launch")] + \
                [(k, C.c_float) for k in ("ms_key", "ms_sort", "ms_build", "ms_upward", "ms_group", "ms_walk",
                                          "ms_p2p", "ms_m2p", "ms_far", "ms_scatter", "ms_kdk")]
 

@@ -46,7 +46,7 @@ def test_create_validation_and_workspace(lib):
         assert lib.dsk_create(C.byref(h), *a) == -1
     assert lib.dsk_create(C.byref(h), 1 << 20, 1.0, 0, 1e-4, 0.5, 4) == 0
     b1 = lib.dsk_workspace_bytes(h)
-    assert 200e6 < b1 < 4e9                     # ~1.3 kB per particle
+    assert 200e6 < b1 < 4e9                     # ~2 kB per particle
     # calls that need a workspace / tree fail cleanly without touching the device
     assert lib.dsk_build_tree(h, C.c_void_p(256), C.c_void_p(256)) == -2
     assert lib.dsk_accel(h, C.c_void_p(256), C.c_void_p(256), C.c_void_p(256), None) == -2

@@ -1,0 +1,55 @@
+"""Host-side logic of the multi-rank bench path on CPU: world_size 2, gloo.  The path does not shard in
+this build (replicas only), so the only cross-rank logic is the aggregation: max over ranks of
+the device time, sum over ranks of the units."""
+import os
+import sys
+
+import pytest
+
+torch = pytest.importorskip("torch")
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+    import bench
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ms, units = bench.aggregate(dist, 10.0 + 5.0 * rank, 1000 * (rank + 1))
+    dist.barrier()
+    dist.destroy_process_group()
+    q.put((rank, ms, units))
+
+
+def test_aggregate_world2_gloo():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=120) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, ms, units in res:
+        assert ms == 15.0 and units == 3000.0
+
+
+def test_aggregate_single():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.aggregate(None, 3.5, 7) == (3.5, 7.0)
+
+
+def test_accounting_matches_kernel_op_counts():
+    """flop accounting (roofline numerator) against the op counts read off the SASS of k_m2p<4> (256 FFMA2)."""
+    from paper_1407_2600_b200 import accounting
+    assert accounting.m2p_ops(4, pot=True)[0] == 256
+    assert accounting.p2p_flops(pot=True) == 19
+    assert accounting.m2p_flops(4) > accounting.m2p_flops(2) and accounting.m2p_flops(8) > accounting.m2p_flops(6)
+    assert abs(accounting.fp32_peak_flops(148, 1965.0) - 74.45e12) < 0.1e12

@@ -1,0 +1,318 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the thin binding) against the fp64 oracle on the
+same seeded inputs.  Bars (BASELINE.json north_star):
+  * keys, sort order, tree topology, groups: bit-exact;
+  * forces: E_rms(GPU vs direct) <= 1.1 * E_rms(oracle tree vs direct) + 1e-6, and the per-particle
+    relative difference from the oracle tree < 1e-4 at the 99.9th percentile.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1407_2600_b200 import workloads
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def dsk():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1407_2600_b200 import dsk as m
+    m.load_library()          # fails loudly if libdsk.so is missing: no CPU fallback
+    return m
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _erms(a, b):
+    return math.sqrt(((a - b) ** 2).sum() / (b ** 2).sum())
+
+
+def _check_structure(orc, d, pos, mass, box, periodic):
+    t = orc.OracleTree(pos, mass, box, periodic)
+    sk, order = t.sorted()
+    k, o = d.get_keys()
+    assert np.array_equal(k.cpu().numpy().view(np.uint64), sk)
+    assert np.array_equal(o.cpu().numpy().view(np.uint32), order)
+    tr, c = d.get_tree(), t.cells()
+    assert tr["ncell"] == t.ncell
+    assert np.array_equal(tr["hotkey"].cpu().numpy().view(np.uint64), c["hotkey"])
+    assert np.array_equal(tr["first"].cpu().numpy().view(np.uint32), c["first"])
+    assert np.array_equal(tr["count"].cpu().numpy().view(np.uint32), c["count"])
+    assert np.array_equal(tr["nchild"].cpu().numpy(), c["nchild"])
+    g, og = d.get_groups(), t.groups()
+    assert g["ngroup"] == t.ngroup
+    assert np.array_equal(g["first"].cpu().numpy().view(np.uint32), og["first"])
+    assert np.array_equal(g["count"].cpu().numpy().view(np.uint32), og["count"])
+    assert np.array_equal(g["bbox"].cpu().numpy(), og["bbox"])
+    return t
+
+
+def _force_gates(acc, ref_tree, ref_direct):
+    e_gpu, e_tree = _erms(acc, ref_direct), _erms(ref_tree, ref_direct)
+    assert e_gpu <= 1.1 * e_tree + 1e-6, (e_gpu, e_tree)
+    rel = np.linalg.norm(acc - ref_tree, axis=1) / np.linalg.norm(ref_tree, axis=1)
+    assert np.quantile(rel, 0.999) < 1e-4, (np.quantile(rel, 0.999), rel.max())
+    return e_gpu, e_tree
+
+
+# ---- structure: bit-exact ---------------------------------------------------------------------------
+STRUCT_CASES = {
+    "C1": lambda: (*workloads.make(1), 1.0, False),
+    "C2/8": lambda: (*workloads.make(2, 1 / 8), 1.0, False),
+    "C3/64": lambda: (*workloads.perturbed_lattice(32), 1.0, True),
+    "C4/512": lambda: (*workloads.clustered_box(32, 40, cfg=4), 1.0, True),
+    "ragged-5003": lambda: (*workloads.uniform_box(5003), 1.0, False),
+}
+
+
+@pytest.mark.parametrize("case", list(STRUCT_CASES))
+def test_keys_sort_tree_groups_bit_exact(dsk, orc, case):
+    pos, mass, box, periodic = STRUCT_CASES[case]()
+    d = dsk.Dsk(len(pos), box, periodic, 1e-3, 0.5, 4)
+    d.build_tree(_dev(pos), _dev(mass))
+    _check_structure(orc, d, pos, mass, box, periodic)
+    d.close()
+
+
+def test_adversarial_keys(dsk, orc):
+    rng = np.random.default_rng(0)
+    n = 3000
+    cases = []
+    cases.append(np.tile(np.array([[0.3, 0.4, 0.5]], np.float32), (n, 1)))                      # all equal
+    two = np.tile(np.array([[0.3, 0.4, 0.5]], np.float32), (n, 1)); two[::3] = [0.7, 0.1, 0.9]
+    cases.append(two)                                                                            # two keys
+    srt = np.sort(rng.random(n).astype(np.float32))
+    cases.append(np.stack([srt, srt, srt], 1))                                                   # sorted
+    cases.append(np.stack([srt[::-1], srt[::-1], srt[::-1]], 1).copy())                          # reversed
+    edge = rng.random((n, 3), dtype=np.float32); edge[:50] = 0.0
+    edge[50:100] = np.nextafter(np.float32(1), np.float32(0))
+    cases.append(edge)                                                                           # box corners
+    cases.append((rng.random((n, 3), dtype=np.float32) * 2.0 - 0.5))                             # periodic wrap
+    for i, pos in enumerate(cases):
+        periodic = i == 5
+        mass = np.full(n, 1.0 / n, np.float32)
+        d = dsk.Dsk(n, 1.0, periodic, 1e-3, 0.5, 2)
+        d.build_tree(_dev(pos), _dev(mass))
+        _check_structure(orc, d, pos, mass, 1.0, periodic)
+        d.close()
+
+
+@pytest.mark.parametrize("n", [1, 2, 17, 64, 65])
+def test_tiny_inputs(dsk, orc, n):
+    rng = np.random.default_rng(n)
+    pos = rng.random((n, 3), dtype=np.float32); mass = rng.uniform(0.5, 1.5, n).astype(np.float32)
+    d = dsk.Dsk(n, 1.0, False, 0.05, 0.5, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    _check_structure(orc, d, pos, mass, 1.0, False)
+    acc, pot = d.accel(tp, tm)
+    ra, rp = orc.direct_iso(pos, mass, 0.05)
+    if n > 1:
+        assert np.max(np.abs(acc.cpu().numpy() - ra)) < 1e-5 * np.abs(ra).max()
+        assert np.max(np.abs(pot.cpu().numpy() - rp)) < 1e-5 * np.abs(rp).max()
+    else:
+        assert np.all(acc.cpu().numpy() == 0) and abs(float(pot[0])) < 1e-6
+    d.close()
+
+
+def test_errors(dsk):
+    n = 100
+    pos = np.random.default_rng(0).random((n, 3), dtype=np.float32); mass = np.ones(n, np.float32)
+    d = dsk.Dsk(n, 1.0, False, 1e-3, 0.5, 4)
+    with pytest.raises(dsk.DskError) as e:
+        d.accel(_dev(pos), _dev(mass))
+    assert e.value.code == -3                                   # no tree
+    bad = pos.copy(); bad[7, 1] = 1.0
+    with pytest.raises(dsk.DskError) as e:
+        d.build_tree(_dev(bad), _dev(mass))
+    assert e.value.code == -4
+    bad[7, 1] = np.nan
+    with pytest.raises(dsk.DskError) as e:
+        d.build_tree(_dev(bad), _dev(mass))
+    assert e.value.code == -5
+    d.build_tree(_dev(pos), _dev(mass))                         # the context recovers
+    d.accel(_dev(pos), _dev(mass))
+    d.close()
+
+
+# ---- moments ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("p", [2, 4, 6, 8])
+def test_moments(dsk, orc, p):
+    pos, mass = workloads.make(2, 1 / 64)
+    mass = (mass * np.random.default_rng(1).uniform(0.5, 1.5, len(mass))).astype(np.float32)
+    d = dsk.Dsk(len(pos), 1.0, False, 1e-4, 0.5, p)
+    d.build_tree(_dev(pos), _dev(mass))
+    t = orc.OracleTree(pos, mass)
+    cm, com, dl, mom = t.moments(p)
+    gcm, gmom = d.get_moments()
+    gcm = gcm.cpu().numpy().astype(np.float64); gmom = gmom.cpu().numpy().astype(np.float64)
+    side = 2.0 ** (-t.cells()["level"].astype(np.float64))
+    assert np.max(np.abs(gcm[:, 3] - cm) / cm) < 1e-6
+    assert np.max(np.abs(gcm[:, :3] - com)) < 1.2e-7          # the getter rounds ctr + off to fp32 (ulp(1) = 1.2e-7)
+    rank = np.array([sum(n) for n in orc.mtable(p)])
+    scale = cm[:, None] * side[:, None] ** rank[None, :]                    # natural size of M_n
+    assert np.max(np.abs(gmom - mom) / scale) < 2e-6
+    d.close()
+
+
+# ---- forces, isolated ---------------------------------------------------------------------------------
+def test_forces_C1_full(dsk, orc):
+    """BASELINE.json configs[0] at full size, every particle a sink."""
+    cfg = workloads.CONFIGS[1]
+    pos, mass = workloads.make(1)
+    d = dsk.Dsk(len(pos), 1.0, False, cfg["eps"], cfg["theta"], cfg["p"])
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    acc, pot = d.accel(tp, tm)
+    acc = acc.cpu().numpy().astype(np.float64); pot = pot.cpu().numpy().astype(np.float64)
+    ta, tpot, n_p2p, n_m2p, tree = orc.tree_force(pos, mass, 1.0, False, cfg["eps"], cfg["theta"], cfg["p"])
+    da, dp = orc.direct_iso(pos, mass, cfg["eps"])
+    _force_gates(acc, ta, da)
+    assert np.max(np.abs(pot - tpot)) < 1e-5 * np.abs(tpot).max()
+    st = d.get_stats()
+    # useful interaction counts agree with the oracle's (MAC ties may flip a handful of cells)
+    assert abs(st["n_m2p"] - n_m2p) <= 1e-4 * n_m2p
+    assert abs(st["n_p2p"] - (n_p2p + len(pos))) <= 1e-4 * n_p2p          # GPU count includes the self pair
+    d.close()
+
+
+def test_forces_C2_sweep_scaled(dsk, orc):
+    """configs[1] recipe at N = 2^16: the full theta x p sweep with one tree (moments per p, lists per theta)."""
+    pos, mass = workloads.make(2, 1 / 16)
+    n = len(pos)
+    sink = workloads.subsample(2, n, 1024)
+    da, _ = orc.direct_iso(pos, mass, 1e-4, sink)
+    d = dsk.Dsk(n, 1.0, False, 1e-4, 0.5, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    tree = orc.OracleTree(pos, mass)
+    errs = {}
+    for p in (2, 4, 6, 8):
+        for theta in (0.3, 0.5, 0.7, 1.0):
+            d.set_params(theta=theta, p=p)
+            acc, _ = d.accel(tp, tm, want_pot=False)
+            acc = acc.cpu().numpy().astype(np.float64)[sink]
+            ta = tree.accel(1e-4, theta, p, sink)[0]
+            errs[(theta, p)] = _force_gates(acc, ta, da)
+    # the sweep behaves like the method should: error falls with p and rises with theta
+    for theta in (0.3, 0.5, 0.7, 1.0):
+        e = [errs[(theta, p)][0] for p in (2, 4, 6, 8)]
+        assert e[0] > e[1] > e[2], e
+    d.close()
+
+
+def test_forces_C2_full_sampled(dsk, orc):
+    """configs[1] at full size (N = 2^20, theta 0.5, p 4 — the bench workload) on a 4096-sink subsample."""
+    cfg = workloads.CONFIGS[2]
+    pos, mass = workloads.make(2)
+    n = len(pos)
+    sink = workloads.subsample(2, n, 4096)
+    d = dsk.Dsk(n, 1.0, False, cfg["eps"], cfg["theta"], cfg["p"])
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    tree = _check_structure(orc, d, pos, mass, 1.0, False)
+    acc, pot = d.accel(tp, tm)
+    acc = acc.cpu().numpy().astype(np.float64)[sink]
+    ta, tpot, _, _ = tree.accel(cfg["eps"], cfg["theta"], cfg["p"], sink)
+    da, _ = orc.direct_iso(pos, mass, cfg["eps"], sink)
+    _force_gates(acc, ta, da)
+    assert np.max(np.abs(pot.cpu().numpy()[sink] - tpot)) < 1e-5 * np.abs(tpot).max()
+    # properties that hold at any size: momentum conservation of the tree force to the tree error
+    a_all = d.accel(tp, tm, want_pot=False)[0].cpu().numpy().astype(np.float64)
+    f = a_all * mass[:, None].astype(np.float64)
+    assert np.linalg.norm(f.sum(0)) < 1e-3 * np.abs(f).sum() / math.sqrt(n) * 30
+    d.close()
+
+
+# ---- forces, periodic ---------------------------------------------------------------------------------
+def test_forces_periodic_lattice_scaled(dsk, orc):
+    """configs[2] recipe at 32^3: Ewald direct sum on 192 sinks, oracle tree on 4096."""
+    ng = 32
+    pos, mass = workloads.perturbed_lattice(ng)
+    n, eps = len(pos), 1.0 / (40 * ng)
+    d = dsk.Dsk(n, 1.0, True, eps, 0.5, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    tree = _check_structure(orc, d, pos, mass, 1.0, True)
+    acc, pot = d.accel(tp, tm)
+    acc = acc.cpu().numpy().astype(np.float64); pot = pot.cpu().numpy().astype(np.float64)
+    sink = workloads.subsample(3, n, 4096)
+    ta, tpot, _, _, _ = orc.tree_force(pos, mass, 1.0, True, eps, 0.5, 4, sink, tree=tree)
+    rel = np.linalg.norm(acc[sink] - ta, axis=1) / np.linalg.norm(ta, axis=1)
+    assert np.quantile(rel, 0.999) < 1e-4, np.quantile(rel, 0.999)
+    assert np.max(np.abs(pot[sink] - tpot)) < 2e-5 * np.abs(tpot).max() + 1e-5
+    s2 = sink[:192]
+    da, _ = orc.direct_per(pos, mass, 1.0, eps, s2)
+    e_gpu, e_tree = _erms(acc[s2], da), _erms(ta[:192], da)
+    assert e_gpu <= 1.1 * e_tree + 1e-6, (e_gpu, e_tree)
+    d.close()
+
+
+def test_forces_periodic_clustered_scaled(dsk, orc):
+    """configs[3] recipe at 32^3 with p = 6."""
+    pos, mass = workloads.clustered_box(32, 40, cfg=4)
+    n, eps = len(pos), 1.0 / (40 * 32)
+    d = dsk.Dsk(n, 1.0, True, eps, 0.5, 6)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    acc, _ = d.accel(tp, tm, want_pot=False)
+    acc = acc.cpu().numpy().astype(np.float64)
+    sink = workloads.subsample(4, n, 2048)
+    ta = orc.tree_force(pos, mass, 1.0, True, eps, 0.5, 6, sink)[0]
+    s2 = sink[:128]
+    da, _ = orc.direct_per(pos, mass, 1.0, eps, s2)
+    rel = np.linalg.norm(acc[sink] - ta, axis=1) / np.linalg.norm(ta, axis=1)
+    assert np.quantile(rel, 0.999) < 1e-4, np.quantile(rel, 0.999)
+    e_gpu, e_tree = _erms(acc[s2], da), _erms(ta[:128], da)
+    assert e_gpu <= 1.1 * e_tree + 1e-6, (e_gpu, e_tree)
+    d.close()
+
+
+def test_perfect_lattice_force_free(dsk):
+    pos, mass = workloads.perfect_lattice(16)
+    d = dsk.Dsk(len(pos), 1.0, True, 1.0 / 640, 0.5, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    acc, _ = d.accel(tp, tm, want_pot=False)
+    nn = (1.0 / 16 ** 3) / (1.0 / 16) ** 2                     # nearest-neighbour pair force
+    assert float(acc.abs().max()) < 2e-3 * nn
+    d.close()
+
+
+# ---- KDK ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("periodic", [False, True])
+def test_kdk_step(dsk, orc, periodic):
+    rng = np.random.default_rng(9)
+    if periodic:
+        pos, mass = workloads.perturbed_lattice(12)
+        eps, a, da = 1.0 / 480, 0.5, 0.01
+    else:
+        pos, mass = workloads.uniform_box(2000)
+        pos = (0.25 + 0.5 * pos).astype(np.float32)
+        eps, a, da = 1e-2, 0.0, 0.01
+    n = len(pos)
+    vel = (0.02 * rng.standard_normal((n, 3))).astype(np.float32)
+    d = dsk.Dsk(n, 1.0, periodic, eps, 0.5, 4)
+    tp, tv, tm = _dev(pos), _dev(vel), _dev(mass)
+    d.kdk_step(tp, tv, tm, a, da)
+    p1, v1, a1 = orc.kdk_step(pos, vel, mass, 1.0, periodic, eps, 0.5, 4, a, da)
+    gp, gv = tp.cpu().numpy(), tv.cpu().numpy()
+    dx = np.abs(gp.astype(np.float64) - p1)
+    if periodic:
+        dx = np.minimum(dx, 1.0 - dx)
+    assert dx.max() < 3e-7
+    assert np.max(np.abs(gv - v1)) < 2e-5 * np.abs(v1).max() + 1e-7
+    # second step reuses the cached force
+    d.kdk_step(tp, tv, tm, a + da, da)
+    p2, v2, _ = orc.kdk_step(p1, v1, mass, 1.0, periodic, eps, 0.5, 4, a + da, da, acc=a1)
+    dx = np.abs(tp.cpu().numpy().astype(np.float64) - p2)
+    if periodic:
+        dx = np.minimum(dx, 1.0 - dx)
+    assert dx.max() < 1e-6
+    assert np.max(np.abs(tv.cpu().numpy() - v2)) < 5e-5 * np.abs(v2).max() + 1e-7
+    d.close()
