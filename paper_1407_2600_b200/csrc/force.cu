@@ -3,9 +3,10 @@
 // set of n sink particles ... perform the full m x n interactions on this block"; PAPER.md:75 direct
 // interactions near the leaves, quadrupole/hexadecapole cell interactions for the rest).
 //
-// One CTA of 64 threads per sink group (<= NCRIT = 64 sinks, one per thread).  Source tiles are staged
-// through shared memory in PAIR-INTERLEAVED form {A,B}, read back with broadcast LDS.64/128 and consumed
-// with packed f32x2 arithmetic: every thread handles 1 sink x 2 sources per instruction (FFMA2 is the
+// One warp per (group, 32-sink half) task, one sink per lane (sub-warp tiling for small tasks, below).
+// Source tiles are staged through per-warp shared memory in PAIR-INTERLEAVED form {A,B}, read back with
+// broadcast LDS.64/128 and consumed with packed f32x2 arithmetic: every thread handles 1 sink x 2 sources
+// per instruction (FFMA2 is the
 // only way to reach the FP32 peak with three distinct operands on sm_100, see dsk_internal.cuh).
 // All coordinates are taken relative to the group's cell centre c_g (exact subtraction for nearby
 // values), which keeps fp32 differences accurate and absorbs the periodic image shift.
@@ -18,9 +19,7 @@
 #include "dsk_internal.cuh"
 #include <type_traits>
 
-#define FT 64                // threads per CTA = NCRIT
-#define P2P_TILE 256         // sources per shared tile
-#define M2P_TC 32            // cells per shared tile
+#define P2P_TILE 128         // sources per warp tile
 
 int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base);   // walk.cu
 
@@ -134,41 +133,98 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float2 *__restr
     ax = vfma(gx, sinv2, ax); ay = vfma(gy, sinv2, ay); az = vfma(gz, sinv2, az);
 }
 
+// ---- work decomposition shared by F1 and F2 -----------------------------------------------------------
+// One WARP per task; task = (group, half): sinks [32 half, 32 half + 32) of the group, so a group of <= 32
+// sinks is one warp and nothing waits at a block barrier (ncu on the first version, one 64-thread CTA per
+// group: 6 barrier-stall cycles per issue, FMA pipe 45 % active, ~18 of 64 lanes useful on the Plummer
+// workload).  Groups are cells, so many hold few sinks: a task with ns <= 16 (<= 8) sinks splits the warp
+// into 2 (4) sub-groups that take alternate source pairs of a tile and are summed at the end.
+struct warp_task {
+    uint32_t g, first, ns;       // group, rank of the task's first sink, sinks in the task
+    int W, S, sub, j;            // sub-group width, number of sub-groups, my sub-group, my sink in the task
+    bool valid;
+};
+__device__ __forceinline__ warp_task make_task(uint32_t g0, uint32_t g1, int fw, const uint32_t *__restrict__ gfirst,
+                                               const uint32_t *__restrict__ gcount)
+{
+    warp_task t;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t task = blockIdx.x * fw + warp;
+    t.g = g0 + (task >> 1);
+    t.valid = false;
+    t.first = 0; t.ns = 0; t.W = 32; t.S = 1; t.sub = 0; t.j = 0;
+    if (t.g >= g1) return t;
+    const uint32_t count = gcount[t.g], h = task & 1u;
+    if (32u * h >= count) return t;
+    t.valid = true;
+    t.ns = min(32u, count - 32u * h);
+    t.first = gfirst[t.g] + 32u * h;
+    t.W = t.ns <= 8 ? 8 : (t.ns <= 16 ? 16 : 32);
+    t.S = 32 / t.W;
+    t.sub = lane / t.W;
+    t.j = min(lane % t.W, (int)t.ns - 1);
+    return t;
+}
+// sum the sub-groups' two-float accumulators (in double) and store; lanes of sub-group 0 own the sinks
+__device__ __forceinline__ void task_store(const warp_task &t, float4 hi, float4 lo, float4 *__restrict__ sacc,
+                                           float4 *__restrict__ sacc_lo)
+{
+    double d[4] = {(double)hi.x + (double)lo.x, (double)hi.y + (double)lo.y, (double)hi.z + (double)lo.z,
+                   (double)hi.w + (double)lo.w};
+    for (int o = 16; o >= t.W; o >>= 1)
+#pragma unroll
+        for (int q = 0; q < 4; q++) d[q] += __shfl_xor_sync(0xffffffffu, d[q], o);
+    const int lane = threadIdx.x & 31;
+    if (lane < (int)t.ns) {
+        float4 oh, ol;
+        oh.x = (float)d[0]; oh.y = (float)d[1]; oh.z = (float)d[2]; oh.w = (float)d[3];
+        ol.x = (float)(d[0] - (double)oh.x); ol.y = (float)(d[1] - (double)oh.y); ol.z = (float)(d[2] - (double)oh.z);
+        ol.w = (float)(d[3] - (double)oh.w);
+        sacc[t.first + lane] = oh; sacc_lo[t.first + lane] = ol;
+    }
+}
+
+#define FW 4                 // warps (tasks) per block
+
 template <int P, bool POT, bool PACKED>
-__global__ void __launch_bounds__(FT) k_m2p(uint32_t g0, int periodic, float box, float eps2,
-                                            const float *__restrict__ rows, const float4 *__restrict__ spos,
-                                            const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
-                                            const uint32_t *__restrict__ gcell, const uint32_t *__restrict__ list,
-                                            const uint64_t *__restrict__ off, uint64_t base,
-                                            const uint32_t *__restrict__ len, float4 *__restrict__ sacc,
-                                            float4 *__restrict__ sacc_lo)
+__global__ void __launch_bounds__(FW * 32) k_m2p(uint32_t g0, uint32_t g1, int periodic, float box, float eps2,
+                                                 const float *__restrict__ rows, const float4 *__restrict__ spos,
+                                                 const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
+                                                 const uint32_t *__restrict__ gcell, const uint32_t *__restrict__ list,
+                                                 const uint64_t *__restrict__ off, uint64_t base,
+                                                 const uint32_t *__restrict__ len, float4 *__restrict__ sacc,
+                                                 float4 *__restrict__ sacc_lo)
 {
     constexpr int NP = dsk_np(P), ROW = dsk_rowlen(P), TROW = M2P_HDR + NP;
-    __shared__ uint32_t s_cell[M2P_TC];
-    __shared__ __align__(16) float2 tile[M2P_TC / 2][TROW];
-    const uint32_t g = g0 + blockIdx.x;
-    const int t = threadIdx.x;
-    const uint32_t first = gfirst[g], count = gcount[g];
-    const float *grow = rows + (size_t)gcell[g] * ROW;
+    constexpr int TC = (P <= 6) ? 32 : 16;                  // cells per tile (one per lane at most)
+    __shared__ uint32_t s_cell_all[FW][TC];
+    __shared__ __align__(16) float2 tile_all[FW][TC / 2][TROW];
+    const warp_task t = make_task(g0, g1, FW, gfirst, gcount);
+    if (!t.valid) return;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint32_t *s_cell = s_cell_all[warp];
+    float2(*tile)[TROW] = tile_all[warp];
+    const float *grow = rows + (size_t)gcell[t.g] * ROW;
     const float cgx = grow[0], cgy = grow[1], cgz = grow[2];
-    float4 me = spos[first + (t < (int)count ? t : 0)];
-    const float xs = me.x - cgx, ys = me.y - cgy, zs = me.z - cgz;
-    const bool warp_active = (uint32_t)(t & ~31) < count;
-    const uint32_t n = len[g];
-    const uint32_t *lst = list + (off[g] - base);
+    const float4 me = spos[t.first + t.j];
+    const uint32_t n = len[t.g];
+    const uint32_t *lst = list + (off[t.g] - base);
     using T = typename std::conditional<PACKED, f2, float>::type;
-    // running sums as two-float (hi, lo) pairs, continued from the P2P kernel; each tile is summed from
-    // zero in plain fp32 and folded in with TwoSum, so no addition ever rounds at the size of the total
+    // running sums as two-float (hi, lo) pairs, continued from the P2P kernel (sub-group 0 carries them);
+    // each tile is summed from zero in plain fp32 and folded in with TwoSum, so no addition ever rounds at
+    // the size of the total
     float4 hi = make_float4(0.f, 0.f, 0.f, 0.f), lo = hi;
-    if (t < (int)count) { hi = sacc[first + t]; lo = sacc_lo[first + t]; }
-    const T X = vdup<T>(xs), Y = vdup<T>(ys), Z = vdup<T>(zs);
-    for (uint32_t b0 = 0; b0 < n; b0 += M2P_TC) {
-        const int ntc = (int)min((uint32_t)M2P_TC, n - b0);
-        if (t < M2P_TC) {
-            float cx = 1.0e5f, cy = 1.0e5f, cz = 1.0e5f, sinv = 1.0f;
+    if (t.sub == 0 && lane < (int)t.ns) { hi = sacc[t.first + lane]; lo = sacc_lo[t.first + lane]; }
+    const T X = vdup<T>(me.x - cgx), Y = vdup<T>(me.y - cgy), Z = vdup<T>(me.z - cgz);
+    const int quantum = PACKED ? 2 * t.S : t.S;             // cells consumed per round of the sub-groups
+    for (uint32_t b0 = 0; b0 < n; b0 += TC) {
+        const int ntc = (int)min((uint32_t)TC, n - b0);
+        const int npad = (ntc + quantum - 1) / quantum * quantum;
+        if (lane < npad) {
+            float cx = 1.0e5f, cy = 1.0e5f, cz = 1.0e5f, sinv = 1.0f;       // dummy cell: far away, no mass
             uint32_t cidx = 0xffffffffu;
-            if (t < ntc) {
-                const uint32_t e = lst[b0 + t];
+            if (lane < ntc) {
+                const uint32_t e = lst[b0 + lane];
                 cidx = e & ((1u << DSK_CELL_BITS) - 1u);
                 const float *r = rows + (size_t)cidx * ROW;
                 const float4 h0 = *reinterpret_cast<const float4 *>(r);
@@ -183,68 +239,71 @@ __global__ void __launch_bounds__(FT) k_m2p(uint32_t g0, int periodic, float box
                 cx = ((h0.x - cgx) + shx) + h1.x; cy = ((h0.y - cgy) + shy) + h1.y; cz = ((h0.z - cgz) + shz) + h1.z;
                 sinv = h0.w;
             }
-            s_cell[t] = cidx;
-            float *hd = reinterpret_cast<float *>(&tile[t >> 1][0]) + (t & 1);
+            s_cell[lane] = cidx;
+            float *hd = reinterpret_cast<float *>(&tile[lane >> 1][0]) + (lane & 1);
             hd[0] = cx; hd[2] = cy; hd[4] = cz; hd[6] = sinv; hd[8] = eps2 * sinv * sinv;
         }
-        __syncthreads();
-        for (int idx = t; idx < M2P_TC * NP; idx += FT) {
+        __syncwarp();
+        for (int idx = lane; idx < npad * NP; idx += 32) {
             const int ci = idx / NP, k = idx - ci * NP;
             const uint32_t cidx = s_cell[ci];
             const float v = cidx != 0xffffffffu ? rows[(size_t)cidx * ROW + 8 + k] : 0.0f;
             reinterpret_cast<float *>(&tile[ci >> 1][M2P_HDR + k])[ci & 1] = v;
         }
-        __syncthreads();
-        if (warp_active) {
+        __syncwarp();
+        {
             T pot = vdup<T>(0.0f), ax = vdup<T>(0.0f), ay = vdup<T>(0.0f), az = vdup<T>(0.0f);
             if constexpr (PACKED) {
-                const int npair = (ntc + 1) >> 1;
-                for (int k = 0; k < npair; k++) m2p_body<P, T, POT>(X, Y, Z, tile[k], 0, pot, ax, ay, az);
+                const int npair = npad >> 1;
+                for (int k = t.sub; k < npair; k += t.S) m2p_body<P, T, POT>(X, Y, Z, tile[k], 0, pot, ax, ay, az);
             } else {
-                for (int k = 0; k < ntc; k++) m2p_body<P, T, POT>(X, Y, Z, tile[k >> 1], k & 1, pot, ax, ay, az);
+                for (int k = t.sub; k < npad; k += t.S) m2p_body<P, T, POT>(X, Y, Z, tile[k >> 1], k & 1, pot, ax, ay, az);
             }
             dsk_fold(hi.x, lo.x, vsum(ax)); dsk_fold(hi.y, lo.y, vsum(ay)); dsk_fold(hi.z, lo.z, vsum(az));
             if (POT) dsk_fold(hi.w, lo.w, -vsum(pot));
         }
-        __syncthreads();
+        __syncwarp();
     }
-    if (t < (int)count) { sacc[first + t] = hi; sacc_lo[first + t] = lo; }
+    task_store(t, hi, lo, sacc, sacc_lo);
 }
 
 // ---- F1 ----------------------------------------------------------------------------------------------
 template <bool POT>
-__global__ void __launch_bounds__(FT) k_p2p(uint32_t g0, int periodic, float box, float eps2, int rowlen,
-                                            const float *__restrict__ rows, const dsk_cellrec *__restrict__ cell,
-                                            const float4 *__restrict__ spos, const uint32_t *__restrict__ gfirst,
-                                            const uint32_t *__restrict__ gcount, const uint32_t *__restrict__ gcell,
-                                            const uint32_t *__restrict__ list, const uint64_t *__restrict__ off,
-                                            uint64_t base, const uint32_t *__restrict__ len,
-                                            float4 *__restrict__ sacc, float4 *__restrict__ sacc_lo)
+__global__ void __launch_bounds__(FW * 32) k_p2p(uint32_t g0, uint32_t g1, int periodic, float box, float eps2,
+                                                 int rowlen, const float *__restrict__ rows,
+                                                 const dsk_cellrec *__restrict__ cell, const float4 *__restrict__ spos,
+                                                 const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
+                                                 const uint32_t *__restrict__ gcell, const uint32_t *__restrict__ list,
+                                                 const uint64_t *__restrict__ off, uint64_t base,
+                                                 const uint32_t *__restrict__ len, float4 *__restrict__ sacc,
+                                                 float4 *__restrict__ sacc_lo)
 {
-    __shared__ uint32_t s_first[FT];
-    __shared__ uint32_t s_pref[FT + 1];
-    __shared__ float s_sh[FT][3];
-    __shared__ uint32_t s_wsum[2];
-    __shared__ __align__(16) float4 tA[P2P_TILE / 2], tB[P2P_TILE / 2];   // {xA,xB,yA,yB}, {zA,zB,mA,mB}
-    const uint32_t g = g0 + blockIdx.x;
-    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-    const uint32_t first = gfirst[g], count = gcount[g];
-    const float *grow = rows + (size_t)gcell[g] * rowlen;
+    __shared__ uint32_t s_first_all[FW][32];
+    __shared__ uint32_t s_pref_all[FW][33];
+    __shared__ float s_sh_all[FW][32][3];
+    __shared__ __align__(16) float4 tA_all[FW][P2P_TILE / 2], tB_all[FW][P2P_TILE / 2];   // {xA,xB,yA,yB}, {zA,zB,mA,mB}
+    const warp_task t = make_task(g0, g1, FW, gfirst, gcount);
+    if (!t.valid) return;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint32_t *s_first = s_first_all[warp], *s_pref = s_pref_all[warp];
+    float(*s_sh)[3] = s_sh_all[warp];
+    float4 *tA = tA_all[warp], *tB = tB_all[warp];
+    const float *grow = rows + (size_t)gcell[t.g] * rowlen;
     const float cgx = grow[0], cgy = grow[1], cgz = grow[2];
-    const float4 me = spos[first + (t < (int)count ? t : 0)];
+    const float4 me = spos[t.first + t.j];
     const f2 X = f2_dup(me.x - cgx), Y = f2_dup(me.y - cgy), Z = f2_dup(me.z - cgz);
     const f2 E2 = f2_dup(eps2);
-    const bool warp_active = (uint32_t)(t & ~31) < count;
-    const uint32_t n = len[g];
-    const uint32_t *lst = list + (off[g] - base);
+    const uint32_t n = len[t.g];
+    const uint32_t *lst = list + (off[t.g] - base);
     float4 hi = make_float4(0.f, 0.f, 0.f, 0.f), lo = hi;     // two-float running sums (see k_m2p)
-    for (uint32_t b0 = 0; b0 < n; b0 += FT) {
-        // one leaf (segment of sources) per thread; exclusive scan of the segment lengths
+    const uint32_t quantum = 2u * (uint32_t)t.S;
+    for (uint32_t b0 = 0; b0 < n; b0 += 32) {
+        // one leaf (segment of sources) per lane; exclusive scan of the segment lengths
         uint32_t cnt = 0;
-        if (b0 + t < n) {
-            const uint32_t e = lst[b0 + t];
+        if (b0 + lane < n) {
+            const uint32_t e = lst[b0 + lane];
             const dsk_cellrec r = cell[e & ((1u << DSK_CELL_BITS) - 1u)];
-            s_first[t] = r.first; cnt = r.count;
+            s_first[lane] = r.first; cnt = r.count;
             float shx = 0.0f, shy = 0.0f, shz = 0.0f;
             if (periodic) {
                 const int img = (int)(e >> DSK_CELL_BITS), side = 2 * DSK_WS + 1;
@@ -252,45 +311,43 @@ __global__ void __launch_bounds__(FT) k_p2p(uint32_t g0, int periodic, float box
                 shy = (float)((img / side) % side - DSK_WS) * box;
                 shx = (float)(img / (side * side) - DSK_WS) * box;
             }
-            s_sh[t][0] = shx; s_sh[t][1] = shy; s_sh[t][2] = shz;
+            s_sh[lane][0] = shx; s_sh[lane][1] = shy; s_sh[lane][2] = shz;
         }
         uint32_t x = cnt;
         for (int o = 1; o < 32; o <<= 1) {
             uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
             if (lane >= o) x += y;
         }
-        if (lane == 31) s_wsum[warp] = x;
-        __syncthreads();
-        const uint32_t wpre = warp ? s_wsum[0] : 0u, total = s_wsum[0] + s_wsum[1];
-        s_pref[t] = wpre + x - cnt;
-        if (t == 0) s_pref[FT] = total;
-        __syncthreads();
+        const uint32_t total = __shfl_sync(0xffffffffu, x, 31);
+        s_pref[lane] = x - cnt;
+        if (lane == 0) s_pref[32] = total;
+        __syncwarp();
         for (uint32_t t0 = 0; t0 < total; t0 += P2P_TILE) {
             const uint32_t nt = min((uint32_t)P2P_TILE, total - t0);
-            const uint32_t npad = (nt + 1u) & ~1u;
-            for (uint32_t j = t; j < npad; j += FT) {
-                float sx = 1.0e10f, sy = 1.0e10f, sz = 1.0e10f, sm = 0.0f;
+            const uint32_t npad = (nt + quantum - 1) / quantum * quantum;
+            for (uint32_t j = lane; j < npad; j += 32) {
+                float sx = 1.0e10f, sy = 1.0e10f, sz = 1.0e10f, sm = 0.0f;      // pad: far away, massless
                 if (j < nt) {
                     const uint32_t gj = t0 + j;
-                    int lo = 0, hi = FT;                      // last segment with pref <= gj
-                    while (hi - lo > 1) {
-                        const int mid = (lo + hi) >> 1;
-                        if (s_pref[mid] <= gj) lo = mid; else hi = mid;
+                    int a = 0, b = 32;                        // last segment with pref <= gj
+                    while (b - a > 1) {
+                        const int mid = (a + b) >> 1;
+                        if (s_pref[mid] <= gj) a = mid; else b = mid;
                     }
-                    const float4 p = spos[s_first[lo] + (gj - s_pref[lo])];
-                    sx = (p.x - cgx) + s_sh[lo][0]; sy = (p.y - cgy) + s_sh[lo][1]; sz = (p.z - cgz) + s_sh[lo][2];
+                    const float4 p = spos[s_first[a] + (gj - s_pref[a])];
+                    sx = (p.x - cgx) + s_sh[a][0]; sy = (p.y - cgy) + s_sh[a][1]; sz = (p.z - cgz) + s_sh[a][2];
                     sm = p.w;
                 }
-                float *a = reinterpret_cast<float *>(&tA[j >> 1]) + (j & 1);
-                float *b = reinterpret_cast<float *>(&tB[j >> 1]) + (j & 1);
-                a[0] = sx; a[2] = sy; b[0] = sz; b[2] = sm;
+                float *pa = reinterpret_cast<float *>(&tA[j >> 1]) + (j & 1);
+                float *pb = reinterpret_cast<float *>(&tB[j >> 1]) + (j & 1);
+                pa[0] = sx; pa[2] = sy; pb[0] = sz; pb[2] = sm;
             }
-            __syncthreads();
-            if (warp_active) {
+            __syncwarp();
+            {
                 f2 ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f), pot = f2_dup(0.0f);
                 const int npair = (int)(npad >> 1);
 #pragma unroll 4
-                for (int k = 0; k < npair; k++) {
+                for (int k = t.sub; k < npair; k += t.S) {
                     const ulonglong2 qa = *reinterpret_cast<const ulonglong2 *>(&tA[k]);
                     const ulonglong2 qb = *reinterpret_cast<const ulonglong2 *>(&tB[k]);
                     f2 sx, sy, sz, sm;
@@ -307,14 +364,12 @@ __global__ void __launch_bounds__(FT) k_p2p(uint32_t g0, int periodic, float box
                 dsk_fold(hi.x, lo.x, vsum(ax)); dsk_fold(hi.y, lo.y, vsum(ay)); dsk_fold(hi.z, lo.z, vsum(az));
                 if (POT) dsk_fold(hi.w, lo.w, vsum(pot));
             }
-            __syncthreads();
+            __syncwarp();
         }
     }
-    if (t < (int)count) {
-        // the sink's own leaf is always in the list: remove its self term -m_i/eps from the potential
-        if (POT) dsk_fold(hi.w, lo.w, me.w * rsqrtf(eps2));
-        sacc[first + t] = hi; sacc_lo[first + t] = lo;
-    }
+    // the sink's own leaf is always in the list: remove its self term -m_i/eps from the potential (once)
+    if (POT && t.sub == 0) dsk_fold(hi.w, lo.w, me.w * rsqrtf(eps2));
+    task_store(t, hi, lo, sacc, sacc_lo);
 }
 
 template <int P>
@@ -323,11 +378,11 @@ static void launch_m2p(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t base, int 
     const float e2 = c->eps * c->eps;
     constexpr bool PACKED = (P <= 6);
     if (want_pot)
-        k_m2p<P, true, PACKED><<<g1 - g0, FT, 0, c->stream>>>(g0, c->periodic, c->box, e2, c->rows, c->spos, c->gfirst,
+        k_m2p<P, true, PACKED><<<(2 * (g1 - g0) + FW - 1) / FW, FW * 32, 0, c->stream>>>(g0, g1, c->periodic, c->box, e2, c->rows, c->spos, c->gfirst,
                                                               c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
                                                               c->g_m2p_len, c->sacc, c->sacc_lo);
     else
-        k_m2p<P, false, PACKED><<<g1 - g0, FT, 0, c->stream>>>(g0, c->periodic, c->box, e2, c->rows, c->spos, c->gfirst,
+        k_m2p<P, false, PACKED><<<(2 * (g1 - g0) + FW - 1) / FW, FW * 32, 0, c->stream>>>(g0, g1, c->periodic, c->box, e2, c->rows, c->spos, c->gfirst,
                                                                c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
                                                                c->g_m2p_len, c->sacc, c->sacc_lo);
 }
@@ -343,10 +398,10 @@ static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t mb, uint64_
     const float e2 = c->eps * c->eps;
     const int rowlen = dsk_rowlen(c->p);
     if (want_pot)
-        k_p2p<true><<<g1 - g0, FT, 0, s>>>(g0, c->periodic, c->box, e2, rowlen, c->rows, c->cell, c->spos, c->gfirst,
+        k_p2p<true><<<(2 * (g1 - g0) + FW - 1) / FW, FW * 32, 0, s>>>(g0, g1, c->periodic, c->box, e2, rowlen, c->rows, c->cell, c->spos, c->gfirst,
                                            c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     else
-        k_p2p<false><<<g1 - g0, FT, 0, s>>>(g0, c->periodic, c->box, e2, rowlen, c->rows, c->cell, c->spos, c->gfirst,
+        k_p2p<false><<<(2 * (g1 - g0) + FW - 1) / FW, FW * 32, 0, s>>>(g0, g1, c->periodic, c->box, e2, rowlen, c->rows, c->cell, c->spos, c->gfirst,
                                             c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     cudaEventRecord(c->ev[9], s);
     switch (c->p) {
