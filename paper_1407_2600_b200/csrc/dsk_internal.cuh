@@ -35,6 +35,7 @@ struct dsk_devstate {         // small device block read back at the end of API 
     uint32_t status;          // bit flags: 1 out-of-box, 2 non-finite, 4 cell overflow, 8 stack overflow,
                               //            16 list overflow
     uint32_t ncell, ngroup, nlevel;
+    uint32_t ntask;           // warp tasks = sum over groups of ceil(count / 32)
     uint32_t lvl_start[DSK_KEY_LEVELS + 3];
     uint32_t nleaf_cells;
     unsigned long long tot_m2p_list, tot_p2p_list, tot_p2p_src;   // over all groups
@@ -73,6 +74,8 @@ struct dsk_ctx {
     uint32_t *gfirst, *gcount, *gcell;     // [ngroup_cap]
     float4 *gbox;             // [2 * ngroup_cap]: min.xyz,_ ; max.xyz,_
     uint32_t *g_m2p_len, *g_p2p_len, *g_p2p_src;   // [ngroup_cap]
+    uint32_t *g_taskoff;      // [ngroup_cap + 1] exclusive scan of ceil(count/32)
+    uint32_t *g_task;         // [2 * ngroup_cap] task -> group << 1 | half
     uint64_t *g_m2p_off, *g_p2p_off;               // [ngroup_cap + 1] exclusive offsets into lists
     uint32_t *list_m2p, *list_p2p;
     size_t list_m2p_cap, list_p2p_cap;             // entries

@@ -144,18 +144,18 @@ struct warp_task {
     int W, S, sub, j;            // sub-group width, number of sub-groups, my sub-group, my sink in the task
     bool valid;
 };
-__device__ __forceinline__ warp_task make_task(uint32_t g0, uint32_t g1, int fw, const uint32_t *__restrict__ gfirst,
-                                               const uint32_t *__restrict__ gcount)
+__device__ __forceinline__ warp_task make_task(uint32_t t0, uint32_t t1, int fw, const uint32_t *__restrict__ taskmap,
+                                               const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount)
 {
     warp_task t;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t task = blockIdx.x * fw + warp;
-    t.g = g0 + (task >> 1);
+    const uint32_t task = t0 + blockIdx.x * fw + warp;
     t.valid = false;
-    t.first = 0; t.ns = 0; t.W = 32; t.S = 1; t.sub = 0; t.j = 0;
-    if (t.g >= g1) return t;
-    const uint32_t count = gcount[t.g], h = task & 1u;
-    if (32u * h >= count) return t;
+    t.g = 0; t.first = 0; t.ns = 0; t.W = 32; t.S = 1; t.sub = 0; t.j = 0;
+    if (task >= t1) return t;
+    const uint32_t m = taskmap[task], h = m & 1u;
+    t.g = m >> 1;
+    const uint32_t count = gcount[t.g];
     t.valid = true;
     t.ns = min(32u, count - 32u * h);
     t.first = gfirst[t.g] + 32u * h;
@@ -187,7 +187,7 @@ __device__ __forceinline__ void task_store(const warp_task &t, float4 hi, float4
 #define FW 4                 // warps (tasks) per block
 
 template <int P, bool POT, bool PACKED>
-__global__ void __launch_bounds__(FW * 32) k_m2p(uint32_t g0, uint32_t g1, int periodic, float box, float eps2,
+__global__ void __launch_bounds__(FW * 32) k_m2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic, float box, float eps2,
                                                  const float *__restrict__ rows, const float4 *__restrict__ spos,
                                                  const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
                                                  const uint32_t *__restrict__ gcell, const uint32_t *__restrict__ list,
@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(FW * 32) k_m2p(uint32_t g0, uint32_t g1, int p
     constexpr int TC = (P <= 6) ? 32 : 16;                  // cells per tile (one per lane at most)
     __shared__ uint32_t s_cell_all[FW][TC];
     __shared__ __align__(16) float2 tile_all[FW][TC / 2][TROW];
-    const warp_task t = make_task(g0, g1, FW, gfirst, gcount);
+    const warp_task t = make_task(t0, t1, FW, taskmap, gfirst, gcount);
     if (!t.valid) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint32_t *s_cell = s_cell_all[warp];
@@ -269,7 +269,7 @@ __global__ void __launch_bounds__(FW * 32) k_m2p(uint32_t g0, uint32_t g1, int p
 
 // ---- F1 ----------------------------------------------------------------------------------------------
 template <bool POT>
-__global__ void __launch_bounds__(FW * 32) k_p2p(uint32_t g0, uint32_t g1, int periodic, float box, float eps2,
+__global__ void __launch_bounds__(FW * 32) k_p2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic, float box, float eps2,
                                                  int rowlen, const float *__restrict__ rows,
                                                  const dsk_cellrec *__restrict__ cell, const float4 *__restrict__ spos,
                                                  const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
@@ -282,7 +282,7 @@ __global__ void __launch_bounds__(FW * 32) k_p2p(uint32_t g0, uint32_t g1, int p
     __shared__ uint32_t s_pref_all[FW][33];
     __shared__ float s_sh_all[FW][32][3];
     __shared__ __align__(16) float4 tA_all[FW][P2P_TILE / 2], tB_all[FW][P2P_TILE / 2];   // {xA,xB,yA,yB}, {zA,zB,mA,mB}
-    const warp_task t = make_task(g0, g1, FW, gfirst, gcount);
+    const warp_task t = make_task(t0, t1, FW, taskmap, gfirst, gcount);
     if (!t.valid) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint32_t *s_first = s_first_all[warp], *s_pref = s_pref_all[warp];
@@ -373,21 +373,22 @@ __global__ void __launch_bounds__(FW * 32) k_p2p(uint32_t g0, uint32_t g1, int p
 }
 
 template <int P>
-static void launch_m2p(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t base, int want_pot)
+static void launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int want_pot)
 {
     const float e2 = c->eps * c->eps;
     constexpr bool PACKED = (P <= 6);
     if (want_pot)
-        k_m2p<P, true, PACKED><<<(2 * (g1 - g0) + FW - 1) / FW, FW * 32, 0, c->stream>>>(g0, g1, c->periodic, c->box, e2, c->rows, c->spos, c->gfirst,
+        k_m2p<P, true, PACKED><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, c->stream>>>(t0, t1, c->g_task, c->periodic, c->box, e2, c->rows, c->spos, c->gfirst,
                                                               c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
                                                               c->g_m2p_len, c->sacc, c->sacc_lo);
     else
-        k_m2p<P, false, PACKED><<<(2 * (g1 - g0) + FW - 1) / FW, FW * 32, 0, c->stream>>>(g0, g1, c->periodic, c->box, e2, c->rows, c->spos, c->gfirst,
+        k_m2p<P, false, PACKED><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, c->stream>>>(t0, t1, c->g_task, c->periodic, c->box, e2, c->rows, c->spos, c->gfirst,
                                                                c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
                                                                c->g_m2p_len, c->sacc, c->sacc_lo);
 }
 
-static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t mb, uint64_t pb, int want_pot, bool fill)
+static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_t t1, uint64_t mb, uint64_t pb,
+                      int want_pot, bool fill)
 {
     cudaStream_t s = c->stream;
     if (fill) {
@@ -398,17 +399,17 @@ static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t mb, uint64_
     const float e2 = c->eps * c->eps;
     const int rowlen = dsk_rowlen(c->p);
     if (want_pot)
-        k_p2p<true><<<(2 * (g1 - g0) + FW - 1) / FW, FW * 32, 0, s>>>(g0, g1, c->periodic, c->box, e2, rowlen, c->rows, c->cell, c->spos, c->gfirst,
+        k_p2p<true><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task, c->periodic, c->box, e2, rowlen, c->rows, c->cell, c->spos, c->gfirst,
                                            c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     else
-        k_p2p<false><<<(2 * (g1 - g0) + FW - 1) / FW, FW * 32, 0, s>>>(g0, g1, c->periodic, c->box, e2, rowlen, c->rows, c->cell, c->spos, c->gfirst,
+        k_p2p<false><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task, c->periodic, c->box, e2, rowlen, c->rows, c->cell, c->spos, c->gfirst,
                                             c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     cudaEventRecord(c->ev[9], s);
     switch (c->p) {
-    case 2: launch_m2p<2>(c, g0, g1, mb, want_pot); break;
-    case 4: launch_m2p<4>(c, g0, g1, mb, want_pot); break;
-    case 6: launch_m2p<6>(c, g0, g1, mb, want_pot); break;
-    case 8: launch_m2p<8>(c, g0, g1, mb, want_pot); break;
+    case 2: launch_m2p<2>(c, t0, t1, mb, want_pot); break;
+    case 4: launch_m2p<4>(c, t0, t1, mb, want_pot); break;
+    case 6: launch_m2p<6>(c, t0, t1, mb, want_pot); break;
+    case 8: launch_m2p<8>(c, t0, t1, mb, want_pot); break;
     default: return DSK_EINVAL;
     }
     cudaEventRecord(c->ev[10], s);
@@ -432,7 +433,7 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     const bool reuse = c->lists_valid && c->lists_theta == c->theta;
     c->stats.ms_p2p = c->stats.ms_m2p = 0.0f;
     if (reuse) {
-        int e = eval_batch(c, 0, ng, 0, 0, want_pot, false);
+        int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, want_pot, false);
         if (e) return e;
         DSK_CUDA(cudaStreamSynchronize(s));
         add_ms(c->ev[8], c->ev[9], &c->stats.ms_p2p);
@@ -449,7 +450,7 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     // reset the interaction counters (filled by the FILL pass)
     DSK_CUDA(cudaMemsetAsync(&c->dstate->tot_m2p_list, 0, sizeof(unsigned long long) * 5, s));
     if (tot[0] <= c->list_m2p_cap && tot[1] <= c->list_p2p_cap) {
-        int e = eval_batch(c, 0, ng, 0, 0, want_pot, true);
+        int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, want_pot, true);
         if (e) return e;
         DSK_CUDA(cudaStreamSynchronize(s));
         add_ms(c->ev[7], c->ev[8], &c->stats.ms_walk);
@@ -460,8 +461,12 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
         return DSK_OK;
     }
     // batches: cut the group range where either list would overflow
-    uint64_t *hm = (uint64_t *)malloc(sizeof(uint64_t) * ((size_t)ng + 1) * 2), *hp = hm + ng + 1;
+    uint64_t *hm = (uint64_t *)malloc(sizeof(uint64_t) * ((size_t)ng + 1) * 2 + sizeof(uint32_t) * ((size_t)ng + 1));
     if (!hm) return DSK_ECUDA;
+    uint64_t *hp = hm + ng + 1;
+    uint32_t *ht = (uint32_t *)(hp + ng + 1);
+    cudaMemcpyAsync(ht, c->g_taskoff, sizeof(uint32_t) * (size_t)ng, cudaMemcpyDeviceToHost, s);
+    ht[ng] = c->hstate->ntask;
     cudaMemcpyAsync(hm, c->g_m2p_off, sizeof(uint64_t) * ((size_t)ng + 1), cudaMemcpyDeviceToHost, s);
     cudaMemcpyAsync(hp, c->g_p2p_off, sizeof(uint64_t) * ((size_t)ng + 1), cudaMemcpyDeviceToHost, s);
     if (cudaStreamSynchronize(s) != cudaSuccess) { free(hm); return DSK_ECUDA; }
@@ -472,7 +477,7 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
         while (g1 < ng && hm[g1 + 1] - hm[g0] <= c->list_m2p_cap && hp[g1 + 1] - hp[g0] <= c->list_p2p_cap) g1++;
         if (g1 == g0) { rc = DSK_ELISTOVERFLOW; break; }           // one group alone does not fit
         cudaEventRecord(c->ev[11], s);
-        rc = eval_batch(c, g0, g1, hm[g0], hp[g0], want_pot, true);
+        rc = eval_batch(c, g0, g1, ht[g0], ht[g1], hm[g0], hp[g0], want_pot, true);
         if (rc) break;
         if (cudaStreamSynchronize(s) != cudaSuccess) { rc = DSK_ECUDA; break; }
         add_ms(c->ev[11], c->ev[8], &c->stats.ms_walk);

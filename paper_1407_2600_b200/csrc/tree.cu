@@ -205,7 +205,7 @@ __global__ void __launch_bounds__(TB) k_group_emit(const uint32_t *__restrict__ 
 __global__ void __launch_bounds__(TB) k_group_bbox(const float4 *__restrict__ spos,
                                                    const uint32_t *__restrict__ gfirst,
                                                    uint32_t *__restrict__ gcount, float4 *__restrict__ gbox,
-                                                   uint32_t n, const dsk_devstate *st)
+                                                   uint32_t *__restrict__ ntask, uint32_t n, const dsk_devstate *st)
 {
     uint32_t ng = st->ngroup;
     uint32_t g = (blockIdx.x * TB + threadIdx.x) >> 5;
@@ -225,10 +225,22 @@ __global__ void __launch_bounds__(TB) k_group_bbox(const float4 *__restrict__ sp
             hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
         }
     if (lane == 0) {
+        ntask[g] = (e - f + 31u) >> 5;
         gcount[g] = e - f;
         gbox[2 * (size_t)g] = make_float4(lo[0], lo[1], lo[2], 0.0f);
         gbox[2 * (size_t)g + 1] = make_float4(hi[0], hi[1], hi[2], 0.0f);
     }
+}
+
+// task -> (group, half) map for the warp-task force kernels
+__global__ void __launch_bounds__(TB) k_task_fill(const uint32_t *__restrict__ taskoff, uint32_t *__restrict__ task,
+                                                  dsk_devstate *st)
+{
+    const uint32_t ng = st->ngroup;
+    const uint32_t g = blockIdx.x * TB + threadIdx.x;
+    if (g >= ng) return;
+    const uint32_t a = taskoff[g], b = (g + 1 < ng) ? taskoff[g + 1] : st->ntask;
+    for (uint32_t k = a; k < b; k++) task[k] = (g << 1) | (k - a);
 }
 
 int dsk_run_build(dsk_ctx *c)
@@ -252,8 +264,10 @@ int dsk_run_build(dsk_ctx *c)
     k_group_emit<<<nb, TB, 0, s>>>(c->gmark, c->gscan, n, (uint32_t)c->ngroup_cap, c->gfirst, c->gcell, c->dstate);
     // one warp per possible group; ngroup is read on the device
     const int64_t nwarp_blocks = (c->ngroup_cap * 32 + TB - 1) / TB;
-    k_group_bbox<<<(unsigned)nwarp_blocks, TB, 0, s>>>(c->spos, c->gfirst, c->gcount, c->gbox, n, c->dstate);
+    k_group_bbox<<<(unsigned)nwarp_blocks, TB, 0, s>>>(c->spos, c->gfirst, c->gcount, c->gbox, c->g_taskoff, n, c->dstate);
+    dsk_exclusive_scan_u32(c, c->g_taskoff, c->g_taskoff, &c->dstate->ngroup, (uint32_t)c->ngroup_cap, &c->dstate->ntask);
+    k_task_fill<<<(unsigned)((c->ngroup_cap + TB - 1) / TB), TB, 0, s>>>(c->g_taskoff, c->g_task, c->dstate);
     cudaEventRecord(c->ev[4], s);
-    DSK_COUNT(c, 1 + 2 * (DSK_KEY_LEVELS + 1) + 4);   // init, count+emit per level, mark/flag/emit/bbox
+    DSK_COUNT(c, 1 + 2 * (DSK_KEY_LEVELS + 1) + 5);   // init, count+emit per level, mark/flag/emit/bbox/taskfill
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
