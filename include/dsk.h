@@ -81,7 +81,8 @@ int dsk_bind_workspace(dsk_ctx *ctx, void *dev_ptr, size_t bytes);
 /* cudaStream_t as void* (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream. */
 int dsk_set_stream(dsk_ctx *ctx, void *cuda_stream);
 /* Change eps / theta / p without rebuilding the tree (moments are recomputed when p changes, lists
- * when theta changes) — the (theta, p) sweep of BASELINE.json configs[1]. */
+ * when theta changes) — the (theta, p) sweep of BASELINE.json configs[1].  p may not exceed the p given
+ * to dsk_create (the workspace is sized for that order): DSK_ENOWORKSPACE otherwise. */
 int dsk_set_params(dsk_ctx *ctx, float eps, float theta, int p);
 
 /* Keys -> sort -> octree -> groups -> upward pass (order p) for these positions and masses.

@@ -4,34 +4,51 @@ Bookkeeping only — none of the method's arithmetic lives here.
 """
 
 
-def _levels(p):
-    for l in range(p + 2):
-        for a in range(l, -1, -1):
-            for b in range(l - a, -1, -1):
-                yield l, a, b, l - a - b
+def _fr_has(p, q, m):
+    return m >= q and 2 * m - q <= p and not (q == 1 and m == 1)
+
+
+def _rank(q):
+    return [(a, b, q - a - b) for a in range(q, -1, -1) for b in range(q - a, -1, -1)]
 
 
 def m2p_ops(p, pot=True):
-    """(ffma, fmul, fadd) per cell-particle interaction of k_m2p at order p."""
-    ffma, fmul, fadd = 3, 3 + 1, 3          # R2 chain; rho = r * sinv, q = D0^2; r = x - com
-    if pot:
-        fmul += 1                           # phi = Mhat_0 * D0
-    for l in range(1, p + 2):
-        fmul += 1 + 3                       # A, u_x[1], u_y[1], u_z[1]
-        fadd += 3 * (l - 1)                 # u_i[k] = u_i[k-1] + u_i[1]
-        fmul += (l - 1)                     # w[k]
-    for l, a, b, c in _levels(p):
-        if l == 0:
-            continue
-        t1 = (a >= 1) + (b >= 1) + (c >= 1)
-        t2 = (a >= 2) + (b >= 2) + (c >= 2)
-        fmul += 1
-        ffma += t1 - 1 + t2                 # recurrence
-        ffma += t1                          # gradient contraction
-        if pot and l <= p:
-            ffma += 1                       # potential contraction
-    fmul += 1                               # sinv^2
-    ffma += 3 + (1 if pot else 0)           # fold the cell's sums with 1/s^2, 1/s
+    """(ffma, fmul, fadd) per cell-particle interaction of k_m2p at order p (pairing form, m2p.cu)."""
+    ffma, fmul, fadd = 3, 3 + 1, 3          # R2 chain; rho = r * sinv, q = h0^2; r = x - com
+    fmul += 3 * (p - 1)                     # rho_i / k, k = 2..p
+    for q in range(p + 1):
+        if q >= 2:
+            fmul += len(_rank(q))           # monomials of degree q
+        for m in range(q, p + 1):
+            if not _fr_has(p, q, m):
+                continue
+            qfirst_s = 0 if (m == 1 or 2 * m - p < 0) else 2 * m - p
+            qfirst_g = max(1, 2 * m - p)
+            for jj, j in enumerate(_rank(q)):
+                if q > 0:                   # S_m += B mu_j  (q = 0: plain assignment)
+                    if q == qfirst_s and jj == 0:
+                        fmul += 1
+                    else:
+                        ffma += 1
+                if m >= 2 and q >= 2:       # G_m,i += B mu_{j - e_i}  (q = 1: plain assignment)
+                    for i in range(3):
+                        if j[i] >= 1:
+                            if q == qfirst_g and jj == i:
+                                fmul += 1
+                            else:
+                                ffma += 1
+    fmul += 1                               # phi = h0 S_0
+    for m in range(1, p + 1):
+        fmul += 2                           # h_m, w = h_m S_m
+        ffma += 1                           # tt += (2m+1) w
+        if pot:
+            fadd += 1
+        if m == 2:
+            fmul += 3
+        elif m > 2:
+            ffma += 3
+    fmul += 3                               # sinv^2, q tt, * -sinv^2
+    ffma += 6 + (1 if pot else 0)           # fold the cell's sums
     return ffma, fmul, fadd
 
 

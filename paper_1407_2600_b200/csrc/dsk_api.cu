@@ -38,7 +38,10 @@ static size_t carve(dsk_ctx *c, char *base)
     c->parent = (uint32_t *)take(4 * nc);
     c->nchild_tmp = (uint32_t *)take(4 * nc);
     c->whdr = (float4 *)take(16 * nc);
-    c->rows = (float *)take(4 * (size_t)dsk_rowlen(DSK_PMAX) * nc);
+    c->rows = (float *)take(4 * (size_t)dsk_rowlen(c->p_cap) * nc);
+    c->frows = (float *)take(4 * (size_t)dsk_frow_len(c->p_cap) * nc);
+    c->frtab_beg = (uint32_t *)take(4 * DSK_FRTAB_BEG);
+    c->frtab_ent = (void *)take(8 * DSK_FRTAB_ENT);
     c->gmark = (uint32_t *)take(4 * n);
     c->gscan = (uint32_t *)take(4 * n);
     c->gfirst = (uint32_t *)take(4 * ng);
@@ -87,7 +90,7 @@ extern "C" int dsk_create(dsk_ctx **out, int64_t N, float box, int periodic, flo
     if (!c) return DSK_ECUDA;
     memset(c, 0, sizeof(*c));
     c->N = N; c->box = box; c->periodic = periodic ? 1 : 0; c->eps = eps; c->theta = theta; c->p = p;
-    c->moments_p = -1;
+    c->moments_p = -1; c->p_cap = p; c->frow_tab_p = -1;
     c->ws_bytes = 0;
     carve(c, nullptr);
     if (c->periodic) dsk_lattice_tensors((double)box, DSK_WS, c->far_T);
@@ -130,7 +133,7 @@ extern "C" int dsk_bind_workspace(dsk_ctx *c, void *dev_ptr, size_t bytes)
     c->ws = (char *)dev_ptr;
     c->ws_bytes = bytes;
     carve(c, c->ws);
-    c->have_tree = 0; c->moments_p = -1; c->lists_valid = 0; c->kdk_have_acc = 0;
+    c->have_tree = 0; c->moments_p = -1; c->lists_valid = 0; c->kdk_have_acc = 0; c->frow_tab_p = -1;
     if (c->periodic)
         DSK_CUDA(cudaMemcpyAsync(c->far_T_dev, c->far_T, sizeof(double) * DSK_NFAR, cudaMemcpyHostToDevice, c->stream));
     DSK_CUDA(cudaMemsetAsync(c->dstate, 0, sizeof(dsk_devstate), c->stream));
@@ -149,6 +152,7 @@ extern "C" int dsk_set_params(dsk_ctx *c, float eps, float theta, int p)
 {
     if (!c) return DSK_EINVAL;
     if (check_params(eps, theta, p)) return DSK_EINVAL;
+    if (p > c->p_cap) return DSK_ENOWORKSPACE;        // rows were sized for dsk_create's p
     c->eps = eps; c->theta = theta; c->p = p;
     return DSK_OK;
 }

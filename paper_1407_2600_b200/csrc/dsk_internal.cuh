@@ -14,6 +14,8 @@
 #define DSK_PMAX 8
 #define DSK_IMG_BITS 7        // list entry = image << 25 | cell ... see below
 #define DSK_CELL_BITS 25
+#define DSK_FRTAB_BEG 320     // >= fr_nc(8) + 1 = 293
+#define DSK_FRTAB_ENT 768     // >= 739 map entries at p = 8
 // A list entry packs (image id, cell id).  With WS = 2 there are 125 images (7 bits) which leaves
 // 25 bits = 33.5 M cells per tree; larger trees use WS-image ids only in periodic mode, so isolated
 // runs could use all 32 bits — kept uniform for simplicity (N <= ~1.3e8 at ~0.25 cells/particle).
@@ -68,7 +70,10 @@ struct dsk_ctx {
     uint32_t *parent;
     uint32_t *nchild_tmp;
     float4 *whdr;             // walk header per cell: com.xyz, delta
-    float *rows;              // [ncell_cap * rowlen(p)]
+    float *rows;              // [ncell_cap * rowlen(p_cap)] moment rows (upward.cu)
+    float *frows;             // [ncell_cap * frow_len(p_cap)] force rows read by M2P (m2p.cu)
+    uint32_t *frtab_beg;      // [DSK_FRTAB_BEG] moment row -> force row map of the current p
+    void *frtab_ent;          // [DSK_FRTAB_ENT] {src, weight}
     uint32_t *gmark;          // [N] group start markers (cell id + 1)
     uint32_t *gscan;          // [N]
     uint32_t *gfirst, *gcount, *gcell;     // [ngroup_cap]
@@ -91,6 +96,8 @@ struct dsk_ctx {
     int ntile;
     // state
     int have_tree, moments_p, lists_valid, kdk_have_acc;
+    int p_cap;                // order the workspace was sized for (dsk_create's p); set_params may lower p
+    int frow_tab_p;           // order of the uploaded force-row map
     float lists_theta;
     double far_T[DSK_NFAR];
     dsk_stats stats;
@@ -114,7 +121,10 @@ int dsk_run_build(dsk_ctx *c);                                                //
 int dsk_run_upward(dsk_ctx *c);                                               // upward.cu: U
 int dsk_run_get_moments(dsk_ctx *c, float *com_mass, float *moments);         // upward.cu
 int dsk_run_walk(dsk_ctx *c);                                                 // walk.cu: W
-int dsk_run_force(dsk_ctx *c, int want_pot);                                  // force.cu: F1, F2
+int dsk_run_force(dsk_ctx *c, int want_pot);                                  // force.cu: F1 + orchestration
+int dsk_frow_len(int p);                                                      // m2p.cu
+int dsk_run_frows(dsk_ctx *c);                                                // m2p.cu: moment rows -> force rows
+int dsk_launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int want_pot);   // m2p.cu: F2
 int dsk_run_farfield(dsk_ctx *c);                                             // farfield.cu: F3
 void dsk_lattice_tensors(double L, int ws, double *T);                        // farfield.cu (host)
 int dsk_run_kick(dsk_ctx *c, float *vel, const float *acc, float k);          // kdk.cu

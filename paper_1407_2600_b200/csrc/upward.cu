@@ -217,6 +217,8 @@ int dsk_run_upward(dsk_ctx *c)
     case 8: launch_upward<8>(c, ls, nl); break;
     default: return DSK_EINVAL;
     }
+    e = dsk_run_frows(c);                      // the fixed linear map to the rows M2P reads (m2p.cu)
+    if (e) return e;
     cudaEventRecord(c->ev[6], c->stream);
     c->moments_p = c->p;
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;

@@ -106,7 +106,8 @@ def _dev_f32(t, shape=None):
 class Dsk:
     """One dsk_ctx plus the torch-owned workspace it borrows."""
 
-    def __init__(self, N, box=1.0, periodic=False, eps=1e-3, theta=0.5, p=4, device="cuda:0", stream=None):
+    def __init__(self, N, box=1.0, periodic=False, eps=1e-3, theta=0.5, p=4, device="cuda:0", stream=None, p_max=None):
+        """p_max: the highest order set_params will be asked for (the workspace is sized for it)."""
         self.lib = load_library()
         if not torch.cuda.is_available():
             raise RuntimeError("dsk needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -114,8 +115,11 @@ class Dsk:
         self.N, self.box, self.periodic = int(N), float(box), bool(periodic)
         self.eps, self.theta, self.p = float(eps), float(theta), int(p)
         h = C.c_void_p(0)
-        _check(self.lib.dsk_create(C.byref(h), self.N, self.box, int(self.periodic), self.eps, self.theta, self.p))
+        p_create = max(self.p, int(p_max)) if p_max is not None else self.p
+        _check(self.lib.dsk_create(C.byref(h), self.N, self.box, int(self.periodic), self.eps, self.theta, p_create))
         self._h = h
+        if p_create != self.p:
+            _check(self.lib.dsk_set_params(self._h, self.eps, self.theta, self.p))
         with torch.cuda.device(self.device):
             nbytes = self.lib.dsk_workspace_bytes(self._h)
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)

@@ -52,7 +52,9 @@ def test_create_validation_and_workspace(lib):
     assert lib.dsk_accel(h, C.c_void_p(256), C.c_void_p(256), C.c_void_p(256), None) == -2
     assert lib.dsk_bind_workspace(h, C.c_void_p(0), b1) == -2
     assert lib.dsk_bind_workspace(h, C.c_void_p(257), b1) == -2
-    assert lib.dsk_set_params(h, 1e-4, 0.3, 8) == 0 and lib.dsk_set_params(h, 1e-4, 0.3, 5) == -1
+    # p may be lowered but not raised above dsk_create's p (the workspace is sized for it)
+    assert lib.dsk_set_params(h, 1e-4, 0.3, 2) == 0 and lib.dsk_set_params(h, 1e-4, 0.3, 5) == -1
+    assert lib.dsk_set_params(h, 1e-4, 0.3, 8) == -2
     assert lib.dsk_destroy(h) == 0
     assert lib.dsk_strerror(-4).decode().startswith("position outside")
     h2 = C.c_void_p(0)

@@ -187,7 +187,7 @@ def test_forces_C2_sweep_scaled(dsk, orc):
     n = len(pos)
     sink = workloads.subsample(2, n, 1024)
     da, _ = orc.direct_iso(pos, mass, 1e-4, sink)
-    d = dsk.Dsk(n, 1.0, False, 1e-4, 0.5, 4)
+    d = dsk.Dsk(n, 1.0, False, 1e-4, 0.5, 4, p_max=8)
     tp, tm = _dev(pos), _dev(mass)
     d.build_tree(tp, tm)
     tree = orc.OracleTree(pos, mass)
