@@ -47,9 +47,24 @@ def test_aggregate_single():
 
 
 def test_accounting_matches_kernel_op_counts():
-    """flop accounting (roofline numerator) against the op counts read off the SASS of k_m2p<4> (256 FFMA2)."""
-    from paper_1407_2600_b200 import accounting
-    assert accounting.m2p_ops(4, pot=True)[0] == 256
+    """flop accounting (roofline numerator) against the op counts in the SASS of k_m2p<P, pot> as built:
+    one FFMA2 / FMUL2 / FADD2 per counted ffma / fmul / fadd (the body is straight-line, inlined once)."""
+    import shutil
+    import subprocess
+    from paper_1407_2600_b200 import accounting, build
+    assert accounting.m2p_ops(4, pot=True) == (118, 67, 7)
     assert accounting.p2p_flops(pot=True) == 19
     assert accounting.m2p_flops(4) > accounting.m2p_flops(2) and accounting.m2p_flops(8) > accounting.m2p_flops(6)
     assert abs(accounting.fp32_peak_flops(148, 1965.0) - 74.45e12) < 0.1e12
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    obj = os.path.join(os.path.dirname(build.LIB), "build", "m2p.o")
+    if not (os.path.exists(cuobjdump) and os.path.exists(obj)):
+        return
+    sass = subprocess.run([cuobjdump, "-sass", obj], capture_output=True, text=True).stdout
+    for p in (2, 4, 6):                                     # the packed (f32x2) instantiations
+        fn = [b for b in sass.split("Function : ")[1:] if b.startswith(f"_Z5k_m2pILi{p}ELb1EE")]
+        assert len(fn) == 1
+        ffma, fmul, fadd = accounting.m2p_ops(p, pot=True)
+        assert fn[0].count(" FFMA2 ") == ffma, (p, fn[0].count(" FFMA2 "), ffma)
+        assert fn[0].count(" FMUL2 ") == fmul, (p, fn[0].count(" FMUL2 "), fmul)
+        assert fn[0].count(" FADD2 ") == fadd, (p, fn[0].count(" FADD2 "), fadd)
