@@ -52,7 +52,7 @@ static size_t carve(dsk_ctx *c, char *base)
     c->g_p2p_len = (uint32_t *)take(4 * ng);
     c->g_p2p_src = (uint32_t *)take(4 * ng);
     c->g_taskoff = (uint32_t *)take(4 * (ng + 1));
-    c->g_task = (uint32_t *)take(8 * ng);
+    c->g_task = (uint32_t *)take(16 * ng);
     c->g_m2p_off = (uint64_t *)take(8 * (ng + 1));
     c->g_p2p_off = (uint64_t *)take(8 * (ng + 1));
     // interaction lists: 256 / 32 entries per particle cover theta >= 0.3 in one batch on the paper-like

@@ -29,6 +29,17 @@ __host__ __device__ constexpr int dsk_midx(int a, int b, int c)
 // ctr = geometric cell centre (exact), off = com - ctr, Mhat_n = (-1)^|n| M_n / (n! s^|n|)
 __host__ __device__ constexpr int dsk_rowlen(int p) { return ((8 + dsk_np(p)) + 3) / 4 * 4; }
 
+// force tasks (force_task.cuh): two sinks per lane; number of tasks a group of n (1..64) sinks is cut into: maximise S(k)/k, S(k) = 32 / ceil(ceil(n/k)/2)
+__host__ __device__ __forceinline__ uint32_t dsk_task_parts(uint32_t n)
+{
+    uint32_t bk = 1, bs = 0;
+    for (uint32_t k = 1; k <= 4; k++) {
+        const uint32_t per = (n + k - 1) / k, w = (per + 1) / 2, s = w ? 32u / w : 0u;
+        if (k == 1 || s * bk > bs * k) { bk = k; bs = s; }
+    }
+    return bk;
+}
+
 struct dsk_cellrec {          // 16 B, one LDG.128 in the walk
     uint32_t first, count, child0, meta;   // meta = nchild | level << 8
 };
@@ -37,7 +48,7 @@ struct dsk_devstate {         // small device block read back at the end of API 
     uint32_t status;          // bit flags: 1 out-of-box, 2 non-finite, 4 cell overflow, 8 stack overflow,
                               //            16 list overflow
     uint32_t ncell, ngroup, nlevel;
-    uint32_t ntask;           // warp tasks = sum over groups of ceil(count / 32)
+    uint32_t ntask;           // warp tasks = sum over groups of dsk_task_parts(count)
     uint32_t lvl_start[DSK_KEY_LEVELS + 3];
     uint32_t nleaf_cells;
     unsigned long long tot_m2p_list, tot_p2p_list, tot_p2p_src;   // over all groups
@@ -79,8 +90,8 @@ struct dsk_ctx {
     uint32_t *gfirst, *gcount, *gcell;     // [ngroup_cap]
     float4 *gbox;             // [2 * ngroup_cap]: min.xyz,_ ; max.xyz,_
     uint32_t *g_m2p_len, *g_p2p_len, *g_p2p_src;   // [ngroup_cap]
-    uint32_t *g_taskoff;      // [ngroup_cap + 1] exclusive scan of ceil(count/32)
-    uint32_t *g_task;         // [2 * ngroup_cap] task -> group << 1 | half
+    uint32_t *g_taskoff;      // [ngroup_cap + 1] exclusive scan of dsk_task_parts(count)
+    uint32_t *g_task;         // [4 * ngroup_cap] task -> group << 2 | part
     uint64_t *g_m2p_off, *g_p2p_off;               // [ngroup_cap + 1] exclusive offsets into lists
     uint32_t *list_m2p, *list_p2p;
     size_t list_m2p_cap, list_p2p_cap;             // entries

@@ -3,23 +3,23 @@
 // set of n sink particles ... perform the full m x n interactions on this block"; PAPER.md:75 direct
 // interactions near the leaves).  F2 (M2P) lives in m2p.cu; the task decomposition in force_task.cuh.
 //
-// One warp per (group, 32-sink half) task, one sink per lane.  Source tiles are staged through per-warp
-// shared memory in PAIR-INTERLEAVED form {A,B}, read back with broadcast LDS.128 and consumed with packed
-// f32x2 arithmetic: every thread handles 1 sink x 2 sources per instruction (FFMA2 is the only way to reach
-// the FP32 peak with three distinct operands on sm_100, see dsk_internal.cuh).
+// One warp per task (force_task.cuh), two sinks per lane in the halves of packed f32x2 registers (FFMA2 is
+// the only way to reach the FP32 peak with three distinct operands on sm_100, see dsk_internal.cuh); source
+// tiles are staged through per-warp shared memory as (x, y, z, m) and enter as broadcast scalar operands.
 // All coordinates are taken relative to the group's cell centre c_g (exact subtraction for nearby
 // values), which keeps fp32 differences accurate and absorbs the periodic image shift.
 //
 // F1: Plummer pair, acc_i += m_j d / (|d|^2+eps^2)^(3/2), pot_i -= m_j / sqrt(...), d = x_j - x_i.
 #include "force_task.cuh"
 
+#define FW 4                 // warps (tasks) per block
 #define P2P_TILE 128         // sources per warp tile
 
 int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base);   // walk.cu
 
 // ---- F1 ----------------------------------------------------------------------------------------------
 template <bool POT>
-__global__ void __launch_bounds__(FW * 32) k_p2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic, float box, float eps2,
+__global__ void __launch_bounds__(FW * 32, 6) k_p2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic, float box, float eps2,
                                                  int rowlen, const float *__restrict__ rows,
                                                  const dsk_cellrec *__restrict__ cell, const float4 *__restrict__ spos,
                                                  const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
@@ -31,23 +31,22 @@ __global__ void __launch_bounds__(FW * 32) k_p2p(uint32_t t0, uint32_t t1, const
     __shared__ uint32_t s_first_all[FW][32];
     __shared__ uint32_t s_pref_all[FW][33];
     __shared__ float s_sh_all[FW][32][3];
-    __shared__ __align__(16) float4 tA_all[FW][P2P_TILE / 2], tB_all[FW][P2P_TILE / 2];   // {xA,xB,yA,yB}, {zA,zB,mA,mB}
-    const warp_task t = make_task(t0, t1, taskmap, gfirst, gcount);
+    __shared__ __align__(16) float4 src_all[FW][P2P_TILE];        // (x, y, z, m) relative to the group centre
+    const warp_task t = make_task(t0, t1, FW, taskmap, gfirst, gcount);
     if (!t.valid) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint32_t *s_first = s_first_all[warp], *s_pref = s_pref_all[warp];
     float(*s_sh)[3] = s_sh_all[warp];
-    float4 *tA = tA_all[warp], *tB = tB_all[warp];
+    float4 *src = src_all[warp];
     const float *grow = rows + (size_t)gcell[t.g] * rowlen;
     const float cgx = grow[0], cgy = grow[1], cgz = grow[2];
-    const float4 me = spos[t.first + t.j];
-    const f2 X = f2_dup(me.x - cgx), Y = f2_dup(me.y - cgy), Z = f2_dup(me.z - cgz);
+    const float4 ma = spos[t.sa], mb = spos[t.sb];
+    const f2 X = f2_make(ma.x - cgx, mb.x - cgx), Y = f2_make(ma.y - cgy, mb.y - cgy), Z = f2_make(ma.z - cgz, mb.z - cgz);
     const f2 E2 = f2_dup(eps2);
     const uint32_t n = len[t.g];
     const uint32_t *lst = list + (off[t.g] - base);
-    float4 hi = make_float4(0.f, 0.f, 0.f, 0.f), lo = hi;     // two-float running sums (see k_m2p)
-    const uint32_t quantum = 2u * (uint32_t)t.S;                   // sources consumed per round of the sub-groups
-    const uint32_t tile = (uint32_t)P2P_TILE / quantum * quantum;  // so that padding never leaves the buffers
+    sink_acc A;                                               // two-float running sums (see k_m2p)
+    acc_zero(A);
     for (uint32_t b0 = 0; b0 < n; b0 += 32) {
         // one leaf (segment of sources) per lane; exclusive scan of the segment lengths
         uint32_t cnt = 0;
@@ -73,55 +72,45 @@ __global__ void __launch_bounds__(FW * 32) k_p2p(uint32_t t0, uint32_t t1, const
         s_pref[lane] = x - cnt;
         if (lane == 0) s_pref[32] = total;
         __syncwarp();
-        for (uint32_t t0 = 0; t0 < total; t0 += tile) {
-            const uint32_t nt = min(tile, total - t0);
-            const uint32_t npad = (nt + quantum - 1) / quantum * quantum;
-            for (uint32_t j = lane; j < npad; j += 32) {
-                float sx = 1.0e10f, sy = 1.0e10f, sz = 1.0e10f, sm = 0.0f;      // pad: far away, massless
-                if (j < nt) {
-                    const uint32_t gj = t0 + j;
-                    int a = 0, b = 32;                        // last segment with pref <= gj
-                    while (b - a > 1) {
-                        const int mid = (a + b) >> 1;
-                        if (s_pref[mid] <= gj) a = mid; else b = mid;
-                    }
-                    const float4 p = spos[s_first[a] + (gj - s_pref[a])];
-                    sx = (p.x - cgx) + s_sh[a][0]; sy = (p.y - cgy) + s_sh[a][1]; sz = (p.z - cgz) + s_sh[a][2];
-                    sm = p.w;
+        for (uint32_t t0 = 0; t0 < total; t0 += P2P_TILE) {
+            const uint32_t nt = min((uint32_t)P2P_TILE, total - t0);
+            for (uint32_t j = lane; j < nt; j += 32) {
+                const uint32_t gj = t0 + j;
+                int a = 0, b = 32;                        // last segment with pref <= gj
+                while (b - a > 1) {
+                    const int mid = (a + b) >> 1;
+                    if (s_pref[mid] <= gj) a = mid; else b = mid;
                 }
-                float *pa = reinterpret_cast<float *>(&tA[j >> 1]) + (j & 1);
-                float *pb = reinterpret_cast<float *>(&tB[j >> 1]) + (j & 1);
-                pa[0] = sx; pa[2] = sy; pb[0] = sz; pb[2] = sm;
+                const float4 p = spos[s_first[a] + (gj - s_pref[a])];
+                src[j] = make_float4((p.x - cgx) + s_sh[a][0], (p.y - cgy) + s_sh[a][1], (p.z - cgz) + s_sh[a][2], p.w);
             }
             __syncwarp();
-            {
+            if (t.active) {
                 f2 ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f), pot = f2_dup(0.0f);
-                const int npair = t.active ? (int)(npad >> 1) : 0;
 #pragma unroll 4
-                for (int k = t.sub; k < npair; k += t.S) {
-                    const ulonglong2 qa = *reinterpret_cast<const ulonglong2 *>(&tA[k]);
-                    const ulonglong2 qb = *reinterpret_cast<const ulonglong2 *>(&tB[k]);
-                    f2 sx, sy, sz, sm;
-                    sx.v = qa.x; sy.v = qa.y; sz.v = qb.x; sm.v = qb.y;
-                    const f2 dx = f2_sub(sx, X), dy = f2_sub(sy, Y), dz = f2_sub(sz, Z);
+                for (int k = t.sub; k < (int)nt; k += t.S) {
+                    const float4 s = src[k];
+                    const f2 dx = f2_sub(f2_dup(s.x), X), dy = f2_sub(f2_dup(s.y), Y), dz = f2_sub(f2_dup(s.z), Z);
                     f2 r2 = f2_fma(dx, dx, E2);
                     r2 = f2_fma(dy, dy, r2);
                     r2 = f2_fma(dz, dz, r2);
                     const f2 ri = f2_rsqrt(r2);
-                    const f2 ri2 = f2_mul(ri, ri), mri = f2_mul(sm, ri), mri3 = f2_mul(mri, ri2);
+                    const f2 ri2 = f2_mul(ri, ri), mri = f2_mul(f2_dup(s.w), ri), mri3 = f2_mul(mri, ri2);
                     ax = f2_fma(dx, mri3, ax); ay = f2_fma(dy, mri3, ay); az = f2_fma(dz, mri3, az);
                     if (POT) pot = f2_sub(pot, mri);
                 }
-                dsk_fold(hi.x, lo.x, vsum(ax)); dsk_fold(hi.y, lo.y, vsum(ay)); dsk_fold(hi.z, lo.z, vsum(az));
-                if (POT) dsk_fold(hi.w, lo.w, vsum(pot));
+                acc_fold(A, ax, ay, az, pot, POT);
             }
             __syncwarp();
         }
     }
     // the sink's own leaf is always in the list: remove its self term -m_i/eps from the potential (once)
-    if (POT && t.active && t.sub == 0) dsk_fold(hi.w, lo.w, me.w * rsqrtf(eps2));
+    if (POT && t.active && t.sub == 0) {
+        dsk_fold(A.hi[0].w, A.lo[0].w, ma.w * rsqrtf(eps2));
+        dsk_fold(A.hi[1].w, A.lo[1].w, mb.w * rsqrtf(eps2));
+    }
     __syncwarp();
-    task_store(t, hi, lo, reinterpret_cast<double *>(tA), sacc, sacc_lo);
+    task_store(t, A, reinterpret_cast<double *>(src), sacc, sacc_lo);
 }
 
 static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_t t1, uint64_t mb, uint64_t pb,

@@ -1,16 +1,19 @@
 // force_task.cuh — work decomposition and small vector abstraction shared by the force kernels
 // F1 (force.cu, P2P) and F2 (m2p.cu, M2P).  DESIGN.md section 5.
 //
-// One WARP per task; task = (group, half): sinks [32 half, 32 half + 32) of the group, so a group of <= 32
-// sinks is one warp and nothing waits at a block barrier.  Groups are tree cells, so many hold few sinks
-// (mean 18 of 64 on the Plummer workload): a task with ns <= 16 sinks splits the warp into S = 32 / ns
-// sub-groups of W = ns lanes that take alternate source pairs of a tile; their partial sums are added at
-// the end through shared memory.  Lanes >= W * S idle.
+// One WARP per task, TWO SINKS PER LANE: the two fp32 halves of every packed f32x2 register belong to two
+// sinks, and a source (cell coefficient, particle coordinate) enters FFMA2/FMUL2/FADD2 as a scalar operand
+// broadcast to both halves (SASS "R.F32"; measured 2.2 cycles per FFMA2 per SMSP against 2.0 for three packed
+// operands).  Sources therefore sit in shared memory exactly as they sit in global memory (no interleaving
+// pass), one LDS.128 brings four coefficients, and a warp covers up to 64 sinks = one whole group.
+// Groups hold 1..64 sinks (mean 18 on the Plummer workload), so a group of n sinks is cut into k <= 4 tasks
+// of ~n/k sinks; a task of ns sinks uses W = ceil(ns/2) lanes per sub-group and S = 32 / W sub-groups that
+// take alternate sources of a tile and are summed at the end through shared memory; k maximises the share of
+// busy lanes n S / (64 k) (0.90 on the Plummer workload against 0.75 with one sink per lane).
 #pragma once
 #include "dsk_internal.cuh"
 #include <type_traits>
 
-#define FW 4                 // warps (tasks) per block
 
 // ---- T = f2 (two sources per op, packed f32x2) or float ----------------------------------------------
 __device__ __forceinline__ f2 vfma(f2 a, f2 b, f2 c) { return f2_fma(a, b, c); }
@@ -62,56 +65,97 @@ __host__ __device__ constexpr MI dsk_mi(int i)
 
 struct warp_task {
     uint32_t g, first, ns;       // group, rank of the task's first sink, sinks in the task
-    int W, S, sub, j;            // sub-group width, number of sub-groups, my sub-group, my sink in the task
-    bool valid, active;          // task exists; this lane belongs to a sub-group
+    int W, S, sub, j;            // lanes per sub-group, number of sub-groups, my sub-group, my lane in it
+    uint32_t sa, sb;             // ranks of my two sinks (sb == sa when the task has an odd sink left over)
+    bool valid, active, has_b;   // task exists; this lane belongs to a sub-group; second sink is a real one
 };
-__device__ __forceinline__ warp_task make_task(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap,
+// taskmap entry = group << 2 | part
+__device__ __forceinline__ warp_task make_task(uint32_t t0, uint32_t t1, int fw, const uint32_t *__restrict__ taskmap,
                                                const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount)
 {
     warp_task t;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t task = t0 + blockIdx.x * FW + warp;
-    t.valid = false; t.active = false;
-    t.g = 0; t.first = 0; t.ns = 0; t.W = 32; t.S = 1; t.sub = 0; t.j = 0;
+    const uint32_t task = t0 + blockIdx.x * fw + warp;      // fw = warps (tasks) per block
+    t.valid = false; t.active = false; t.has_b = false;
+    t.g = 0; t.first = 0; t.ns = 0; t.W = 32; t.S = 1; t.sub = 0; t.j = 0; t.sa = t.sb = 0;
     if (task >= t1) return t;
-    const uint32_t m = taskmap[task], h = m & 1u;
-    t.g = m >> 1;
-    const uint32_t count = gcount[t.g];
+    const uint32_t m = taskmap[task], part = m & 3u;
+    t.g = m >> 2;
+    const uint32_t count = gcount[t.g], k = dsk_task_parts(count);
+    const uint32_t base = count / k, rem = count % k;
     t.valid = true;
-    t.ns = min(32u, count - 32u * h);
-    t.first = gfirst[t.g] + 32u * h;
-    t.W = (int)t.ns;
+    t.ns = base + (part < rem ? 1u : 0u);
+    t.first = gfirst[t.g] + part * base + min(part, rem);
+    t.W = (int)((t.ns + 1u) >> 1);
     t.S = 32 / t.W;
     t.sub = lane / t.W;
     t.active = t.sub < t.S;
     t.j = lane - t.sub * t.W;
     if (!t.active) { t.sub = 0; t.j = 0; }
+    t.has_b = 2u * (uint32_t)t.j + 1u < t.ns;
+    t.sa = t.first + 2u * (uint32_t)t.j;
+    t.sb = t.has_b ? t.sa + 1u : t.sa;
     return t;
 }
 
-// Add the sub-groups' two-float accumulators (in double, through the warp's scratch: >= 32 x 4 doubles,
-// 16-byte aligned, free for reuse) and store; lane j < ns owns sink j.
-__device__ __forceinline__ void task_store(const warp_task &t, float4 hi, float4 lo, double *scratch,
+// two-float running sums of (ax, ay, az, pot) for the lane's two sinks
+struct sink_acc {
+    float4 hi[2], lo[2];
+};
+__device__ __forceinline__ void acc_zero(sink_acc &a)
+{
+    a.hi[0] = a.hi[1] = a.lo[0] = a.lo[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+}
+__device__ __forceinline__ void acc_load(sink_acc &a, const warp_task &t, const float4 *__restrict__ sacc,
+                                         const float4 *__restrict__ sacc_lo)
+{
+    acc_zero(a);
+    if (t.active && t.sub == 0) {
+        a.hi[0] = sacc[t.sa]; a.lo[0] = sacc_lo[t.sa];
+        if (t.has_b) { a.hi[1] = sacc[t.sb]; a.lo[1] = sacc_lo[t.sb]; }
+    }
+}
+// fold one tile's plain-fp32 sums (packed: lo half = sink a, hi half = sink b) into the running sums
+__device__ __forceinline__ void acc_fold(sink_acc &a, f2 ax, f2 ay, f2 az, f2 pot, bool want_pot)
+{
+    dsk_fold(a.hi[0].x, a.lo[0].x, f2_lo(ax)); dsk_fold(a.hi[1].x, a.lo[1].x, f2_hi(ax));
+    dsk_fold(a.hi[0].y, a.lo[0].y, f2_lo(ay)); dsk_fold(a.hi[1].y, a.lo[1].y, f2_hi(ay));
+    dsk_fold(a.hi[0].z, a.lo[0].z, f2_lo(az)); dsk_fold(a.hi[1].z, a.lo[1].z, f2_hi(az));
+    if (want_pot) { dsk_fold(a.hi[0].w, a.lo[0].w, f2_lo(pot)); dsk_fold(a.hi[1].w, a.lo[1].w, f2_hi(pot)); }
+}
+
+// Add the sub-groups' two-float accumulators (in double, through the warp's scratch: >= 32 x 8 doubles,
+// 16-byte aligned, free for reuse) and store; lane j < W of sub-group 0 owns sinks 2j, 2j+1.
+__device__ __forceinline__ void task_store(const warp_task &t, const sink_acc &a, double *scratch,
                                            float4 *__restrict__ sacc, float4 *__restrict__ sacc_lo)
 {
     const int lane = threadIdx.x & 31;
-    double d[4] = {(double)hi.x + (double)lo.x, (double)hi.y + (double)lo.y, (double)hi.z + (double)lo.z,
-                   (double)hi.w + (double)lo.w};
+    double d[8];
+#pragma unroll
+    for (int h = 0; h < 2; h++) {
+        d[4 * h + 0] = (double)a.hi[h].x + (double)a.lo[h].x; d[4 * h + 1] = (double)a.hi[h].y + (double)a.lo[h].y;
+        d[4 * h + 2] = (double)a.hi[h].z + (double)a.lo[h].z; d[4 * h + 3] = (double)a.hi[h].w + (double)a.lo[h].w;
+    }
     if (t.S > 1) {
         __syncwarp();
 #pragma unroll
-        for (int q = 0; q < 4; q++) scratch[q * 32 + lane] = t.active ? d[q] : 0.0;
+        for (int q = 0; q < 8; q++) scratch[q * 32 + lane] = t.active ? d[q] : 0.0;
         __syncwarp();
-        if (lane < (int)t.ns)
+        if (lane < t.W)
             for (int s = 1; s < t.S; s++)
 #pragma unroll
-                for (int q = 0; q < 4; q++) d[q] += scratch[q * 32 + lane + s * t.W];
+                for (int q = 0; q < 8; q++) d[q] += scratch[q * 32 + lane + s * t.W];
     }
-    if (lane < (int)t.ns) {
-        float4 oh, ol;
-        oh.x = (float)d[0]; oh.y = (float)d[1]; oh.z = (float)d[2]; oh.w = (float)d[3];
-        ol.x = (float)(d[0] - (double)oh.x); ol.y = (float)(d[1] - (double)oh.y); ol.z = (float)(d[2] - (double)oh.z);
-        ol.w = (float)(d[3] - (double)oh.w);
-        sacc[t.first + lane] = oh; sacc_lo[t.first + lane] = ol;
+    if (lane < t.W) {
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
+            if (h == 1 && !t.has_b) break;
+            float4 oh, ol;
+            oh.x = (float)d[4 * h]; oh.y = (float)d[4 * h + 1]; oh.z = (float)d[4 * h + 2]; oh.w = (float)d[4 * h + 3];
+            ol.x = (float)(d[4 * h] - (double)oh.x); ol.y = (float)(d[4 * h + 1] - (double)oh.y);
+            ol.z = (float)(d[4 * h + 2] - (double)oh.z); ol.w = (float)(d[4 * h + 3] - (double)oh.w);
+            const uint32_t r = h ? t.sb : t.sa;
+            sacc[r] = oh; sacc_lo[r] = ol;
+        }
     }
 }

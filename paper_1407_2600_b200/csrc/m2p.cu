@@ -111,21 +111,11 @@ int dsk_run_frows(dsk_ctx *c)
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
-// ---- F2 body: one sink against one cell (float) or a pair of cells (f2) ------------------------------
-// tile row (float2 = {cell A, cell B}): [0..2] com' xyz, [3] 1/s, [4] eps^2/s^2, [5] -1/s^2, [6+i] B_i
-#define M2P_HDR 6
-template <typename T> __device__ __forceinline__ void vld2(const float2 *p, int half, T &a, T &b);
-template <> __device__ __forceinline__ void vld2<f2>(const float2 *p, int, f2 &a, f2 &b)
-{
-    const ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(p);
-    a.v = v.x; b.v = v.y;
-}
-template <> __device__ __forceinline__ void vld2<float>(const float2 *p, int half, float &a, float &b)
-{
-    const float4 v = *reinterpret_cast<const float4 *>(p);
-    a = half ? v.y : v.x; b = half ? v.w : v.z;
-}
-
+// ---- F2 body: the lane's sink(s) against one cell ----------------------------------------------------
+// T = f2: two sinks in the halves of every register; T = float: one sink.  The cell's row is read from
+// shared memory as scalars (LDS.128 = four coefficients) that enter the packed ops as broadcast operands.
+// row (floats): [0..2] com' xyz (relative to the sink group's centre), [3] 1/s, [4] eps^2/s^2, [5] -1/s^2,
+//               [6] -1/s, [7] unused, [8+i] B_i
 __host__ __device__ constexpr int mi_comp(MI j, int i) { return i == 0 ? j.a : (i == 1 ? j.b : j.c); }
 __host__ __device__ constexpr int mi_lower(MI j, int i)
 {
@@ -143,15 +133,15 @@ __host__ __device__ constexpr int mi_pick(MI j)
 }
 
 template <int P, typename T, bool POT>
-__device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float2 *__restrict__ row, int half,
-                                         T &pot, T &ax, T &ay, T &az)
+__device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restrict__ row, T &pot, T &ax, T &ay, T &az)
 {
     constexpr int NP = dsk_np(P);
-    T cx, cy, cz, sinv, e2s, nsinv2;
-    vld2<T>(row + 0, half, cx, cy); vld2<T>(row + 2, half, cz, sinv); vld2<T>(row + 4, half, e2s, nsinv2);
+    const float4 hA = *reinterpret_cast<const float4 *>(row), hB = *reinterpret_cast<const float4 *>(row + 4);
+    const T sinv = vdup<T>(hA.w);
     T rho[3];
-    rho[0] = vmul(vsub(xs, cx), sinv); rho[1] = vmul(vsub(ys, cy), sinv); rho[2] = vmul(vsub(zs, cz), sinv);
-    T R2 = vfma(rho[0], rho[0], e2s);
+    rho[0] = vmul(vsub(xs, vdup<T>(hA.x)), sinv); rho[1] = vmul(vsub(ys, vdup<T>(hA.y)), sinv);
+    rho[2] = vmul(vsub(zs, vdup<T>(hA.z)), sinv);
+    T R2 = vfma(rho[0], rho[0], vdup<T>(hB.x));
     R2 = vfma(rho[1], rho[1], R2);
     R2 = vfma(rho[2], rho[2], R2);
     const T h0 = vrsqrt(R2);
@@ -168,8 +158,8 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float2 *__restr
     T mu[NP];                          // scaled monomials rho^j / j!  (mu[0] = 1 is never read)
     mu[1] = rho[0]; mu[2] = rho[1]; mu[3] = rho[2];
     T S[P + 1], G[P + 1][3];
-    const float2 *Bp = row + M2P_HDR;
-    T bc, bn;                          // coefficients arrive two at a time (one LDS.128)
+    const float *Bp = row + 8;
+    float4 bq;                         // coefficients arrive four at a time (one LDS.128)
     static_for<0, P + 1>([&](auto Q) {
         constexpr int q = decltype(Q)::value;
         constexpr int base = q * (q + 1) * (q + 2) / 6;
@@ -185,9 +175,8 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float2 *__restr
                 constexpr int off = fr_off(P, q, m);
                 static_for<0, fr_bsize(q)>([&](auto JJ) {
                     constexpr int jj = decltype(JJ)::value, ci = off + jj;
-                    T B;
-                    if constexpr (ci % 2 == 0) { vld2<T>(Bp + ci, half, bc, bn); B = bc; }
-                    else B = bn;
+                    if constexpr (ci % 4 == 0) bq = *reinterpret_cast<const float4 *>(Bp + ci);
+                    const T B = vdup<T>(ci % 4 == 0 ? bq.x : (ci % 4 == 1 ? bq.y : (ci % 4 == 2 ? bq.z : bq.w)));
                     if constexpr (q == 0) S[m] = B;
                     else if constexpr (q == fr_qfirst_S(P, m) && jj == 0) S[m] = vmul(B, mu[base + jj]);
                     else S[m] = vfma(B, mu[base + jj], S[m]);
@@ -222,28 +211,62 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float2 *__restr
         }
     });
     const T sinv2 = vmul(sinv, sinv);
-    const T u = vmul(vmul(qi, tt), nsinv2);
+    const T u = vmul(vmul(qi, tt), vdup<T>(hB.y));
     ax = vfma(g[0], sinv2, ax); ay = vfma(g[1], sinv2, ay); az = vfma(g[2], sinv2, az);
     ax = vfma(rho[0], u, ax); ay = vfma(rho[1], u, ay); az = vfma(rho[2], u, az);
-    if constexpr (POT) pot = vfma(phi, sinv, pot);        // caller subtracts
+    if constexpr (POT) pot = vfma(phi, vdup<T>(hB.z), pot);
 }
 
 // ---- F2 kernel ------------------------------------------------------------------------------------------
-// Per warp: a tile of up to NPAIR cell pairs in shared memory, PAIR-INTERLEAVED ({cell A, cell B} per float2) so
-// one broadcast LDS.128 feeds two packed f32x2 operands.  Staging: one lane per listed cell builds the header
-// (centre of mass relative to the sink group's cell centre, image shift absorbed exactly), then the lanes
-// copy the coefficient rows 16 bytes at a time (2 LDG.128 -> 2 STS.128 per pair and chunk).
+// Per warp: tiles of up to NCELL listed cells.  The force rows of a tile are brought into shared memory as they
+// are (one cp.async.bulk = TMA 1-D copy per cell, issued by the lane that holds the list entry, completion on a
+// per-buffer mbarrier); the NEXT tile's rows are in flight while the current tile is evaluated and the list
+// entries one tile further ahead sit in a register, so no global-memory latency is exposed between tiles.
+// When a tile has arrived, one lane per cell rewrites the row's 8-float header in place (centre of mass relative
+// to the sink group's cell centre, image shift absorbed exactly; 1/s, eps^2/s^2, -1/s^2, -1/s) and the sub-groups
+// run the body over alternate cells.
+// One task (warp) per block: tasks differ in length by more than 10x (list length, sub-group count), and a
+// multi-warp block holds its registers and shared memory until its longest warp ends.
+#define FW 1
 template <int P> struct m2p_cfg {
-    static constexpr int NPAIR = (P <= 6) ? 16 : 8;
+    static constexpr int NCELL = (P <= 4) ? 32 : (P == 6 ? 16 : 8);   // cells per tile
     static constexpr int FROW = fr_rowlen(P);
-    static constexpr int NCH = (FROW - 8) / 4;             // 16-byte chunks of coefficients per cell
-    static constexpr int TROW = M2P_HDR + (FROW - 8);      // float2 per pair row
-    static constexpr size_t WARP_BYTES = (size_t)NPAIR * TROW * sizeof(float2) + 32 * sizeof(uint32_t);
+    static constexpr uint32_t ROW_BYTES = FROW * sizeof(float);
+    static constexpr size_t BUF_BYTES = (size_t)NCELL * ROW_BYTES;
+    static constexpr size_t WARP_BYTES = 2 * BUF_BYTES + 16;           // two buffers + two mbarriers
     static constexpr bool PACKED = (P <= 6);
 };
 
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 template <int P, bool POT>
-__global__ void __launch_bounds__(FW * 32) k_m2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic,
+__global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic,
                                                  float box, float eps2, const float *__restrict__ frows,
                                                  const float4 *__restrict__ spos, const uint32_t *__restrict__ gfirst,
                                                  const uint32_t *__restrict__ gcount, const uint32_t *__restrict__ gcell,
@@ -252,80 +275,94 @@ __global__ void __launch_bounds__(FW * 32) k_m2p(uint32_t t0, uint32_t t1, const
                                                  float4 *__restrict__ sacc, float4 *__restrict__ sacc_lo)
 {
     using C = m2p_cfg<P>;
-    constexpr int NPAIR = C::NPAIR, FROW = C::FROW, NCH = C::NCH, TROW = C::TROW;
+    constexpr int NCELL = C::NCELL, FROW = C::FROW;
     constexpr bool PACKED = C::PACKED;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const warp_task t = make_task(t0, t1, taskmap, gfirst, gcount);
+    constexpr uint32_t CELL_MASK = (1u << DSK_CELL_BITS) - 1u;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const warp_task t = make_task(t0, t1, FW, taskmap, gfirst, gcount);
     if (!t.valid) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float2(*tile)[TROW] = reinterpret_cast<float2(*)[TROW]>(smem_raw + (size_t)warp * C::WARP_BYTES);
-    uint32_t *s_cell = reinterpret_cast<uint32_t *>(smem_raw + (size_t)warp * C::WARP_BYTES + (size_t)NPAIR * TROW * sizeof(float2));
+    unsigned char *wbase = smem_raw + (size_t)warp * C::WARP_BYTES;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(wbase + 2 * C::BUF_BYTES);
+    if (lane == 0) { mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); }
     const float *grow = frows + (size_t)gcell[t.g] * FROW;
     const float cgx = grow[0], cgy = grow[1], cgz = grow[2];
-    const float4 me = spos[t.first + t.j];
+    const float4 ma = spos[t.sa], mb = spos[t.sb];
     const uint32_t n = len[t.g];
     const uint32_t *lst = list + (off[t.g] - base);
-    using T = typename std::conditional<PACKED, f2, float>::type;
     // running sums as two-float (hi, lo) pairs, continued from the P2P kernel (sub-group 0 carries them);
     // each tile is summed from zero in plain fp32 and folded in with TwoSum, so no addition ever rounds at
     // the size of the total
-    float4 hi = make_float4(0.f, 0.f, 0.f, 0.f), lo = hi;
-    if (t.sub == 0 && lane < (int)t.ns) { hi = sacc[t.first + lane]; lo = sacc_lo[t.first + lane]; }
-    const T X = vdup<T>(me.x - cgx), Y = vdup<T>(me.y - cgy), Z = vdup<T>(me.z - cgz);
-    // pairs per tile: a multiple of the number of sub-groups, so that they finish together
-    const int tp = t.S >= NPAIR ? NPAIR : (NPAIR / t.S) * t.S;
-    const uint32_t tc = 2u * (uint32_t)tp;                  // cells per tile (<= 32: one list entry per lane)
-    for (uint32_t b0 = 0; b0 < n; b0 += tc) {
+    sink_acc A;
+    acc_load(A, t, sacc, sacc_lo);
+    const f2 X = f2_make(ma.x - cgx, mb.x - cgx), Y = f2_make(ma.y - cgy, mb.y - cgy), Z = f2_make(ma.z - cgz, mb.z - cgz);
+    // cells per tile: a multiple of the number of sub-groups, so that they finish together
+    const uint32_t tc = (uint32_t)(t.S >= NCELL ? NCELL : (NCELL / t.S) * t.S);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncwarp();
+
+    // issue the copies of one tile: lane l holds the list entry of cell l of the tile
+    auto fetch = [&](uint32_t e, int ncell, int b) {
+        fence_proxy_async();                                 // earlier generic reads of this buffer are done
+        if (lane == 0) mbar_expect_tx(&bar[b], (uint32_t)ncell * C::ROW_BYTES);
+        __syncwarp();
+        if (lane < ncell) bulk_g2s(reinterpret_cast<float *>(wbase + (size_t)b * C::BUF_BYTES) + (size_t)lane * FROW, frows + (size_t)(e & CELL_MASK) * FROW, C::ROW_BYTES, &bar[b]);
+    };
+    uint32_t e_cur = (lane < (int)tc && (uint32_t)lane < n) ? lst[lane] : 0u;
+    fetch(e_cur, (int)min(tc, n), 0);
+    uint32_t e_nxt = (lane < (int)tc && tc + lane < n) ? lst[tc + lane] : 0u;
+
+    uint32_t it = 0;
+    for (uint32_t b0 = 0; b0 < n; b0 += tc, it++) {
         const int ntc = (int)min(tc, n - b0);
-        const int npair = (ntc + 1) >> 1;
-        if (lane < 2 * npair) {
-            float cx = 4.0f * box, cy = cx, cz = cx, sinv = 1.0f / box;     // dummy cell: away from every sink, no mass
-            uint32_t cidx = 0xffffffffu;
-            if (lane < ntc) {
-                const uint32_t e = lst[b0 + lane];
-                cidx = e & ((1u << DSK_CELL_BITS) - 1u);
-                const float *r = frows + (size_t)cidx * FROW;
-                const float4 h0 = __ldg(reinterpret_cast<const float4 *>(r));
-                const float4 h1 = __ldg(reinterpret_cast<const float4 *>(r + 4));
-                float shx = 0.0f, shy = 0.0f, shz = 0.0f;
-                if (periodic) {
-                    const int img = (int)(e >> DSK_CELL_BITS), side = 2 * DSK_WS + 1;
-                    shz = (float)(img % side - DSK_WS) * box;
-                    shy = (float)((img / side) % side - DSK_WS) * box;
-                    shx = (float)(img / (side * side) - DSK_WS) * box;
-                }
-                cx = ((h0.x - cgx) + shx) + h1.x; cy = ((h0.y - cgy) + shy) + h1.y; cz = ((h0.z - cgz) + shz) + h1.z;
-                sinv = h0.w;
+        const int b = (int)(it & 1u);
+        float *rows = reinterpret_cast<float *>(wbase + (size_t)b * C::BUF_BYTES);
+        mbar_wait(&bar[b], (it >> 1) & 1u);
+        // ---- header in place ----
+        if (lane < ntc) {
+            float *r = rows + (size_t)lane * FROW;
+            const float4 h0 = *reinterpret_cast<const float4 *>(r);
+            const float4 h1 = *reinterpret_cast<const float4 *>(r + 4);
+            float shx = 0.0f, shy = 0.0f, shz = 0.0f;
+            if (periodic) {
+                const int img = (int)(e_cur >> DSK_CELL_BITS), side = 2 * DSK_WS + 1;
+                shz = (float)(img % side - DSK_WS) * box;
+                shy = (float)((img / side) % side - DSK_WS) * box;
+                shx = (float)(img / (side * side) - DSK_WS) * box;
             }
-            s_cell[lane] = cidx;
-            float *hd = reinterpret_cast<float *>(&tile[lane >> 1][0]) + (lane & 1);
-            hd[0] = cx; hd[2] = cy; hd[4] = cz; hd[6] = sinv; hd[8] = eps2 * sinv * sinv; hd[10] = -sinv * sinv;
+            const float sinv = h0.w;
+            *reinterpret_cast<float4 *>(r) = make_float4(((h0.x - cgx) + shx) + h1.x, ((h0.y - cgy) + shy) + h1.y,
+                                                         ((h0.z - cgz) + shz) + h1.z, sinv);
+            *reinterpret_cast<float4 *>(r + 4) = make_float4(eps2 * sinv * sinv, -sinv * sinv, -sinv, 0.0f);
         }
         __syncwarp();
-        for (int idx = lane; idx < npair * NCH; idx += 32) {
-            const int k = idx / NCH, ch = idx - k * NCH;
-            const uint32_t ca = s_cell[2 * k], cb = s_cell[2 * k + 1];
-            float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
-            if (ca != 0xffffffffu) a = __ldg(reinterpret_cast<const float4 *>(frows + (size_t)ca * FROW + 8) + ch);
-            if (cb != 0xffffffffu) b = __ldg(reinterpret_cast<const float4 *>(frows + (size_t)cb * FROW + 8) + ch);
-            float4 *dst = reinterpret_cast<float4 *>(&tile[k][M2P_HDR + 4 * ch]);
-            dst[0] = make_float4(a.x, b.x, a.y, b.y);
-            dst[1] = make_float4(a.z, b.z, a.w, b.w);
+        // ---- next tile on its way while this one is evaluated ----
+        e_cur = e_nxt;
+        if (b0 + tc < n) {
+            fetch(e_cur, (int)min(tc, n - b0 - tc), b ^ 1);
+            const uint32_t b2 = b0 + 2u * tc;
+            e_nxt = (lane < (int)tc && b2 + lane < n) ? lst[b2 + lane] : 0u;
         }
-        __syncwarp();
         if (t.active) {
-            T pot = vdup<T>(0.0f), ax = vdup<T>(0.0f), ay = vdup<T>(0.0f), az = vdup<T>(0.0f);
             if constexpr (PACKED) {
-                for (int k = t.sub; k < npair; k += t.S) m2p_body<P, T, POT>(X, Y, Z, tile[k], 0, pot, ax, ay, az);
+                f2 pot = f2_dup(0.0f), ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f);
+                for (int k = t.sub; k < ntc; k += t.S) m2p_body<P, f2, POT>(X, Y, Z, rows + (size_t)k * FROW, pot, ax, ay, az);
+                acc_fold(A, ax, ay, az, pot, POT);
             } else {
-                for (int k = t.sub; k < 2 * npair; k += t.S) m2p_body<P, T, POT>(X, Y, Z, tile[k >> 1], k & 1, pot, ax, ay, az);
+                // one sink at a time (p = 8 keeps 81 monomials live: no room for packed pairs)
+                static_for<0, 2>([&](auto H) {
+                    constexpr int h = decltype(H)::value;
+                    const float xs = h ? f2_hi(X) : f2_lo(X), ys = h ? f2_hi(Y) : f2_lo(Y), zs = h ? f2_hi(Z) : f2_lo(Z);
+                    float pot = 0.0f, ax = 0.0f, ay = 0.0f, az = 0.0f;
+                    for (int k = t.sub; k < ntc; k += t.S) m2p_body<P, float, POT>(xs, ys, zs, rows + (size_t)k * FROW, pot, ax, ay, az);
+                    dsk_fold(A.hi[h].x, A.lo[h].x, ax); dsk_fold(A.hi[h].y, A.lo[h].y, ay); dsk_fold(A.hi[h].z, A.lo[h].z, az);
+                    if (POT) dsk_fold(A.hi[h].w, A.lo[h].w, pot);
+                });
             }
-            dsk_fold(hi.x, lo.x, vsum(ax)); dsk_fold(hi.y, lo.y, vsum(ay)); dsk_fold(hi.z, lo.z, vsum(az));
-            if (POT) dsk_fold(hi.w, lo.w, -vsum(pot));
         }
         __syncwarp();
     }
-    task_store(t, hi, lo, reinterpret_cast<double *>(tile), sacc, sacc_lo);
+    task_store(t, A, reinterpret_cast<double *>(wbase), sacc, sacc_lo);
 }
 
 template <int P>

@@ -225,14 +225,14 @@ __global__ void __launch_bounds__(TB) k_group_bbox(const float4 *__restrict__ sp
             hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
         }
     if (lane == 0) {
-        ntask[g] = (e - f + 31u) >> 5;
+        ntask[g] = dsk_task_parts(e - f);
         gcount[g] = e - f;
         gbox[2 * (size_t)g] = make_float4(lo[0], lo[1], lo[2], 0.0f);
         gbox[2 * (size_t)g + 1] = make_float4(hi[0], hi[1], hi[2], 0.0f);
     }
 }
 
-// task -> (group, half) map for the warp-task force kernels
+// task -> (group, part) map for the warp-task force kernels
 __global__ void __launch_bounds__(TB) k_task_fill(const uint32_t *__restrict__ taskoff, uint32_t *__restrict__ task,
                                                   dsk_devstate *st)
 {
@@ -240,7 +240,7 @@ __global__ void __launch_bounds__(TB) k_task_fill(const uint32_t *__restrict__ t
     const uint32_t g = blockIdx.x * TB + threadIdx.x;
     if (g >= ng) return;
     const uint32_t a = taskoff[g], b = (g + 1 < ng) ? taskoff[g + 1] : st->ntask;
-    for (uint32_t k = a; k < b; k++) task[k] = (g << 1) | (k - a);
+    for (uint32_t k = a; k < b; k++) task[k] = (g << 2) | (k - a);
 }
 
 int dsk_run_build(dsk_ctx *c)
