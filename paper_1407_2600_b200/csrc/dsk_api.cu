@@ -53,6 +53,8 @@ static size_t carve(dsk_ctx *c, char *base)
     c->g_p2p_src = (uint32_t *)take(4 * ng);
     c->g_taskoff = (uint32_t *)take(4 * (ng + 1));
     c->g_task = (uint32_t *)take(16 * ng);
+    c->g_task_sorted = (uint32_t *)take(16 * ng);
+    c->task_hist = (uint32_t *)take(4 * 1024);
     c->g_m2p_off = (uint64_t *)take(8 * (ng + 1));
     c->g_p2p_off = (uint64_t *)take(8 * (ng + 1));
     // interaction lists: 256 / 32 entries per particle cover theta >= 0.3 in one batch on the paper-like

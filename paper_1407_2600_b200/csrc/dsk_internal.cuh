@@ -92,6 +92,8 @@ struct dsk_ctx {
     uint32_t *g_m2p_len, *g_p2p_len, *g_p2p_src;   // [ngroup_cap]
     uint32_t *g_taskoff;      // [ngroup_cap + 1] exclusive scan of dsk_task_parts(count)
     uint32_t *g_task;         // [4 * ngroup_cap] task -> group << 2 | part
+    uint32_t *g_task_sorted;  // [4 * ngroup_cap] the tasks of the current batch, longest first (m2p.cu)
+    uint32_t *task_hist;      // [1024] counting-sort bins
     uint64_t *g_m2p_off, *g_p2p_off;               // [ngroup_cap + 1] exclusive offsets into lists
     uint32_t *list_m2p, *list_p2p;
     size_t list_m2p_cap, list_p2p_cap;             // entries

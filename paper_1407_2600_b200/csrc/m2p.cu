@@ -219,9 +219,11 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
 
 // ---- F2 kernel ------------------------------------------------------------------------------------------
 // Per warp: tiles of up to NCELL listed cells.  The force rows of a tile are brought into shared memory as they
-// are (one cp.async.bulk = TMA 1-D copy per cell, issued by the lane that holds the list entry, completion on a
-// per-buffer mbarrier); the NEXT tile's rows are in flight while the current tile is evaluated and the list
-// entries one tile further ahead sit in a register, so no global-memory latency is exposed between tiles.
+// are, with cp.async (LDGSTS, 16 B): the lane that holds a cell's list entry copies that cell's row, so there is
+// no index arithmetic (LPC = 32 / NCELL lanes share a row when rows are long).  (A cp.async.bulk per row was
+// tried: UBLKCP takes uniform registers, so 32 different rows become a 32-trip serial loop, 18 % of all
+// instructions under ncu.)  The NEXT tile's rows are in flight while the current tile is evaluated and the
+// list entries one tile further ahead sit in a register, so no global-memory latency is exposed between tiles.
 // When a tile has arrived, one lane per cell rewrites the row's 8-float header in place (centre of mass relative
 // to the sink group's cell centre, image shift absorbed exactly; 1/s, eps^2/s^2, -1/s^2, -1/s) and the sub-groups
 // run the body over alternate cells.
@@ -230,40 +232,21 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
 #define FW 1
 template <int P> struct m2p_cfg {
     static constexpr int NCELL = (P <= 4) ? 32 : (P == 6 ? 16 : 8);   // cells per tile
+    static constexpr int LPC = 32 / NCELL;                             // lanes that share the copy of one row
     static constexpr int FROW = fr_rowlen(P);
-    static constexpr uint32_t ROW_BYTES = FROW * sizeof(float);
-    static constexpr size_t BUF_BYTES = (size_t)NCELL * ROW_BYTES;
-    static constexpr size_t WARP_BYTES = 2 * BUF_BYTES + 16;           // two buffers + two mbarriers
+    static constexpr int NCH = FROW / 4;                               // 16-byte chunks per row
+    static constexpr size_t BUF_BYTES = (size_t)NCELL * FROW * sizeof(float);
+    static constexpr size_t WARP_BYTES = 2 * BUF_BYTES;                // two buffers
     static constexpr bool PACKED = (P <= 6);
 };
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
 {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 template <int P, bool POT>
 __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic,
@@ -275,7 +258,7 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
                                                  float4 *__restrict__ sacc, float4 *__restrict__ sacc_lo)
 {
     using C = m2p_cfg<P>;
-    constexpr int NCELL = C::NCELL, FROW = C::FROW;
+    constexpr int NCELL = C::NCELL, LPC = C::LPC, FROW = C::FROW, NCH = C::NCH;
     constexpr bool PACKED = C::PACKED;
     constexpr uint32_t CELL_MASK = (1u << DSK_CELL_BITS) - 1u;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -283,8 +266,6 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
     if (!t.valid) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned char *wbase = smem_raw + (size_t)warp * C::WARP_BYTES;
-    uint64_t *bar = reinterpret_cast<uint64_t *>(wbase + 2 * C::BUF_BYTES);
-    if (lane == 0) { mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); }
     const float *grow = frows + (size_t)gcell[t.g] * FROW;
     const float cgx = grow[0], cgy = grow[1], cgz = grow[2];
     const float4 ma = spos[t.sa], mb = spos[t.sb];
@@ -298,29 +279,32 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
     const f2 X = f2_make(ma.x - cgx, mb.x - cgx), Y = f2_make(ma.y - cgy, mb.y - cgy), Z = f2_make(ma.z - cgz, mb.z - cgz);
     // cells per tile: a multiple of the number of sub-groups, so that they finish together
     const uint32_t tc = (uint32_t)(t.S >= NCELL ? NCELL : (NCELL / t.S) * t.S);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    __syncwarp();
+    const int mycell = lane / LPC, mypart = lane - mycell * LPC;     // the row (and share of it) this lane copies
 
-    // issue the copies of one tile: lane l holds the list entry of cell l of the tile
+    // issue the copies of one tile: entry e = list entry of cell `mycell` of the tile
     auto fetch = [&](uint32_t e, int ncell, int b) {
-        fence_proxy_async();                                 // earlier generic reads of this buffer are done
-        if (lane == 0) mbar_expect_tx(&bar[b], (uint32_t)ncell * C::ROW_BYTES);
-        __syncwarp();
-        if (lane < ncell) bulk_g2s(reinterpret_cast<float *>(wbase + (size_t)b * C::BUF_BYTES) + (size_t)lane * FROW, frows + (size_t)(e & CELL_MASK) * FROW, C::ROW_BYTES, &bar[b]);
+        if (mycell < ncell) {
+            const float4 *src = reinterpret_cast<const float4 *>(frows + (size_t)(e & CELL_MASK) * FROW);
+            float4 *dst = reinterpret_cast<float4 *>(wbase + (size_t)b * C::BUF_BYTES) + (size_t)mycell * NCH;
+#pragma unroll
+            for (int ch = mypart; ch < NCH; ch += LPC) cp_async16(dst + ch, src + ch);
+        }
+        cp_async_commit();
     };
-    uint32_t e_cur = (lane < (int)tc && (uint32_t)lane < n) ? lst[lane] : 0u;
+    uint32_t e_cur = (mycell < (int)tc && (uint32_t)mycell < n) ? lst[mycell] : 0u;
     fetch(e_cur, (int)min(tc, n), 0);
-    uint32_t e_nxt = (lane < (int)tc && tc + lane < n) ? lst[tc + lane] : 0u;
+    uint32_t e_nxt = (mycell < (int)tc && tc + mycell < n) ? lst[tc + mycell] : 0u;
 
     uint32_t it = 0;
     for (uint32_t b0 = 0; b0 < n; b0 += tc, it++) {
         const int ntc = (int)min(tc, n - b0);
         const int b = (int)(it & 1u);
         float *rows = reinterpret_cast<float *>(wbase + (size_t)b * C::BUF_BYTES);
-        mbar_wait(&bar[b], (it >> 1) & 1u);
+        cp_async_wait_all();
+        __syncwarp();
         // ---- header in place ----
-        if (lane < ntc) {
-            float *r = rows + (size_t)lane * FROW;
+        if (mycell < ntc && mypart == 0) {
+            float *r = rows + (size_t)mycell * FROW;
             const float4 h0 = *reinterpret_cast<const float4 *>(r);
             const float4 h1 = *reinterpret_cast<const float4 *>(r + 4);
             float shx = 0.0f, shy = 0.0f, shz = 0.0f;
@@ -341,7 +325,7 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
         if (b0 + tc < n) {
             fetch(e_cur, (int)min(tc, n - b0 - tc), b ^ 1);
             const uint32_t b2 = b0 + 2u * tc;
-            e_nxt = (lane < (int)tc && b2 + lane < n) ? lst[b2 + lane] : 0u;
+            e_nxt = (mycell < (int)tc && b2 + mycell < n) ? lst[b2 + mycell] : 0u;
         }
         if (t.active) {
             if constexpr (PACKED) {
@@ -365,6 +349,52 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
     task_store(t, A, reinterpret_cast<double *>(wbase), sacc, sacc_lo);
 }
 
+// ---- longest task first ----------------------------------------------------------------------------------
+// Task lengths differ by more than 10x (list length / sub-groups) and the longest run for milliseconds, so in
+// list order the kernel ends with a few SMs busy (ncu: SMs active 90 % of the elapsed cycles, 10.6 of 16 warp
+// slots occupied on average).  A one-pass counting sort by descending cost fixes the order; within a bin the
+// order is arbitrary, which cannot change any result (a task owns its sinks).
+#define TASK_BINS 1024
+__device__ __forceinline__ uint32_t task_cost_bin(uint32_t m, const uint32_t *__restrict__ gcount,
+                                                  const uint32_t *__restrict__ len)
+{
+    const uint32_t g = m >> 2, count = gcount[g], k = dsk_task_parts(count);
+    const uint32_t ns = (count + k - 1) / k, w = (ns + 1) >> 1, S = 32u / w;
+    const uint32_t cost = (len[g] + S - 1) / S;                      // body executions per lane
+    return TASK_BINS - 1u - min((uint32_t)TASK_BINS - 1u, cost >> 3);
+}
+__global__ void __launch_bounds__(256) k_task_hist(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap,
+                                                   const uint32_t *__restrict__ gcount, const uint32_t *__restrict__ len,
+                                                   uint32_t *__restrict__ hist)
+{
+    const uint32_t t = t0 + blockIdx.x * 256 + threadIdx.x;
+    if (t < t1) atomicAdd(&hist[task_cost_bin(taskmap[t], gcount, len)], 1u);
+}
+__global__ void __launch_bounds__(TASK_BINS) k_task_scan(uint32_t *__restrict__ hist)
+{
+    __shared__ uint32_t s[TASK_BINS];
+    const int i = threadIdx.x;
+    const uint32_t v = hist[i];
+    s[i] = v;
+    __syncthreads();
+    for (int o = 1; o < TASK_BINS; o <<= 1) {
+        const uint32_t y = i >= o ? s[i - o] : 0u;
+        __syncthreads();
+        s[i] += y;
+        __syncthreads();
+    }
+    hist[i] = s[i] - v;
+}
+__global__ void __launch_bounds__(256) k_task_scatter(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap,
+                                                      const uint32_t *__restrict__ gcount, const uint32_t *__restrict__ len,
+                                                      uint32_t *__restrict__ hist, uint32_t *__restrict__ sorted)
+{
+    const uint32_t t = t0 + blockIdx.x * 256 + threadIdx.x;
+    if (t >= t1) return;
+    const uint32_t m = taskmap[t];
+    sorted[t0 + atomicAdd(&hist[task_cost_bin(m, gcount, len)], 1u)] = m;
+}
+
 template <int P>
 static int launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int want_pot)
 {
@@ -374,16 +404,23 @@ static int launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int w
     if (!attr_done) {
         DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         attr_done = true;
     }
     const float e2 = c->eps * c->eps;
-    const unsigned grid = (t1 - t0 + FW - 1) / FW;
+    const unsigned grid = (t1 - t0 + FW - 1) / FW, nb = (t1 - t0 + 255) / 256;
+    DSK_CUDA(cudaMemsetAsync(c->task_hist, 0, sizeof(uint32_t) * TASK_BINS, c->stream));
+    k_task_hist<<<nb, 256, 0, c->stream>>>(t0, t1, c->g_task, c->gcount, c->g_m2p_len, c->task_hist);
+    k_task_scan<<<1, TASK_BINS, 0, c->stream>>>(c->task_hist);
+    k_task_scatter<<<nb, 256, 0, c->stream>>>(t0, t1, c->g_task, c->gcount, c->g_m2p_len, c->task_hist, c->g_task_sorted);
+    DSK_COUNT(c, 3);
     if (want_pot)
-        k_m2p<P, true><<<grid, FW * 32, smem, c->stream>>>(t0, t1, c->g_task, c->periodic, c->box, e2, c->frows, c->spos, c->gfirst,
+        k_m2p<P, true><<<grid, FW * 32, smem, c->stream>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->frows, c->spos, c->gfirst,
                                                            c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
                                                            c->g_m2p_len, c->sacc, c->sacc_lo);
     else
-        k_m2p<P, false><<<grid, FW * 32, smem, c->stream>>>(t0, t1, c->g_task, c->periodic, c->box, e2, c->frows, c->spos, c->gfirst,
+        k_m2p<P, false><<<grid, FW * 32, smem, c->stream>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->frows, c->spos, c->gfirst,
                                                             c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
                                                             c->g_m2p_len, c->sacc, c->sacc_lo);
     return DSK_OK;
