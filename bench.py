@@ -41,7 +41,7 @@ def workload():
 def config_dict(cfg, n_gpus):
     return {"workload": "BASELINE.json configs[1]: isolated Plummer sphere, a=0.01 cut 20a, equal masses",
             "N": cfg["N"], "eps": cfg["eps"], "theta": cfg["theta"], "p": cfg["p"], "periodic": False,
-            "step": "dsk_build_tree + dsk_accel (acc+pot)", "NLEAF": 16, "NCRIT": 64,
+            "step": "dsk_build_tree + dsk_accel (acc+pot)", "NLEAF": 64, "NCRIT": 64,
             "l2": "256 MiB buffer written between steps (outside the event pairs); working set ~1 GB > L2",
             "parallelism": f"replicas x{n_gpus}" if n_gpus > 1 else "single GPU"}
 

@@ -22,7 +22,7 @@ import numpy as np
 
 from . import build as _build
 
-NLEAF = 16
+NLEAF = 64
 NCRIT = 64
 WS = 2     # measured: WS = 1 floors the periodic force error at ~3e-3 on near-lattice inputs
 KEY_LEVELS = 21

@@ -15,6 +15,7 @@ LIB = os.path.join(HERE, "libdsk.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "-ftz=true", "-prec-div=true", "-prec-sqrt=true"]
+FLAGS += os.environ.get("DSK_EXTRA_NVCC_FLAGS", "").split()      # tuning sweeps only (e.g. -DDSK_NLEAF=32)
 
 
 def _stale(target, deps):

@@ -6,8 +6,12 @@
 #include "../../include/dsk.h"
 
 #define DSK_KEY_LEVELS 21
-#define DSK_NLEAF 16
-#define DSK_NCRIT 64
+#ifndef DSK_NLEAF
+#define DSK_NLEAF 64         // leaf bucket: a cell is split iff count > NLEAF (the oracle's NLEAF must match)
+#endif
+#ifndef DSK_NCRIT
+#define DSK_NCRIT 64         // sink group: first cell from the root with count <= NCRIT
+#endif
 #define DSK_WS 2              // image block half-width (WS = 1 floors the error at ~3e-3)
 #define DSK_FAR_ORDER 8
 #define DSK_NFAR 165          // C(8+3,3)
@@ -137,6 +141,7 @@ int dsk_run_walk(dsk_ctx *c);                                                 //
 int dsk_run_force(dsk_ctx *c, int want_pot);                                  // force.cu: F1 + orchestration
 int dsk_frow_len(int p);                                                      // m2p.cu
 int dsk_run_frows(dsk_ctx *c);                                                // m2p.cu: moment rows -> force rows
+int dsk_order_tasks(dsk_ctx *c, uint32_t t0, uint32_t t1, const uint32_t *len, int shift);   // m2p.cu
 int dsk_launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int want_pot);   // m2p.cu: F2
 int dsk_run_farfield(dsk_ctx *c);                                             // farfield.cu: F3
 void dsk_lattice_tensors(double L, int ws, double *T);                        // farfield.cu (host)

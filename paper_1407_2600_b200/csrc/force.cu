@@ -13,7 +13,7 @@
 #include "force_task.cuh"
 
 #define FW 4                 // warps (tasks) per block
-#define P2P_TILE 128         // sources per warp tile
+#define P2P_TILE 512         // sources per warp tile
 
 int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base);   // walk.cu
 
@@ -28,15 +28,10 @@ __global__ void __launch_bounds__(FW * 32, 6) k_p2p(uint32_t t0, uint32_t t1, co
                                                  const uint32_t *__restrict__ len, float4 *__restrict__ sacc,
                                                  float4 *__restrict__ sacc_lo)
 {
-    __shared__ uint32_t s_first_all[FW][32];
-    __shared__ uint32_t s_pref_all[FW][33];
-    __shared__ float s_sh_all[FW][32][3];
     __shared__ __align__(16) float4 src_all[FW][P2P_TILE];        // (x, y, z, m) relative to the group centre
     const warp_task t = make_task(t0, t1, FW, taskmap, gfirst, gcount);
     if (!t.valid) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    uint32_t *s_first = s_first_all[warp], *s_pref = s_pref_all[warp];
-    float(*s_sh)[3] = s_sh_all[warp];
     float4 *src = src_all[warp];
     const float *grow = rows + (size_t)gcell[t.g] * rowlen;
     const float cgx = grow[0], cgy = grow[1], cgz = grow[2];
@@ -47,61 +42,59 @@ __global__ void __launch_bounds__(FW * 32, 6) k_p2p(uint32_t t0, uint32_t t1, co
     const uint32_t *lst = list + (off[t.g] - base);
     sink_acc A;                                               // two-float running sums (see k_m2p)
     acc_zero(A);
+    // evaluate the nt staged sources against the lane's two sinks
+    auto eval_tile = [&](uint32_t nt) {
+        __syncwarp();
+        if (t.active) {
+            f2 ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f), pot = f2_dup(0.0f);
+#pragma unroll 4
+            for (int k = t.sub; k < (int)nt; k += t.S) {
+                const float4 s = src[k];
+                const f2 dx = f2_sub(f2_dup(s.x), X), dy = f2_sub(f2_dup(s.y), Y), dz = f2_sub(f2_dup(s.z), Z);
+                f2 r2 = f2_fma(dx, dx, E2);
+                r2 = f2_fma(dy, dy, r2);
+                r2 = f2_fma(dz, dz, r2);
+                const f2 ri = f2_rsqrt(r2);
+                const f2 ri2 = f2_mul(ri, ri), mri = f2_mul(f2_dup(s.w), ri), mri3 = f2_mul(mri, ri2);
+                ax = f2_fma(dx, mri3, ax); ay = f2_fma(dy, mri3, ay); az = f2_fma(dz, mri3, az);
+                if (POT) pot = f2_sub(pot, mri);
+            }
+            acc_fold(A, ax, ay, az, pot, POT);
+        }
+        __syncwarp();
+    };
+    // Staging: 32 listed leaves at a time, one per lane.  A leaf is a contiguous run of the sorted particle
+    // array; its lane copies it (shifted into the group's frame) to the run's place in the tile, which is the
+    // exclusive prefix sum of the run lengths.  Windows of P2P_TILE sources are evaluated in turn, a run that
+    // straddles two windows is copied in two parts.
     for (uint32_t b0 = 0; b0 < n; b0 += 32) {
-        // one leaf (segment of sources) per lane; exclusive scan of the segment lengths
-        uint32_t cnt = 0;
+        uint32_t my_first = 0, cnt = 0;
+        float shx = 0.0f, shy = 0.0f, shz = 0.0f;
         if (b0 + lane < n) {
             const uint32_t e = lst[b0 + lane];
             const dsk_cellrec r = cell[e & ((1u << DSK_CELL_BITS) - 1u)];
-            s_first[lane] = r.first; cnt = r.count;
-            float shx = 0.0f, shy = 0.0f, shz = 0.0f;
+            my_first = r.first; cnt = r.count;
             if (periodic) {
                 const int img = (int)(e >> DSK_CELL_BITS), side = 2 * DSK_WS + 1;
                 shz = (float)(img % side - DSK_WS) * box;
                 shy = (float)((img / side) % side - DSK_WS) * box;
                 shx = (float)(img / (side * side) - DSK_WS) * box;
             }
-            s_sh[lane][0] = shx; s_sh[lane][1] = shy; s_sh[lane][2] = shz;
         }
         uint32_t x = cnt;
         for (int o = 1; o < 32; o <<= 1) {
-            uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
             if (lane >= o) x += y;
         }
-        const uint32_t total = __shfl_sync(0xffffffffu, x, 31);
-        s_pref[lane] = x - cnt;
-        if (lane == 0) s_pref[32] = total;
-        __syncwarp();
-        for (uint32_t t0 = 0; t0 < total; t0 += P2P_TILE) {
-            const uint32_t nt = min((uint32_t)P2P_TILE, total - t0);
-            for (uint32_t j = lane; j < nt; j += 32) {
-                const uint32_t gj = t0 + j;
-                int a = 0, b = 32;                        // last segment with pref <= gj
-                while (b - a > 1) {
-                    const int mid = (a + b) >> 1;
-                    if (s_pref[mid] <= gj) a = mid; else b = mid;
-                }
-                const float4 p = spos[s_first[a] + (gj - s_pref[a])];
-                src[j] = make_float4((p.x - cgx) + s_sh[a][0], (p.y - cgy) + s_sh[a][1], (p.z - cgz) + s_sh[a][2], p.w);
+        const uint32_t total = __shfl_sync(0xffffffffu, x, 31), pref = x - cnt;
+        for (uint32_t lo = 0; lo < total; lo += P2P_TILE) {
+            const uint32_t hi = min(lo + (uint32_t)P2P_TILE, total);
+            const uint32_t i0 = max(pref, lo) - pref, i1 = min(pref + cnt, hi) > pref ? min(pref + cnt, hi) - pref : 0u;
+            for (uint32_t i = i0; i < i1; i++) {
+                const float4 p = spos[my_first + i];
+                src[pref + i - lo] = make_float4((p.x - cgx) + shx, (p.y - cgy) + shy, (p.z - cgz) + shz, p.w);
             }
-            __syncwarp();
-            if (t.active) {
-                f2 ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f), pot = f2_dup(0.0f);
-#pragma unroll 4
-                for (int k = t.sub; k < (int)nt; k += t.S) {
-                    const float4 s = src[k];
-                    const f2 dx = f2_sub(f2_dup(s.x), X), dy = f2_sub(f2_dup(s.y), Y), dz = f2_sub(f2_dup(s.z), Z);
-                    f2 r2 = f2_fma(dx, dx, E2);
-                    r2 = f2_fma(dy, dy, r2);
-                    r2 = f2_fma(dz, dz, r2);
-                    const f2 ri = f2_rsqrt(r2);
-                    const f2 ri2 = f2_mul(ri, ri), mri = f2_mul(f2_dup(s.w), ri), mri3 = f2_mul(mri, ri2);
-                    ax = f2_fma(dx, mri3, ax); ay = f2_fma(dy, mri3, ay); az = f2_fma(dz, mri3, az);
-                    if (POT) pot = f2_sub(pot, mri);
-                }
-                acc_fold(A, ax, ay, az, pot, POT);
-            }
-            __syncwarp();
+            eval_tile(hi - lo);
         }
     }
     // the sink's own leaf is always in the list: remove its self term -m_i/eps from the potential (once)
@@ -124,11 +117,15 @@ static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_
     cudaEventRecord(c->ev[8], s);
     const float e2 = c->eps * c->eps;
     const int rowlen = dsk_frow_len(c->p);
+    {
+        int e = dsk_order_tasks(c, t0, t1, c->g_p2p_src, 6);      // longest first (m2p.cu)
+        if (e) return e;
+    }
     if (want_pot)
-        k_p2p<true><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task, c->periodic, c->box, e2, rowlen, c->frows, c->cell, c->spos, c->gfirst,
+        k_p2p<true><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, rowlen, c->frows, c->cell, c->spos, c->gfirst,
                                            c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     else
-        k_p2p<false><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task, c->periodic, c->box, e2, rowlen, c->frows, c->cell, c->spos, c->gfirst,
+        k_p2p<false><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, rowlen, c->frows, c->cell, c->spos, c->gfirst,
                                             c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     cudaEventRecord(c->ev[9], s);
     {

@@ -356,19 +356,19 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
 // order is arbitrary, which cannot change any result (a task owns its sinks).
 #define TASK_BINS 1024
 __device__ __forceinline__ uint32_t task_cost_bin(uint32_t m, const uint32_t *__restrict__ gcount,
-                                                  const uint32_t *__restrict__ len)
+                                                  const uint32_t *__restrict__ len, int shift)
 {
     const uint32_t g = m >> 2, count = gcount[g], k = dsk_task_parts(count);
     const uint32_t ns = (count + k - 1) / k, w = (ns + 1) >> 1, S = 32u / w;
     const uint32_t cost = (len[g] + S - 1) / S;                      // body executions per lane
-    return TASK_BINS - 1u - min((uint32_t)TASK_BINS - 1u, cost >> 3);
+    return TASK_BINS - 1u - min((uint32_t)TASK_BINS - 1u, cost >> shift);
 }
 __global__ void __launch_bounds__(256) k_task_hist(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap,
                                                    const uint32_t *__restrict__ gcount, const uint32_t *__restrict__ len,
-                                                   uint32_t *__restrict__ hist)
+                                                   int shift, uint32_t *__restrict__ hist)
 {
     const uint32_t t = t0 + blockIdx.x * 256 + threadIdx.x;
-    if (t < t1) atomicAdd(&hist[task_cost_bin(taskmap[t], gcount, len)], 1u);
+    if (t < t1) atomicAdd(&hist[task_cost_bin(taskmap[t], gcount, len, shift)], 1u);
 }
 __global__ void __launch_bounds__(TASK_BINS) k_task_scan(uint32_t *__restrict__ hist)
 {
@@ -387,12 +387,24 @@ __global__ void __launch_bounds__(TASK_BINS) k_task_scan(uint32_t *__restrict__ 
 }
 __global__ void __launch_bounds__(256) k_task_scatter(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap,
                                                       const uint32_t *__restrict__ gcount, const uint32_t *__restrict__ len,
-                                                      uint32_t *__restrict__ hist, uint32_t *__restrict__ sorted)
+                                                      int shift, uint32_t *__restrict__ hist, uint32_t *__restrict__ sorted)
 {
     const uint32_t t = t0 + blockIdx.x * 256 + threadIdx.x;
     if (t >= t1) return;
     const uint32_t m = taskmap[t];
-    sorted[t0 + atomicAdd(&hist[task_cost_bin(m, gcount, len)], 1u)] = m;
+    sorted[t0 + atomicAdd(&hist[task_cost_bin(m, gcount, len, shift)], 1u)] = m;
+}
+
+// g_task_sorted[t0, t1) = the tasks of g_task[t0, t1) by descending (len[group] >> shift) / sub-groups
+int dsk_order_tasks(dsk_ctx *c, uint32_t t0, uint32_t t1, const uint32_t *len, int shift)
+{
+    const unsigned nb = (t1 - t0 + 255) / 256;
+    DSK_CUDA(cudaMemsetAsync(c->task_hist, 0, sizeof(uint32_t) * TASK_BINS, c->stream));
+    k_task_hist<<<nb, 256, 0, c->stream>>>(t0, t1, c->g_task, c->gcount, len, shift, c->task_hist);
+    k_task_scan<<<1, TASK_BINS, 0, c->stream>>>(c->task_hist);
+    k_task_scatter<<<nb, 256, 0, c->stream>>>(t0, t1, c->g_task, c->gcount, len, shift, c->task_hist, c->g_task_sorted);
+    DSK_COUNT(c, 3);
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
 template <int P>
@@ -409,12 +421,9 @@ static int launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int w
         attr_done = true;
     }
     const float e2 = c->eps * c->eps;
-    const unsigned grid = (t1 - t0 + FW - 1) / FW, nb = (t1 - t0 + 255) / 256;
-    DSK_CUDA(cudaMemsetAsync(c->task_hist, 0, sizeof(uint32_t) * TASK_BINS, c->stream));
-    k_task_hist<<<nb, 256, 0, c->stream>>>(t0, t1, c->g_task, c->gcount, c->g_m2p_len, c->task_hist);
-    k_task_scan<<<1, TASK_BINS, 0, c->stream>>>(c->task_hist);
-    k_task_scatter<<<nb, 256, 0, c->stream>>>(t0, t1, c->g_task, c->gcount, c->g_m2p_len, c->task_hist, c->g_task_sorted);
-    DSK_COUNT(c, 3);
+    const unsigned grid = (t1 - t0 + FW - 1) / FW;
+    int e = dsk_order_tasks(c, t0, t1, c->g_m2p_len, 3);
+    if (e) return e;
     if (want_pot)
         k_m2p<P, true><<<grid, FW * 32, smem, c->stream>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->frows, c->spos, c->gfirst,
                                                            c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
