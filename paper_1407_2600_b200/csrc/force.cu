@@ -12,44 +12,119 @@
 // F1: Plummer pair, acc_i += m_j d / (|d|^2+eps^2)^(3/2), pot_i -= m_j / sqrt(...), d = x_j - x_i.
 #include "force_task.cuh"
 
-#define FW 4                 // warps (tasks) per block
-#define P2P_TILE 512         // sources per warp tile
+#define FW 1                 // warps (tasks) per block: tasks differ in length, see m2p.cu
+#define P2P_TILE 256         // sources per window (two windows per warp)
 
 int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base);   // walk.cu
 
 // ---- F1 ----------------------------------------------------------------------------------------------
+// Sources are staged as they are stored: a listed leaf is a contiguous run of the sorted (x, y, z, m) array,
+// its lane copies it with cp.async (LDGSTS, 16 B per particle) to the run's place in the window, which is the
+// exclusive prefix sum of the run lengths of the 32 leaves handled at a time.  Windows of P2P_TILE sources are
+// double-buffered: the next window travels while the current one is evaluated, and the cell records of the
+// next 32 leaves are already in registers, so no global latency is exposed (ncu of the synchronous version:
+// 2.6 warps per issue waiting on a long scoreboard).  Differences are taken between raw coordinates (one
+// rounding of the exact difference); a periodic image shift is added to the staged copy of a run in place.
+__device__ __forceinline__ void cp_async16_p2p(void *smem_dst, const void *gmem_src)
+{
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+
+struct leaf_batch {              // one leaf per lane
+    uint32_t first, cnt, pref, total;
+    float shx, shy, shz;
+};
+
 template <bool POT>
-__global__ void __launch_bounds__(FW * 32, 6) k_p2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic, float box, float eps2,
-                                                 int rowlen, const float *__restrict__ rows,
+__global__ void __launch_bounds__(FW * 32, 12) k_p2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic, float box, float eps2,
                                                  const dsk_cellrec *__restrict__ cell, const float4 *__restrict__ spos,
                                                  const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
-                                                 const uint32_t *__restrict__ gcell, const uint32_t *__restrict__ list,
+                                                 const uint32_t *__restrict__ list,
                                                  const uint64_t *__restrict__ off, uint64_t base,
                                                  const uint32_t *__restrict__ len, float4 *__restrict__ sacc,
                                                  float4 *__restrict__ sacc_lo)
 {
-    __shared__ __align__(16) float4 src_all[FW][P2P_TILE];        // (x, y, z, m) relative to the group centre
+    __shared__ __align__(16) float4 src_all[FW][2][P2P_TILE];     // two windows of raw (x, y, z, m) per warp
     const warp_task t = make_task(t0, t1, FW, taskmap, gfirst, gcount);
     if (!t.valid) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float4 *src = src_all[warp];
-    const float *grow = rows + (size_t)gcell[t.g] * rowlen;
-    const float cgx = grow[0], cgy = grow[1], cgz = grow[2];
     const float4 ma = spos[t.sa], mb = spos[t.sb];
-    const f2 X = f2_make(ma.x - cgx, mb.x - cgx), Y = f2_make(ma.y - cgy, mb.y - cgy), Z = f2_make(ma.z - cgz, mb.z - cgz);
+    const f2 X = f2_make(ma.x, mb.x), Y = f2_make(ma.y, mb.y), Z = f2_make(ma.z, mb.z);
     const f2 E2 = f2_dup(eps2);
     const uint32_t n = len[t.g];
     const uint32_t *lst = list + (off[t.g] - base);
     sink_acc A;                                               // two-float running sums (see k_m2p)
     acc_zero(A);
-    // evaluate the nt staged sources against the lane's two sinks
-    auto eval_tile = [&](uint32_t nt) {
+
+    // cell records of the 32 leaves [b0, b0 + 32) of the list, their prefix sums and image shifts
+    auto load_batch = [&](uint32_t b0) {
+        leaf_batch L;
+        L.first = 0; L.cnt = 0; L.shx = L.shy = L.shz = 0.0f;
+        if (b0 + lane < n) {
+            const uint32_t e = lst[b0 + lane];
+            const dsk_cellrec r = cell[e & ((1u << DSK_CELL_BITS) - 1u)];
+            L.first = r.first; L.cnt = r.count;
+            if (periodic) {
+                const int img = (int)(e >> DSK_CELL_BITS), side = 2 * DSK_WS + 1;
+                L.shz = (float)(img % side - DSK_WS) * box;
+                L.shy = (float)((img / side) % side - DSK_WS) * box;
+                L.shx = (float)(img / (side * side) - DSK_WS) * box;
+            }
+        }
+        uint32_t x = L.cnt;
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        L.total = __shfl_sync(0xffffffffu, x, 31);
+        L.pref = x - L.cnt;
+        return L;
+    };
+    // my part of window [lo, lo + P2P_TILE) of batch L: particles [i0, i1) of my leaf
+    auto my_part = [&](const leaf_batch &L, uint32_t lo, uint32_t &i0, uint32_t &i1) {
+        const uint32_t hi = min(lo + (uint32_t)P2P_TILE, L.total), e = min(L.pref + L.cnt, hi);
+        i0 = max(L.pref, lo) - L.pref;
+        i1 = e > L.pref ? e - L.pref : 0u;
+    };
+    auto issue = [&](const leaf_batch &L, uint32_t lo, int b) {
+        uint32_t i0, i1;
+        my_part(L, lo, i0, i1);
+        float4 *dst = src_all[warp][b] + (L.pref - lo);
+        const float4 *sp = spos + L.first;
+        for (uint32_t i = i0; i < i1; i++) cp_async16_p2p(dst + i, sp + i);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    leaf_batch cur = load_batch(0), nxt = load_batch(32);
+    uint32_t bcur = 0, lo = 0;                    // current window: batch at list position bcur, offset lo
+    int buf = 0;
+    if (cur.total) issue(cur, 0, 0);
+    while (bcur < n) {
+        // the window after this one
+        const bool same = lo + (uint32_t)P2P_TILE < cur.total;
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncwarp();
-        if (t.active) {
+        float4 *src = src_all[warp][buf];
+        const uint32_t nt = min((uint32_t)P2P_TILE, cur.total - lo);
+        if (periodic && (cur.shx != 0.0f || cur.shy != 0.0f || cur.shz != 0.0f)) {
+            uint32_t i0, i1;
+            my_part(cur, lo, i0, i1);
+            for (uint32_t i = i0; i < i1; i++) {
+                float4 v = src[cur.pref - lo + i];
+                v.x += cur.shx; v.y += cur.shy; v.z += cur.shz;
+                src[cur.pref - lo + i] = v;
+            }
+        }
+        __syncwarp();
+        if (same) {
+            issue(cur, lo + P2P_TILE, buf ^ 1);
+        } else if (bcur + 32 < n) {
+            issue(nxt, 0, buf ^ 1);
+        }
+        if (t.active && cur.total) {
             f2 ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f), pot = f2_dup(0.0f);
-#pragma unroll 4
-            for (int k = t.sub; k < (int)nt; k += t.S) {
-                const float4 s = src[k];
+            auto pair = [&](const float4 s) {
                 const f2 dx = f2_sub(f2_dup(s.x), X), dy = f2_sub(f2_dup(s.y), Y), dz = f2_sub(f2_dup(s.z), Z);
                 f2 r2 = f2_fma(dx, dx, E2);
                 r2 = f2_fma(dy, dy, r2);
@@ -58,44 +133,27 @@ __global__ void __launch_bounds__(FW * 32, 6) k_p2p(uint32_t t0, uint32_t t1, co
                 const f2 ri2 = f2_mul(ri, ri), mri = f2_mul(f2_dup(s.w), ri), mri3 = f2_mul(mri, ri2);
                 ax = f2_fma(dx, mri3, ax); ay = f2_fma(dy, mri3, ay); az = f2_fma(dz, mri3, az);
                 if (POT) pot = f2_sub(pot, mri);
+            };
+            // my sub-group's sources: src[sub], src[sub + S], ...; pointer stepping keeps index arithmetic out of the loop
+            const float4 *q = src + t.sub;
+            const int S1 = t.S, S2 = 2 * t.S, S3 = 3 * t.S, S4 = 4 * t.S;
+            int left = ((int)nt - t.sub + t.S - 1) / t.S;
+            for (; left >= 4; left -= 4, q += S4) {
+                const float4 s0 = q[0], s1 = q[S1], s2 = q[S2], s3 = q[S3];
+                pair(s0); pair(s1); pair(s2); pair(s3);
             }
+            for (; left > 0; left--, q += S1) pair(q[0]);
             acc_fold(A, ax, ay, az, pot, POT);
         }
         __syncwarp();
-    };
-    // Staging: 32 listed leaves at a time, one per lane.  A leaf is a contiguous run of the sorted particle
-    // array; its lane copies it (shifted into the group's frame) to the run's place in the tile, which is the
-    // exclusive prefix sum of the run lengths.  Windows of P2P_TILE sources are evaluated in turn, a run that
-    // straddles two windows is copied in two parts.
-    for (uint32_t b0 = 0; b0 < n; b0 += 32) {
-        uint32_t my_first = 0, cnt = 0;
-        float shx = 0.0f, shy = 0.0f, shz = 0.0f;
-        if (b0 + lane < n) {
-            const uint32_t e = lst[b0 + lane];
-            const dsk_cellrec r = cell[e & ((1u << DSK_CELL_BITS) - 1u)];
-            my_first = r.first; cnt = r.count;
-            if (periodic) {
-                const int img = (int)(e >> DSK_CELL_BITS), side = 2 * DSK_WS + 1;
-                shz = (float)(img % side - DSK_WS) * box;
-                shy = (float)((img / side) % side - DSK_WS) * box;
-                shx = (float)(img / (side * side) - DSK_WS) * box;
-            }
+        if (same) {
+            lo += P2P_TILE;
+        } else {
+            bcur += 32; lo = 0;
+            cur = nxt;
+            nxt = load_batch(bcur + 32);
         }
-        uint32_t x = cnt;
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
-            if (lane >= o) x += y;
-        }
-        const uint32_t total = __shfl_sync(0xffffffffu, x, 31), pref = x - cnt;
-        for (uint32_t lo = 0; lo < total; lo += P2P_TILE) {
-            const uint32_t hi = min(lo + (uint32_t)P2P_TILE, total);
-            const uint32_t i0 = max(pref, lo) - pref, i1 = min(pref + cnt, hi) > pref ? min(pref + cnt, hi) - pref : 0u;
-            for (uint32_t i = i0; i < i1; i++) {
-                const float4 p = spos[my_first + i];
-                src[pref + i - lo] = make_float4((p.x - cgx) + shx, (p.y - cgy) + shy, (p.z - cgz) + shz, p.w);
-            }
-            eval_tile(hi - lo);
-        }
+        buf ^= 1;
     }
     // the sink's own leaf is always in the list: remove its self term -m_i/eps from the potential (once)
     if (POT && t.active && t.sub == 0) {
@@ -103,7 +161,7 @@ __global__ void __launch_bounds__(FW * 32, 6) k_p2p(uint32_t t0, uint32_t t1, co
         dsk_fold(A.hi[1].w, A.lo[1].w, mb.w * rsqrtf(eps2));
     }
     __syncwarp();
-    task_store(t, A, reinterpret_cast<double *>(src), sacc, sacc_lo);
+    task_store(t, A, reinterpret_cast<double *>(src_all[warp][0]), sacc, sacc_lo);
 }
 
 static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_t t1, uint64_t mb, uint64_t pb,
@@ -116,17 +174,16 @@ static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_
     }
     cudaEventRecord(c->ev[8], s);
     const float e2 = c->eps * c->eps;
-    const int rowlen = dsk_frow_len(c->p);
     {
         int e = dsk_order_tasks(c, t0, t1, c->g_p2p_src, 6);      // longest first (m2p.cu)
         if (e) return e;
     }
     if (want_pot)
-        k_p2p<true><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, rowlen, c->frows, c->cell, c->spos, c->gfirst,
-                                           c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
+        k_p2p<true><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->cell, c->spos, c->gfirst,
+                                           c->gcount, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     else
-        k_p2p<false><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, rowlen, c->frows, c->cell, c->spos, c->gfirst,
-                                            c->gcount, c->gcell, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
+        k_p2p<false><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->cell, c->spos, c->gfirst,
+                                            c->gcount, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     cudaEventRecord(c->ev[9], s);
     {
         int e = dsk_launch_m2p(c, t0, t1, mb, want_pot);
