@@ -38,6 +38,7 @@ static size_t carve(dsk_ctx *c, char *base)
     c->parent = (uint32_t *)take(4 * nc);
     c->nchild_tmp = (uint32_t *)take(4 * nc);
     c->whdr = (float4 *)take(16 * nc);
+    c->wmac = (float4 *)take(16 * nc);
     c->rows = (float *)take(4 * (size_t)dsk_rowlen(c->p_cap) * nc);
     c->frows = (float *)take(4 * (size_t)dsk_frow_len(c->p_cap) * nc);
     c->frtab_beg = (uint32_t *)take(4 * DSK_FRTAB_BEG);

@@ -85,6 +85,7 @@ struct dsk_ctx {
     uint32_t *parent;
     uint32_t *nchild_tmp;
     float4 *whdr;             // walk header per cell: com.xyz, delta
+    float4 *wmac;             // what the MAC reads: com.xyz, s/theta + delta (walk.cu, per theta)
     float *rows;              // [ncell_cap * rowlen(p_cap)] moment rows (upward.cu)
     float *frows;             // [ncell_cap * frow_len(p_cap)] force rows read by M2P (m2p.cu)
     uint32_t *frtab_beg;      // [DSK_FRTAB_BEG] moment row -> force row map of the current p

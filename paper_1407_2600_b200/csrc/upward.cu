@@ -11,11 +11,13 @@
 //   E_j = prod_i e_i^{j_i}/j_i!,  e = -(com_child - com_parent)/s_parent.
 // One warp per cell, lanes over the multi-indices n; one launch per level, deepest first.
 #include "dsk_internal.cuh"
+#include <type_traits>
 
 #define UW 4                     // warps (cells) per block
 #define UNP dsk_np(DSK_PMAX)     // 165
 
 __constant__ uint8_t c_ea[UNP], c_eb[UNP], c_ec[UNP], c_rank[UNP];
+__device__ uint8_t g_ea[UNP], g_eb[UNP], g_ec[UNP], g_rank[UNP];   // the same tables for per-lane (divergent) indexing
 __constant__ float c_sgn_invfact[UNP];   // (-1)^|n| / (a! b! c!)
 __constant__ float c_invfact1[DSK_PMAX + 1];
 
@@ -40,6 +42,10 @@ static int upload_tables()
     DSK_CUDA(cudaMemcpyToSymbol(c_eb, eb, sizeof(eb)));
     DSK_CUDA(cudaMemcpyToSymbol(c_ec, ec, sizeof(ec)));
     DSK_CUDA(cudaMemcpyToSymbol(c_rank, rk, sizeof(rk)));
+    DSK_CUDA(cudaMemcpyToSymbol(g_ea, ea, sizeof(ea)));
+    DSK_CUDA(cudaMemcpyToSymbol(g_eb, eb, sizeof(eb)));
+    DSK_CUDA(cudaMemcpyToSymbol(g_ec, ec, sizeof(ec)));
+    DSK_CUDA(cudaMemcpyToSymbol(g_rank, rk, sizeof(rk)));
     DSK_CUDA(cudaMemcpyToSymbol(c_sgn_invfact, sif, sizeof(sif)));
     DSK_CUDA(cudaMemcpyToSymbol(c_invfact1, if1, sizeof(if1)));
     g_tables_done = true;
@@ -72,6 +78,142 @@ __device__ __forceinline__ float warp_sum(float v)
     return v;
 }
 
+// scratch of one warp
+template <int P> struct up_smem {
+    float crow[8][dsk_np(P)];     // the children's moments, pre-scaled by 2^-|k|
+    float pw[8][3][12];           // per child: e_d^j / j!
+    float out[dsk_np(P)];         // the parent's moments being summed
+};
+
+// multi-index helpers for compile-time unrolled monomials (same scheme as the M2P body)
+struct UMI { int a, b, c; };
+__host__ __device__ constexpr UMI up_mi(int i)
+{
+    int l = 0;
+    while ((l + 1) * (l + 2) * (l + 3) / 6 <= i) l++;
+    int rem = i - l * (l + 1) * (l + 2) / 6, k = 0;
+    while ((k + 1) * (k + 2) / 2 <= rem) k++;
+    int c = rem - k * (k + 1) / 2;
+    return UMI{l - k, k - c, c};
+}
+template <int I, int N, typename F>
+__device__ __forceinline__ void up_static_for(F &&f)
+{
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        up_static_for<I + 1, N>(f);
+    }
+}
+
+// One warp computes one cell.  P2M: one particle per lane and round, all N_p monomials in registers, one
+// shuffle reduction per moment at the end.  M2M: the (child, moment) pairs are spread over the lanes.
+template <int P>
+__device__ __forceinline__ void upward_cell(uint32_t c, int level, float box, const dsk_cellrec *__restrict__ cell,
+                                            const uint64_t *__restrict__ hotkey, const float4 *__restrict__ spos,
+                                            float *__restrict__ rows, float4 *__restrict__ whdr, up_smem<P> &sm)
+{
+    constexpr int NP = dsk_np(P), ROW = dsk_rowlen(P);
+    const int lane = threadIdx.x & 31;
+    const dsk_cellrec r = cell[c];
+    const int nchild = r.meta & 255;
+    float s, ctr[3];
+    cell_centre(hotkey[c], level, box, s, ctr);
+    const float sinv = 1.0f / s;
+    float M, off[3];
+    float *row = rows + (size_t)c * ROW;
+    if (nchild == 0) {
+        // ---- P2M ----
+        float m = 0, sx = 0, sy = 0, sz = 0;
+        for (uint32_t j = r.first + lane; j < r.first + r.count; j += 32) {
+            const float4 q = spos[j];
+            m += q.w; sx += q.w * (q.x - ctr[0]); sy += q.w * (q.y - ctr[1]); sz += q.w * (q.z - ctr[2]);
+        }
+        M = warp_sum(m); sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
+        const float minv = M > 0.0f ? 1.0f / M : 0.0f;
+        off[0] = sx * minv; off[1] = sy * minv; off[2] = sz * minv;
+        float acc[NP];
+#pragma unroll
+        for (int n = 0; n < NP; n++) acc[n] = 0.0f;
+        for (uint32_t j = r.first + lane; j < r.first + r.count; j += 32) {
+            const float4 q = spos[j];
+            const float u0 = ((q.x - ctr[0]) - off[0]) * sinv, u1 = ((q.y - ctr[1]) - off[1]) * sinv,
+                        u2 = ((q.z - ctr[2]) - off[2]) * sinv;
+            float mu[NP];
+            mu[0] = q.w;
+            up_static_for<1, NP>([&](auto I) {
+                constexpr int i = decltype(I)::value;
+                constexpr UMI n = up_mi(i);
+                // multiply the lower monomial along the first non-zero axis
+                if constexpr (n.a > 0) mu[i] = mu[dsk_midx(n.a - 1, n.b, n.c)] * u0;
+                else if constexpr (n.b > 0) mu[i] = mu[dsk_midx(n.a, n.b - 1, n.c)] * u1;
+                else mu[i] = mu[dsk_midx(n.a, n.b, n.c - 1)] * u2;
+                acc[i] += mu[i];
+            });
+        }
+        up_static_for<1, NP>([&](auto I) {
+            constexpr int i = decltype(I)::value;
+            const float v = warp_sum(acc[i]);
+            if (lane == (i & 31)) row[8 + i] = v * c_sgn_invfact[i];
+        });
+        if (lane == 0) row[8] = M;
+    } else {
+        // ---- M2M ----
+        const float sc = 0.5f * s;              // child side
+        float m = 0, sx = 0, sy = 0, sz = 0, cx = 0, cy = 0, cz = 0;
+        if (lane < nchild) {
+            const uint32_t ch = r.child0 + lane;
+            const float *cr = rows + (size_t)ch * ROW;
+            const int o = (int)(hotkey[ch] & 7ull);
+            m = cr[8];
+            cx = ((o & 4) ? 0.5f : -0.5f) * sc + cr[4];        // child com - parent centre
+            cy = ((o & 2) ? 0.5f : -0.5f) * sc + cr[5];
+            cz = ((o & 1) ? 0.5f : -0.5f) * sc + cr[6];
+            sx = m * cx; sy = m * cy; sz = m * cz;
+        }
+        M = warp_sum(m); sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
+        const float minv = M > 0.0f ? 1.0f / M : 0.0f;
+        off[0] = sx * minv; off[1] = sy * minv; off[2] = sz * minv;
+        // powers of e = -(com_child - com_parent)/s_parent, divided by j!
+        if (lane < nchild) {
+            const float e[3] = {-(cx - off[0]) * sinv, -(cy - off[1]) * sinv, -(cz - off[2]) * sinv};
+#pragma unroll
+            for (int d = 0; d < 3; d++) {
+                float v = 1.0f;
+                for (int j = 0; j <= P; j++) { sm.pw[lane][d][j] = v * c_invfact1[j]; v *= e[d]; }
+            }
+        }
+        for (int i = lane; i < nchild * NP; i += 32) {
+            const int k = i / NP, n = i - k * NP;
+            sm.crow[k][n] = rows[(size_t)(r.child0 + k) * ROW + 8 + n] * exp2f(-(float)g_rank[n]);
+        }
+        for (int n = lane; n < NP; n += 32) sm.out[n] = 0.0f;
+        __syncwarp();
+        for (int i = lane; i < nchild * NP; i += 32) {
+            const int k = i / NP, n = i - k * NP;
+            const int a = g_ea[n], b = g_eb[n], cc = g_ec[n];
+            float sum = 0.0f;
+            for (int ka = 0; ka <= a; ka++)
+                for (int kb = 0; kb <= b; kb++) {
+                    const float pab = sm.pw[k][0][a - ka] * sm.pw[k][1][b - kb];
+                    for (int kc = 0; kc <= cc; kc++) sum += sm.crow[k][dsk_midx(ka, kb, kc)] * pab * sm.pw[k][2][cc - kc];
+                }
+            atomicAdd(&sm.out[n], sum);
+        }
+        __syncwarp();
+        for (int n = lane; n < NP; n += 32) row[8 + n] = (n == 0) ? M : sm.out[n];
+        __syncwarp();
+    }
+    // ---- header + walk header ----
+    if (lane == 0) {
+        const float delta = sqrtf(off[0] * off[0] + off[1] * off[1] + off[2] * off[2]);
+        row[0] = ctr[0]; row[1] = ctr[1]; row[2] = ctr[2]; row[3] = sinv;
+        row[4] = off[0]; row[5] = off[1]; row[6] = off[2]; row[7] = delta;
+        whdr[c] = make_float4(ctr[0] + off[0], ctr[1] + off[1], ctr[2] + off[2], delta);
+    }
+    for (int n = 8 + NP + lane; n < ROW; n += 32) row[n] = 0.0f;
+}
+
+// one level per launch (deep levels: many cells)
 template <int P>
 __global__ void __launch_bounds__(UW * 32) k_upward(uint32_t cbeg, uint32_t ncells, int level, float box,
                                                     const dsk_cellrec *__restrict__ cell,
@@ -79,128 +221,61 @@ __global__ void __launch_bounds__(UW * 32) k_upward(uint32_t cbeg, uint32_t ncel
                                                     const float4 *__restrict__ spos,
                                                     float *__restrict__ rows, float4 *__restrict__ whdr)
 {
-    constexpr int NP = dsk_np(P), ROW = dsk_rowlen(P), NSLOT = (NP + 31) / 32;
-    __shared__ float pw[UW][3][12];
-    __shared__ float crow[UW][NP];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __shared__ up_smem<P> sm[UW];
+    const int warp = threadIdx.x >> 5;
     const uint32_t ci = blockIdx.x * UW + warp;
     if (ci >= ncells) return;
-    const uint32_t c = cbeg + ci;
-    const dsk_cellrec r = cell[c];
-    const int nchild = r.meta & 255;
-    float s, ctr[3];
-    cell_centre(hotkey[c], level, box, s, ctr);
-    const float sinv = 1.0f / s;
-    float acc[NSLOT];
-#pragma unroll
-    for (int k = 0; k < NSLOT; k++) acc[k] = 0.0f;
-    float M, off[3];
-    if (nchild == 0) {
-        // ---- P2M ----
-        float m = 0, sx = 0, sy = 0, sz = 0;
-        for (uint32_t j = r.first + lane; j < r.first + r.count; j += 32) {
-            float4 q = spos[j];
-            m += q.w; sx += q.w * (q.x - ctr[0]); sy += q.w * (q.y - ctr[1]); sz += q.w * (q.z - ctr[2]);
-        }
-        M = warp_sum(m); sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
-        float minv = M > 0.0f ? 1.0f / M : 0.0f;
-        off[0] = sx * minv; off[1] = sy * minv; off[2] = sz * minv;
-        for (uint32_t j = r.first; j < r.first + r.count; j++) {
-            float4 q = spos[j];
-            if (lane < 27) {
-                int d = lane / 9, e = lane % 9;
-                float x = d == 0 ? q.x : (d == 1 ? q.y : q.z);
-                float u = ((x - ctr[d]) - off[d]) * sinv, v = 1.0f;
-                for (int t = 0; t < e; t++) v *= u;
-                pw[warp][d][e] = v;
-            }
-            __syncwarp();
-#pragma unroll
-            for (int k = 0; k < NSLOT; k++) {
-                int n = lane + 32 * k;
-                if (n < NP) acc[k] += q.w * pw[warp][0][c_ea[n]] * pw[warp][1][c_eb[n]] * pw[warp][2][c_ec[n]];
-            }
-            __syncwarp();
-        }
-#pragma unroll
-        for (int k = 0; k < NSLOT; k++) {
-            int n = lane + 32 * k;
-            if (n < NP) acc[k] *= c_sgn_invfact[n];
-        }
-    } else {
-        // ---- M2M ----
-        const float sc = 0.5f * s;              // child side
-        float m = 0, sx = 0, sy = 0, sz = 0;
-        if (lane < nchild) {
-            uint32_t ch = r.child0 + lane;
-            const float *cr = rows + (size_t)ch * ROW;
-            int o = (int)(hotkey[ch] & 7ull);
-            m = cr[8];
-            sx = m * (((o & 4) ? 0.5f : -0.5f) * sc + cr[4]);
-            sy = m * (((o & 2) ? 0.5f : -0.5f) * sc + cr[5]);
-            sz = m * (((o & 1) ? 0.5f : -0.5f) * sc + cr[6]);
-        }
-        M = warp_sum(m); sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
-        float minv = M > 0.0f ? 1.0f / M : 0.0f;
-        off[0] = sx * minv; off[1] = sy * minv; off[2] = sz * minv;
-        for (int k = 0; k < nchild; k++) {
-            uint32_t ch = r.child0 + k;
-            const float *cr = rows + (size_t)ch * ROW;
-            int o = (int)(hotkey[ch] & 7ull);
-            // child moments, pre-scaled by 2^-|k|
-            for (int n = lane; n < NP; n += 32) crow[warp][n] = cr[8 + n] * exp2f(-(float)c_rank[n]);
-            if (lane < 27) {
-                int d = lane / 9, e = lane % 9;
-                int bit = d == 0 ? 4 : (d == 1 ? 2 : 1);
-                float dd = ((o & bit) ? 0.5f : -0.5f) * sc + (cr[4 + d] - off[d]);   // com_child - com_parent
-                float u = -dd * sinv, v = 1.0f;
-                for (int t = 0; t < e; t++) v *= u;
-                pw[warp][d][e] = v * c_invfact1[e];
-            }
-            __syncwarp();
-#pragma unroll
-            for (int q = 0; q < NSLOT; q++) {
-                int n = lane + 32 * q;
-                if (n < NP) {
-                    int a = c_ea[n], b = c_eb[n], cc = c_ec[n];
-                    float sum = 0.0f;
-                    for (int ka = 0; ka <= a; ka++)
-                        for (int kb = 0; kb <= b; kb++)
-                            for (int kc = 0; kc <= cc; kc++)
-                                sum += crow[warp][dsk_midx(ka, kb, kc)] * pw[warp][0][a - ka] * pw[warp][1][b - kb] *
-                                       pw[warp][2][cc - kc];
-                    acc[q] += sum;
-                }
-            }
-            __syncwarp();
-        }
+    upward_cell<P>(cbeg + ci, level, box, cell, hotkey, spos, rows, whdr, sm[warp]);
+}
+
+// the top of the tree in ONE block: levels ltop-1 .. 0, a block barrier between levels (the levels near the
+// root hold a handful of cells each; a launch per level costs ~45 us of dependent latency apiece)
+#define UTOP_WARPS 8
+struct up_levels { uint32_t start[DSK_KEY_LEVELS + 3]; };
+template <int P>
+__global__ void __launch_bounds__(UTOP_WARPS * 32) k_upward_top(up_levels lv, int ltop, float box,
+                                                                const dsk_cellrec *__restrict__ cell,
+                                                                const uint64_t *__restrict__ hotkey,
+                                                                const float4 *__restrict__ spos,
+                                                                float *__restrict__ rows, float4 *__restrict__ whdr)
+{
+    extern __shared__ __align__(16) unsigned char up_raw[];
+    up_smem<P> *sm = reinterpret_cast<up_smem<P> *>(up_raw);
+    const int warp = threadIdx.x >> 5;
+    for (int l = ltop - 1; l >= 0; l--) {
+        for (uint32_t c = lv.start[l] + warp; c < lv.start[l + 1]; c += UTOP_WARPS)
+            upward_cell<P>(c, l, box, cell, hotkey, spos, rows, whdr, sm[warp]);
+        __threadfence_block();
+        __syncthreads();
     }
-    // ---- store row + walk header ----
-    float *row = rows + (size_t)c * ROW;
-    if (lane == 0) {
-        float delta = sqrtf(off[0] * off[0] + off[1] * off[1] + off[2] * off[2]);
-        row[0] = ctr[0]; row[1] = ctr[1]; row[2] = ctr[2]; row[3] = sinv;
-        row[4] = off[0]; row[5] = off[1]; row[6] = off[2]; row[7] = delta;
-        whdr[c] = make_float4(ctr[0] + off[0], ctr[1] + off[1], ctr[2] + off[2], delta);
-    }
-#pragma unroll
-    for (int k = 0; k < NSLOT; k++) {
-        int n = lane + 32 * k;
-        if (n < NP) row[8 + n] = (n == 0) ? M : acc[k];
-    }
-    for (int n = 8 + NP + lane; n < ROW; n += 32) row[n] = 0.0f;
 }
 
 template <int P>
-static void launch_upward(dsk_ctx *c, const uint32_t *lvl_start, int nlevel)
+static int launch_upward(dsk_ctx *c, const uint32_t *lvl_start, int nlevel)
 {
-    for (int l = nlevel - 1; l >= 0; l--) {
+    // levels [0, ltop) go to the single-block kernel: as many levels from the root as hold <= 96 cells together
+    int ltop = 0;
+    while (ltop < nlevel && lvl_start[ltop + 1] <= 96u) ltop++;
+    for (int l = nlevel - 1; l >= ltop; l--) {
         uint32_t beg = lvl_start[l], n = lvl_start[l + 1] - beg;
         if (!n) continue;
         k_upward<P><<<(n + UW - 1) / UW, UW * 32, 0, c->stream>>>(beg, n, l, c->box, c->cell, c->hotkey,
                                                                   c->spos, c->rows, c->whdr);
         DSK_COUNT(c, 1);
     }
+    if (ltop > 0) {
+        static bool attr_done = false;
+        const size_t smem = sizeof(up_smem<P>) * UTOP_WARPS;
+        if (!attr_done) {
+            DSK_CUDA(cudaFuncSetAttribute(k_upward_top<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr_done = true;
+        }
+        up_levels lv;
+        for (int i = 0; i < DSK_KEY_LEVELS + 3; i++) lv.start[i] = lvl_start[i];
+        k_upward_top<P><<<1, UTOP_WARPS * 32, smem, c->stream>>>(lv, ltop, c->box, c->cell, c->hotkey, c->spos, c->rows, c->whdr);
+        DSK_COUNT(c, 1);
+    }
+    return DSK_OK;
 }
 
 int dsk_run_upward(dsk_ctx *c)
@@ -211,12 +286,13 @@ int dsk_run_upward(dsk_ctx *c)
     int nl = (int)c->hstate->nlevel;
     cudaEventRecord(c->ev[5], c->stream);
     switch (c->p) {
-    case 2: launch_upward<2>(c, ls, nl); break;
-    case 4: launch_upward<4>(c, ls, nl); break;
-    case 6: launch_upward<6>(c, ls, nl); break;
-    case 8: launch_upward<8>(c, ls, nl); break;
+    case 2: e = launch_upward<2>(c, ls, nl); break;
+    case 4: e = launch_upward<4>(c, ls, nl); break;
+    case 6: e = launch_upward<6>(c, ls, nl); break;
+    case 8: e = launch_upward<8>(c, ls, nl); break;
     default: return DSK_EINVAL;
     }
+    if (e) return e;
     e = dsk_run_frows(c);                      // the fixed linear map to the rows M2P reads (m2p.cu)
     if (e) return e;
     cudaEventRecord(c->ev[6], c->stream);

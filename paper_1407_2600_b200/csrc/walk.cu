@@ -9,7 +9,7 @@
 // Run twice: COUNT (list lengths, for the offsets) and FILL.
 #include "dsk_internal.cuh"
 
-#define WW 4                 // warps per block
+#define WW 1                 // warps (groups) per block: walks differ in length, a block ends with its longest
 #define WSTACK 2048          // stack entries per warp
 
 __device__ __forceinline__ void image_shift(int img, int periodic, float box, float sh[3])
@@ -22,9 +22,8 @@ __device__ __forceinline__ void image_shift(int img, int periodic, float box, fl
 
 template <bool FILL>
 __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int periodic, float box,
-                                                  float inv_theta,
                                                   const dsk_cellrec *__restrict__ cell,
-                                                  const float4 *__restrict__ whdr,
+                                                  const float4 *__restrict__ wmac,
                                                   const float4 *__restrict__ gbox,
                                                   const uint32_t *__restrict__ gcount,
                                                   uint32_t *__restrict__ m2p_len, uint32_t *__restrict__ p2p_len,
@@ -60,8 +59,7 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
         if (act) {
             const uint32_t c = e & ((1u << DSK_CELL_BITS) - 1u);
             const int img = (int)(e >> DSK_CELL_BITS);
-            const dsk_cellrec r = cell[c];
-            const float4 h = whdr[c];
+            const float4 h = wmac[c];                      // com.xyz, critical radius s/theta + delta
             float sh[3];
             image_shift(img, periodic, box, sh);
             const float zx = h.x + sh[0], zy = h.y + sh[1], zz = h.z + sh[2];
@@ -69,12 +67,12 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
             const float dy = fmaxf(fmaxf(blo.y - zy, zy - bhi.y), 0.0f);
             const float dz = fmaxf(fmaxf(blo.z - zz, zz - bhi.z), 0.0f);
             const float d2 = dx * dx + dy * dy + dz * dz;
-            const int level = (int)(r.meta >> 8);
-            const float s = box * exp2f((float)-level);
-            const float rc = s * inv_theta + h.w;
-            accept = d2 > rc * rc;
-            nchild = r.meta & 255u; child0 = r.child0; cnt = r.count;
-            leaf = !accept && nchild == 0;
+            accept = d2 > h.w * h.w;
+            if (!accept) {                                 // only a rejected cell needs its record
+                const dsk_cellrec r = cell[c];
+                nchild = r.meta & 255u; child0 = r.child0; cnt = r.count;
+                leaf = nchild == 0;
+            }
         }
         const uint32_t bm = __ballot_sync(0xffffffffu, accept);
         const uint32_t bl = __ballot_sync(0xffffffffu, leaf);
@@ -119,34 +117,88 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
     }
 }
 
-// u32 lengths -> u64 exclusive offsets (single block per 64K-element strip, serial over strips: the
-// group count is small next to N, this is not a hot spot)
-__global__ void __launch_bounds__(1024) k_scan_u64(const uint32_t *__restrict__ len, uint32_t n,
-                                                   uint64_t *__restrict__ off)
+// u32 lengths -> u64 exclusive offsets, off[n] = total.  Two launches over a fixed grid: per-block sums, then
+// each block adds the sums of the blocks before it to the scan of its own contiguous chunk.
+#define S64_THREADS 256
+__global__ void __launch_bounds__(S64_THREADS) k_scan64_reduce(const uint32_t *__restrict__ len, uint32_t n,
+                                                              uint64_t *__restrict__ bsum)
 {
-    __shared__ uint64_t wsum[32];
-    __shared__ uint64_t carry_s;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0;
+    __shared__ uint64_t sh[S64_THREADS / 32];
+    const uint32_t chunk = ((n + gridDim.x - 1) / gridDim.x + S64_THREADS - 1) / S64_THREADS * S64_THREADS;
+    const uint64_t lo = (uint64_t)blockIdx.x * chunk, hi = min((uint64_t)n, lo + chunk);
+    uint64_t s = 0;
+    for (uint64_t i = lo + threadIdx.x; i < hi; i += S64_THREADS) s += len[i];
+    for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
     __syncthreads();
-    for (uint32_t i0 = 0; i0 < n; i0 += 1024) {
-        uint32_t i = i0 + threadIdx.x;
-        uint64_t v = i < n ? len[i] : 0, x = v;
+    if (threadIdx.x == 0) {
+        uint64_t t = 0;
+        for (int w = 0; w < S64_THREADS / 32; w++) t += sh[w];
+        bsum[blockIdx.x] = t;
+    }
+}
+__global__ void __launch_bounds__(S64_THREADS) k_scan64_apply(const uint32_t *__restrict__ len, uint32_t n,
+                                                             const uint64_t *__restrict__ bsum,
+                                                             uint64_t *__restrict__ off)
+{
+    __shared__ uint64_t wsum[S64_THREADS / 32];
+    __shared__ uint64_t s_pre, s_all;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (warp == 0) {
+        uint64_t pre = 0, all = 0;
+        for (uint32_t b = lane; b < gridDim.x; b += 32) {
+            const uint64_t v = bsum[b];
+            all += v;
+            if (b < blockIdx.x) pre += v;
+        }
+        for (int o = 16; o; o >>= 1) { pre += __shfl_xor_sync(0xffffffffu, pre, o); all += __shfl_xor_sync(0xffffffffu, all, o); }
+        if (lane == 0) { s_pre = pre; s_all = all; }
+    }
+    __syncthreads();
+    if (blockIdx.x == 0 && threadIdx.x == 0) off[n] = s_all;
+    const uint32_t chunk = ((n + gridDim.x - 1) / gridDim.x + S64_THREADS - 1) / S64_THREADS * S64_THREADS;
+    const uint64_t lo = (uint64_t)blockIdx.x * chunk, hi = min((uint64_t)n, lo + chunk);
+    uint64_t carry = s_pre;
+    for (uint64_t i0 = lo; i0 < hi; i0 += S64_THREADS) {
+        const uint64_t i = i0 + threadIdx.x;
+        const uint64_t v = i < hi ? len[i] : 0;
+        uint64_t x = v;
         for (int o = 1; o < 32; o <<= 1) {
-            uint64_t y = __shfl_up_sync(0xffffffffu, x, o);
+            const uint64_t y = __shfl_up_sync(0xffffffffu, x, o);
             if (lane >= o) x += y;
         }
         if (lane == 31) wsum[warp] = x;
         __syncthreads();
         uint64_t wpre = 0, tot = 0;
-        for (int w = 0; w < 32; w++) { uint64_t t = wsum[w]; if (w < warp) wpre += t; tot += t; }
-        uint64_t carry = carry_s;
-        if (i < n) off[i] = carry + wpre + x - v;
-        __syncthreads();
-        if (threadIdx.x == 0) carry_s = carry + tot;
+        for (int w = 0; w < S64_THREADS / 32; w++) { const uint64_t t = wsum[w]; if (w < warp) wpre += t; tot += t; }
+        if (i < hi) off[i] = carry + wpre + x - v;
+        carry += tot;
         __syncthreads();
     }
-    if (threadIdx.x == 0) off[n] = carry_s;
+}
+static void scan64(dsk_ctx *c, const uint32_t *len, uint32_t n, uint64_t *off)
+{
+    int grid = c->nsm * 2;
+    if ((uint64_t)grid * S64_THREADS > (uint64_t)n) grid = (int)((n + S64_THREADS - 1) / S64_THREADS);
+    if (grid < 1) grid = 1;
+    uint64_t *bsum = reinterpret_cast<uint64_t *>(c->scan_tmp);        // 4096 u32 = 2048 u64 >= grid
+    k_scan64_reduce<<<grid, S64_THREADS, 0, c->stream>>>(len, n, bsum);
+    k_scan64_apply<<<grid, S64_THREADS, 0, c->stream>>>(len, n, bsum, off);
+    DSK_COUNT(c, 2);
+}
+
+// the 16 bytes the MAC reads per tested cell: centre of mass and critical radius s/theta + delta
+__global__ void __launch_bounds__(256) k_walk_mac(uint32_t ncell, float box, float inv_theta,
+                                                  const dsk_cellrec *__restrict__ cell, const float4 *__restrict__ whdr,
+                                                  float4 *__restrict__ wmac)
+{
+    const uint32_t c = blockIdx.x * 256 + threadIdx.x;
+    if (c >= ncell) return;
+    float4 h = whdr[c];
+    const int level = (int)(cell[c].meta >> 8);
+    const float s = box * exp2f((float)-level);
+    h.w = s * inv_theta + h.w;
+    wmac[c] = h;
 }
 
 // W, COUNT pass + offsets.  The FILL pass is issued per batch by dsk_walk_fill (force.cu drives it).
@@ -156,21 +208,22 @@ int dsk_run_walk(dsk_ctx *c)
     cudaStream_t s = c->stream;
     const float inv_theta = 1.0f / c->theta;
     cudaEventRecord(c->ev[7], s);
-    k_walk<false><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic, c->box, inv_theta, c->cell, c->whdr,
+    const uint32_t nc = c->hstate->ncell;
+    k_walk_mac<<<(nc + 255) / 256, 256, 0, s>>>(nc, c->box, inv_theta, c->cell, c->whdr, c->wmac);
+    k_walk<false><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic, c->box, c->cell, c->wmac,
                                                          c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len,
                                                          c->g_p2p_src, nullptr, nullptr, 0, 0, nullptr, nullptr,
                                                          c->dstate);
-    k_scan_u64<<<1, 1024, 0, s>>>(c->g_m2p_len, ng, c->g_m2p_off);
-    k_scan_u64<<<1, 1024, 0, s>>>(c->g_p2p_len, ng, c->g_p2p_off);
-    DSK_COUNT(c, 3);
+    scan64(c, c->g_m2p_len, ng, c->g_m2p_off);
+    scan64(c, c->g_p2p_len, ng, c->g_p2p_off);
+    DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
 int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base)
 {
-    const float inv_theta = 1.0f / c->theta;
     k_walk<true><<<(g1 - g0 + WW - 1) / WW, WW * 32, 0, c->stream>>>(
-        g0, g1, c->periodic, c->box, inv_theta, c->cell, c->whdr, c->gbox, c->gcount, c->g_m2p_len,
+        g0, g1, c->periodic, c->box, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len,
         c->g_p2p_len, c->g_p2p_src, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p,
         c->dstate);
     DSK_COUNT(c, 1);
