@@ -230,13 +230,14 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
 // One task (warp) per block: tasks differ in length by more than 10x (list length, sub-group count), and a
 // multi-warp block holds its registers and shared memory until its longest warp ends.
 #define FW 1
-template <int P> struct m2p_cfg {
+template <int P, bool M64> struct m2p_cfg {
     static constexpr int NCELL = (P <= 4) ? 32 : (P == 6 ? 16 : 8);   // cells per tile
     static constexpr int LPC = 32 / NCELL;                             // lanes that share the copy of one row
     static constexpr int FROW = fr_rowlen(P);
     static constexpr int NCH = FROW / 4;                               // 16-byte chunks per row
     static constexpr size_t BUF_BYTES = (size_t)NCELL * FROW * sizeof(float);
-    static constexpr size_t WARP_BYTES = 2 * BUF_BYTES;                // two buffers
+    static constexpr size_t M64_BYTES = M64 ? (size_t)NCELL * 4 * sizeof(double) : 0;   // com' xyz and mass of a tile's cells
+    static constexpr size_t WARP_BYTES = 2 * BUF_BYTES + M64_BYTES;    // two row buffers + fp64 monopoles
     static constexpr bool PACKED = (P <= 6);
 };
 
@@ -248,7 +249,7 @@ __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-template <int P, bool POT>
+template <int P, bool POT, bool M64>
 __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic,
                                                  float box, float eps2, const float *__restrict__ frows,
                                                  const float4 *__restrict__ spos, const uint32_t *__restrict__ gfirst,
@@ -257,7 +258,7 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
                                                  uint64_t base, const uint32_t *__restrict__ len,
                                                  float4 *__restrict__ sacc, float4 *__restrict__ sacc_lo)
 {
-    using C = m2p_cfg<P>;
+    using C = m2p_cfg<P, M64>;
     constexpr int NCELL = C::NCELL, LPC = C::LPC, FROW = C::FROW, NCH = C::NCH;
     constexpr bool PACKED = C::PACKED;
     constexpr uint32_t CELL_MASK = (1u << DSK_CELL_BITS) - 1u;
@@ -266,6 +267,7 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
     if (!t.valid) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned char *wbase = smem_raw + (size_t)warp * C::WARP_BYTES;
+    double *mono = reinterpret_cast<double *>(wbase + 2 * C::BUF_BYTES);   // [NCELL][4], M64 only
     const float *grow = frows + (size_t)gcell[t.g] * FROW;
     const float cgx = grow[0], cgy = grow[1], cgz = grow[2];
     const float4 ma = spos[t.sa], mb = spos[t.sb];
@@ -318,6 +320,16 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
             *reinterpret_cast<float4 *>(r) = make_float4(((h0.x - cgx) + shx) + h1.x, ((h0.y - cgy) + shy) + h1.y,
                                                          ((h0.z - cgz) + shz) + h1.z, sinv);
             *reinterpret_cast<float4 *>(r + 4) = make_float4(eps2 * sinv * sinv, -sinv * sinv, -sinv, 0.0f);
+            if constexpr (M64) {
+                // the monopole of this cell is evaluated in fp64 below: centre of mass in double (the two
+                // differences are exact), mass out of the fp32 row
+                double *m4 = mono + 4 * mycell;
+                m4[0] = ((double)(h0.x - cgx) + (double)shx) + (double)h1.x;
+                m4[1] = ((double)(h0.y - cgy) + (double)shy) + (double)h1.y;
+                m4[2] = ((double)(h0.z - cgz) + (double)shz) + (double)h1.z;
+                m4[3] = (double)r[8];
+                r[8] = 0.0f;
+            }
         }
         __syncwarp();
         // ---- next tile on its way while this one is evaluated ----
@@ -326,6 +338,34 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
             fetch(e_cur, (int)min(tc, n - b0 - tc), b ^ 1);
             const uint32_t b2 = b0 + 2u * tc;
             e_nxt = (mycell < (int)tc && b2 + mycell < n) ? lst[b2 + mycell] : 0u;
+        }
+        if constexpr (M64) {
+            if (t.active) {
+                // Monopoles in fp64.  In a periodic, nearly uniform box the image block's monopole terms are
+                // O(M/L^2) each and cancel to a net force hundreds of times smaller, so their fp32 rounding
+                // (1e-7 of each term) alone exceeds the 1e-4 per-particle gate (measured on C3: p99.9 = 6e-4).
+                const double e2d = (double)eps2;
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const double xs = (double)(h ? mb.x : ma.x) - (double)cgx, ys = (double)(h ? mb.y : ma.y) - (double)cgy,
+                                 zs = (double)(h ? mb.z : ma.z) - (double)cgz;
+                    double sx = 0.0, sy = 0.0, sz = 0.0, sp = 0.0;
+                    for (int k = t.sub; k < ntc; k += t.S) {
+                        const double2 c01 = *reinterpret_cast<const double2 *>(mono + 4 * k);
+                        const double2 c23 = *reinterpret_cast<const double2 *>(mono + 4 * k + 2);
+                        const double dx = c01.x - xs, dy = c01.y - ys, dz = c23.x - zs;
+                        const double ri = rsqrt(fma(dx, dx, fma(dy, dy, fma(dz, dz, e2d))));
+                        const double mri = c23.y * ri, mri3 = mri * ri * ri;
+                        sx = fma(dx, mri3, sx); sy = fma(dy, mri3, sy); sz = fma(dz, mri3, sz);
+                        sp -= mri;
+                    }
+                    double v;
+                    v = ((double)A.hi[h].x + (double)A.lo[h].x) + sx; A.hi[h].x = (float)v; A.lo[h].x = (float)(v - (double)A.hi[h].x);
+                    v = ((double)A.hi[h].y + (double)A.lo[h].y) + sy; A.hi[h].y = (float)v; A.lo[h].y = (float)(v - (double)A.hi[h].y);
+                    v = ((double)A.hi[h].z + (double)A.lo[h].z) + sz; A.hi[h].z = (float)v; A.lo[h].z = (float)(v - (double)A.hi[h].z);
+                    if (POT) { v = ((double)A.hi[h].w + (double)A.lo[h].w) + sp; A.hi[h].w = (float)v; A.lo[h].w = (float)(v - (double)A.hi[h].w); }
+                }
+            }
         }
         if (t.active) {
             if constexpr (PACKED) {
@@ -407,32 +447,33 @@ int dsk_order_tasks(dsk_ctx *c, uint32_t t0, uint32_t t1, const uint32_t *len, i
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
-template <int P>
-static int launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int want_pot)
+template <int P, bool POT, bool M64>
+static int launch_m2p_v(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base)
 {
-    using C = m2p_cfg<P>;
+    using C = m2p_cfg<P, M64>;
     static bool attr_done = false;
     const size_t smem = FW * C::WARP_BYTES;
     if (!attr_done) {
-        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, POT, M64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, POT, M64>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         attr_done = true;
     }
     const float e2 = c->eps * c->eps;
     const unsigned grid = (t1 - t0 + FW - 1) / FW;
+    k_m2p<P, POT, M64><<<grid, FW * 32, smem, c->stream>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->frows, c->spos,
+                                                           c->gfirst, c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
+                                                           c->g_m2p_len, c->sacc, c->sacc_lo);
+    return DSK_OK;
+}
+
+template <int P>
+static int launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int want_pot)
+{
     int e = dsk_order_tasks(c, t0, t1, c->g_m2p_len, 3);
     if (e) return e;
-    if (want_pot)
-        k_m2p<P, true><<<grid, FW * 32, smem, c->stream>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->frows, c->spos, c->gfirst,
-                                                           c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
-                                                           c->g_m2p_len, c->sacc, c->sacc_lo);
-    else
-        k_m2p<P, false><<<grid, FW * 32, smem, c->stream>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->frows, c->spos, c->gfirst,
-                                                            c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
-                                                            c->g_m2p_len, c->sacc, c->sacc_lo);
-    return DSK_OK;
+    // periodic boxes: monopoles in fp64 (see the kernel)
+    if (c->periodic) return want_pot ? launch_m2p_v<P, true, true>(c, t0, t1, base) : launch_m2p_v<P, false, true>(c, t0, t1, base);
+    return want_pot ? launch_m2p_v<P, true, false>(c, t0, t1, base) : launch_m2p_v<P, false, false>(c, t0, t1, base);
 }
 
 int dsk_launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int want_pot)

@@ -316,3 +316,43 @@ def test_kdk_step(dsk, orc, periodic):
     assert dx.max() < 1e-6
     assert np.max(np.abs(tv.cpu().numpy() - v2)) < 5e-5 * np.abs(v2).max() + 1e-7
     d.close()
+
+
+# ---- full-size periodic configs, sampled (whole sink groups against the full oracle tree) ---------------
+def _group_sample(tree, order, nsink, seed):
+    g = tree.groups()
+    rng = np.random.default_rng(seed)
+    picked, tot = [], 0
+    for gi in rng.permutation(tree.ngroup):
+        picked.append(order[g["first"][gi]:g["first"][gi] + g["count"][gi]].astype(np.int64))
+        tot += int(g["count"][gi])
+        if tot >= nsink:
+            break
+    return np.concatenate(picked)
+
+
+@pytest.mark.parametrize("cfgid", [3, 4])
+def test_forces_periodic_full_sampled(dsk, orc, cfgid):
+    """configs[2] (128^3 perturbed lattice, p = 4) and configs[3] (256^3 clustered box, p = 6) at FULL size:
+    keys, order and cell count bit-exact; forces of ~512 sinks (whole groups) against the oracle tree.
+    The near-lattice case is the hard one for fp32: the net force is hundreds of times smaller than the
+    image block's partial sums (monopoles in fp64 when periodic)."""
+    cfg = workloads.CONFIGS[cfgid]
+    pos, mass = workloads.make(cfgid)
+    n = len(pos)
+    d = dsk.Dsk(n, 1.0, True, cfg["eps"], cfg["theta"], cfg["p"])
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    acc, _ = d.accel(tp, tm, want_pot=False)
+    tree = orc.OracleTree(pos, mass, 1.0, True)
+    sk, order = tree.sorted()
+    k, o = d.get_keys()
+    assert np.array_equal(k.cpu().numpy().view(np.uint64), sk)
+    assert np.array_equal(o.cpu().numpy().view(np.uint32), order)
+    assert d.get_tree()["ncell"] == tree.ncell
+    sink = _group_sample(tree, order, 512, 1)
+    ta = orc.tree_force(pos, mass, 1.0, True, cfg["eps"], cfg["theta"], cfg["p"], sink, tree=tree)[0]
+    a = acc.cpu().numpy().astype(np.float64)[sink]
+    rel = np.linalg.norm(a - ta, axis=1) / np.linalg.norm(ta, axis=1)
+    assert np.quantile(rel, 0.999) < 1e-4, (np.median(rel), np.quantile(rel, 0.999))
+    d.close()
