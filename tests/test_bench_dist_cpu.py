@@ -61,8 +61,8 @@ def test_accounting_matches_kernel_op_counts():
     if not (os.path.exists(cuobjdump) and os.path.exists(obj)):
         return
     sass = subprocess.run([cuobjdump, "-sass", obj], capture_output=True, text=True).stdout
-    for p in (2, 4, 6):                                     # the packed (f32x2) instantiations
-        fn = [b for b in sass.split("Function : ")[1:] if b.startswith(f"_Z5k_m2pILi{p}ELb1EE")]
+    for p in (2, 4, 6):                                     # the packed (f32x2) instantiations: <P, pot, fp32 monopoles>
+        fn = [b for b in sass.split("Function : ")[1:] if b.startswith(f"_Z5k_m2pILi{p}ELb1ELb0EE")]
         assert len(fn) == 1
         ffma, fmul, fadd = accounting.m2p_ops(p, pot=True)
         assert fn[0].count(" FFMA2 ") == ffma, (p, fn[0].count(" FFMA2 "), ffma)
