@@ -154,42 +154,65 @@ static int far_tables()
 }
 
 #define FM_THREADS 192
-#define FM_TILE 256
-// (a) block partials of the root moments about the box centre, fp64; thread = multi-index
-__global__ void __launch_bounds__(FM_THREADS) k_far_moments(const float4 *__restrict__ spos, uint32_t n,
-                                                            float half_box, double *__restrict__ partial)
+#define FM_WARPS 8
+template <int I, int N, typename F>
+__device__ __forceinline__ void sfor(F &&f)
 {
-    __shared__ double4 tile[FM_TILE];
-    const uint32_t chunk = ((n + gridDim.x - 1) / gridDim.x + FM_TILE - 1) / FM_TILE * FM_TILE;
-    const uint64_t lo = (uint64_t)blockIdx.x * chunk, hi = min((uint64_t)n, lo + chunk);
-    const int t = threadIdx.x;
-    const int a = t < NF ? f_ea[t] : 0, b = t < NF ? f_eb[t] : 0, c = t < NF ? f_ec[t] : 0;
-    double acc = 0.0;
-    for (uint64_t i0 = lo; i0 < hi; i0 += FM_TILE) {
-        for (int j = t; j < FM_TILE; j += FM_THREADS) {
-            double4 q = make_double4(0, 0, 0, 0);
-            if (i0 + j < hi) {
-                float4 p = spos[i0 + j];
-                q = make_double4((double)p.x - (double)half_box, (double)p.y - (double)half_box,
-                                 (double)p.z - (double)half_box, (double)p.w);
-            }
-            tile[j] = q;
-        }
-        __syncthreads();
-        if (t < NF) {
-            const int m = (int)min((uint64_t)FM_TILE, hi - i0);
-            for (int j = 0; j < m; j++) {
-                const double4 q = tile[j];
-                double v = q.w;
-                for (int e = 0; e < a; e++) v *= q.x;
-                for (int e = 0; e < b; e++) v *= q.y;
-                for (int e = 0; e < c; e++) v *= q.z;
-                acc += v;
-            }
-        }
-        __syncthreads();
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        sfor<I + 1, N>(f);
     }
-    if (t < NF) partial[(size_t)blockIdx.x * NF + t] = acc;
+}
+// (a) block partials of the root moments about the box centre, fp64.  One particle per lane: its 165 monomials
+// come from the power tables of x, y, z, each is summed over the warp with a butterfly and lane n % 32 keeps
+// the running sum of moment n (6 doubles per lane).  (The first version gave each of 165 threads one moment and
+// walked the particles serially: 3.9 ms at N = 2^21 against 0.17 ms for the evaluation.)
+__global__ void __launch_bounds__(FM_WARPS * 32) k_far_moments(const float4 *__restrict__ spos, uint32_t n,
+                                                               float half_box, double *__restrict__ partial)
+{
+    constexpr int NSLOT = (NF + 31) / 32;
+    __shared__ double red[FM_WARPS][NF];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double acc[NSLOT];
+#pragma unroll
+    for (int k = 0; k < NSLOT; k++) acc[k] = 0.0;
+    const uint32_t stride = gridDim.x * FM_WARPS * 32;
+    for (uint32_t i0 = (blockIdx.x * FM_WARPS + warp) * 32; i0 < n; i0 += stride) {   // whole warps stay together
+        const uint32_t i = i0 + lane;
+        double px[FO + 1], py[FO + 1], pz[FO + 1];
+        double m = 0.0, X = 0.0, Y = 0.0, Z = 0.0;
+        if (i < n) {
+            const float4 p = spos[i];
+            m = (double)p.w; X = (double)p.x - (double)half_box; Y = (double)p.y - (double)half_box; Z = (double)p.z - (double)half_box;
+        }
+        px[0] = m; py[0] = 1.0; pz[0] = 1.0;
+#pragma unroll
+        for (int e = 1; e <= FO; e++) { px[e] = px[e - 1] * X; py[e] = py[e - 1] * Y; pz[e] = pz[e - 1] * Z; }
+        sfor<0, FO + 1>([&](auto LL) {
+            constexpr int l = decltype(LL)::value;
+            sfor<0, l + 1>([&](auto KK) {
+                constexpr int k = decltype(KK)::value;          // k = b + c, a = l - k
+                sfor<0, k + 1>([&](auto CC) {
+                    constexpr int c = decltype(CC)::value, b = k - c, a = l - k;
+                    constexpr int idx = dsk_midx(a, b, c);
+                    double v = px[a] * (py[b] * pz[c]);
+#pragma unroll
+                    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                    if (lane == (idx & 31)) acc[idx >> 5] += v;
+                });
+            });
+        });
+    }
+#pragma unroll
+    for (int k = 0; k < NSLOT; k++)
+        if (k * 32 + lane < NF) red[warp][k * 32 + lane] = acc[k];
+    __syncthreads();
+    for (int t = threadIdx.x; t < NF; t += FM_WARPS * 32) {
+        double sum = 0.0;
+#pragma unroll
+        for (int w = 0; w < FM_WARPS; w++) sum += red[w][t];
+        partial[(size_t)blockIdx.x * NF + t] = sum;
+    }
 }
 
 // (b) reduce partials, then Lambda_n = sum_{|k| <= 8-|n|} (-1)^|k| C(n+k,k) M_k T_{n+k}
@@ -221,15 +244,6 @@ __global__ void __launch_bounds__(FM_THREADS) k_far_lambda(const double *__restr
             s += sg * binom[a + ka][ka] * binom[b + kb][kb] * binom[c + kc][kc] * sM[k] * T[dsk_midx(a + ka, b + kb, c + kc)];
         }
         lambda[t] = s;
-    }
-}
-
-template <int I, int N, typename F>
-__device__ __forceinline__ void sfor(F &&f)
-{
-    if constexpr (I < N) {
-        f(std::integral_constant<int, I>{});
-        sfor<I + 1, N>(f);
     }
 }
 
@@ -283,8 +297,8 @@ int dsk_run_farfield(dsk_ctx *c)
     if (e) return e;
     const uint32_t n = (uint32_t)c->N;
     int nblk = c->nsm * 2;
-    if ((int64_t)nblk * FM_TILE > c->N) nblk = (int)((c->N + FM_TILE - 1) / FM_TILE);
-    k_far_moments<<<nblk, FM_THREADS, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_partial);
+    if ((int64_t)nblk * FM_WARPS * 32 > c->N) nblk = (int)((c->N + FM_WARPS * 32 - 1) / (FM_WARPS * 32));
+    k_far_moments<<<nblk, FM_WARPS * 32, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_partial);
     k_far_lambda<<<1, FM_THREADS, 0, c->stream>>>(c->far_partial, nblk, c->far_T_dev, c->far_M, c->far_lambda);
     k_far_eval<<<(n + 127) / 128, 128, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_lambda, c->sacc, c->sacc_lo);
     DSK_COUNT(c, 3);
