@@ -31,6 +31,15 @@ UNIT = "particles/s"
 CFG = 2
 
 
+WORKLOADS = {
+    1: "BASELINE.json configs[0]: isolated uniform random box",
+    2: "BASELINE.json configs[1]: isolated Plummer sphere, a=0.01 cut 20a, equal masses",
+    3: "BASELINE.json configs[2]: periodic perturbed lattice 128^3, P(k)~k^-2, rms displacement 0.2 spacings",
+    4: "BASELINE.json configs[3]: periodic clustered box 256^3, 2000 Plummer halos + uniform background",
+    5: "BASELINE.json configs[4]: periodic clustered box 512^3 (force evaluation of the KDK run)",
+}
+
+
 def workload():
     from paper_1407_2600_b200 import workloads
     cfg = dict(workloads.CONFIGS[CFG])
@@ -39,8 +48,8 @@ def workload():
 
 
 def config_dict(cfg, n_gpus):
-    return {"workload": "BASELINE.json configs[1]: isolated Plummer sphere, a=0.01 cut 20a, equal masses",
-            "N": cfg["N"], "eps": cfg["eps"], "theta": cfg["theta"], "p": cfg["p"], "periodic": False,
+    return {"workload": WORKLOADS[CFG],
+            "N": cfg["N"], "eps": cfg["eps"], "theta": cfg["theta"], "p": cfg["p"], "periodic": bool(cfg["periodic"]),
             "step": "dsk_build_tree + dsk_accel (acc+pot)", "NLEAF": 64, "NCRIT": 64,
             "l2": "256 MiB buffer written between steps (outside the event pairs); working set ~1 GB > L2",
             "parallelism": f"replicas x{n_gpus}" if n_gpus > 1 else "single GPU"}
@@ -133,7 +142,10 @@ def oracle_rate(cfg, pos, mass, nsink, seconds_hint=None):
             break
     sink = np.concatenate(picked)
     t0 = time.perf_counter()
-    tree.accel(cfg["eps"], cfg["theta"], cfg["p"], sink, want_pot=True)
+    if cfg["periodic"]:
+        oracle.tree_force(pos, mass, cfg["box"], True, cfg["eps"], cfg["theta"], cfg["p"], sink, tree=tree)
+    else:
+        tree.accel(cfg["eps"], cfg["theta"], cfg["p"], sink, want_pot=True)
     t_force = time.perf_counter() - t0
     t_step = t_build + t_force * (n / len(sink))
     return n / t_step, dict(t_build_s=round(t_build, 3), t_force_sample_s=round(t_force, 3), nsink=int(len(sink)),
@@ -290,7 +302,7 @@ def run_ours(args):
                "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                "config": config_dict(cfg, world),
-               "roofline": {"bound": "alu", "kernel": "k_m2p<4,pot,packed>", "achieved": ach_m2p / 1e12,
+               "roofline": {"bound": "alu", "kernel": f"k_m2p<{cfg['p']},pot>", "achieved": ach_m2p / 1e12,
                             "peak": peak_fp32 / 1e12, "unit": "TFLOP/s", "frac": ach_m2p / peak_fp32,
                             "traffic": traffic,
                             "peak_source": f"nominal FP32: {prop.multi_processor_count} SMs x 128 lanes x 2 x {sm_max:.0f} MHz "
@@ -326,7 +338,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5],
+                    help="BASELINE.json config number (1-based); the default 2 is the workload the metric is quoted on")
     args = ap.parse_args()
+    global CFG
+    CFG = args.config
     if args.impl == "reference":
         run_reference(args)
     else:
