@@ -50,7 +50,7 @@ def workload():
 def config_dict(cfg, n_gpus):
     return {"workload": WORKLOADS[CFG],
             "N": cfg["N"], "eps": cfg["eps"], "theta": cfg["theta"], "p": cfg["p"], "periodic": bool(cfg["periodic"]),
-            "step": "dsk_build_tree + dsk_accel (acc+pot)", "NLEAF": 64, "NCRIT": 64,
+            "step": "dsk_build_tree + dsk_accel (acc+pot)", "NLEAF": 80, "NCRIT": 128,
             "l2": "256 MiB buffer written between steps (outside the event pairs); working set ~1 GB > L2",
             "parallelism": f"replicas x{n_gpus}" if n_gpus > 1 else "single GPU"}
 

@@ -22,8 +22,8 @@ import numpy as np
 
 from . import build as _build
 
-NLEAF = 64
-NCRIT = 64
+NLEAF = 80
+NCRIT = 128
 WS = 2     # measured: WS = 1 floors the periodic force error at ~3e-3 on near-lattice inputs
 KEY_LEVELS = 21
 FAR_ORDER = 8

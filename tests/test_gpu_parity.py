@@ -102,7 +102,7 @@ def test_adversarial_keys(dsk, orc):
         d.close()
 
 
-@pytest.mark.parametrize("n", [1, 2, 17, 64, 65])
+@pytest.mark.parametrize("n", [1, 2, 17, 64, 65, 80, 81, 128, 129])
 def test_tiny_inputs(dsk, orc, n):
     rng = np.random.default_rng(n)
     pos = rng.random((n, 3), dtype=np.float32); mass = rng.uniform(0.5, 1.5, n).astype(np.float32)

@@ -158,17 +158,18 @@ def test_tree_invariants(orc):
 
 
 def test_coincident_particles_level21(orc):
-    pos = np.tile(np.array([[0.3, 0.4, 0.5]], dtype=np.float32), (100, 1))
+    nco = 2 * orc.NCRIT + 36                   # coincident particles: one over-full level-21 leaf
+    pos = np.tile(np.array([[0.3, 0.4, 0.5]], dtype=np.float32), (nco, 1))
     pos = np.concatenate([pos, np.random.default_rng(0).random((50, 3), dtype=np.float32)])
-    t = orc.OracleTree(pos, np.ones(150, dtype=np.float32))
+    t = orc.OracleTree(pos, np.ones(nco + 50, dtype=np.float32))
     c = t.cells()
     deep = c["level"] == 21
-    assert deep.any() and c["count"][deep].max() == 100 and np.all(c["nchild"][deep] == 0)
+    assert deep.any() and c["count"][deep].max() == nco and np.all(c["nchild"][deep] == 0)
     g = t.groups()
-    assert g["count"].sum() == 150 and g["count"].max() <= orc.NCRIT
+    assert g["count"].sum() == nco + 50 and g["count"].max() <= orc.NCRIT
     # the over-full level-21 leaf is cut in chunks of NCRIT
-    big = g["cell"] == np.nonzero(deep & (c["count"] == 100))[0][0]
-    assert sorted(g["count"][big].tolist()) == [36, 64]
+    big = g["cell"] == np.nonzero(deep & (c["count"] == nco))[0][0]
+    assert sorted(g["count"][big].tolist()) == [36, orc.NCRIT, orc.NCRIT]
 
 
 def test_groups(orc):
