@@ -17,15 +17,16 @@ def m2p_ops(p, pot=True):
     ffma, fmul, fadd = 3, 3 + 1, 3          # R2 chain; rho = r * sinv, q = h0^2; r = x - com
     fmul += 3 * (p - 1)                     # rho_i / k, k = 2..p
     for q in range(p + 1):
-        if q >= 2:
-            fmul += len(_rank(q))           # monomials of degree q
+        if q >= 2 and not (q == p and p >= 3):
+            fmul += len(_rank(q))           # monomials of degree q (degree p is never read: its block uses Euler)
         for m in range(q, p + 1):
             if not _fr_has(p, q, m):
                 continue
             qfirst_s = 0 if (m == 1 or 2 * m - p < 0) else 2 * m - p
             qfirst_g = max(1, 2 * m - p)
+            eul = (q == m and m >= 3)           # top block: value from the gradient (Euler), m2p.cu
             for jj, j in enumerate(_rank(q)):
-                if q > 0:                   # S_m += B mu_j  (q = 0: plain assignment)
+                if q > 0 and not eul:       # S_m += B mu_j  (q = 0: plain assignment)
                     if q == qfirst_s and jj == 0:
                         fmul += 1
                     else:
@@ -33,10 +34,17 @@ def m2p_ops(p, pot=True):
                 if m >= 2 and q >= 2:       # G_m,i += B mu_{j - e_i}  (q = 1: plain assignment)
                     for i in range(3):
                         if j[i] >= 1:
-                            if q == qfirst_g and jj == i:
+                            if (q == qfirst_g or eul) and jj == i:
                                 fmul += 1
                             else:
                                 ffma += 1
+            if eul:
+                if qfirst_s == q:
+                    fmul += 1; ffma += 2    # S_m = (rho/q) . G
+                else:
+                    ffma += 3
+                if qfirst_g != q:
+                    fadd += 3               # merge with the lower blocks' gradient
     fmul += 1                               # phi = h0 S_0
     for m in range(1, p + 1):
         fmul += 2                           # h_m, w = h_m S_m

@@ -173,24 +173,44 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
             constexpr int m = decltype(M)::value;
             if constexpr (fr_has(P, q, m)) {
                 constexpr int off = fr_off(P, q, m);
+                // Top block of S_m (q = m, the homogeneous part of highest degree): by Euler's theorem
+                // sum_j B_j mu_j = (1/q) rho . grad, so only the gradient is accumulated (separately) and the
+                // value costs 3 FMAs instead of one per coefficient.
+                constexpr bool EUL = (q == m && m >= 3);
+                T Gt[3];
                 static_for<0, fr_bsize(q)>([&](auto JJ) {
                     constexpr int jj = decltype(JJ)::value, ci = off + jj;
                     if constexpr (ci % 4 == 0) bq = *reinterpret_cast<const float4 *>(Bp + ci);
                     const T B = vdup<T>(ci % 4 == 0 ? bq.x : (ci % 4 == 1 ? bq.y : (ci % 4 == 2 ? bq.z : bq.w)));
-                    if constexpr (q == 0) S[m] = B;
-                    else if constexpr (q == fr_qfirst_S(P, m) && jj == 0) S[m] = vmul(B, mu[base + jj]);
-                    else S[m] = vfma(B, mu[base + jj], S[m]);
+                    if constexpr (!EUL) {
+                        if constexpr (q == 0) S[m] = B;
+                        else if constexpr (q == fr_qfirst_S(P, m) && jj == 0) S[m] = vmul(B, mu[base + jj]);
+                        else S[m] = vfma(B, mu[base + jj], S[m]);
+                    }
                     if constexpr (m >= 2 && q >= 1)
                         static_for<0, 3>([&](auto I) {
                             constexpr int i = decltype(I)::value;
                             constexpr MI ji = dsk_mi(base + jj);
                             if constexpr (mi_comp(ji, i) >= 1) {
-                                if constexpr (q == 1) G[m][i] = B;
-                                else if constexpr (q == fr_qfirst_G(P, m) && jj == i) G[m][i] = vmul(B, mu[mi_lower(ji, i)]);
-                                else G[m][i] = vfma(B, mu[mi_lower(ji, i)], G[m][i]);
+                                if constexpr (EUL) {
+                                    if constexpr (jj == i) Gt[i] = vmul(B, mu[mi_lower(ji, i)]);
+                                    else Gt[i] = vfma(B, mu[mi_lower(ji, i)], Gt[i]);
+                                } else {
+                                    if constexpr (q == 1) G[m][i] = B;
+                                    else if constexpr (q == fr_qfirst_G(P, m) && jj == i) G[m][i] = vmul(B, mu[mi_lower(ji, i)]);
+                                    else G[m][i] = vfma(B, mu[mi_lower(ji, i)], G[m][i]);
+                                }
                             }
                         });
                 });
+                if constexpr (EUL) {
+                    if constexpr (fr_qfirst_S(P, m) == q) S[m] = vmul(rd[0][q], Gt[0]);
+                    else S[m] = vfma(rd[0][q], Gt[0], S[m]);
+                    S[m] = vfma(rd[1][q], Gt[1], S[m]);
+                    S[m] = vfma(rd[2][q], Gt[2], S[m]);
+                    if constexpr (fr_qfirst_G(P, m) == q) { G[m][0] = Gt[0]; G[m][1] = Gt[1]; G[m][2] = Gt[2]; }
+                    else { G[m][0] = vadd(G[m][0], Gt[0]); G[m][1] = vadd(G[m][1], Gt[1]); G[m][2] = vadd(G[m][2], Gt[2]); }
+                }
             }
         });
     });
