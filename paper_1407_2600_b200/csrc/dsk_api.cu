@@ -39,6 +39,7 @@ static size_t carve(dsk_ctx *c, char *base)
     c->cell = (dsk_cellrec *)take(16 * nc);
     c->parent = (uint32_t *)take(4 * nc);
     c->nchild_tmp = (uint32_t *)take(4 * nc);
+    c->cbounds = (uint32_t *)take(32 * nc);
     c->whdr = (float4 *)take(16 * nc);
     c->wmac = (float4 *)take(16 * nc);
     c->rows = (float *)take(4 * (size_t)dsk_rowlen(c->p_cap) * nc);

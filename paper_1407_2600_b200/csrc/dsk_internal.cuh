@@ -84,6 +84,7 @@ struct dsk_ctx {
     dsk_cellrec *cell;
     uint32_t *parent;
     uint32_t *nchild_tmp;
+    uint32_t *cbounds;        // [8 * ncell_cap] first rank of each octant of a cell being split (tree.cu)
     float4 *whdr;             // walk header per cell: com.xyz, delta
     float4 *wmac;             // what the MAC reads: com.xyz, s/theta + delta (walk.cu, per theta)
     float *rows;              // [ncell_cap * rowlen(p_cap)] moment rows (upward.cu)

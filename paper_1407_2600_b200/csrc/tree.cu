@@ -7,6 +7,8 @@
 // Level sizes stay on the device (dsk_devstate.lvl_start); kernels use a fixed grid and each block
 // takes a contiguous chunk of the level, which makes the child-offset scan a two-launch affair.
 #include "dsk_internal.cuh"
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
 
 #define TB 256
 
@@ -45,27 +47,44 @@ __device__ __forceinline__ void level_chunk(const dsk_devstate *st, int l, uint3
     hi = (uint32_t)min(a + chunk, (uint64_t)e);
 }
 
-__global__ void __launch_bounds__(TB) k_tree_count(int l, const uint64_t *__restrict__ key,
-                                                   const dsk_cellrec *__restrict__ cell,
-                                                   uint32_t *__restrict__ nchild_tmp,
-                                                   uint32_t *__restrict__ bsum, const dsk_devstate *st)
+// (the arrays written by one phase and read by the next inside the fused kernel carry no __restrict__/const:
+// they must not be read through the non-coherent path)
+__device__ __forceinline__ void tree_count_level(int l, const uint64_t *__restrict__ key, const dsk_cellrec *cell,
+                                                 uint32_t *nchild_tmp, uint32_t *cbounds, uint32_t *bsum,
+                                                 const dsk_devstate *st, uint32_t *sh)
 {
-    __shared__ uint32_t sh[TB / 32];
     uint32_t lo, hi;
     level_chunk(st, l, lo, hi);
     const int shift = 3 * (DSK_KEY_LEVELS - 1 - l);
     uint32_t s = 0;
-    for (uint32_t c = lo + threadIdx.x; c < hi; c += TB) {
-        uint32_t nc = 0;
-        dsk_cellrec r = cell[c];
-        if (r.count > DSK_NLEAF && l < DSK_KEY_LEVELS) {
-            uint32_t b[9];
-            octant_bounds(key, r.first, r.count, shift, b);
-#pragma unroll
-            for (int o = 0; o < 8; o++) nc += (b[o + 1] > b[o]);
+    // eight lanes per cell, lane o finds the first rank whose digit is >= o: the seven binary searches of a cell
+    // (20 dependent loads each near the root) run side by side instead of one after the other, and the
+    // bounds are kept for the emit phase
+    const int lane = threadIdx.x & 31, sub = lane & 7;
+    for (uint32_t c0 = lo + (threadIdx.x >> 5) * 4; c0 < hi; c0 += TB / 8) {
+        const uint32_t c = c0 + (lane >> 3);
+        const bool valid = c < hi;
+        dsk_cellrec r;
+        r.first = 0; r.count = 0; r.child0 = 0; r.meta = 0;
+        if (valid) r = cell[c];
+        const bool split = valid && r.count > DSK_NLEAF && l < DSK_KEY_LEVELS;
+        uint32_t b = r.first;
+        if (split && sub > 0) {
+            uint32_t a = r.first, e = r.first + r.count;
+            while (a < e) {
+                const uint32_t mid = a + ((e - a) >> 1);
+                if (((key[mid] >> shift) & 7ull) < (uint64_t)sub) a = mid + 1; else e = mid;
+            }
+            b = a;
         }
-        nchild_tmp[c] = nc;
-        s += nc;
+        uint32_t nb = __shfl_down_sync(0xffffffffu, b, 1, 8);
+        if (sub == 7) nb = r.first + r.count;
+        const uint32_t bal = __ballot_sync(0xffffffffu, split && nb > b);
+        const uint32_t nc = __popc((bal >> (lane & 24)) & 0xffu);
+        if (valid) {
+            cbounds[(size_t)c * 8 + sub] = b;
+            if (sub == 0) { nchild_tmp[c] = nc; s += nc; }
+        }
     }
     for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
@@ -77,15 +96,12 @@ __global__ void __launch_bounds__(TB) k_tree_count(int l, const uint64_t *__rest
     }
 }
 
-__global__ void __launch_bounds__(TB) k_tree_emit(int l, const uint64_t *__restrict__ key,
-                                                  dsk_cellrec *cell, uint64_t *hotkey, uint32_t *parent,
-                                                  const uint32_t *__restrict__ nchild_tmp,
-                                                  const uint32_t *__restrict__ bsum, uint32_t ncell_cap,
-                                                  dsk_devstate *st)
+__device__ __forceinline__ void tree_emit_level(int l, const uint64_t *__restrict__ key,
+                                                dsk_cellrec *cell, uint64_t *hotkey, uint32_t *parent,
+                                                const uint32_t *nchild_tmp, const uint32_t *cbounds, const uint32_t *bsum,
+                                                uint32_t ncell_cap, dsk_devstate *st, uint32_t *sh, uint32_t *wsum, uint32_t &s_pre,
+                                                uint32_t &s_all)
 {
-    __shared__ uint32_t sh[TB / 32];
-    __shared__ uint32_t wsum[TB / 32];
-    __shared__ uint32_t s_pre, s_all;
     // offset of this block's chunk = sum of the sums of the blocks before it
     uint32_t pre = 0, all = 0;
     for (uint32_t b = threadIdx.x; b < gridDim.x; b += TB) {
@@ -140,7 +156,9 @@ __global__ void __launch_bounds__(TB) k_tree_emit(int l, const uint64_t *__restr
                 r.child0 = ch; r.meta = v | ((uint32_t)l << 8);
                 cell[c] = r;
                 uint32_t b[9];
-                octant_bounds(key, r.first, r.count, shift, b);
+#pragma unroll
+                for (int o = 0; o < 8; o++) b[o] = cbounds[(size_t)c * 8 + o];
+                b[8] = r.first + r.count;
                 uint64_t hk = hotkey[c];
 #pragma unroll
                 for (int o = 0; o < 8; o++)
@@ -156,6 +174,27 @@ __global__ void __launch_bounds__(TB) k_tree_emit(int l, const uint64_t *__restr
         }
         carry += tot;
         __syncthreads();
+    }
+}
+
+// T in ONE cooperative launch: all levels, a grid barrier between the count and emit phases of a level and
+// between levels; the loop ends at the first level that produces no children.  (One launch pair per level
+// cost 44 launches of ~15-25 us each, most of them on empty levels.)
+__global__ void __launch_bounds__(TB) k_tree_build(const uint64_t *__restrict__ key, dsk_cellrec *cell,
+                                                   uint64_t *hotkey, uint32_t *parent, uint32_t *nchild_tmp,
+                                                   uint32_t *cbounds, uint32_t *bsum, uint32_t ncell_cap, dsk_devstate *st)
+{
+    __shared__ uint32_t sh[TB / 32];
+    __shared__ uint32_t wsum[TB / 32];
+    __shared__ uint32_t s_pre, s_all;
+    cg::grid_group grid = cg::this_grid();
+    for (int l = 0; l <= DSK_KEY_LEVELS; l++) {
+        tree_count_level(l, key, cell, nchild_tmp, cbounds, bsum, st, sh);
+        grid.sync();
+        tree_emit_level(l, key, cell, hotkey, parent, nchild_tmp, cbounds, bsum, ncell_cap, st, sh, wsum, s_pre, s_all);
+        grid.sync();
+        const volatile dsk_devstate *vs = st;
+        if (vs->lvl_start[l + 2] == vs->lvl_start[l + 1]) break;      // no cells at level l + 1
     }
 }
 
@@ -249,10 +288,12 @@ int dsk_run_build(dsk_ctx *c)
     cudaStream_t s = c->stream;
     int grid = c->nsm * 4;
     k_tree_init<<<1, 1, 0, s>>>(c->cell, c->hotkey, c->parent, n, c->dstate);
-    for (int l = 0; l <= DSK_KEY_LEVELS; l++) {
-        k_tree_count<<<grid, TB, 0, s>>>(l, c->key_a, c->cell, c->nchild_tmp, c->scan_tmp, c->dstate);
-        k_tree_emit<<<grid, TB, 0, s>>>(l, c->key_a, c->cell, c->hotkey, c->parent, c->nchild_tmp,
-                                        c->scan_tmp, (uint32_t)c->ncell_cap, c->dstate);
+    {
+        const uint64_t *key = c->key_a;
+        uint32_t cap = (uint32_t)c->ncell_cap;
+        void *args[] = {(void *)&key, (void *)&c->cell, (void *)&c->hotkey, (void *)&c->parent, (void *)&c->nchild_tmp,
+                        (void *)&c->cbounds, (void *)&c->scan_tmp, (void *)&cap, (void *)&c->dstate};
+        DSK_CUDA(cudaLaunchCooperativeKernel((const void *)k_tree_build, dim3(grid), dim3(TB), args, 0, s));
     }
     cudaEventRecord(c->ev[3], s);
     // groups
@@ -268,6 +309,6 @@ int dsk_run_build(dsk_ctx *c)
     dsk_exclusive_scan_u32(c, c->g_taskoff, c->g_taskoff, &c->dstate->ngroup, (uint32_t)c->ngroup_cap, &c->dstate->ntask);
     k_task_fill<<<(unsigned)((c->ngroup_cap + TB - 1) / TB), TB, 0, s>>>(c->g_taskoff, c->g_task, c->dstate);
     cudaEventRecord(c->ev[4], s);
-    DSK_COUNT(c, 1 + 2 * (DSK_KEY_LEVELS + 1) + 5);   // init, count+emit per level, mark/flag/emit/bbox/taskfill
+    DSK_COUNT(c, 1 + 1 + 5);   // init, the fused level loop, mark/flag/emit/bbox/taskfill
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
