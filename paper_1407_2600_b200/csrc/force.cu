@@ -157,8 +157,7 @@ __global__ void __launch_bounds__(FW * 32, 12) k_p2p(uint32_t t0, uint32_t t1, c
     }
     // the sink's own leaf is always in the list: remove its self term -m_i/eps from the potential (once)
     if (POT && t.active && t.sub == 0) {
-        dsk_fold(A.hi[0].w, A.lo[0].w, ma.w * rsqrtf(eps2));
-        dsk_fold(A.hi[1].w, A.lo[1].w, mb.w * rsqrtf(eps2));
+        f2_fold(A.hi[3], A.lo[3], f2_make(ma.w * rsqrtf(eps2), mb.w * rsqrtf(eps2)));
     }
     __syncwarp();
     task_store(t, A, reinterpret_cast<double *>(src_all[warp][0]), sacc, sacc_lo);

@@ -98,30 +98,56 @@ __device__ __forceinline__ warp_task make_task(uint32_t t0, uint32_t t1, int fw,
     return t;
 }
 
-// two-float running sums of (ax, ay, az, pot) for the lane's two sinks
+// two-float running sums of (ax, ay, az, pot) for the lane's two sinks, PACKED like the arithmetic: component c
+// of both sinks in one f32x2 (lo half = sink a, hi half = sink b), so a TwoSum fold is six packed adds
 struct sink_acc {
-    float4 hi[2], lo[2];
+    f2 hi[4], lo[4];
 };
+__device__ __forceinline__ float f2_half(f2 v, int h) { return h ? f2_hi(v) : f2_lo(v); }
+__device__ __forceinline__ f2 f2_with(f2 v, int h, float x) { return h ? f2_make(f2_lo(v), x) : f2_make(x, f2_hi(v)); }
 __device__ __forceinline__ void acc_zero(sink_acc &a)
 {
-    a.hi[0] = a.hi[1] = a.lo[0] = a.lo[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int c = 0; c < 4; c++) a.hi[c] = a.lo[c] = f2_dup(0.0f);
 }
 __device__ __forceinline__ void acc_load(sink_acc &a, const warp_task &t, const float4 *__restrict__ sacc,
                                          const float4 *__restrict__ sacc_lo)
 {
     acc_zero(a);
     if (t.active && t.sub == 0) {
-        a.hi[0] = sacc[t.sa]; a.lo[0] = sacc_lo[t.sa];
-        if (t.has_b) { a.hi[1] = sacc[t.sb]; a.lo[1] = sacc_lo[t.sb]; }
+        const float4 ha = sacc[t.sa], la = sacc_lo[t.sa];
+        float4 hb = make_float4(0.f, 0.f, 0.f, 0.f), lb = hb;
+        if (t.has_b) { hb = sacc[t.sb]; lb = sacc_lo[t.sb]; }
+        a.hi[0] = f2_make(ha.x, hb.x); a.hi[1] = f2_make(ha.y, hb.y); a.hi[2] = f2_make(ha.z, hb.z); a.hi[3] = f2_make(ha.w, hb.w);
+        a.lo[0] = f2_make(la.x, lb.x); a.lo[1] = f2_make(la.y, lb.y); a.lo[2] = f2_make(la.z, lb.z); a.lo[3] = f2_make(la.w, lb.w);
     }
 }
-// fold one tile's plain-fp32 sums (packed: lo half = sink a, hi half = sink b) into the running sums
+// (hi, lo) += t without losing the rounding error of the addition (TwoSum), both sinks at once
+__device__ __forceinline__ void f2_fold(f2 &hi, f2 &lo, f2 t)
+{
+    const f2 s = f2_add(hi, t);
+    const f2 bb = f2_sub(s, hi);
+    lo = f2_add(lo, f2_add(f2_sub(hi, f2_sub(s, bb)), f2_sub(t, bb)));
+    hi = s;
+}
+// fold one tile's plain-fp32 sums into the running sums
 __device__ __forceinline__ void acc_fold(sink_acc &a, f2 ax, f2 ay, f2 az, f2 pot, bool want_pot)
 {
-    dsk_fold(a.hi[0].x, a.lo[0].x, f2_lo(ax)); dsk_fold(a.hi[1].x, a.lo[1].x, f2_hi(ax));
-    dsk_fold(a.hi[0].y, a.lo[0].y, f2_lo(ay)); dsk_fold(a.hi[1].y, a.lo[1].y, f2_hi(ay));
-    dsk_fold(a.hi[0].z, a.lo[0].z, f2_lo(az)); dsk_fold(a.hi[1].z, a.lo[1].z, f2_hi(az));
-    if (want_pot) { dsk_fold(a.hi[0].w, a.lo[0].w, f2_lo(pot)); dsk_fold(a.hi[1].w, a.lo[1].w, f2_hi(pot)); }
+    f2_fold(a.hi[0], a.lo[0], ax); f2_fold(a.hi[1], a.lo[1], ay); f2_fold(a.hi[2], a.lo[2], az);
+    if (want_pot) f2_fold(a.hi[3], a.lo[3], pot);
+}
+// scalar access: component c of sink h
+__device__ __forceinline__ void acc_fold1(sink_acc &a, int h, int c, float t)
+{
+    float hi = f2_half(a.hi[c], h), lo = f2_half(a.lo[c], h);
+    dsk_fold(hi, lo, t);
+    a.hi[c] = f2_with(a.hi[c], h, hi); a.lo[c] = f2_with(a.lo[c], h, lo);
+}
+__device__ __forceinline__ void acc_add_double(sink_acc &a, int h, int c, double v)
+{
+    const double s = ((double)f2_half(a.hi[c], h) + (double)f2_half(a.lo[c], h)) + v;
+    const float hi = (float)s;
+    a.hi[c] = f2_with(a.hi[c], h, hi); a.lo[c] = f2_with(a.lo[c], h, (float)(s - (double)hi));
 }
 
 // Add the sub-groups' two-float accumulators (in double, through the warp's scratch: >= 32 x 8 doubles,
@@ -132,10 +158,9 @@ __device__ __forceinline__ void task_store(const warp_task &t, const sink_acc &a
     const int lane = threadIdx.x & 31;
     double d[8];
 #pragma unroll
-    for (int h = 0; h < 2; h++) {
-        d[4 * h + 0] = (double)a.hi[h].x + (double)a.lo[h].x; d[4 * h + 1] = (double)a.hi[h].y + (double)a.lo[h].y;
-        d[4 * h + 2] = (double)a.hi[h].z + (double)a.lo[h].z; d[4 * h + 3] = (double)a.hi[h].w + (double)a.lo[h].w;
-    }
+    for (int h = 0; h < 2; h++)
+#pragma unroll
+        for (int c = 0; c < 4; c++) d[4 * h + c] = (double)f2_half(a.hi[c], h) + (double)f2_half(a.lo[c], h);
     if (t.S > 1) {
         __syncwarp();
 #pragma unroll

@@ -379,11 +379,8 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
                         sx = fma(dx, mri3, sx); sy = fma(dy, mri3, sy); sz = fma(dz, mri3, sz);
                         sp -= mri;
                     }
-                    double v;
-                    v = ((double)A.hi[h].x + (double)A.lo[h].x) + sx; A.hi[h].x = (float)v; A.lo[h].x = (float)(v - (double)A.hi[h].x);
-                    v = ((double)A.hi[h].y + (double)A.lo[h].y) + sy; A.hi[h].y = (float)v; A.lo[h].y = (float)(v - (double)A.hi[h].y);
-                    v = ((double)A.hi[h].z + (double)A.lo[h].z) + sz; A.hi[h].z = (float)v; A.lo[h].z = (float)(v - (double)A.hi[h].z);
-                    if (POT) { v = ((double)A.hi[h].w + (double)A.lo[h].w) + sp; A.hi[h].w = (float)v; A.lo[h].w = (float)(v - (double)A.hi[h].w); }
+                    acc_add_double(A, h, 0, sx); acc_add_double(A, h, 1, sy); acc_add_double(A, h, 2, sz);
+                    if (POT) acc_add_double(A, h, 3, sp);
                 }
             }
         }
@@ -399,8 +396,8 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
                     const float xs = h ? f2_hi(X) : f2_lo(X), ys = h ? f2_hi(Y) : f2_lo(Y), zs = h ? f2_hi(Z) : f2_lo(Z);
                     float pot = 0.0f, ax = 0.0f, ay = 0.0f, az = 0.0f;
                     for (int k = t.sub; k < ntc; k += t.S) m2p_body<P, float, POT>(xs, ys, zs, rows + (size_t)k * FROW, pot, ax, ay, az);
-                    dsk_fold(A.hi[h].x, A.lo[h].x, ax); dsk_fold(A.hi[h].y, A.lo[h].y, ay); dsk_fold(A.hi[h].z, A.lo[h].z, az);
-                    if (POT) dsk_fold(A.hi[h].w, A.lo[h].w, pot);
+                    acc_fold1(A, h, 0, ax); acc_fold1(A, h, 1, ay); acc_fold1(A, h, 2, az);
+                    if (POT) acc_fold1(A, h, 3, pot);
                 });
             }
         }

@@ -67,4 +67,6 @@ def test_accounting_matches_kernel_op_counts():
         ffma, fmul, fadd = accounting.m2p_ops(p, pot=True)
         assert fn[0].count(" FFMA2 ") == ffma, (p, fn[0].count(" FFMA2 "), ffma)
         assert fn[0].count(" FMUL2 ") == fmul, (p, fn[0].count(" FMUL2 "), fmul)
-        assert fn[0].count(" FADD2 ") == fadd, (p, fn[0].count(" FADD2 "), fadd)
+        # + the packed TwoSum fold of the tile sums into the two-float accumulators: 6 adds x 4 components
+        # (a few more where the compiler packs scalar pairs itself, e.g. the sinks' offsets from the group centre)
+        assert fadd + 24 <= fn[0].count(" FADD2 ") <= fadd + 32, (p, fn[0].count(" FADD2 "), fadd)
