@@ -50,7 +50,9 @@ def workload():
 def config_dict(cfg, n_gpus):
     return {"workload": WORKLOADS[CFG],
             "N": cfg["N"], "eps": cfg["eps"], "theta": cfg["theta"], "p": cfg["p"], "periodic": bool(cfg["periodic"]),
-            "step": "dsk_build_tree + dsk_accel (acc+pot)", "NLEAF": 80, "NCRIT": 128,
+            "step": ("dsk_kdk_step, da = 0.01 from a = 0.5, Einstein-de Sitter (one force evaluation per step; the e2e arm "
+                     "pays two: it restarts from the host copy)") if CFG == 5 else "dsk_build_tree + dsk_accel (acc+pot)",
+            "NLEAF": 80, "NCRIT": 128,
             "l2": "256 MiB buffer written between steps (outside the event pairs); working set ~1 GB > L2",
             "parallelism": f"replicas x{n_gpus}" if n_gpus > 1 else "single GPU"}
 
@@ -208,15 +210,33 @@ def run_ours(args):
     hpot = torch.empty(n, dtype=torch.float32).pin_memory()
     tp2, tm2 = torch.empty_like(tp), torch.empty_like(tm)
 
-    def step():
-        d.build_tree(tp, tm)
-        d.accel(tp, tm, acc, pot)
+    kdk = CFG == 5          # configs[4] is a run: a step is one dsk_kdk_step (kick, drift, tree, force, kick)
+    if kdk:
+        vel = torch.zeros_like(tp)              # cold start
+        hv = torch.zeros((n, 3), dtype=torch.float32).pin_memory()
+        vel2 = torch.empty_like(tp)
+        clock = {"a": 0.5}
+        DA = 0.01
 
-    def step_e2e():
-        tp2.copy_(hp, non_blocking=True); tm2.copy_(hm, non_blocking=True)
-        d.build_tree(tp2, tm2)
-        d.accel(tp2, tm2, acc, pot)
-        hacc.copy_(acc, non_blocking=True); hpot.copy_(pot, non_blocking=True)
+        def step():
+            d.kdk_step(tp, vel, tm, clock["a"], DA)
+            clock["a"] += DA
+
+        def step_e2e():
+            tp2.copy_(hp, non_blocking=True); tm2.copy_(hm, non_blocking=True); vel2.copy_(hv, non_blocking=True)
+            d.kdk_reset()
+            d.kdk_step(tp2, vel2, tm2, 0.5, DA)
+            hacc.copy_(tp2, non_blocking=True); hv.copy_(vel2, non_blocking=True)
+    else:
+        def step():
+            d.build_tree(tp, tm)
+            d.accel(tp, tm, acc, pot)
+
+        def step_e2e():
+            tp2.copy_(hp, non_blocking=True); tm2.copy_(hm, non_blocking=True)
+            d.build_tree(tp2, tm2)
+            d.accel(tp2, tm2, acc, pot)
+            hacc.copy_(acc, non_blocking=True); hpot.copy_(pot, non_blocking=True)
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -273,8 +293,8 @@ def run_ours(args):
             pass
         sm_max = float(peaks.get("sm_max_mhz", 1965.0))
         peak_fp32 = accounting.fp32_peak_flops(prop.multi_processor_count, sm_max)
-        f_m2p = accounting.m2p_flops(cfg["p"], pot=True)
-        f_p2p = accounting.p2p_flops(pot=True)
+        f_m2p = accounting.m2p_flops(cfg["p"], pot=not kdk)      # dsk_kdk_step asks for no potential
+        f_p2p = accounting.p2p_flops(pot=not kdk)
         ach_m2p = f_m2p * st["n_m2p"] / (phase["ms_m2p"] * 1e-3)
         ach_p2p = f_p2p * st["n_p2p"] / (phase["ms_p2p"] * 1e-3) if phase["ms_p2p"] > 0 else 0.0
         hbm = float(peaks.get("hbm_gbs", 6650.0))
@@ -286,7 +306,7 @@ def run_ours(args):
                 hbm_phases[key] = {"GBps": b / (phase[k] * 1e-3) / 1e9, "frac": b / (phase[k] * 1e-3) / 1e9 / hbm}
         traffic = None
         tpath = os.path.join(ROOT, "profiles", "m2p_dram_bytes_per_launch.txt")
-        if os.path.exists(tpath):
+        if CFG == 2 and os.path.exists(tpath):                   # captured on the default workload only
             try:
                 traffic = float(open(tpath).read().split()[0])
             except Exception:
@@ -302,7 +322,7 @@ def run_ours(args):
                "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                "config": config_dict(cfg, world),
-               "roofline": {"bound": "alu", "kernel": f"k_m2p<{cfg['p']},pot>", "achieved": ach_m2p / 1e12,
+               "roofline": {"bound": "alu", "kernel": f"k_m2p<{cfg['p']},{'nopot' if kdk else 'pot'},{'fp64 monopoles' if cfg['periodic'] else 'fp32'}>", "achieved": ach_m2p / 1e12,
                             "peak": peak_fp32 / 1e12, "unit": "TFLOP/s", "frac": ach_m2p / peak_fp32,
                             "traffic": traffic,
                             "peak_source": f"nominal FP32: {prop.multi_processor_count} SMs x 128 lanes x 2 x {sm_max:.0f} MHz "

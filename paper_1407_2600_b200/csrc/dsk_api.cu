@@ -110,7 +110,7 @@ extern "C" int dsk_destroy(dsk_ctx *c)
     if (!c) return DSK_EINVAL;
     if (c->hstate) {
         cudaFreeHost(c->hstate);
-        for (int i = 0; i < 16; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+        for (int i = 0; i < 20; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     }
     delete c;
     return DSK_OK;
@@ -134,7 +134,7 @@ extern "C" int dsk_bind_workspace(dsk_ctx *c, void *dev_ptr, size_t bytes)
     if (!c->hstate) {
         DSK_CUDA(cudaMallocHost((void **)&c->hstate, 4096));
         memset(c->hstate, 0, 4096);
-        for (int i = 0; i < 16; i++) DSK_CUDA(cudaEventCreate(&c->ev[i]));
+        for (int i = 0; i < 20; i++) DSK_CUDA(cudaEventCreate(&c->ev[i]));
     }
     c->ws = (char *)dev_ptr;
     c->ws_bytes = bytes;
@@ -293,14 +293,19 @@ extern "C" int dsk_kdk_step(dsk_ctx *c, float *pos, float *vel, const float *mas
     if (e) return e;
     e = dsk_run_drift(c, pos, vel, (float)d);
     if (e) return e;
+    cudaEventRecord(c->ev[16], c->stream);
     c->kdk_have_acc = 0;
     e = dsk_build_tree(c, pos, mass);
     if (e) return e;
     e = dsk_accel(c, pos, mass, c->kdk_acc, nullptr);
     if (e) return e;
+    cudaEventRecord(c->ev[17], c->stream);
     e = dsk_run_kick(c, vel, c->kdk_acc, (float)k2);
     if (e) return e;
+    cudaEventRecord(c->ev[18], c->stream);
     DSK_CUDA(cudaStreamSynchronize(c->stream));
+    c->stats.ms_kdk = ev_ms(c->ev[15], c->ev[16]) + ev_ms(c->ev[17], c->ev[18]);
+    c->stats.n_launch += 2;                      // the first kick and the drift (build_tree reset the counter)
     c->kdk_have_acc = 1;
     return DSK_OK;
 }

@@ -120,7 +120,7 @@ struct dsk_ctx {
     float lists_theta;
     double far_T[DSK_NFAR];
     dsk_stats stats;
-    cudaEvent_t ev[16];
+    cudaEvent_t ev[20];
     int nsm;
 };
 
