@@ -258,7 +258,6 @@ template <int P, bool M64> struct m2p_cfg {
     static constexpr size_t BUF_BYTES = (size_t)NCELL * FROW * sizeof(float);
     static constexpr size_t M64_BYTES = M64 ? (size_t)NCELL * 4 * sizeof(double) : 0;   // com' xyz and mass of a tile's cells
     static constexpr size_t WARP_BYTES = 2 * BUF_BYTES + M64_BYTES;    // two row buffers + fp64 monopoles
-    static constexpr bool PACKED = (P <= 6);
 };
 
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
@@ -280,7 +279,6 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
 {
     using C = m2p_cfg<P, M64>;
     constexpr int NCELL = C::NCELL, LPC = C::LPC, FROW = C::FROW, NCH = C::NCH;
-    constexpr bool PACKED = C::PACKED;
     constexpr uint32_t CELL_MASK = (1u << DSK_CELL_BITS) - 1u;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const warp_task t = make_task(t0, t1, FW, taskmap, gfirst, gcount);
@@ -385,21 +383,9 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
             }
         }
         if (t.active) {
-            if constexpr (PACKED) {
-                f2 pot = f2_dup(0.0f), ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f);
-                for (int k = t.sub; k < ntc; k += t.S) m2p_body<P, f2, POT>(X, Y, Z, rows + (size_t)k * FROW, pot, ax, ay, az);
-                acc_fold(A, ax, ay, az, pot, POT);
-            } else {
-                // one sink at a time (p = 8 keeps 81 monomials live: no room for packed pairs)
-                static_for<0, 2>([&](auto H) {
-                    constexpr int h = decltype(H)::value;
-                    const float xs = h ? f2_hi(X) : f2_lo(X), ys = h ? f2_hi(Y) : f2_lo(Y), zs = h ? f2_hi(Z) : f2_lo(Z);
-                    float pot = 0.0f, ax = 0.0f, ay = 0.0f, az = 0.0f;
-                    for (int k = t.sub; k < ntc; k += t.S) m2p_body<P, float, POT>(xs, ys, zs, rows + (size_t)k * FROW, pot, ax, ay, az);
-                    acc_fold1(A, h, 0, ax); acc_fold1(A, h, 1, ay); acc_fold1(A, h, 2, az);
-                    if (POT) acc_fold1(A, h, 3, pot);
-                });
-            }
+            f2 pot = f2_dup(0.0f), ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f);
+            for (int k = t.sub; k < ntc; k += t.S) m2p_body<P, f2, POT>(X, Y, Z, rows + (size_t)k * FROW, pot, ax, ay, az);
+            acc_fold(A, ax, ay, az, pot, POT);
         }
         __syncwarp();
     }
