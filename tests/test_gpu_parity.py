@@ -229,6 +229,28 @@ def test_forces_C2_full_sampled(dsk, orc):
     d.close()
 
 
+
+def test_forces_degenerate_inputs(dsk, orc):
+    """300 coincident particles (one over-full level-21 leaf, cut into chunks of NCRIT) among 200 random ones,
+    and a case where every particle sits in one octant corner: forces and potentials against the direct sum."""
+    rng = np.random.default_rng(4)
+    a = rng.random((500, 3), dtype=np.float32); a[:300] = np.float32([0.3, 0.4, 0.5])
+    b = (rng.random((700, 3), dtype=np.float32) * np.float32(1e-4)).astype(np.float32)
+    for pos in (a, b):
+        n = len(pos)
+        mass = rng.uniform(0.5, 1.5, n).astype(np.float32)
+        eps = 0.05 if pos is a else 1e-5
+        d = dsk.Dsk(n, 1.0, False, eps, 0.3, 4)
+        tp, tm = _dev(pos), _dev(mass)
+        d.build_tree(tp, tm)
+        _check_structure(orc, d, pos, mass, 1.0, False)
+        acc, pot = d.accel(tp, tm)
+        ra, rp = orc.direct_iso(pos, mass, eps)
+        assert np.max(np.abs(acc.cpu().numpy() - ra)) < 2e-4 * np.abs(ra).max()
+        assert np.max(np.abs(pot.cpu().numpy() - rp)) < 2e-4 * np.abs(rp).max()
+        d.close()
+
+
 # ---- forces, periodic ---------------------------------------------------------------------------------
 def test_forces_periodic_lattice_scaled(dsk, orc):
     """configs[2] recipe at 32^3: Ewald direct sum on 192 sinks, oracle tree on 4096."""
