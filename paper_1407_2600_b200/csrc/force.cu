@@ -19,8 +19,8 @@ int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint6
 
 // ---- F1 ----------------------------------------------------------------------------------------------
 // Sources are staged as they are stored: a listed leaf is a contiguous run of the sorted (x, y, z, m) array,
-// its lane copies it with cp.async (LDGSTS, 16 B per particle) to the run's place in the window, which is the
-// exclusive prefix sum of the run lengths of the 32 leaves handled at a time.  Windows of P2P_TILE sources are
+// its lane copies it with ONE cp.async.bulk (TMA 1-D copy, completion on the window's mbarrier) to the run's place
+// in the window, which is the exclusive prefix sum of the run lengths of the 32 leaves handled at a time.  Windows of P2P_TILE sources are
 // double-buffered: the next window travels while the current one is evaluated, and the cell records of the
 // next 32 leaves are already in registers, so no global latency is exposed (ncu of the synchronous version:
 // 2.6 warps per issue waiting on a long scoreboard).  Differences are taken between raw coordinates (one
@@ -31,13 +31,41 @@ __device__ __forceinline__ void cp_async16_p2p(void *smem_dst, const void *gmem_
     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
 
+__device__ __forceinline__ uint32_t p2p_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void p2p_mbar_init(uint64_t *bar)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(p2p_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void p2p_mbar_expect(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(p2p_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void p2p_mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(p2p_smem_u32(bar)), "r"(parity) : "memory");
+}
+// one TMA bulk copy: a leaf's run (or the part of it inside the window), bytes a multiple of 16
+__device__ __forceinline__ void p2p_bulk(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(p2p_smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(p2p_smem_u32(bar)) : "memory");
+}
+
 struct leaf_batch {              // one leaf per lane
     uint32_t first, cnt, pref, total;
     float shx, shy, shz;
 };
 
 template <bool POT>
-__global__ void __launch_bounds__(FW * 32, 12) k_p2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic, float box, float eps2,
+__global__ void __launch_bounds__(FW * 32, 16) k_p2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic, float box, float eps2,
                                                  const dsk_cellrec *__restrict__ cell, const float4 *__restrict__ spos,
                                                  const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
                                                  const uint32_t *__restrict__ list,
@@ -46,6 +74,7 @@ __global__ void __launch_bounds__(FW * 32, 12) k_p2p(uint32_t t0, uint32_t t1, c
                                                  float4 *__restrict__ sacc_lo)
 {
     __shared__ __align__(16) float4 src_all[FW][2][P2P_TILE];     // two windows of raw (x, y, z, m) per warp
+    __shared__ __align__(8) uint64_t bar_all[FW][2];              // one mbarrier per window buffer
     const warp_task t = make_task(t0, t1, FW, taskmap, gfirst, gcount);
     if (!t.valid) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -87,15 +116,21 @@ __global__ void __launch_bounds__(FW * 32, 12) k_p2p(uint32_t t0, uint32_t t1, c
         i0 = max(L.pref, lo) - L.pref;
         i1 = e > L.pref ? e - L.pref : 0u;
     };
+    // copy window [lo, lo + P2P_TILE) of batch L into buffer b: one cp.async.bulk per leaf run (a per-particle
+    // LDGSTS loop kept 3.8 of 32 lanes busy and made 16 % of the kernel's instructions)
     auto issue = [&](const leaf_batch &L, uint32_t lo, int b) {
         uint32_t i0, i1;
         my_part(L, lo, i0, i1);
-        float4 *dst = src_all[warp][b] + (L.pref - lo);
-        const float4 *sp = spos + L.first;
-        for (uint32_t i = i0; i < i1; i++) cp_async16_p2p(dst + i, sp + i);
-        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // earlier generic reads of the buffer are done
+        if (lane == 0) p2p_mbar_expect(&bar_all[warp][b], (min(lo + (uint32_t)P2P_TILE, L.total) - lo) * 16u);
+        __syncwarp();
+        if (i1 > i0) p2p_bulk(src_all[warp][b] + (L.pref - lo) + i0, spos + L.first + i0, (i1 - i0) * 16u, &bar_all[warp][b]);
     };
 
+    if (lane == 0) { p2p_mbar_init(&bar_all[warp][0]); p2p_mbar_init(&bar_all[warp][1]); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncwarp();
+    uint32_t phase = 0;                           // bit b: parity of the next completion of buffer b's mbarrier
     leaf_batch cur = load_batch(0), nxt = load_batch(32);
     uint32_t bcur = 0, lo = 0;                    // current window: batch at list position bcur, offset lo
     int buf = 0;
@@ -103,8 +138,8 @@ __global__ void __launch_bounds__(FW * 32, 12) k_p2p(uint32_t t0, uint32_t t1, c
     while (bcur < n) {
         // the window after this one
         const bool same = lo + (uint32_t)P2P_TILE < cur.total;
-        asm volatile("cp.async.wait_group 0;" ::: "memory");
-        __syncwarp();
+        p2p_mbar_wait(&bar_all[warp][buf], (phase >> buf) & 1u);
+        phase ^= 1u << buf;
         float4 *src = src_all[warp][buf];
         const uint32_t nt = min((uint32_t)P2P_TILE, cur.total - lo);
         if (periodic && (cur.shx != 0.0f || cur.shy != 0.0f || cur.shz != 0.0f)) {
