@@ -372,7 +372,10 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
                         const double2 c01 = *reinterpret_cast<const double2 *>(mono + 4 * k);
                         const double2 c23 = *reinterpret_cast<const double2 *>(mono + 4 * k + 2);
                         const double dx = c01.x - xs, dy = c01.y - ys, dz = c23.x - zs;
-                        const double ri = rsqrt(fma(dx, dx, fma(dy, dy, fma(dz, dz, e2d))));
+                        // 1/sqrt in double: fp32 MUFU seed (1e-7) + one Newton step (1.5e-14)
+                        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, e2d)));
+                        const double y0 = (double)rsqrtf((float)r2);
+                        const double ri = y0 * fma(-0.5 * r2, y0 * y0, 1.5);
                         const double mri = c23.y * ri, mri3 = mri * ri * ri;
                         sx = fma(dx, mri3, sx); sy = fma(dy, mri3, sy); sz = fma(dz, mri3, sz);
                         sp -= mri;
