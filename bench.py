@@ -300,10 +300,20 @@ def run_ours(args):
         hbm = float(peaks.get("hbm_gbs", 6650.0))
         bpp = accounting.BYTES_PER_PARTICLE
         hbm_phases = {}
-        for k, key in (("ms_key", "key"), ("ms_sort", "sort")):
-            if phase.get(k, 0) > 0:
-                b = (bpp[key] + (bpp["gather"] if key == "sort" else 0)) * n
-                hbm_phases[key] = {"GBps": b / (phase[k] * 1e-3) / 1e9, "frac": b / (phase[k] * 1e-3) / 1e9 / hbm}
+        # algorithmic bytes of the HBM-bound phases: per particle and per cell / list entry
+        rowb = 4 * (8 + (cfg["p"] + 1) * (cfg["p"] + 2) * (cfg["p"] + 3) // 6)
+        alg_bytes = {
+            "key": bpp["key"] * n,
+            "sort": (bpp["sort"] + bpp["gather"]) * n,
+            "build": 8 * n + 60 * st["ncell"],
+            "upward": 16 * n + st["ncell"] * 4 * rowb,                       # particles once; rows written, read by M2M, force rows written
+            "walk": 4 * (st["list_m2p"] + st["list_p2p"]),                  # list entries written (the cell tests hit L2)
+            "scatter": bpp["scatter"] * n,
+        }
+        for key, b in alg_bytes.items():
+            ms = phase.get("ms_" + key, 0)
+            if ms > 0:
+                hbm_phases[key] = {"GBps": b / (ms * 1e-3) / 1e9, "frac": b / (ms * 1e-3) / 1e9 / hbm}
         traffic = None
         tpath = os.path.join(ROOT, "profiles", "m2p_dram_bytes_per_launch.txt")
         if CFG == 2 and os.path.exists(tpath):                   # captured on the default workload only
