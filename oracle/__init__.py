@@ -288,14 +288,21 @@ def farfield_eval(lam, L, pos, sink=None, order=FAR_ORDER):
 
 
 # ---- O9 --------------------------------------------------------------------------------------------
-def kdk_factors(periodic, mtot, box, a, da):
+def kdk_factors(periodic, mtot, box, a, da, cosmology=None):
+    """cosmology = (Omega_m, Omega_Lambda) selects the Friedmann factors (O9b); None: Einstein-de Sitter (O9)."""
     k1 = C.c_double(0); d = C.c_double(0); k2 = C.c_double(0)
+    if periodic and cosmology is not None:
+        f = lib().orc_kdk_factors_friedmann
+        f.restype = None
+        f(C.c_double(mtot), C.c_double(box), C.c_double(cosmology[0]), C.c_double(cosmology[1]), C.c_double(a),
+          C.c_double(da), C.byref(k1), C.byref(d), C.byref(k2))
+        return k1.value, d.value, k2.value
     lib().orc_kdk_factors(C.c_int(int(periodic)), C.c_double(mtot), C.c_double(box), C.c_double(a),
                           C.c_double(da), C.byref(k1), C.byref(d), C.byref(k2))
     return k1.value, d.value, k2.value
 
 
-def kdk_step(pos, vel, mass, box, periodic, eps, theta, p, a, da, acc=None, force=None):
+def kdk_step(pos, vel, mass, box, periodic, eps, theta, p, a, da, acc=None, force=None, cosmology=None):
     """One KDK step (O9).  State is fp32 (positions/velocities are 32-bit floats); the
     arithmetic of each update is fp64 and the result is rounded once to fp32.  `acc` is the cached
     force at `pos` (None: computed first).  `force(pos)` defaults to the oracle tree force Tr.
@@ -305,7 +312,7 @@ def kdk_step(pos, vel, mass, box, periodic, eps, theta, p, a, da, acc=None, forc
         def force(x):
             return tree_force(x, mass, box, periodic, eps, theta, p)[0]
     mtot = float(np.sum(mass.astype(np.float64)))
-    k1, d, k2 = kdk_factors(periodic, mtot, box, a, da)
+    k1, d, k2 = kdk_factors(periodic, mtot, box, a, da, cosmology)
     if acc is None:
         acc = force(pos)
     vel = (vel.astype(np.float64) + acc * k1).astype(np.float32)

@@ -98,4 +98,6 @@ void orc_farfield_eval(const double *Lambda, int order, double L, int64_t nsink,
 /* O9 (orc_kdk.c) */
 void orc_kdk_factors(int periodic, double mtot, double box, double a, double da, double *k1,
                      double *drift, double *k2);
+void orc_kdk_factors_friedmann(double mtot, double box, double omega_m, double omega_l, double a,
+                               double da, double *k1, double *drift, double *k2);
 #endif

@@ -427,3 +427,36 @@ void orc_kdk_factors(int periodic, double mtot, double box, double a, double da,
     *k2 = 2.0 / H0 * (sqrt(a1) - sqrt(am));
     *drift = 2.0 / H0 * (1.0 / sqrt(a) - 1.0 / sqrt(a1));
 }
+
+/* ---- O9b Friedmann kick/drift factors ("All of these simulations utilize the
+ * exact same cosmology with (Omega_m, ..., Omega_Lambda, ...) = (0.295, ..., 0.705, ...)") -------------------------
+ * Same state and composition as O9; only H(a) changes:
+ *   H(a) = H0 E(a),  E(a)^2 = Omega_m a^-3 + Omega_k a^-2 + Omega_L,  Omega_k = 1 - Omega_m - Omega_L,
+ *   H0^2 = (8 pi/3) G rho_crit, and the box holds the MATTER: M_tot/box^3 = Omega_m rho_crit,
+ *   kick  K(a1,a2) = int dt/a   = (1/H0) int_{a1}^{a2} da / (a^2 E(a))
+ *   drift D(a1,a2) = int dt/a^2 = (1/H0) int_{a1}^{a2} da / (a^3 E(a))
+ * (dt = da / (a H)).  Omega_m = 1, Omega_L = 0 is Einstein-de Sitter and must reproduce orc_kdk_factors.
+ * Plain composite Simpson rule, 4096 panels per integral. */
+static double simpson_friedmann(double a1, double a2, int apow, double om, double ol)
+{
+    const int n = 4096;
+    const double ok = 1.0 - om - ol, h = (a2 - a1) / n;
+    double sum = 0.0;
+    for (int i = 0; i <= n; i++) {
+        const double a = a1 + h * i;
+        const double E = sqrt(om / (a * a * a) + ok / (a * a) + ol);
+        const double f = 1.0 / (pow(a, (double)apow) * E);
+        sum += f * ((i == 0 || i == n) ? 1.0 : ((i & 1) ? 4.0 : 2.0));
+    }
+    return sum * h / 3.0;
+}
+
+void orc_kdk_factors_friedmann(double mtot, double box, double omega_m, double omega_l, double a, double da,
+                               double *k1, double *drift, double *k2)
+{
+    const double H0 = sqrt(8.0 * PI / 3.0 * mtot / (box * box * box) / omega_m);
+    const double am = a + 0.5 * da, a1 = a + da;
+    *k1 = simpson_friedmann(a, am, 2, omega_m, omega_l) / H0;
+    *k2 = simpson_friedmann(am, a1, 2, omega_m, omega_l) / H0;
+    *drift = simpson_friedmann(a, a1, 3, omega_m, omega_l) / H0;
+}

@@ -212,6 +212,29 @@ def test_kdk_factors(orc):
     assert np.isclose(d, D(a, a + da), rtol=1e-10)
 
 
+def test_kdk_factors_friedmann(orc):
+    """O9b pins: Omega_m = 1 is the Einstein-de Sitter closed form; the paper's cosmology (PAPER.md:139,
+    Omega_m = 0.295, Omega_Lambda = 0.705) against an independent adaptive quadrature of int da/(a^2 E), int da/(a^3 E);
+    an open model too; and the exact relation D = int dK / a between the two integrands."""
+    from scipy.integrate import quad
+    for a, da in ((0.5, 0.01), (0.02, 0.001), (0.9, 0.1)):
+        e = orc.kdk_factors(True, 2.5, 2.0, a, da)
+        f = orc.kdk_factors(True, 2.5, 2.0, a, da, (1.0, 0.0))
+        assert np.allclose(e, f, rtol=1e-12, atol=0)
+    mtot, box = 1.0, 1.0
+    for om, ol in ((0.295, 0.705), (0.3, 0.0), (1.0, 0.0)):
+        H0 = math.sqrt(8 * math.pi / 3 * mtot / box ** 3 / om)
+        E = lambda x: math.sqrt(om / x ** 3 + (1 - om - ol) / x ** 2 + ol)   # noqa: E731
+        K = lambda a1, a2: quad(lambda x: 1 / (x * x * E(x)), a1, a2, epsabs=0, epsrel=1e-13)[0] / H0   # noqa: E731
+        D = lambda a1, a2: quad(lambda x: 1 / (x ** 3 * E(x)), a1, a2, epsabs=0, epsrel=1e-13)[0] / H0  # noqa: E731
+        for a, da in ((0.5, 0.01), (0.1, 0.02), (0.98, 0.02)):
+            k1, d, k2 = orc.kdk_factors(True, mtot, box, a, da, (om, ol))
+            assert abs(k1 - K(a, a + da / 2)) < 1e-11 * k1 and abs(k2 - K(a + da / 2, a + da)) < 1e-11 * k2
+            assert abs(d - D(a, a + da)) < 1e-11 * d
+            # Lambda slows the expansion less at late times: at fixed H0-from-matter, factors shrink with Omega_m < 1
+            assert k1 > 0 and d > k1 + k2        # D integrand = K integrand / a, a < 1
+
+
 def test_kdk_free_drift_and_time_reversal(orc):
     rng = np.random.default_rng(4)
     n = 200
