@@ -102,6 +102,12 @@ int dsk_accel(dsk_ctx *ctx, const float *pos, const float *mass, float *acc, flo
 int dsk_kdk_step(dsk_ctx *ctx, float *pos, float *vel, const float *mass, double a, double da);
 int dsk_kdk_reset(dsk_ctx *ctx);
 
+/* Background cosmology of the periodic leapfrog (the paper's runs use
+ * Omega_m = 0.295, Omega_Lambda = 0.705).  H(a) = H0 sqrt(Omega_m a^-3 + (1 - Omega_m - Omega_Lambda) a^-2 + Omega_Lambda),
+ * H0^2 = (8 pi/3) M_tot / (box^3 Omega_m); kick = int da/(a^2 H), drift = int da/(a^3 H), integrated on the host in
+ * fp64.  Default (1, 0) = Einstein-de Sitter.  omega_m > 0 and H^2 > 0 on the steps taken; DSK_EINVAL otherwise. */
+int dsk_set_cosmology(dsk_ctx *ctx, double omega_m, double omega_lambda);
+
 /* ---- introspection (parity tests, reporting) ---------------------------------------------------- */
 /* sorted keys and the permutation: sorted_keys[r] = key(order[r]); dev [N] each (either may be NULL). */
 int dsk_get_keys(dsk_ctx *ctx, uint64_t *sorted_keys, uint32_t *order);

@@ -97,6 +97,7 @@ extern "C" int dsk_create(dsk_ctx **out, int64_t N, float box, int periodic, flo
     memset(c, 0, sizeof(*c));
     c->N = N; c->box = box; c->periodic = periodic ? 1 : 0; c->eps = eps; c->theta = theta; c->p = p;
     c->moments_p = -1; c->p_cap = p; c->frow_tab_p = -1;
+    c->omega_m = 1.0; c->omega_l = 0.0;
     c->ws_bytes = 0;
     carve(c, nullptr);
     if (c->periodic) dsk_lattice_tensors((double)box, DSK_WS, c->far_T);
@@ -250,16 +251,50 @@ extern "C" int dsk_accel(dsk_ctx *c, const float *pos, const float *mass, float 
     return e;
 }
 
-// Einstein-de Sitter leapfrog factors (O9): H0^2 = (8 pi/3) M_tot / box^3
+// Leapfrog factors (O9 / O9b): H0^2 = (8 pi/3) M_tot / (box^3 Omega_m),
+// K(a1,a2) = int da / (a^2 H), D(a1,a2) = int da / (a^3 H).  Einstein-de Sitter in closed form, any other
+// Friedmann background by 16-point Gauss-Legendre on each (short) interval, fp64 on the host.
+static double gl16(double a1, double a2, int apow, double om, double ol)
+{
+    static const double x[8] = {0.0950125098376374401853193, 0.2816035507792589132304605, 0.4580167776572273863424194,
+                                0.6178762444026437484466718, 0.7554044083550030338951012, 0.8656312023878317438804679,
+                                0.9445750230732325760779884, 0.9894009349916499325961542};
+    static const double w[8] = {0.1894506104550684962853967, 0.1826034150449235888667637, 0.1691565193950025381893121,
+                                0.1495959888165767320815017, 0.1246289712555338720524763, 0.0951585116824927848099251,
+                                0.0622535239386478928628438, 0.0271524594117540948517806};
+    const double ok = 1.0 - om - ol, c = 0.5 * (a1 + a2), h = 0.5 * (a2 - a1);
+    double sum = 0.0;
+    for (int i = 0; i < 8; i++)
+        for (int sgn = -1; sgn <= 1; sgn += 2) {
+            const double a = c + sgn * h * x[i];
+            sum += w[i] / (pow(a, (double)apow) * sqrt(om / (a * a * a) + ok / (a * a) + ol));
+        }
+    return sum * h;
+}
+
 static void kdk_factors(const dsk_ctx *c, double mtot, double a, double da, double *k1, double *d, double *k2)
 {
     if (!c->periodic) { *k1 = 0.5 * da; *d = da; *k2 = 0.5 * da; return; }
     const double PI = 3.14159265358979323846;
-    const double H0 = sqrt(8.0 * PI / 3.0 * mtot / ((double)c->box * c->box * c->box));
+    const double H0 = sqrt(8.0 * PI / 3.0 * mtot / ((double)c->box * c->box * c->box) / c->omega_m);
     const double am = a + 0.5 * da, a1 = a + da;
-    *k1 = 2.0 / H0 * (sqrt(am) - sqrt(a));
-    *k2 = 2.0 / H0 * (sqrt(a1) - sqrt(am));
-    *d = 2.0 / H0 * (1.0 / sqrt(a) - 1.0 / sqrt(a1));
+    if (c->omega_m == 1.0 && c->omega_l == 0.0) {
+        *k1 = 2.0 / H0 * (sqrt(am) - sqrt(a));
+        *k2 = 2.0 / H0 * (sqrt(a1) - sqrt(am));
+        *d = 2.0 / H0 * (1.0 / sqrt(a) - 1.0 / sqrt(a1));
+        return;
+    }
+    *k1 = gl16(a, am, 2, c->omega_m, c->omega_l) / H0;
+    *k2 = gl16(am, a1, 2, c->omega_m, c->omega_l) / H0;
+    *d = gl16(a, a1, 3, c->omega_m, c->omega_l) / H0;
+}
+
+extern "C" int dsk_set_cosmology(dsk_ctx *c, double omega_m, double omega_lambda)
+{
+    if (!c) return DSK_EINVAL;
+    if (!(omega_m > 0.0) || !isfinite(omega_m) || !isfinite(omega_lambda)) return DSK_EINVAL;
+    c->omega_m = omega_m; c->omega_l = omega_lambda;
+    return DSK_OK;
 }
 
 extern "C" int dsk_kdk_reset(dsk_ctx *c)
@@ -274,6 +309,11 @@ extern "C" int dsk_kdk_step(dsk_ctx *c, float *pos, float *vel, const float *mas
     if (!c || !pos || !vel || !mass) return DSK_EINVAL;
     if (!c->ws) return DSK_ENOWORKSPACE;
     if (c->periodic && !(a > 0.0 && a + da > 0.0)) return DSK_EINVAL;
+    if (c->periodic) {
+        const double ok = 1.0 - c->omega_m - c->omega_l, e0 = a, e1 = a + da;
+        if (!(c->omega_m / (e0 * e0 * e0) + ok / (e0 * e0) + c->omega_l > 0.0) ||
+            !(c->omega_m / (e1 * e1 * e1) + ok / (e1 * e1) + c->omega_l > 0.0)) return DSK_EINVAL;
+    }
     int e;
     if (!c->kdk_have_acc) {
         e = dsk_build_tree(c, pos, mass);

@@ -115,6 +115,7 @@ struct dsk_ctx {
     int ntile;
     // state
     int have_tree, moments_p, lists_valid, kdk_have_acc;
+    double omega_m, omega_l;  // background cosmology of dsk_kdk_step (default 1, 0)
     int p_cap;                // order the workspace was sized for (dsk_create's p); set_params may lower p
     int frow_tab_p;           // order of the uploaded force-row map
     float lists_theta;

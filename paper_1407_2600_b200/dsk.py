@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libdsk.so")
 
 SYMBOLS = [
     "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
-    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_kdk_step", "dsk_kdk_reset", "dsk_get_keys",
+    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_kdk_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_get_keys",
     "dsk_get_tree", "dsk_get_moments", "dsk_get_groups", "dsk_get_stats", "dsk_get_param",
     "dsk_get_lattice_tensors", "dsk_strerror",
 ]
@@ -60,6 +60,7 @@ def load_library(path=LIB_PATH):
     lib.dsk_accel.argtypes = [vp, vp, vp, vp, vp]
     lib.dsk_kdk_step.argtypes = [vp, vp, vp, vp, f64, f64]
     lib.dsk_kdk_reset.argtypes = [vp]
+    lib.dsk_set_cosmology.argtypes = [vp, f64, f64]
     lib.dsk_get_keys.argtypes = [vp, vp, vp]
     lib.dsk_get_tree.argtypes = [vp, C.POINTER(i64), vp, vp, vp, vp]
     lib.dsk_get_moments.argtypes = [vp, vp, vp]
@@ -168,6 +169,9 @@ class Dsk:
     def kdk_step(self, pos, vel, mass, a, da):
         _dev_f32(pos, (self.N, 3)); _dev_f32(vel, (self.N, 3)); _dev_f32(mass, (self.N,))
         _check(self.lib.dsk_kdk_step(self._h, _ptr(pos), _ptr(vel), _ptr(mass), float(a), float(da)))
+
+    def set_cosmology(self, omega_m, omega_lambda):
+        _check(self.lib.dsk_set_cosmology(self._h, float(omega_m), float(omega_lambda)))
 
     def kdk_reset(self):
         _check(self.lib.dsk_kdk_reset(self._h))

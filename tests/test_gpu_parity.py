@@ -340,6 +340,35 @@ def test_kdk_step(dsk, orc, periodic):
     d.close()
 
 
+def test_kdk_step_lcdm(dsk, orc):
+    """One periodic KDK step in the paper's cosmology (Omega_m 0.295, Omega_Lambda 0.705; reading O9b)
+    against the oracle step; and the invalid backgrounds are refused."""
+    rng = np.random.default_rng(11)
+    pos, mass = workloads.perturbed_lattice(12)
+    n = len(pos)
+    eps, a, da, cosmo = 1.0 / 480, 0.5, 0.01, (0.295, 0.705)
+    vel = (0.02 * rng.standard_normal((n, 3))).astype(np.float32)
+    d = dsk.Dsk(n, 1.0, True, eps, 0.5, 4)
+    d.set_cosmology(*cosmo)
+    tp, tv, tm = _dev(pos), _dev(vel), _dev(mass)
+    d.kdk_step(tp, tv, tm, a, da)
+    p1, v1, _ = orc.kdk_step(pos, vel, mass, 1.0, True, eps, 0.5, 4, a, da, cosmology=cosmo)
+    dx = np.abs(tp.cpu().numpy().astype(np.float64) - p1)
+    dx = np.minimum(dx, 1.0 - dx)
+    assert dx.max() < 3e-7
+    assert np.max(np.abs(tv.cpu().numpy() - v1)) < 2e-5 * np.abs(v1).max() + 1e-7
+    # the factors differ from Einstein-de Sitter by ~12 % here: the test would notice the wrong background
+    pe, _, _ = orc.kdk_step(pos, vel, mass, 1.0, True, eps, 0.5, 4, a, da)
+    de = np.abs(pe.astype(np.float64) - p1); de = np.minimum(de, 1.0 - de)
+    assert de.max() > 1e-5
+    with pytest.raises(Exception):
+        d.set_cosmology(0.0, 1.0)
+    d.set_cosmology(5.0, 0.0)                   # closed model, turns around at a = 1.25: H^2 < 0 beyond, refused
+    with pytest.raises(Exception):
+        d.kdk_step(tp, tv, tm, 1.3, 0.01)
+    d.close()
+
+
 # ---- full-size periodic configs, sampled (whole sink groups against the full oracle tree) ---------------
 def _group_sample(tree, order, nsink, seed):
     g = tree.groups()
