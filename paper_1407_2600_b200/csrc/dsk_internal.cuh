@@ -166,18 +166,8 @@ __device__ __forceinline__ f2 f2_make(float lo, float hi)
     return r;
 }
 __device__ __forceinline__ f2 f2_dup(float x) { return f2_make(x, x); }
-__device__ __forceinline__ float f2_lo(f2 a)
-{
-    float lo, hi;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.v));
-    return lo;
-}
-__device__ __forceinline__ float f2_hi(f2 a)
-{
-    float lo, hi;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.v));
-    return hi;
-}
+__device__ __forceinline__ float f2_lo(f2 a) { return __uint_as_float((unsigned int)(a.v & 0xffffffffull)); }
+__device__ __forceinline__ float f2_hi(f2 a) { return __uint_as_float((unsigned int)(a.v >> 32)); }
 __device__ __forceinline__ f2 f2_fma(f2 a, f2 b, f2 c)
 {
     f2 r;

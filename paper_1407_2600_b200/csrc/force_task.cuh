@@ -15,7 +15,7 @@
 #include <type_traits>
 
 
-// ---- T = f2 (two sources per op, packed f32x2) or float ----------------------------------------------
+// ---- T = f2 (two sinks per op, packed f32x2) or float ------------------------------------------------
 __device__ __forceinline__ f2 vfma(f2 a, f2 b, f2 c) { return f2_fma(a, b, c); }
 __device__ __forceinline__ f2 vmul(f2 a, f2 b) { return f2_mul(a, b); }
 __device__ __forceinline__ f2 vadd(f2 a, f2 b) { return f2_add(a, b); }
@@ -29,20 +29,6 @@ __device__ __forceinline__ float vrsqrt(float a) { return rsqrtf(a); }
 template <typename T> __device__ __forceinline__ T vdup(float x);
 template <> __device__ __forceinline__ f2 vdup<f2>(float x) { return f2_dup(x); }
 template <> __device__ __forceinline__ float vdup<float>(float x) { return x; }
-template <typename T> __device__ __forceinline__ T vld(const float2 *p, int half);
-template <> __device__ __forceinline__ f2 vld<f2>(const float2 *p, int)
-{
-    f2 r;
-    r.v = *reinterpret_cast<const unsigned long long *>(p);
-    return r;
-}
-template <> __device__ __forceinline__ float vld<float>(const float2 *p, int half)
-{
-    return reinterpret_cast<const float *>(p)[half];
-}
-__device__ __forceinline__ float vsum(f2 a) { return f2_lo(a) + f2_hi(a); }
-__device__ __forceinline__ float vsum(float a) { return a; }
-
 template <int I, int N, typename F>
 __device__ __forceinline__ void static_for(F &&f)
 {

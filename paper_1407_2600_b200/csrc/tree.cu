@@ -22,22 +22,6 @@ __global__ void k_tree_init(dsk_cellrec *cell, uint64_t *hotkey, uint32_t *paren
     for (int l = 2; l < DSK_KEY_LEVELS + 3; l++) st->lvl_start[l] = 1;
 }
 
-// boundaries of the 8 octants of a cell's range: b[o] = first rank whose child digit is >= o
-__device__ __forceinline__ void octant_bounds(const uint64_t *__restrict__ key, uint32_t first,
-                                              uint32_t count, int shift, uint32_t b[9])
-{
-    b[0] = first; b[8] = first + count;
-#pragma unroll
-    for (int o = 1; o < 8; o++) {
-        uint32_t lo = first, hi = first + count;
-        while (lo < hi) {
-            uint32_t mid = lo + ((hi - lo) >> 1);
-            if (((key[mid] >> shift) & 7ull) < (uint64_t)o) lo = mid + 1; else hi = mid;
-        }
-        b[o] = lo;
-    }
-}
-
 __device__ __forceinline__ void level_chunk(const dsk_devstate *st, int l, uint32_t &lo, uint32_t &hi)
 {
     uint32_t s = st->lvl_start[l], e = st->lvl_start[l + 1], n = e - s;
@@ -130,7 +114,6 @@ __device__ __forceinline__ void tree_emit_level(int l, const uint64_t *__restric
     }
     uint32_t lo, hi;
     level_chunk(st, l, lo, hi);
-    const int shift = 3 * (DSK_KEY_LEVELS - 1 - l);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint32_t carry = s_pre;
     __syncthreads();
