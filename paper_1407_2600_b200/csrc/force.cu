@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(FW * 32, 16) k_p2p(uint32_t t0, uint32_t t1, c
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // earlier generic reads of the buffer are done
         if (lane == 0) p2p_mbar_expect(&bar_all[warp][b], (min(lo + (uint32_t)P2P_TILE, L.total) - lo) * 16u);
         __syncwarp();
-        if (i1 > i0) p2p_bulk(src_all[warp][b] + (L.pref - lo) + i0, spos + L.first + i0, (i1 - i0) * 16u, &bar_all[warp][b]);
+        if (i1 > i0) p2p_bulk(src_all[warp][b] + ((L.pref + i0) - lo), spos + L.first + i0, (i1 - i0) * 16u, &bar_all[warp][b]);
     };
 
     if (lane == 0) { p2p_mbar_init(&bar_all[warp][0]); p2p_mbar_init(&bar_all[warp][1]); }
