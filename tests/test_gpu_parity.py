@@ -251,6 +251,43 @@ def test_forces_degenerate_inputs(dsk, orc):
         d.close()
 
 
+@pytest.mark.parametrize("seed", range(64))
+def test_forces_random_small_cases(dsk, orc, seed):
+    """Differential sweep over small random problems: N, clustering, periodicity, theta, p and eps drawn at
+    random; structure bit-exact, every particle's force and potential against the oracle tree."""
+    rng = np.random.default_rng(1000 + seed)
+    n = int(rng.choice([3, 31, 129, 257, 700, 1500, 3000, 9000]))
+    periodic = bool(rng.integers(2))
+    theta = float(rng.choice([0.3, 0.5, 0.7, 1.0]))
+    p = int(rng.choice([2, 4, 6, 8]))
+    kind = int(rng.integers(4))
+    if kind == 0:
+        pos = rng.random((n, 3))
+    elif kind == 1:                                        # a few tight clumps
+        c = rng.random((max(1, n // 200 + 1), 3))
+        pos = c[rng.integers(len(c), size=n)] + 0.01 * rng.standard_normal((n, 3))
+    elif kind == 2:                                        # a sheet
+        pos = rng.random((n, 3)); pos[:, 2] = 0.5 + 1e-3 * rng.standard_normal(n)
+    else:                                                  # clump + coincident pairs
+        pos = 0.5 + 0.05 * rng.standard_normal((n, 3)); pos[1::7] = pos[0::7][:len(pos[1::7])]
+    pos = (np.mod(pos, 1.0) if periodic else np.clip(pos, 0.0, 0.999999)).astype(np.float32)
+    pos[pos >= 1.0] = 0.0
+    mass = rng.uniform(0.2, 2.0, n).astype(np.float32) / n
+    eps = float(rng.choice([1e-2, 1e-3]))
+    d = dsk.Dsk(n, 1.0, periodic, eps, theta, p)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    _check_structure(orc, d, pos, mass, 1.0, periodic)
+    acc, pot = d.accel(tp, tm)
+    acc = acc.cpu().numpy().astype(np.float64); pot = pot.cpu().numpy().astype(np.float64)
+    ta, tpot, _, _, _ = orc.tree_force(pos, mass, 1.0, periodic, eps, theta, p)
+    scale = np.sqrt((ta ** 2).sum(1).mean())
+    err = np.linalg.norm(acc - ta, axis=1) / np.maximum(np.linalg.norm(ta, axis=1), 1e-3 * scale)
+    assert np.quantile(err, 0.999) < 2e-4 and err.max() < 2e-3, (n, periodic, theta, p, kind, np.quantile(err, 0.999), err.max())
+    assert np.max(np.abs(pot - tpot)) < 1e-4 * np.abs(tpot).max() + 1e-6
+    d.close()
+
+
 # ---- forces, periodic ---------------------------------------------------------------------------------
 def test_forces_periodic_lattice_scaled(dsk, orc):
     """configs[2] recipe at 32^3: Ewald direct sum on 192 sinks, oracle tree on 4096."""
