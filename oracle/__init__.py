@@ -127,7 +127,10 @@ class OracleTree:
 
     def __del__(self):
         if getattr(self, "_h", None):
-            lib().orc_tree_free(self._h)
+            try:
+                lib().orc_tree_free(self._h)
+            except TypeError:          # interpreter shutdown: the module globals are already gone
+                pass
             self._h = None
 
     def sorted(self):
