@@ -444,6 +444,10 @@ __global__ void __launch_bounds__(256) k_task_scatter(uint32_t t0, uint32_t t1, 
 // g_task_sorted[t0, t1) = the tasks of g_task[t0, t1) by descending (len[group] >> shift) / sub-groups
 int dsk_order_tasks(dsk_ctx *c, uint32_t t0, uint32_t t1, const uint32_t *len, int shift)
 {
+#ifdef DSK_NO_TASK_ORDER        // tuning experiments only: list (Morton) order
+    DSK_CUDA(cudaMemcpyAsync(c->g_task_sorted + t0, c->g_task + t0, sizeof(uint32_t) * (size_t)(t1 - t0), cudaMemcpyDeviceToDevice, c->stream));
+    return DSK_OK;
+#endif
     const unsigned nb = (t1 - t0 + 255) / 256;
     DSK_CUDA(cudaMemsetAsync(c->task_hist, 0, sizeof(uint32_t) * TASK_BINS, c->stream));
     k_task_hist<<<nb, 256, 0, c->stream>>>(t0, t1, c->g_task, c->gcount, len, shift, c->task_hist);
