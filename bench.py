@@ -337,7 +337,10 @@ def run_ours(args):
                             "traffic": traffic,
                             "peak_source": f"nominal FP32: {prop.multi_processor_count} SMs x 128 lanes x 2 x {sm_max:.0f} MHz "
                                            "(DESIGN.md; FFMA2 microbenchmark measured 74.06 TFLOP/s on this pool)",
-                            "flop_per_interaction": f_m2p, "interactions_per_launch": st["n_m2p"],
+                            "flop_per_interaction": f_m2p,
+                            "flop_per_interaction_survey_estimate": 8 * ((cfg["p"] + 1) * (cfg["p"] + 2) * (cfg["p"] + 3) // 6)
+                            + 5 * ((cfg["p"] + 2) * (cfg["p"] + 3) * (cfg["p"] + 4) // 6),
+                            "interactions_per_launch": st["n_m2p"],
                             "ms_per_launch": phase["ms_m2p"]},
                "kernels": {"p2p": {"TFLOPs": ach_p2p / 1e12, "frac_fp32_peak": ach_p2p / peak_fp32,
                                    "pairs_per_s": st["n_p2p"] / (phase["ms_p2p"] * 1e-3) if phase["ms_p2p"] > 0 else None,
