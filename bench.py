@@ -161,6 +161,11 @@ def run_reference(args):
     cfg, pos, mass = workload()
     n = len(pos)
     nsink = 16384
+    try:        # torchrun exports OMP_NUM_THREADS=1; the other ranks have left, this one takes the host's cores
+        import oracle
+        oracle.set_threads(len(os.sched_getaffinity(0)))
+    except Exception:
+        pass
     rates, info = [], None
     for it in range(args.warmup + args.steps):
         r, info = oracle_rate(cfg, pos, mass, nsink)
