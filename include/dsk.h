@@ -94,6 +94,12 @@ int dsk_build_tree(dsk_ctx *ctx, const float *pos, const float *mass);
  * PAPER.md:69-75 (lists, P2P, multipole interactions), :63 (periodic far field). */
 int dsk_accel(dsk_ctx *ctx, const float *pos, const float *mass, float *acc, float *pot);
 
+/* The same for an ACTIVE SUBSET of sinks: the force evaluation a hierarchical (block) time-step scheme needs
+ * ("adaptive symplectic integrator (Quinn et al. 1997)").  active dev uint8 [N],
+ * caller order: active[i] != 0 marks particle i as a sink; every particle remains a source.  Only sink groups that
+ * hold an active particle are walked and evaluated; acc/pot entries of inactive particles are left untouched. */
+int dsk_accel_active(dsk_ctx *ctx, const float *pos, const float *mass, const uint8_t *active, float *acc, float *pot);
+
 /* One kick-drift-kick step of the comoving leapfrog (O9), in place:
  * vel is the canonical momentum per unit mass a^2 dx/dt; periodic: Einstein-de Sitter factors from
  * the total mass in the box, positions wrapped to [0,box); isolated: Newtonian with dt = da.

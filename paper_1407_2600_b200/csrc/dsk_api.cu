@@ -56,6 +56,7 @@ static size_t carve(dsk_ctx *c, char *base)
     c->g_p2p_len = (uint32_t *)take(4 * ng);
     c->g_p2p_src = (uint32_t *)take(4 * ng);
     c->g_taskoff = (uint32_t *)take(4 * (ng + 1));
+    c->gact = (uint8_t *)take(ng);
     c->g_task = (uint32_t *)take(16 * ng);
     c->g_task_sorted = (uint32_t *)take(16 * ng);
     c->task_hist = (uint32_t *)take(4 * 1024);
@@ -215,9 +216,8 @@ extern "C" int dsk_build_tree(dsk_ctx *c, const float *pos, const float *mass)
     return DSK_OK;
 }
 
-extern "C" int dsk_accel(dsk_ctx *c, const float *pos, const float *mass, float *acc, float *pot)
+static int accel_impl(dsk_ctx *c, const uint8_t *active, float *acc, float *pot)
 {
-    (void)pos; (void)mass;
     if (!c || !acc) return DSK_EINVAL;
     if (!c->ws) return DSK_ENOWORKSPACE;
     if (!c->have_tree) return DSK_ENOTREE;
@@ -228,11 +228,20 @@ extern "C" int dsk_accel(dsk_ctx *c, const float *pos, const float *mass, float 
         DSK_CUDA(cudaStreamSynchronize(c->stream));
         c->stats.ms_upward = ev_ms(c->ev[5], c->ev[6]);
     }
+    c->gact_cur = nullptr;
+    if (active) {                                   // lists of an active subset are never reused
+        e = dsk_run_group_active(c, active);
+        if (e) return e;
+        c->gact_cur = c->gact;
+        c->lists_valid = 0;
+    }
     if (!(c->lists_valid && c->lists_theta == c->theta)) {
         e = dsk_run_walk(c);
-        if (e) return e;
+        if (e) { c->gact_cur = nullptr; return e; }
     }
     e = dsk_run_force(c, pot != nullptr);
+    c->gact_cur = nullptr;
+    if (active) c->lists_valid = 0;
     if (e) return e;
     cudaEventRecord(c->ev[12], c->stream);
     if (c->periodic) {
@@ -240,7 +249,7 @@ extern "C" int dsk_accel(dsk_ctx *c, const float *pos, const float *mass, float 
         if (e) return e;
     }
     cudaEventRecord(c->ev[13], c->stream);
-    e = dsk_run_scatter(c, acc, pot);
+    e = dsk_run_scatter(c, acc, pot, active);
     if (e) return e;
     cudaEventRecord(c->ev[14], c->stream);
     e = read_state(c);
@@ -249,6 +258,20 @@ extern "C" int dsk_accel(dsk_ctx *c, const float *pos, const float *mass, float 
     c->stats.n_p2p = (int64_t)c->hstate->n_p2p; c->stats.n_m2p = (int64_t)c->hstate->n_m2p;
     c->stats.list_m2p = (int64_t)c->hstate->tot_m2p_list; c->stats.list_p2p = (int64_t)c->hstate->tot_p2p_list;
     return e;
+}
+
+extern "C" int dsk_accel(dsk_ctx *c, const float *pos, const float *mass, float *acc, float *pot)
+{
+    (void)pos; (void)mass;
+    return accel_impl(c, nullptr, acc, pot);
+}
+
+extern "C" int dsk_accel_active(dsk_ctx *c, const float *pos, const float *mass, const uint8_t *active, float *acc,
+                                float *pot)
+{
+    (void)pos; (void)mass;
+    if (!active) return DSK_EINVAL;
+    return accel_impl(c, active, acc, pot);
 }
 
 // Leapfrog factors (O9 / O9b): H0^2 = (8 pi/3) M_tot / (box^3 Omega_m),

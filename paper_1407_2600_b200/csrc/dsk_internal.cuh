@@ -98,6 +98,8 @@ struct dsk_ctx {
     uint32_t *g_m2p_len, *g_p2p_len, *g_p2p_src;   // [ngroup_cap]
     uint32_t *g_taskoff;      // [ngroup_cap + 1] exclusive scan of dsk_task_parts(count)
     uint32_t *g_task;         // [4 * ngroup_cap] task -> group << 2 | part
+    uint8_t *gact;            // [ngroup_cap] group holds an active sink (dsk_accel_active)
+    const uint8_t *gact_cur;  // gact during an active-subset evaluation, else nullptr
     uint32_t *g_task_sorted;  // [4 * ngroup_cap] the tasks of the current batch, longest first (m2p.cu)
     uint32_t *task_hist;      // [1024] counting-sort bins
     uint64_t *g_m2p_off, *g_p2p_off;               // [ngroup_cap + 1] exclusive offsets into lists
@@ -134,7 +136,8 @@ struct dsk_ctx {
 
 // ---- internal entry points (one per source file) -------------------------------------------------
 int dsk_run_keysort(dsk_ctx *c, const float *pos, const float *mass);         // keysort.cu: K, S, gather
-int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot);                      // keysort.cu: X
+int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot, const uint8_t *active);   // keysort.cu: X
+int dsk_run_group_active(dsk_ctx *c, const uint8_t *active);                  // keysort.cu
 void dsk_exclusive_scan_u32(dsk_ctx *c, const uint32_t *in, uint32_t *out, const uint32_t *n_dev,
                             uint32_t n_max, uint32_t *total_dev);             // keysort.cu
 int dsk_run_build(dsk_ctx *c);                                                // tree.cu: T, G

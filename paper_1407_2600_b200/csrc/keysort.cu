@@ -259,11 +259,13 @@ __global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pos, c
 
 __global__ void __launch_bounds__(256) k_scatter(const float4 *__restrict__ sacc, const float4 *__restrict__ sacc_lo,
                                                  const uint32_t *__restrict__ order, int64_t n,
-                                                 float *__restrict__ acc, float *__restrict__ pot)
+                                                 float *__restrict__ acc, float *__restrict__ pot,
+                                                 const uint8_t *__restrict__ active)
 {
     int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n) return;
     uint32_t i = order[r];
+    if (active && !active[i]) return;            // dsk_accel_active: inactive entries are left untouched
     float4 a = sacc[r];
     const float4 l = sacc_lo[r];
     a.x = (float)((double)a.x + (double)l.x); a.y = (float)((double)a.y + (double)l.y);
@@ -298,10 +300,33 @@ int dsk_run_keysort(dsk_ctx *c, const float *pos, const float *mass)
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
-int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot)
+// one warp per group: does it hold a particle with active[caller index] != 0 ?
+__global__ void __launch_bounds__(256) k_group_active(const uint8_t *__restrict__ active, const uint32_t *__restrict__ order,
+                                                      const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
+                                                      uint32_t ngroup, uint8_t *__restrict__ gact)
+{
+    const uint32_t g = (blockIdx.x * 256 + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (g >= ngroup) return;
+    const uint32_t f = gfirst[g], n = gcount[g];
+    bool any = false;
+    for (uint32_t r = f + lane; r < f + n; r += 32) any |= active[order[r]] != 0;
+    any = __any_sync(0xffffffffu, any);
+    if (lane == 0) gact[g] = any ? 1 : 0;
+}
+
+int dsk_run_group_active(dsk_ctx *c, const uint8_t *active)
+{
+    const uint32_t ng = c->hstate->ngroup;
+    k_group_active<<<(unsigned)(((size_t)ng * 32 + 255) / 256), 256, 0, c->stream>>>(active, c->idx_a, c->gfirst, c->gcount, ng, c->gact);
+    DSK_COUNT(c, 1);
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
+}
+
+int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot, const uint8_t *active)
 {
     const int nb = (int)((c->N + 255) / 256);
-    k_scatter<<<nb, 256, 0, c->stream>>>(c->sacc, c->sacc_lo, c->idx_a, c->N, acc, pot);
+    k_scatter<<<nb, 256, 0, c->stream>>>(c->sacc, c->sacc_lo, c->idx_a, c->N, acc, pot, active);
     DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }

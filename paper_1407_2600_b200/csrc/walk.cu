@@ -31,12 +31,17 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
                                                   const uint64_t *__restrict__ m2p_off,
                                                   const uint64_t *__restrict__ p2p_off, uint64_t m2p_base,
                                                   uint64_t p2p_base, uint32_t *__restrict__ list_m2p,
-                                                  uint32_t *__restrict__ list_p2p, dsk_devstate *st)
+                                                  uint32_t *__restrict__ list_p2p, const uint8_t *__restrict__ gact,
+                                                  dsk_devstate *st)
 {
     __shared__ uint32_t stack[WW][WSTACK];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t g = g0 + blockIdx.x * WW + warp;
     if (g >= g1) return;
+    if (gact && !gact[g]) {                          // no active sink in this group (dsk_accel_active): empty lists
+        if (!FILL && lane == 0) { m2p_len[g] = 0; p2p_len[g] = 0; p2p_src[g] = 0; }
+        return;
+    }
     const float4 blo = gbox[2 * (size_t)g], bhi = gbox[2 * (size_t)g + 1];
     uint32_t *stk = stack[warp];
     const int nimg = periodic ? (2 * DSK_WS + 1) * (2 * DSK_WS + 1) * (2 * DSK_WS + 1) : 1;
@@ -213,7 +218,7 @@ int dsk_run_walk(dsk_ctx *c)
     k_walk<false><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic, c->box, c->cell, c->wmac,
                                                          c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len,
                                                          c->g_p2p_src, nullptr, nullptr, 0, 0, nullptr, nullptr,
-                                                         c->dstate);
+                                                         c->gact_cur, c->dstate);
     scan64(c, c->g_m2p_len, ng, c->g_m2p_off);
     scan64(c, c->g_p2p_len, ng, c->g_p2p_off);
     DSK_COUNT(c, 1);
@@ -225,7 +230,7 @@ int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint6
     k_walk<true><<<(g1 - g0 + WW - 1) / WW, WW * 32, 0, c->stream>>>(
         g0, g1, c->periodic, c->box, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len,
         c->g_p2p_len, c->g_p2p_src, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p,
-        c->dstate);
+        c->gact_cur, c->dstate);
     DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }

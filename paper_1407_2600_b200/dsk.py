@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libdsk.so")
 
 SYMBOLS = [
     "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
-    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_kdk_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_get_keys",
+    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_kdk_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_get_keys",
     "dsk_get_tree", "dsk_get_moments", "dsk_get_groups", "dsk_get_stats", "dsk_get_param",
     "dsk_get_lattice_tensors", "dsk_strerror",
 ]
@@ -58,6 +58,7 @@ def load_library(path=LIB_PATH):
     lib.dsk_set_params.argtypes = [vp, f32, f32, i32]
     lib.dsk_build_tree.argtypes = [vp, vp, vp]
     lib.dsk_accel.argtypes = [vp, vp, vp, vp, vp]
+    lib.dsk_accel_active.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.dsk_kdk_step.argtypes = [vp, vp, vp, vp, f64, f64]
     lib.dsk_kdk_reset.argtypes = [vp]
     lib.dsk_set_cosmology.argtypes = [vp, f64, f64]
@@ -164,6 +165,15 @@ class Dsk:
             pot = torch.empty(self.N, dtype=torch.float32, device=self.device)
         _check(self.lib.dsk_accel(self._h, _ptr(pos), _ptr(mass), _ptr(_dev_f32(acc, (self.N, 3))),
                                   _ptr(pot) if pot is not None else None))
+        return acc, pot
+
+    def accel_active(self, pos, mass, active, acc, pot=None):
+        """forces of the particles with active[i] != 0 (uint8 CUDA tensor [N]) written into acc/pot in place"""
+        _dev_f32(pos, (self.N, 3)); _dev_f32(mass, (self.N,)); _dev_f32(acc, (self.N, 3))
+        if not (active.is_cuda and active.dtype == torch.uint8 and active.is_contiguous() and active.numel() == self.N):
+            raise TypeError("active: contiguous uint8 CUDA tensor [N]")
+        _check(self.lib.dsk_accel_active(self._h, _ptr(pos), _ptr(mass), C.c_void_p(active.data_ptr()), _ptr(acc),
+                                         _ptr(pot) if pot is not None else None))
         return acc, pot
 
     def kdk_step(self, pos, vel, mass, a, da):

@@ -288,6 +288,43 @@ def test_forces_random_small_cases(dsk, orc, seed):
     d.close()
 
 
+@pytest.mark.parametrize("periodic", [False, True])
+def test_accel_active_subset(dsk, orc, periodic):
+    """dsk_accel_active: forces of an active subset (every particle still a source) equal the full evaluation's
+    for the active particles bit for bit, inactive entries stay untouched, and the work shrinks with the subset."""
+    pos, mass = (workloads.clustered_box(24, 20, cfg=4) if periodic else workloads.make(2, 1 / 32))
+    n = len(pos)
+    eps = 1e-3
+    d = dsk.Dsk(n, 1.0, periodic, eps, 0.5, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    full, fpot = d.accel(tp, tm)
+    n_full = d.get_stats()["n_m2p"]
+    rng = np.random.default_rng(3)
+    act = np.zeros(n, np.uint8)
+    act[rng.choice(n, n // 50, replace=False)] = 1                 # a sparse rung
+    k = n // 7
+    act[np.argsort(pos[:, 0])[:k]] = 1                             # and a slab
+    ta = torch.from_numpy(act).cuda()
+    acc = torch.full((n, 3), 7.0, dtype=torch.float32, device="cuda")
+    pot = torch.full((n,), -3.0, dtype=torch.float32, device="cuda")
+    d.accel_active(tp, tm, ta, acc, pot)
+    m = act.astype(bool)
+    assert torch.equal(acc[ta.bool()], full[ta.bool()]) and torch.equal(pot[ta.bool()], fpot[ta.bool()])
+    assert bool((acc[~ta.bool()] == 7.0).all()) and bool((pot[~ta.bool()] == -3.0).all())
+    assert d.get_stats()["n_m2p"] < 0.9 * n_full          # whole groups are evaluated: a sparse subset touches many
+    # against the oracle tree on a sample of the active sinks
+    sink = np.nonzero(m)[0][:: max(1, m.sum() // 400)]
+    ref = orc.tree_force(pos, mass, 1.0, periodic, eps, 0.5, 4, sink)[0]
+    a = acc.cpu().numpy().astype(np.float64)[sink]
+    rel = np.linalg.norm(a - ref, axis=1) / np.linalg.norm(ref, axis=1)
+    assert np.quantile(rel, 0.999) < 1e-4
+    # a full evaluation afterwards is unaffected by the subset run
+    again, _ = d.accel(tp, tm)
+    assert torch.equal(again, full)
+    d.close()
+
+
 # ---- forces, periodic ---------------------------------------------------------------------------------
 def test_forces_periodic_lattice_scaled(dsk, orc):
     """configs[2] recipe at 32^3: Ewald direct sum on 192 sinks, oracle tree on 4096."""
