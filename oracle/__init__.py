@@ -325,3 +325,67 @@ def kdk_step(pos, vel, mass, box, periodic, eps, theta, p, a, da, acc=None, forc
     acc = force(pos)
     vel = (vel.astype(np.float64) + acc * k2).astype(np.float32)
     return pos, vel, acc
+
+
+# ---- O9c: hierarchical (block) time steps --------------------------------------------------------------
+def _kick_factor(periodic, mtot, box, a1, a2, cosmology=None):
+    """K(a1, a2) = int dt/a over [a1, a2] (isolated: a2 - a1), through the O9/O9b factors."""
+    return kdk_factors(periodic, mtot, box, a1, 2.0 * (a2 - a1), cosmology)[0]
+
+
+def _drift_factor(periodic, mtot, box, a1, a2, cosmology=None):
+    return kdk_factors(periodic, mtot, box, a1, a2 - a1, cosmology)[1]
+
+
+def rung_wanted(acc, eps, da, eta, rmax):
+    """Rung the step criterion asks for, decided in fp32 (the precision the library decides it in):
+    step_i = eta sqrt(eps / |acc_i|), rung = ceil(log2(da / step_i)) clamped to [0, rmax]."""
+    a = acc.astype(np.float32)
+    amag = np.sqrt(a[:, 0] * a[:, 0] + a[:, 1] * a[:, 1] + a[:, 2] * a[:, 2], dtype=np.float32)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        step = np.float32(eta) * np.sqrt(np.float32(eps) / amag, dtype=np.float32)
+        r = np.ceil(np.log2(np.float32(da) / step, dtype=np.float32))
+    r = np.where(np.isfinite(r), r, 0.0)
+    return np.clip(r, 0, rmax).astype(np.int64)
+
+
+def kdk_block_step(pos, vel, mass, rung, box, periodic, eps, theta, p, a, da, rmax, eta, acc=None, cosmology=None):
+    """One block step of size da with power-of-two individual steps (reading O9c; "adaptive
+    symplectic integrator (Quinn et al. 1997)").  nsub = 2^rmax substeps h = da/nsub; a particle on rung r
+    takes steps of L(r) = nsub >> r substeps.  Per substep s: particles whose step starts at s get their
+    opening half kick K(a_s, a_s + L h/2); everybody drifts by D(a_s, a_s + h); the particles whose step ends
+    at t = s + 1 get new forces (all particles are sources) and their closing half kick K(a_t - L h/2, a_t);
+    then their rung follows the criterion: finer at once, coarser by one level and only when t is a multiple
+    of the coarser step.  Returns pos', vel', rung', acc' (forces of all particles at a + da)."""
+    pos = _f32(pos).copy(); vel = _f32(vel).copy(); mass = _f32(mass)
+    rung = np.asarray(rung, dtype=np.int64).copy()
+    n = len(pos)
+    mtot = float(np.sum(mass.astype(np.float64)))
+    nsub = 1 << rmax
+    h = da / nsub
+    if acc is None:
+        acc = tree_force(pos, mass, box, periodic, eps, theta, p)[0]
+    acc = np.array(acc, dtype=np.float64)
+    for s in range(nsub):
+        a_s = a + s * h
+        L = nsub >> rung
+        start = (s % L) == 0
+        K1 = np.array([_kick_factor(periodic, mtot, box, a_s, a_s + (nsub >> r) * h / 2, cosmology) for r in range(rmax + 1)])
+        vel[start] = (vel[start].astype(np.float64) + acc[start] * K1[rung[start]][:, None]).astype(np.float32)
+        d = _drift_factor(periodic, mtot, box, a_s, a_s + h, cosmology)
+        pos = (pos.astype(np.float64) + vel.astype(np.float64) * d).astype(np.float32)
+        if periodic:
+            pos = keys(pos, box, True)[1]
+        t = s + 1
+        a_t = a + t * h
+        act = (t % L) == 0
+        sink = np.nonzero(act)[0]
+        acc[sink] = tree_force(pos, mass, box, periodic, eps, theta, p, sink)[0]
+        K2 = np.array([_kick_factor(periodic, mtot, box, a_t - (nsub >> r) * h / 2, a_t, cosmology) for r in range(rmax + 1)])
+        vel[act] = (vel[act].astype(np.float64) + acc[act] * K2[rung[act]][:, None]).astype(np.float32)
+        want = rung_wanted(acc, eps, da, eta, rmax)
+        finer = act & (want > rung)
+        coarser = act & (want < rung) & (rung > 0) & ((t % (nsub >> np.maximum(rung - 1, 0))) == 0)
+        rung[finer] = want[finer]
+        rung[coarser] -= 1
+    return pos, vel, rung, acc

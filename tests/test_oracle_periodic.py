@@ -235,6 +235,40 @@ def test_kdk_factors_friedmann(orc):
             assert k1 > 0 and d > k1 + k2        # D integrand = K integrand / a, a < 1
 
 
+def test_kdk_block_step_pins(orc):
+    """O9c pins: rmax = 0 is the plain KDK step; all particles on the deepest rung is 2^rmax plain steps (bit for bit);
+    the rungs stay in range; and with the criterion switched on the block step lands closer to the all-fine
+    reference than the single coarse step does."""
+    from paper_1407_2600_b200 import workloads
+    pos, mass = workloads.make(2, 1 / 2048)
+    n = len(pos)
+    rng = np.random.default_rng(1)
+    vel = (3.0 * rng.standard_normal((n, 3))).astype(np.float32)
+    eps, da = 1e-3, 2e-4
+    p1, v1, a1 = orc.kdk_step(pos, vel, mass, 1.0, False, eps, 0.5, 4, 0.0, da)
+    p0, v0, r0, a0 = orc.kdk_block_step(pos, vel, mass, np.zeros(n), 1.0, False, eps, 0.5, 4, 0.0, da, 0, 0.1)
+    assert np.array_equal(p0, p1) and np.array_equal(v0, v1) and np.array_equal(a0, a1)
+    pf, vf, rf, _ = orc.kdk_block_step(pos, vel, mass, np.full(n, 2), 1.0, False, eps, 0.5, 4, 0.0, da, 2, 1e-9)
+    pp, vv, aa = pos, vel, None
+    for k in range(4):
+        pp, vv, aa = orc.kdk_step(pp, vv, mass, 1.0, False, eps, 0.5, 4, k * da / 4, da / 4, acc=aa)
+    assert np.array_equal(pf, pp) and np.array_equal(vf, vv) and rf.min() == 2 and rf.max() == 2
+    acc = orc.tree_force(pos, mass, 1.0, False, eps, 0.5, 4)[0]
+    eta = 0.08
+    rs = orc.rung_wanted(acc, eps, da, eta, 3)
+    assert len(np.unique(rs)) >= 3                                   # the case exercises several rungs
+    pa, va, ra, _ = orc.kdk_block_step(pos, vel, mass, rs, 1.0, False, eps, 0.5, 4, 0.0, da, 3, eta, acc=acc)
+    assert ra.min() >= 0 and ra.max() <= 3
+    pfine, vfine, _, _ = orc.kdk_block_step(pos, vel, mass, np.full(n, 3), 1.0, False, eps, 0.5, 4, 0.0, da, 3, 1e-9, acc=acc)
+    e_adapt = np.sqrt(((va - vfine) ** 2).sum() / (vfine ** 2).sum())
+    e_coarse = np.sqrt(((v1 - vfine) ** 2).sum() / (vfine ** 2).sum())
+    assert e_adapt < 0.5 * e_coarse, (e_adapt, e_coarse)
+    # fp32 criterion: a four times larger acceleration asks for exactly one rung more
+    a4 = np.array([[1.0, 0, 0], [4.0, 0, 0], [16.0, 0, 0]]) * 1.3e3
+    w = orc.rung_wanted(a4, eps, da, eta, 8)
+    assert w[1] == w[0] + 1 and w[2] == w[0] + 2
+
+
 def test_kdk_free_drift_and_time_reversal(orc):
     rng = np.random.default_rng(4)
     n = 200
