@@ -108,6 +108,16 @@ int dsk_accel_active(dsk_ctx *ctx, const float *pos, const float *mass, const ui
 int dsk_kdk_step(dsk_ctx *ctx, float *pos, float *vel, const float *mass, double a, double da);
 int dsk_kdk_reset(dsk_ctx *ctx);
 
+/* One BLOCK step of size da with hierarchical individual time steps (reading O9c of DESIGN.md; "adaptive
+ * symplectic integrator (Quinn et al. 1997)").  rung dev uint8 [N], in/out: particle i takes steps of da / 2^rung[i],
+ * 0 <= rung <= rmax <= 8.  The block is cut into 2^rmax substeps; per substep: opening half kicks of the particles whose
+ * step starts, drift of all, tree + forces of the particles whose step ends (dsk_accel_active), their closing half kicks,
+ * and their new rung from step_i = eta sqrt(eps / |acc_i|), rung = ceil(log2(da / step_i)) (decided in fp32; finer at
+ * once, coarser one level at a time and only when synchronised).  rmax = 0 is dsk_kdk_step.  Same state, cached force
+ * and factors as dsk_kdk_step. */
+int dsk_kdk_block_step(dsk_ctx *ctx, float *pos, float *vel, const float *mass, uint8_t *rung, double a, double da,
+                       int rmax, float eta);
+
 /* Background cosmology of the periodic leapfrog (the paper's runs use
  * Omega_m = 0.295, Omega_Lambda = 0.705).  H(a) = H0 sqrt(Omega_m a^-3 + (1 - Omega_m - Omega_Lambda) a^-2 + Omega_Lambda),
  * H0^2 = (8 pi/3) M_tot / (box^3 Omega_m); kick = int da/(a^2 H), drift = int da/(a^3 H), integrated on the host in

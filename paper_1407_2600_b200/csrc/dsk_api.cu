@@ -72,6 +72,7 @@ static size_t carve(dsk_ctx *c, char *base)
     c->list_m2p = (uint32_t *)take(4 * c->list_m2p_cap);
     c->list_p2p = (uint32_t *)take(4 * c->list_p2p_cap);
     c->kdk_acc = (float *)take(12 * n);
+    c->kdk_active = (uint8_t *)take(n);
     c->far_partial = (double *)take(8 * DSK_NFAR * 1024);
     c->far_M = (double *)take(8 * DSK_NFAR);
     c->far_T_dev = (double *)take(8 * DSK_NFAR);
@@ -312,6 +313,20 @@ static void kdk_factors(const dsk_ctx *c, double mtot, double a, double da, doub
     *d = gl16(a, a1, 3, c->omega_m, c->omega_l) / H0;
 }
 
+// K(a1, a2) = int dt/a, D(a1, a2) = int dt/a^2 over an arbitrary interval (isolated: a2 - a1)
+static double kick_factor(const dsk_ctx *c, double mtot, double a1, double a2)
+{
+    double k1, d, k2;
+    kdk_factors(c, mtot, a1, 2.0 * (a2 - a1), &k1, &d, &k2);
+    return k1;
+}
+static double drift_factor(const dsk_ctx *c, double mtot, double a1, double a2)
+{
+    double k1, d, k2;
+    kdk_factors(c, mtot, a1, a2 - a1, &k1, &d, &k2);
+    return d;
+}
+
 extern "C" int dsk_set_cosmology(dsk_ctx *c, double omega_m, double omega_lambda)
 {
     if (!c) return DSK_EINVAL;
@@ -370,6 +385,55 @@ extern "C" int dsk_kdk_step(dsk_ctx *c, float *pos, float *vel, const float *mas
     c->stats.ms_kdk = ev_ms(c->ev[15], c->ev[16]) + ev_ms(c->ev[17], c->ev[18]);
     c->stats.n_launch += 2;                      // the first kick and the drift (build_tree reset the counter)
     c->kdk_have_acc = 1;
+    return DSK_OK;
+}
+
+
+// One block step with hierarchical individual time steps (O9c).
+extern "C" int dsk_kdk_block_step(dsk_ctx *c, float *pos, float *vel, const float *mass, uint8_t *rung, double a,
+                                  double da, int rmax, float eta)
+{
+    if (!c || !pos || !vel || !mass || !rung) return DSK_EINVAL;
+    if (!c->ws) return DSK_ENOWORKSPACE;
+    if (rmax < 0 || rmax > DSK_RMAX || !(eta > 0.0f) || !(da > 0.0)) return DSK_EINVAL;
+    if (c->periodic && !(a > 0.0)) return DSK_EINVAL;
+    int e;
+    if (!c->kdk_have_acc) {
+        e = dsk_build_tree(c, pos, mass);
+        if (e) return e;
+        e = dsk_accel(c, pos, mass, c->kdk_acc, nullptr);
+        if (e) return e;
+        c->kdk_have_acc = 1;
+    }
+    float mroot = 0.0f;
+    DSK_CUDA(cudaMemcpyAsync(&mroot, c->rows + 8, sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    DSK_CUDA(cudaStreamSynchronize(c->stream));
+    const double mtot = (double)mroot;
+    const uint32_t nsub = 1u << rmax;
+    const double h = da / (double)nsub;
+    float kf[DSK_RMAX + 1];
+    for (uint32_t s = 0; s < nsub; s++) {
+        const double as = a + (double)s * h, at = a + (double)(s + 1) * h;
+        for (int r = 0; r <= DSK_RMAX; r++) kf[r] = r <= rmax ? (float)kick_factor(c, mtot, as, as + (double)(nsub >> r) * h * 0.5) : 0.0f;
+        e = dsk_run_kick_rung(c, vel, c->kdk_acc, rung, s, nsub, kf);
+        if (e) return e;
+        e = dsk_run_drift(c, pos, vel, (float)drift_factor(c, mtot, as, at));
+        if (e) return e;
+        c->kdk_have_acc = 0;
+        e = dsk_run_rung_active(c, rung, s + 1, nsub, c->kdk_active);
+        if (e) return e;
+        e = dsk_build_tree(c, pos, mass);
+        if (e) return e;
+        e = dsk_accel_active(c, pos, mass, c->kdk_active, c->kdk_acc, nullptr);
+        if (e) return e;
+        for (int r = 0; r <= DSK_RMAX; r++) kf[r] = r <= rmax ? (float)kick_factor(c, mtot, at - (double)(nsub >> r) * h * 0.5, at) : 0.0f;
+        e = dsk_run_kick_rung(c, vel, c->kdk_acc, rung, s + 1, nsub, kf);      // the same test: t % L == 0
+        if (e) return e;
+        e = dsk_run_rung_update(c, c->kdk_acc, c->kdk_active, rung, s + 1, nsub, rmax, (float)da, eta);
+        if (e) return e;
+    }
+    DSK_CUDA(cudaStreamSynchronize(c->stream));
+    c->kdk_have_acc = 1;          // t = nsub ends every rung's step: kdk_acc holds the forces of all particles
     return DSK_OK;
 }
 

@@ -16,6 +16,7 @@
 #define DSK_FAR_ORDER 8
 #define DSK_NFAR 165          // C(8+3,3)
 #define DSK_PMAX 8
+#define DSK_RMAX 8            // deepest rung of the block time steps: 256 substeps per block step
 #define DSK_IMG_BITS 7        // list entry = image << 25 | cell ... see below
 #define DSK_CELL_BITS 25
 #define DSK_FRTAB_BEG 320     // >= fr_nc(8) + 1 = 293
@@ -106,6 +107,7 @@ struct dsk_ctx {
     uint32_t *list_m2p, *list_p2p;
     size_t list_m2p_cap, list_p2p_cap;             // entries
     float *kdk_acc;           // [N,3] cached force, caller order
+    uint8_t *kdk_active;      // [N] particles whose step ends at the current substep (dsk_kdk_block_step)
     double *far_partial;      // [nblk * 165]
     double *far_M;            // [165]
     double *far_lambda;       // [165]
@@ -153,6 +155,11 @@ int dsk_run_farfield(dsk_ctx *c);                                             //
 void dsk_lattice_tensors(double L, int ws, double *T);                        // farfield.cu (host)
 int dsk_run_kick(dsk_ctx *c, float *vel, const float *acc, float k);          // kdk.cu
 int dsk_run_drift(dsk_ctx *c, float *pos, const float *vel, float d);         // kdk.cu
+int dsk_run_kick_rung(dsk_ctx *c, float *vel, const float *acc, const uint8_t *rung, uint32_t s, uint32_t nsub,
+                      const float *k);                                        // kdk.cu
+int dsk_run_rung_active(dsk_ctx *c, const uint8_t *rung, uint32_t t, uint32_t nsub, uint8_t *active);   // kdk.cu
+int dsk_run_rung_update(dsk_ctx *c, const float *acc, const uint8_t *active, uint8_t *rung, uint32_t t, uint32_t nsub,
+                        int rmax, float da, float eta);                       // kdk.cu
 
 // ---- packed f32x2 arithmetic (sm_100a: FFMA2 / FADD2 / FMUL2) ----------------------------------
 // One 64-bit register pair carries two independent fp32 lanes.  Measured on B200: scalar FFMA with

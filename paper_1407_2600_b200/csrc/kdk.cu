@@ -39,3 +39,73 @@ int dsk_run_drift(dsk_ctx *c, float *pos, const float *vel, float d)
     DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
+
+// ---- hierarchical (block) time steps (O9c; "adaptive symplectic integrator (Quinn et al.
+// 1997)") -------------------------------------------------------------------------------------------------
+// nsub = 2^rmax substeps per block step; a particle on rung r takes steps of L(r) = nsub >> r substeps.
+struct dsk_rung_factors { float k[DSK_RMAX + 1]; };
+
+// v += acc * k[rung] for the particles whose step starts (mode 0: s % L == 0) or ends (mode 1: active) now
+__global__ void __launch_bounds__(256) k_kick_rung(float *__restrict__ vel, const float *__restrict__ acc,
+                                                   const uint8_t *__restrict__ rung, int64_t n, uint32_t s,
+                                                   uint32_t nsub, dsk_rung_factors f)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t r = rung[i], L = nsub >> r;
+    if (s % L) return;
+    const float k = f.k[r];
+#pragma unroll
+    for (int d = 0; d < 3; d++) vel[3 * i + d] = fmaf(acc[3 * i + d], k, vel[3 * i + d]);
+}
+
+__global__ void __launch_bounds__(256) k_rung_active(const uint8_t *__restrict__ rung, int64_t n, uint32_t t,
+                                                     uint32_t nsub, uint8_t *__restrict__ active)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) active[i] = (t % (nsub >> rung[i])) == 0 ? 1 : 0;
+}
+
+// the step criterion, decided in fp32: step_i = eta sqrt(eps / |acc_i|), wanted rung = ceil(log2(da / step_i)) in
+// [0, rmax]; a particle that just ended a step moves to a finer rung at once, to a coarser one by one level and
+// only when t is a multiple of the coarser step
+__global__ void __launch_bounds__(256) k_rung_update(const float *__restrict__ acc, const uint8_t *__restrict__ active,
+                                                     uint8_t *__restrict__ rung, int64_t n, uint32_t t, uint32_t nsub,
+                                                     int rmax, float da, float eta, float eps)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || !active[i]) return;
+    const float ax = acc[3 * i], ay = acc[3 * i + 1], az = acc[3 * i + 2];
+    const float amag = __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(ax, ax), __fmul_rn(ay, ay)), __fmul_rn(az, az)));
+    const float step = __fmul_rn(eta, __fsqrt_rn(__fdiv_rn(eps, amag)));
+    const float w = ceilf(log2f(__fdiv_rn(da, step)));
+    int want = isfinite(w) ? (int)fminf(fmaxf(w, 0.0f), (float)rmax) : 0;
+    const int r = rung[i];
+    if (want > r) rung[i] = (uint8_t)want;
+    else if (want < r && r > 0 && (t % (nsub >> (r - 1))) == 0) rung[i] = (uint8_t)(r - 1);
+}
+
+int dsk_run_kick_rung(dsk_ctx *c, float *vel, const float *acc, const uint8_t *rung, uint32_t s, uint32_t nsub,
+                      const float *k)
+{
+    dsk_rung_factors f;
+    for (int r = 0; r <= DSK_RMAX; r++) f.k[r] = k[r];
+    k_kick_rung<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(vel, acc, rung, c->N, s, nsub, f);
+    DSK_COUNT(c, 1);
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
+}
+
+int dsk_run_rung_active(dsk_ctx *c, const uint8_t *rung, uint32_t t, uint32_t nsub, uint8_t *active)
+{
+    k_rung_active<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(rung, c->N, t, nsub, active);
+    DSK_COUNT(c, 1);
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
+}
+
+int dsk_run_rung_update(dsk_ctx *c, const float *acc, const uint8_t *active, uint8_t *rung, uint32_t t, uint32_t nsub,
+                        int rmax, float da, float eta)
+{
+    k_rung_update<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(acc, active, rung, c->N, t, nsub, rmax, da, eta, c->eps);
+    DSK_COUNT(c, 1);
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
+}

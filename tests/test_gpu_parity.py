@@ -443,6 +443,49 @@ def test_kdk_step_lcdm(dsk, orc):
     d.close()
 
 
+@pytest.mark.parametrize("periodic", [False, True])
+def test_kdk_block_step(dsk, orc, periodic):
+    """dsk_kdk_block_step (hierarchical time steps, reading O9c) against the oracle's block step: the rungs are integer
+    decisions taken in fp32 from forces that agree to ~1e-6, so a borderline particle may land on a neighbouring rung;
+    at least 99 % must agree, and those must agree in position and velocity."""
+    rng = np.random.default_rng(5)
+    if periodic:
+        pos, mass = workloads.clustered_box(8, 6, cfg=4)
+        eps, a, da, eta, vs = 1.0 / 320, 0.5, 0.01, 0.05, 0.02
+    else:
+        pos, mass = workloads.make(2, 1 / 2048)
+        eps, a, da, eta, vs = 1e-3, 0.0, 2e-4, 0.08, 3.0
+    n = len(pos)
+    vel = (vs * rng.standard_normal((n, 3))).astype(np.float32)
+    acc0 = orc.tree_force(pos, mass, 1.0, periodic, eps, 0.5, 4)[0]
+    r0 = orc.rung_wanted(acc0, eps, da, eta, 3)
+    assert len(np.unique(r0)) >= 2
+    d = dsk.Dsk(n, 1.0, periodic, eps, 0.5, 4)
+    tp, tv, tm = _dev(pos), _dev(vel), _dev(mass)
+    tr = torch.from_numpy(r0.astype(np.uint8)).cuda()
+    d.kdk_block_step(tp, tv, tm, tr, a, da, 3, eta)
+    p1, v1, r1, _ = orc.kdk_block_step(pos, vel, mass, r0, 1.0, periodic, eps, 0.5, 4, a, da, 3, eta, acc=acc0)
+    gr = tr.cpu().numpy().astype(np.int64)
+    same = gr == r1
+    assert same.mean() >= 0.99, same.mean()
+    dx = np.abs(tp.cpu().numpy().astype(np.float64) - p1)
+    if periodic:
+        dx = np.minimum(dx, 1.0 - dx)
+    dv = np.abs(tv.cpu().numpy().astype(np.float64) - v1)
+    assert dx[same].max() < 1e-6, dx[same].max()
+    assert dv[same].max() < 1e-4 * np.abs(v1).max() + 1e-7, dv[same].max()
+    # rmax = 0 is the plain step
+    d.kdk_reset()
+    tp2, tv2 = _dev(pos), _dev(vel)
+    tr2 = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    d.kdk_block_step(tp2, tv2, tm, tr2, a, da, 0, eta)
+    d.kdk_reset()
+    tp3, tv3 = _dev(pos), _dev(vel)
+    d.kdk_step(tp3, tv3, tm, a, da)
+    assert torch.equal(tp2, tp3) and torch.equal(tv2, tv3)
+    d.close()
+
+
 # ---- full-size periodic configs, sampled (whole sink groups against the full oracle tree) ---------------
 def _group_sample(tree, order, nsink, seed):
     g = tree.groups()
