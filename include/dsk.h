@@ -108,6 +108,11 @@ int dsk_accel_active(dsk_ctx *ctx, const float *pos, const float *mass, const ui
 int dsk_kdk_step(dsk_ctx *ctx, float *pos, float *vel, const float *mass, double a, double da);
 int dsk_kdk_reset(dsk_ctx *ctx);
 
+/* Diagnostic: mode 0 (default) lets the walk try its one-pass form (lists written into a fixed capacity per group,
+ * fallback to COUNT + FILL when one does not fit); mode 1 always takes the two-pass form; mode 2 gives the one-pass
+ * attempt capacities that overflow, so that every evaluation exercises the fallback.  Results are identical. */
+int dsk_set_walk_mode(dsk_ctx *ctx, int mode);
+
 /* One BLOCK step of size da with hierarchical individual time steps (reading O9c of DESIGN.md; "adaptive
  * symplectic integrator (Quinn et al. 1997)").  rung dev uint8 [N], in/out: particle i takes steps of da / 2^rung[i],
  * 0 <= rung <= rmax <= 8.  The block is cut into 2^rmax substeps; per substep: opening half kicks of the particles whose

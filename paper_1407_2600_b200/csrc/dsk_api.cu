@@ -100,6 +100,7 @@ extern "C" int dsk_create(dsk_ctx **out, int64_t N, float box, int periodic, flo
     c->N = N; c->box = box; c->periodic = periodic ? 1 : 0; c->eps = eps; c->theta = theta; c->p = p;
     c->moments_p = -1; c->p_cap = p; c->frow_tab_p = -1;
     c->omega_m = 1.0; c->omega_l = 0.0;
+    c->onepass_bad_theta = -1.0f;
     c->ws_bytes = 0;
     carve(c, nullptr);
     if (c->periodic) dsk_lattice_tensors((double)box, DSK_WS, c->far_T);
@@ -332,6 +333,14 @@ extern "C" int dsk_set_cosmology(dsk_ctx *c, double omega_m, double omega_lambda
     if (!c) return DSK_EINVAL;
     if (!(omega_m > 0.0) || !isfinite(omega_m) || !isfinite(omega_lambda)) return DSK_EINVAL;
     c->omega_m = omega_m; c->omega_l = omega_lambda;
+    return DSK_OK;
+}
+
+extern "C" int dsk_set_walk_mode(dsk_ctx *c, int mode)
+{
+    if (!c || mode < 0 || mode > 2) return DSK_EINVAL;
+    c->walk_two_pass_only = mode;
+    c->lists_valid = 0;
     return DSK_OK;
 }
 

@@ -123,6 +123,9 @@ struct dsk_ctx {
     int p_cap;                // order the workspace was sized for (dsk_create's p); set_params may lower p
     int frow_tab_p;           // order of the uploaded force-row map
     float lists_theta;
+    int walk_two_pass_only;   // dsk_set_walk_mode(1)
+    int walk_onepass;         // the lists of the current evaluation were written by the one-pass walk
+    float onepass_bad_theta;  // theta at which a list overflowed its fixed capacity (skip the one-pass attempt)
     double far_T[DSK_NFAR];
     dsk_stats stats;
     cudaEvent_t ev[20];

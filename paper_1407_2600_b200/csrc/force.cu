@@ -253,6 +253,17 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
         return DSK_OK;
     }
     c->stats.ms_walk = 0.0f;
+    if (c->walk_onepass) {                        // the lists are already there (walk.cu): one batch, no FILL pass
+        int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, want_pot, false);
+        if (e) return e;
+        DSK_CUDA(cudaStreamSynchronize(s));
+        add_ms(c->ev[7], c->ev[8], &c->stats.ms_walk);
+        add_ms(c->ev[8], c->ev[9], &c->stats.ms_p2p);
+        add_ms(c->ev[9], c->ev[10], &c->stats.ms_m2p);
+        c->stats.nbatch = 1;
+        c->lists_valid = 1; c->lists_theta = c->theta;
+        return DSK_OK;
+    }
     // totals of the COUNT pass
     uint64_t tot[2];
     DSK_CUDA(cudaMemcpyAsync(&tot[0], c->g_m2p_off + ng, sizeof(uint64_t), cudaMemcpyDeviceToHost, s));

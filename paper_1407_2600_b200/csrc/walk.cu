@@ -6,7 +6,8 @@
 // accepted -> M2P list; rejected leaf -> P2P list; rejected internal -> children are visited.
 // One warp per group, 32 cells tested per step from a LIFO stack in shared memory (depth-first order
 // keeps it short); list entries are compacted with ballots and written as contiguous runs.
-// Run twice: COUNT (list lengths, for the offsets) and FILL.
+// Run once into a fixed capacity per group when every list fits (the usual case), else twice: COUNT (list
+// lengths, for the offsets) and FILL.
 #include "dsk_internal.cuh"
 
 #define WW 1                 // warps (groups) per block: walks differ in length, a block ends with its longest
@@ -20,7 +21,7 @@ __device__ __forceinline__ void image_shift(int img, int periodic, float box, fl
     sh[0] = ix * box; sh[1] = iy * box; sh[2] = iz * box;
 }
 
-template <bool FILL>
+template <int MODE>          // 0 COUNT, 1 FILL at the scanned offsets, 2 ONE pass into a fixed capacity per group
 __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int periodic, float box,
                                                   const dsk_cellrec *__restrict__ cell,
                                                   const float4 *__restrict__ wmac,
@@ -32,14 +33,19 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
                                                   const uint64_t *__restrict__ p2p_off, uint64_t m2p_base,
                                                   uint64_t p2p_base, uint32_t *__restrict__ list_m2p,
                                                   uint32_t *__restrict__ list_p2p, const uint8_t *__restrict__ gact,
-                                                  dsk_devstate *st)
+                                                  uint32_t cap_m, uint32_t cap_p, uint64_t *__restrict__ m2p_off_out,
+                                                  uint64_t *__restrict__ p2p_off_out, dsk_devstate *st)
 {
+    constexpr bool FILL = MODE != 0;
     __shared__ uint32_t stack[WW][WSTACK];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t g = g0 + blockIdx.x * WW + warp;
     if (g >= g1) return;
     if (gact && !gact[g]) {                          // no active sink in this group (dsk_accel_active): empty lists
-        if (!FILL && lane == 0) { m2p_len[g] = 0; p2p_len[g] = 0; p2p_src[g] = 0; }
+        if (MODE != 1 && lane == 0) {
+            m2p_len[g] = 0; p2p_len[g] = 0; p2p_src[g] = 0;
+            if (MODE == 2) { m2p_off_out[g] = (uint64_t)g * cap_m; p2p_off_out[g] = (uint64_t)g * cap_p; }
+        }
         return;
     }
     const float4 blo = gbox[2 * (size_t)g], bhi = gbox[2 * (size_t)g + 1];
@@ -50,7 +56,8 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
     int sp = nimg;
     uint32_t nm = 0, np = 0, nsrc = 0;
     uint64_t mo = 0, po = 0;
-    if (FILL) { mo = m2p_off[g] - m2p_base; po = p2p_off[g] - p2p_base; }
+    if (MODE == 1) { mo = m2p_off[g] - m2p_base; po = p2p_off[g] - p2p_base; }
+    if (MODE == 2) { mo = (uint64_t)g * cap_m; po = (uint64_t)g * cap_p; }
     const uint32_t lt = (1u << lane) - 1u;
     while (sp > 0) {
         const int take = sp < 32 ? sp : 32;
@@ -82,8 +89,9 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
         const uint32_t bm = __ballot_sync(0xffffffffu, accept);
         const uint32_t bl = __ballot_sync(0xffffffffu, leaf);
         if (FILL) {
-            if (accept) list_m2p[mo + nm + __popc(bm & lt)] = e;
-            if (leaf) list_p2p[po + np + __popc(bl & lt)] = e;
+            const uint32_t im = nm + __popc(bm & lt), ip = np + __popc(bl & lt);
+            if (accept && (MODE == 1 || im < cap_m)) list_m2p[mo + im] = e;
+            if (leaf && (MODE == 1 || ip < cap_p)) list_p2p[po + ip] = e;
         }
         nm += __popc(bm); np += __popc(bl);
         if (leaf) nsrc += cnt;
@@ -109,9 +117,12 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
     }
     for (int o = 16; o; o >>= 1) nsrc += __shfl_xor_sync(0xffffffffu, nsrc, o);
     if (lane == 0) {
-        if (!FILL) {
-            m2p_len[g] = nm; p2p_len[g] = np; p2p_src[g] = nsrc;
-        } else {
+        if (MODE != 1) { m2p_len[g] = nm; p2p_len[g] = np; p2p_src[g] = nsrc; }
+        if (MODE == 2) {
+            m2p_off_out[g] = (uint64_t)g * cap_m; p2p_off_out[g] = (uint64_t)g * cap_p;
+            if (nm > cap_m || np > cap_p) st->scratch[0] = 1ull;      // a list did not fit: the host falls back to two passes
+        }
+        if (FILL) {
             const unsigned long long ns = gcount[g];
             atomicAdd(&st->n_m2p, ns * nm);
             atomicAdd(&st->n_p2p, ns * nsrc);
@@ -206,7 +217,9 @@ __global__ void __launch_bounds__(256) k_walk_mac(uint32_t ncell, float box, flo
     wmac[c] = h;
 }
 
-// W, COUNT pass + offsets.  The FILL pass is issued per batch by dsk_walk_fill (force.cu drives it).
+// W.  First choice: ONE pass into a fixed capacity per group (list buffer / number of groups), which saves the COUNT
+// pass and the scans whenever every list fits — checked with one flag read; a context that saw an overflow at this
+// theta goes straight to the general form: COUNT pass + offsets here, FILL per batch from dsk_walk_fill (force.cu).
 int dsk_run_walk(dsk_ctx *c)
 {
     const uint32_t ng = c->hstate->ngroup;
@@ -215,10 +228,30 @@ int dsk_run_walk(dsk_ctx *c)
     cudaEventRecord(c->ev[7], s);
     const uint32_t nc = c->hstate->ncell;
     k_walk_mac<<<(nc + 255) / 256, 256, 0, s>>>(nc, c->box, inv_theta, c->cell, c->whdr, c->wmac);
-    k_walk<false><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic, c->box, c->cell, c->wmac,
-                                                         c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len,
-                                                         c->g_p2p_src, nullptr, nullptr, 0, 0, nullptr, nullptr,
-                                                         c->gact_cur, c->dstate);
+    DSK_COUNT(c, 1);
+    c->walk_onepass = 0;
+    const uint64_t cap_m = ng ? c->list_m2p_cap / ng : 0, cap_p = ng ? c->list_p2p_cap / ng : 0;
+    const bool tiny = c->walk_two_pass_only == 2;          // diagnostic: capacities that overflow, to exercise the fallback
+    if (cap_m >= 4096 && cap_p >= 512 && (c->onepass_bad_theta != c->theta || tiny) && c->walk_two_pass_only != 1) {
+        DSK_CUDA(cudaMemsetAsync(&c->dstate->tot_m2p_list, 0, sizeof(unsigned long long) * 5, s));
+        DSK_CUDA(cudaMemsetAsync(&c->dstate->scratch[0], 0, sizeof(unsigned long long), s));
+        const uint32_t cm = tiny ? 64u : (uint32_t)(cap_m > 0xffffff00ull ? 0xffffff00ull : cap_m),
+                       cp = tiny ? 8u : (uint32_t)(cap_p > 0xffffff00ull ? 0xffffff00ull : cap_p);
+        k_walk<2><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic, c->box, c->cell, c->wmac, c->gbox, c->gcount,
+                                                         c->g_m2p_len, c->g_p2p_len, c->g_p2p_src, nullptr, nullptr, 0, 0,
+                                                         c->list_m2p, c->list_p2p, c->gact_cur, cm, cp, c->g_m2p_off,
+                                                         c->g_p2p_off, c->dstate);
+        DSK_COUNT(c, 1);
+        unsigned long long ovf = 0;
+        DSK_CUDA(cudaMemcpyAsync(&ovf, &c->dstate->scratch[0], sizeof(ovf), cudaMemcpyDeviceToHost, s));
+        DSK_CUDA(cudaStreamSynchronize(s));
+        if (!ovf) { c->walk_onepass = 1; return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA; }
+        c->onepass_bad_theta = c->theta;
+    }
+    k_walk<0><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic, c->box, c->cell, c->wmac,
+                                                     c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len,
+                                                     c->g_p2p_src, nullptr, nullptr, 0, 0, nullptr, nullptr,
+                                                     c->gact_cur, 0, 0, nullptr, nullptr, c->dstate);
     scan64(c, c->g_m2p_len, ng, c->g_m2p_off);
     scan64(c, c->g_p2p_len, ng, c->g_p2p_off);
     DSK_COUNT(c, 1);
@@ -227,10 +260,10 @@ int dsk_run_walk(dsk_ctx *c)
 
 int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base)
 {
-    k_walk<true><<<(g1 - g0 + WW - 1) / WW, WW * 32, 0, c->stream>>>(
+    k_walk<1><<<(g1 - g0 + WW - 1) / WW, WW * 32, 0, c->stream>>>(
         g0, g1, c->periodic, c->box, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len,
         c->g_p2p_len, c->g_p2p_src, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p,
-        c->gact_cur, c->dstate);
+        c->gact_cur, 0, 0, nullptr, nullptr, c->dstate);
     DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }

@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libdsk.so")
 
 SYMBOLS = [
     "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
-    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_get_keys",
+    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_get_keys",
     "dsk_get_tree", "dsk_get_moments", "dsk_get_groups", "dsk_get_stats", "dsk_get_param",
     "dsk_get_lattice_tensors", "dsk_strerror",
 ]
@@ -62,6 +62,7 @@ def load_library(path=LIB_PATH):
     lib.dsk_kdk_step.argtypes = [vp, vp, vp, vp, f64, f64]
     lib.dsk_kdk_block_step.argtypes = [vp, vp, vp, vp, vp, f64, f64, i32, f32]
     lib.dsk_kdk_reset.argtypes = [vp]
+    lib.dsk_set_walk_mode.argtypes = [vp, i32]
     lib.dsk_set_cosmology.argtypes = [vp, f64, f64]
     lib.dsk_get_keys.argtypes = [vp, vp, vp]
     lib.dsk_get_tree.argtypes = [vp, C.POINTER(i64), vp, vp, vp, vp]
@@ -187,6 +188,9 @@ class Dsk:
             raise TypeError("rung: contiguous uint8 CUDA tensor [N]")
         _check(self.lib.dsk_kdk_block_step(self._h, _ptr(pos), _ptr(vel), _ptr(mass), C.c_void_p(rung.data_ptr()),
                                            float(a), float(da), int(rmax), float(eta)))
+
+    def set_walk_mode(self, mode):
+        _check(self.lib.dsk_set_walk_mode(self._h, int(mode)))
 
     def set_cosmology(self, omega_m, omega_lambda):
         _check(self.lib.dsk_set_cosmology(self._h, float(omega_m), float(omega_lambda)))

@@ -325,6 +325,30 @@ def test_accel_active_subset(dsk, orc, periodic):
     d.close()
 
 
+@pytest.mark.parametrize("periodic", [False, True])
+def test_walk_one_pass_equals_two_pass(dsk, periodic):
+    """The one-pass walk (fixed list capacity per group) and the COUNT + FILL form give the same lists: forces,
+    potentials and interaction counts are bit-identical."""
+    pos, mass = (workloads.clustered_box(24, 20, cfg=4) if periodic else workloads.make(2, 1 / 16))
+    n = len(pos)
+    d = dsk.Dsk(n, 1.0, periodic, 1e-3, 0.4, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    a1, p1 = d.accel(tp, tm)
+    s1 = d.get_stats()
+    d.set_walk_mode(1)
+    a2, p2 = d.accel(tp, tm)
+    s2 = d.get_stats()
+    assert torch.equal(a1, a2) and torch.equal(p1, p2)
+    assert s1["n_m2p"] == s2["n_m2p"] and s1["n_p2p"] == s2["n_p2p"] and s1["list_m2p"] == s2["list_m2p"]
+    d.set_walk_mode(2)                       # one-pass attempt with capacities that overflow: the fallback runs
+    a3, p3 = d.accel(tp, tm)
+    s3 = d.get_stats()
+    assert torch.equal(a1, a3) and torch.equal(p1, p3)
+    assert s1["n_m2p"] == s3["n_m2p"] and s1["n_p2p"] == s3["n_p2p"] and s1["list_m2p"] == s3["list_m2p"]
+    d.close()
+
+
 # ---- forces, periodic ---------------------------------------------------------------------------------
 def test_forces_periodic_lattice_scaled(dsk, orc):
     """configs[2] recipe at 32^3: Ewald direct sum on 192 sinks, oracle tree on 4096."""
