@@ -18,6 +18,13 @@
 
 __constant__ uint8_t c_ea[UNP], c_eb[UNP], c_ec[UNP], c_rank[UNP];
 __device__ uint8_t g_ea[UNP], g_eb[UNP], g_ec[UNP], g_rank[UNP];   // the same tables for per-lane (divergent) indexing
+// M2M pair table of the current order: for moment n (visited heaviest first through g_m2m_perm) the entries
+// k <= n packed as k_index | (n-k).a << 8 | (n-k).b << 12 | (n-k).c << 16
+#define M2M_MAXPAIR 3003       // C(14, 6): pairs (k <= n, |n| <= 8)
+__device__ uint32_t g_m2m_ent[M2M_MAXPAIR];
+__device__ uint16_t g_m2m_beg[UNP + 1];
+__device__ uint8_t g_m2m_perm[UNP];
+static int g_m2m_p = -1;
 __constant__ float c_sgn_invfact[UNP];   // (-1)^|n| / (a! b! c!)
 __constant__ float c_invfact1[DSK_PMAX + 1];
 
@@ -52,6 +59,48 @@ static int upload_tables()
     return DSK_OK;
 }
 
+
+// pair table for order p (rebuilt when p changes; single stream of use: the upward pass of one context at a time)
+static int upload_m2m_table(int p, cudaStream_t s)
+{
+    if (g_m2m_p == p) return DSK_OK;
+    const int np = dsk_np(p);
+    static uint32_t ent[M2M_MAXPAIR];
+    static uint16_t beg[UNP + 1];
+    static uint8_t perm[UNP];
+    int cnt[UNP], ea[UNP], eb[UNP], ec[UNP];
+    for (int l = 0; l <= p; l++)
+        for (int a = l; a >= 0; a--)
+            for (int b = l - a; b >= 0; b--) {
+                const int c = l - a - b, i = dsk_midx(a, b, c);
+                ea[i] = a; eb[i] = b; ec[i] = c; cnt[i] = (a + 1) * (b + 1) * (c + 1);
+            }
+    int ne = 0;
+    for (int n = 0; n < np; n++) {
+        beg[n] = (uint16_t)ne;
+        for (int ka = 0; ka <= ea[n]; ka++)
+            for (int kb = 0; kb <= eb[n]; kb++)
+                for (int kc = 0; kc <= ec[n]; kc++)
+                    ent[ne++] = (uint32_t)dsk_midx(ka, kb, kc) | (uint32_t)(ea[n] - ka) << 8 | (uint32_t)(eb[n] - kb) << 12 |
+                                (uint32_t)(ec[n] - kc) << 16;
+    }
+    beg[np] = (uint16_t)ne;
+    for (int i = 0; i < np; i++) perm[i] = (uint8_t)i;
+    for (int i = 1; i < np; i++) {            // insertion sort, heaviest moment first: a warp's 32 lanes get similar work
+        const uint8_t v = perm[i];
+        int j = i;
+        while (j > 0 && cnt[perm[j - 1]] < cnt[v]) { perm[j] = perm[j - 1]; j--; }
+        perm[j] = v;
+    }
+    (void)s;
+    DSK_CUDA(cudaDeviceSynchronize());           // an upward pass of another order (any context) may still read the old table
+    DSK_CUDA(cudaMemcpyToSymbol(g_m2m_ent, ent, sizeof(uint32_t) * ne));
+    DSK_CUDA(cudaMemcpyToSymbol(g_m2m_beg, beg, sizeof(uint16_t) * (np + 1)));
+    DSK_CUDA(cudaMemcpyToSymbol(g_m2m_perm, perm, sizeof(uint8_t) * np));
+    g_m2m_p = p;
+    return DSK_OK;
+}
+
 __device__ __forceinline__ uint32_t compact3(uint64_t x)
 {   // every third bit -> 21 contiguous bits
     x &= 0x1249249249249249ull;
@@ -80,9 +129,8 @@ __device__ __forceinline__ float warp_sum(float v)
 
 // scratch of one warp
 template <int P> struct up_smem {
-    float crow[8][dsk_np(P)];     // the children's moments, pre-scaled by 2^-|k|
+    float crow[8][dsk_np(P) | 1]; // the children's moments, pre-scaled by 2^-|k| (odd stride: children on distinct banks)
     float pw[8][3][12];           // per child: e_d^j / j!
-    float out[dsk_np(P)];         // the parent's moments being summed
 };
 
 // multi-index helpers for compile-time unrolled monomials (same scheme as the M2P body)
@@ -186,21 +234,29 @@ __device__ __forceinline__ void upward_cell(uint32_t c, int level, float box, co
             const int k = i / NP, n = i - k * NP;
             sm.crow[k][n] = rows[(size_t)(r.child0 + k) * ROW + 8 + n] * exp2f(-(float)g_rank[n]);
         }
-        for (int n = lane; n < NP; n += 32) sm.out[n] = 0.0f;
         __syncwarp();
-        for (int i = lane; i < nchild * NP; i += 32) {
-            const int k = i / NP, n = i - k * NP;
-            const int a = g_ea[n], b = g_eb[n], cc = g_ec[n];
-            float sum = 0.0f;
-            for (int ka = 0; ka <= a; ka++)
-                for (int kb = 0; kb <= b; kb++) {
-                    const float pab = sm.pw[k][0][a - ka] * sm.pw[k][1][b - kb];
-                    for (int kc = 0; kc <= cc; kc++) sum += sm.crow[k][dsk_midx(ka, kb, kc)] * pab * sm.pw[k][2][cc - kc];
+        // lane = (moment slot, child): 4 moments per round, heaviest first so the 4 have similar pair counts; the
+        // pairs (k <= n) come from the table (no index arithmetic) and the 8 children are summed by 3 shuffles
+        {
+            const int ch = lane & 7;
+            const bool live = ch < nchild;
+            const float *cr = sm.crow[live ? ch : 0];
+            const float *px = sm.pw[live ? ch : 0][0], *py = sm.pw[live ? ch : 0][1], *pz = sm.pw[live ? ch : 0][2];
+            for (int q0 = 0; q0 < NP; q0 += 4) {
+                const int q = q0 + (lane >> 3);
+                const int n = g_m2m_perm[q < NP ? q : NP - 1];
+                const int t1 = (q < NP && live) ? g_m2m_beg[n + 1] : 0;
+                float sum = 0.0f;
+                for (int t = g_m2m_beg[n]; t < t1; t++) {
+                    const uint32_t e = g_m2m_ent[t];
+                    sum = fmaf(cr[e & 255u], px[(e >> 8) & 15u] * py[(e >> 12) & 15u] * pz[(e >> 16) & 15u], sum);
                 }
-            atomicAdd(&sm.out[n], sum);
+                sum += __shfl_xor_sync(0xffffffffu, sum, 1);
+                sum += __shfl_xor_sync(0xffffffffu, sum, 2);
+                sum += __shfl_xor_sync(0xffffffffu, sum, 4);
+                if (ch == 0 && q < NP) row[8 + n] = (n == 0) ? M : sum;
+            }
         }
-        __syncwarp();
-        for (int n = lane; n < NP; n += 32) row[8 + n] = (n == 0) ? M : sm.out[n];
         __syncwarp();
     }
     // ---- header + walk header ----
@@ -281,6 +337,8 @@ static int launch_upward(dsk_ctx *c, const uint32_t *lvl_start, int nlevel)
 int dsk_run_upward(dsk_ctx *c)
 {
     int e = upload_tables();
+    if (e) return e;
+    e = upload_m2m_table(c->p, c->stream);
     if (e) return e;
     const uint32_t *ls = c->hstate->lvl_start;
     int nl = (int)c->hstate->nlevel;
