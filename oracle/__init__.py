@@ -190,6 +190,8 @@ class OracleTree:
         return acc, pot, int(n_p2p.value), int(n_m2p.value)
 
     def list_counts(self, theta, g, ws=WS):
+        if self.p < 0:
+            self.moments(2)          # the MAC reads the centres of mass (any order fills them)
         a = C.c_int64(0); b = C.c_int64(0); c = C.c_int64(0)
         lib().orc_group_list_counts(self._h, C.c_double(theta), C.c_int(ws), C.c_int64(g), C.byref(a),
                                     C.byref(b), C.byref(c))

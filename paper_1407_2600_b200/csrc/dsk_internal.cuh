@@ -34,15 +34,62 @@ __host__ __device__ constexpr int dsk_midx(int a, int b, int c)
 // ctr = geometric cell centre (exact), off = com - ctr, Mhat_n = (-1)^|n| M_n / (n! s^|n|)
 __host__ __device__ constexpr int dsk_rowlen(int p) { return ((8 + dsk_np(p)) + 3) / 4 * 4; }
 
-// force tasks (force_task.cuh): two sinks per lane; number of tasks a group of n (1..64) sinks is cut into: maximise S(k)/k, S(k) = 32 / ceil(ceil(n/k)/2)
-__host__ __device__ __forceinline__ uint32_t dsk_task_parts(uint32_t n)
+// Force tasks (force_task.cuh): two sinks per lane, so a group of n <= NCRIT sinks is L = ceil(n/2) sink lanes wide.
+// A task (warp) takes w <= 32 of them and runs S = 32 / w sub-groups over alternate list entries; per list
+// entry it costs one body pass per S entries plus a fixed share of the tile staging.  The group is cut into at
+// most 4 tasks of widths w_1 + .. + w_k = L that minimise  sum_i (1/S_i + c)  (exact, by dynamic programming at
+// compile time; c = 40/960 from the measured ~240 staging instructions per 32-entry tile against 185 per body
+// pass).  Unequal widths matter: L = 33 is (1, 32), 33/32 of a pass per entry, where four equal parts cost 4/3.
+#define DSK_LMAX ((DSK_NCRIT + 1) / 2)
+#ifndef DSK_PART_COST
+#define DSK_PART_COST 40       // c in units of 1/960 of a body pass
+#endif
+static_assert(DSK_LMAX <= 128, "a group must fit 4 tasks of 32 sink lanes");
+struct dsk_parts_tab { uint32_t w[DSK_LMAX + 1]; };      // widths of the parts of L sink lanes, one byte each
+constexpr dsk_parts_tab dsk_make_parts_tab()
 {
-    uint32_t bk = 1, bs = 0;
-    for (uint32_t k = 1; k <= 4; k++) {
-        const uint32_t per = (n + k - 1) / k, w = (per + 1) / 2, s = w ? 32u / w : 0u;
-        if (k == 1 || s * bk > bs * k) { bk = k; bs = s; }
+    dsk_parts_tab t{};
+    const int INF = 1 << 28;
+    int best[5][DSK_LMAX + 1] = {}, pick[5][DSK_LMAX + 1] = {};
+    for (int L = 0; L <= DSK_LMAX; L++) best[0][L] = L ? INF : 0;
+    for (int k = 1; k <= 4; k++)
+        for (int L = 0; L <= DSK_LMAX; L++) {
+            best[k][L] = best[k - 1][L];                 // pick 0: fewer parts do as well
+            pick[k][L] = 0;
+            for (int w = 1; w <= 32 && w <= L; w++) {
+                const int v = 960 / (32 / w) + DSK_PART_COST + best[k - 1][L - w];
+                if (v < best[k][L]) { best[k][L] = v; pick[k][L] = w; }
+            }
+        }
+    for (int L = 0; L <= DSK_LMAX; L++) {
+        uint32_t word = 0;
+        int k = 4, rem = L, n = 0;
+        while (rem > 0) {
+            const int w = pick[k][rem];
+            k--;
+            if (w == 0) continue;
+            word |= (uint32_t)w << (8 * n);
+            n++;
+            rem -= w;
+        }
+        t.w[L] = word;
     }
-    return bk;
+    return t;
+}
+static __device__ const dsk_parts_tab dsk_parts_dev = dsk_make_parts_tab();
+// number of tasks of a group of n sinks, and the sink range [off, off + ns) of part `part`
+__device__ __forceinline__ uint32_t dsk_task_parts(uint32_t n)
+{
+    const uint32_t word = dsk_parts_dev.w[(n + 1u) >> 1];
+    return (word != 0u) + ((word >> 8) != 0u) + ((word >> 16) != 0u) + ((word >> 24) != 0u);
+}
+__device__ __forceinline__ void dsk_task_range(uint32_t n, uint32_t part, uint32_t &off, uint32_t &ns)
+{
+    const uint32_t word = dsk_parts_dev.w[(n + 1u) >> 1];
+    const uint32_t before = word & ((1u << (8u * part)) - 1u);            // widths of the parts before this one
+    const uint32_t lanes = (before & 255u) + ((before >> 8) & 255u) + ((before >> 16) & 255u);
+    off = 2u * lanes;
+    ns = min(2u * ((word >> (8u * part)) & 255u), n - off);
 }
 
 struct dsk_cellrec {          // 16 B, one LDG.128 in the walk

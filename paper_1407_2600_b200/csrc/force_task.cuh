@@ -67,11 +67,11 @@ __device__ __forceinline__ warp_task make_task(uint32_t t0, uint32_t t1, int fw,
     if (task >= t1) return t;
     const uint32_t m = taskmap[task], part = m & 3u;
     t.g = m >> 2;
-    const uint32_t count = gcount[t.g], k = dsk_task_parts(count);
-    const uint32_t base = count / k, rem = count % k;
+    uint32_t off, ns;
+    dsk_task_range(gcount[t.g], part, off, ns);
     t.valid = true;
-    t.ns = base + (part < rem ? 1u : 0u);
-    t.first = gfirst[t.g] + part * base + min(part, rem);
+    t.ns = ns;
+    t.first = gfirst[t.g] + off;
     t.W = (int)((t.ns + 1u) >> 1);
     t.S = 32 / t.W;
     t.sub = lane / t.W;

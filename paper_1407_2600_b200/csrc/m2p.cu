@@ -404,8 +404,10 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
 __device__ __forceinline__ uint32_t task_cost_bin(uint32_t m, const uint32_t *__restrict__ gcount,
                                                   const uint32_t *__restrict__ len, int shift)
 {
-    const uint32_t g = m >> 2, count = gcount[g], k = dsk_task_parts(count);
-    const uint32_t ns = (count + k - 1) / k, w = (ns + 1) >> 1, S = 32u / w;
+    const uint32_t g = m >> 2;
+    uint32_t soff, ns;
+    dsk_task_range(gcount[g], m & 3u, soff, ns);
+    const uint32_t w = (ns + 1) >> 1, S = 32u / w;
     const uint32_t cost = (len[g] + S - 1) / S;                      // body executions per lane
     return TASK_BINS - 1u - min((uint32_t)TASK_BINS - 1u, cost >> shift);
 }
