@@ -146,6 +146,10 @@ int dsk_get_groups(dsk_ctx *ctx, int64_t *ngroup, uint32_t *first, uint32_t *cou
 int dsk_get_stats(dsk_ctx *ctx, dsk_stats *out /* host */);
 /* library constants: "NLEAF", "NCRIT", "WS", "KEY_LEVELS", "FAR_ORDER"; host pointer. */
 int dsk_get_param(const char *name, double *value);
+/* How the force kernels cut a sink group of n (1..NCRIT) sinks into warp tasks: widths[k] =
+ * sink lanes (two sinks each) of task k, 0 for unused tasks; the widths sum to ceil(n/2), each <= 32.  Host pointer;
+ * DSK_EINVAL outside 1..NCRIT.  Introspection for tests and for the bench's accounting; no device work. */
+int dsk_get_task_widths(int n, int widths[4]);
 /* far-field lattice tensors T_n (|n| <= 8, 165 doubles, host) of this context; periodic only. */
 int dsk_get_lattice_tensors(dsk_ctx *ctx, double *T /* host [165] */);
 const char *dsk_strerror(int err);

@@ -537,6 +537,15 @@ extern "C" int dsk_get_param(const char *name, double *v)
     return DSK_OK;
 }
 
+extern "C" int dsk_get_task_widths(int n, int widths[4])
+{
+    static constexpr dsk_parts_tab tab = dsk_make_parts_tab();
+    if (!widths || n < 1 || n > DSK_NCRIT) return DSK_EINVAL;
+    const uint32_t word = tab.w[(n + 1) / 2];
+    for (int k = 0; k < 4; k++) widths[k] = (int)((word >> (8 * k)) & 255u);
+    return DSK_OK;
+}
+
 extern "C" int dsk_get_lattice_tensors(dsk_ctx *c, double *T)
 {
     if (!c || !T || !c->periodic) return DSK_EINVAL;

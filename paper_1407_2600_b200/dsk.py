@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libdsk.so")
 SYMBOLS = [
     "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
     "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_get_keys",
-    "dsk_get_tree", "dsk_get_moments", "dsk_get_groups", "dsk_get_stats", "dsk_get_param",
+    "dsk_get_tree", "dsk_get_moments", "dsk_get_groups", "dsk_get_stats", "dsk_get_param", "dsk_get_task_widths",
     "dsk_get_lattice_tensors", "dsk_strerror",
 ]
 
@@ -70,6 +70,7 @@ def load_library(path=LIB_PATH):
     lib.dsk_get_groups.argtypes = [vp, C.POINTER(i64), vp, vp, vp, vp, vp]
     lib.dsk_get_stats.argtypes = [vp, C.POINTER(DskStats)]
     lib.dsk_get_param.argtypes = [C.c_char_p, C.POINTER(f64)]
+    lib.dsk_get_task_widths.argtypes = [C.c_int, C.POINTER(C.c_int)]
     lib.dsk_get_lattice_tensors.argtypes = [vp, vp]
     lib.dsk_strerror.argtypes = [i32]
     lib.dsk_strerror.restype = C.c_char_p
@@ -84,6 +85,12 @@ def get_param(name):
     v = C.c_double(0)
     _check(load_library().dsk_get_param(name.encode(), C.byref(v)))
     return v.value
+
+
+def get_task_widths(n):
+    w = (C.c_int * 4)()
+    _check(load_library().dsk_get_task_widths(int(n), w))
+    return [int(x) for x in w if x]
 
 
 def _check(code):

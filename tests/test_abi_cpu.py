@@ -37,6 +37,37 @@ def test_constants_match_oracle_conventions(lib, orc):
         dsk.get_param("NOPE")
 
 
+def test_task_widths_cover_every_group_size(lib):
+    """Host logic of the force kernels' task split: for every group size the widths tile the sink
+    lanes exactly, respect the warp width, and no split of <= 4 parts is cheaper under the stated cost model."""
+    import functools
+    from paper_1407_2600_b200 import dsk
+    ncrit = int(dsk.get_param("NCRIT"))
+
+    def cost(w):                                       # 1/S + c in units of 1/960, S = sub-groups of a w-lane task
+        return 960 // (32 // w) + 40
+
+    @functools.lru_cache(None)
+    def best(lanes, k):
+        if lanes == 0:
+            return 0
+        if k == 0:
+            return 10 ** 9
+        return min(cost(w) + best(lanes - w, k - 1) for w in range(1, min(32, lanes) + 1))
+
+    for n in range(1, ncrit + 1):
+        w = dsk.get_task_widths(n)
+        lanes = (n + 1) // 2
+        assert 1 <= len(w) <= 4 and all(1 <= x <= 32 for x in w), (n, w)
+        assert sum(w) == lanes, (n, w)
+        assert sum(cost(x) for x in w) == best(lanes, 4), (n, w)
+    # the examples DESIGN.md quotes
+    assert sorted(dsk.get_task_widths(65)) == [1, 32] and sorted(dsk.get_task_widths(37)) == [3, 16]
+    for bad in (0, -1, ncrit + 1):
+        with pytest.raises(dsk.DskError):
+            dsk.get_task_widths(bad)
+
+
 def test_create_validation_and_workspace(lib):
     h = C.c_void_p(0)
     bad = [(0, 1.0, 0, 1e-3, 0.5, 4), (10, -1.0, 0, 1e-3, 0.5, 4), (10, 1.0, 0, 0.0, 0.5, 4),

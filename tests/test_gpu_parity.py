@@ -251,6 +251,40 @@ def test_forces_degenerate_inputs(dsk, orc):
         d.close()
 
 
+@pytest.mark.parametrize("periodic", [False, True])
+def test_forces_every_group_size(dsk, orc, periodic):
+    """One tight clump of n particles for every n = 1..NCRIT, each in its own cell of a coarse grid, so the sink
+    groups take every size (and with them every task split of DESIGN.md 5.1) while all clumps see each other as
+    M2P cells: structure bit-exact, every particle's force and potential against the oracle tree."""
+    ncrit = int(dsk.get_param("NCRIT"))
+    rng = np.random.default_rng(77)
+    cells = rng.permutation(8 ** 3)[:ncrit]                # clump k sits in cell cells[k] of an 8^3 grid
+    pos, sizes = [], np.arange(1, ncrit + 1)
+    for n, c in zip(sizes, cells):
+        ctr = (np.array([c // 64, (c // 8) % 8, c % 8]) + 0.5) / 8.0
+        pos.append(ctr + (rng.random((n, 3)) - 0.5) * 0.02)
+    pos = np.concatenate(pos).astype(np.float32)
+    n = len(pos)
+    mass = rng.uniform(0.5, 1.5, n).astype(np.float32) / n
+    eps, theta, p = 1e-3, 0.5, 4
+    d = dsk.Dsk(n, 1.0, periodic, eps, theta, p)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    t = _check_structure(orc, d, pos, mass, 1.0, periodic)
+    got = set(int(x) for x in t.groups()["count"])
+    assert len(got) >= ncrit * 2 // 3, len(got)            # most sizes appear as groups (neighbouring small clumps merge)
+    acc, pot = d.accel(tp, tm)
+    st = d.get_stats()
+    assert st["n_m2p"] > 0 and st["n_p2p"] > 0
+    acc = acc.cpu().numpy().astype(np.float64); pot = pot.cpu().numpy().astype(np.float64)
+    ta, tpot, _, _, _ = orc.tree_force(pos, mass, 1.0, periodic, eps, theta, p)
+    scale = np.sqrt((ta ** 2).sum(1).mean())
+    err = np.linalg.norm(acc - ta, axis=1) / np.maximum(np.linalg.norm(ta, axis=1), 1e-3 * scale)
+    assert err.max() < 1e-4, (err.max(), np.argmax(err))
+    assert np.max(np.abs(pot - tpot)) < 1e-5 * np.abs(tpot).max()
+    d.close()
+
+
 @pytest.mark.parametrize("seed", range(64))
 def test_forces_random_small_cases(dsk, orc, seed):
     """Differential sweep over small random problems: N, clustering, periodicity, theta, p and eps drawn at
