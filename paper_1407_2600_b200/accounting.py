@@ -14,7 +14,7 @@ def _rank(q):
 
 def m2p_ops(p, pot=True):
     """(ffma, fmul, fadd) per cell-particle interaction of k_m2p at order p (pairing form, m2p.cu)."""
-    ffma, fmul, fadd = 3, 3 + 1, 3          # R2 chain; rho = r * sinv, q = h0^2; r = x - com
+    ffma, fmul, fadd = 3 + 3, 1, 0          # R2 chain and rho = x * sinv - com'/s (one FMA each); q = h0^2
     fmul += 3 * (p - 1)                     # rho_i / k, k = 2..p
     for q in range(p + 1):
         if q >= 2 and not (q == p and p >= 3):
@@ -55,7 +55,7 @@ def m2p_ops(p, pot=True):
             fmul += 3
         elif m > 2:
             ffma += 3
-    fmul += 3                               # sinv^2, q tt, * -sinv^2
+    fmul += 2                               # q tt, * -sinv^2  (sinv^2 itself comes with the row)
     ffma += 6 + (1 if pot else 0)           # fold the cell's sums
     return ffma, fmul, fadd
 

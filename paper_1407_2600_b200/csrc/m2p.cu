@@ -114,8 +114,10 @@ int dsk_run_frows(dsk_ctx *c)
 // ---- F2 body: the lane's sink(s) against one cell ----------------------------------------------------
 // T = f2: two sinks in the halves of every register; T = float: one sink.  The cell's row is read from
 // shared memory as scalars (LDS.128 = four coefficients) that enter the packed ops as broadcast operands.
-// row (floats): [0..2] com' xyz (relative to the sink group's centre), [3] 1/s, [4] eps^2/s^2, [5] -1/s^2,
-//               [6] -1/s, [7] unused, [8+i] B_i
+// row (floats): [0..2] -com'/s xyz (com' relative to the sink group's centre), [3] 1/s, [4] eps^2/s^2, [5] -1/s^2,
+//               [6] -1/s, [7] 1/s^2, [8+i] B_i
+// rho = x/s - com'/s is one FMA per component; both terms are O(d/s) with no cancellation beyond the MAC's
+// separation, so this rounds like (x - com')/s.
 __host__ __device__ constexpr int mi_comp(MI j, int i) { return i == 0 ? j.a : (i == 1 ? j.b : j.c); }
 __host__ __device__ constexpr int mi_lower(MI j, int i)
 {
@@ -139,8 +141,8 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
     const float4 hA = *reinterpret_cast<const float4 *>(row), hB = *reinterpret_cast<const float4 *>(row + 4);
     const T sinv = vdup<T>(hA.w);
     T rho[3];
-    rho[0] = vmul(vsub(xs, vdup<T>(hA.x)), sinv); rho[1] = vmul(vsub(ys, vdup<T>(hA.y)), sinv);
-    rho[2] = vmul(vsub(zs, vdup<T>(hA.z)), sinv);
+    rho[0] = vfma(xs, sinv, vdup<T>(hA.x)); rho[1] = vfma(ys, sinv, vdup<T>(hA.y));
+    rho[2] = vfma(zs, sinv, vdup<T>(hA.z));
     T R2 = vfma(rho[0], rho[0], vdup<T>(hB.x));
     R2 = vfma(rho[1], rho[1], R2);
     R2 = vfma(rho[2], rho[2], R2);
@@ -230,7 +232,7 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
             g[0] = vfma(h, G[m][0], g[0]); g[1] = vfma(h, G[m][1], g[1]); g[2] = vfma(h, G[m][2], g[2]);
         }
     });
-    const T sinv2 = vmul(sinv, sinv);
+    const T sinv2 = vdup<T>(hB.w);
     const T u = vmul(vmul(qi, tt), vdup<T>(hB.y));
     ax = vfma(g[0], sinv2, ax); ay = vfma(g[1], sinv2, ay); az = vfma(g[2], sinv2, az);
     ax = vfma(rho[0], u, ax); ay = vfma(rho[1], u, ay); az = vfma(rho[2], u, az);
@@ -245,7 +247,7 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
 // instructions under ncu.)  The NEXT tile's rows are in flight while the current tile is evaluated and the
 // list entries one tile further ahead sit in a register, so no global-memory latency is exposed between tiles.
 // When a tile has arrived, one lane per cell rewrites the row's 8-float header in place (centre of mass relative
-// to the sink group's cell centre, image shift absorbed exactly; 1/s, eps^2/s^2, -1/s^2, -1/s) and the sub-groups
+// to the sink group's cell centre, image shift absorbed exactly, times -1/s; 1/s, eps^2/s^2, -1/s^2, -1/s, 1/s^2) and the sub-groups
 // run the body over alternate cells.
 // One task (warp) per block: tasks differ in length by more than 10x (list length, sub-group count), and a
 // multi-warp block holds its registers and shared memory until its longest warp ends.
@@ -335,9 +337,10 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
                 shx = (float)(img / (side * side) - DSK_WS) * box;
             }
             const float sinv = h0.w;
-            *reinterpret_cast<float4 *>(r) = make_float4(((h0.x - cgx) + shx) + h1.x, ((h0.y - cgy) + shy) + h1.y,
-                                                         ((h0.z - cgz) + shz) + h1.z, sinv);
-            *reinterpret_cast<float4 *>(r + 4) = make_float4(eps2 * sinv * sinv, -sinv * sinv, -sinv, 0.0f);
+            const float nsinv = -sinv, sinv2 = sinv * sinv;
+            *reinterpret_cast<float4 *>(r) = make_float4((((h0.x - cgx) + shx) + h1.x) * nsinv, (((h0.y - cgy) + shy) + h1.y) * nsinv,
+                                                         (((h0.z - cgz) + shz) + h1.z) * nsinv, sinv);
+            *reinterpret_cast<float4 *>(r + 4) = make_float4(eps2 * sinv2, -sinv2, nsinv, sinv2);
             if constexpr (M64) {
                 // the monopole of this cell is evaluated in fp64 below: centre of mass in double (the two
                 // differences are exact), mass out of the fp32 row
