@@ -45,18 +45,13 @@ def m2p_ops(p, pot=True):
                     ffma += 3
                 if qfirst_g != q:
                     fadd += 3               # merge with the lower blocks' gradient
-    fmul += 1                               # phi = h0 S_0
-    for m in range(1, p + 1):
-        fmul += 2                           # h_m, w = h_m S_m
-        ffma += 1                           # tt += (2m+1) w
-        if pot:
-            fadd += 1
-        if m == 2:
-            fmul += 3
-        elif m > 2:
-            ffma += 3
-    fmul += 2                               # q tt, * -sinv^2  (sinv^2 itself comes with the row)
-    ffma += 6 + (1 if pot else 0)           # fold the cell's sums
+    ffma += 2 * p - 1                       # Horner in q for Pq = sum S_m q^m and its derivative
+    fmul += 1; ffma += 1                    # Pq + 2 q Pq'
+    ffma += 3 * (p - 2)                     # Horner for the gradient sums G_p .. G_2
+    fmul += 3 + 3                           # u = (q (h0 * -1/s^2)) * tt ; k2 = (q (h0 / s^2)) q
+    ffma += 6                               # fold the cell's sums into the tile sums
+    if pot:
+        fmul += 1; ffma += 1
     return ffma, fmul, fadd
 
 

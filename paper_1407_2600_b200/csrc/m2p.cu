@@ -216,27 +216,26 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
             }
         });
     });
-    // pot = -(1/s) sum_m h_m S_m ;  acc_i = (1/s^2) [ sum_m h_m G_m,i - rho_i q sum_m (2m+1) h_m S_m ]
-    T h = h0;
-    T phi = vmul(h, S[0]);
-    T tt = phi;
-    T g[3];
-    static_for<1, P + 1>([&](auto M) {
-        constexpr int m = decltype(M)::value;
-        h = vmul(h, qi);
-        const T w = vmul(h, S[m]);
-        if constexpr (POT) phi = vadd(phi, w);
-        tt = vfma(w, vdup<T>((float)(2 * m + 1)), tt);
-        if constexpr (m == 2) { g[0] = vmul(h, G[m][0]); g[1] = vmul(h, G[m][1]); g[2] = vmul(h, G[m][2]); }
-        else if constexpr (m > 2) {
-            g[0] = vfma(h, G[m][0], g[0]); g[1] = vfma(h, G[m][1], g[1]); g[2] = vfma(h, G[m][2], g[2]);
-        }
+    // pot = -(1/s) sum_m h_m S_m ;  acc_i = (1/s^2) [ sum_m h_m G_m,i - rho_i q sum_m (2m+1) h_m S_m ],  h_m = h0 q^m.
+    // With Pq(q) = sum_m S_m q^m the last sum is h0 (Pq + 2 q Pq'), so value and derivative come from one Horner pass
+    // in q, and sum_m h_m G_m,i = h0 q^2 Horner(G_P,i .. G_2,i): 5P + 9 packed instructions instead of 7P + 7.
+    T pq = S[P], dq = S[P];
+    static_for<1, P + 1>([&](auto K) {
+        constexpr int m = P - decltype(K)::value;                 // P-1 .. 0
+        if constexpr (m < P - 1) dq = vfma(dq, qi, pq);
+        pq = vfma(pq, qi, S[m]);
     });
-    const T sinv2 = vdup<T>(hB.w);
-    const T u = vmul(vmul(qi, tt), vdup<T>(hB.y));
-    ax = vfma(g[0], sinv2, ax); ay = vfma(g[1], sinv2, ay); az = vfma(g[2], sinv2, az);
+    const T tt = vfma(vmul(dq, qi), vdup<T>(2.0f), pq);
+    T gh[3] = {G[P][0], G[P][1], G[P][2]};
+    static_for<1, P - 1>([&](auto K) {
+        constexpr int m = P - decltype(K)::value;                 // P-1 .. 2
+        gh[0] = vfma(gh[0], qi, G[m][0]); gh[1] = vfma(gh[1], qi, G[m][1]); gh[2] = vfma(gh[2], qi, G[m][2]);
+    });
+    const T u = vmul(vmul(qi, vmul(h0, vdup<T>(hB.y))), tt);       // -h0 q (Pq + 2 q Pq') / s^2
+    const T k2 = vmul(vmul(qi, vmul(h0, vdup<T>(hB.w))), qi);      // h0 q^2 / s^2
+    ax = vfma(gh[0], k2, ax); ay = vfma(gh[1], k2, ay); az = vfma(gh[2], k2, az);
     ax = vfma(rho[0], u, ax); ay = vfma(rho[1], u, ay); az = vfma(rho[2], u, az);
-    if constexpr (POT) pot = vfma(phi, vdup<T>(hB.z), pot);
+    if constexpr (POT) pot = vfma(vmul(pq, h0), vdup<T>(hB.z), pot);
 }
 
 // ---- F2 kernel ------------------------------------------------------------------------------------------
