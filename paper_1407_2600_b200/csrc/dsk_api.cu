@@ -41,7 +41,7 @@ static size_t carve(dsk_ctx *c, char *base)
     c->nchild_tmp = (uint32_t *)take(4 * nc);
     c->cbounds = (uint32_t *)take(32 * nc);
     c->whdr = (float4 *)take(16 * nc);
-    c->wmac = (float4 *)take(16 * nc);
+    c->wmac = (float4 *)take(32 * nc);     // MAC record + cell record per cell
     c->rows = (float *)take(4 * (size_t)dsk_rowlen(c->p_cap) * nc);
     c->frows = (float *)take(4 * (size_t)dsk_frow_len(c->p_cap) * nc);
     c->frtab_beg = (uint32_t *)take(4 * DSK_FRTAB_BEG);

@@ -10,8 +10,12 @@
 // lengths, for the offsets) and FILL.
 #include "dsk_internal.cuh"
 
+#ifndef WW
 #define WW 1                 // warps (groups) per block: walks differ in length, a block ends with its longest
+#endif
+#ifndef WSTACK
 #define WSTACK 2048          // stack entries per warp
+#endif
 
 __device__ __forceinline__ void image_shift(int img, int periodic, float box, float sh[3])
 {
@@ -71,7 +75,8 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
         if (act) {
             const uint32_t c = e & ((1u << DSK_CELL_BITS) - 1u);
             const int img = (int)(e >> DSK_CELL_BITS);
-            const float4 h = wmac[c];                      // com.xyz, critical radius s/theta + delta
+            const float4 h = wmac[2 * (size_t)c];          // com.xyz, critical radius s/theta + delta
+            const float4 rr = wmac[2 * (size_t)c + 1];     // the cell record (same sector)
             float sh[3];
             image_shift(img, periodic, box, sh);
             const float zx = h.x + sh[0], zy = h.y + sh[1], zz = h.z + sh[2];
@@ -80,9 +85,8 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
             const float dz = fmaxf(fmaxf(blo.z - zz, zz - bhi.z), 0.0f);
             const float d2 = dx * dx + dy * dy + dz * dz;
             accept = d2 > h.w * h.w;
-            if (!accept) {                                 // only a rejected cell needs its record
-                const dsk_cellrec r = cell[c];
-                nchild = r.meta & 255u; child0 = r.child0; cnt = r.count;
+            if (!accept) {
+                nchild = __float_as_uint(rr.w) & 255u; child0 = __float_as_uint(rr.z); cnt = __float_as_uint(rr.y);
                 leaf = nchild == 0;
             }
         }
@@ -203,7 +207,7 @@ static void scan64(dsk_ctx *c, const uint32_t *len, uint32_t n, uint64_t *off)
     DSK_COUNT(c, 2);
 }
 
-// the 16 bytes the MAC reads per tested cell: centre of mass and critical radius s/theta + delta
+// the 32 bytes the walk reads per tested cell: centre of mass and critical radius s/theta + delta | the cell record
 __global__ void __launch_bounds__(256) k_walk_mac(uint32_t ncell, float box, float inv_theta,
                                                   const dsk_cellrec *__restrict__ cell, const float4 *__restrict__ whdr,
                                                   float4 *__restrict__ wmac)
@@ -214,7 +218,12 @@ __global__ void __launch_bounds__(256) k_walk_mac(uint32_t ncell, float box, flo
     const int level = (int)(cell[c].meta >> 8);
     const float s = box * exp2f((float)-level);
     h.w = s * inv_theta + h.w;
-    wmac[c] = h;
+    wmac[2 * (size_t)c] = h;
+    // the cell record rides in the same 32-byte sector: a rejected cell needs it, and a second, dependent load would
+    // double the latency of every walk iteration
+    const dsk_cellrec r = cell[c];
+    wmac[2 * (size_t)c + 1] = make_float4(__uint_as_float(r.first), __uint_as_float(r.count), __uint_as_float(r.child0),
+                                          __uint_as_float(r.meta));
 }
 
 // W.  First choice: ONE pass into a fixed capacity per group (list buffer / number of groups), which saves the COUNT
