@@ -15,7 +15,7 @@ def _rank(q):
 def m2p_ops(p, pot=True):
     """(ffma, fmul, fadd) per cell-particle interaction of k_m2p at order p (pairing form, m2p.cu)."""
     ffma, fmul, fadd = 3 + 3, 1, 0          # R2 chain and rho = x * sinv - com'/s (one FMA each); q = h0^2
-    fmul += 3 * (p - 1)                     # rho_i / k, k = 2..p
+    fmul += 3 * (p - 1) if p < 3 else 3 * (p - 2) + 1   # rho_i / k, k = 2..p; for p >= 3 the top block needs q/p, not rho_i/p
     for q in range(p + 1):
         if q >= 2 and not (q == p and p >= 3):
             fmul += len(_rank(q))           # monomials of degree q (degree p is never read: its block uses Euler)

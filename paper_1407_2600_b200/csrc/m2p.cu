@@ -206,10 +206,13 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
                         });
                 });
                 if constexpr (EUL) {
-                    if constexpr (fr_qfirst_S(P, m) == q) S[m] = vmul(rd[0][q], Gt[0]);
-                    else S[m] = vfma(rd[0][q], Gt[0], S[m]);
-                    S[m] = vfma(rd[1][q], Gt[1], S[m]);
-                    S[m] = vfma(rd[2][q], Gt[2], S[m]);
+                    // the block of highest degree (q = m = P) is all of S_P: it is left as P S_P = rho . grad and the
+                    // 1/P goes into the Horner steps below, so rho_i / P is never formed
+                    constexpr int qd = (q == P) ? 1 : q;
+                    if constexpr (fr_qfirst_S(P, m) == q) S[m] = vmul(rd[0][qd], Gt[0]);
+                    else S[m] = vfma(rd[0][qd], Gt[0], S[m]);
+                    S[m] = vfma(rd[1][qd], Gt[1], S[m]);
+                    S[m] = vfma(rd[2][qd], Gt[2], S[m]);
                     if constexpr (fr_qfirst_G(P, m) == q) { G[m][0] = Gt[0]; G[m][1] = Gt[1]; G[m][2] = Gt[2]; }
                     else { G[m][0] = vadd(G[m][0], Gt[0]); G[m][1] = vadd(G[m][1], Gt[1]); G[m][2] = vadd(G[m][2], Gt[2]); }
                 }
@@ -219,11 +222,16 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
     // pot = -(1/s) sum_m h_m S_m ;  acc_i = (1/s^2) [ sum_m h_m G_m,i - rho_i q sum_m (2m+1) h_m S_m ],  h_m = h0 q^m.
     // With Pq(q) = sum_m S_m q^m the last sum is h0 (Pq + 2 q Pq'), so value and derivative come from one Horner pass
     // in q, and sum_m h_m G_m,i = h0 q^2 Horner(G_P,i .. G_2,i): 5P + 9 packed instructions instead of 7P + 7.
+    // (for P >= 3, S[P] holds P S_P: its two uses, the first step of each recurrence, multiply by q / P instead of q)
+    constexpr bool TOPEUL = P >= 3;
+    const T qs = TOPEUL ? vmul(qi, vdup<T>(1.0f / (float)P)) : qi;
     T pq = S[P], dq = S[P];
     static_for<1, P + 1>([&](auto K) {
         constexpr int m = P - decltype(K)::value;                 // P-1 .. 0
-        if constexpr (m < P - 1) dq = vfma(dq, qi, pq);
-        pq = vfma(pq, qi, S[m]);
+        if constexpr (m == P - 2) dq = vfma(dq, qs, pq);
+        else if constexpr (m < P - 2) dq = vfma(dq, qi, pq);
+        if constexpr (m == P - 1) pq = vfma(pq, qs, S[m]);
+        else pq = vfma(pq, qi, S[m]);
     });
     const T tt = vfma(vmul(dq, qi), vdup<T>(2.0f), pq);
     T gh[3] = {G[P][0], G[P][1], G[P][2]};

@@ -52,7 +52,7 @@ def test_accounting_matches_kernel_op_counts():
     import shutil
     import subprocess
     from paper_1407_2600_b200 import accounting, build
-    assert accounting.m2p_ops(4, pot=True) == (103, 45, 3)
+    assert accounting.m2p_ops(4, pot=True) == (103, 43, 3)
     assert accounting.p2p_flops(pot=True) == 19
     assert accounting.m2p_flops(4) > accounting.m2p_flops(2) and accounting.m2p_flops(8) > accounting.m2p_flops(6)
     assert abs(accounting.fp32_peak_flops(148, 1965.0) - 74.45e12) < 0.1e12
