@@ -24,7 +24,7 @@ def m2p_ops(p, pot=True):
                 continue
             qfirst_s = 0 if (m == 1 or 2 * m - p < 0) else 2 * m - p
             qfirst_g = max(1, 2 * m - p)
-            eul = (q == m and m >= 3)           # top block: value from the gradient (Euler), m2p.cu
+            eul = q >= 3                        # blocks of degree >= 3: value from the gradient (Euler), m2p.cu
             for jj, j in enumerate(_rank(q)):
                 if q > 0 and not eul:       # S_m += B mu_j  (q = 0: plain assignment)
                     if q == qfirst_s and jj == 0:

@@ -175,10 +175,10 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
             constexpr int m = decltype(M)::value;
             if constexpr (fr_has(P, q, m)) {
                 constexpr int off = fr_off(P, q, m);
-                // Top block of S_m (q = m, the homogeneous part of highest degree): by Euler's theorem
-                // sum_j B_j mu_j = (1/q) rho . grad, so only the gradient is accumulated (separately) and the
-                // value costs 3 FMAs instead of one per coefficient.
-                constexpr bool EUL = (q == m && m >= 3);
+                // A block is homogeneous of degree q, so by Euler's theorem sum_j B_j mu_j = (1/q) rho . grad: from
+                // degree 3 on (10 coefficients or more) only the gradient is accumulated (separately) and the value
+                // costs 3 FMAs (+ 3 adds to merge the gradient) instead of one FMA per coefficient.
+                constexpr bool EUL = (q >= 3);
                 T Gt[3];
                 static_for<0, fr_bsize(q)>([&](auto JJ) {
                     constexpr int jj = decltype(JJ)::value, ci = off + jj;
