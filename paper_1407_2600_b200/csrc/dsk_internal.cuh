@@ -169,6 +169,7 @@ struct dsk_ctx {
     double omega_m, omega_l;  // background cosmology of dsk_kdk_step (default 1, 0)
     int p_cap;                // order the workspace was sized for (dsk_create's p); set_params may lower p
     int frow_tab_p;           // order of the uploaded force-row map
+    uint32_t m2m_tab_mask;    // orders whose M2M pair table this context has uploaded (bit p/2 - 1)
     float lists_theta;
     int walk_two_pass_only;   // dsk_set_walk_mode(1)
     int walk_onepass;         // the lists of the current evaluation were written by the one-pass walk

@@ -18,13 +18,12 @@
 
 __constant__ uint8_t c_ea[UNP], c_eb[UNP], c_ec[UNP], c_rank[UNP];
 __device__ uint8_t g_ea[UNP], g_eb[UNP], g_ec[UNP], g_rank[UNP];   // the same tables for per-lane (divergent) indexing
-// M2M pair table of the current order: for moment n (visited heaviest first through g_m2m_perm) the entries
+// M2M pair tables, one per order p = 2, 4, 6, 8 (slot p/2 - 1): for moment n (visited heaviest first through g_m2m_perm) the entries
 // k <= n packed as k_index | (n-k).a << 8 | (n-k).b << 12 | (n-k).c << 16
 #define M2M_MAXPAIR 3003       // C(14, 6): pairs (k <= n, |n| <= 8)
-__device__ uint32_t g_m2m_ent[M2M_MAXPAIR];
-__device__ uint16_t g_m2m_beg[UNP + 1];
-__device__ uint8_t g_m2m_perm[UNP];
-static int g_m2m_p = -1;
+__device__ uint32_t g_m2m_ent[4][M2M_MAXPAIR];
+__device__ uint16_t g_m2m_beg[4][UNP + 1];
+__device__ uint8_t g_m2m_perm[4][UNP];
 __constant__ float c_sgn_invfact[UNP];   // (-1)^|n| / (a! b! c!)
 __constant__ float c_invfact1[DSK_PMAX + 1];
 
@@ -60,14 +59,16 @@ static int upload_tables()
 }
 
 
-// pair table for order p (rebuilt when p changes; single stream of use: the upward pass of one context at a time)
-static int upload_m2m_table(int p, cudaStream_t s)
+// pair table for order p: each context uploads it the first time it runs that order (the contents depend on p only, so
+// a second context writing the same bytes while another reads them is harmless; no state is shared on the host)
+static int upload_m2m_table(dsk_ctx *c, int p)
 {
-    if (g_m2m_p == p) return DSK_OK;
+    const int slot = p / 2 - 1;
+    if (c->m2m_tab_mask & (1u << slot)) return DSK_OK;
     const int np = dsk_np(p);
-    static uint32_t ent[M2M_MAXPAIR];
-    static uint16_t beg[UNP + 1];
-    static uint8_t perm[UNP];
+    uint32_t ent[M2M_MAXPAIR];
+    uint16_t beg[UNP + 1];
+    uint8_t perm[UNP];
     int cnt[UNP], ea[UNP], eb[UNP], ec[UNP];
     for (int l = 0; l <= p; l++)
         for (int a = l; a >= 0; a--)
@@ -92,12 +93,10 @@ static int upload_m2m_table(int p, cudaStream_t s)
         while (j > 0 && cnt[perm[j - 1]] < cnt[v]) { perm[j] = perm[j - 1]; j--; }
         perm[j] = v;
     }
-    (void)s;
-    DSK_CUDA(cudaDeviceSynchronize());           // an upward pass of another order (any context) may still read the old table
-    DSK_CUDA(cudaMemcpyToSymbol(g_m2m_ent, ent, sizeof(uint32_t) * ne));
-    DSK_CUDA(cudaMemcpyToSymbol(g_m2m_beg, beg, sizeof(uint16_t) * (np + 1)));
-    DSK_CUDA(cudaMemcpyToSymbol(g_m2m_perm, perm, sizeof(uint8_t) * np));
-    g_m2m_p = p;
+    DSK_CUDA(cudaMemcpyToSymbol(g_m2m_ent, ent, sizeof(uint32_t) * ne, sizeof(uint32_t) * M2M_MAXPAIR * slot));
+    DSK_CUDA(cudaMemcpyToSymbol(g_m2m_beg, beg, sizeof(uint16_t) * (np + 1), sizeof(uint16_t) * (UNP + 1) * slot));
+    DSK_CUDA(cudaMemcpyToSymbol(g_m2m_perm, perm, sizeof(uint8_t) * np, sizeof(uint8_t) * UNP * slot));
+    c->m2m_tab_mask |= 1u << slot;
     return DSK_OK;
 }
 
@@ -244,11 +243,11 @@ __device__ __forceinline__ void upward_cell(uint32_t c, int level, float box, co
             const float *px = sm.pw[live ? ch : 0][0], *py = sm.pw[live ? ch : 0][1], *pz = sm.pw[live ? ch : 0][2];
             for (int q0 = 0; q0 < NP; q0 += 4) {
                 const int q = q0 + (lane >> 3);
-                const int n = g_m2m_perm[q < NP ? q : NP - 1];
-                const int t1 = (q < NP && live) ? g_m2m_beg[n + 1] : 0;
+                const int n = g_m2m_perm[P / 2 - 1][q < NP ? q : NP - 1];
+                const int t1 = (q < NP && live) ? g_m2m_beg[P / 2 - 1][n + 1] : 0;
                 float sum = 0.0f;
-                for (int t = g_m2m_beg[n]; t < t1; t++) {
-                    const uint32_t e = g_m2m_ent[t];
+                for (int t = g_m2m_beg[P / 2 - 1][n]; t < t1; t++) {
+                    const uint32_t e = g_m2m_ent[P / 2 - 1][t];
                     sum = fmaf(cr[e & 255u], px[(e >> 8) & 15u] * py[(e >> 12) & 15u] * pz[(e >> 16) & 15u], sum);
                 }
                 sum += __shfl_xor_sync(0xffffffffu, sum, 1);
@@ -338,7 +337,7 @@ int dsk_run_upward(dsk_ctx *c)
 {
     int e = upload_tables();
     if (e) return e;
-    e = upload_m2m_table(c->p, c->stream);
+    e = upload_m2m_table(c, c->p);
     if (e) return e;
     const uint32_t *ls = c->hstate->lvl_start;
     int nl = (int)c->hstate->nlevel;
