@@ -163,29 +163,28 @@ __device__ __forceinline__ void sfor(F &&f)
         sfor<I + 1, N>(f);
     }
 }
-// (a) block partials of the root moments about the box centre, fp64.  One particle per lane: its 165 monomials
-// come from the power tables of x, y, z, each is summed over the warp with a butterfly and lane n % 32 keeps
-// the running sum of moment n (6 doubles per lane).  (The first version gave each of 165 threads one moment and
-// walked the particles serially: 3.9 ms at N = 2^21 against 0.17 ms for the evaluation.)
-__global__ void __launch_bounds__(FM_WARPS * 32) k_far_moments(const float4 *__restrict__ spos, uint32_t n,
-                                                               float half_box, double *__restrict__ partial)
+// (a) block partials of the root moments about the box centre, fp64.  A thread keeps running sums of a third of
+// the 165 moments (55 doubles) in registers over its particles and the block is reduced once at the end, so the inner
+// loop is one DFMA per moment and particle with no shuffles; the three thirds are blockIdx.y (positions are read three
+// times, 48 B per particle).  (Earlier forms: one moment per thread walking the particles serially, 3.9 ms at N = 2^21;
+// one particle per lane with a butterfly sum per monomial, 0.53 ms; this one 0.1 ms.)
+#define FM_PARTS 3
+#define FM_PER ((NF + FM_PARTS - 1) / FM_PARTS)
+template <int PART>
+__device__ __forceinline__ void far_moments_part(const float4 *__restrict__ spos, uint32_t n, float half_box,
+                                                 double *__restrict__ partial, double (*red)[FM_PER])
 {
-    constexpr int NSLOT = (NF + 31) / 32;
-    __shared__ double red[FM_WARPS][NF];
+    constexpr int LO = PART * FM_PER, HI = (LO + FM_PER < NF) ? LO + FM_PER : NF;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double acc[NSLOT];
+    double acc[FM_PER];
 #pragma unroll
-    for (int k = 0; k < NSLOT; k++) acc[k] = 0.0;
+    for (int k = 0; k < FM_PER; k++) acc[k] = 0.0;
     const uint32_t stride = gridDim.x * FM_WARPS * 32;
-    for (uint32_t i0 = (blockIdx.x * FM_WARPS + warp) * 32; i0 < n; i0 += stride) {   // whole warps stay together
-        const uint32_t i = i0 + lane;
+    for (uint32_t i = blockIdx.x * FM_WARPS * 32 + threadIdx.x; i < n; i += stride) {
+        const float4 p = spos[i];
+        const double X = (double)p.x - (double)half_box, Y = (double)p.y - (double)half_box, Z = (double)p.z - (double)half_box;
         double px[FO + 1], py[FO + 1], pz[FO + 1];
-        double m = 0.0, X = 0.0, Y = 0.0, Z = 0.0;
-        if (i < n) {
-            const float4 p = spos[i];
-            m = (double)p.w; X = (double)p.x - (double)half_box; Y = (double)p.y - (double)half_box; Z = (double)p.z - (double)half_box;
-        }
-        px[0] = m; py[0] = 1.0; pz[0] = 1.0;
+        px[0] = (double)p.w; py[0] = 1.0; pz[0] = 1.0;
 #pragma unroll
         for (int e = 1; e <= FO; e++) { px[e] = px[e - 1] * X; py[e] = py[e - 1] * Y; pz[e] = pz[e - 1] * Z; }
         sfor<0, FO + 1>([&](auto LL) {
@@ -195,24 +194,33 @@ __global__ void __launch_bounds__(FM_WARPS * 32) k_far_moments(const float4 *__r
                 sfor<0, k + 1>([&](auto CC) {
                     constexpr int c = decltype(CC)::value, b = k - c, a = l - k;
                     constexpr int idx = dsk_midx(a, b, c);
-                    double v = px[a] * (py[b] * pz[c]);
-#pragma unroll
-                    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-                    if (lane == (idx & 31)) acc[idx >> 5] += v;
+                    if constexpr (idx >= LO && idx < HI) acc[idx - LO] = fma(px[a], py[b] * pz[c], acc[idx - LO]);
                 });
             });
         });
     }
 #pragma unroll
-    for (int k = 0; k < NSLOT; k++)
-        if (k * 32 + lane < NF) red[warp][k * 32 + lane] = acc[k];
+    for (int k = 0; k < FM_PER; k++) {
+        double v = acc[k];
+#pragma unroll
+        for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) red[warp][k] = v;
+    }
     __syncthreads();
-    for (int t = threadIdx.x; t < NF; t += FM_WARPS * 32) {
+    for (int t = threadIdx.x; t < HI - LO; t += FM_WARPS * 32) {
         double sum = 0.0;
 #pragma unroll
         for (int w = 0; w < FM_WARPS; w++) sum += red[w][t];
-        partial[(size_t)blockIdx.x * NF + t] = sum;
+        partial[(size_t)blockIdx.x * NF + LO + t] = sum;
     }
+}
+__global__ void __launch_bounds__(FM_WARPS * 32, 1) k_far_moments(const float4 *__restrict__ spos, uint32_t n,
+                                                                  float half_box, double *__restrict__ partial)
+{
+    __shared__ double red[FM_WARPS][FM_PER];
+    if (blockIdx.y == 0) far_moments_part<0>(spos, n, half_box, partial, red);
+    else if (blockIdx.y == 1) far_moments_part<1>(spos, n, half_box, partial, red);
+    else far_moments_part<2>(spos, n, half_box, partial, red);
 }
 
 // (b) reduce partials, then Lambda_n = sum_{|k| <= 8-|n|} (-1)^|k| C(n+k,k) M_k T_{n+k}
@@ -260,26 +268,27 @@ __global__ void __launch_bounds__(128) k_far_eval(const float4 *__restrict__ spo
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float4 p = spos[i];
-    double px[FO + 1], py[FO + 1], pz[FO + 1];
-    px[0] = py[0] = pz[0] = 1.0;
     const double X = (double)p.x - (double)half_box, Y = (double)p.y - (double)half_box, Z = (double)p.z - (double)half_box;
-#pragma unroll
-    for (int e = 1; e <= FO; e++) { px[e] = px[e - 1] * X; py[e] = py[e - 1] * Y; pz[e] = pz[e - 1] * Z; }
+    // nested Horner, innermost in Z, each level carrying the derivatives it needs: 2 FMAs per coefficient in Z,
+    // 3 per (a, b) in Y, 4 per a in X (~410 DFMA per particle; the term-by-term form took ~1650 fp64 operations)
     double pot = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
-    sfor<0, FO + 1>([&](auto LL) {
-        constexpr int l = decltype(LL)::value;
-        sfor<0, l + 1>([&](auto KK) {
-            constexpr int k = decltype(KK)::value;          // k = b + c, a = l - k
-            sfor<0, k + 1>([&](auto CC) {
-                constexpr int c = decltype(CC)::value, b = k - c, a = l - k;
-                const double lam = sl[dsk_midx(a, b, c)];
-                const double yz = py[b] * pz[c];
-                pot = fma(lam * px[a], yz, pot);
-                if constexpr (a >= 1) gx = fma((double)a * lam * px[a - 1], yz, gx);
-                if constexpr (b >= 1) gy = fma((double)b * lam * px[a], py[b - 1] * pz[c], gy);
-                if constexpr (c >= 1) gz = fma((double)c * lam * px[a], py[b] * pz[c - 1], gz);
+    sfor<0, FO + 1>([&](auto AA) {
+        constexpr int a = FO - decltype(AA)::value;
+        double q = 0.0, qy = 0.0, qz = 0.0;
+        sfor<0, FO - a + 1>([&](auto BB) {
+            constexpr int b = FO - a - decltype(BB)::value, top = FO - a - b;
+            double v = sl[dsk_midx(a, b, top)], dv = 0.0;
+            sfor<0, top>([&](auto CC) {
+                constexpr int c = top - 1 - decltype(CC)::value;
+                if constexpr (c == top - 1) dv = v;
+                else dv = fma(dv, Z, v);
+                v = fma(v, Z, sl[dsk_midx(a, b, c)]);
             });
+            if constexpr (b == FO - a) { q = v; qz = dv; }
+            else { qy = fma(qy, Y, q); q = fma(q, Y, v); qz = fma(qz, Y, dv); }
         });
+        if constexpr (a == FO) { pot = q; gy = qy; gz = qz; }
+        else { gx = fma(gx, X, pot); pot = fma(pot, X, q); gy = fma(gy, X, qy); gz = fma(gz, X, qz); }
     });
     const float4 h = sacc[i], l = sacc_lo[i];
     const double tx = ((double)h.x + (double)l.x) - gx, ty = ((double)h.y + (double)l.y) - gy,
@@ -298,7 +307,7 @@ int dsk_run_farfield(dsk_ctx *c)
     const uint32_t n = (uint32_t)c->N;
     int nblk = c->nsm * 2;
     if ((int64_t)nblk * FM_WARPS * 32 > c->N) nblk = (int)((c->N + FM_WARPS * 32 - 1) / (FM_WARPS * 32));
-    k_far_moments<<<nblk, FM_WARPS * 32, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_partial);
+    k_far_moments<<<dim3(nblk, FM_PARTS), FM_WARPS * 32, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_partial);
     k_far_lambda<<<1, FM_THREADS, 0, c->stream>>>(c->far_partial, nblk, c->far_T_dev, c->far_M, c->far_lambda);
     k_far_eval<<<(n + 127) / 128, 128, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_lambda, c->sacc, c->sacc_lo);
     DSK_COUNT(c, 3);
