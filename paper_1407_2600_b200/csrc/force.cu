@@ -13,7 +13,12 @@
 #include "force_task.cuh"
 
 #define FW 1                 // warps (tasks) per block: tasks differ in length, see m2p.cu
-#define P2P_TILE 256         // sources per window (two windows per warp)
+#ifndef P2P_MINB
+#define P2P_MINB 16          // resident warps per SM the register budget is cut for
+#endif
+#ifndef P2P_TILE
+#define P2P_TILE 384         // sources per window (two windows per warp): 16 warps x 12 KB per SM; measured 256: 1.916 ms, 320: 1.890, 384: 1.872, 416: 1.874, 512: 1.898 (13 warps) on C2
+#endif
 
 int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base);   // walk.cu
 
@@ -61,11 +66,12 @@ __device__ __forceinline__ void p2p_bulk(void *dst, const void *src, uint32_t by
 
 struct leaf_batch {              // one leaf per lane
     uint32_t first, cnt, pref, total;
+    uint32_t mcnt;               // sources of the run that STARTS at my leaf (my leaf + the listed leaves after it that continue it in memory), else 0
     float shx, shy, shz;
 };
 
 template <bool POT>
-__global__ void __launch_bounds__(FW * 32, 16) k_p2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic, float box, float eps2,
+__global__ void __launch_bounds__(FW * 32, P2P_MINB) k_p2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic, float box, float eps2,
                                                  const dsk_cellrec *__restrict__ cell, const float4 *__restrict__ spos,
                                                  const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
                                                  const uint32_t *__restrict__ list,
@@ -85,20 +91,23 @@ __global__ void __launch_bounds__(FW * 32, 16) k_p2p(uint32_t t0, uint32_t t1, c
     const uint32_t *lst = list + (off[t.g] - base);
     sink_acc A;                                               // two-float running sums (see k_m2p)
     acc_zero(A);
+    const uint32_t sinv16 = (65536u + (uint32_t)t.S - 1u) / (uint32_t)t.S;    // n / S == (n * sinv16) >> 16 for n < 1024, S <= 32
 
     // cell records of the 32 leaves [b0, b0 + 32) of the list, their prefix sums and image shifts
     auto load_batch = [&](uint32_t b0) {
         leaf_batch L;
         L.first = 0; L.cnt = 0; L.shx = L.shy = L.shz = 0.0f;
+        uint32_t img = 0;
         if (b0 + lane < n) {
             const uint32_t e = lst[b0 + lane];
+            img = e >> DSK_CELL_BITS;
             const dsk_cellrec r = cell[e & ((1u << DSK_CELL_BITS) - 1u)];
             L.first = r.first; L.cnt = r.count;
             if (periodic) {
-                const int img = (int)(e >> DSK_CELL_BITS), side = 2 * DSK_WS + 1;
-                L.shz = (float)(img % side - DSK_WS) * box;
-                L.shy = (float)((img / side) % side - DSK_WS) * box;
-                L.shx = (float)(img / (side * side) - DSK_WS) * box;
+                const int im = (int)img, side = 2 * DSK_WS + 1;
+                L.shz = (float)(im % side - DSK_WS) * box;
+                L.shy = (float)((im / side) % side - DSK_WS) * box;
+                L.shx = (float)(im / (side * side) - DSK_WS) * box;
             }
         }
         uint32_t x = L.cnt;
@@ -108,6 +117,16 @@ __global__ void __launch_bounds__(FW * 32, 16) k_p2p(uint32_t t0, uint32_t t1, c
         }
         L.total = __shfl_sync(0xffffffffu, x, 31);
         L.pref = x - L.cnt;
+        // Runs: the walk emits sibling leaves next to each other, and siblings are neighbours in the sorted array, so
+        // a leaf that starts where the previous lane's leaf ends (same image) continues its run and ONE bulk copy
+        // moves the whole run (the copies are issued one lane at a time, ~10 instructions each).
+        const uint32_t pend = __shfl_up_sync(0xffffffffu, L.first + L.cnt, 1), pimg = __shfl_up_sync(0xffffffffu, img, 1);
+        const bool head = L.cnt != 0u && (lane == 0 || pend != L.first || pimg != img);
+        const uint32_t heads = __ballot_sync(0xffffffffu, head);
+        const uint32_t above = lane < 31 ? heads >> (lane + 1) : 0u;
+        const int nh = above ? lane + __ffs((int)above) : 31;              // lane of the next run's first leaf
+        const uint32_t npref = __shfl_sync(0xffffffffu, L.pref, nh);
+        L.mcnt = head ? (above ? npref : L.total) - L.pref : 0u;
         return L;
     };
     // my part of window [lo, lo + P2P_TILE) of batch L: particles [i0, i1) of my leaf
@@ -119,8 +138,8 @@ __global__ void __launch_bounds__(FW * 32, 16) k_p2p(uint32_t t0, uint32_t t1, c
     // copy window [lo, lo + P2P_TILE) of batch L into buffer b: one cp.async.bulk per leaf run (a per-particle
     // LDGSTS loop kept 3.8 of 32 lanes busy and made 16 % of the kernel's instructions)
     auto issue = [&](const leaf_batch &L, uint32_t lo, int b) {
-        uint32_t i0, i1;
-        my_part(L, lo, i0, i1);
+        const uint32_t hiw = min(lo + (uint32_t)P2P_TILE, L.total), ew = min(L.pref + L.mcnt, hiw);
+        const uint32_t i0 = max(L.pref, lo) - L.pref, i1 = ew > L.pref ? ew - L.pref : 0u;      // my run's part of the window
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // earlier generic reads of the buffer are done
         if (lane == 0) p2p_mbar_expect(&bar_all[warp][b], (min(lo + (uint32_t)P2P_TILE, L.total) - lo) * 16u);
         __syncwarp();
@@ -172,7 +191,7 @@ __global__ void __launch_bounds__(FW * 32, 16) k_p2p(uint32_t t0, uint32_t t1, c
             // my sub-group's sources: src[sub], src[sub + S], ...; pointer stepping keeps index arithmetic out of the loop
             const float4 *q = src + t.sub;
             const int S1 = t.S, S2 = 2 * t.S, S3 = 3 * t.S, S4 = 4 * t.S;
-            int left = ((int)nt - t.sub + t.S - 1) / t.S;
+            int left = (int)(((nt - (uint32_t)t.sub + (uint32_t)t.S - 1u) * sinv16) >> 16);   // = ceil((nt - sub) / S), nt <= 256
             for (; left >= 4; left -= 4, q += S4) {
                 const float4 s0 = q[0], s1 = q[S1], s2 = q[S2], s3 = q[S3];
                 pair(s0); pair(s1); pair(s2); pair(s3);

@@ -373,26 +373,33 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
                 // O(M/L^2) each and cancel to a net force hundreds of times smaller, so their fp32 rounding
                 // (1e-7 of each term) alone exceeds the 1e-4 per-particle gate (measured on C3: p99.9 = 6e-4).
                 const double e2d = (double)eps2;
-#pragma unroll
-                for (int h = 0; h < 2; h++) {
-                    const double xs = (double)(h ? mb.x : ma.x) - (double)cgx, ys = (double)(h ? mb.y : ma.y) - (double)cgy,
-                                 zs = (double)(h ? mb.z : ma.z) - (double)cgz;
-                    double sx = 0.0, sy = 0.0, sz = 0.0, sp = 0.0;
-                    for (int k = t.sub; k < ntc; k += t.S) {
-                        const double2 c01 = *reinterpret_cast<const double2 *>(mono + 4 * k);
-                        const double2 c23 = *reinterpret_cast<const double2 *>(mono + 4 * k + 2);
-                        const double dx = c01.x - xs, dy = c01.y - ys, dz = c23.x - zs;
-                        // 1/sqrt in double: fp32 MUFU seed (1e-7) + one Newton step (1.5e-14)
-                        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, e2d)));
-                        const double y0 = (double)rsqrtf((float)r2);
-                        const double ri = y0 * fma(-0.5 * r2, y0 * y0, 1.5);
-                        const double mri = c23.y * ri, mri3 = mri * ri * ri;
-                        sx = fma(dx, mri3, sx); sy = fma(dy, mri3, sy); sz = fma(dz, mri3, sz);
-                        sp -= mri;
-                    }
-                    acc_add_double(A, h, 0, sx); acc_add_double(A, h, 1, sy); acc_add_double(A, h, 2, sz);
-                    if (POT) acc_add_double(A, h, 3, sp);
+                // both sinks in one pass over the cells, two cells per trip: four independent chains (the chain
+                // difference -> r2 -> MUFU seed -> Newton -> products is ~150 cycles long and one at a time left the
+                // fp64 pipe 7 % busy while the warp waited)
+                const double xs0 = (double)ma.x - (double)cgx, ys0 = (double)ma.y - (double)cgy, zs0 = (double)ma.z - (double)cgz;
+                const double xs1 = (double)mb.x - (double)cgx, ys1 = (double)mb.y - (double)cgy, zs1 = (double)mb.z - (double)cgz;
+                double s0[4] = {0.0, 0.0, 0.0, 0.0}, s1[4] = {0.0, 0.0, 0.0, 0.0};
+                auto mono1 = [&](int k, double xs, double ys, double zs, double *sm) {
+                    const double2 c01 = *reinterpret_cast<const double2 *>(mono + 4 * k);
+                    const double2 c23 = *reinterpret_cast<const double2 *>(mono + 4 * k + 2);
+                    const double dx = c01.x - xs, dy = c01.y - ys, dz = c23.x - zs;
+                    // 1/sqrt in double: fp32 MUFU seed (1e-7) + one Newton step (1.5e-14)
+                    const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, e2d)));
+                    const double y0 = (double)rsqrtf((float)r2);
+                    const double ri = y0 * fma(-0.5 * r2, y0 * y0, 1.5);
+                    const double mri = c23.y * ri, mri3 = mri * ri * ri;
+                    sm[0] = fma(dx, mri3, sm[0]); sm[1] = fma(dy, mri3, sm[1]); sm[2] = fma(dz, mri3, sm[2]);
+                    sm[3] -= mri;
+                };
+                int k = t.sub;
+                for (; k + t.S < ntc; k += 2 * t.S) {
+                    mono1(k, xs0, ys0, zs0, s0); mono1(k, xs1, ys1, zs1, s1);
+                    mono1(k + t.S, xs0, ys0, zs0, s0); mono1(k + t.S, xs1, ys1, zs1, s1);
                 }
+                if (k < ntc) { mono1(k, xs0, ys0, zs0, s0); mono1(k, xs1, ys1, zs1, s1); }
+                acc_add_double(A, 0, 0, s0[0]); acc_add_double(A, 0, 1, s0[1]); acc_add_double(A, 0, 2, s0[2]);
+                acc_add_double(A, 1, 0, s1[0]); acc_add_double(A, 1, 1, s1[1]); acc_add_double(A, 1, 2, s1[2]);
+                if (POT) { acc_add_double(A, 0, 3, s0[3]); acc_add_double(A, 1, 3, s1[3]); }
             }
         }
         if (t.active) {
