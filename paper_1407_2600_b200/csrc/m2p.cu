@@ -259,6 +259,7 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
 // One task (warp) per block: tasks differ in length by more than 10x (list length, sub-group count), and a
 // multi-warp block holds its registers and shared memory until its longest warp ends.
 #define FW 1
+#define M64_MINB 12          // resident warps per SM of the fp64-monopole variants at p <= 4 (164 registers; at 16 they spill: C3 19.05 vs 18.78 ms)
 template <int P, bool M64> struct m2p_cfg {
     static constexpr int NCELL = (P <= 4) ? 32 : (P == 6 ? 16 : 8);   // cells per tile
     static constexpr int LPC = 32 / NCELL;                             // lanes that share the copy of one row
@@ -278,7 +279,7 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 template <int P, bool POT, bool M64>
-__global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic,
+__global__ void __launch_bounds__(FW * 32, (P <= 4 ? (M64 ? M64_MINB : 16) : 1)) k_m2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic,
                                                  float box, float eps2, const float *__restrict__ frows,
                                                  const float4 *__restrict__ spos, const uint32_t *__restrict__ gfirst,
                                                  const uint32_t *__restrict__ gcount, const uint32_t *__restrict__ gcell,
@@ -367,44 +368,42 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? 16 : 1)) k_m2p(uint32_t t0,
             const uint32_t b2 = b0 + 2u * tc;
             e_nxt = (mycell < (int)tc && b2 + mycell < n) ? lst[b2 + mycell] : 0u;
         }
-        if constexpr (M64) {
-            if (t.active) {
+        if (t.active) {
+            f2 pot = f2_dup(0.0f), ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f);
+            if constexpr (M64) {
                 // Monopoles in fp64.  In a periodic, nearly uniform box the image block's monopole terms are
                 // O(M/L^2) each and cancel to a net force hundreds of times smaller, so their fp32 rounding
                 // (1e-7 of each term) alone exceeds the 1e-4 per-particle gate (measured on C3: p99.9 = 6e-4).
+                // The fp64 monopole of a cell rides in the same loop trip as its fp32 body: the chain difference ->
+                // r2 -> MUFU seed (1e-7) -> one Newton step (1.5e-14) -> products is ~150 cycles long and hides under the
+                // ~150 independent packed fp32 instructions of the same warp (other pipes).  As a pass of its own,
+                // one chain at a time: C3 19.9 ms, C4 641; four chains: 19.2, 602; in the body's loop: 18.8, 596.
                 const double e2d = (double)eps2;
-                // both sinks in one pass over the cells, two cells per trip: four independent chains (the chain
-                // difference -> r2 -> MUFU seed -> Newton -> products is ~150 cycles long and one at a time left the
-                // fp64 pipe 7 % busy while the warp waited)
                 const double xs0 = (double)ma.x - (double)cgx, ys0 = (double)ma.y - (double)cgy, zs0 = (double)ma.z - (double)cgz;
                 const double xs1 = (double)mb.x - (double)cgx, ys1 = (double)mb.y - (double)cgy, zs1 = (double)mb.z - (double)cgz;
                 double s0[4] = {0.0, 0.0, 0.0, 0.0}, s1[4] = {0.0, 0.0, 0.0, 0.0};
-                auto mono1 = [&](int k, double xs, double ys, double zs, double *sm) {
-                    const double2 c01 = *reinterpret_cast<const double2 *>(mono + 4 * k);
-                    const double2 c23 = *reinterpret_cast<const double2 *>(mono + 4 * k + 2);
+                auto mono1 = [&](const double2 c01, const double2 c23, double xs, double ys, double zs, double *sm) {
                     const double dx = c01.x - xs, dy = c01.y - ys, dz = c23.x - zs;
-                    // 1/sqrt in double: fp32 MUFU seed (1e-7) + one Newton step (1.5e-14)
                     const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, e2d)));
                     const double y0 = (double)rsqrtf((float)r2);
                     const double ri = y0 * fma(-0.5 * r2, y0 * y0, 1.5);
                     const double mri = c23.y * ri, mri3 = mri * ri * ri;
                     sm[0] = fma(dx, mri3, sm[0]); sm[1] = fma(dy, mri3, sm[1]); sm[2] = fma(dz, mri3, sm[2]);
-                    sm[3] -= mri;
+                    if (POT) sm[3] -= mri;
                 };
-                int k = t.sub;
-                for (; k + t.S < ntc; k += 2 * t.S) {
-                    mono1(k, xs0, ys0, zs0, s0); mono1(k, xs1, ys1, zs1, s1);
-                    mono1(k + t.S, xs0, ys0, zs0, s0); mono1(k + t.S, xs1, ys1, zs1, s1);
+                for (int k = t.sub; k < ntc; k += t.S) {
+                    const double2 c01 = *reinterpret_cast<const double2 *>(mono + 4 * k);
+                    const double2 c23 = *reinterpret_cast<const double2 *>(mono + 4 * k + 2);
+                    mono1(c01, c23, xs0, ys0, zs0, s0);
+                    mono1(c01, c23, xs1, ys1, zs1, s1);
+                    m2p_body<P, f2, POT>(X, Y, Z, rows + (size_t)k * FROW, pot, ax, ay, az);
                 }
-                if (k < ntc) { mono1(k, xs0, ys0, zs0, s0); mono1(k, xs1, ys1, zs1, s1); }
                 acc_add_double(A, 0, 0, s0[0]); acc_add_double(A, 0, 1, s0[1]); acc_add_double(A, 0, 2, s0[2]);
                 acc_add_double(A, 1, 0, s1[0]); acc_add_double(A, 1, 1, s1[1]); acc_add_double(A, 1, 2, s1[2]);
                 if (POT) { acc_add_double(A, 0, 3, s0[3]); acc_add_double(A, 1, 3, s1[3]); }
+            } else {
+                for (int k = t.sub; k < ntc; k += t.S) m2p_body<P, f2, POT>(X, Y, Z, rows + (size_t)k * FROW, pot, ax, ay, az);
             }
-        }
-        if (t.active) {
-            f2 pot = f2_dup(0.0f), ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f);
-            for (int k = t.sub; k < ntc; k += t.S) m2p_body<P, f2, POT>(X, Y, Z, rows + (size_t)k * FROW, pot, ax, ay, az);
             acc_fold(A, ax, ay, az, pot, POT);
         }
         __syncwarp();
