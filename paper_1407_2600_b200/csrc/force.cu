@@ -13,9 +13,6 @@
 #include "force_task.cuh"
 
 #define FW 1                 // warps (tasks) per block: tasks differ in length, see m2p.cu
-#ifndef P2P_PERSIST
-#define P2P_PERSIST 0
-#endif
 #ifndef P2P_MINB
 #define P2P_MINB 16          // resident warps per SM the register budget is cut for
 #endif
@@ -80,27 +77,13 @@ __global__ void __launch_bounds__(FW * 32, P2P_MINB) k_p2p(uint32_t t0, uint32_t
                                                  const uint32_t *__restrict__ list,
                                                  const uint64_t *__restrict__ off, uint64_t base,
                                                  const uint32_t *__restrict__ len, float4 *__restrict__ sacc,
-                                                 float4 *__restrict__ sacc_lo, uint32_t *__restrict__ next_task)
+                                                 float4 *__restrict__ sacc_lo)
 {
     __shared__ __align__(16) float4 src_all[FW][2][P2P_TILE];     // two windows of raw (x, y, z, m) per warp
     __shared__ __align__(8) uint64_t bar_all[FW][2];              // one mbarrier per window buffer
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (lane == 0) { p2p_mbar_init(&bar_all[warp][0]); p2p_mbar_init(&bar_all[warp][1]); }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    __syncwarp();
-    uint32_t phase = 0;                           // bit b: parity of the next completion of buffer b's mbarrier
-#if P2P_PERSIST
-    // resident warps take tasks (longest first) from a counter: no block launch between tasks
-    for (;;) {
-    uint32_t task = 0;
-    if (lane == 0) task = t0 + atomicAdd(next_task, 1u);
-    task = __shfl_sync(0xffffffffu, task, 0);
-    if (task >= t1) break;
-    const warp_task t = make_task_at(task, t1, taskmap, gfirst, gcount);
-#else
     const warp_task t = make_task(t0, t1, FW, taskmap, gfirst, gcount);
     if (!t.valid) return;
-#endif
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const float4 ma = spos[t.sa], mb = spos[t.sb];
     const f2 X = f2_make(ma.x, mb.x), Y = f2_make(ma.y, mb.y), Z = f2_make(ma.z, mb.z);
     const f2 E2 = f2_dup(eps2);
@@ -163,6 +146,10 @@ __global__ void __launch_bounds__(FW * 32, P2P_MINB) k_p2p(uint32_t t0, uint32_t
         if (i1 > i0) p2p_bulk(src_all[warp][b] + ((L.pref + i0) - lo), spos + L.first + i0, (i1 - i0) * 16u, &bar_all[warp][b]);
     };
 
+    if (lane == 0) { p2p_mbar_init(&bar_all[warp][0]); p2p_mbar_init(&bar_all[warp][1]); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncwarp();
+    uint32_t phase = 0;                           // bit b: parity of the next completion of buffer b's mbarrier
     leaf_batch cur = load_batch(0), nxt = load_batch(32);
     uint32_t bcur = 0, lo = 0;                    // current window: batch at list position bcur, offset lo
     int buf = 0;
@@ -228,10 +215,6 @@ __global__ void __launch_bounds__(FW * 32, P2P_MINB) k_p2p(uint32_t t0, uint32_t
     }
     __syncwarp();
     task_store(t, A, reinterpret_cast<double *>(src_all[warp][0]), sacc, sacc_lo);
-#if P2P_PERSIST
-    __syncwarp();
-    }
-#endif
 }
 
 static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_t t1, uint64_t mb, uint64_t pb,
@@ -248,18 +231,12 @@ static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_
         int e = dsk_order_tasks(c, t0, t1, c->g_p2p_src, 6);      // longest first (m2p.cu)
         if (e) return e;
     }
-#if P2P_PERSIST
-    cudaMemsetAsync(c->task_hist, 0, sizeof(uint32_t), s);          // the bins are free between the two task sorts
-    const unsigned p2p_grid = min((unsigned)(t1 - t0), (unsigned)(c->nsm * P2P_MINB));
-#else
-    const unsigned p2p_grid = (t1 - t0 + FW - 1) / FW;
-#endif
     if (want_pot)
-        k_p2p<true><<<p2p_grid, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->cell, c->spos, c->gfirst,
-                                           c->gcount, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo, c->task_hist);
+        k_p2p<true><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->cell, c->spos, c->gfirst,
+                                           c->gcount, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     else
-        k_p2p<false><<<p2p_grid, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->cell, c->spos, c->gfirst,
-                                            c->gcount, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo, c->task_hist);
+        k_p2p<false><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->cell, c->spos, c->gfirst,
+                                            c->gcount, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
     cudaEventRecord(c->ev[9], s);
     {
         int e = dsk_launch_m2p(c, t0, t1, mb, want_pot);

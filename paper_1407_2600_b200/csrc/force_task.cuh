@@ -56,11 +56,12 @@ struct warp_task {
     bool valid, active, has_b;   // task exists; this lane belongs to a sub-group; second sink is a real one
 };
 // taskmap entry = group << 2 | part
-__device__ __forceinline__ warp_task make_task_at(uint32_t task, uint32_t t1, const uint32_t *__restrict__ taskmap,
-                                                  const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount)
+__device__ __forceinline__ warp_task make_task(uint32_t t0, uint32_t t1, int fw, const uint32_t *__restrict__ taskmap,
+                                               const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount)
 {
     warp_task t;
-    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t task = t0 + blockIdx.x * fw + warp;      // fw = warps (tasks) per block
     t.valid = false; t.active = false; t.has_b = false;
     t.g = 0; t.first = 0; t.ns = 0; t.W = 32; t.S = 1; t.sub = 0; t.j = 0; t.sa = t.sb = 0;
     if (task >= t1) return t;
@@ -81,11 +82,6 @@ __device__ __forceinline__ warp_task make_task_at(uint32_t task, uint32_t t1, co
     t.sa = t.first + 2u * (uint32_t)t.j;
     t.sb = t.has_b ? t.sa + 1u : t.sa;
     return t;
-}
-__device__ __forceinline__ warp_task make_task(uint32_t t0, uint32_t t1, int fw, const uint32_t *__restrict__ taskmap,
-                                               const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount)
-{
-    return make_task_at(t0 + blockIdx.x * fw + (threadIdx.x >> 5), t1, taskmap, gfirst, gcount);      // fw = warps (tasks) per block
 }
 
 // two-float running sums of (ax, ay, az, pot) for the lane's two sinks, PACKED like the arithmetic: component c
