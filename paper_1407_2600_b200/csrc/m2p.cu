@@ -432,7 +432,10 @@ __global__ void __launch_bounds__(256) k_task_hist(uint32_t t0, uint32_t t1, con
                                                    int shift, uint32_t *__restrict__ hist)
 {
     const uint32_t t = t0 + blockIdx.x * 256 + threadIdx.x;
-    if (t < t1) atomicAdd(&hist[task_cost_bin(taskmap[t], gcount, len, shift)], 1u);
+    // neighbouring tasks cost about the same: one atomic per distinct bin and warp, not per task
+    const uint32_t bin = t < t1 ? task_cost_bin(taskmap[t], gcount, len, shift) : 0xffffffffu;
+    const uint32_t peers = __match_any_sync(0xffffffffu, bin), lane = threadIdx.x & 31u;
+    if (t < t1 && (peers & ((1u << lane) - 1u)) == 0u) atomicAdd(&hist[bin], (uint32_t)__popc(peers));
 }
 __global__ void __launch_bounds__(TASK_BINS) k_task_scan(uint32_t *__restrict__ hist)
 {
@@ -454,9 +457,14 @@ __global__ void __launch_bounds__(256) k_task_scatter(uint32_t t0, uint32_t t1, 
                                                       int shift, uint32_t *__restrict__ hist, uint32_t *__restrict__ sorted)
 {
     const uint32_t t = t0 + blockIdx.x * 256 + threadIdx.x;
-    if (t >= t1) return;
-    const uint32_t m = taskmap[t];
-    sorted[t0 + atomicAdd(&hist[task_cost_bin(m, gcount, len, shift)], 1u)] = m;
+    const uint32_t m = t < t1 ? taskmap[t] : 0u;
+    const uint32_t bin = t < t1 ? task_cost_bin(m, gcount, len, shift) : 0xffffffffu;
+    const uint32_t peers = __match_any_sync(0xffffffffu, bin), lane = threadIdx.x & 31u;
+    const uint32_t before = __popc(peers & ((1u << lane) - 1u));
+    uint32_t at = 0;
+    if (t < t1 && before == 0u) at = atomicAdd(&hist[bin], (uint32_t)__popc(peers));      // the first lane of each bin reserves for all
+    at = __shfl_sync(0xffffffffu, at, __ffs((int)peers) - 1);
+    if (t < t1) sorted[t0 + at + before] = m;
 }
 
 // g_task_sorted[t0, t1) = the tasks of g_task[t0, t1) by descending (len[group] >> shift) / sub-groups

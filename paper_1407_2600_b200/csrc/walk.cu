@@ -13,6 +13,9 @@
 #ifndef WW
 #define WW 1                 // warps (groups) per block: walks differ in length, a block ends with its longest
 #endif
+#ifndef WEPL
+#define WEPL 2               // stack entries per lane and trip
+#endif
 #ifndef WSTACK
 #define WSTACK 2048          // stack entries per warp
 #endif
@@ -63,45 +66,59 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
     if (MODE == 1) { mo = m2p_off[g] - m2p_base; po = p2p_off[g] - p2p_base; }
     if (MODE == 2) { mo = (uint64_t)g * cap_m; po = (uint64_t)g * cap_p; }
     const uint32_t lt = (1u << lane) - 1u;
+    // WEPL stack entries per lane and trip: their loads are independent, so a trip exposes one L2 round trip for
+    // 32 * WEPL cells
     while (sp > 0) {
-        const int take = sp < 32 ? sp : 32;
-        uint32_t e = 0;
-        bool act = lane < take;
-        if (act) e = stk[sp - 1 - lane];
+        const int take = sp < 32 * WEPL ? sp : 32 * WEPL;
+        uint32_t e[WEPL], nchild[WEPL], child0[WEPL];
+        bool act[WEPL], accept[WEPL], leaf[WEPL];
+        float4 h[WEPL], rr[WEPL];
+#pragma unroll
+        for (int q = 0; q < WEPL; q++) {
+            act[q] = lane + 32 * q < take;
+            e[q] = act[q] ? stk[sp - 1 - lane - 32 * q] : 0u;
+        }
         sp -= take;
         __syncwarp();
-        bool accept = false, leaf = false;
-        uint32_t nchild = 0, child0 = 0, cnt = 0;
-        if (act) {
-            const uint32_t c = e & ((1u << DSK_CELL_BITS) - 1u);
-            const int img = (int)(e >> DSK_CELL_BITS);
-            const float4 h = wmac[2 * (size_t)c];          // com.xyz, critical radius s/theta + delta
-            const float4 rr = wmac[2 * (size_t)c + 1];     // the cell record (same sector)
-            float sh[3];
-            image_shift(img, periodic, box, sh);
-            const float zx = h.x + sh[0], zy = h.y + sh[1], zz = h.z + sh[2];
-            const float dx = fmaxf(fmaxf(blo.x - zx, zx - bhi.x), 0.0f);
-            const float dy = fmaxf(fmaxf(blo.y - zy, zy - bhi.y), 0.0f);
-            const float dz = fmaxf(fmaxf(blo.z - zz, zz - bhi.z), 0.0f);
-            const float d2 = dx * dx + dy * dy + dz * dz;
-            accept = d2 > h.w * h.w;
-            if (!accept) {
-                nchild = __float_as_uint(rr.w) & 255u; child0 = __float_as_uint(rr.z); cnt = __float_as_uint(rr.y);
-                leaf = nchild == 0;
+#pragma unroll
+        for (int q = 0; q < WEPL; q++)
+            if (act[q]) {
+                const uint32_t c = e[q] & ((1u << DSK_CELL_BITS) - 1u);
+                h[q] = wmac[2 * (size_t)c];            // com.xyz, critical radius s/theta + delta
+                rr[q] = wmac[2 * (size_t)c + 1];       // the cell record (same sector)
             }
+        uint32_t push[WEPL], ptot = 0;
+#pragma unroll
+        for (int q = 0; q < WEPL; q++) {
+            accept[q] = false; leaf[q] = false; nchild[q] = 0; child0[q] = 0;
+            uint32_t cnt = 0;
+            if (act[q]) {
+                float sh[3];
+                image_shift((int)(e[q] >> DSK_CELL_BITS), periodic, box, sh);
+                const float zx = h[q].x + sh[0], zy = h[q].y + sh[1], zz = h[q].z + sh[2];
+                const float dx = fmaxf(fmaxf(blo.x - zx, zx - bhi.x), 0.0f);
+                const float dy = fmaxf(fmaxf(blo.y - zy, zy - bhi.y), 0.0f);
+                const float dz = fmaxf(fmaxf(blo.z - zz, zz - bhi.z), 0.0f);
+                const float d2 = dx * dx + dy * dy + dz * dz;
+                accept[q] = d2 > h[q].w * h[q].w;
+                if (!accept[q]) {
+                    nchild[q] = __float_as_uint(rr[q].w) & 255u; child0[q] = __float_as_uint(rr[q].z); cnt = __float_as_uint(rr[q].y);
+                    leaf[q] = nchild[q] == 0;
+                }
+            }
+            const uint32_t bm = __ballot_sync(0xffffffffu, accept[q]);
+            const uint32_t bl = __ballot_sync(0xffffffffu, leaf[q]);
+            if (FILL) {
+                const uint32_t im = nm + __popc(bm & lt), ip = np + __popc(bl & lt);
+                if (accept[q] && (MODE == 1 || im < cap_m)) list_m2p[mo + im] = e[q];
+                if (leaf[q] && (MODE == 1 || ip < cap_p)) list_p2p[po + ip] = e[q];
+            }
+            nm += __popc(bm); np += __popc(bl);
+            if (leaf[q]) nsrc += cnt;
+            push[q] = (act[q] && !accept[q]) ? nchild[q] : 0u;      // children of rejected internal cells
+            ptot += push[q];
         }
-        const uint32_t bm = __ballot_sync(0xffffffffu, accept);
-        const uint32_t bl = __ballot_sync(0xffffffffu, leaf);
-        if (FILL) {
-            const uint32_t im = nm + __popc(bm & lt), ip = np + __popc(bl & lt);
-            if (accept && (MODE == 1 || im < cap_m)) list_m2p[mo + im] = e;
-            if (leaf && (MODE == 1 || ip < cap_p)) list_p2p[po + ip] = e;
-        }
-        nm += __popc(bm); np += __popc(bl);
-        if (leaf) nsrc += cnt;
-        // push the children of rejected internal cells
-        const bool open = act && !accept && nchild != 0;
-        uint32_t push = open ? nchild : 0u, x = push;
+        uint32_t x = ptot;
         for (int o = 1; o < 32; o <<= 1) {
             uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
             if (lane >= o) x += y;
@@ -111,10 +128,12 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
             if (lane == 0) atomicOr(&st->status, ST_STACKOVF);
             break;
         }
-        if (open) {
-            uint32_t at = sp + x - push;
-            const uint32_t img = e & ~((1u << DSK_CELL_BITS) - 1u);
-            for (uint32_t k = 0; k < nchild; k++) stk[at + k] = img | (child0 + k);
+        uint32_t at = sp + x - ptot;
+#pragma unroll
+        for (int q = 0; q < WEPL; q++) {
+            const uint32_t img = e[q] & ~((1u << DSK_CELL_BITS) - 1u);
+            for (uint32_t k = 0; k < push[q]; k++) stk[at + k] = img | (child0[q] + k);
+            at += push[q];
         }
         sp += (int)tot;
         __syncwarp();
