@@ -13,6 +13,7 @@
 #ifndef WW
 #define WW 1                 // warps (groups) per block: walks differ in length, a block ends with its longest
 #endif
+#define WRESERVE 160         // stack entries kept free for the depth-first tail (7 per level, 21 levels)
 #ifndef WEPL
 #define WEPL 2               // stack entries per lane and trip
 #endif
@@ -69,7 +70,12 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
     // WEPL stack entries per lane and trip: their loads are independent, so a trip exposes one L2 round trip for
     // 32 * WEPL cells
     while (sp > 0) {
-        const int take = sp < 32 * WEPL ? sp : 32 * WEPL;
+        // A popped cell pushes at most 8 children (net +7), so a trip of `take` cells needs 7 * take free entries.  Trips
+        // shrink as the stack fills and end as a plain depth-first walk (take = 1), whose height above its starting
+        // point is at most 7 per level = 147 < WRESERVE: the stack cannot overflow on any tree of <= 21 levels.
+        const int room = (WSTACK - WRESERVE - sp) / 7;
+        int take = sp < 32 * WEPL ? sp : 32 * WEPL;
+        take = min(take, max(room, 1));
         uint32_t e[WEPL], nchild[WEPL], child0[WEPL];
         bool act[WEPL], accept[WEPL], leaf[WEPL];
         float4 h[WEPL], rr[WEPL];

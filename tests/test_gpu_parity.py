@@ -253,6 +253,39 @@ def test_forces_degenerate_inputs(dsk, orc):
 
 
 @pytest.mark.parametrize("periodic", [False, True])
+def test_forces_deep_cascade(dsk, orc, periodic):
+    """A geometric cascade of clumps, each 1/2 the size of the one before, down to the key resolution: a tree of
+    21 levels in which every level holds rejected internal cells for a sink near the focus.  This is the worst case
+    for the walk's stack (trips shrink to a depth-first walk when it fills, walk.cu) and for the fp32 coordinate
+    frames of the force kernels.  Structure bit-exact, forces through the two gates."""
+    rng = np.random.default_rng(77 + int(periodic))
+    focus = np.array([0.37, 0.52, 0.61])
+    parts = []
+    for k in range(22):
+        parts.append(focus + (rng.random((900, 3)) - 0.5) * 0.7 * 2.0 ** (-k))
+    pos = np.concatenate(parts).astype(np.float32)
+    pos = np.clip(pos, 0.0, np.nextafter(np.float32(1.0), np.float32(0.0)))
+    n = len(pos)
+    mass = np.full(n, 1.0 / n, np.float32)
+    eps, theta, p = 1e-7, 0.5, 4
+    d = dsk.Dsk(n, 1.0, periodic, eps, theta, p)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    t = _check_structure(orc, d, pos, mass, 1.0, periodic)
+    assert int(t.cells()["level"].max()) >= 20
+    acc, _ = d.accel(tp, tm, want_pot=False)
+    sink = np.concatenate([np.arange(0, n, 37), np.arange(n - 900, n)])          # a spread + the innermost clump
+    ta = orc.tree_force(pos, mass, 1.0, periodic, eps, theta, p, sink, tree=t)[0]
+    a = acc.cpu().numpy().astype(np.float64)[sink]
+    rel = np.linalg.norm(a - ta, axis=1) / np.linalg.norm(ta, axis=1)
+    assert np.quantile(rel, 0.999) < 1e-4, (np.median(rel), np.quantile(rel, 0.999), rel.max())
+    if not periodic:
+        da = orc.direct_iso(pos, mass, eps, sink)[0]
+        _force_gates(a, ta, da)
+    d.close()
+
+
+@pytest.mark.parametrize("periodic", [False, True])
 def test_forces_every_group_size(dsk, orc, periodic):
     """One tight clump of n particles for every n = 1..NCRIT, each in its own cell of a coarse grid, so the sink
     groups take every size (and with them every task split of DESIGN.md 5.1) while all clumps see each other as
@@ -585,5 +618,6 @@ def test_forces_periodic_full_sampled(dsk, orc, cfgid):
     ta = orc.tree_force(pos, mass, 1.0, True, cfg["eps"], cfg["theta"], cfg["p"], sink, tree=tree)[0]
     a = acc.cpu().numpy().astype(np.float64)[sink]
     rel = np.linalg.norm(a - ta, axis=1) / np.linalg.norm(ta, axis=1)
+    print(f"config {cfgid}: N = {n}, {len(sink)} sinks, median rel. difference {np.median(rel):.3g}, p99.9 {np.quantile(rel, 0.999):.3g}")
     assert np.quantile(rel, 0.999) < 1e-4, (np.median(rel), np.quantile(rel, 0.999))
     d.close()
