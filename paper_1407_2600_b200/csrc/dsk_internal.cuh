@@ -181,6 +181,15 @@ struct dsk_ctx {
 };
 
 #define DSK_COUNT(c, k) ((c)->stats.n_launch += (k))
+// Constant tables and function attributes are per device: a "done once" flag is kept per device ordinal (a process
+// normally drives one GPU, but two contexts on two devices must both get their tables).
+#define DSK_MAXDEV 64
+static inline bool *dsk_device_flag(bool *flags)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= DSK_MAXDEV) dev = 0;
+    return flags + dev;
+}
 #define DSK_CUDA(x)                                 \
     do {                                            \
         cudaError_t e__ = (x);                      \

@@ -139,17 +139,18 @@ void dsk_lattice_tensors(double L, int ws, double *T)
 // ---------------------------------------------------------------------------------------------------
 // device
 __constant__ uint8_t f_ea[NF], f_eb[NF], f_ec[NF];
-static bool g_far_tables = false;
+static bool g_far_tables[DSK_MAXDEV];
 static int far_tables()
 {
-    if (g_far_tables) return DSK_OK;
+    bool *done = dsk_device_flag(g_far_tables);
+    if (*done) return DSK_OK;
     const Tab &t = tab();
     uint8_t a[NF], b[NF], c[NF];
     for (int i = 0; i < NF; i++) { a[i] = (uint8_t)t.a[i]; b[i] = (uint8_t)t.b[i]; c[i] = (uint8_t)t.c[i]; }
     DSK_CUDA(cudaMemcpyToSymbol(f_ea, a, NF));
     DSK_CUDA(cudaMemcpyToSymbol(f_eb, b, NF));
     DSK_CUDA(cudaMemcpyToSymbol(f_ec, c, NF));
-    g_far_tables = true;
+    *done = true;
     return DSK_OK;
 }
 

@@ -487,12 +487,13 @@ template <int P, bool POT, bool M64>
 static int launch_m2p_v(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base)
 {
     using C = m2p_cfg<P, M64>;
-    static bool attr_done = false;
+    static bool attr_flags[DSK_MAXDEV];
+    bool *attr_done = dsk_device_flag(attr_flags);
     const size_t smem = FW * C::WARP_BYTES;
-    if (!attr_done) {
+    if (!*attr_done) {
         DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, POT, M64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, POT, M64>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-        attr_done = true;
+        *attr_done = true;
     }
     const float e2 = c->eps * c->eps;
     const unsigned grid = (t1 - t0 + FW - 1) / FW;

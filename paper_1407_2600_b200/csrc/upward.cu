@@ -27,10 +27,11 @@ __device__ uint8_t g_m2m_perm[4][UNP];
 __constant__ float c_sgn_invfact[UNP];   // (-1)^|n| / (a! b! c!)
 __constant__ float c_invfact1[DSK_PMAX + 1];
 
-static bool g_tables_done = false;
+static bool g_tables_done[DSK_MAXDEV];
 static int upload_tables()
 {
-    if (g_tables_done) return DSK_OK;
+    bool *done = dsk_device_flag(g_tables_done);
+    if (*done) return DSK_OK;
     uint8_t ea[UNP], eb[UNP], ec[UNP], rk[UNP];
     float sif[UNP], if1[DSK_PMAX + 1];
     double fact[DSK_PMAX + 1];
@@ -54,7 +55,7 @@ static int upload_tables()
     DSK_CUDA(cudaMemcpyToSymbol(g_rank, rk, sizeof(rk)));
     DSK_CUDA(cudaMemcpyToSymbol(c_sgn_invfact, sif, sizeof(sif)));
     DSK_CUDA(cudaMemcpyToSymbol(c_invfact1, if1, sizeof(if1)));
-    g_tables_done = true;
+    *done = true;
     return DSK_OK;
 }
 
@@ -319,11 +320,12 @@ static int launch_upward(dsk_ctx *c, const uint32_t *lvl_start, int nlevel)
         DSK_COUNT(c, 1);
     }
     if (ltop > 0) {
-        static bool attr_done = false;
+        static bool attr_flags[DSK_MAXDEV];
+        bool *attr_done = dsk_device_flag(attr_flags);
         const size_t smem = sizeof(up_smem<P>) * UTOP_WARPS;
-        if (!attr_done) {
+        if (!*attr_done) {
             DSK_CUDA(cudaFuncSetAttribute(k_upward_top<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            attr_done = true;
+            *attr_done = true;
         }
         up_levels lv;
         for (int i = 0; i < DSK_KEY_LEVELS + 3; i++) lv.start[i] = lvl_start[i];
