@@ -47,12 +47,12 @@ def workload():
     return cfg, pos, mass
 
 
-def config_dict(cfg, n_gpus):
+def config_dict(cfg, n_gpus, consts):
     return {"workload": WORKLOADS[CFG],
             "N": cfg["N"], "eps": cfg["eps"], "theta": cfg["theta"], "p": cfg["p"], "periodic": bool(cfg["periodic"]),
             "step": ("dsk_kdk_step, da = 0.01 from a = 0.5, Einstein-de Sitter (one force evaluation per step; the e2e arm "
                      "pays two: it restarts from the host copy)") if CFG == 5 else "dsk_build_tree + dsk_accel (acc+pot)",
-            "NLEAF": 80, "NCRIT": 128,
+            "NLEAF": int(consts[0]), "NCRIT": int(consts[1]),
             "l2": "256 MiB buffer written between steps (outside the event pairs); working set ~1 GB > L2",
             "parallelism": f"replicas x{n_gpus}" if n_gpus > 1 else "single GPU"}
 
@@ -177,7 +177,7 @@ def run_reference(args):
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * n / value, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": config_dict(cfg, 1),
+           "config": config_dict(cfg, 1, (oracle.NLEAF, oracle.NCRIT)),
            "cpu_baseline": {"value": value, "unit": UNIT, "cores": info["cores"], "kind": "oracle", "sample": sample},
            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
@@ -336,7 +336,7 @@ def run_ours(args):
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-               "config": config_dict(cfg, world),
+               "config": config_dict(cfg, world, (dsk.get_param("NLEAF"), dsk.get_param("NCRIT"))),
                "roofline": {"bound": "alu", "kernel": f"k_m2p<{cfg['p']},{'nopot' if kdk else 'pot'},{'fp64 monopoles' if cfg['periodic'] else 'fp32'}>", "achieved": ach_m2p / 1e12,
                             "peak": peak_fp32 / 1e12, "unit": "TFLOP/s", "frac": ach_m2p / peak_fp32,
                             "traffic": traffic,

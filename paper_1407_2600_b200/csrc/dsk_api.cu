@@ -19,7 +19,7 @@ static size_t carve(dsk_ctx *c, char *base)
         return p;
     };
     c->ntile = (int)((n + 2047) / 2048);
-    // measured <= 0.06 cells and <= 0.05 groups per particle (NLEAF 64-80, NCRIT 64-128) on every config; a pathological
+    // measured <= 0.06 cells and <= 0.05 groups per particle (NLEAF 64-112, NCRIT 64-192) on every config; a pathological
     // input (deep chains of near-coincident clumps) that needs more ends in DSK_ECELLOVERFLOW, not in a fault
     c->ncell_cap = (int64_t)(n / 4 + 4096);
     if (c->ncell_cap > (1ll << DSK_CELL_BITS)) c->ncell_cap = 1ll << DSK_CELL_BITS;

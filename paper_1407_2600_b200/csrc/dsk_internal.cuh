@@ -7,10 +7,10 @@
 
 #define DSK_KEY_LEVELS 21
 #ifndef DSK_NLEAF
-#define DSK_NLEAF 80         // leaf bucket: a cell is split iff count > NLEAF (the oracle's NLEAF must match)
+#define DSK_NLEAF 112        // leaf bucket: a cell is split iff count > NLEAF (the oracle's NLEAF must match; sweep)
 #endif
 #ifndef DSK_NCRIT
-#define DSK_NCRIT 128        // sink group: first cell from the root with count <= NCRIT
+#define DSK_NCRIT 192        // sink group: first cell from the root with count <= NCRIT (at most 4 tasks of 32 lanes x 2 sinks)
 #endif
 #define DSK_WS 2              // image block half-width (WS = 1 floors the error at ~3e-3)
 #define DSK_FAR_ORDER 8

@@ -6,7 +6,7 @@
 // broadcast to both halves (SASS "R.F32"; measured 2.2 cycles per FFMA2 per SMSP against 2.0 for three packed
 // operands).  Sources therefore sit in shared memory exactly as they sit in global memory (no interleaving
 // pass), one LDS.128 brings four coefficients, and a warp covers up to 64 sinks.
-// Groups hold 1..NCRIT = 128 sinks (most far fewer: groups are tree cells), so a group of n sinks is cut into
+// Groups hold 1..NCRIT = 192 sinks (most far fewer: groups are tree cells), so a group of n sinks is cut into
 // k <= 4 tasks of ~n/k sinks; a task of ns sinks uses W = ceil(ns/2) lanes per sub-group and S = 32 / W sub-groups
 // that take alternate sources of a tile and are summed at the end through shared memory; k maximises the share
 // of busy lanes n S / (64 k) (ncu: 29.3 of 32 threads per instruction on the Plummer workload).
