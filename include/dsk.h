@@ -74,7 +74,8 @@ typedef struct dsk_stats {
 int dsk_create(dsk_ctx **out, int64_t N, float box, int periodic, float eps, float theta, int p);
 int dsk_destroy(dsk_ctx *ctx);
 
-/* Bytes of device workspace this context needs (depends on N and the largest order, p = 8). */
+/* Bytes of device workspace this context needs (depends on N and on the order p given to dsk_create: the
+ * moment rows are sized for that order, so dsk_set_params may lower p but not raise it). */
 size_t dsk_workspace_bytes(const dsk_ctx *ctx);
 /* Lend the workspace (device pointer, >= dsk_workspace_bytes(), 256-byte aligned). */
 int dsk_bind_workspace(dsk_ctx *ctx, void *dev_ptr, size_t bytes);
@@ -89,8 +90,9 @@ int dsk_set_params(dsk_ctx *ctx, float eps, float theta, int p);
  * PAPER.md:61 (keys, tree), :57/:75 (moments).  pos dev [N,3], mass dev [N]; not retained. */
 int dsk_build_tree(dsk_ctx *ctx, const float *pos, const float *mass);
 
-/* Walk + evaluate: acc dev [N,3], pot dev [N] or NULL, caller order.  pos/mass must be the arrays the
- * tree was built from (they are not re-read: the sorted copy made by dsk_build_tree is used).
+/* Walk + evaluate: acc dev [N,3], pot dev [N] or NULL, caller order.  pos and mass are IGNORED (they may be NULL):
+ * the forces are those of the positions and masses given to the last dsk_build_tree, whose sorted copy is used.  A
+ * caller who has moved particles since must call dsk_build_tree again (dsk_kdk_step does).
  * PAPER.md:69-75 (lists, P2P, multipole interactions), :63 (periodic far field). */
 int dsk_accel(dsk_ctx *ctx, const float *pos, const float *mass, float *acc, float *pot);
 
@@ -115,7 +117,7 @@ int dsk_set_walk_mode(dsk_ctx *ctx, int mode);
 
 /* One BLOCK step of size da with hierarchical individual time steps (reading O9c of DESIGN.md; "adaptive
  * symplectic integrator (Quinn et al. 1997)").  rung dev uint8 [N], in/out: particle i takes steps of da / 2^rung[i],
- * 0 <= rung <= rmax <= 8.  The block is cut into 2^rmax substeps; per substep: opening half kicks of the particles whose
+ * 0 <= rung <= rmax <= 8 (a larger entry is read as rmax and written back clamped).  The block is cut into 2^rmax substeps; per substep: opening half kicks of the particles whose
  * step starts, drift of all, tree + forces of the particles whose step ends (dsk_accel_active), their closing half kicks,
  * and their new rung from step_i = eta sqrt(eps / |acc_i|), rung = ceil(log2(da / step_i)) (decided in fp32; finer at
  * once, coarser one level at a time and only when synchronised).  rmax = 0 is dsk_kdk_step.  Same state, cached force

@@ -196,6 +196,7 @@ extern "C" int dsk_build_tree(dsk_ctx *c, const float *pos, const float *mass)
     if (!c || !pos || !mass) return DSK_EINVAL;
     if (!c->ws) return DSK_ENOWORKSPACE;
     c->have_tree = 0; c->moments_p = -1; c->lists_valid = 0;
+    c->onepass_bad_theta = -1.0f;          // a new tree gets a new one-pass attempt (an old overflow says nothing about it)
     c->stats.n_launch = 0;
     DSK_CUDA(cudaMemsetAsync(c->dstate, 0, sizeof(dsk_devstate), c->stream));
     int e = dsk_run_keysort(c, pos, mass);
@@ -340,6 +341,7 @@ extern "C" int dsk_set_walk_mode(dsk_ctx *c, int mode)
 {
     if (!c || mode < 0 || mode > 2) return DSK_EINVAL;
     c->walk_two_pass_only = mode;
+    c->onepass_bad_theta = -1.0f;
     c->lists_valid = 0;
     return DSK_OK;
 }
@@ -351,16 +353,20 @@ extern "C" int dsk_kdk_reset(dsk_ctx *c)
     return DSK_OK;
 }
 
+// H^2 > 0 at both ends of the step (a closed model turns around; beyond that the factors are not defined)
+static bool friedmann_ok(const dsk_ctx *c, double e0, double e1)
+{
+    const double ok = 1.0 - c->omega_m - c->omega_l;
+    return c->omega_m / (e0 * e0 * e0) + ok / (e0 * e0) + c->omega_l > 0.0 &&
+           c->omega_m / (e1 * e1 * e1) + ok / (e1 * e1) + c->omega_l > 0.0;
+}
+
 extern "C" int dsk_kdk_step(dsk_ctx *c, float *pos, float *vel, const float *mass, double a, double da)
 {
     if (!c || !pos || !vel || !mass) return DSK_EINVAL;
     if (!c->ws) return DSK_ENOWORKSPACE;
     if (c->periodic && !(a > 0.0 && a + da > 0.0)) return DSK_EINVAL;
-    if (c->periodic) {
-        const double ok = 1.0 - c->omega_m - c->omega_l, e0 = a, e1 = a + da;
-        if (!(c->omega_m / (e0 * e0 * e0) + ok / (e0 * e0) + c->omega_l > 0.0) ||
-            !(c->omega_m / (e1 * e1 * e1) + ok / (e1 * e1) + c->omega_l > 0.0)) return DSK_EINVAL;
-    }
+    if (c->periodic && !friedmann_ok(c, a, a + da)) return DSK_EINVAL;
     int e;
     if (!c->kdk_have_acc) {
         e = dsk_build_tree(c, pos, mass);
@@ -406,6 +412,7 @@ extern "C" int dsk_kdk_block_step(dsk_ctx *c, float *pos, float *vel, const floa
     if (!c->ws) return DSK_ENOWORKSPACE;
     if (rmax < 0 || rmax > DSK_RMAX || !(eta > 0.0f) || !(da > 0.0)) return DSK_EINVAL;
     if (c->periodic && !(a > 0.0)) return DSK_EINVAL;
+    if (c->periodic && !friedmann_ok(c, a, a + da)) return DSK_EINVAL;
     int e;
     if (!c->kdk_have_acc) {
         e = dsk_build_tree(c, pos, mass);
@@ -424,19 +431,19 @@ extern "C" int dsk_kdk_block_step(dsk_ctx *c, float *pos, float *vel, const floa
     for (uint32_t s = 0; s < nsub; s++) {
         const double as = a + (double)s * h, at = a + (double)(s + 1) * h;
         for (int r = 0; r <= DSK_RMAX; r++) kf[r] = r <= rmax ? (float)kick_factor(c, mtot, as, as + (double)(nsub >> r) * h * 0.5) : 0.0f;
-        e = dsk_run_kick_rung(c, vel, c->kdk_acc, rung, s, nsub, kf);
+        e = dsk_run_kick_rung(c, vel, c->kdk_acc, rung, s, nsub, rmax, kf);
         if (e) return e;
         e = dsk_run_drift(c, pos, vel, (float)drift_factor(c, mtot, as, at));
         if (e) return e;
         c->kdk_have_acc = 0;
-        e = dsk_run_rung_active(c, rung, s + 1, nsub, c->kdk_active);
+        e = dsk_run_rung_active(c, rung, s + 1, nsub, rmax, c->kdk_active);
         if (e) return e;
         e = dsk_build_tree(c, pos, mass);
         if (e) return e;
         e = dsk_accel_active(c, pos, mass, c->kdk_active, c->kdk_acc, nullptr);
         if (e) return e;
         for (int r = 0; r <= DSK_RMAX; r++) kf[r] = r <= rmax ? (float)kick_factor(c, mtot, at - (double)(nsub >> r) * h * 0.5, at) : 0.0f;
-        e = dsk_run_kick_rung(c, vel, c->kdk_acc, rung, s + 1, nsub, kf);      // the same test: t % L == 0
+        e = dsk_run_kick_rung(c, vel, c->kdk_acc, rung, s + 1, nsub, rmax, kf);      // the same test: t % L == 0
         if (e) return e;
         e = dsk_run_rung_update(c, c->kdk_acc, c->kdk_active, rung, s + 1, nsub, rmax, (float)da, eta);
         if (e) return e;

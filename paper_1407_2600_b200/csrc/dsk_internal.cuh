@@ -216,8 +216,8 @@ void dsk_lattice_tensors(double L, int ws, double *T);                        //
 int dsk_run_kick(dsk_ctx *c, float *vel, const float *acc, float k);          // kdk.cu
 int dsk_run_drift(dsk_ctx *c, float *pos, const float *vel, float d);         // kdk.cu
 int dsk_run_kick_rung(dsk_ctx *c, float *vel, const float *acc, const uint8_t *rung, uint32_t s, uint32_t nsub,
-                      const float *k);                                        // kdk.cu
-int dsk_run_rung_active(dsk_ctx *c, const uint8_t *rung, uint32_t t, uint32_t nsub, uint8_t *active);   // kdk.cu
+                      int rmax, const float *k);                              // kdk.cu
+int dsk_run_rung_active(dsk_ctx *c, const uint8_t *rung, uint32_t t, uint32_t nsub, int rmax, uint8_t *active);   // kdk.cu
 int dsk_run_rung_update(dsk_ctx *c, const float *acc, const uint8_t *active, uint8_t *rung, uint32_t t, uint32_t nsub,
                         int rmax, float da, float eta);                       // kdk.cu
 

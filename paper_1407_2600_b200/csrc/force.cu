@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(FW * 32, P2P_MINB) k_p2p(uint32_t t0, uint32_t
             // my sub-group's sources: src[sub], src[sub + S], ...; pointer stepping keeps index arithmetic out of the loop
             const float4 *q = src + t.sub;
             const int S1 = t.S, S2 = 2 * t.S, S3 = 3 * t.S, S4 = 4 * t.S;
-            int left = (int)(((nt - (uint32_t)t.sub + (uint32_t)t.S - 1u) * sinv16) >> 16);   // = ceil((nt - sub) / S), nt <= 256
+            int left = (int)(((nt - (uint32_t)t.sub + (uint32_t)t.S - 1u) * sinv16) >> 16);   // = ceil((nt - sub) / S), nt <= P2P_TILE < 1024
             for (; left >= 4; left -= 4, q += S4) {
                 const float4 s0 = q[0], s1 = q[S1], s2 = q[S2], s3 = q[S3];
                 pair(s0); pair(s1); pair(s2); pair(s3);

@@ -13,9 +13,9 @@
 // the sums S_m = sum_q sum_j B^(q,m)_j mu_j and their gradients G_m,i = sum B^(q,m)_j mu_{j-e_i} give
 //     pot = -(1/s) sum_m h_m S_m ,
 //     acc_i = (1/s^2) [ sum_m h_m G_m,i - rho_i q sum_m (2m+1) h_m S_m ],  h_m = R^-(2m+1), q = 1/R^2,
-// in cell-scaled coordinates rho = r/s, eps~ = eps/s.  This needs about half the FP32 instructions of the
-// derivative recurrence (p = 4: 188 against ~410 per interaction) and holds only two degrees of monomials
-// in registers.  The coefficients ("force row") are a fixed linear map of the moment row, applied once per
+// in cell-scaled coordinates rho = r/s, eps~ = eps/s.  This needs well under half the FP32 instructions of the
+// derivative recurrence (p = 4: 149 packed instructions = 252 flop per interaction against 636 flop)
+// and holds only two degrees of monomials in registers.  The coefficients ("force row") are a fixed linear map of the moment row, applied once per
 // cell after the upward pass by k_frows.  The dipole (l = 1) vanishes about the centre of mass and is skipped.
 #include "force_task.cuh"
 #include <vector>

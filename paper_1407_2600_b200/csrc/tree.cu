@@ -227,9 +227,12 @@ __global__ void __launch_bounds__(TB) k_group_emit(const uint32_t *__restrict__ 
 __global__ void __launch_bounds__(TB) k_group_bbox(const float4 *__restrict__ spos,
                                                    const uint32_t *__restrict__ gfirst,
                                                    uint32_t *__restrict__ gcount, float4 *__restrict__ gbox,
-                                                   uint32_t *__restrict__ ntask, uint32_t n, const dsk_devstate *st)
+                                                   uint32_t *__restrict__ ntask, uint32_t n, uint32_t ngroup_cap,
+                                                   const dsk_devstate *st)
 {
-    uint32_t ng = st->ngroup;
+    // more groups than the workspace holds (k_group_emit has set ST_CELLOVF, the call will fail): stay inside the arrays
+    if (st->status & ST_CELLOVF) return;
+    uint32_t ng = min(st->ngroup, ngroup_cap);
     uint32_t g = (blockIdx.x * TB + threadIdx.x) >> 5;
     int lane = threadIdx.x & 31;
     if (g >= ng) return;
@@ -247,7 +250,7 @@ __global__ void __launch_bounds__(TB) k_group_bbox(const float4 *__restrict__ sp
             hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
         }
     if (lane == 0) {
-        ntask[g] = dsk_task_parts(e - f);
+        ntask[g] = dsk_task_parts(min(e - f, (uint32_t)DSK_NCRIT));
         gcount[g] = e - f;
         gbox[2 * (size_t)g] = make_float4(lo[0], lo[1], lo[2], 0.0f);
         gbox[2 * (size_t)g + 1] = make_float4(hi[0], hi[1], hi[2], 0.0f);
@@ -256,9 +259,10 @@ __global__ void __launch_bounds__(TB) k_group_bbox(const float4 *__restrict__ sp
 
 // task -> (group, part) map for the warp-task force kernels
 __global__ void __launch_bounds__(TB) k_task_fill(const uint32_t *__restrict__ taskoff, uint32_t *__restrict__ task,
-                                                  dsk_devstate *st)
+                                                  uint32_t ngroup_cap, dsk_devstate *st)
 {
-    const uint32_t ng = st->ngroup;
+    if (st->status & ST_CELLOVF) return;
+    const uint32_t ng = min(st->ngroup, ngroup_cap);
     const uint32_t g = blockIdx.x * TB + threadIdx.x;
     if (g >= ng) return;
     const uint32_t a = taskoff[g], b = (g + 1 < ng) ? taskoff[g + 1] : st->ntask;
@@ -288,9 +292,9 @@ int dsk_run_build(dsk_ctx *c)
     k_group_emit<<<nb, TB, 0, s>>>(c->gmark, c->gscan, n, (uint32_t)c->ngroup_cap, c->gfirst, c->gcell, c->dstate);
     // one warp per possible group; ngroup is read on the device
     const int64_t nwarp_blocks = (c->ngroup_cap * 32 + TB - 1) / TB;
-    k_group_bbox<<<(unsigned)nwarp_blocks, TB, 0, s>>>(c->spos, c->gfirst, c->gcount, c->gbox, c->g_taskoff, n, c->dstate);
+    k_group_bbox<<<(unsigned)nwarp_blocks, TB, 0, s>>>(c->spos, c->gfirst, c->gcount, c->gbox, c->g_taskoff, n, (uint32_t)c->ngroup_cap, c->dstate);
     dsk_exclusive_scan_u32(c, c->g_taskoff, c->g_taskoff, &c->dstate->ngroup, (uint32_t)c->ngroup_cap, &c->dstate->ntask);
-    k_task_fill<<<(unsigned)((c->ngroup_cap + TB - 1) / TB), TB, 0, s>>>(c->g_taskoff, c->g_task, c->dstate);
+    k_task_fill<<<(unsigned)((c->ngroup_cap + TB - 1) / TB), TB, 0, s>>>(c->g_taskoff, c->g_task, (uint32_t)c->ngroup_cap, c->dstate);
     cudaEventRecord(c->ev[4], s);
     DSK_COUNT(c, 1 + 1 + 5);   // init, the fused level loop, mark/flag/emit/bbox/taskfill
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;

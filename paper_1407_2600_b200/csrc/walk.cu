@@ -4,7 +4,7 @@
 //   accept cell c (image shift nL) for group g  iff  d^2 > (s_c/theta + delta_c)^2   (strict)
 //   d = distance from com_c + nL to the AABB of g's members.
 // accepted -> M2P list; rejected leaf -> P2P list; rejected internal -> children are visited.
-// One warp per group, 32 cells tested per step from a LIFO stack in shared memory (depth-first order
+// One warp per group, 64 cells tested per trip (two stack entries per lane) from a LIFO stack in shared memory (depth-first order
 // keeps it short); list entries are compacted with ballots and written as contiguous runs.
 // Run once into a fixed capacity per group when every list fits (the usual case), else twice: COUNT (list
 // lengths, for the offsets) and FILL.
