@@ -198,6 +198,29 @@ class OracleTree:
         return int(a.value), int(b.value), int(c.value)
 
 
+    def lists(self, theta, g, ws=WS):
+        """the two interaction lists of group g as (m2p_cell, m2p_img, p2p_cell, p2p_img), walk order"""
+        if self.p < 0:
+            self.moments(2)
+        nm = C.c_int64(0); npp = C.c_int64(0)
+        f = lib().orc_group_lists
+        f(self._h, C.c_double(theta), C.c_int(ws), C.c_int64(g), C.c_int64(0), None, None, C.byref(nm), None, None,
+          C.byref(npp))
+        cap = max(nm.value, npp.value, 1)
+        mc = np.empty(cap, np.int64); mi = np.empty(cap, np.int32); pc = np.empty(cap, np.int64); pi = np.empty(cap, np.int32)
+        f(self._h, C.c_double(theta), C.c_int(ws), C.c_int64(g), C.c_int64(cap), _p(mc), _p(mi), C.byref(nm), _p(pc), _p(pi),
+          C.byref(npp))
+        return mc[:nm.value], mi[:nm.value], pc[:npp.value], pi[:npp.value]
+
+
+def image_shift(img, box, periodic, ws=WS):
+    """image id -> shift vector n L (ids run over ix, iy, iz in {-ws..ws}, iz fastest)"""
+    if not periodic:
+        return np.zeros(3)
+    side = 2 * ws + 1
+    return box * np.array([img // (side * side) - ws, (img // side) % side - ws, img % side - ws], dtype=np.float64)
+
+
 def tree_force(pos, mass, box, periodic, eps, theta, p, sink=None, tree=None, ws=WS):
     """The whole oracle path Tr: tree sum over the image block (+ O7 far field when periodic).
     Returns acc, pot, n_p2p, n_m2p, tree."""

@@ -79,6 +79,9 @@ int orc_tree_accel(orc_tree *t, double eps, double theta, int ws, int64_t nsink,
 void orc_group_list_counts(orc_tree *t, double theta, int ws, int64_t g, int64_t *n_m2p_cells,
                            int64_t *n_p2p_leaves, int64_t *n_p2p_particles);
 
+void orc_group_lists(orc_tree *t, double theta, int ws, int64_t g, int64_t cap, int64_t *m2p_cell,
+                     int32_t *m2p_img, int64_t *n_m2p, int64_t *p2p_cell, int32_t *p2p_img, int64_t *n_p2p);
+
 /* D-per, O7 (orc_periodic.c) */
 void orc_ewald_pair(const double x[3], double L, double alpha, int nmax, int hmax, double *psi,
                     double a[3]);

@@ -168,6 +168,19 @@ void orc_group_list_counts(orc_tree *t, double theta, int ws, int64_t g, int64_t
     free(m2p.cell); free(m2p.img); free(p2p.cell); free(p2p.img);
 }
 
+/* The two lists of group g themselves (for the tests that pin the acceptance rule): cell indices (canonical
+ * order) and image ids, in walk order.  Call with cap = 0 to get the lengths, then with buffers of that size. */
+void orc_group_lists(orc_tree *t, double theta, int ws, int64_t g, int64_t cap, int64_t *m2p_cell,
+                     int32_t *m2p_img, int64_t *n_m2p, int64_t *p2p_cell, int32_t *p2p_img, int64_t *n_p2p)
+{
+    ilist_t m2p = {0}, p2p = {0};
+    walk_group(t, g, theta, ws, &m2p, &p2p);
+    *n_m2p = m2p.n; *n_p2p = p2p.n;
+    for (int64_t k = 0; k < m2p.n && k < cap; k++) { m2p_cell[k] = m2p.cell[k]; m2p_img[k] = m2p.img[k]; }
+    for (int64_t k = 0; k < p2p.n && k < cap; k++) { p2p_cell[k] = p2p.cell[k]; p2p_img[k] = p2p.img[k]; }
+    free(m2p.cell); free(m2p.img); free(p2p.cell); free(p2p.img);
+}
+
 /* group containing sorted rank r (groups tile [0,n) in Morton order) */
 static int64_t group_of_rank(const orc_tree *t, int64_t r)
 {

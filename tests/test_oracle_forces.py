@@ -230,3 +230,118 @@ def test_tree_subset_equals_full(orc):
     sink = np.array([5, 17, 2999, 1234, 0])
     sub, sp, _, _ = t.accel(1e-3, 0.5, 4, sink)
     assert np.array_equal(sub, full[sink]) and np.array_equal(sp, fp[sink])
+
+
+# ---- O5: the acceptance rule itself (PAPER.md:61 traversal, :73 "grouping and multipole acceptance tests") --------
+def _lists_case(orc, periodic):
+    rng = np.random.default_rng(21 + int(periodic))
+    n = 5000
+    c = rng.random((12, 3))
+    pos = c[rng.integers(12, size=n)] + 0.03 * rng.standard_normal((n, 3))
+    pos[: n // 4] = rng.random((n // 4, 3))
+    pos = (np.mod(pos, 1.0) if periodic else np.clip(pos, 0.0, 0.999999)).astype(np.float32)
+    pos[pos >= 1.0] = 0.0
+    mass = rng.uniform(0.5, 1.5, n).astype(np.float32) / n
+    t = orc.OracleTree(pos, mass, 1.0, periodic, nleaf=16, ncrit=32)
+    return pos, mass, t
+
+
+@pytest.mark.parametrize("periodic", [False, True])
+@pytest.mark.parametrize("theta", [0.3, 0.7, 1.0])
+def test_lists_partition_and_validity(orc, periodic, theta):
+    """What the mathematics fixes about the lists of reading O5, whatever the MAC's exact form:
+    PARTITION  per group and image, the listed leaves' particles plus the accepted cells' particles are all N
+               particles exactly once (every source is summed once, either directly or inside one expansion);
+    VALIDITY   for every accepted (cell, image) every sink of the group is farther from the expansion centre
+               z_c + nL than every source of the cell (the expansion converges), with the margin the rule promises:
+               min sink distance >= d_AABB > s/theta + delta >= max source distance + s (1/theta - sqrt(3)/2);
+    RULE       recomputed here from cells(), moments() and the group's box: every accepted entry satisfies
+               d^2 > (s/theta + delta)^2 and every listed leaf and every opened ancestor fails it."""
+    ws = 1
+    pos, mass, t = _lists_case(orc, periodic)
+    n = len(pos)
+    cm, com, dl, _ = t.moments(2)
+    cells, grp = t.cells(), t.groups()
+    _, order = t.sorted()
+    wp = t.wrapped_pos().astype(np.float64)
+    spos = wp[order]
+    side = 2.0 ** (-cells["level"].astype(np.float64))
+    nimg = (2 * ws + 1) ** 3 if periodic else 1
+    # farthest source of every cell from its centre of mass
+    rmax = np.array([np.linalg.norm(spos[f:f + c] - com[i], axis=1).max() for i, (f, c) in enumerate(zip(cells["first"], cells["count"]))])
+    parent = np.full(t.ncell, -1)
+    for c in range(t.ncell):
+        for k in range(cells["nchild"][c]):
+            parent[cells["child0"][c] + k] = c
+
+    def d2_aabb(bb, z):
+        lo = bb[:3].astype(np.float64) - z; hi = z - bb[3:].astype(np.float64)
+        d = np.maximum(np.maximum(lo, hi), 0.0)
+        return float(d @ d)
+
+    for g in np.random.default_rng(5).choice(t.ngroup, 40, replace=False):
+        mc, mi, pc, pi = t.lists(theta, int(g), ws)
+        sinks = spos[grp["first"][g]:grp["first"][g] + grp["count"][g]]
+        bb = grp["bbox"][g]
+        per_img = np.zeros(nimg, np.int64)
+        np.add.at(per_img, mi, cells["count"][mc])
+        np.add.at(per_img, pi, cells["count"][pc])
+        assert np.all(per_img == n), (g, per_img)
+        opened = set()
+        for c, im in zip(mc, mi):
+            z = com[c] + orc.image_shift(int(im), 1.0, periodic, ws)
+            dmin = np.linalg.norm(sinks - z, axis=1).min()
+            assert dmin > rmax[c] + side[c] * (1.0 / theta - math.sqrt(3) / 2) * (1 - 1e-12) - 1e-15
+            assert d2_aabb(bb, z) > (side[c] / theta + dl[c]) ** 2
+            a = parent[c]
+            while a >= 0 and (a, int(im)) not in opened:
+                opened.add((int(a), int(im))); a = parent[a]
+        for c, im in zip(pc, pi):
+            assert cells["nchild"][c] == 0
+            z = com[c] + orc.image_shift(int(im), 1.0, periodic, ws)
+            assert not d2_aabb(bb, z) > (side[c] / theta + dl[c]) ** 2
+            a = parent[c]
+            while a >= 0 and (a, int(im)) not in opened:
+                opened.add((int(a), int(im))); a = parent[a]
+        for a, im in opened:
+            z = com[a] + orc.image_shift(im, 1.0, periodic, ws)
+            assert not d2_aabb(bb, z) > (side[a] / theta + dl[a]) ** 2
+        # counts agree with the separate counter
+        assert t.list_counts(theta, int(g), ws) == (len(mc), len(pc), int(cells["count"][pc].sum()))
+
+
+def test_lists_hand_built_case(orc):
+    """Four particles whose tree and lists are worked out by hand (all coordinates are exact binary fractions):
+        S  = (1/16, 1/8, 1/8)  m 1     S' = (3/8, 1/8, 1/8)  m 1     A1 = (13/16, 1/8, 1/8)  m 1     A2 = (15/16, 1/8, 1/8)  m 3
+    NLEAF = NCRIT = 1, so every particle is a leaf and a group.  Cells (hotkey): root 1; octant 0 = 8 {S, S'} with leaves
+    64 (S) and 68 (S'); octant 4 = 12 {A1, A2} -> its only child 100 (side 1/4, centre (7/8, 1/8, 1/8)) -> leaves 803 (A1), 807 (A2).
+    Cell 100: centre of mass x = (13/16 + 3 * 15/16)/4 = 29/32, so delta = 1/32 and s/theta + delta = 1/(4 theta) + 1/32.
+    Sink S (group box = the point S, 1/16 off the centre of its own cell): d = 29/32 - 1/16 = 27/32 = 0.84375 from 100's centre of mass.
+      theta = 0.30: 0.8333 + 0.03125 = 0.8646 > d  -> 100 is opened, its leaves (d = 0.75, 0.875 > 0.4167 + 0.0884) are accepted.
+                    Dropping delta (0.8333 < d) would accept 100 instead.
+      theta = 0.31: 0.8065 + 0.03125 = 0.8377 < d  -> 100 is accepted.  Measuring d to the centre of S's cell (1/8, 1/8, 1/8),
+                    d = 25/32 = 0.78125 < 0.8377, would open it instead.
+    Sink S': d = 29/32 - 3/8 = 17/32 = 0.53125 = 1/(4 * 0.5) + 1/32 EXACTLY at theta = 0.5: the test is strict, 100 is opened
+                    (its leaves, d = 0.4375 and 0.5625 > 0.25 + 0.0884, are accepted); '>=' would accept 100."""
+    pos = np.array([[1 / 16, 1 / 8, 1 / 8], [3 / 8, 1 / 8, 1 / 8], [13 / 16, 1 / 8, 1 / 8], [15 / 16, 1 / 8, 1 / 8]], np.float32)
+    mass = np.array([1, 1, 1, 3], np.float32)
+    t = orc.OracleTree(pos, mass, 1.0, False, nleaf=1, ncrit=1)
+    cells, grp = t.cells(), t.groups()
+    assert [int(h) for h in cells["hotkey"]] == [1, 8, 12, 64, 68, 100, 803, 807]
+    cm, com, dl, _ = t.moments(2)
+    c100 = list(cells["hotkey"]).index(100)
+    assert com[c100][0] == 29 / 32 and dl[c100] == 1 / 32
+    assert t.ngroup == 4 and list(grp["first"]) == [0, 1, 2, 3]          # Morton order: S, S', A1, A2
+    hk = lambda idx: sorted(int(cells["hotkey"][i]) for i in idx)       # noqa: E731
+
+    mc, _, pc, _ = t.lists(0.30, 0)
+    assert hk(mc) == [803, 807] and hk(pc) == [64, 68]
+    mc, _, pc, _ = t.lists(0.31, 0)
+    assert hk(mc) == [100] and hk(pc) == [64, 68]
+    mc, _, pc, _ = t.lists(0.5, 1)
+    assert hk(mc) == [803, 807] and hk(pc) == [64, 68]
+    # and the sources' side: A1 at theta = 0.5 sees octant 0 as one cell?  cell 8: centre of mass x = 7/32, centre 1/4,
+    # delta = 1/32; d = 13/16 - 7/32 = 19/32 = 0.594 < 1.0 + 0.031 -> opened; leaves 64 (delta 1/16, d 0.75 > 0.5625) and
+    # 68 (delta 0, d 0.4375 < 0.5) -> 64 accepted, 68 direct; its own cell 12 and sibling leaf 807 are direct.
+    mc, _, pc, _ = t.lists(0.5, 2)
+    assert hk(mc) == [64] and hk(pc) == [68, 803, 807]
