@@ -185,23 +185,16 @@ def run_reference(args):
 
 
 # ---- our arm ------------------------------------------------------------------------------------------------
-def run_ours(args):
+def measure_config(cfgid, steps, warmup, dev, world, rank, dist, want_e2e, want_cpu, peak_meas):
+    """Time `steps` steps of BASELINE.json config `cfgid` on this rank's device (after max(warmup, 3) untimed ones) and
+    return the dict of everything the JSON line reports about it (rank 0; None on the other ranks)."""
     import torch
-    import torch.distributed as dist
-    from paper_1407_2600_b200 import accounting, dsk
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
+    from paper_1407_2600_b200 import accounting, dsk, workloads
+    global CFG
+    CFG = cfgid
     use_dist = world > 1
-    if use_dist:
-        dist.init_process_group("nccl", device_id=dev)
-
-    cfg, pos, mass = workload()
+    cfg = dict(workloads.CONFIGS[cfgid])
+    pos, mass = workloads.make(cfgid)
     n = len(pos)
     d = dsk.Dsk(n, cfg["box"], cfg["periodic"], cfg["eps"], cfg["theta"], cfg["p"], device=dev)
     stream = torch.cuda.current_stream(dev)
@@ -209,19 +202,19 @@ def run_ours(args):
     acc = torch.empty((n, 3), dtype=torch.float32, device=dev)
     pot = torch.empty(n, dtype=torch.float32, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    # pinned host buffers for the end-to-end arm
-    hp, hm = torch.from_numpy(pos).pin_memory(), torch.from_numpy(mass).pin_memory()
-    hacc = torch.empty((n, 3), dtype=torch.float32).pin_memory()
-    hpot = torch.empty(n, dtype=torch.float32).pin_memory()
-    tp2, tm2 = torch.empty_like(tp), torch.empty_like(tm)
-
-    kdk = CFG == 5          # configs[4] is a run: a step is one dsk_kdk_step (kick, drift, tree, force, kick)
+    kdk = cfgid == 5          # configs[4] is a run: a step is one dsk_kdk_step (kick, drift, tree, force, kick)
+    if want_e2e:              # pinned host buffers for the end-to-end arm
+        hp, hm = torch.from_numpy(pos).pin_memory(), torch.from_numpy(mass).pin_memory()
+        hacc = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+        hpot = torch.empty(n, dtype=torch.float32).pin_memory()
+        tp2, tm2 = torch.empty_like(tp), torch.empty_like(tm)
     if kdk:
         vel = torch.zeros_like(tp)              # cold start
-        hv = torch.zeros((n, 3), dtype=torch.float32).pin_memory()
-        vel2 = torch.empty_like(tp)
         clock = {"a": 0.5}
         DA = 0.01
+        if want_e2e:
+            hv = torch.zeros((n, 3), dtype=torch.float32).pin_memory()
+            vel2 = torch.empty_like(tp)
 
         def step():
             d.kdk_step(tp, vel, tm, clock["a"], DA)
@@ -249,11 +242,12 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    def timed(fn, steps):
+    def timed(fn, nsteps):
         """sum over steps of the CUDA-event time of each step on the launching stream; L2 flushed between"""
         tot = 0.0
         phase = {}
-        for _ in range(steps):
+        st = None
+        for _ in range(nsteps):
             flush.fill_(1)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(stream)
@@ -265,28 +259,33 @@ def run_ours(args):
             for k, v in st.items():
                 if k.startswith("ms_"):
                     phase[k] = phase.get(k, 0.0) + v
-        return tot, {k: v / steps for k, v in phase.items()}, st
+        return tot, {k: v / nsteps for k, v in phase.items()}, st
 
-    for _ in range(max(args.warmup, 3)):
+    nwarm = max(warmup, 3)
+    for _ in range(nwarm):
         step()
     barrier()
-    clocks = ClockSampler(local)
+    clocks = ClockSampler(dev.index or 0)
     if rank == 0:
         clocks.start()
-    ms_total, phase, st = timed(step, args.steps)
+    ms_total, phase, st = timed(step, steps)
     barrier()
     clk = clocks.stop() if rank == 0 else None
-    ms_max, units = aggregate(dist if use_dist else None, ms_total, n * args.steps, dev)
+    ms_max, units = aggregate(dist if use_dist else None, ms_total, n * steps, dev)
     value = units / (ms_max * 1e-3)
 
-    # end-to-end: pinned host -> device, the same step, device -> pinned host, all inside the event pair
-    for _ in range(2):
-        step_e2e()
-    barrier()
-    ms_e2e, _, _ = timed(step_e2e, args.steps)
-    barrier()
-    ms_e2e_max, units_e = aggregate(dist if use_dist else None, ms_e2e, n * args.steps, dev)
-    e2e_value = units_e / (ms_e2e_max * 1e-3)
+    e2e = None
+    if want_e2e:      # pinned host -> device, the same step, device -> pinned host, all inside the event pair
+        for _ in range(2):
+            step_e2e()
+        barrier()
+        ms_e2e, _, _ = timed(step_e2e, steps)
+        barrier()
+        ms_e2e_max, units_e = aggregate(dist if use_dist else None, ms_e2e, n * steps, dev)
+        e2e = {"value": units_e / (ms_e2e_max * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": int(hp.numel() * 4 + hm.numel() * 4 + (hv.numel() * 4 if kdk else 0)),
+               "d2h_bytes_per_step": int(hacc.numel() * 4 + (hv.numel() * 4 if kdk else hpot.numel() * 4)),
+               "ms_per_step": ms_e2e_max / steps}
 
     out = None
     if rank == 0:
@@ -298,6 +297,7 @@ def run_ours(args):
             pass
         sm_max = float(peaks.get("sm_max_mhz", 1965.0))
         peak_fp32 = accounting.fp32_peak_flops(prop.multi_processor_count, sm_max)
+        pm = peak_meas["tflops"] * 1e12 if peak_meas else None          # best measured FFMA2 rate (dsk_probe_fp32_peak)
         f_m2p = accounting.m2p_flops(cfg["p"], pot=not kdk)      # dsk_kdk_step asks for no potential
         f_p2p = accounting.p2p_flops(pot=not kdk)
         ach_m2p = f_m2p * st["n_m2p"] / (phase["ms_m2p"] * 1e-3)
@@ -321,48 +321,106 @@ def run_ours(args):
                 hbm_phases[key] = {"GBps": b / (ms * 1e-3) / 1e9, "frac": b / (ms * 1e-3) / 1e9 / hbm}
         traffic = None
         tpath = os.path.join(ROOT, "profiles", "m2p_dram_bytes_per_launch.txt")
-        if CFG == 2 and os.path.exists(tpath):                   # captured on the default workload only
+        if cfgid == 2 and os.path.exists(tpath):                 # captured on the default workload only
             try:
                 traffic = float(open(tpath).read().split()[0])
             except Exception:
                 traffic = None
-        # CPU oracle beside it (bounded sample, rank 0, N = 1 only)
         cpu = None
-        if world == 1 and not args.no_cpu_baseline:
+        if want_cpu:          # CPU oracle beside it (bounded sample, rank 0, N = 1 only)
             v, info = oracle_rate(cfg, pos, mass, 16384)
             cpu = {"value": v, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
                    "sample": (f"oracle tree Tr fp64 OpenMP: build+moments on all N ({info['t_build_s']} s), forces on "
                               f"{info['nsink']} of {n} sinks = whole groups ({info['t_force_sample_s']} s) extrapolated to N")}
-        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-               "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        variant = "nopot" if kdk else "pot"
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
+               "warmup": nwarm, "ms_per_step": ms_max / steps, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                "config": config_dict(cfg, world, (dsk.get_param("NLEAF"), dsk.get_param("NCRIT"))),
-               "roofline": {"bound": "alu", "kernel": f"k_m2p<{cfg['p']},{'nopot' if kdk else 'pot'},{'fp64 monopoles' if cfg['periodic'] else 'fp32'}>", "achieved": ach_m2p / 1e12,
-                            "peak": peak_fp32 / 1e12, "unit": "TFLOP/s", "frac": ach_m2p / peak_fp32,
+               "roofline": {"bound": "alu", "kernel": f"k_m2p<{cfg['p']},{variant},{'periodic' if cfg['periodic'] else 'isolated'}>",
+                            "achieved": ach_m2p / 1e12, "peak": peak_fp32 / 1e12, "unit": "TFLOP/s", "frac": ach_m2p / peak_fp32,
+                            "peak_measured": pm / 1e12 if pm else None, "frac_measured": ach_m2p / pm if pm else None,
                             "traffic": traffic,
-                            "peak_source": f"nominal FP32: {prop.multi_processor_count} SMs x 128 lanes x 2 x {sm_max:.0f} MHz "
-                                           "(DESIGN.md; FFMA2 microbenchmark measured 74.06 TFLOP/s on this pool)",
+                            "traffic_source": "profiles/m2p_dram_bytes_per_launch.txt (one ncu --set full capture of this launch, not re-measured here)" if traffic else None,
+                            "peak_source": f"nominal FP32: {prop.multi_processor_count} SMs x 128 lanes x 2 x {sm_max:.0f} MHz; "
+                                           "peak_measured = best FFMA2 form of dsk_probe_fp32_peak in this run (fp32_peak_probe)",
                             "flop_per_interaction": f_m2p,
                             "flop_per_interaction_survey_estimate": 8 * ((cfg["p"] + 1) * (cfg["p"] + 2) * (cfg["p"] + 3) // 6)
                             + 5 * ((cfg["p"] + 2) * (cfg["p"] + 3) * (cfg["p"] + 4) // 6),
                             "interactions_per_launch": st["n_m2p"],
                             "ms_per_launch": phase["ms_m2p"]},
                "kernels": {"p2p": {"TFLOPs": ach_p2p / 1e12, "frac_fp32_peak": ach_p2p / peak_fp32,
+                                   "frac_fp32_measured": ach_p2p / pm if pm else None,
                                    "pairs_per_s": st["n_p2p"] / (phase["ms_p2p"] * 1e-3) if phase["ms_p2p"] > 0 else None,
                                    "flop_per_pair": f_p2p},
                            "m2p": {"interactions_per_s": st["n_m2p"] / (phase["ms_m2p"] * 1e-3)},
                            "hbm_phases": hbm_phases},
-               "interactions_per_s": (st["n_m2p"] + st["n_p2p"]) * world / (ms_max / args.steps * 1e-3),
+               "interactions_per_s": (st["n_m2p"] + st["n_p2p"]) * world / (ms_max / steps * 1e-3),
                "phase_ms": {k[3:]: round(v, 4) for k, v in phase.items()},
                "tree": {"ncell": st["ncell"], "ngroup": st["ngroup"], "nlevel": st["nlevel"],
                         "n_p2p": st["n_p2p"], "n_m2p": st["n_m2p"], "nbatch": st["nbatch"]},
                "cpu_baseline": cpu,
-               "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(hp.numel() * 4 + hm.numel() * 4),
-                       "d2h_bytes_per_step": int(hacc.numel() * 4 + hpot.numel() * 4),
-                       "ms_per_step": ms_e2e_max / args.steps},
-               "gpu_launches": int(st["n_launch"]) * args.steps,
+               "e2e": e2e,
+               "gpu_launches": int(st["n_launch"]) * steps,
                "clocks": clk}
     d.close()
+    del d, tp, tm, acc, pot, flush
+    torch.cuda.empty_cache()
+    return out
+
+
+def probe_peak():
+    """dsk_probe_fp32_peak, all three operand forms (include/dsk.h): the measured FP32 denominator."""
+    from paper_1407_2600_b200 import dsk
+    forms = ("ffma2_three_packed_operands", "ffma2_one_scalar_broadcast_operand", "scalar_ffma_three_registers")
+    res = {}
+    for v, name in enumerate(forms):
+        t, c, m = dsk.probe_fp32_peak(v)
+        res[name] = {"TFLOPs": round(t, 3), "cycles_per_warp_inst_per_smsp": round(c, 4), "sm_mhz": round(m, 1)}
+    res["tflops"] = max(res[forms[0]]["TFLOPs"], res[forms[1]]["TFLOPs"])
+    return res
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    use_dist = world > 1
+    if use_dist:
+        dist.init_process_group("nccl", device_id=dev)
+    if args.peak:
+        if rank == 0:
+            print(json.dumps({"fp32_peak_probe": probe_peak()}))
+        if use_dist:
+            dist.destroy_process_group()
+        return
+    peak_meas = probe_peak() if rank == 0 else None
+    head_cfg = args.config
+    out = measure_config(head_cfg, args.steps, args.warmup, dev, world, rank, dist, True,
+                         world == 1 and not args.no_cpu_baseline, peak_meas)
+    if rank == 0:
+        out["fp32_peak_probe"] = peak_meas
+    # The other BASELINE.json configs, AFTER the headline's timed region (so that it does not move): fewer steps, no
+    # end-to-end arm, no CPU leg; same timing protocol.  N = 1 only.
+    if world == 1 and head_cfg == 2 and not args.no_other_configs:
+        others = {}
+        for cid, nst in ((1, 5), (3, 3), (4, 3), (5, 2)):
+            try:
+                o = measure_config(cid, nst, 3 if cid != 5 else 1, dev, 1, 0, None, False, False, peak_meas)
+                others[f"configs[{cid - 1}]"] = {k: o[k] for k in ("value", "unit", "steps", "warmup", "ms_per_step", "config", "phase_ms",
+                                                                 "tree", "interactions_per_s", "clocks", "gpu_launches")} | {
+                    "m2p_frac_fp32_peak": o["roofline"]["frac"], "m2p_frac_fp32_measured": o["roofline"]["frac_measured"],
+                    "p2p_frac_fp32_peak": o["kernels"]["p2p"]["frac_fp32_peak"], "hbm_phases": o["kernels"]["hbm_phases"]}
+            except Exception as ex:          # e.g. not enough device memory for 512^3 on a shared box: say so, keep the headline
+                others[f"configs[{cid - 1}]"] = {"error": repr(ex)[:300]}
+        out["other_configs"] = others
     if use_dist:
         dist.destroy_process_group()
     if rank == 0:
@@ -376,6 +434,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the C1/C3/C4/C5 lines appended to the default run")
+    ap.add_argument("--peak", action="store_true", help="only run the FP32 issue-rate probe (dsk_probe_fp32_peak) and print it")
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5],
                     help="BASELINE.json config number (1-based); the default 2 is the workload the metric is quoted on")
     args = ap.parse_args()

@@ -112,7 +112,10 @@ int dsk_kdk_reset(dsk_ctx *ctx);
 
 /* Diagnostic: mode 0 (default) lets the walk try its one-pass form (lists written into a fixed capacity per group,
  * fallback to COUNT + FILL when one does not fit); mode 1 always takes the two-pass form; mode 2 gives the one-pass
- * attempt capacities that overflow, so that every evaluation exercises the fallback.  Results are identical. */
+ * attempt capacities that overflow, so that every evaluation exercises the fallback; mode 3 takes the two-pass form and
+ * pretends the list buffers hold 65536 / 8192 entries, so that even a small input is evaluated in batches of groups (the
+ * path a 512^3 run takes).  Results are identical in modes 0-3.  Mode 4 pretends they hold 256 / 8 entries: a group whose
+ * lists are longer cannot be evaluated and dsk_accel returns DSK_ELISTOVERFLOW (the context stays usable). */
 int dsk_set_walk_mode(dsk_ctx *ctx, int mode);
 
 /* One BLOCK step of size da with hierarchical individual time steps (reading O9c of DESIGN.md; "adaptive
@@ -141,6 +144,9 @@ int dsk_get_tree(dsk_ctx *ctx, int64_t *ncell, uint64_t *hotkey, uint32_t *first
 /* per cell (canonical order): com_mass dev [ncell,4] = (com x,y,z, mass); moments dev [ncell,N_p] =
  * raw (unscaled) Cartesian moments M_n = sum m (y - com)^n of the current order p.  Either may be NULL. */
 int dsk_get_moments(dsk_ctx *ctx, float *com_mass, float *moments);
+/* the same with the moments in units of the cell side s = box 2^-level: M_n / s^|n| (what the library stores: at p = 8
+ * the raw moments of a level >= 15 cell, ~ m s^8, are below the fp32 range, SURVEY.md section 7 hard part 2). */
+int dsk_get_moments_scaled(dsk_ctx *ctx, float *com_mass, float *moments);
 /* sink groups in Morton order: *ngroup host; first/count dev [ngroup], bbox dev [ngroup,6] (min, max);
  * m2p_len/p2p_len dev [ngroup] = list lengths of the last walk (cells / leaves).  Arrays may be NULL. */
 int dsk_get_groups(dsk_ctx *ctx, int64_t *ngroup, uint32_t *first, uint32_t *count, float *bbox,
@@ -154,6 +160,13 @@ int dsk_get_param(const char *name, double *value);
 int dsk_get_task_widths(int n, int widths[4]);
 /* far-field lattice tensors T_n (|n| <= 8, 165 doubles, host) of this context; periodic only. */
 int dsk_get_lattice_tensors(dsk_ctx *ctx, double *T /* host [165] */);
+/* FP32 issue-rate probe: the measured denominator of the force kernels' roofline (the force path of
+ * PAPER.md:73-75 is FP32 FMA work).  Runs a pure FMA kernel on the current device (default stream, its own few MB of
+ * device memory) and writes to HOST pointers: TFLOP/s (FMA = 2 flop per lane), cycles per warp instruction per SM
+ * sub-partition, and the SM clock in MHz the kernel ran at.  variant 0: packed fma.rn.f32x2 with three register operands;
+ * 1: packed, one operand a scalar broadcast to both halves (the form the force kernels feed sources in); 2: scalar FFMA
+ * with three distinct registers.  DSK_EINVAL for another variant or a NULL pointer, DSK_ECUDA without a device. */
+int dsk_probe_fp32_peak(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz);
 const char *dsk_strerror(int err);
 
 #ifdef __cplusplus

@@ -194,9 +194,19 @@ void orc_direct_per(int64_t n, const float *pos, const float *mass, double L, do
             double d[3], m = (double)mass[j], a[3] = {0, 0, 0}, ph = mtot_term;
             for (int k = 0; k < 3; k++) d[k] = xi[k] - (double)pos[3 * j + k];
             int zero = (d[0] == 0.0 && d[1] == 0.0 && d[2] == 0.0);
-            for (int ix = -nmax; ix <= nmax; ix++)
-                for (int iy = -nmax; iy <= nmax; iy++)
-                    for (int iz = -nmax; iz <= nmax; iz++) {
+            /* only the images that can contribute are visited: the real-space term needs |d - nL| < rcut, so per axis
+             * n lies in [(d - rcut)/L, (d + rcut)/L]; the range is widened to hold the whole image block */
+            int lo[3], hi[3];
+            for (int k = 0; k < 3; k++) {
+                lo[k] = (int)ceil((d[k] - rcut) / L); hi[k] = (int)floor((d[k] + rcut) / L);
+                if (lo[k] > -ws) lo[k] = -ws;
+                if (hi[k] < ws) hi[k] = ws;
+                if (lo[k] < -nmax) lo[k] = -nmax;
+                if (hi[k] > nmax) hi[k] = nmax;
+            }
+            for (int ix = lo[0]; ix <= hi[0]; ix++)
+                for (int iy = lo[1]; iy <= hi[1]; iy++)
+                    for (int iz = lo[2]; iz <= hi[2]; iz++) {
                         double dn[3] = { d[0] - ix * L, d[1] - iy * L, d[2] - iz * L };
                         int inblock = (abs(ix) <= ws && abs(iy) <= ws && abs(iz) <= ws);
                         if (zero && !ix && !iy && !iz) {

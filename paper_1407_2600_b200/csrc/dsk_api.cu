@@ -339,7 +339,7 @@ extern "C" int dsk_set_cosmology(dsk_ctx *c, double omega_m, double omega_lambda
 
 extern "C" int dsk_set_walk_mode(dsk_ctx *c, int mode)
 {
-    if (!c || mode < 0 || mode > 2) return DSK_EINVAL;
+    if (!c || mode < 0 || mode > 4) return DSK_EINVAL;
     c->walk_two_pass_only = mode;
     c->onepass_bad_theta = -1.0f;
     c->lists_valid = 0;
@@ -488,7 +488,7 @@ extern "C" int dsk_get_tree(dsk_ctx *c, int64_t *ncell, uint64_t *hotkey, uint32
     return DSK_OK;
 }
 
-extern "C" int dsk_get_moments(dsk_ctx *c, float *com_mass, float *moments)
+static int get_moments_impl(dsk_ctx *c, float *com_mass, float *moments, int scaled)
 {
     if (!c) return DSK_EINVAL;
     if (!c->have_tree) return DSK_ENOTREE;
@@ -496,8 +496,10 @@ extern "C" int dsk_get_moments(dsk_ctx *c, float *com_mass, float *moments)
         int e = dsk_run_upward(c);
         if (e) return e;
     }
-    return dsk_run_get_moments(c, com_mass, moments);
+    return dsk_run_get_moments(c, com_mass, moments, scaled);
 }
+extern "C" int dsk_get_moments(dsk_ctx *c, float *com_mass, float *moments) { return get_moments_impl(c, com_mass, moments, 0); }
+extern "C" int dsk_get_moments_scaled(dsk_ctx *c, float *com_mass, float *moments) { return get_moments_impl(c, com_mass, moments, 1); }
 
 __global__ void k_unpack_gbox(const float4 *__restrict__ gbox, uint32_t n, float *out)
 {

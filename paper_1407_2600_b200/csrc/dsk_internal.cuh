@@ -204,7 +204,7 @@ void dsk_exclusive_scan_u32(dsk_ctx *c, const uint32_t *in, uint32_t *out, const
                             uint32_t n_max, uint32_t *total_dev);             // keysort.cu
 int dsk_run_build(dsk_ctx *c);                                                // tree.cu: T, G
 int dsk_run_upward(dsk_ctx *c);                                               // upward.cu: U
-int dsk_run_get_moments(dsk_ctx *c, float *com_mass, float *moments);         // upward.cu
+int dsk_run_get_moments(dsk_ctx *c, float *com_mass, float *moments, int scaled);         // upward.cu
 int dsk_run_walk(dsk_ctx *c);                                                 // walk.cu: W
 int dsk_run_force(dsk_ctx *c, int want_pot);                                  // force.cu: F1 + orchestration
 int dsk_frow_len(int p);                                                      // m2p.cu

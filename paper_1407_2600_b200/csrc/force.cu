@@ -290,7 +290,11 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     DSK_CUDA(cudaStreamSynchronize(s));
     // reset the interaction counters (filled by the FILL pass)
     DSK_CUDA(cudaMemsetAsync(&c->dstate->tot_m2p_list, 0, sizeof(unsigned long long) * 5, s));
-    if (tot[0] <= c->list_m2p_cap && tot[1] <= c->list_p2p_cap) {
+    // diagnostic modes 3 / 4 (dsk_set_walk_mode): pretend the list buffers are small (batches on small inputs) or tiny
+    // (not even one group fits: DSK_ELISTOVERFLOW)
+    const size_t cap_m = c->walk_two_pass_only == 3 ? (size_t)65536 : c->walk_two_pass_only == 4 ? (size_t)256 : c->list_m2p_cap;
+    const size_t cap_p = c->walk_two_pass_only == 3 ? (size_t)8192 : c->walk_two_pass_only == 4 ? (size_t)8 : c->list_p2p_cap;
+    if (tot[0] <= cap_m && tot[1] <= cap_p) {
         int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, want_pot, true);
         if (e) return e;
         DSK_CUDA(cudaStreamSynchronize(s));
@@ -315,7 +319,7 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     int nb = 0, rc = DSK_OK;
     while (g0 < ng) {
         uint32_t g1 = g0;
-        while (g1 < ng && hm[g1 + 1] - hm[g0] <= c->list_m2p_cap && hp[g1 + 1] - hp[g0] <= c->list_p2p_cap) g1++;
+        while (g1 < ng && hm[g1 + 1] - hm[g0] <= cap_m && hp[g1 + 1] - hp[g0] <= cap_p) g1++;
         if (g1 == g0) { rc = DSK_ELISTOVERFLOW; break; }           // one group alone does not fit
         cudaEventRecord(c->ev[11], s);
         rc = eval_batch(c, g0, g1, ht[g0], ht[g1], hm[g0], hp[g0], want_pot, true);

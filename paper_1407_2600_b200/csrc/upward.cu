@@ -362,7 +362,7 @@ int dsk_run_upward(dsk_ctx *c)
 // raw moments for parity tests: M_n = Mhat_n (-1)^|n| n! s^|n|
 template <int P>
 __global__ void k_get_moments(uint32_t ncell, const float *__restrict__ rows, float *__restrict__ com_mass,
-                              float *__restrict__ mom)
+                              float *__restrict__ mom, int scaled)
 {
     constexpr int NP = dsk_np(P), ROW = dsk_rowlen(P);
     uint32_t c = blockIdx.x;
@@ -376,19 +376,20 @@ __global__ void k_get_moments(uint32_t ncell, const float *__restrict__ rows, fl
     if (mom)
         for (int n = threadIdx.x; n < NP; n += blockDim.x) {
             float sp = 1.0f;
-            for (int t = 0; t < c_rank[n]; t++) sp *= s;
+            if (!scaled)
+                for (int t = 0; t < c_rank[n]; t++) sp *= s;
             mom[(size_t)c * NP + n] = row[8 + n] / c_sgn_invfact[n] * sp;
         }
 }
 
-int dsk_run_get_moments(dsk_ctx *c, float *com_mass, float *moments)
+int dsk_run_get_moments(dsk_ctx *c, float *com_mass, float *moments, int scaled)
 {
     uint32_t nc = c->hstate->ncell;
     switch (c->p) {
-    case 2: k_get_moments<2><<<nc, 32, 0, c->stream>>>(nc, c->rows, com_mass, moments); break;
-    case 4: k_get_moments<4><<<nc, 64, 0, c->stream>>>(nc, c->rows, com_mass, moments); break;
-    case 6: k_get_moments<6><<<nc, 96, 0, c->stream>>>(nc, c->rows, com_mass, moments); break;
-    case 8: k_get_moments<8><<<nc, 192, 0, c->stream>>>(nc, c->rows, com_mass, moments); break;
+    case 2: k_get_moments<2><<<nc, 32, 0, c->stream>>>(nc, c->rows, com_mass, moments, scaled); break;
+    case 4: k_get_moments<4><<<nc, 64, 0, c->stream>>>(nc, c->rows, com_mass, moments, scaled); break;
+    case 6: k_get_moments<6><<<nc, 96, 0, c->stream>>>(nc, c->rows, com_mass, moments, scaled); break;
+    case 8: k_get_moments<8><<<nc, 192, 0, c->stream>>>(nc, c->rows, com_mass, moments, scaled); break;
     default: return DSK_EINVAL;
     }
     DSK_CUDA(cudaStreamSynchronize(c->stream));

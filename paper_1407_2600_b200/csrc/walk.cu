@@ -266,7 +266,8 @@ int dsk_run_walk(dsk_ctx *c)
     c->walk_onepass = 0;
     const uint64_t cap_m = ng ? c->list_m2p_cap / ng : 0, cap_p = ng ? c->list_p2p_cap / ng : 0;
     const bool tiny = c->walk_two_pass_only == 2;          // diagnostic: capacities that overflow, to exercise the fallback
-    if (cap_m >= 4096 && cap_p >= 512 && (c->onepass_bad_theta != c->theta || tiny) && c->walk_two_pass_only != 1) {
+    if (cap_m >= 4096 && cap_p >= 512 && (c->onepass_bad_theta != c->theta || tiny) && c->walk_two_pass_only != 1 &&
+        c->walk_two_pass_only < 3) {
         DSK_CUDA(cudaMemsetAsync(&c->dstate->tot_m2p_list, 0, sizeof(unsigned long long) * 5, s));
         DSK_CUDA(cudaMemsetAsync(&c->dstate->scratch[0], 0, sizeof(unsigned long long), s));
         const uint32_t cm = tiny ? 64u : (uint32_t)(cap_m > 0xffffff00ull ? 0xffffff00ull : cap_m),

@@ -15,8 +15,8 @@ LIB_PATH = os.path.join(_HERE, "libdsk.so")
 SYMBOLS = [
     "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
     "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_get_keys",
-    "dsk_get_tree", "dsk_get_moments", "dsk_get_groups", "dsk_get_stats", "dsk_get_param", "dsk_get_task_widths",
-    "dsk_get_lattice_tensors", "dsk_strerror",
+    "dsk_get_tree", "dsk_get_moments", "dsk_get_moments_scaled", "dsk_get_groups", "dsk_get_stats", "dsk_get_param", "dsk_get_task_widths",
+    "dsk_get_lattice_tensors", "dsk_probe_fp32_peak", "dsk_strerror",
 ]
 
 
@@ -67,11 +67,13 @@ def load_library(path=LIB_PATH):
     lib.dsk_get_keys.argtypes = [vp, vp, vp]
     lib.dsk_get_tree.argtypes = [vp, C.POINTER(i64), vp, vp, vp, vp]
     lib.dsk_get_moments.argtypes = [vp, vp, vp]
+    lib.dsk_get_moments_scaled.argtypes = [vp, vp, vp]
     lib.dsk_get_groups.argtypes = [vp, C.POINTER(i64), vp, vp, vp, vp, vp]
     lib.dsk_get_stats.argtypes = [vp, C.POINTER(DskStats)]
     lib.dsk_get_param.argtypes = [C.c_char_p, C.POINTER(f64)]
     lib.dsk_get_task_widths.argtypes = [C.c_int, C.POINTER(C.c_int)]
     lib.dsk_get_lattice_tensors.argtypes = [vp, vp]
+    lib.dsk_probe_fp32_peak.argtypes = [i32, C.POINTER(f64), C.POINTER(f64), C.POINTER(f64)]
     lib.dsk_strerror.argtypes = [i32]
     lib.dsk_strerror.restype = C.c_char_p
     for s in SYMBOLS:
@@ -91,6 +93,13 @@ def get_task_widths(n):
     w = (C.c_int * 4)()
     _check(load_library().dsk_get_task_widths(int(n), w))
     return [int(x) for x in w if x]
+
+
+def probe_fp32_peak(variant):
+    """dsk_probe_fp32_peak: (TFLOP/s, cycles per warp instruction per SM sub-partition, SM MHz) of a pure FMA kernel"""
+    t, c, m = C.c_double(0), C.c_double(0), C.c_double(0)
+    _check(load_library().dsk_probe_fp32_peak(int(variant), C.byref(t), C.byref(c), C.byref(m)))
+    return t.value, c.value, m.value
 
 
 def _check(code):
@@ -223,11 +232,13 @@ class Dsk:
         _check(self.lib.dsk_get_tree(self._h, C.byref(n), _ptr(hot), _ptr(first), _ptr(count), _ptr(nchild)))
         return dict(ncell=nc, hotkey=hot, first=first, count=count, nchild=nchild)
 
-    def get_moments(self):
+    def get_moments(self, scaled=False):
+        """scaled=True: moments in units of the cell side, M_n / s^|n| (dsk_get_moments_scaled)"""
         nc = self.get_stats()["ncell"]
         com_mass = torch.empty((nc, 4), dtype=torch.float32, device=self.device)
         mom = torch.empty((nc, nparams(self.p)), dtype=torch.float32, device=self.device)
-        _check(self.lib.dsk_get_moments(self._h, _ptr(com_mass), _ptr(mom)))
+        f = self.lib.dsk_get_moments_scaled if scaled else self.lib.dsk_get_moments
+        _check(f(self._h, _ptr(com_mass), _ptr(mom)))
         return com_mass, mom
 
     def get_groups(self):

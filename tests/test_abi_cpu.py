@@ -20,7 +20,7 @@ def lib():
 
 def test_exports_every_declared_symbol(lib):
     hdr = open(os.path.join(ROOT, "include", "dsk.h")).read()
-    declared = set(re.findall(r"\b(dsk_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(dsk_[a-z0-9_]+)\s*\(", hdr))
     assert len(declared) >= 18
     from paper_1407_2600_b200 import dsk
     assert declared == set(dsk.SYMBOLS)

@@ -59,7 +59,7 @@ def test_accounting_matches_kernel_op_counts():
     cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
     obj = os.path.join(os.path.dirname(build.LIB), "build", "m2p.o")
     if not (os.path.exists(cuobjdump) and os.path.exists(obj)):
-        return
+        pytest.skip("cuobjdump or build/m2p.o missing: the SASS half of this test did not run")
     sass = subprocess.run([cuobjdump, "-sass", obj], capture_output=True, text=True).stdout
     for p in (2, 4, 6):                                     # the packed (f32x2) instantiations: <P, pot, fp32 monopoles>
         fn = [b for b in sass.split("Function : ")[1:] if b.startswith(f"_Z5k_m2pILi{p}ELb1ELb0EE")]
