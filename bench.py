@@ -375,8 +375,9 @@ def probe_peak():
     forms = ("ffma2_three_packed_operands", "ffma2_one_scalar_broadcast_operand", "scalar_ffma_three_registers")
     res = {}
     for v, name in enumerate(forms):
-        t, c, m = dsk.probe_fp32_peak(v)
-        res[name] = {"TFLOPs": round(t, 3), "cycles_per_warp_inst_per_smsp": round(c, 4), "sm_mhz": round(m, 1)}
+        t, c, m, tc = dsk.probe_fp32_peak_ex(v)
+        res[name] = {"TFLOPs": round(t, 3), "TFLOPs_by_sm_cycle_counters": round(tc, 3),
+                     "cycles_per_warp_inst_per_smsp": round(c, 4), "sm_mhz": round(m, 1)}
     res["tflops"] = max(res[forms[0]]["TFLOPs"], res[forms[1]]["TFLOPs"])
     return res
 

@@ -167,6 +167,8 @@ int dsk_get_lattice_tensors(dsk_ctx *ctx, double *T /* host [165] */);
  * 1: packed, one operand a scalar broadcast to both halves (the form the force kernels feed sources in); 2: scalar FFMA
  * with three distinct registers.  DSK_EINVAL for another variant or a NULL pointer, DSK_ECUDA without a device. */
 int dsk_probe_fp32_peak(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz);
+/* the same, plus TFLOP/s as implied by the SMs' own cycle counters and clock (cross-check of the event timing) */
+int dsk_probe_fp32_peak_ex(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz, double *tflops_by_cycles);
 const char *dsk_strerror(int err);
 
 #ifdef __cplusplus

@@ -27,6 +27,7 @@ NCRIT = 192
 WS = 2     # measured: WS = 1 floors the periodic force error at ~3e-3 on near-lattice inputs
 KEY_LEVELS = 21
 FAR_ORDER = 8
+BG_DEFAULT = False   # background subtraction (reading O4b) in periodic boxes; switched on together with the CUDA path
 
 _lib = None
 
@@ -175,15 +176,27 @@ class OracleTree:
         lib().orc_moments_m2m(self._h, C.c_int(p), _p(out))
         return out
 
-    def accel(self, eps, theta, p, sink=None, ws=WS, want_pot=True):
-        """Tr over the explicit image block only (the far field is added by tree_force)."""
+    def moments_bg(self, p):
+        """O4b: (l_b, rho_bar, M'[ntop, NP(p)]) — the moments of particles - rho_bar over the cube of every cell of level <= l_b"""
         if self.p != p:
             self.moments(p)
+        lb = C.c_int32(0); ntop = C.c_int64(0); rho = C.c_double(0)
+        lib().orc_tree_get_moments_bg(self._h, C.byref(lb), C.byref(ntop), C.byref(rho), None)
+        out = np.empty((ntop.value, nparams(p)))
+        lib().orc_tree_get_moments_bg(self._h, C.byref(lb), C.byref(ntop), C.byref(rho), _p(out))
+        return lb.value, rho.value, out
+
+    def accel(self, eps, theta, p, sink=None, ws=WS, want_pot=True, bg=None):
+        """Tr over the explicit image block only (the far field is added by tree_force).  bg: background subtraction
+        (reading O4b; periodic trees only)."""
+        if self.p != p:
+            self.moments(p)
+        bg = (BG_DEFAULT if bg is None else bg) and self.periodic
         sink = _sink(sink)
         ns = self.n if sink is None else sink.shape[0]
         acc = np.empty((ns, 3)); pot = np.empty(ns) if want_pot else None
         n_p2p = C.c_int64(0); n_m2p = C.c_int64(0)
-        err = lib().orc_tree_accel(self._h, C.c_double(eps), C.c_double(theta), C.c_int(ws), C.c_int64(ns),
+        err = lib().orc_tree_accel(self._h, C.c_double(eps), C.c_double(theta), C.c_int(ws), C.c_int(int(bg)), C.c_int64(ns),
                                    _p(sink), _p(acc), _p(pot), C.byref(n_p2p), C.byref(n_m2p))
         if err:
             raise RuntimeError(f"orc_tree_accel error {err}")
@@ -198,19 +211,24 @@ class OracleTree:
         return int(a.value), int(b.value), int(c.value)
 
 
-    def lists(self, theta, g, ws=WS):
-        """the two interaction lists of group g as (m2p_cell, m2p_img, p2p_cell, p2p_img), walk order"""
+    def lists(self, theta, g, ws=WS, bg=False, full=False):
+        """the two interaction lists of group g as (m2p_cell, m2p_img, p2p_cell, p2p_img), walk order; full=True adds
+        (m2p_sub, left[k, 6], window[6]): which entries carry subtracted moments, the cubes summed one by one and the
+        window, both as inclusive index ranges lo xyz, hi xyz in level-l_b cells (reading O4b)"""
         if self.p < 0:
             self.moments(2)
-        nm = C.c_int64(0); npp = C.c_int64(0)
+        nm = C.c_int64(0); npp = C.c_int64(0); nl = C.c_int64(0)
+        win = np.zeros(6, np.int64)
         f = lib().orc_group_lists
-        f(self._h, C.c_double(theta), C.c_int(ws), C.c_int64(g), C.c_int64(0), None, None, C.byref(nm), None, None,
-          C.byref(npp))
-        cap = max(nm.value, npp.value, 1)
-        mc = np.empty(cap, np.int64); mi = np.empty(cap, np.int32); pc = np.empty(cap, np.int64); pi = np.empty(cap, np.int32)
-        f(self._h, C.c_double(theta), C.c_int(ws), C.c_int64(g), C.c_int64(cap), _p(mc), _p(mi), C.byref(nm), _p(pc), _p(pi),
-          C.byref(npp))
-        return mc[:nm.value], mi[:nm.value], pc[:npp.value], pi[:npp.value]
+        f(self._h, C.c_double(theta), C.c_int(ws), C.c_int(int(bg)), C.c_int64(g), C.c_int64(0), None, None, None, C.byref(nm),
+          None, None, C.byref(npp), None, C.byref(nl), _p(win))
+        cap = max(nm.value, npp.value, nl.value, 1)
+        mc = np.empty(cap, np.int64); mi = np.empty(cap, np.int32); ms = np.empty(cap, np.int8)
+        pc = np.empty(cap, np.int64); pi = np.empty(cap, np.int32); left = np.empty((cap, 6), np.int64)
+        f(self._h, C.c_double(theta), C.c_int(ws), C.c_int(int(bg)), C.c_int64(g), C.c_int64(cap), _p(mc), _p(mi), _p(ms),
+          C.byref(nm), _p(pc), _p(pi), C.byref(npp), _p(left), C.byref(nl), _p(win))
+        out = (mc[:nm.value], mi[:nm.value], pc[:npp.value], pi[:npp.value])
+        return out + (ms[:nm.value].astype(bool), left[:nl.value], win) if full else out
 
 
 def image_shift(img, box, periodic, ws=WS):
@@ -221,15 +239,16 @@ def image_shift(img, box, periodic, ws=WS):
     return box * np.array([img // (side * side) - ws, (img // side) % side - ws, img % side - ws], dtype=np.float64)
 
 
-def tree_force(pos, mass, box, periodic, eps, theta, p, sink=None, tree=None, ws=WS):
+def tree_force(pos, mass, box, periodic, eps, theta, p, sink=None, tree=None, ws=WS, bg=None):
     """The whole oracle path Tr: tree sum over the image block (+ O7 far field when periodic).
-    Returns acc, pot, n_p2p, n_m2p, tree."""
+    bg: background subtraction (reading O4b) in a periodic box.  Returns acc, pot, n_p2p, n_m2p, tree."""
     if tree is None:
         tree = OracleTree(pos, mass, box, periodic)
-    acc, pot, n_p2p, n_m2p = tree.accel(eps, theta, p, sink, ws)
+    bg = (BG_DEFAULT if bg is None else bg) and bool(periodic)
+    acc, pot, n_p2p, n_m2p = tree.accel(eps, theta, p, sink, ws, bg=bg)
     if periodic:
         wp = tree.wrapped_pos()
-        lam = farfield_local(wp, mass, box, ws)
+        lam = farfield_local(wp, mass, box, ws, bg=bg)
         fa, fp = farfield_eval(lam, box, wp, sink)
         acc = acc + fa
         pot = pot + fp
@@ -249,6 +268,31 @@ def m2p(p, mom, r, eps2):
     acc = np.zeros(3); pot = C.c_double(0.0)
     lib().orc_m2p(C.c_int(p), _p(mom), _p(r), C.c_double(eps2), _p(acc), C.byref(pot))
     return acc, pot.value
+
+
+# ---- O4b background subtraction -------------------------------------------------------------------------
+def cuboid_field(lo, hi, x):
+    """I = int d^3y/|y-x| and g = int (y-x)/|y-x|^3 d^3y over the homogeneous unit-density cuboid [lo, hi]"""
+    lo = np.ascontiguousarray(lo, dtype=np.float64); hi = np.ascontiguousarray(hi, dtype=np.float64)
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    I = C.c_double(0.0); g = np.empty(3)
+    lib().orc_cuboid_field(_p(lo), _p(hi), _p(x), C.byref(I), _p(g))
+    return I.value, g
+
+
+def cube_moments(s, ctr, z, p):
+    ctr = np.ascontiguousarray(ctr, dtype=np.float64); z = np.ascontiguousarray(z, dtype=np.float64)
+    out = np.empty(nparams(p))
+    lib().orc_cube_moments(C.c_double(s), _p(ctr), _p(z), C.c_int(p), _p(out))
+    return out
+
+
+def bg_level(n):
+    return int(lib().orc_bg_level(C.c_int64(n)))
+
+
+def bg_halfwidth(theta, lb, ws=WS):
+    return int(lib().orc_bg_halfwidth(C.c_double(theta), C.c_int(ws), C.c_int(lb)))
 
 
 # ---- D ---------------------------------------------------------------------------------------------
@@ -298,11 +342,11 @@ def farfield_phi(u, L=1.0, ws=WS):
     return float(phi), a
 
 
-def farfield_local(pos, mass, L=1.0, ws=WS, order=FAR_ORDER):
+def farfield_local(pos, mass, L=1.0, ws=WS, order=FAR_ORDER, bg=False):
     pos = _f32(pos); mass = _f32(mass)
     lam = np.empty(nparams(order))
     lib().orc_farfield_local(C.c_int64(pos.shape[0]), _p(pos), _p(mass), C.c_double(L), C.c_int(ws),
-                             C.c_int(order), _p(lam))
+                             C.c_int(order), C.c_int(int(bg)), _p(lam))
     return lam
 
 

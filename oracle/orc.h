@@ -49,6 +49,11 @@ typedef struct orc_tree {
     double *com;           /* [ncell,3]                                                     */
     double *delta;         /* [ncell]  |com - centre|                                       */
     double *mom;           /* [ncell, NP(p)] raw moments about com                          */
+    /* O4b background subtraction (periodic only; filled by orc_moments) */
+    int bg_level;          /* l_b                                                           */
+    int64_t ntop;          /* cells of level <= l_b: the first ntop cells (level-major)     */
+    double rhobar;         /* M_tot / box^3                                                 */
+    double *mom_bg;        /* [ntop, NP(p)] moments of particles - rho_bar over the cube    */
 } orc_tree;
 
 /* multi-index helpers (orc_tree.c) */
@@ -74,13 +79,21 @@ void orc_bn(int pmax, const double r[3], double eps2, double *b);
 void orc_m2p(int p, const double *mom, const double r[3], double eps2, double acc[3], double *pot);
 void orc_direct_iso(int64_t n, const float *pos, const float *mass, double eps, int64_t nsink,
                     const int64_t *sink, double *acc, double *pot);
-int orc_tree_accel(orc_tree *t, double eps, double theta, int ws, int64_t nsink,
+int orc_tree_accel(orc_tree *t, double eps, double theta, int ws, int bg, int64_t nsink,
                    const int64_t *sink, double *acc, double *pot, int64_t *n_p2p, int64_t *n_m2p);
 void orc_group_list_counts(orc_tree *t, double theta, int ws, int64_t g, int64_t *n_m2p_cells,
                            int64_t *n_p2p_leaves, int64_t *n_p2p_particles);
 
-void orc_group_lists(orc_tree *t, double theta, int ws, int64_t g, int64_t cap, int64_t *m2p_cell,
-                     int32_t *m2p_img, int64_t *n_m2p, int64_t *p2p_cell, int32_t *p2p_img, int64_t *n_p2p);
+void orc_group_lists(orc_tree *t, double theta, int ws, int bg, int64_t g, int64_t cap, int64_t *m2p_cell,
+                     int32_t *m2p_img, int8_t *m2p_sub, int64_t *n_m2p, int64_t *p2p_cell, int32_t *p2p_img,
+                     int64_t *n_p2p, int64_t *left_lohi, int64_t *n_left, int64_t window[6]);
+void orc_cell_coords(const orc_tree *t, int64_t c, int64_t q[3]);
+
+/* background subtraction, reading O4b (orc_bg.c) */
+void orc_cuboid_field(const double lo[3], const double hi[3], const double x[3], double *I, double g[3]);
+void orc_cube_moments(double s, const double ctr[3], const double z[3], int p, double *C);
+int orc_bg_level(int64_t n);
+int orc_bg_halfwidth(double theta, int ws, int lb);
 
 /* D-per, O7 (orc_periodic.c) */
 void orc_ewald_pair(const double x[3], double L, double alpha, int nmax, int hmax, double *psi,
@@ -94,7 +107,7 @@ void orc_direct_per_pairwise(int64_t n, const float *pos, const float *mass, dou
 void orc_farfield_T(double L, int ws, int order, double *T);
 double orc_farfield_phi(const double u[3], double L, int ws, double a[3]);
 void orc_farfield_local(int64_t n, const float *pos, const float *mass, double L, int ws,
-                        int order, double *Lambda);
+                        int order, int bg, double *Lambda);
 void orc_farfield_eval(const double *Lambda, int order, double L, int64_t nsink, const float *pos,
                        const int64_t *sink, double *acc, double *pot);
 

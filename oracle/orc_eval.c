@@ -99,52 +99,136 @@ void orc_m2p(int p, const double *mom, const double r[3], double eps2, double ac
 
 /* ---- O5: walk of one sink group ------------------------------------------------------------- */
 typedef struct {
-    int64_t *cell; int32_t *img; int64_t n, cap;
+    int64_t *cell; int32_t *img; int8_t *sub; int64_t n, cap;
 } ilist_t;
 
-static void il_push(ilist_t *l, int64_t c, int32_t im)
+static void il_push(ilist_t *l, int64_t c, int32_t im, int8_t sub)
 {
     if (l->n == l->cap) {
         l->cap = l->cap ? 2 * l->cap : 1024;
         l->cell = realloc(l->cell, sizeof(int64_t) * l->cap);
         l->img = realloc(l->img, sizeof(int32_t) * l->cap);
+        l->sub = realloc(l->sub, sizeof(int8_t) * l->cap);
     }
-    l->cell[l->n] = c; l->img[l->n] = im; l->n++;
+    l->cell[l->n] = c; l->img[l->n] = im; l->sub[l->n] = sub; l->n++;
 }
+static void il_free(ilist_t *l) { free(l->cell); free(l->img); free(l->sub); }
+
+/* cubes whose background is summed one by one: index ranges [lo, hi] (inclusive) in level-l_b cells, unwrapped frame */
+typedef struct { int64_t *lohi; int64_t n, cap; } cubes_t;
 
 typedef struct {
-    const orc_tree *t; const float *bb; double theta; double shift[3]; int32_t im;
+    const orc_tree *t; const float *bb; double theta; double shift[3]; int32_t im; int64_t ishift[3];
     ilist_t *m2p, *p2p;
+    /* O4b */
+    int bg, lb; int64_t wlo[3], whi[3]; cubes_t *left;
 } walk_t;
+
+/* O4b: a cube of the image block whose background no accepted cell carries.  Inside the window it is part of the
+ * window's cuboid; otherwise it is kept and summed by itself (minus its overlap with the window). */
+static void expose(walk_t *w, const int64_t lo[3], const int64_t hi[3])
+{
+    int inside = 1;
+    for (int k = 0; k < 3; k++) if (lo[k] < w->wlo[k] || hi[k] > w->whi[k]) inside = 0;
+    if (inside) return;
+    cubes_t *q = w->left;
+    if (q->n == q->cap) { q->cap = q->cap ? 2 * q->cap : 64; q->lohi = realloc(q->lohi, sizeof(int64_t) * 6 * q->cap); }
+    for (int k = 0; k < 3; k++) { q->lohi[6 * q->n + k] = lo[k]; q->lohi[6 * q->n + 3 + k] = hi[k]; }
+    q->n++;
+}
 
 static void walk_rec(walk_t *w, int64_t c)
 {
     const orc_tree *t = w->t;
-    double s = (double)t->box * ldexp(1.0, -t->level[c]);
+    const int level = t->level[c];
+    double s = (double)t->box * ldexp(1.0, -level);
+    /* O4b: cells of level <= l_b know where they lie relative to the group's window (integer test on level-l_b cells) */
+    const int top = w->bg && level <= w->lb;
+    int inside = 0, inter = 0;
+    int64_t lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0}, q[3] = {0, 0, 0};
+    if (top) {
+        orc_cell_coords(t, c, q);
+        inside = inter = 1;
+        for (int k = 0; k < 3; k++) {
+            lo[k] = (q[k] << (w->lb - level)) + (w->ishift[k] << w->lb);
+            hi[k] = lo[k] + ((int64_t)1 << (w->lb - level)) - 1;
+            if (lo[k] < w->wlo[k] || hi[k] > w->whi[k]) inside = 0;
+            if (lo[k] > w->whi[k] || hi[k] < w->wlo[k]) inter = 0;
+        }
+    }
     /* d = Euclidean distance from the shifted centre of mass to the group's AABB (0 if inside) */
     double d2 = 0.0;
     for (int k = 0; k < 3; k++) {
         double z = t->com[3 * c + k] + w->shift[k];
-        double lo = (double)w->bb[k] - z, hi = z - (double)w->bb[3 + k];
-        double dk = lo > 0.0 ? lo : (hi > 0.0 ? hi : 0.0);
+        double l0 = (double)w->bb[k] - z, h0 = z - (double)w->bb[3 + k];
+        double dk = l0 > 0.0 ? l0 : (h0 > 0.0 ? h0 : 0.0);
         d2 += dk * dk;
     }
     double rc = s / w->theta + t->delta[c];
-    if (d2 > rc * rc) { il_push(w->m2p, c, w->im); return; }           /* accept (strict)    */
-    if (t->nchild[c] == 0) { il_push(w->p2p, c, w->im); return; }      /* leaf -> direct     */
-    for (int k = 0; k < t->nchild[c]; k++) walk_rec(w, t->child0[c] + k);
+    /* a cell that sticks out of the window (partly in, partly out) is never accepted: its cube's background would be
+     * counted twice inside the window */
+    const int straddles = top && inter && !inside;
+    if (!straddles && d2 > rc * rc) {                                   /* accept (strict)    */
+        il_push(w->m2p, c, w->im, (int8_t)(top && !inter));              /* outside the window: background subtracted */
+        return;
+    }
+    if (t->nchild[c] == 0) {                                            /* leaf -> direct     */
+        il_push(w->p2p, c, w->im, 0);
+        if (top) expose(w, lo, hi);
+        return;
+    }
+    if (top && level == w->lb) expose(w, lo, hi);                       /* below l_b nothing carries a background */
+    int present = 0;
+    for (int k = 0; k < t->nchild[c]; k++) {
+        present |= 1 << (int)(t->hotkey[t->child0[c] + k] & 7u);
+        walk_rec(w, t->child0[c] + k);
+    }
+    if (top && level < w->lb)                                           /* empty octants hold background only */
+        for (int o = 0; o < 8; o++) {
+            if (present & (1 << o)) continue;
+            int64_t lo2[3], hi2[3];
+            const int bit[3] = { (o >> 2) & 1, (o >> 1) & 1, o & 1 };
+            for (int k = 0; k < 3; k++) {
+                lo2[k] = ((2 * q[k] + bit[k]) << (w->lb - level - 1)) + (w->ishift[k] << w->lb);
+                hi2[k] = lo2[k] + ((int64_t)1 << (w->lb - level - 1)) - 1;
+            }
+            expose(w, lo2, hi2);
+        }
 }
 
-static void walk_group(const orc_tree *t, int64_t g, double theta, int ws, ilist_t *m2p, ilist_t *p2p)
+/* lists of group g; bg != 0 (periodic only): reading O4b, `left` receives the cubes to be summed one by one and
+ * window[6] the window's index range (lo xyz, hi xyz; level-l_b cells) */
+static void walk_group(const orc_tree *t, int64_t g, double theta, int ws, int bg, ilist_t *m2p, ilist_t *p2p,
+                       cubes_t *left, int64_t window[6])
 {
-    walk_t w = { t, t->gbox + 6 * g, theta, {0, 0, 0}, 0, m2p, p2p };
+    walk_t w;
+    memset(&w, 0, sizeof(w));
+    w.t = t; w.bb = t->gbox + 6 * g; w.theta = theta; w.m2p = m2p; w.p2p = p2p;
+    w.bg = bg && t->periodic; w.left = left;
     m2p->n = 0; p2p->n = 0;
+    if (left) left->n = 0;
+    if (w.bg) {
+        w.lb = t->bg_level;
+        const int k = orc_bg_halfwidth(theta, ws, w.lb);
+        const int64_t cg = t->gcell[g];
+        const int lg = t->level[cg];
+        int64_t qg[3];
+        orc_cell_coords(t, cg, qg);
+        for (int d = 0; d < 3; d++) {
+            int64_t flo, fhi;                 /* footprint of the group's cell in level-l_b cells */
+            if (lg >= w.lb) flo = fhi = qg[d] >> (lg - w.lb);
+            else { flo = qg[d] << (w.lb - lg); fhi = flo + ((int64_t)1 << (w.lb - lg)) - 1; }
+            w.wlo[d] = flo - k; w.whi[d] = fhi + k;
+            if (window) { window[d] = w.wlo[d]; window[3 + d] = w.whi[d]; }
+        }
+    }
     int W = t->periodic ? ws : 0, im = 0;
     for (int ix = -W; ix <= W; ix++)
         for (int iy = -W; iy <= W; iy++)
             for (int iz = -W; iz <= W; iz++, im++) {
                 w.shift[0] = ix * (double)t->box; w.shift[1] = iy * (double)t->box;
                 w.shift[2] = iz * (double)t->box; w.im = im;
+                w.ishift[0] = ix; w.ishift[1] = iy; w.ishift[2] = iz;
                 walk_rec(&w, 0);
             }
 }
@@ -160,25 +244,32 @@ void orc_group_list_counts(orc_tree *t, double theta, int ws, int64_t g, int64_t
                            int64_t *n_p2p_leaves, int64_t *n_p2p_particles)
 {
     ilist_t m2p = {0}, p2p = {0};
-    walk_group(t, g, theta, ws, &m2p, &p2p);
+    walk_group(t, g, theta, ws, 0, &m2p, &p2p, NULL, NULL);
     *n_m2p_cells = m2p.n; *n_p2p_leaves = p2p.n;
     int64_t np = 0;
     for (int64_t k = 0; k < p2p.n; k++) np += t->count[p2p.cell[k]];
     *n_p2p_particles = np;
-    free(m2p.cell); free(m2p.img); free(p2p.cell); free(p2p.img);
+    il_free(&m2p); il_free(&p2p);
 }
 
-/* The two lists of group g themselves (for the tests that pin the acceptance rule): cell indices (canonical
- * order) and image ids, in walk order.  Call with cap = 0 to get the lengths, then with buffers of that size. */
-void orc_group_lists(orc_tree *t, double theta, int ws, int64_t g, int64_t cap, int64_t *m2p_cell,
-                     int32_t *m2p_img, int64_t *n_m2p, int64_t *p2p_cell, int32_t *p2p_img, int64_t *n_p2p)
+/* The lists of group g themselves (for the tests that pin the acceptance rule): cell indices (canonical order), image
+ * ids and, with bg, whether the entry carries the background-subtracted moments; the cubes summed one by one
+ * (left_lohi: 6 int64 each) and the window.  Call with cap = 0 to get the lengths, then with buffers of that size. */
+void orc_group_lists(orc_tree *t, double theta, int ws, int bg, int64_t g, int64_t cap, int64_t *m2p_cell,
+                     int32_t *m2p_img, int8_t *m2p_sub, int64_t *n_m2p, int64_t *p2p_cell, int32_t *p2p_img,
+                     int64_t *n_p2p, int64_t *left_lohi, int64_t *n_left, int64_t window[6])
 {
     ilist_t m2p = {0}, p2p = {0};
-    walk_group(t, g, theta, ws, &m2p, &p2p);
+    cubes_t left = {0};
+    int64_t win[6] = {0, 0, 0, 0, 0, 0};
+    walk_group(t, g, theta, ws, bg, &m2p, &p2p, &left, win);
     *n_m2p = m2p.n; *n_p2p = p2p.n;
-    for (int64_t k = 0; k < m2p.n && k < cap; k++) { m2p_cell[k] = m2p.cell[k]; m2p_img[k] = m2p.img[k]; }
+    if (n_left) *n_left = left.n;
+    if (window) for (int k = 0; k < 6; k++) window[k] = win[k];
+    for (int64_t k = 0; k < m2p.n && k < cap; k++) { m2p_cell[k] = m2p.cell[k]; m2p_img[k] = m2p.img[k]; if (m2p_sub) m2p_sub[k] = m2p.sub[k]; }
     for (int64_t k = 0; k < p2p.n && k < cap; k++) { p2p_cell[k] = p2p.cell[k]; p2p_img[k] = p2p.img[k]; }
-    free(m2p.cell); free(m2p.img); free(p2p.cell); free(p2p.img);
+    if (left_lohi) for (int64_t k = 0; k < left.n && k < cap; k++) memcpy(left_lohi + 6 * k, left.lohi + 6 * k, sizeof(int64_t) * 6);
+    il_free(&m2p); il_free(&p2p); free(left.lohi);
 }
 
 /* group containing sorted rank r (groups tile [0,n) in Morton order) */
@@ -205,7 +296,7 @@ static int gs_cmp(const void *a, const void *b)
  * number of particle-particle and cell-particle interactions evaluated for these sinks.
  * Periodic: only the (2 ws + 1)^3 image block is summed here; O7's far field is added by the
  * caller (orc_farfield_*). */
-int orc_tree_accel(orc_tree *t, double eps, double theta, int ws, int64_t nsink,
+int orc_tree_accel(orc_tree *t, double eps, double theta, int ws, int bg, int64_t nsink,
                    const int64_t *sink, double *acc, double *pot, int64_t *n_p2p, int64_t *n_m2p)
 {
     if (t->p < 0) return -3;
@@ -225,10 +316,14 @@ int orc_tree_accel(orc_tree *t, double eps, double theta, int ws, int64_t nsink,
 #pragma omp parallel reduction(+ : tot_p2p, tot_m2p)
     {
         ilist_t m2p = {0}, p2p = {0};
+        cubes_t left = {0};
+        int64_t win[6];
+        const int use_bg = bg && t->periodic;
+        const double sb = use_bg ? (double)t->box * ldexp(1.0, -t->bg_level) : 0.0;     /* side of a level-l_b cell */
 #pragma omp for schedule(dynamic, 1)
         for (int64_t q = 0; q < nrun; q++) {
             int64_t g = gs[run[q]].g;
-            walk_group(t, g, theta, ws, &m2p, &p2p);
+            walk_group(t, g, theta, ws, bg, &m2p, &p2p, &left, win);
             for (int64_t u = run[q]; u < run[q + 1]; u++) {
                 int64_t s = gs[u].s, i = sink ? sink[s] : s, r = t->rank_of[i];
                 const double *x = t->spos + 3 * r;
@@ -253,14 +348,42 @@ int orc_tree_accel(orc_tree *t, double eps, double theta, int ws, int64_t nsink,
                     int64_t c = m2p.cell[k];
                     double sh[3], rr[3]; img_shift(t, ws, m2p.img[k], sh);
                     for (int d = 0; d < 3; d++) rr[d] = x[d] - (t->com[3 * c + d] + sh[d]);
-                    orc_m2p(p, t->mom + (size_t)np * c, rr, e2, a, &ph);
+                    orc_m2p(p, (m2p.sub[k] ? t->mom_bg : t->mom) + (size_t)np * c, rr, e2, a, &ph);
                     tot_m2p++;
+                }
+                /* O4b: the background (density -rho_bar) that no accepted cell carries, summed exactly: the window's
+                 * cuboid, and every kept cube minus its part inside the window.  Newtonian closed form. */
+                if (use_bg) {
+                    double lo[3], hi[3], I, gg[3];
+                    for (int d = 0; d < 3; d++) { lo[d] = win[d] * sb; hi[d] = (win[3 + d] + 1) * sb; }
+                    orc_cuboid_field(lo, hi, x, &I, gg);
+                    ph += t->rhobar * I;
+                    for (int d = 0; d < 3; d++) a[d] -= t->rhobar * gg[d];
+                    for (int64_t k = 0; k < left.n; k++) {
+                        const int64_t *c6 = left.lohi + 6 * k;
+                        int overlap = 1;
+                        double olo[3], ohi[3];
+                        for (int d = 0; d < 3; d++) {
+                            lo[d] = c6[d] * sb; hi[d] = (c6[3 + d] + 1) * sb;
+                            int64_t ol = c6[d] > win[d] ? c6[d] : win[d], oh = c6[3 + d] < win[3 + d] ? c6[3 + d] : win[3 + d];
+                            if (ol > oh) overlap = 0;
+                            olo[d] = ol * sb; ohi[d] = (oh + 1) * sb;
+                        }
+                        orc_cuboid_field(lo, hi, x, &I, gg);
+                        ph += t->rhobar * I;
+                        for (int d = 0; d < 3; d++) a[d] -= t->rhobar * gg[d];
+                        if (overlap) {
+                            orc_cuboid_field(olo, ohi, x, &I, gg);
+                            ph -= t->rhobar * I;
+                            for (int d = 0; d < 3; d++) a[d] += t->rhobar * gg[d];
+                        }
+                    }
                 }
                 acc[3 * s] = a[0]; acc[3 * s + 1] = a[1]; acc[3 * s + 2] = a[2];
                 if (pot) pot[s] = ph;
             }
         }
-        free(m2p.cell); free(m2p.img); free(p2p.cell); free(p2p.img);
+        il_free(&m2p); il_free(&p2p); free(left.lohi);
     }
     if (n_p2p) *n_p2p = tot_p2p;
     if (n_m2p) *n_m2p = tot_m2p;

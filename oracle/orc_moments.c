@@ -55,6 +55,27 @@ void orc_moments(orc_tree *t, int p)
         t->delta[c] = sqrt(d2);
         orc_p2m_range(t, t->first[c], t->count[c], p, z, t->mom + (size_t)np * c);
     }
+    /* O4b: for the cells of level <= l_b, the moments of  particles - rho_bar  over the cell's cube about the same
+     * expansion centre (the centre of mass of the particles): M'_n = M_n - rho_bar C_n, C_n = orc_cube_moments. */
+    free(t->mom_bg); t->mom_bg = NULL; t->ntop = 0;
+    if (t->periodic && t->ncell > 0) {
+        t->bg_level = orc_bg_level(t->n);
+        t->rhobar = t->cmass[0] / ((double)t->box * t->box * t->box);
+        while (t->ntop < t->ncell && t->level[t->ntop] <= t->bg_level) t->ntop++;
+        t->mom_bg = malloc(sizeof(double) * (size_t)np * (size_t)t->ntop);
+        for (int64_t c = 0; c < t->ntop; c++) {
+            double side, ctr[3], C[ORC_NP(ORC_PMAX)];
+            orc_cell_geometry(t, c, &side, ctr);
+            orc_cube_moments(side, ctr, t->com + 3 * c, p, C);
+            for (int i = 0; i < np; i++) t->mom_bg[(size_t)np * c + i] = t->mom[(size_t)np * c + i] - t->rhobar * C[i];
+        }
+    }
+}
+
+void orc_tree_get_moments_bg(const orc_tree *t, int32_t *bg_level, int64_t *ntop, double *rhobar, double *mom_bg)
+{
+    *bg_level = t->bg_level; *ntop = t->ntop; *rhobar = t->rhobar;
+    if (mom_bg && t->mom_bg) memcpy(mom_bg, t->mom_bg, sizeof(double) * (size_t)ORC_NP(t->p) * (size_t)t->ntop);
 }
 
 /* M_n^parent = sum_children sum_{k<=n} C(n,k) M_k^child (z_child - z_parent)^(n-k)   (O4) */

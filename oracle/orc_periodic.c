@@ -357,7 +357,7 @@ void orc_farfield_T(double L, int ws, int order, double *T)
 /* Lambda_n = sum_{|k| <= order-|n|} (-1)^|k| C(n+k,k) M_k^c T_{n+k},
  * M_k^c = sum_j m_j (s_j - c)^k about the box centre c = (L/2,L/2,L/2)   (O7 steps 2-3) */
 void orc_farfield_local(int64_t n, const float *pos, const float *mass, double L, int ws, int order,
-                        double *Lambda)
+                        int bg, double *Lambda)
 {
     int np = ORC_NP(order);
     int ea[ORC_NP(ORC_PMAX)], eb[ORC_NP(ORC_PMAX)], ec[ORC_NP(ORC_PMAX)];
@@ -372,6 +372,15 @@ void orc_farfield_local(int64_t n, const float *pos, const float *mass, double L
             for (int e = 1; e <= order; e++) pw[k][e] = pw[k][e - 1] * d;
         }
         for (int i = 0; i < np; i++) M[i] += (double)mass[j] * pw[0][ea[i]] * pw[1][eb[i]] * pw[2][ec[i]];
+    }
+    /* O4b: with background subtraction the far images come with their backgrounds, i.e. the far-field operator acts
+     * on delta rho = particles - rho_bar: M_k -= rho_bar int_box (y - c)^k d^3y  (exact: int_box psi = 0, so
+     * int_box rho_bar Phi_far(x - y) d^3y is the potential of the homogeneous image block). */
+    if (bg) {
+        double cbox[3] = { 0.5 * L, 0.5 * L, 0.5 * L }, Cb[ORC_NP(ORC_PMAX)];
+        orc_cube_moments(L, cbox, cbox, order, Cb);
+        const double rhobar = M[0] / (L * L * L);
+        for (int i = 0; i < np; i++) M[i] -= rhobar * Cb[i];            /* M_0 becomes 0: the box is neutral */
     }
     double binom[2 * ORC_PMAX + 1][2 * ORC_PMAX + 1];
     for (int i = 0; i <= 2 * ORC_PMAX; i++) {

@@ -110,6 +110,19 @@ void orc_cell_geometry(const orc_tree *t, int64_t c, double *side, double centre
     for (int d = 0; d < 3; d++) centre[d] = s * (double)q[d] + 0.5 * s;
 }
 
+/* integer coordinates of cell c at its own level (de-interleaved hotkey prefix) */
+void orc_cell_coords(const orc_tree *t, int64_t c, int64_t q[3])
+{
+    int l = t->level[c];
+    uint64_t prefix = t->hotkey[c] & ~(1ull << (3 * l));
+    q[0] = q[1] = q[2] = 0;
+    for (int b = 0; b < l; b++) {
+        q[0] |= (int64_t)((prefix >> (3 * b + 2)) & 1u) << b;
+        q[1] |= (int64_t)((prefix >> (3 * b + 1)) & 1u) << b;
+        q[2] |= (int64_t)((prefix >> (3 * b + 0)) & 1u) << b;
+    }
+}
+
 static void build_groups_rec(orc_tree *t, int64_t c, int64_t *cap)
 {
     if (t->count[c] <= t->ncrit || t->nchild[c] == 0) {
@@ -210,7 +223,7 @@ void orc_tree_free(orc_tree *t)
     free(t->spos); free(t->smass);
     free(t->hotkey); free(t->first); free(t->count); free(t->child0); free(t->nchild); free(t->level);
     free(t->gcell); free(t->gfirst); free(t->gcount); free(t->gbox);
-    free(t->cmass); free(t->com); free(t->delta); free(t->mom);
+    free(t->cmass); free(t->com); free(t->delta); free(t->mom); free(t->mom_bg);
     free(t);
 }
 

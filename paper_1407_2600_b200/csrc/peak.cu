@@ -11,8 +11,8 @@
 
 #define PK_CHAINS 8          // independent accumulators per thread
 #define PK_UNROLL 16         // loop body = PK_UNROLL x PK_CHAINS instructions
-#define PK_THREADS 512       // 16 warps per SM = 4 per sub-partition
-#define PK_BLOCKS_PER_SM 2
+#define PK_THREADS 1024      // one block per SM: 32 warps = 8 per sub-partition (two blocks of 512 per SM did not always
+#define PK_BLOCKS_PER_SM 1   // land two to an SM: the event time then read 25 % below what the SMs' own clocks showed)
 
 __device__ __forceinline__ unsigned long long pk_globaltimer()
 {
@@ -70,7 +70,18 @@ __global__ void __launch_bounds__(PK_THREADS, PK_BLOCKS_PER_SM) k_fp32_peak(int 
 }
 
 // Host pointers.  Allocates and frees its own few MB of device memory (it is a diagnostic, not part of the path).
+static int probe_impl(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz, double *tflops_by_cycles);
 extern "C" int dsk_probe_fp32_peak(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz)
+{
+    return probe_impl(variant, tflops, cycles_per_inst_smsp, sm_mhz, nullptr);
+}
+// the same plus the rate implied by the in-kernel cycle counters (a cross-check of the event timing)
+extern "C" int dsk_probe_fp32_peak_ex(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz, double *tflops_by_cycles)
+{
+    if (!tflops_by_cycles) return DSK_EINVAL;
+    return probe_impl(variant, tflops, cycles_per_inst_smsp, sm_mhz, tflops_by_cycles);
+}
+static int probe_impl(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz, double *tflops_by_cycles)
 {
     if (variant < 0 || variant > 2 || !tflops || !cycles_per_inst_smsp || !sm_mhz) return DSK_EINVAL;
     int dev = 0, nsm = 0;
@@ -110,6 +121,10 @@ extern "C" int dsk_probe_fp32_peak(int variant, double *tflops, double *cycles_p
     const double inst_per_thread = (double)iters * PK_UNROLL * PK_CHAINS;
     const double lanes = variant == 2 ? 1.0 : 2.0;
     *tflops = inst_per_thread * 2.0 * lanes * (double)grid * PK_THREADS / ((double)best * 1e-3) / 1e12;
+    if (tflops_by_cycles) {      // the same from the SMs' own cycle counters: flop per block / (its cycles / its clock), all blocks at once
+        const double sec = (cyc / grid) / (cyc / ns * 1e9);
+        *tflops_by_cycles = inst_per_thread * 2.0 * lanes * (double)grid * PK_THREADS / sec / 1e12;
+    }
     // warp instructions issued by one sub-partition while a block's clock ran: the SM holds PK_BLOCKS_PER_SM blocks of
     // PK_THREADS / 32 warps, a quarter of them on each sub-partition
     const double warps_per_smsp = (double)PK_BLOCKS_PER_SM * (PK_THREADS / 32) / 4.0;

@@ -16,7 +16,7 @@ SYMBOLS = [
     "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
     "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_get_keys",
     "dsk_get_tree", "dsk_get_moments", "dsk_get_moments_scaled", "dsk_get_groups", "dsk_get_stats", "dsk_get_param", "dsk_get_task_widths",
-    "dsk_get_lattice_tensors", "dsk_probe_fp32_peak", "dsk_strerror",
+    "dsk_get_lattice_tensors", "dsk_probe_fp32_peak", "dsk_probe_fp32_peak_ex", "dsk_strerror",
 ]
 
 
@@ -74,6 +74,7 @@ def load_library(path=LIB_PATH):
     lib.dsk_get_task_widths.argtypes = [C.c_int, C.POINTER(C.c_int)]
     lib.dsk_get_lattice_tensors.argtypes = [vp, vp]
     lib.dsk_probe_fp32_peak.argtypes = [i32, C.POINTER(f64), C.POINTER(f64), C.POINTER(f64)]
+    lib.dsk_probe_fp32_peak_ex.argtypes = [i32, C.POINTER(f64), C.POINTER(f64), C.POINTER(f64), C.POINTER(f64)]
     lib.dsk_strerror.argtypes = [i32]
     lib.dsk_strerror.restype = C.c_char_p
     for s in SYMBOLS:
@@ -100,6 +101,13 @@ def probe_fp32_peak(variant):
     t, c, m = C.c_double(0), C.c_double(0), C.c_double(0)
     _check(load_library().dsk_probe_fp32_peak(int(variant), C.byref(t), C.byref(c), C.byref(m)))
     return t.value, c.value, m.value
+
+
+def probe_fp32_peak_ex(variant):
+    """(TFLOP/s by CUDA events, cycles per warp instruction per sub-partition, SM MHz, TFLOP/s by the SMs' cycle counters)"""
+    t, c, m, tc = C.c_double(0), C.c_double(0), C.c_double(0), C.c_double(0)
+    _check(load_library().dsk_probe_fp32_peak_ex(int(variant), C.byref(t), C.byref(c), C.byref(m), C.byref(tc)))
+    return t.value, c.value, m.value, tc.value
 
 
 def _check(code):
