@@ -62,6 +62,7 @@ typedef struct dsk_stats {
     int64_t list_p2p;         /* total P2P list entries (leaves) over all groups                       */
     int64_t nbatch;           /* list batches the evaluation was split in                              */
     int64_t n_launch;         /* kernels launched since the last dsk_build_tree began (inclusive)      */
+    int64_t list_bg;          /* background subtraction: cubes kept outside the groups' windows        */
     float ms_key, ms_sort, ms_build, ms_upward, ms_group, ms_walk, ms_p2p, ms_m2p, ms_far, ms_scatter,
           ms_kdk;
 } dsk_stats;
@@ -109,6 +110,22 @@ int dsk_accel_active(dsk_ctx *ctx, const float *pos, const float *mass, const ui
  * step (call dsk_kdk_reset after changing pos/vel by hand).  One force evaluation per step. */
 int dsk_kdk_step(dsk_ctx *ctx, float *pos, float *vel, const float *mass, double a, double da);
 int dsk_kdk_reset(dsk_ctx *ctx);
+
+/* Background subtraction in a periodic box ("a technique to subtract the uniform background density";
+ * reading O4b of DESIGN.md): the sources become particles - rho_bar, rho_bar = M_tot / box^3.  Cells of level <= l_b that
+ * the walk accepts outside the sink group's window (a cube of level-l_b cells reaching k = ceil(1/theta) cells beyond the
+ * group's cell) carry the moments of that difference over their cube; the background of the window and of the few coarse
+ * cubes that stick out of it is summed exactly (closed-form field of a homogeneous cuboid); the far field acts on the
+ * neutral box.  ON BY DEFAULT in a periodic context; on = 0 restores plain particle moments with the neutralising
+ * background in the far field alone (and fp64 monopoles).
+ * DSK_EINVAL for on != 0 in an isolated context.  Changing it invalidates moments, lists and the cached KDK force. */
+int dsk_set_background(dsk_ctx *ctx, int on);
+/* host pointers, each may be NULL: on / off, l_b, the window half-width k for the current theta, the number of cells of
+ * level <= l_b in the current tree (0 when off or no tree) and rho_bar (0 unless the moments are up to date). */
+int dsk_get_background(dsk_ctx *ctx, int *on, int *level, int *halfwidth, int64_t *ntop, double *rhobar);
+/* the subtracted moments of those cells (canonical order: they are the first ntop cells) in units of the cell side,
+ * M'_n / s^|n|, dev [ntop, N_p]; DSK_EINVAL when subtraction is off. */
+int dsk_get_bg_moments(dsk_ctx *ctx, float *moments);
 
 /* Diagnostic: mode 0 (default) lets the walk try its one-pass form (lists written into a fixed capacity per group,
  * fallback to COUNT + FILL when one does not fit); mode 1 always takes the two-pass form; mode 2 gives the one-pass

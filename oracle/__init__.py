@@ -27,7 +27,7 @@ NCRIT = 192
 WS = 2     # measured: WS = 1 floors the periodic force error at ~3e-3 on near-lattice inputs
 KEY_LEVELS = 21
 FAR_ORDER = 8
-BG_DEFAULT = False   # background subtraction (reading O4b) in periodic boxes; switched on together with the CUDA path
+BG_DEFAULT = True    # background subtraction (reading O4b) in periodic boxes: on by default on both sides (dsk_set_background)
 
 _lib = None
 

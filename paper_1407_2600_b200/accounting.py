@@ -4,23 +4,24 @@ Bookkeeping only — none of the method's arithmetic lives here.
 """
 
 
-def _fr_has(p, q, m):
-    return m >= q and 2 * m - q <= p and not (q == 1 and m == 1)
+def _fr_has(p, q, m, dip=False):
+    return m >= q and 2 * m - q <= p and (dip or not (q == 1 and m == 1))
 
 
 def _rank(q):
     return [(a, b, q - a - b) for a in range(q, -1, -1) for b in range(q - a, -1, -1)]
 
 
-def m2p_ops(p, pot=True):
-    """(ffma, fmul, fadd) per cell-particle interaction of k_m2p at order p (pairing form, m2p.cu)."""
+def m2p_ops(p, pot=True, dip=False):
+    """(ffma, fmul, fadd) per cell-particle interaction of k_m2p at order p (pairing form, m2p.cu).
+    dip: rows with a dipole block (periodic runs with background subtraction, kernel MODE 2)."""
     ffma, fmul, fadd = 3 + 3, 1, 0          # R2 chain and rho = x * sinv - com'/s (one FMA each); q = h0^2
     fmul += 3 * (p - 1) if p < 3 else 3 * (p - 2) + 1   # rho_i / k, k = 2..p; for p >= 3 the top block needs q/p, not rho_i/p
     for q in range(p + 1):
         if q >= 2 and not (q == p and p >= 3):
             fmul += len(_rank(q))           # monomials of degree q (degree p is never read: its block uses Euler)
         for m in range(q, p + 1):
-            if not _fr_has(p, q, m):
+            if not _fr_has(p, q, m, dip):
                 continue
             qfirst_s = 0 if (m == 1 or 2 * m - p < 0) else 2 * m - p
             qfirst_g = max(1, 2 * m - p)
@@ -47,16 +48,16 @@ def m2p_ops(p, pot=True):
                     fadd += 3               # merge with the lower blocks' gradient
     ffma += 2 * p - 1                       # Horner in q for Pq = sum S_m q^m and its derivative
     fmul += 1; ffma += 1                    # Pq + 2 q Pq'
-    ffma += 3 * (p - 2)                     # Horner for the gradient sums G_p .. G_2
-    fmul += 3 + 3                           # u = (q (h0 * -1/s^2)) * tt ; k2 = (q (h0 / s^2)) q
+    ffma += 3 * (p - 1 if dip else p - 2)   # Horner for the gradient sums G_p .. G_2 (.. G_1 with a dipole block)
+    fmul += 3 + (2 if dip else 3)           # u = (q (h0 * -1/s^2)) * tt ; k2 = (q (h0 / s^2)) q  (no last q with a dipole block)
     ffma += 6                               # fold the cell's sums into the tile sums
     if pot:
         fmul += 1; ffma += 1
     return ffma, fmul, fadd
 
 
-def m2p_flops(p, pot=True):
-    f, m, a = m2p_ops(p, pot)
+def m2p_flops(p, pot=True, dip=False):
+    f, m, a = m2p_ops(p, pot, dip)
     return 2 * f + m + a
 
 

@@ -43,7 +43,23 @@ static size_t carve(dsk_ctx *c, char *base)
     c->whdr = (float4 *)take(16 * nc);
     c->wmac = (float4 *)take(32 * nc);     // MAC record + cell record per cell
     c->rows = (float *)take(4 * (size_t)dsk_rowlen(c->p_cap) * nc);
-    c->frows = (float *)take(4 * (size_t)dsk_frow_len(c->p_cap) * nc);
+    // background subtraction (periodic): cells of level <= l_b have a second, subtracted force row behind the ncell plain ones
+    c->bg_level = dsk_bg_level(c->N);
+    c->ntop_cap = 0;
+    if (c->periodic) {
+        int64_t full = 0;
+        for (int l = 0; l <= c->bg_level; l++) full += (int64_t)1 << (3 * l);
+        c->ntop_cap = full < c->ncell_cap ? full : c->ncell_cap;
+    }
+    const size_t nt = (size_t)c->ntop_cap;
+    c->frows = (float *)take(4 * (size_t)dsk_frow_len(c->p_cap, c->periodic) * (nc + nt));
+    c->topgeo = (int4 *)take(16 * nt);
+    c->mass64 = (double *)take(8 * nt);
+    c->rows_bg = (float *)take(4 * (size_t)dsk_rowlen(c->p_cap) * nt);
+    c->g_left_len = (uint32_t *)take(4 * (c->periodic ? ng : 0));
+    c->g_left_off = (uint64_t *)take(8 * (c->periodic ? ng + 1 : 0));
+    c->list_left_cap = c->periodic ? n / 8 + (1u << 16) : 0;
+    c->list_left = (uint4 *)take(16 * c->list_left_cap);
     c->frtab_beg = (uint32_t *)take(4 * DSK_FRTAB_BEG);
     c->frtab_ent = (void *)take(8 * DSK_FRTAB_ENT);
     c->gmark = (uint32_t *)take(4 * n);
@@ -98,7 +114,8 @@ extern "C" int dsk_create(dsk_ctx **out, int64_t N, float box, int periodic, flo
     if (!c) return DSK_ECUDA;
     memset(c, 0, sizeof(*c));
     c->N = N; c->box = box; c->periodic = periodic ? 1 : 0; c->eps = eps; c->theta = theta; c->p = p;
-    c->moments_p = -1; c->p_cap = p; c->frow_tab_p = -1;
+    c->moments_p = -1; c->p_cap = p; c->frow_tab_p = -1; c->frow_tab_dip = -1;
+    c->bg = c->periodic;                         // background subtraction is the default in periodic boxes (dsk_set_background)
     c->omega_m = 1.0; c->omega_l = 0.0;
     c->onepass_bad_theta = -1.0f;
     c->ws_bytes = 0;
@@ -143,7 +160,7 @@ extern "C" int dsk_bind_workspace(dsk_ctx *c, void *dev_ptr, size_t bytes)
     c->ws = (char *)dev_ptr;
     c->ws_bytes = bytes;
     carve(c, c->ws);
-    c->have_tree = 0; c->moments_p = -1; c->lists_valid = 0; c->kdk_have_acc = 0; c->frow_tab_p = -1;
+    c->have_tree = 0; c->moments_p = -1; c->lists_valid = 0; c->kdk_have_acc = 0; c->frow_tab_p = -1; c->frow_tab_dip = -1;
     if (c->periodic)
         DSK_CUDA(cudaMemcpyAsync(c->far_T_dev, c->far_T, sizeof(double) * DSK_NFAR, cudaMemcpyHostToDevice, c->stream));
     DSK_CUDA(cudaMemsetAsync(c->dstate, 0, sizeof(dsk_devstate), c->stream));
@@ -250,6 +267,10 @@ static int accel_impl(dsk_ctx *c, const uint8_t *active, float *acc, float *pot)
     if (c->periodic) {
         e = dsk_run_farfield(c);
         if (e) return e;
+        if (c->bg) {                                 // the exact background of the windows (background.cu)
+            e = dsk_run_bg_window(c, pot != nullptr);
+            if (e) return e;
+        }
     }
     cudaEventRecord(c->ev[13], c->stream);
     e = dsk_run_scatter(c, acc, pot, active);
@@ -260,6 +281,7 @@ static int accel_impl(dsk_ctx *c, const uint8_t *active, float *acc, float *pot)
     c->stats.ms_scatter = ev_ms(c->ev[13], c->ev[14]);
     c->stats.n_p2p = (int64_t)c->hstate->n_p2p; c->stats.n_m2p = (int64_t)c->hstate->n_m2p;
     c->stats.list_m2p = (int64_t)c->hstate->tot_m2p_list; c->stats.list_p2p = (int64_t)c->hstate->tot_p2p_list;
+    c->stats.list_bg = (int64_t)c->hstate->tot_left_list;
     return e;
 }
 
@@ -335,6 +357,45 @@ extern "C" int dsk_set_cosmology(dsk_ctx *c, double omega_m, double omega_lambda
     if (!(omega_m > 0.0) || !isfinite(omega_m) || !isfinite(omega_lambda)) return DSK_EINVAL;
     c->omega_m = omega_m; c->omega_l = omega_lambda;
     return DSK_OK;
+}
+
+extern "C" int dsk_set_background(dsk_ctx *c, int on)
+{
+    if (!c) return DSK_EINVAL;
+    if (on && !c->periodic) return DSK_EINVAL;
+    if ((on != 0) != (c->bg != 0)) { c->moments_p = -1; c->lists_valid = 0; c->kdk_have_acc = 0; }   // rows and lists depend on it
+    c->bg = on ? 1 : 0;
+    return DSK_OK;
+}
+
+extern "C" int dsk_get_background(dsk_ctx *c, int *on, int *level, int *halfwidth, int64_t *ntop, double *rhobar)
+{
+    if (!c) return DSK_EINVAL;
+    if (on) *on = c->bg;
+    if (level) *level = c->bg_level;
+    if (halfwidth) *halfwidth = dsk_bg_halfwidth(c->theta, c->bg_level);
+    if (ntop) *ntop = c->bg && c->have_tree ? (int64_t)c->ntop : 0;
+    if (rhobar) {
+        *rhobar = 0.0;
+        if (c->bg && c->have_tree && c->moments_p == c->p) {
+            double m = 0.0;
+            DSK_CUDA(cudaMemcpyAsync(&m, c->mass64, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+            DSK_CUDA(cudaStreamSynchronize(c->stream));
+            *rhobar = m / ((double)c->box * c->box * c->box);
+        }
+    }
+    return DSK_OK;
+}
+
+extern "C" int dsk_get_bg_moments(dsk_ctx *c, float *moments)
+{
+    if (!c || !moments || !c->bg) return DSK_EINVAL;
+    if (!c->have_tree) return DSK_ENOTREE;
+    if (c->moments_p != c->p) {
+        int e = dsk_run_upward(c);
+        if (e) return e;
+    }
+    return dsk_run_get_bg_moments(c, moments);
 }
 
 extern "C" int dsk_set_walk_mode(dsk_ctx *c, int mode)

@@ -106,6 +106,7 @@ struct dsk_devstate {         // small device block read back at the end of API 
     unsigned long long tot_m2p_list, tot_p2p_list, tot_p2p_src;   // over all groups
     unsigned long long n_p2p, n_m2p;                               // useful interactions
     unsigned long long scratch[4];
+    unsigned long long tot_left_list;                              // cubes kept outside the windows (background.cu), all groups
 };
 
 enum { ST_OUTOFBOX = 1, ST_NONFINITE = 2, ST_CELLOVF = 4, ST_STACKOVF = 8, ST_LISTOVF = 16 };
@@ -153,6 +154,18 @@ struct dsk_ctx {
     uint64_t *g_m2p_off, *g_p2p_off;               // [ngroup_cap + 1] exclusive offsets into lists
     uint32_t *list_m2p, *list_p2p;
     size_t list_m2p_cap, list_p2p_cap;             // entries
+    // background subtraction (background.cu; periodic contexts only)
+    int bg;                   // on / off (dsk_set_background)
+    int bg_level;             // l_b
+    uint32_t ntop;            // cells of level <= l_b of the current tree
+    int64_t ntop_cap;
+    int4 *topgeo;             // [ntop_cap] integer coordinates, level | child octant mask << 8
+    double *mass64;           // [ntop_cap] fp64 masses
+    float *rows_bg;           // [ntop_cap * rowlen(p_cap)] subtracted moment rows (their force rows are frows[ncell ..])
+    uint32_t *g_left_len;     // [ngroup_cap] cubes kept outside the window, per group (the walk's third list)
+    uint64_t *g_left_off;     // [ngroup_cap + 1]
+    uint4 *list_left;         // records: lo | hi << 16 per axis (int16 each), level-l_b cells
+    size_t list_left_cap;
     float *kdk_acc;           // [N,3] cached force, caller order
     uint8_t *kdk_active;      // [N] particles whose step ends at the current substep (dsk_kdk_block_step)
     double *far_partial;      // [nblk * 165]
@@ -169,6 +182,8 @@ struct dsk_ctx {
     double omega_m, omega_l;  // background cosmology of dsk_kdk_step (default 1, 0)
     int p_cap;                // order the workspace was sized for (dsk_create's p); set_params may lower p
     int frow_tab_p;           // order of the uploaded force-row map
+    int frow_tab_dip;         // and whether it has the dipole block
+    int frow_dip;             // layout of the force rows in memory: dipole block present (periodic with subtraction)
     uint32_t m2m_tab_mask;    // orders whose M2M pair table this context has uploaded (bit p/2 - 1)
     float lists_theta;
     int walk_two_pass_only;   // dsk_set_walk_mode(1)
@@ -207,8 +222,15 @@ int dsk_run_upward(dsk_ctx *c);                                               //
 int dsk_run_get_moments(dsk_ctx *c, float *com_mass, float *moments, int scaled);         // upward.cu
 int dsk_run_walk(dsk_ctx *c);                                                 // walk.cu: W
 int dsk_run_force(dsk_ctx *c, int want_pot);                                  // force.cu: F1 + orchestration
-int dsk_frow_len(int p);                                                      // m2p.cu
+int dsk_frow_len(int p, int dip);                                             // m2p.cu
 int dsk_run_frows(dsk_ctx *c);                                                // m2p.cu: moment rows -> force rows
+int dsk_run_frows_bg(dsk_ctx *c, uint32_t ntop);                              // m2p.cu: subtracted rows -> force rows [ncell ..]
+int dsk_bg_level(int64_t n);                                                  // background.cu
+int dsk_bg_halfwidth(float theta, int lb);                                    // background.cu
+int dsk_run_bg_rows(dsk_ctx *c);                                              // background.cu: after the upward pass
+int dsk_run_bg_window(dsk_ctx *c, int want_pot);                              // background.cu: after all batches
+int dsk_run_bg_left(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t base, int want_pot);   // background.cu: per batch
+int dsk_run_get_bg_moments(dsk_ctx *c, float *moments);                       // background.cu
 int dsk_order_tasks(dsk_ctx *c, uint32_t t0, uint32_t t1, const uint32_t *len, int shift);   // m2p.cu
 int dsk_launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int want_pot);   // m2p.cu: F2
 int dsk_run_farfield(dsk_ctx *c);                                             // farfield.cu: F3

@@ -225,9 +225,12 @@ __global__ void __launch_bounds__(FM_WARPS * 32, 1) k_far_moments(const float4 *
 }
 
 // (b) reduce partials, then Lambda_n = sum_{|k| <= 8-|n|} (-1)^|k| C(n+k,k) M_k T_{n+k}
+// bg (reading O4b): the operator acts on the NEUTRAL box, M_k -= rho_bar int_box (y - c)^k d^3y = M_0 prod_i (L/2)^k_i / (k_i + 1)
+// for even k_i (0 otherwise) — exact: the zero-mean Ewald potential integrates to 0 over the box, so int_box rho_bar Phi_far
+// is the potential of the homogeneous image block, which the tree side now carries.
 __global__ void __launch_bounds__(FM_THREADS) k_far_lambda(const double *__restrict__ partial, int nblk,
                                                            const double *__restrict__ T, double *__restrict__ M,
-                                                           double *__restrict__ lambda)
+                                                           double *__restrict__ lambda, int bg, double half_box)
 {
     __shared__ double sM[NF];
     __shared__ double binom[2 * FO + 1][2 * FO + 1];
@@ -236,6 +239,15 @@ __global__ void __launch_bounds__(FM_THREADS) k_far_lambda(const double *__restr
         double s = 0.0;
         for (int b = 0; b < nblk; b++) s += partial[(size_t)b * NF + t];
         sM[t] = s; M[t] = s;
+    }
+    __syncthreads();
+    const double m0 = sM[0];
+    __syncthreads();
+    if (bg && t < NF) {
+        const int a = f_ea[t], b = f_eb[t], c = f_ec[t];
+        double cube = 0.0;
+        if (!((a | b | c) & 1)) cube = pow(half_box, (double)(a + b + c)) / (double)((a + 1) * (b + 1) * (c + 1));
+        sM[t] -= m0 * cube;
     }
     if (t == 0)
         for (int i = 0; i <= 2 * FO; i++) {
@@ -309,7 +321,7 @@ int dsk_run_farfield(dsk_ctx *c)
     int nblk = c->nsm * 2;
     if ((int64_t)nblk * FM_WARPS * 32 > c->N) nblk = (int)((c->N + FM_WARPS * 32 - 1) / (FM_WARPS * 32));
     k_far_moments<<<dim3(nblk, FM_PARTS), FM_WARPS * 32, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_partial);
-    k_far_lambda<<<1, FM_THREADS, 0, c->stream>>>(c->far_partial, nblk, c->far_T_dev, c->far_M, c->far_lambda);
+    k_far_lambda<<<1, FM_THREADS, 0, c->stream>>>(c->far_partial, nblk, c->far_T_dev, c->far_M, c->far_lambda, c->bg, 0.5 * (double)c->box);
     k_far_eval<<<(n + 127) / 128, 128, 0, c->stream>>>(c->spos, n, 0.5f * c->box, c->far_lambda, c->sacc, c->sacc_lo);
     DSK_COUNT(c, 3);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;

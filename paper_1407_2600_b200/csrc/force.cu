@@ -20,7 +20,7 @@
 #define P2P_TILE 384         // sources per window (two windows per warp): 16 warps x 12 KB per SM; measured 256: 1.916 ms, 320: 1.890, 384: 1.872, 416: 1.874, 512: 1.898 (13 warps) on C2
 #endif
 
-int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base);   // walk.cu
+int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base, uint64_t left_base);   // walk.cu
 
 // ---- F1 ----------------------------------------------------------------------------------------------
 // Sources are staged as they are stored: a listed leaf is a contiguous run of the sorted (x, y, z, m) array,
@@ -217,12 +217,12 @@ __global__ void __launch_bounds__(FW * 32, P2P_MINB) k_p2p(uint32_t t0, uint32_t
     task_store(t, A, reinterpret_cast<double *>(src_all[warp][0]), sacc, sacc_lo);
 }
 
-static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_t t1, uint64_t mb, uint64_t pb,
+static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_t t1, uint64_t mb, uint64_t pb, uint64_t lb,
                       int want_pot, bool fill)
 {
     cudaStream_t s = c->stream;
     if (fill) {
-        int e = dsk_walk_fill(c, g0, g1, mb, pb);
+        int e = dsk_walk_fill(c, g0, g1, mb, pb, lb);
         if (e) return e;
     }
     cudaEventRecord(c->ev[8], s);
@@ -240,6 +240,10 @@ static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_
     cudaEventRecord(c->ev[9], s);
     {
         int e = dsk_launch_m2p(c, t0, t1, mb, want_pot);
+        if (e) return e;
+    }
+    if (c->periodic && c->bg) {                      // the cubes kept outside the groups' windows (background.cu)
+        int e = dsk_run_bg_left(c, g0, g1, lb, want_pot);
         if (e) return e;
     }
     cudaEventRecord(c->ev[10], s);
@@ -263,7 +267,7 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     const bool reuse = c->lists_valid && c->lists_theta == c->theta;
     c->stats.ms_p2p = c->stats.ms_m2p = 0.0f;
     if (reuse) {
-        int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, want_pot, false);
+        int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, 0, want_pot, false);
         if (e) return e;
         DSK_CUDA(cudaStreamSynchronize(s));
         add_ms(c->ev[8], c->ev[9], &c->stats.ms_p2p);
@@ -273,7 +277,7 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     }
     c->stats.ms_walk = 0.0f;
     if (c->walk_onepass) {                        // the lists are already there (walk.cu): one batch, no FILL pass
-        int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, want_pot, false);
+        int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, 0, want_pot, false);
         if (e) return e;
         DSK_CUDA(cudaStreamSynchronize(s));
         add_ms(c->ev[7], c->ev[8], &c->stats.ms_walk);
@@ -284,18 +288,22 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
         return DSK_OK;
     }
     // totals of the COUNT pass
-    uint64_t tot[2];
+    const bool BG = c->periodic && c->bg;
+    uint64_t tot[3] = {0, 0, 0};
     DSK_CUDA(cudaMemcpyAsync(&tot[0], c->g_m2p_off + ng, sizeof(uint64_t), cudaMemcpyDeviceToHost, s));
     DSK_CUDA(cudaMemcpyAsync(&tot[1], c->g_p2p_off + ng, sizeof(uint64_t), cudaMemcpyDeviceToHost, s));
+    if (BG) DSK_CUDA(cudaMemcpyAsync(&tot[2], c->g_left_off + ng, sizeof(uint64_t), cudaMemcpyDeviceToHost, s));
     DSK_CUDA(cudaStreamSynchronize(s));
     // reset the interaction counters (filled by the FILL pass)
     DSK_CUDA(cudaMemsetAsync(&c->dstate->tot_m2p_list, 0, sizeof(unsigned long long) * 5, s));
+    DSK_CUDA(cudaMemsetAsync(&c->dstate->tot_left_list, 0, sizeof(unsigned long long), s));
     // diagnostic modes 3 / 4 (dsk_set_walk_mode): pretend the list buffers are small (batches on small inputs) or tiny
     // (not even one group fits: DSK_ELISTOVERFLOW)
     const size_t cap_m = c->walk_two_pass_only == 3 ? (size_t)65536 : c->walk_two_pass_only == 4 ? (size_t)256 : c->list_m2p_cap;
     const size_t cap_p = c->walk_two_pass_only == 3 ? (size_t)8192 : c->walk_two_pass_only == 4 ? (size_t)8 : c->list_p2p_cap;
-    if (tot[0] <= cap_m && tot[1] <= cap_p) {
-        int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, want_pot, true);
+    const size_t cap_l = BG ? c->list_left_cap : (size_t)1;
+    if (tot[0] <= cap_m && tot[1] <= cap_p && tot[2] <= cap_l) {
+        int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, 0, want_pot, true);
         if (e) return e;
         DSK_CUDA(cudaStreamSynchronize(s));
         add_ms(c->ev[7], c->ev[8], &c->stats.ms_walk);
@@ -306,10 +314,12 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
         return DSK_OK;
     }
     // batches: cut the group range where either list would overflow
-    uint64_t *hm = (uint64_t *)malloc(sizeof(uint64_t) * ((size_t)ng + 1) * 2 + sizeof(uint32_t) * ((size_t)ng + 1));
+    uint64_t *hm = (uint64_t *)malloc(sizeof(uint64_t) * ((size_t)ng + 1) * 3 + sizeof(uint32_t) * ((size_t)ng + 1));
     if (!hm) return DSK_ECUDA;
-    uint64_t *hp = hm + ng + 1;
-    uint32_t *ht = (uint32_t *)(hp + ng + 1);
+    uint64_t *hp = hm + ng + 1, *hl = hp + ng + 1;
+    uint32_t *ht = (uint32_t *)(hl + ng + 1);
+    if (BG) cudaMemcpyAsync(hl, c->g_left_off, sizeof(uint64_t) * ((size_t)ng + 1), cudaMemcpyDeviceToHost, s);
+    else memset(hl, 0, sizeof(uint64_t) * ((size_t)ng + 1));
     cudaMemcpyAsync(ht, c->g_taskoff, sizeof(uint32_t) * (size_t)ng, cudaMemcpyDeviceToHost, s);
     ht[ng] = c->hstate->ntask;
     cudaMemcpyAsync(hm, c->g_m2p_off, sizeof(uint64_t) * ((size_t)ng + 1), cudaMemcpyDeviceToHost, s);
@@ -319,10 +329,10 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     int nb = 0, rc = DSK_OK;
     while (g0 < ng) {
         uint32_t g1 = g0;
-        while (g1 < ng && hm[g1 + 1] - hm[g0] <= cap_m && hp[g1 + 1] - hp[g0] <= cap_p) g1++;
+        while (g1 < ng && hm[g1 + 1] - hm[g0] <= cap_m && hp[g1 + 1] - hp[g0] <= cap_p && hl[g1 + 1] - hl[g0] <= cap_l) g1++;
         if (g1 == g0) { rc = DSK_ELISTOVERFLOW; break; }           // one group alone does not fit
         cudaEventRecord(c->ev[11], s);
-        rc = eval_batch(c, g0, g1, ht[g0], ht[g1], hm[g0], hp[g0], want_pot, true);
+        rc = eval_batch(c, g0, g1, ht[g0], ht[g1], hm[g0], hp[g0], hl[g0], want_pot, true);
         if (rc) break;
         if (cudaStreamSynchronize(s) != cudaSuccess) { rc = DSK_ECUDA; break; }
         add_ms(c->ev[11], c->ev[8], &c->stats.ms_walk);

@@ -21,30 +21,37 @@
 #include <vector>
 
 // ---- force-row layout: header of 8 floats as in the moment row, then blocks (q, m) in q-major order ----
-__host__ __device__ constexpr bool fr_has(int P, int q, int m) { return m >= q && 2 * m - q <= P && !(q == 1 && m == 1); }
+// D: the row carries a dipole block (q = m = 1).  About the centre of mass the particles' dipole vanishes and the block is
+// skipped; with background subtraction (reading O4b) the subtracted cube is centred on the cell, not on the centre of mass,
+// so the rows of a periodic run with subtraction have it (zero for the plain rows, rho_bar s^3 (com - centre) for the others).
+__host__ __device__ constexpr bool fr_has(int P, int q, int m, bool D) { return m >= q && 2 * m - q <= P && (D || !(q == 1 && m == 1)); }
 __host__ __device__ constexpr int fr_bsize(int q) { return (q + 1) * (q + 2) / 2; }
-__host__ __device__ constexpr int fr_off(int P, int q, int m)
+__host__ __device__ constexpr int fr_off(int P, int q, int m, bool D)
 {
     int o = 0;
     for (int qq = 0; qq <= P; qq++)
         for (int mm = qq; mm <= P; mm++) {
             if (qq == q && mm == m) return o;
             if (qq > q) return o;
-            if (fr_has(P, qq, mm)) o += fr_bsize(qq);
+            if (fr_has(P, qq, mm, D)) o += fr_bsize(qq);
         }
     return o;
 }
-__host__ __device__ constexpr int fr_nc(int P) { return fr_off(P, P + 1, 0); }
-__host__ __device__ constexpr int fr_rowlen(int P) { return (8 + fr_nc(P) + 3) / 4 * 4; }
+__host__ __device__ constexpr int fr_nc(int P, bool D) { return fr_off(P, P + 1, 0, D); }
+__host__ __device__ constexpr int fr_rowlen(int P, bool D) { return (8 + fr_nc(P, D) + 3) / 4 * 4; }
 __host__ __device__ constexpr int fr_qfirst_S(int P, int m) { return (m == 1 || 2 * m - P < 0) ? 0 : 2 * m - P; }
 __host__ __device__ constexpr int fr_qfirst_G(int P, int m) { return 2 * m - P < 1 ? 1 : 2 * m - P; }
 
-int dsk_frow_len(int p) { return p == 2 ? fr_rowlen(2) : p == 4 ? fr_rowlen(4) : p == 6 ? fr_rowlen(6) : fr_rowlen(8); }
+static int frow_nc(int p, bool d)
+{
+    return p == 2 ? fr_nc(2, d) : p == 4 ? fr_nc(4, d) : p == 6 ? fr_nc(6, d) : fr_nc(8, d);
+}
+int dsk_frow_len(int p, int dip) { return (8 + frow_nc(p, dip != 0) + 3) / 4 * 4; }
 
 // ---- k_frows: moment row -> force row -------------------------------------------------------------------
 struct fr_entry { uint32_t src; float w; };
 
-static void build_frow_table(int P, std::vector<uint32_t> &beg, std::vector<fr_entry> &ent)
+static void build_frow_table(int P, bool D, std::vector<uint32_t> &beg, std::vector<fr_entry> &ent)
 {
     double fact[2 * DSK_PMAX + 2];
     fact[0] = 1.0;
@@ -52,7 +59,7 @@ static void build_frow_table(int P, std::vector<uint32_t> &beg, std::vector<fr_e
     beg.clear(); ent.clear();
     for (int q = 0; q <= P; q++)
         for (int m = q; m <= P; m++) {
-            if (!fr_has(P, q, m)) continue;
+            if (!fr_has(P, q, m, D)) continue;
             const int k = m - q;
             double cm = (m & 1) ? -1.0 : 1.0;
             for (int i = 2 * m - 1; i > 0; i -= 2) cm *= i;
@@ -91,25 +98,31 @@ __global__ void __launch_bounds__(128) k_frows(uint32_t ncell, int rowlen, int f
     }
 }
 
-int dsk_run_frows(dsk_ctx *c)
+// rows [r0, r0 + n) of `rows_in` (moment rows of the current order) -> force rows [f0, f0 + n)
+static int run_frows_range(dsk_ctx *c, const float *rows_in, uint32_t n, size_t f0)
 {
-    const int P = c->p, nc = P == 2 ? fr_nc(2) : P == 4 ? fr_nc(4) : P == 6 ? fr_nc(6) : fr_nc(8);
-    if (c->frow_tab_p != P) {
+    const int P = c->p, dip = c->frow_dip, nc = frow_nc(P, dip != 0);
+    if (c->frow_tab_p != P || c->frow_tab_dip != dip) {
         std::vector<uint32_t> beg;
         std::vector<fr_entry> ent;
-        build_frow_table(P, beg, ent);
+        build_frow_table(P, dip != 0, beg, ent);
         if (beg.size() > DSK_FRTAB_BEG || ent.size() > DSK_FRTAB_ENT) return DSK_EINVAL;
         DSK_CUDA(cudaMemcpyAsync(c->frtab_beg, beg.data(), beg.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, c->stream));
         DSK_CUDA(cudaMemcpyAsync(c->frtab_ent, ent.data(), ent.size() * sizeof(fr_entry), cudaMemcpyHostToDevice, c->stream));
         DSK_CUDA(cudaStreamSynchronize(c->stream));      // the vectors die here
-        c->frow_tab_p = P;
+        c->frow_tab_p = P; c->frow_tab_dip = dip;
     }
-    const uint32_t n = c->hstate->ncell;
-    k_frows<<<(n + 3) / 4, 128, 0, c->stream>>>(n, dsk_rowlen(P), dsk_frow_len(P), nc, c->frtab_beg,
-                                                (const fr_entry *)c->frtab_ent, c->rows, c->frows);
+    if (!n) return DSK_OK;
+    const int frl = dsk_frow_len(P, dip);
+    k_frows<<<(n + 3) / 4, 128, 0, c->stream>>>(n, dsk_rowlen(P), frl, nc, c->frtab_beg,
+                                                (const fr_entry *)c->frtab_ent, rows_in, c->frows + f0 * (size_t)frl);
     DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
+
+int dsk_run_frows(dsk_ctx *c) { return run_frows_range(c, c->rows, c->hstate->ncell, 0); }
+// the background-subtracted copies of the cells of level <= l_b: force rows [ncell, ncell + ntop)   (background.cu)
+int dsk_run_frows_bg(dsk_ctx *c, uint32_t ntop) { return run_frows_range(c, c->rows_bg, ntop, c->hstate->ncell); }
 
 // ---- F2 body: the lane's sink(s) against one cell ----------------------------------------------------
 // T = f2: two sinks in the halves of every register; T = float: one sink.  The cell's row is read from
@@ -134,7 +147,7 @@ __host__ __device__ constexpr int mi_pick(MI j)
     return best;
 }
 
-template <int P, typename T, bool POT>
+template <int P, typename T, bool POT, bool DIP>
 __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restrict__ row, T &pot, T &ax, T &ay, T &az)
 {
     constexpr int NP = dsk_np(P);
@@ -173,8 +186,8 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
             });
         static_for<q, P + 1>([&](auto M) {
             constexpr int m = decltype(M)::value;
-            if constexpr (fr_has(P, q, m)) {
-                constexpr int off = fr_off(P, q, m);
+            if constexpr (fr_has(P, q, m, DIP)) {
+                constexpr int off = fr_off(P, q, m, DIP);
                 // A block is homogeneous of degree q, so by Euler's theorem sum_j B_j mu_j = (1/q) rho . grad: from
                 // degree 3 on (10 coefficients or more) only the gradient is accumulated (separately) and the value
                 // costs 3 FMAs (+ 3 adds to merge the gradient) instead of one FMA per coefficient.
@@ -189,7 +202,7 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
                         else if constexpr (q == fr_qfirst_S(P, m) && jj == 0) S[m] = vmul(B, mu[base + jj]);
                         else S[m] = vfma(B, mu[base + jj], S[m]);
                     }
-                    if constexpr (m >= 2 && q >= 1)
+                    if constexpr ((m >= 2 || DIP) && q >= 1)
                         static_for<0, 3>([&](auto I) {
                             constexpr int i = decltype(I)::value;
                             constexpr MI ji = dsk_mi(base + jj);
@@ -235,12 +248,13 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
     });
     const T tt = vfma(vmul(dq, qi), vdup<T>(2.0f), pq);
     T gh[3] = {G[P][0], G[P][1], G[P][2]};
-    static_for<1, P - 1>([&](auto K) {
-        constexpr int m = P - decltype(K)::value;                 // P-1 .. 2
+    static_for<1, (DIP ? P : P - 1)>([&](auto K) {
+        constexpr int m = P - decltype(K)::value;                 // P-1 .. 2 (.. 1 with a dipole: G_1 = the dipole itself)
         gh[0] = vfma(gh[0], qi, G[m][0]); gh[1] = vfma(gh[1], qi, G[m][1]); gh[2] = vfma(gh[2], qi, G[m][2]);
     });
     const T u = vmul(vmul(qi, vmul(h0, vdup<T>(hB.y))), tt);       // -h0 q (Pq + 2 q Pq') / s^2
-    const T k2 = vmul(vmul(qi, vmul(h0, vdup<T>(hB.w))), qi);      // h0 q^2 / s^2
+    const T k1 = vmul(qi, vmul(h0, vdup<T>(hB.w)));                // h0 q / s^2
+    const T k2 = DIP ? k1 : vmul(k1, qi);                          // h0 q^2 / s^2 when the gradient sums start at m = 2
     ax = vfma(gh[0], k2, ax); ay = vfma(gh[1], k2, ay); az = vfma(gh[2], k2, az);
     ax = vfma(rho[0], u, ax); ay = vfma(rho[1], u, ay); az = vfma(rho[2], u, az);
     if constexpr (POT) pot = vfma(vmul(pq, h0), vdup<T>(hB.z), pot);
@@ -260,10 +274,13 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
 // multi-warp block holds its registers and shared memory until its longest warp ends.
 #define FW 1
 #define M64_MINB 12          // resident warps per SM of the fp64-monopole variants at p <= 4 (164 registers; at 16 they spill: C3 19.05 vs 18.78 ms)
-template <int P, bool M64> struct m2p_cfg {
+// MODE 0: isolated (fp32, no dipole block); 1: periodic without background subtraction (monopoles in fp64, see the kernel);
+// 2: periodic with background subtraction (reading O4b: fp32 throughout, rows carry a dipole block)
+template <int P, int MODE> struct m2p_cfg {
+    static constexpr bool M64 = MODE == 1, DIP = MODE == 2;
     static constexpr int NCELL = (P <= 4) ? 32 : (P == 6 ? 16 : 8);   // cells per tile
     static constexpr int LPC = 32 / NCELL;                             // lanes that share the copy of one row
-    static constexpr int FROW = fr_rowlen(P);
+    static constexpr int FROW = fr_rowlen(P, DIP);
     static constexpr int NCH = FROW / 4;                               // 16-byte chunks per row
     static constexpr size_t BUF_BYTES = (size_t)NCELL * FROW * sizeof(float);
     static constexpr size_t M64_BYTES = M64 ? (size_t)NCELL * 4 * sizeof(double) : 0;   // com' xyz and mass of a tile's cells
@@ -278,8 +295,8 @@ __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-template <int P, bool POT, bool M64>
-__global__ void __launch_bounds__(FW * 32, (P <= 4 ? (M64 ? M64_MINB : 16) : 1)) k_m2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic,
+template <int P, bool POT, int MODE>
+__global__ void __launch_bounds__(FW * 32, (P <= 4 ? (MODE == 1 ? M64_MINB : 16) : 1)) k_m2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic,
                                                  float box, float eps2, const float *__restrict__ frows,
                                                  const float4 *__restrict__ spos, const uint32_t *__restrict__ gfirst,
                                                  const uint32_t *__restrict__ gcount, const uint32_t *__restrict__ gcell,
@@ -287,7 +304,8 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? (M64 ? M64_MINB : 16) : 1))
                                                  uint64_t base, const uint32_t *__restrict__ len,
                                                  float4 *__restrict__ sacc, float4 *__restrict__ sacc_lo)
 {
-    using C = m2p_cfg<P, M64>;
+    using C = m2p_cfg<P, MODE>;
+    constexpr bool M64 = C::M64, DIP = C::DIP;
     constexpr int NCELL = C::NCELL, LPC = C::LPC, FROW = C::FROW, NCH = C::NCH;
     constexpr uint32_t CELL_MASK = (1u << DSK_CELL_BITS) - 1u;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -396,13 +414,13 @@ __global__ void __launch_bounds__(FW * 32, (P <= 4 ? (M64 ? M64_MINB : 16) : 1))
                     const double2 c23 = *reinterpret_cast<const double2 *>(mono + 4 * k + 2);
                     mono1(c01, c23, xs0, ys0, zs0, s0);
                     mono1(c01, c23, xs1, ys1, zs1, s1);
-                    m2p_body<P, f2, POT>(X, Y, Z, rows + (size_t)k * FROW, pot, ax, ay, az);
+                    m2p_body<P, f2, POT, DIP>(X, Y, Z, rows + (size_t)k * FROW, pot, ax, ay, az);
                 }
                 acc_add_double(A, 0, 0, s0[0]); acc_add_double(A, 0, 1, s0[1]); acc_add_double(A, 0, 2, s0[2]);
                 acc_add_double(A, 1, 0, s1[0]); acc_add_double(A, 1, 1, s1[1]); acc_add_double(A, 1, 2, s1[2]);
                 if (POT) { acc_add_double(A, 0, 3, s0[3]); acc_add_double(A, 1, 3, s1[3]); }
             } else {
-                for (int k = t.sub; k < ntc; k += t.S) m2p_body<P, f2, POT>(X, Y, Z, rows + (size_t)k * FROW, pot, ax, ay, az);
+                for (int k = t.sub; k < ntc; k += t.S) m2p_body<P, f2, POT, DIP>(X, Y, Z, rows + (size_t)k * FROW, pot, ax, ay, az);
             }
             acc_fold(A, ax, ay, az, pot, POT);
         }
@@ -483,23 +501,23 @@ int dsk_order_tasks(dsk_ctx *c, uint32_t t0, uint32_t t1, const uint32_t *len, i
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
-template <int P, bool POT, bool M64>
+template <int P, bool POT, int MODE>
 static int launch_m2p_v(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base)
 {
-    using C = m2p_cfg<P, M64>;
+    using C = m2p_cfg<P, MODE>;
     static bool attr_flags[DSK_MAXDEV];
     bool *attr_done = dsk_device_flag(attr_flags);
     const size_t smem = FW * C::WARP_BYTES;
     if (!*attr_done) {
-        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, POT, M64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, POT, M64>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, POT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, POT, MODE>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         *attr_done = true;
     }
     const float e2 = c->eps * c->eps;
     const unsigned grid = (t1 - t0 + FW - 1) / FW;
-    k_m2p<P, POT, M64><<<grid, FW * 32, smem, c->stream>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->frows, c->spos,
-                                                           c->gfirst, c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
-                                                           c->g_m2p_len, c->sacc, c->sacc_lo);
+    k_m2p<P, POT, MODE><<<grid, FW * 32, smem, c->stream>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->frows, c->spos,
+                                                            c->gfirst, c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,
+                                                            c->g_m2p_len, c->sacc, c->sacc_lo);
     return DSK_OK;
 }
 
@@ -508,9 +526,11 @@ static int launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int w
 {
     int e = dsk_order_tasks(c, t0, t1, c->g_m2p_len, 3);
     if (e) return e;
-    // periodic boxes: monopoles in fp64 (see the kernel)
-    if (c->periodic) return want_pot ? launch_m2p_v<P, true, true>(c, t0, t1, base) : launch_m2p_v<P, false, true>(c, t0, t1, base);
-    return want_pot ? launch_m2p_v<P, true, false>(c, t0, t1, base) : launch_m2p_v<P, false, false>(c, t0, t1, base);
+    // the rows' layout (dipole block or not) was fixed when they were made: the kernel must match it
+    if (c->frow_dip) return want_pot ? launch_m2p_v<P, true, 2>(c, t0, t1, base) : launch_m2p_v<P, false, 2>(c, t0, t1, base);
+    // periodic without background subtraction: monopoles in fp64 (see the kernel)
+    if (c->periodic) return want_pot ? launch_m2p_v<P, true, 1>(c, t0, t1, base) : launch_m2p_v<P, false, 1>(c, t0, t1, base);
+    return want_pot ? launch_m2p_v<P, true, 0>(c, t0, t1, base) : launch_m2p_v<P, false, 0>(c, t0, t1, base);
 }
 
 int dsk_launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int want_pot)

@@ -352,8 +352,14 @@ int dsk_run_upward(dsk_ctx *c)
     default: return DSK_EINVAL;
     }
     if (e) return e;
+    c->frow_dip = c->periodic && c->bg;        // rows of a periodic run with background subtraction carry a dipole block
     e = dsk_run_frows(c);                      // the fixed linear map to the rows M2P reads (m2p.cu)
     if (e) return e;
+    c->ntop = 0;
+    if (c->frow_dip) {                         // the subtracted copies of the cells of level <= l_b (background.cu)
+        e = dsk_run_bg_rows(c);
+        if (e) return e;
+    }
     cudaEventRecord(c->ev[6], c->stream);
     c->moments_p = c->p;
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;

@@ -9,6 +9,7 @@
 // Run once into a fixed capacity per group when every list fits (the usual case), else twice: COUNT (list
 // lengths, for the offsets) and FILL.
 #include "dsk_internal.cuh"
+#include <string.h>
 
 #ifndef WW
 #define WW 1                 // warps (groups) per block: walks differ in length, a block ends with its longest
@@ -29,6 +30,76 @@ __device__ __forceinline__ void image_shift(int img, int periodic, float box, fl
     sh[0] = ix * box; sh[1] = iy * box; sh[2] = iz * box;
 }
 
+// Background subtraction (reading O4b of DESIGN.md, background.cu).  lb < 0: off.  The cells of level <= lb are the first
+// ntop cells (canonical order is level-major); topgeo holds their integer coordinates, level and child-octant mask.
+struct walk_bg {
+    int lb, k;
+    uint32_t ntop, ncell;
+    const int4 *topgeo;
+    const uint32_t *gcell;
+    const uint64_t *hotkey;
+    uint32_t *left_len;            // [ngroup] cubes kept outside the window (third list)
+    const uint64_t *left_off;      // FILL: scanned offsets
+    uint64_t left_base;
+    uint4 *list_left;
+    uint32_t cap_l;                // ONE pass: fixed capacity per group
+    uint64_t *left_off_out;
+};
+
+__device__ __forceinline__ uint32_t wk_compact3(uint64_t x)
+{
+    x &= 0x1249249249249249ull;
+    x = (x | x >> 2) & 0x10c30c30c30c30c3ull;
+    x = (x | x >> 4) & 0x100f00f00f00f00full;
+    x = (x | x >> 8) & 0x1f0000ff0000ffull;
+    x = (x | x >> 16) & 0x1f00000000ffffull;
+    x = (x | x >> 32) & 0x1fffffull;
+    return (uint32_t)x;
+}
+
+// The cubes a rejected cell of level <= lb exposes (cubes of the image block whose background no accepted cell carries): the
+// cell's own cube if it is a leaf or sits at level lb (below lb nothing carries a background), else its empty octants.  Those
+// inside the window are part of the window's cuboid; the others are kept: returns their number and, with out != nullptr, writes
+// their records (lo | hi << 16 per axis, int16 index ranges in level-lb cells).
+__device__ __forceinline__ uint32_t wk_exposed(bool whole, int lvl, int lb, const int4 geo, const int ish[3], const int wlo[3],
+                                               const int whi[3], uint4 *out)
+{
+    uint32_t n = 0;
+    const int q[3] = {geo.x, geo.y, geo.z};
+    if (whole) {
+        int lo[3], hi[3];
+        bool inside = true;
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            lo[d] = (q[d] << (lb - lvl)) + (ish[d] << lb); hi[d] = lo[d] + (1 << (lb - lvl)) - 1;
+            inside = inside && lo[d] >= wlo[d] && hi[d] <= whi[d];
+        }
+        if (!inside) {
+            if (out) out[0] = make_uint4((uint32_t)(lo[0] & 0xffff) | (uint32_t)hi[0] << 16, (uint32_t)(lo[1] & 0xffff) | (uint32_t)hi[1] << 16,
+                                         (uint32_t)(lo[2] & 0xffff) | (uint32_t)hi[2] << 16, 0u);
+            n = 1;
+        }
+        return n;
+    }
+    const int mask = (geo.w >> 8) & 255, sh = lb - lvl - 1;
+    for (int o = 0; o < 8; o++) {
+        if (mask & (1 << o)) continue;
+        const int bit[3] = {(o >> 2) & 1, (o >> 1) & 1, o & 1};
+        int lo[3], hi[3];
+        bool inside = true;
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            lo[d] = ((2 * q[d] + bit[d]) << sh) + (ish[d] << lb); hi[d] = lo[d] + (1 << sh) - 1;
+            inside = inside && lo[d] >= wlo[d] && hi[d] <= whi[d];
+        }
+        if (inside) continue;
+        if (out) out[n] = make_uint4((uint32_t)(lo[0] & 0xffff) | (uint32_t)hi[0] << 16, (uint32_t)(lo[1] & 0xffff) | (uint32_t)hi[1] << 16,
+                                     (uint32_t)(lo[2] & 0xffff) | (uint32_t)hi[2] << 16, 0u);
+        n++;
+    }
+    return n;
+}
+
 template <int MODE>          // 0 COUNT, 1 FILL at the scanned offsets, 2 ONE pass into a fixed capacity per group
 __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int periodic, float box,
                                                   const dsk_cellrec *__restrict__ cell,
@@ -42,30 +113,51 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
                                                   uint64_t p2p_base, uint32_t *__restrict__ list_m2p,
                                                   uint32_t *__restrict__ list_p2p, const uint8_t *__restrict__ gact,
                                                   uint32_t cap_m, uint32_t cap_p, uint64_t *__restrict__ m2p_off_out,
-                                                  uint64_t *__restrict__ p2p_off_out, dsk_devstate *st)
+                                                  uint64_t *__restrict__ p2p_off_out, const walk_bg bg, dsk_devstate *st)
 {
     constexpr bool FILL = MODE != 0;
+    constexpr uint32_t CELL_MASK = (1u << DSK_CELL_BITS) - 1u;
     __shared__ uint32_t stack[WW][WSTACK];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t g = g0 + blockIdx.x * WW + warp;
     if (g >= g1) return;
+    const bool BG = bg.lb >= 0;
     if (gact && !gact[g]) {                          // no active sink in this group (dsk_accel_active): empty lists
         if (MODE != 1 && lane == 0) {
             m2p_len[g] = 0; p2p_len[g] = 0; p2p_src[g] = 0;
-            if (MODE == 2) { m2p_off_out[g] = (uint64_t)g * cap_m; p2p_off_out[g] = (uint64_t)g * cap_p; }
+            if (BG) bg.left_len[g] = 0;
+            if (MODE == 2) {
+                m2p_off_out[g] = (uint64_t)g * cap_m; p2p_off_out[g] = (uint64_t)g * cap_p;
+                if (BG) bg.left_off_out[g] = (uint64_t)g * bg.cap_l;
+            }
         }
         return;
     }
     const float4 blo = gbox[2 * (size_t)g], bhi = gbox[2 * (size_t)g + 1];
+    // the group's window: the level-lb cells within k of the footprint of its cell (integer index range, unwrapped frame)
+    int wlo[3] = {0, 0, 0}, whi[3] = {0, 0, 0};
+    if (BG) {
+        const uint32_t cg = bg.gcell[g];
+        const int lg = (int)(cell[cg].meta >> 8);
+        const uint64_t prefix = bg.hotkey[cg] & ~(1ull << (3 * lg));
+        const int q[3] = {(int)wk_compact3(prefix >> 2), (int)wk_compact3(prefix >> 1), (int)wk_compact3(prefix)};
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            int flo, fhi;
+            if (lg >= bg.lb) flo = fhi = q[d] >> (lg - bg.lb);
+            else { flo = q[d] << (bg.lb - lg); fhi = flo + (1 << (bg.lb - lg)) - 1; }
+            wlo[d] = flo - bg.k; whi[d] = fhi + bg.k;
+        }
+    }
     uint32_t *stk = stack[warp];
     const int nimg = periodic ? (2 * DSK_WS + 1) * (2 * DSK_WS + 1) * (2 * DSK_WS + 1) : 1;
     for (int i = lane; i < nimg; i += 32) stk[i] = (uint32_t)i << DSK_CELL_BITS;   // root of every image
     __syncwarp();
     int sp = nimg;
-    uint32_t nm = 0, np = 0, nsrc = 0;
-    uint64_t mo = 0, po = 0;
-    if (MODE == 1) { mo = m2p_off[g] - m2p_base; po = p2p_off[g] - p2p_base; }
-    if (MODE == 2) { mo = (uint64_t)g * cap_m; po = (uint64_t)g * cap_p; }
+    uint32_t nm = 0, np = 0, nsrc = 0, nl = 0;
+    uint64_t mo = 0, po = 0, lo_ = 0;
+    if (MODE == 1) { mo = m2p_off[g] - m2p_base; po = p2p_off[g] - p2p_base; if (BG) lo_ = bg.left_off[g] - bg.left_base; }
+    if (MODE == 2) { mo = (uint64_t)g * cap_m; po = (uint64_t)g * cap_p; if (BG) lo_ = (uint64_t)g * bg.cap_l; }
     const uint32_t lt = (1u << lane) - 1u;
     // WEPL stack entries per lane and trip: their loads are independent, so a trip exposes one L2 round trip for
     // 32 * WEPL cells
@@ -79,6 +171,7 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
         uint32_t e[WEPL], nchild[WEPL], child0[WEPL];
         bool act[WEPL], accept[WEPL], leaf[WEPL];
         float4 h[WEPL], rr[WEPL];
+        int4 geo[WEPL];
 #pragma unroll
         for (int q = 0; q < WEPL; q++) {
             act[q] = lane + 32 * q < take;
@@ -89,38 +182,75 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
 #pragma unroll
         for (int q = 0; q < WEPL; q++)
             if (act[q]) {
-                const uint32_t c = e[q] & ((1u << DSK_CELL_BITS) - 1u);
+                const uint32_t c = e[q] & CELL_MASK;
                 h[q] = wmac[2 * (size_t)c];            // com.xyz, critical radius s/theta + delta
                 rr[q] = wmac[2 * (size_t)c + 1];       // the cell record (same sector)
+                if (BG && c < bg.ntop) geo[q] = bg.topgeo[c];
             }
         uint32_t push[WEPL], ptot = 0;
 #pragma unroll
         for (int q = 0; q < WEPL; q++) {
             accept[q] = false; leaf[q] = false; nchild[q] = 0; child0[q] = 0;
-            uint32_t cnt = 0;
+            uint32_t cnt = 0, nexp = 0, entry = e[q];
+            const uint32_t c = e[q] & CELL_MASK;
+            const bool top = BG && act[q] && c < bg.ntop;
+            int ish[3] = {0, 0, 0};
+            bool whole = false;
             if (act[q]) {
                 float sh[3];
-                image_shift((int)(e[q] >> DSK_CELL_BITS), periodic, box, sh);
+                const int img = (int)(e[q] >> DSK_CELL_BITS);
+                image_shift(img, periodic, box, sh);
                 const float zx = h[q].x + sh[0], zy = h[q].y + sh[1], zz = h[q].z + sh[2];
                 const float dx = fmaxf(fmaxf(blo.x - zx, zx - bhi.x), 0.0f);
                 const float dy = fmaxf(fmaxf(blo.y - zy, zy - bhi.y), 0.0f);
                 const float dz = fmaxf(fmaxf(blo.z - zz, zz - bhi.z), 0.0f);
                 const float d2 = dx * dx + dy * dy + dz * dz;
-                accept[q] = d2 > h[q].w * h[q].w;
+                bool straddles = false;
+                if (top) {
+                    // where the cell's cube lies relative to the window (integers: both sides decide alike)
+                    const int side = 2 * DSK_WS + 1, lvl = geo[q].w & 255;
+                    ish[2] = img % side - DSK_WS; ish[1] = (img / side) % side - DSK_WS; ish[0] = img / (side * side) - DSK_WS;
+                    const int qq[3] = {geo[q].x, geo[q].y, geo[q].z};
+                    bool inside = true, inter = true;
+#pragma unroll
+                    for (int d = 0; d < 3; d++) {
+                        const int lo = (qq[d] << (bg.lb - lvl)) + (ish[d] << bg.lb), hi = lo + (1 << (bg.lb - lvl)) - 1;
+                        inside = inside && lo >= wlo[d] && hi <= whi[d];
+                        inter = inter && lo <= whi[d] && hi >= wlo[d];
+                    }
+                    straddles = inter && !inside;      // partly inside the window: never accepted (its background would count twice)
+                    if (!inter) entry = (e[q] & ~CELL_MASK) | (bg.ncell + c);      // outside: the background-subtracted copy
+                }
+                accept[q] = !straddles && d2 > h[q].w * h[q].w;
                 if (!accept[q]) {
                     nchild[q] = __float_as_uint(rr[q].w) & 255u; child0[q] = __float_as_uint(rr[q].z); cnt = __float_as_uint(rr[q].y);
                     leaf[q] = nchild[q] == 0;
+                    if (top) {
+                        whole = leaf[q] || (geo[q].w & 255) == bg.lb;
+                        nexp = wk_exposed(whole, geo[q].w & 255, bg.lb, geo[q], ish, wlo, whi, nullptr);
+                    }
                 }
             }
             const uint32_t bm = __ballot_sync(0xffffffffu, accept[q]);
             const uint32_t bl = __ballot_sync(0xffffffffu, leaf[q]);
             if (FILL) {
                 const uint32_t im = nm + __popc(bm & lt), ip = np + __popc(bl & lt);
-                if (accept[q] && (MODE == 1 || im < cap_m)) list_m2p[mo + im] = e[q];
+                if (accept[q] && (MODE == 1 || im < cap_m)) list_m2p[mo + im] = entry;
                 if (leaf[q] && (MODE == 1 || ip < cap_p)) list_p2p[po + ip] = e[q];
             }
             nm += __popc(bm); np += __popc(bl);
             if (leaf[q]) nsrc += cnt;
+            if (BG && __any_sync(0xffffffffu, nexp != 0u)) {           // rare: cubes kept outside the window
+                uint32_t x = nexp;
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+                    if (lane >= o) x += y;
+                }
+                const uint32_t tot = __shfl_sync(0xffffffffu, x, 31), at = nl + x - nexp;
+                if (FILL && nexp && (MODE == 1 || at + nexp <= bg.cap_l))
+                    wk_exposed(whole, geo[q].w & 255, bg.lb, geo[q], ish, wlo, whi, bg.list_left + lo_ + at);
+                nl += tot;
+            }
             push[q] = (act[q] && !accept[q]) ? nchild[q] : 0u;      // children of rejected internal cells
             ptot += push[q];
         }
@@ -137,7 +267,7 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
         uint32_t at = sp + x - ptot;
 #pragma unroll
         for (int q = 0; q < WEPL; q++) {
-            const uint32_t img = e[q] & ~((1u << DSK_CELL_BITS) - 1u);
+            const uint32_t img = e[q] & ~CELL_MASK;
             for (uint32_t k = 0; k < push[q]; k++) stk[at + k] = img | (child0[q] + k);
             at += push[q];
         }
@@ -146,10 +276,14 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
     }
     for (int o = 16; o; o >>= 1) nsrc += __shfl_xor_sync(0xffffffffu, nsrc, o);
     if (lane == 0) {
-        if (MODE != 1) { m2p_len[g] = nm; p2p_len[g] = np; p2p_src[g] = nsrc; }
+        if (MODE != 1) {
+            m2p_len[g] = nm; p2p_len[g] = np; p2p_src[g] = nsrc;
+            if (BG) bg.left_len[g] = nl;
+        }
         if (MODE == 2) {
             m2p_off_out[g] = (uint64_t)g * cap_m; p2p_off_out[g] = (uint64_t)g * cap_p;
-            if (nm > cap_m || np > cap_p) st->scratch[0] = 1ull;      // a list did not fit: the host falls back to two passes
+            if (BG) bg.left_off_out[g] = (uint64_t)g * bg.cap_l;
+            if (nm > cap_m || np > cap_p || (BG && nl > bg.cap_l)) st->scratch[0] = 1ull;      // a list did not fit: the host falls back to two passes
         }
         if (FILL) {
             const unsigned long long ns = gcount[g];
@@ -158,6 +292,7 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
             atomicAdd(&st->tot_m2p_list, (unsigned long long)nm);
             atomicAdd(&st->tot_p2p_list, (unsigned long long)np);
             atomicAdd(&st->tot_p2p_src, (unsigned long long)nsrc);
+            if (BG && nl) atomicAdd(&st->tot_left_list, (unsigned long long)nl);
         }
     }
 }
@@ -251,6 +386,21 @@ __global__ void __launch_bounds__(256) k_walk_mac(uint32_t ncell, float box, flo
                                           __uint_as_float(r.meta));
 }
 
+static walk_bg make_walk_bg(dsk_ctx *c, uint64_t left_base, uint32_t cap_l)
+{
+    walk_bg b;
+    memset(&b, 0, sizeof(b));
+    b.lb = -1;
+    if (c->periodic && c->bg) {
+        b.lb = c->bg_level; b.k = dsk_bg_halfwidth(c->theta, c->bg_level);
+        b.ntop = c->ntop; b.ncell = c->hstate->ncell;
+        b.topgeo = c->topgeo; b.gcell = c->gcell; b.hotkey = c->hotkey;
+        b.left_len = c->g_left_len; b.left_off = c->g_left_off; b.left_base = left_base;
+        b.list_left = c->list_left; b.cap_l = cap_l; b.left_off_out = c->g_left_off;
+    }
+    return b;
+}
+
 // W.  First choice: ONE pass into a fixed capacity per group (list buffer / number of groups), which saves the COUNT
 // pass and the scans whenever every list fits — checked with one flag read; a context that saw an overflow at this
 // theta goes straight to the general form: COUNT pass + offsets here, FILL per batch from dsk_walk_fill (force.cu).
@@ -264,18 +414,21 @@ int dsk_run_walk(dsk_ctx *c)
     k_walk_mac<<<(nc + 255) / 256, 256, 0, s>>>(nc, c->box, inv_theta, c->cell, c->whdr, c->wmac);
     DSK_COUNT(c, 1);
     c->walk_onepass = 0;
-    const uint64_t cap_m = ng ? c->list_m2p_cap / ng : 0, cap_p = ng ? c->list_p2p_cap / ng : 0;
+    const bool BG = c->periodic && c->bg;
+    const uint64_t cap_m = ng ? c->list_m2p_cap / ng : 0, cap_p = ng ? c->list_p2p_cap / ng : 0, cap_l = ng && BG ? c->list_left_cap / ng : 0;
     const bool tiny = c->walk_two_pass_only == 2;          // diagnostic: capacities that overflow, to exercise the fallback
     if (cap_m >= 4096 && cap_p >= 512 && (c->onepass_bad_theta != c->theta || tiny) && c->walk_two_pass_only != 1 &&
         c->walk_two_pass_only < 3) {
         DSK_CUDA(cudaMemsetAsync(&c->dstate->tot_m2p_list, 0, sizeof(unsigned long long) * 5, s));
         DSK_CUDA(cudaMemsetAsync(&c->dstate->scratch[0], 0, sizeof(unsigned long long), s));
+        DSK_CUDA(cudaMemsetAsync(&c->dstate->tot_left_list, 0, sizeof(unsigned long long), s));
         const uint32_t cm = tiny ? 64u : (uint32_t)(cap_m > 0xffffff00ull ? 0xffffff00ull : cap_m),
-                       cp = tiny ? 8u : (uint32_t)(cap_p > 0xffffff00ull ? 0xffffff00ull : cap_p);
+                       cp = tiny ? 8u : (uint32_t)(cap_p > 0xffffff00ull ? 0xffffff00ull : cap_p),
+                       cl = (uint32_t)(cap_l > 0xffffff00ull ? 0xffffff00ull : cap_l);
         k_walk<2><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic, c->box, c->cell, c->wmac, c->gbox, c->gcount,
                                                          c->g_m2p_len, c->g_p2p_len, c->g_p2p_src, nullptr, nullptr, 0, 0,
                                                          c->list_m2p, c->list_p2p, c->gact_cur, cm, cp, c->g_m2p_off,
-                                                         c->g_p2p_off, c->dstate);
+                                                         c->g_p2p_off, make_walk_bg(c, 0, cl), c->dstate);
         DSK_COUNT(c, 1);
         unsigned long long ovf = 0;
         DSK_CUDA(cudaMemcpyAsync(&ovf, &c->dstate->scratch[0], sizeof(ovf), cudaMemcpyDeviceToHost, s));
@@ -286,19 +439,20 @@ int dsk_run_walk(dsk_ctx *c)
     k_walk<0><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic, c->box, c->cell, c->wmac,
                                                      c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len,
                                                      c->g_p2p_src, nullptr, nullptr, 0, 0, nullptr, nullptr,
-                                                     c->gact_cur, 0, 0, nullptr, nullptr, c->dstate);
+                                                     c->gact_cur, 0, 0, nullptr, nullptr, make_walk_bg(c, 0, 0), c->dstate);
     scan64(c, c->g_m2p_len, ng, c->g_m2p_off);
     scan64(c, c->g_p2p_len, ng, c->g_p2p_off);
+    if (BG) scan64(c, c->g_left_len, ng, c->g_left_off);
     DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
-int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base)
+int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base, uint64_t left_base)
 {
     k_walk<1><<<(g1 - g0 + WW - 1) / WW, WW * 32, 0, c->stream>>>(
         g0, g1, c->periodic, c->box, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len,
         c->g_p2p_len, c->g_p2p_src, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p,
-        c->gact_cur, 0, 0, nullptr, nullptr, c->dstate);
+        c->gact_cur, 0, 0, nullptr, nullptr, make_walk_bg(c, left_base, 0), c->dstate);
     DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }

@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libdsk.so")
 
 SYMBOLS = [
     "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
-    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_get_keys",
+    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_set_background", "dsk_get_background", "dsk_get_bg_moments", "dsk_get_keys",
     "dsk_get_tree", "dsk_get_moments", "dsk_get_moments_scaled", "dsk_get_groups", "dsk_get_stats", "dsk_get_param", "dsk_get_task_widths",
     "dsk_get_lattice_tensors", "dsk_probe_fp32_peak", "dsk_probe_fp32_peak_ex", "dsk_strerror",
 ]
@@ -22,7 +22,7 @@ SYMBOLS = [
 
 class DskStats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("n", "ncell", "nleaf_cells", "ngroup", "nlevel", "n_p2p", "n_m2p",
-                                         "list_m2p", "list_p2p", "nbatch", "n_launch")] + \
+                                         "list_m2p", "list_p2p", "nbatch", "n_launch", "list_bg")] + \
                [(k, C.c_float) for k in ("ms_key", "ms_sort", "ms_build", "ms_upward", "ms_group", "ms_walk",
                                          "ms_p2p", "ms_m2p", "ms_far", "ms_scatter", "ms_kdk")]
 
@@ -63,6 +63,9 @@ def load_library(path=LIB_PATH):
     lib.dsk_kdk_block_step.argtypes = [vp, vp, vp, vp, vp, f64, f64, i32, f32]
     lib.dsk_kdk_reset.argtypes = [vp]
     lib.dsk_set_walk_mode.argtypes = [vp, i32]
+    lib.dsk_set_background.argtypes = [vp, i32]
+    lib.dsk_get_background.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i64), C.POINTER(f64)]
+    lib.dsk_get_bg_moments.argtypes = [vp, vp]
     lib.dsk_set_cosmology.argtypes = [vp, f64, f64]
     lib.dsk_get_keys.argtypes = [vp, vp, vp]
     lib.dsk_get_tree.argtypes = [vp, C.POINTER(i64), vp, vp, vp, vp]
@@ -212,6 +215,20 @@ class Dsk:
             raise TypeError("rung: contiguous uint8 CUDA tensor [N]")
         _check(self.lib.dsk_kdk_block_step(self._h, _ptr(pos), _ptr(vel), _ptr(mass), C.c_void_p(rung.data_ptr()),
                                            float(a), float(da), int(rmax), float(eta)))
+
+    def set_background(self, on):
+        _check(self.lib.dsk_set_background(self._h, int(bool(on))))
+
+    def get_background(self):
+        on, lv, k, nt, rho = C.c_int(0), C.c_int(0), C.c_int(0), C.c_int64(0), C.c_double(0)
+        _check(self.lib.dsk_get_background(self._h, C.byref(on), C.byref(lv), C.byref(k), C.byref(nt), C.byref(rho)))
+        return dict(on=bool(on.value), level=lv.value, halfwidth=k.value, ntop=nt.value, rhobar=rho.value)
+
+    def get_bg_moments(self):
+        nt = self.get_background()["ntop"]
+        mom = torch.empty((nt, nparams(self.p)), dtype=torch.float32, device=self.device)
+        _check(self.lib.dsk_get_bg_moments(self._h, _ptr(mom)))
+        return mom
 
     def set_walk_mode(self, mode):
         _check(self.lib.dsk_set_walk_mode(self._h, int(mode)))

@@ -61,12 +61,14 @@ def test_accounting_matches_kernel_op_counts():
     if not (os.path.exists(cuobjdump) and os.path.exists(obj)):
         pytest.skip("cuobjdump or build/m2p.o missing: the SASS half of this test did not run")
     sass = subprocess.run([cuobjdump, "-sass", obj], capture_output=True, text=True).stdout
-    for p in (2, 4, 6):                                     # the packed (f32x2) instantiations: <P, pot, fp32 monopoles>
-        fn = [b for b in sass.split("Function : ")[1:] if b.startswith(f"_Z5k_m2pILi{p}ELb1ELb0EE")]
-        assert len(fn) == 1
-        ffma, fmul, fadd = accounting.m2p_ops(p, pot=True)
-        assert fn[0].count(" FFMA2 ") == ffma, (p, fn[0].count(" FFMA2 "), ffma)
-        assert fn[0].count(" FMUL2 ") == fmul, (p, fn[0].count(" FMUL2 "), fmul)
-        # + the packed TwoSum fold of the tile sums into the two-float accumulators: 6 adds x 4 components
-        # (a few more where the compiler packs scalar pairs itself, e.g. the sinks' offsets from the group centre)
-        assert fadd + 24 <= fn[0].count(" FADD2 ") <= fadd + 32, (p, fn[0].count(" FADD2 "), fadd)
+    for mode, dip in ((0, False), (2, True)):               # isolated rows; periodic rows with the dipole block (background subtraction)
+        for p in (2, 4, 6):                                 # the packed (f32x2) instantiations: <P, pot, MODE>
+            fn = [b for b in sass.split("Function : ")[1:] if b.startswith(f"_Z5k_m2pILi{p}ELb1ELi{mode}EE")]
+            assert len(fn) == 1
+            ffma, fmul, fadd = accounting.m2p_ops(p, pot=True, dip=dip)
+            assert fn[0].count(" FFMA2 ") == ffma, (p, mode, fn[0].count(" FFMA2 "), ffma)
+            assert fn[0].count(" FMUL2 ") == fmul, (p, mode, fn[0].count(" FMUL2 "), fmul)
+            # + the packed TwoSum fold of the tile sums into the two-float accumulators: 6 adds x 4 components
+            # (a few more where the compiler packs scalar pairs itself, e.g. the sinks' offsets from the group centre)
+            assert fadd + 24 <= fn[0].count(" FADD2 ") <= fadd + 32, (p, mode, fn[0].count(" FADD2 "), fadd)
+    assert accounting.m2p_flops(4, dip=True) - accounting.m2p_flops(4) == 2 * 6 - 1

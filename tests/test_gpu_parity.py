@@ -601,6 +601,116 @@ def test_perfect_lattice_force_free(dsk):
     d.close()
 
 
+# ---- background subtraction (reading O4b) ------------------------------------------------------
+def _clumpy(n, seed, nclump=3, spread=0.02):
+    rng = np.random.default_rng(seed)
+    c = rng.random((nclump, 3))
+    pos = np.mod(c[rng.integers(nclump, size=n)] + spread * rng.standard_normal((n, 3)), 1.0).astype(np.float32)
+    pos[pos >= 1.0] = 0.0
+    mass = (rng.uniform(0.5, 1.5, n) / n).astype(np.float32)
+    return pos, mass
+
+
+@pytest.mark.parametrize("case", ["lattice", "clustered", "clumpy"])
+def test_background_level_window_and_moments(dsk, orc, case):
+    """The integers of reading O4b (l_b, the window half-width k, the number of cells of level <= l_b) and rho_bar agree with
+    the oracle; the subtracted moments of every such cell agree with the oracle's closed-form cube moments to 2e-6 of the
+    natural size rho_bar s^3 s^|n| + M s^|n| (the subtraction itself is done in fp64 on the device)."""
+    if case == "lattice":
+        pos, mass = workloads.perturbed_lattice(24)
+    elif case == "clustered":
+        pos, mass = workloads.clustered_box(24, 20, cfg=4)
+    else:
+        pos, mass = _clumpy(3000, 3, nclump=5)
+    mass = (mass * np.random.default_rng(2).uniform(0.5, 1.5, len(mass))).astype(np.float32)
+    for p in (2, 4, 8):
+        d = dsk.Dsk(len(pos), 1.0, True, 1e-3, 0.5, p)
+        assert d.get_background()["on"]
+        d.build_tree(_dev(pos), _dev(mass))
+        t = orc.OracleTree(pos, mass, 1.0, True)
+        lb, rho, mb = t.moments_bg(p)
+        d.get_moments()                                     # makes sure the upward pass of order p has run
+        b = d.get_background()
+        assert b["level"] == lb == orc.bg_level(len(pos)) and b["ntop"] == len(mb)
+        for theta in (0.3, 0.5, 0.6, 1.0):
+            d.set_params(theta=theta)
+            assert d.get_background()["halfwidth"] == orc.bg_halfwidth(theta, lb)
+        assert abs(b["rhobar"] - rho) < 1e-12 * rho
+        g = d.get_bg_moments().cpu().numpy().astype(np.float64)
+        cm = t.moments(p)[0][:len(mb)]
+        side = 2.0 ** (-t.cells()["level"][:len(mb)].astype(np.float64))
+        rank = np.array([sum(n) for n in orc.mtable(p)])
+        sn = side[:, None] ** rank[None, :]
+        scale = (cm + rho * side ** 3)[:, None]
+        assert np.max(np.abs(g - mb / sn) / scale) < 2e-6, np.max(np.abs(g - mb / sn) / scale)
+        # the monopole is the fp64 difference rounded once: 1e-7 of ITSELF, not of the cell's mass
+        assert np.max(np.abs(g[:, 0] - mb[:, 0]) / (np.abs(mb[:, 0]) + 1e-9 * cm)) < 2e-7
+        d.close()
+
+
+@pytest.mark.parametrize("theta", [0.4, 0.7, 1.0])
+def test_background_coarse_cubes_outside_the_window(dsk, orc, theta):
+    """A few tight clumps in an otherwise empty periodic box: the tree is shallow and lopsided, so the walk meets coarse leaves
+    and empty octants that stick out of the window and keeps them in its third list; their background is summed cube by
+    cube.  Every particle's force and potential against the oracle; the list must not be empty (the case does what it is for),
+    and the one-pass, two-pass and batched walks agree bit for bit."""
+    pos, mass = _clumpy(1200, 11, nclump=4)
+    n = len(pos)
+    eps = 2e-3
+    d = dsk.Dsk(n, 1.0, True, eps, theta, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    _check_structure(orc, d, pos, mass, 1.0, True)
+    acc, pot = d.accel(tp, tm)
+    st = d.get_stats()
+    assert st["list_bg"] > 0
+    ta, tpot, _, n_m2p, _ = orc.tree_force(pos, mass, 1.0, True, eps, theta, 4)
+    assert abs(st["n_m2p"] - n_m2p) <= 1e-3 * n_m2p
+    a = acc.cpu().numpy().astype(np.float64); ph = pot.cpu().numpy().astype(np.float64)
+    scale = np.sqrt((ta ** 2).sum(1).mean())
+    err = np.linalg.norm(a - ta, axis=1) / np.maximum(np.linalg.norm(ta, axis=1), 1e-3 * scale)
+    assert np.quantile(err, 0.999) < 1e-4, (np.quantile(err, 0.999), err.max())
+    assert np.max(np.abs(ph - tpot)) < 1e-4 * np.abs(tpot).max() + 1e-6
+    for mode in (1, 2, 3):
+        d.set_walk_mode(mode)
+        a2, p2 = d.accel(tp, tm)
+        assert torch.equal(a2, acc) and torch.equal(p2, pot), mode
+        assert d.get_stats()["list_bg"] == st["list_bg"]
+    d.close()
+
+
+@pytest.mark.parametrize("case", ["lattice", "clustered"])
+def test_background_off_is_the_round1_definition(dsk, orc, case):
+    """dsk_set_background(0): plain particle moments, the neutralising background only in the far field (and fp64 monopoles):
+    parity with the oracle's bg = False path; and the two definitions approximate the same field."""
+    pos, mass = workloads.perturbed_lattice(20) if case == "lattice" else workloads.clustered_box(20, 10, cfg=4)
+    n = len(pos)
+    eps = 1.0 / 800
+    d = dsk.Dsk(n, 1.0, True, eps, 0.5, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    a_on = d.accel(tp, tm, want_pot=False)[0].cpu().numpy().astype(np.float64)
+    d.set_background(False)
+    assert not d.get_background()["on"] and d.get_background()["ntop"] == 0
+    a_off = d.accel(tp, tm, want_pot=False)[0].cpu().numpy().astype(np.float64)
+    assert d.get_stats()["list_bg"] == 0
+    sink = workloads.subsample(3, n, 1500)
+    t = orc.OracleTree(pos, mass, 1.0, True)
+    for a, bg in ((a_on, True), (a_off, False)):
+        ta = orc.tree_force(pos, mass, 1.0, True, eps, 0.5, 4, sink, tree=t, bg=bg)[0]
+        rel = np.linalg.norm(a[sink] - ta, axis=1) / np.linalg.norm(ta, axis=1)
+        assert np.quantile(rel, 0.999) < 1e-4, (bg, np.quantile(rel, 0.999))
+    assert _erms(a_on, a_off) < 5e-3
+    d.set_background(True)
+    again = d.accel(tp, tm, want_pot=False)[0].cpu().numpy().astype(np.float64)
+    assert np.array_equal(again, a_on)
+    iso = dsk.Dsk(100, 1.0, False, 1e-3, 0.5, 4)
+    with pytest.raises(dsk.DskError):
+        iso.set_background(True)
+    iso.close()
+    d.close()
+
+
 # ---- KDK ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("periodic", [False, True])
 def test_kdk_step(dsk, orc, periodic):

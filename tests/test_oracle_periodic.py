@@ -190,10 +190,15 @@ def test_tree_force_periodic_vs_ewald(orc):
         e[(theta, p)] = math.sqrt(((acc - ref) ** 2).sum() / (ref ** 2).sum())
         assert np.max(np.abs(pot - refp)) < 5e-3 * np.abs(refp).max()
     assert e[(1e-6, 4)] < 2e-5            # only the WS=2 / order-8 far-field truncation remains
-    # the same with WS = 1 floors at ~1.6e-3: the measurement behind WS = 2
-    a1 = orc.tree_force(pos, mass, 1.0, True, eps, 1e-6, 4, sink, ws=1)[0]
+    # the same with WS = 1 and no background subtraction floors at ~1.6e-3: the measurement behind WS = 2
     r1 = orc.direct_per(pos, mass, 1.0, eps, sink, ws=1)[0]
-    assert 3e-4 < math.sqrt(((a1 - r1) ** 2).sum() / (r1 ** 2).sum()) < 5e-3
+    a1 = orc.tree_force(pos, mass, 1.0, True, eps, 1e-6, 4, sink, ws=1, bg=False)[0]
+    f_plain = math.sqrt(((a1 - r1) ** 2).sum() / (r1 ** 2).sum())
+    assert 3e-4 < f_plain < 5e-3
+    # with subtraction (reading O4b) the far field sees the neutral box and the WS = 1 floor drops ~10x (still above WS = 2's)
+    a1 = orc.tree_force(pos, mass, 1.0, True, eps, 1e-6, 4, sink, ws=1, bg=True)[0]
+    f_bg = math.sqrt(((a1 - r1) ** 2).sum() / (r1 ** 2).sum())
+    assert e[(1e-6, 4)] < f_bg < f_plain / 5
     assert e[(0.5, 4)] < 5e-3 and e[(0.5, 8)] < e[(0.5, 4)]
 
 
