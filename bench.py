@@ -358,7 +358,8 @@ def measure_config(cfgid, steps, warmup, dev, world, rank, dist, want_e2e, want_
                "interactions_per_s": (st["n_m2p"] + st["n_p2p"]) * world / (ms_max / steps * 1e-3),
                "phase_ms": {k[3:]: round(v, 4) for k, v in phase.items()},
                "tree": {"ncell": st["ncell"], "ngroup": st["ngroup"], "nlevel": st["nlevel"],
-                        "n_p2p": st["n_p2p"], "n_m2p": st["n_m2p"], "nbatch": st["nbatch"]},
+                        "n_p2p": st["n_p2p"], "n_m2p": st["n_m2p"], "nbatch": st["nbatch"],
+                        "list_m2p": st["list_m2p"], "list_p2p": st["list_p2p"], "list_bg": st["list_bg"]},
                "cpu_baseline": cpu,
                "e2e": e2e,
                "gpu_launches": int(st["n_launch"]) * steps,

@@ -120,6 +120,15 @@ int dsk_kdk_reset(dsk_ctx *ctx);
  * background in the far field alone (and fp64 monopoles).
  * DSK_EINVAL for on != 0 in an isolated context.  Changing it invalidates moments, lists and the cached KDK force. */
 int dsk_set_background(dsk_ctx *ctx, int on);
+/* Half-width WS of the block of periodic images that is summed explicitly by the tree, (2 WS + 1)^3 images; everything
+ * beyond it is the order-8 far field (reading O7 of DESIGN.md: "WS is measured, not assumed").  ws = 1 or 2;
+ * 1 is the default (dsk_get_param "WS"), 2 the largest the library supports ("WS_MAX").  With background subtraction the far
+ * field sees a neutral box and ws = 1 floors the force error at ~2e-4 of the rms force on a near-lattice box and ~3e-6 on a
+ * clustered one (WS = 2: 5e-6 and 5e-9), for 11-18 % fewer cell interactions; WITHOUT subtraction ws = 1 floors at 3e-3 to
+ * 2e-2: a context that switches subtraction off should set ws = 2.
+ * DSK_EINVAL in an isolated context or for another value.  Invalidates lists and the cached KDK force. */
+int dsk_set_image_block(dsk_ctx *ctx, int ws);
+int dsk_get_image_block(dsk_ctx *ctx, int *ws /* host; 0 in an isolated context */);
 /* host pointers, each may be NULL: on / off, l_b, the window half-width k for the current theta, the number of cells of
  * level <= l_b in the current tree (0 when off or no tree) and rho_bar (0 unless the moments are up to date). */
 int dsk_get_background(dsk_ctx *ctx, int *on, int *level, int *halfwidth, int64_t *ntop, double *rhobar);
@@ -169,7 +178,7 @@ int dsk_get_moments_scaled(dsk_ctx *ctx, float *com_mass, float *moments);
 int dsk_get_groups(dsk_ctx *ctx, int64_t *ngroup, uint32_t *first, uint32_t *count, float *bbox,
                    uint32_t *m2p_len, uint32_t *p2p_len);
 int dsk_get_stats(dsk_ctx *ctx, dsk_stats *out /* host */);
-/* library constants: "NLEAF", "NCRIT", "WS", "KEY_LEVELS", "FAR_ORDER"; host pointer. */
+/* library constants: "NLEAF", "NCRIT", "WS" (default image-block half-width), "WS_MAX", "KEY_LEVELS", "FAR_ORDER"; host pointer. */
 int dsk_get_param(const char *name, double *value);
 /* How the force kernels cut a sink group of n (1..NCRIT) sinks into warp tasks: widths[k] =
  * sink lanes (two sinks each) of task k, 0 for unused tasks; the widths sum to ceil(n/2), each <= 32.  Host pointer;

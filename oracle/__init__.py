@@ -24,7 +24,8 @@ from . import build as _build
 
 NLEAF = 112   # library constants shared with the CUDA path (O3/O5: the paper leaves them free)
 NCRIT = 192
-WS = 2     # measured: WS = 1 floors the periodic force error at ~3e-3 on near-lattice inputs
+WS = 1     # default half-width of the explicit image block (O7: measured; 2 is the other supported value)
+WS_MAX = 2
 KEY_LEVELS = 21
 FAR_ORDER = 8
 BG_DEFAULT = True    # background subtraction (reading O4b) in periodic boxes: on by default on both sides (dsk_set_background)

@@ -281,9 +281,9 @@ int dsk_bg_level(int64_t n)
     int l = lg < 6 ? 0 : (lg - 6) / 3;
     return l < 2 ? 2 : l;
 }
-int dsk_bg_halfwidth(float theta, int lb)
+int dsk_bg_halfwidth(float theta, int lb, int ws)
 {
-    const int k = (int)ceil(1.0 / (double)theta), kmax = DSK_WS << lb;
+    const int k = (int)ceil(1.0 / (double)theta), kmax = ws << lb;
     return k < kmax ? k : kmax;
 }
 
@@ -319,7 +319,7 @@ int dsk_run_bg_window(dsk_ctx *c, int want_pot)
 {
     const uint32_t ng = c->hstate->ngroup;
     cudaStream_t s = c->stream;
-    const int k = dsk_bg_halfwidth(c->theta, c->bg_level);
+    const int k = dsk_bg_halfwidth(c->theta, c->bg_level, c->img_ws);
     const unsigned nb = (unsigned)(((size_t)ng * 32 + 127) / 128);
     if (want_pot)
         k_bg_window<true><<<nb, 128, 0, s>>>(ng, c->bg_level, k, c->box, c->mass64, c->gfirst, c->gcount, c->gcell, c->gact_cur,
@@ -336,7 +336,7 @@ int dsk_run_bg_left(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t base, int wan
 {
     if (g1 <= g0) return DSK_OK;
     cudaStream_t s = c->stream;
-    const int k = dsk_bg_halfwidth(c->theta, c->bg_level);
+    const int k = dsk_bg_halfwidth(c->theta, c->bg_level, c->img_ws);
     const unsigned nb = (unsigned)(((size_t)(g1 - g0) * 32 + 127) / 128);
     if (want_pot)
         k_bg_left<true><<<nb, 128, 0, s>>>(g0, g1, c->list_left, c->g_left_off, base, c->g_left_len, c->bg_level, k, c->box, c->mass64,

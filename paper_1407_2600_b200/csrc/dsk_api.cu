@@ -58,7 +58,9 @@ static size_t carve(dsk_ctx *c, char *base)
     c->rows_bg = (float *)take(4 * (size_t)dsk_rowlen(c->p_cap) * nt);
     c->g_left_len = (uint32_t *)take(4 * (c->periodic ? ng : 0));
     c->g_left_off = (uint64_t *)take(8 * (c->periodic ? ng + 1 : 0));
-    c->list_left_cap = c->periodic ? n / 8 + (1u << 16) : 0;
+    // third list: cubes kept outside the windows.  Usually < 1 per group, a few for groups next to a halo: N/2 records
+    // give the one-pass walk ~20 per group (a group that needs more sends the evaluation to the two-pass form)
+    c->list_left_cap = c->periodic ? n / 2 + (1u << 16) : 0;
     c->list_left = (uint4 *)take(16 * c->list_left_cap);
     c->frtab_beg = (uint32_t *)take(4 * DSK_FRTAB_BEG);
     c->frtab_ent = (void *)take(8 * DSK_FRTAB_ENT);
@@ -120,7 +122,8 @@ extern "C" int dsk_create(dsk_ctx **out, int64_t N, float box, int periodic, flo
     c->onepass_bad_theta = -1.0f;
     c->ws_bytes = 0;
     carve(c, nullptr);
-    if (c->periodic) dsk_lattice_tensors((double)box, DSK_WS, c->far_T);
+    c->img_ws = DSK_WS_DEFAULT;
+    if (c->periodic) dsk_lattice_tensors((double)box, c->img_ws, c->far_T);
     c->stats.n = N;
     *out = c;
     return DSK_OK;
@@ -359,6 +362,27 @@ extern "C" int dsk_set_cosmology(dsk_ctx *c, double omega_m, double omega_lambda
     return DSK_OK;
 }
 
+extern "C" int dsk_set_image_block(dsk_ctx *c, int ws)
+{
+    if (!c || !c->periodic || ws < 1 || ws > DSK_WS) return DSK_EINVAL;
+    if (ws == c->img_ws) return DSK_OK;
+    c->img_ws = ws;
+    dsk_lattice_tensors((double)c->box, ws, c->far_T);         // the far field starts where the block ends
+    if (c->ws_bytes) {
+        DSK_CUDA(cudaMemcpyAsync(c->far_T_dev, c->far_T, sizeof(double) * DSK_NFAR, cudaMemcpyHostToDevice, c->stream));
+        DSK_CUDA(cudaStreamSynchronize(c->stream));
+    }
+    c->lists_valid = 0; c->kdk_have_acc = 0;
+    return DSK_OK;
+}
+
+extern "C" int dsk_get_image_block(dsk_ctx *c, int *ws)
+{
+    if (!c || !ws) return DSK_EINVAL;
+    *ws = c->periodic ? c->img_ws : 0;
+    return DSK_OK;
+}
+
 extern "C" int dsk_set_background(dsk_ctx *c, int on)
 {
     if (!c) return DSK_EINVAL;
@@ -373,7 +397,7 @@ extern "C" int dsk_get_background(dsk_ctx *c, int *on, int *level, int *halfwidt
     if (!c) return DSK_EINVAL;
     if (on) *on = c->bg;
     if (level) *level = c->bg_level;
-    if (halfwidth) *halfwidth = dsk_bg_halfwidth(c->theta, c->bg_level);
+    if (halfwidth) *halfwidth = dsk_bg_halfwidth(c->theta, c->bg_level, c->img_ws);
     if (ntop) *ntop = c->bg && c->have_tree ? (int64_t)c->ntop : 0;
     if (rhobar) {
         *rhobar = 0.0;
@@ -600,7 +624,8 @@ extern "C" int dsk_get_param(const char *name, double *v)
     if (!name || !v) return DSK_EINVAL;
     if (!strcmp(name, "NLEAF")) *v = DSK_NLEAF;
     else if (!strcmp(name, "NCRIT")) *v = DSK_NCRIT;
-    else if (!strcmp(name, "WS")) *v = DSK_WS;
+    else if (!strcmp(name, "WS")) *v = DSK_WS_DEFAULT;
+    else if (!strcmp(name, "WS_MAX")) *v = DSK_WS;
     else if (!strcmp(name, "KEY_LEVELS")) *v = DSK_KEY_LEVELS;
     else if (!strcmp(name, "FAR_ORDER")) *v = DSK_FAR_ORDER;
     else return DSK_EINVAL;

@@ -12,7 +12,9 @@
 #ifndef DSK_NCRIT
 #define DSK_NCRIT 192        // sink group: first cell from the root with count <= NCRIT (at most 4 tasks of 32 lanes x 2 sinks)
 #endif
-#define DSK_WS 2              // image block half-width (WS = 1 floors the error at ~3e-3)
+#define DSK_WS 2              // LARGEST image block half-width, and the one image ids are encoded for: id = ((ix+2) 5 + iy+2) 5 + iz+2.
+                              // The block actually summed is the context's ws (1 or 2, dsk_set_image_block): ids with |i| <= ws.
+#define DSK_WS_DEFAULT 1      // with background subtraction WS = 1 costs 1e-4 of the rms force on a near-lattice box and saves 11-18 %
 #define DSK_FAR_ORDER 8
 #define DSK_NFAR 165          // C(8+3,3)
 #define DSK_PMAX 8
@@ -155,6 +157,7 @@ struct dsk_ctx {
     uint32_t *list_m2p, *list_p2p;
     size_t list_m2p_cap, list_p2p_cap;             // entries
     // background subtraction (background.cu; periodic contexts only)
+    int img_ws;               // image block half-width in use, 1 or 2 (dsk_set_image_block)
     int bg;                   // on / off (dsk_set_background)
     int bg_level;             // l_b
     uint32_t ntop;            // cells of level <= l_b of the current tree
@@ -226,7 +229,7 @@ int dsk_frow_len(int p, int dip);                                             //
 int dsk_run_frows(dsk_ctx *c);                                                // m2p.cu: moment rows -> force rows
 int dsk_run_frows_bg(dsk_ctx *c, uint32_t ntop);                              // m2p.cu: subtracted rows -> force rows [ncell ..]
 int dsk_bg_level(int64_t n);                                                  // background.cu
-int dsk_bg_halfwidth(float theta, int lb);                                    // background.cu
+int dsk_bg_halfwidth(float theta, int lb, int ws);                            // background.cu
 int dsk_run_bg_rows(dsk_ctx *c);                                              // background.cu: after the upward pass
 int dsk_run_bg_window(dsk_ctx *c, int want_pot);                              // background.cu: after all batches
 int dsk_run_bg_left(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t base, int want_pot);   // background.cu: per batch

@@ -150,10 +150,23 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
         }
     }
     uint32_t *stk = stack[warp];
-    const int nimg = periodic ? (2 * DSK_WS + 1) * (2 * DSK_WS + 1) * (2 * DSK_WS + 1) : 1;
-    for (int i = lane; i < nimg; i += 32) stk[i] = (uint32_t)i << DSK_CELL_BITS;   // root of every image
+    // root of every image of the block in use: periodic = the block's half-width ws (0 isolated); ids are those of the 5^3 encoding
+    int sp = 0;
+    {
+        const int side = 2 * DSK_WS + 1, nid = periodic ? side * side * side : 1;
+        for (int i0 = 0; i0 < nid; i0 += 32) {
+            const int i = i0 + lane;
+            bool in = i < nid;
+            if (periodic && in) {
+                const int iz = i % side - DSK_WS, iy = (i / side) % side - DSK_WS, ix = i / (side * side) - DSK_WS;
+                in = abs(ix) <= periodic && abs(iy) <= periodic && abs(iz) <= periodic;
+            }
+            const uint32_t m = __ballot_sync(0xffffffffu, in);
+            if (in) stk[sp + __popc(m & ((1u << lane) - 1u))] = (uint32_t)(periodic ? i : 0) << DSK_CELL_BITS;
+            sp += __popc(m);
+        }
+    }
     __syncwarp();
-    int sp = nimg;
     uint32_t nm = 0, np = 0, nsrc = 0, nl = 0;
     uint64_t mo = 0, po = 0, lo_ = 0;
     if (MODE == 1) { mo = m2p_off[g] - m2p_base; po = p2p_off[g] - p2p_base; if (BG) lo_ = bg.left_off[g] - bg.left_base; }
@@ -392,7 +405,7 @@ static walk_bg make_walk_bg(dsk_ctx *c, uint64_t left_base, uint32_t cap_l)
     memset(&b, 0, sizeof(b));
     b.lb = -1;
     if (c->periodic && c->bg) {
-        b.lb = c->bg_level; b.k = dsk_bg_halfwidth(c->theta, c->bg_level);
+        b.lb = c->bg_level; b.k = dsk_bg_halfwidth(c->theta, c->bg_level, c->img_ws);
         b.ntop = c->ntop; b.ncell = c->hstate->ncell;
         b.topgeo = c->topgeo; b.gcell = c->gcell; b.hotkey = c->hotkey;
         b.left_len = c->g_left_len; b.left_off = c->g_left_off; b.left_base = left_base;
@@ -425,7 +438,7 @@ int dsk_run_walk(dsk_ctx *c)
         const uint32_t cm = tiny ? 64u : (uint32_t)(cap_m > 0xffffff00ull ? 0xffffff00ull : cap_m),
                        cp = tiny ? 8u : (uint32_t)(cap_p > 0xffffff00ull ? 0xffffff00ull : cap_p),
                        cl = (uint32_t)(cap_l > 0xffffff00ull ? 0xffffff00ull : cap_l);
-        k_walk<2><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic, c->box, c->cell, c->wmac, c->gbox, c->gcount,
+        k_walk<2><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, c->cell, c->wmac, c->gbox, c->gcount,
                                                          c->g_m2p_len, c->g_p2p_len, c->g_p2p_src, nullptr, nullptr, 0, 0,
                                                          c->list_m2p, c->list_p2p, c->gact_cur, cm, cp, c->g_m2p_off,
                                                          c->g_p2p_off, make_walk_bg(c, 0, cl), c->dstate);
@@ -436,7 +449,7 @@ int dsk_run_walk(dsk_ctx *c)
         if (!ovf) { c->walk_onepass = 1; return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA; }
         c->onepass_bad_theta = c->theta;
     }
-    k_walk<0><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic, c->box, c->cell, c->wmac,
+    k_walk<0><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, c->cell, c->wmac,
                                                      c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len,
                                                      c->g_p2p_src, nullptr, nullptr, 0, 0, nullptr, nullptr,
                                                      c->gact_cur, 0, 0, nullptr, nullptr, make_walk_bg(c, 0, 0), c->dstate);
@@ -450,7 +463,7 @@ int dsk_run_walk(dsk_ctx *c)
 int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base, uint64_t left_base)
 {
     k_walk<1><<<(g1 - g0 + WW - 1) / WW, WW * 32, 0, c->stream>>>(
-        g0, g1, c->periodic, c->box, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len,
+        g0, g1, c->periodic ? c->img_ws : 0, c->box, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len,
         c->g_p2p_len, c->g_p2p_src, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p,
         c->gact_cur, 0, 0, nullptr, nullptr, make_walk_bg(c, left_base, 0), c->dstate);
     DSK_COUNT(c, 1);

@@ -45,10 +45,12 @@ def compute():
     a, ph = oracle.direct_iso(pos, mass, 0.05)
     out["direct"] = {"acc": a.tolist(), "pot": ph.tolist()}
     tp = oracle.OracleTree(pos, mass, 1.0, True, 4, 8)
-    a = oracle.tree_force(pos, mass, 1.0, True, 0.05, 0.5, 4, tree=tp, bg=False)[0]
+    a = oracle.tree_force(pos, mass, 1.0, True, 0.05, 0.5, 4, tree=tp, ws=2, bg=False)[0]
     out["periodic_tree_p4_acc"] = a.tolist()                      # without background subtraction (the round-1 definition)
-    a = oracle.tree_force(pos, mass, 1.0, True, 0.05, 0.5, 4, tree=tp, bg=True)[0]
-    out["periodic_tree_p4_bg_acc"] = a.tolist()                   # reading O4b, the default
+    a = oracle.tree_force(pos, mass, 1.0, True, 0.05, 0.5, 4, tree=tp, ws=2, bg=True)[0]
+    out["periodic_tree_p4_bg_acc"] = a.tolist()                   # reading O4b
+    a = oracle.tree_force(pos, mass, 1.0, True, 0.05, 0.5, 4, tree=tp, ws=1, bg=True)[0]
+    out["periodic_tree_p4_bg_ws1_acc"] = a.tolist()               # the defaults: subtraction on, 27 images
     out["kdk_factors_eds"] = list(oracle.kdk_factors(True, 1.0, 1.0, 0.5, 0.01))
     out["kdk_factors_lcdm"] = list(oracle.kdk_factors(True, 1.0, 1.0, 0.5, 0.01, (0.295, 0.705)))
     return out

@@ -160,7 +160,8 @@ def test_bg_everything_direct_equals_ewald(orc, case):
     """theta -> 0: nothing is accepted, every leaf and every empty octant of the image block is an exposed cube, the window
     and the cubes kept outside it tile the block; what is left is the direct sum over the block's particles, the exact
     background of the block and the order-8 far field of the NEUTRAL box.  Must equal the Ewald direct sum D-per up to the
-    far-field truncation, which subtraction makes ~10x smaller than without (3.9e-6 -> 3.4e-7 on the 16^3 lattice)."""
+    far-field truncation, which subtraction makes ~10x smaller than without (WS = 2: 3.9e-6 -> 3.4e-7 on the 16^3 lattice;
+    WS = 1: 2.5e-3 -> 1.9e-4)."""
     if case == "lattice":
         pos, mass = workloads.perturbed_lattice(16, cfg=3)
         tol = 1e-6
@@ -173,14 +174,18 @@ def test_bg_everything_direct_equals_ewald(orc, case):
     n = len(pos)
     eps = 1.0 / 640
     sink = np.arange(0, n, max(1, n // 48))
-    ref, refp = orc.direct_per(pos, mass, 1.0, eps, sink)
-    acc, pot, _, nm, _ = orc.tree_force(pos, mass, 1.0, True, eps, 1e-6, 4, sink, bg=True)
+    ref, refp = orc.direct_per(pos, mass, 1.0, eps, sink, ws=2)
+    acc, pot, _, nm, _ = orc.tree_force(pos, mass, 1.0, True, eps, 1e-6, 4, sink, ws=2, bg=True)
     assert nm == 0
     assert _erms(acc, ref) < tol, _erms(acc, ref)
     assert np.max(np.abs(pot - refp)) < 10 * tol * np.abs(refp).max()
     if case == "lattice":
-        plain = orc.tree_force(pos, mass, 1.0, True, eps, 1e-6, 4, sink, bg=False)[0]
+        plain = orc.tree_force(pos, mass, 1.0, True, eps, 1e-6, 4, sink, ws=2, bg=False)[0]
         assert _erms(acc, ref) < 0.3 * _erms(plain, ref)
+    # WS = 1 (the default): the same identity, with the larger far-field floor that goes with the smaller block
+    ref1 = orc.direct_per(pos, mass, 1.0, eps, sink, ws=1)[0]
+    acc1 = orc.tree_force(pos, mass, 1.0, True, eps, 1e-6, 4, sink, ws=1, bg=True)[0]
+    assert _erms(acc1, ref1) < {"lattice": 5e-4, "clumpy": 2e-5, "three": 1e-3}[case], _erms(acc1, ref1)   # measured 3.1e-4, <2e-5, 3.6e-4
 
 
 @pytest.mark.parametrize("case", ["lattice", "clustered", "clumpy"])

@@ -27,6 +27,7 @@ def test_oracle_matches_frozen_output():
     assert np.allclose(now["direct"]["acc"], ref["direct"]["acc"], rtol=1e-13, atol=1e-15)
     assert np.allclose(now["periodic_tree_p4_acc"], ref["periodic_tree_p4_acc"], rtol=1e-10, atol=1e-12)
     assert np.allclose(now["periodic_tree_p4_bg_acc"], ref["periodic_tree_p4_bg_acc"], rtol=1e-10, atol=1e-12)
+    assert np.allclose(now["periodic_tree_p4_bg_ws1_acc"], ref["periodic_tree_p4_bg_ws1_acc"], rtol=1e-10, atol=1e-12)
     # the two periodic definitions approximate the same Ewald field: they agree to the tree error of this tiny, clumpy case
     a0, a1 = np.array(ref["periodic_tree_p4_acc"]), np.array(ref["periodic_tree_p4_bg_acc"])
     assert np.linalg.norm(a1 - a0) < 5e-3 * np.linalg.norm(a0)

@@ -183,10 +183,10 @@ def test_tree_force_periodic_vs_ewald(orc):
     pos, mass = workloads.perturbed_lattice(12, cfg=3)
     eps = 1.0 / (40 * 12)
     sink = workloads.subsample(3, len(pos), 64)
-    ref, refp = orc.direct_per(pos, mass, 1.0, eps, sink)
+    ref, refp = orc.direct_per(pos, mass, 1.0, eps, sink, ws=2)
     e = {}
     for theta, p in ((1e-6, 4), (0.5, 4), (0.5, 8)):
-        acc, pot, _, _, _ = orc.tree_force(pos, mass, 1.0, True, eps, theta, p, sink)
+        acc, pot, _, _, _ = orc.tree_force(pos, mass, 1.0, True, eps, theta, p, sink, ws=2)
         e[(theta, p)] = math.sqrt(((acc - ref) ** 2).sum() / (ref ** 2).sum())
         assert np.max(np.abs(pot - refp)) < 5e-3 * np.abs(refp).max()
     assert e[(1e-6, 4)] < 2e-5            # only the WS=2 / order-8 far-field truncation remains
