@@ -373,13 +373,14 @@ def measure_config(cfgid, steps, warmup, dev, world, rank, dist, want_e2e, want_
 def probe_peak():
     """dsk_probe_fp32_peak, all three operand forms (include/dsk.h): the measured FP32 denominator."""
     from paper_1407_2600_b200 import dsk
-    forms = ("ffma2_three_packed_operands", "ffma2_one_scalar_broadcast_operand", "scalar_ffma_three_registers")
+    forms = ("ffma2_three_packed_operands", "ffma2_one_scalar_broadcast_operand", "scalar_ffma_three_registers",
+             "ffma2_sources_repeated", "scalar_ffma_sources_repeated")
     res = {}
     for v, name in enumerate(forms):
         t, c, m, tc = dsk.probe_fp32_peak_ex(v)
         res[name] = {"TFLOPs": round(t, 3), "TFLOPs_by_sm_cycle_counters": round(tc, 3),
                      "cycles_per_warp_inst_per_smsp": round(c, 4), "sm_mhz": round(m, 1)}
-    res["tflops"] = max(res[forms[0]]["TFLOPs"], res[forms[1]]["TFLOPs"])
+    res["tflops"] = max(res[f]["TFLOPs"] for f in forms)
     return res
 
 

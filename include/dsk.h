@@ -191,7 +191,9 @@ int dsk_get_lattice_tensors(dsk_ctx *ctx, double *T /* host [165] */);
  * device memory) and writes to HOST pointers: TFLOP/s (FMA = 2 flop per lane), cycles per warp instruction per SM
  * sub-partition, and the SM clock in MHz the kernel ran at.  variant 0: packed fma.rn.f32x2 with three register operands;
  * 1: packed, one operand a scalar broadcast to both halves (the form the force kernels feed sources in); 2: scalar FFMA
- * with three distinct registers.  DSK_EINVAL for another variant or a NULL pointer, DSK_ECUDA without a device. */
+ * with three distinct registers; 3 and 4: packed and scalar with the two source operands repeated from one instruction to
+ * the next (operand-reuse cache; 0-2 are register-bandwidth bound).  DSK_EINVAL for another variant or a NULL pointer,
+ * DSK_ECUDA without a device. */
 int dsk_probe_fp32_peak(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz);
 /* the same, plus TFLOP/s as implied by the SMs' own cycle counters and clock (cross-check of the event timing) */
 int dsk_probe_fp32_peak_ex(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz, double *tflops_by_cycles);

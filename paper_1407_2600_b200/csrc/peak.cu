@@ -5,6 +5,11 @@
 //   variant 0  FFMA2, three packed register operands                  a = fma(x, y, a)     x, y, a: 64-bit register pairs
 //   variant 1  FFMA2, one operand a scalar broadcast to both halves   a = fma(a, {s,s}, y) the form M2P/P2P feed sources in
 //   variant 2  scalar FFMA, three distinct registers                  a = fma(x, y, a)
+//   variant 3  FFMA2, the two source operands shared by all chains    a_k = fma(a_k, {s,s}, y)   (operand-reuse cache hits)
+//   variant 4  scalar FFMA, the two source operands shared            a_k = fma(a_k, s, y)
+// Variants 0-2 read five or six, three distinct registers per instruction and are bound by register-file bandwidth (measured:
+// one FFMA2 per 2.6 - 3.0 cycles, one FFMA per 1.5); 3 and 4 show what the pipe itself issues when operands repeat, which is
+// what a real inner loop (one coefficient against many monomials) looks like.
 // Reported: TFLOP/s (2 flop per lane and FMA) from CUDA events, cycles per warp instruction per SM sub-partition from
 // clock64() inside the kernel, and the SM clock the kernel ran at (clock64 cycles over globaltimer nanoseconds).
 #include "dsk_internal.cuh"
@@ -30,7 +35,19 @@ __global__ void __launch_bounds__(PK_THREADS, PK_BLOCKS_PER_SM) k_fp32_peak(int 
     const unsigned long long t0 = pk_globaltimer();
     const long long c0 = clock64();
     float res = 0.0f;
-    if (VARIANT == 2) {
+    if (VARIANT == 4) {
+        float a[PK_CHAINS];
+        const float x = s1 + 1e-3f * (float)threadIdx.x, y = s0 * 0.5f;
+#pragma unroll
+        for (int k = 0; k < PK_CHAINS; k++) a[k] = s0 + (float)k;
+        for (int it = 0; it < iters; it++)
+#pragma unroll
+            for (int u = 0; u < PK_UNROLL; u++)
+#pragma unroll
+                for (int k = 0; k < PK_CHAINS; k++) a[k] = fmaf(a[k], x, y);
+#pragma unroll
+        for (int k = 0; k < PK_CHAINS; k++) res += a[k];
+    } else if (VARIANT == 2) {
         float a[PK_CHAINS], x[PK_CHAINS], y[PK_CHAINS];
 #pragma unroll
         for (int k = 0; k < PK_CHAINS; k++) { a[k] = s0 + (float)k; x[k] = s1 + 1e-3f * (float)(k + threadIdx.x); y[k] = s0 * 0.5f + 1e-3f * (float)k; }
@@ -58,7 +75,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_BLOCKS_PER_SM) k_fp32_peak(int 
 #pragma unroll
                 for (int k = 0; k < PK_CHAINS; k++) {
                     if (VARIANT == 0) a[k] = f2_fma(x[k], y[k], a[k]);
-                    else a[k] = f2_fma(a[k], f2_dup(sc[k]), y[k]);
+                    else if (VARIANT == 1) a[k] = f2_fma(a[k], f2_dup(sc[k]), y[k]);
+                    else a[k] = f2_fma(a[k], f2_dup(sc[0]), y[0]);
                 }
 #pragma unroll
         for (int k = 0; k < PK_CHAINS; k++) res += f2_lo(a[k]) + f2_hi(a[k]);
@@ -83,7 +101,7 @@ extern "C" int dsk_probe_fp32_peak_ex(int variant, double *tflops, double *cycle
 }
 static int probe_impl(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz, double *tflops_by_cycles)
 {
-    if (variant < 0 || variant > 2 || !tflops || !cycles_per_inst_smsp || !sm_mhz) return DSK_EINVAL;
+    if (variant < 0 || variant > 4 || !tflops || !cycles_per_inst_smsp || !sm_mhz) return DSK_EINVAL;
     int dev = 0, nsm = 0;
     DSK_CUDA(cudaGetDevice(&dev));
     DSK_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
@@ -103,7 +121,9 @@ static int probe_impl(int variant, double *tflops, double *cycles_per_inst_smsp,
         cudaEventRecord(e0);
         if (variant == 0) k_fp32_peak<0><<<grid, PK_THREADS>>>(iters, seed, out, clk);
         else if (variant == 1) k_fp32_peak<1><<<grid, PK_THREADS>>>(iters, seed, out, clk);
-        else k_fp32_peak<2><<<grid, PK_THREADS>>>(iters, seed, out, clk);
+        else if (variant == 2) k_fp32_peak<2><<<grid, PK_THREADS>>>(iters, seed, out, clk);
+        else if (variant == 3) k_fp32_peak<3><<<grid, PK_THREADS>>>(iters, seed, out, clk);
+        else k_fp32_peak<4><<<grid, PK_THREADS>>>(iters, seed, out, clk);
         cudaEventRecord(e1);
         if (cudaEventSynchronize(e1) != cudaSuccess) break;
         float ms = 0.0f;
@@ -119,7 +139,7 @@ static int probe_impl(int variant, double *tflops, double *cycles_per_inst_smsp,
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     if (err != cudaSuccess || cudaGetLastError() != cudaSuccess || best > 1e29f) return DSK_ECUDA;
     const double inst_per_thread = (double)iters * PK_UNROLL * PK_CHAINS;
-    const double lanes = variant == 2 ? 1.0 : 2.0;
+    const double lanes = (variant == 2 || variant == 4) ? 1.0 : 2.0;
     *tflops = inst_per_thread * 2.0 * lanes * (double)grid * PK_THREADS / ((double)best * 1e-3) / 1e12;
     if (tflops_by_cycles) {      // the same from the SMs' own cycle counters: flop per block / (its cycles / its clock), all blocks at once
         const double sec = (cyc / grid) / (cyc / ns * 1e9);
