@@ -120,6 +120,14 @@ int dsk_kdk_reset(dsk_ctx *ctx);
  * background in the far field alone (and fp64 monopoles).
  * DSK_EINVAL for on != 0 in an isolated context.  Changing it invalidates moments, lists and the cached KDK force. */
 int dsk_set_background(dsk_ctx *ctx, int on);
+/* Acceptance rule of the walk.  kind 0 (default): the opening angle of dsk_create / dsk_set_params, accept iff
+ * d^2 > (s/theta + delta)^2.  kind 1: an ABSOLUTE ERROR BOUND per cell interaction ("We adjust the error tolerance
+ * parameter to limit absolute errors ..."; reading O5b of DESIGN.md): accept iff d^2 > (s + delta)^2 and
+ *     (p + 2) Q b^(p-1) / (d^(p+1) (d - b)^2) <= tol,
+ * Q = sum m |y - z|^2 over the cell (plus rho_bar times the cube's for a background-subtracted copy), b = sqrt(3)/2 s + delta,
+ * d the distance from the cell's expansion centre to the sink group's box; tol > 0 in units of acceleration (G = 1).
+ * theta still sets the window of background subtraction.  DSK_EINVAL for another kind or tol <= 0 with kind 1. */
+int dsk_set_mac(dsk_ctx *ctx, int kind, float tol);
 /* Half-width WS of the block of periodic images that is summed explicitly by the tree, (2 WS + 1)^3 images; everything
  * beyond it is the order-8 far field (reading O7 of DESIGN.md: "WS is measured, not assumed").  ws = 1 or 2;
  * 1 is the default (dsk_get_param "WS"), 2 the largest the library supports ("WS_MAX").  With background subtraction the far

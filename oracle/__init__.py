@@ -177,6 +177,15 @@ class OracleTree:
         lib().orc_moments_m2m(self._h, C.c_int(p), _p(out))
         return out
 
+    def set_mac(self, kind="theta", tol=0.0):
+        """acceptance rule of the walks that follow: "theta" (opening angle, O5) or "abs" (error bound <= tol per cell, O5b)"""
+        lib().orc_tree_set_mac(self._h, C.c_int(0 if kind == "theta" else 1), C.c_double(tol))
+
+    def mac_bound(self, c, d, sub=False):
+        f = lib().orc_mac_bound
+        f.restype = C.c_double
+        return float(f(self._h, C.c_int64(c), C.c_int(int(sub)), C.c_double(d)))
+
     def moments_bg(self, p):
         """O4b: (l_b, rho_bar, M'[ntop, NP(p)]) — the moments of particles - rho_bar over the cube of every cell of level <= l_b"""
         if self.p != p:
@@ -240,11 +249,14 @@ def image_shift(img, box, periodic, ws=WS):
     return box * np.array([img // (side * side) - ws, (img // side) % side - ws, img % side - ws], dtype=np.float64)
 
 
-def tree_force(pos, mass, box, periodic, eps, theta, p, sink=None, tree=None, ws=WS, bg=None):
+def tree_force(pos, mass, box, periodic, eps, theta, p, sink=None, tree=None, ws=WS, bg=None, mac=None):
     """The whole oracle path Tr: tree sum over the image block (+ O7 far field when periodic).
-    bg: background subtraction (reading O4b) in a periodic box.  Returns acc, pot, n_p2p, n_m2p, tree."""
+    bg: background subtraction (reading O4b) in a periodic box; mac: ("theta",) or ("abs", tol) sets the tree's acceptance
+    rule (it stays set).  Returns acc, pot, n_p2p, n_m2p, tree."""
     if tree is None:
         tree = OracleTree(pos, mass, box, periodic)
+    if mac is not None:
+        tree.set_mac(*mac)
     bg = (BG_DEFAULT if bg is None else bg) and bool(periodic)
     acc, pot, n_p2p, n_m2p = tree.accel(eps, theta, p, sink, ws, bg=bg)
     if periodic:

@@ -54,6 +54,9 @@ typedef struct orc_tree {
     int64_t ntop;          /* cells of level <= l_b: the first ntop cells (level-major)     */
     double rhobar;         /* M_tot / box^3                                                 */
     double *mom_bg;        /* [ntop, NP(p)] moments of particles - rho_bar over the cube    */
+    /* O5b acceptance rule in use (orc_tree_set_mac): 0 opening angle, 1 absolute error bound   */
+    int mac_kind;
+    double mac_tol;
 } orc_tree;
 
 /* multi-index helpers (orc_tree.c) */
@@ -88,6 +91,8 @@ void orc_group_lists(orc_tree *t, double theta, int ws, int bg, int64_t g, int64
                      int32_t *m2p_img, int8_t *m2p_sub, int64_t *n_m2p, int64_t *p2p_cell, int32_t *p2p_img,
                      int64_t *n_p2p, int64_t *left_lohi, int64_t *n_left, int64_t window[6]);
 void orc_cell_coords(const orc_tree *t, int64_t c, int64_t q[3]);
+void orc_tree_set_mac(orc_tree *t, int kind, double tol);
+double orc_mac_bound(const orc_tree *t, int64_t c, int sub, double d);
 
 /* background subtraction, reading O4b (orc_bg.c) */
 void orc_cuboid_field(const double lo[3], const double hi[3], const double x[3], double *I, double g[3]);

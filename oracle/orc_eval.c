@@ -137,6 +137,30 @@ static void expose(walk_t *w, const int64_t lo[3], const int64_t hi[3])
     q->n++;
 }
 
+/* O5b (reading; "We adjust the error tolerance parameter to limit absolute errors ..."): an upper bound on the
+ * acceleration error of the order-p expansion of cell c at distance d from its expansion centre z,
+ *     E_c(d) = (p + 2) B_{p+1} / (d^(p+1) (d - b)^2),     d > b,
+ * b = (sqrt(3)/2) s + delta  the radius of the ball about z that holds the cell's cube, B_{p+1} = sum m |y - z|^(p+1) bounded by
+ * Q b^(p-1), Q = sum m |y - z|^2 = M_200 + M_020 + M_002 (an exact moment).  It follows from |grad (P_n(cos g)/r^(n+1))| ~ (n+1)/r^(n+2):
+ * sum_{n>p} (n+1) B_n / d^(n+2) <= B_{p+1}/d^(p+3) sum_k (p+2+k)(b/d)^k <= (p+2) B_{p+1}/(d^(p+1)(d-b)^2)   (Salmon & Warren 1994's form).
+ * sub: the cell is listed with background-subtracted moments (O4b): the sources are |particles| + |rho_bar cube|,
+ * Q' = Q + rho_bar tr C = 2 Q - tr M'. */
+double orc_mac_bound(const orc_tree *t, int64_t c, int sub, double d)
+{
+    const int p = t->p, np = ORC_NP(p);
+    const double s = (double)t->box * ldexp(1.0, -t->level[c]), b = 0.5 * sqrt(3.0) * s + t->delta[c];
+    const double *M = t->mom + (size_t)np * c;
+    double Q = M[orc_midx(2, 0, 0)] + M[orc_midx(0, 2, 0)] + M[orc_midx(0, 0, 2)];
+    if (sub) {
+        const double *Mb = t->mom_bg + (size_t)np * c;
+        Q = 2.0 * Q - (Mb[orc_midx(2, 0, 0)] + Mb[orc_midx(0, 2, 0)] + Mb[orc_midx(0, 0, 2)]);
+    }
+    if (!(d > b)) return INFINITY;
+    return (p + 2) * Q * pow(b, p - 1) / (pow(d, p + 1) * (d - b) * (d - b));
+}
+
+void orc_tree_set_mac(orc_tree *t, int kind, double tol) { t->mac_kind = kind; t->mac_tol = tol; }
+
 static void walk_rec(walk_t *w, int64_t c)
 {
     const orc_tree *t = w->t;
@@ -168,7 +192,13 @@ static void walk_rec(walk_t *w, int64_t c)
     /* a cell that sticks out of the window (partly in, partly out) is never accepted: its cube's background would be
      * counted twice inside the window */
     const int straddles = top && inter && !inside;
-    if (!straddles && d2 > rc * rc) {                                   /* accept (strict)    */
+    int ok;
+    if (t->mac_kind == 0) ok = d2 > rc * rc;                            /* opening angle (strict) */
+    else {                                                              /* O5b: theta = 1 for validity, then the error bound */
+        double r1 = s + t->delta[c];
+        ok = d2 > r1 * r1 && orc_mac_bound(t, c, top && !inter, sqrt(d2)) <= t->mac_tol;
+    }
+    if (!straddles && ok) {                                             /* accept             */
         il_push(w->m2p, c, w->im, (int8_t)(top && !inter));              /* outside the window: background subtracted */
         return;
     }

@@ -55,6 +55,7 @@ static size_t carve(dsk_ctx *c, char *base)
     c->frows = (float *)take(4 * (size_t)dsk_frow_len(c->p_cap, c->periodic) * (nc + nt));
     c->topgeo = (int4 *)take(16 * nt);
     c->mass64 = (double *)take(8 * nt);
+    c->kbg = (float *)take(4 * nt);
     c->rows_bg = (float *)take(4 * (size_t)dsk_rowlen(c->p_cap) * nt);
     c->g_left_len = (uint32_t *)take(4 * (c->periodic ? ng : 0));
     c->g_left_off = (uint64_t *)take(8 * (c->periodic ? ng + 1 : 0));
@@ -359,6 +360,15 @@ extern "C" int dsk_set_cosmology(dsk_ctx *c, double omega_m, double omega_lambda
     if (!c) return DSK_EINVAL;
     if (!(omega_m > 0.0) || !isfinite(omega_m) || !isfinite(omega_lambda)) return DSK_EINVAL;
     c->omega_m = omega_m; c->omega_l = omega_lambda;
+    return DSK_OK;
+}
+
+extern "C" int dsk_set_mac(dsk_ctx *c, int kind, float tol)
+{
+    if (!c || (kind != 0 && kind != 1)) return DSK_EINVAL;
+    if (kind == 1 && (!(tol > 0.0f) || !isfinite(tol))) return DSK_EINVAL;
+    c->mac_kind = kind; c->mac_tol = kind == 1 ? tol : 0.0f;
+    c->lists_valid = 0; c->kdk_have_acc = 0;
     return DSK_OK;
 }
 

@@ -164,6 +164,7 @@ struct dsk_ctx {
     int64_t ntop_cap;
     int4 *topgeo;             // [ntop_cap] integer coordinates, level | child octant mask << 8
     double *mass64;           // [ntop_cap] fp64 masses
+    float *kbg;               // [ntop_cap] error-bound constants of the subtracted copies (absolute-error MAC, walk.cu)
     float *rows_bg;           // [ntop_cap * rowlen(p_cap)] subtracted moment rows (their force rows are frows[ncell ..])
     uint32_t *g_left_len;     // [ngroup_cap] cubes kept outside the window, per group (the walk's third list)
     uint64_t *g_left_off;     // [ngroup_cap + 1]
@@ -188,6 +189,8 @@ struct dsk_ctx {
     int frow_tab_dip;         // and whether it has the dipole block
     int frow_dip;             // layout of the force rows in memory: dipole block present (periodic with subtraction)
     uint32_t m2m_tab_mask;    // orders whose M2M pair table this context has uploaded (bit p/2 - 1)
+    int mac_kind;             // 0 opening angle, 1 absolute error bound (dsk_set_mac)
+    float mac_tol;
     float lists_theta;
     int walk_two_pass_only;   // dsk_set_walk_mode(1)
     int walk_onepass;         // the lists of the current evaluation were written by the one-pass walk

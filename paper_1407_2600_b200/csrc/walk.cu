@@ -44,6 +44,7 @@ struct walk_bg {
     uint4 *list_left;
     uint32_t cap_l;                // ONE pass: fixed capacity per group
     uint64_t *left_off_out;
+    const float *kbg;              // [ntop] error-bound constant of the subtracted copies (absolute-error MAC)
 };
 
 __device__ __forceinline__ uint32_t wk_compact3(uint64_t x)
@@ -100,8 +101,12 @@ __device__ __forceinline__ uint32_t wk_exposed(bool whole, int lvl, int lb, cons
     return n;
 }
 
-template <int MODE>          // 0 COUNT, 1 FILL at the scanned offsets, 2 ONE pass into a fixed capacity per group
-__global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int periodic, float box,
+// ABS: the absolute-error acceptance rule (reading O5b of DESIGN.md) instead of the opening angle: accept iff
+//   d^2 > (s + delta)^2   (theta = 1: the expansion converges)   and   (d/b)^(p+1) (d - b)^2 >= kappa_c,
+// b = sqrt(3)/2 s + delta, kappa_c = (p + 2) Q_c / (tol b^2), i.e. E_c(d) = (p+2) Q b^(p-1) / (d^(p+1) (d-b)^2) <= tol.
+// The MAC record then holds s + delta in .w and kappa_c in the slot of `first` (which the walk does not use).
+template <int MODE, bool ABS>          // MODE 0 COUNT, 1 FILL at the scanned offsets, 2 ONE pass into a fixed capacity per group
+__global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int periodic, float box, int pow1,
                                                   const dsk_cellrec *__restrict__ cell,
                                                   const float4 *__restrict__ wmac,
                                                   const float4 *__restrict__ gbox,
@@ -234,7 +239,16 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
                     straddles = inter && !inside;      // partly inside the window: never accepted (its background would count twice)
                     if (!inter) entry = (e[q] & ~CELL_MASK) | (bg.ncell + c);      // outside: the background-subtracted copy
                 }
-                accept[q] = !straddles && d2 > h[q].w * h[q].w;
+                bool ok = d2 > h[q].w * h[q].w;
+                if (ABS && ok) {
+                    const float s = box * exp2f(-(float)((__float_as_uint(rr[q].w) >> 8) & 255u));
+                    const float b = h[q].w - 0.1339746f * s, d = sqrtf(d2), x = d / b;
+                    float xp = x;
+                    for (int k = 1; k < pow1; k++) xp *= x;
+                    const float kappa = (top && entry != e[q]) ? bg.kbg[c] : rr[q].x;      // the subtracted copy has its own bound
+                    ok = xp * (d - b) * (d - b) >= kappa;
+                }
+                accept[q] = !straddles && ok;
                 if (!accept[q]) {
                     nchild[q] = __float_as_uint(rr[q].w) & 255u; child0[q] = __float_as_uint(rr[q].z); cnt = __float_as_uint(rr[q].y);
                     leaf[q] = nchild[q] == 0;
@@ -380,23 +394,37 @@ static void scan64(dsk_ctx *c, const uint32_t *len, uint32_t n, uint64_t *off)
     DSK_COUNT(c, 2);
 }
 
-// the 32 bytes the walk reads per tested cell: centre of mass and critical radius s/theta + delta | the cell record
-__global__ void __launch_bounds__(256) k_walk_mac(uint32_t ncell, float box, float inv_theta,
+// the 32 bytes the walk reads per tested cell: centre of mass and critical radius s/theta + delta | the cell record.
+// abs_tol > 0 (absolute-error MAC): critical radius s + delta, and kappa_c = (p + 2) Q_c / (tol b_c^2) in the slot of `first`;
+// kbg[c] = the same for the background-subtracted copy of a top cell, Q' = Q + rho_bar tr C = 2 Q - tr M'.
+__global__ void __launch_bounds__(256) k_walk_mac(uint32_t ncell, float box, float inv_theta, float abs_tol, int p, int rowlen,
+                                                  const float *__restrict__ rows, uint32_t ntop, const float *__restrict__ rows_bg,
                                                   const dsk_cellrec *__restrict__ cell, const float4 *__restrict__ whdr,
-                                                  float4 *__restrict__ wmac)
+                                                  float4 *__restrict__ wmac, float *__restrict__ kbg)
 {
     const uint32_t c = blockIdx.x * 256 + threadIdx.x;
     if (c >= ncell) return;
     float4 h = whdr[c];
     const int level = (int)(cell[c].meta >> 8);
-    const float s = box * exp2f((float)-level);
-    h.w = s * inv_theta + h.w;
+    const float s = box * exp2f((float)-level), delta = h.w;
+    h.w = s * inv_theta + delta;
     wmac[2 * (size_t)c] = h;
     // the cell record rides in the same 32-byte sector: a rejected cell needs it, and a second, dependent load would
     // double the latency of every walk iteration
     const dsk_cellrec r = cell[c];
-    wmac[2 * (size_t)c + 1] = make_float4(__uint_as_float(r.first), __uint_as_float(r.count), __uint_as_float(r.child0),
-                                          __uint_as_float(r.meta));
+    float4 rec = make_float4(__uint_as_float(r.first), __uint_as_float(r.count), __uint_as_float(r.child0), __uint_as_float(r.meta));
+    if (abs_tol > 0.0f) {
+        const float *row = rows + (size_t)c * rowlen;
+        const float tr = row[8 + dsk_midx(2, 0, 0)] + row[8 + dsk_midx(0, 2, 0)] + row[8 + dsk_midx(0, 0, 2)];   // sum Mhat_2 = Q / (2 s^2)
+        const float bs = 0.8660254f + delta / s;                                                         // b / s
+        rec.x = (float)(p + 2) * 2.0f * tr / (abs_tol * bs * bs);
+        if (c < ntop && kbg) {
+            const float *rb = rows_bg + (size_t)c * rowlen;
+            const float trb = rb[8 + dsk_midx(2, 0, 0)] + rb[8 + dsk_midx(0, 2, 0)] + rb[8 + dsk_midx(0, 0, 2)];
+            kbg[c] = (float)(p + 2) * 2.0f * (2.0f * tr - trb) / (abs_tol * bs * bs);
+        }
+    }
+    wmac[2 * (size_t)c + 1] = rec;
 }
 
 static walk_bg make_walk_bg(dsk_ctx *c, uint64_t left_base, uint32_t cap_l)
@@ -410,6 +438,7 @@ static walk_bg make_walk_bg(dsk_ctx *c, uint64_t left_base, uint32_t cap_l)
         b.topgeo = c->topgeo; b.gcell = c->gcell; b.hotkey = c->hotkey;
         b.left_len = c->g_left_len; b.left_off = c->g_left_off; b.left_base = left_base;
         b.list_left = c->list_left; b.cap_l = cap_l; b.left_off_out = c->g_left_off;
+        b.kbg = c->kbg;
     }
     return b;
 }
@@ -422,9 +451,12 @@ int dsk_run_walk(dsk_ctx *c)
     const uint32_t ng = c->hstate->ngroup;
     cudaStream_t s = c->stream;
     const float inv_theta = 1.0f / c->theta;
+    const int pow1 = c->p + 1;
     cudaEventRecord(c->ev[7], s);
     const uint32_t nc = c->hstate->ncell;
-    k_walk_mac<<<(nc + 255) / 256, 256, 0, s>>>(nc, c->box, inv_theta, c->cell, c->whdr, c->wmac);
+    const bool ABS = c->mac_kind == 1;
+    k_walk_mac<<<(nc + 255) / 256, 256, 0, s>>>(nc, c->box, ABS ? 1.0f : inv_theta, ABS ? c->mac_tol : 0.0f, c->p, dsk_rowlen(c->p), c->rows,
+                                                c->periodic && c->bg ? c->ntop : 0u, c->rows_bg, c->cell, c->whdr, c->wmac, c->kbg);
     DSK_COUNT(c, 1);
     c->walk_onepass = 0;
     const bool BG = c->periodic && c->bg;
@@ -438,7 +470,7 @@ int dsk_run_walk(dsk_ctx *c)
         const uint32_t cm = tiny ? 64u : (uint32_t)(cap_m > 0xffffff00ull ? 0xffffff00ull : cap_m),
                        cp = tiny ? 8u : (uint32_t)(cap_p > 0xffffff00ull ? 0xffffff00ull : cap_p),
                        cl = (uint32_t)(cap_l > 0xffffff00ull ? 0xffffff00ull : cap_l);
-        k_walk<2><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, c->cell, c->wmac, c->gbox, c->gcount,
+        (ABS ? k_walk<2, true> : k_walk<2, false>)<<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, pow1, c->cell, c->wmac, c->gbox, c->gcount,
                                                          c->g_m2p_len, c->g_p2p_len, c->g_p2p_src, nullptr, nullptr, 0, 0,
                                                          c->list_m2p, c->list_p2p, c->gact_cur, cm, cp, c->g_m2p_off,
                                                          c->g_p2p_off, make_walk_bg(c, 0, cl), c->dstate);
@@ -449,7 +481,7 @@ int dsk_run_walk(dsk_ctx *c)
         if (!ovf) { c->walk_onepass = 1; return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA; }
         c->onepass_bad_theta = c->theta;
     }
-    k_walk<0><<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, c->cell, c->wmac,
+    (ABS ? k_walk<0, true> : k_walk<0, false>)<<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, pow1, c->cell, c->wmac,
                                                      c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len,
                                                      c->g_p2p_src, nullptr, nullptr, 0, 0, nullptr, nullptr,
                                                      c->gact_cur, 0, 0, nullptr, nullptr, make_walk_bg(c, 0, 0), c->dstate);
@@ -462,8 +494,8 @@ int dsk_run_walk(dsk_ctx *c)
 
 int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base, uint64_t left_base)
 {
-    k_walk<1><<<(g1 - g0 + WW - 1) / WW, WW * 32, 0, c->stream>>>(
-        g0, g1, c->periodic ? c->img_ws : 0, c->box, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len,
+    (c->mac_kind == 1 ? k_walk<1, true> : k_walk<1, false>)<<<(g1 - g0 + WW - 1) / WW, WW * 32, 0, c->stream>>>(
+        g0, g1, c->periodic ? c->img_ws : 0, c->box, c->p + 1, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len,
         c->g_p2p_len, c->g_p2p_src, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p,
         c->gact_cur, 0, 0, nullptr, nullptr, make_walk_bg(c, left_base, 0), c->dstate);
     DSK_COUNT(c, 1);

@@ -751,6 +751,55 @@ def test_image_block_one_and_two(dsk, orc, case):
     d.close()
 
 
+# ---- absolute-error acceptance rule (reading O5b) ----------------------------------------------------
+@pytest.mark.parametrize("case", ["plummer", "periodic-clustered", "periodic-lattice"])
+def test_abs_mac_parity(dsk, orc, case):
+    """dsk_set_mac(1, tol): forces, potentials and interaction counts against the oracle under the same rule (the rule is
+    evaluated in fp32 here and fp64 there, so a cell within rounding of the threshold may fall either way: both lists are valid);
+    the error against the direct sum falls with tol; invalid arguments are refused; kind 0 restores the opening angle."""
+    if case == "plummer":
+        pos, mass = workloads.make(2, 1 / 16); periodic, eps = False, 1e-4
+    elif case == "periodic-clustered":
+        pos, mass = workloads.clustered_box(24, 20, cfg=4); periodic, eps = True, 1.0 / 960
+    else:
+        pos, mass = workloads.perturbed_lattice(24); periodic, eps = True, 1.0 / 960
+    n = len(pos)
+    sink = workloads.subsample(2, n, 1500)
+    d = dsk.Dsk(n, 1.0, periodic, eps, 0.5, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    ref_theta = d.accel(tp, tm)[0].clone()
+    t = orc.OracleTree(pos, mass, 1.0, periodic)
+    direct = (orc.direct_per(pos, mass, 1.0, eps, sink[:96]) if periodic else orc.direct_iso(pos, mass, eps, sink))[0]
+    arms = float(np.sqrt((direct ** 2).sum(1).mean()))
+    errs = []
+    for rel in (3e-2, 1e-3):
+        tol = rel * arms
+        d.set_mac("abs", tol)
+        acc, pot = d.accel(tp, tm)
+        st = d.get_stats()
+        a = acc.cpu().numpy().astype(np.float64); ph = pot.cpu().numpy().astype(np.float64)
+        ta, tpot, n_p2p, n_m2p, _ = orc.tree_force(pos, mass, 1.0, periodic, eps, 0.5, 4, sink, tree=t, mac=("abs", tol))
+        relerr = np.linalg.norm(a[sink] - ta, axis=1) / np.linalg.norm(ta, axis=1)
+        assert np.quantile(relerr, 0.999) < 1e-4, (rel, np.quantile(relerr, 0.999))
+        assert np.max(np.abs(ph[sink] - tpot)) < 1e-4 * np.abs(tpot).max() + 1e-6
+        m = len(direct)
+        errs.append(_erms(a[sink[:m]], direct))
+        assert errs[-1] <= 1.1 * _erms(ta[:m], direct) + 1e-6
+        full = orc.tree_force(pos, mass, 1.0, periodic, eps, 0.5, 4, None, tree=t)[3] if n <= 20000 else None
+        if full is not None:
+            assert abs(st["n_m2p"] - full) <= 2e-3 * full, (st["n_m2p"], full)
+    assert errs[1] < errs[0]
+    for bad in ((1, 0.0), (1, -1.0), (2, 1.0)):
+        with pytest.raises(dsk.DskError):
+            dsk._check(d.lib.dsk_set_mac(d._h, bad[0], bad[1]))
+    t.set_mac("theta")
+    d.set_mac("theta")
+    again = d.accel(tp, tm)[0]
+    assert torch.equal(again, ref_theta)
+    d.close()
+
+
 # ---- KDK ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("periodic", [False, True])
 def test_kdk_step(dsk, orc, periodic):

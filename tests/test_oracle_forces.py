@@ -345,3 +345,114 @@ def test_lists_hand_built_case(orc):
     # 68 (delta 0, d 0.4375 < 0.5) -> 64 accepted, 68 direct; its own cell 12 and sibling leaf 807 are direct.
     mc, _, pc, _ = t.lists(0.5, 2)
     assert hk(mc) == [64] and hk(pc) == [68, 803, 807]
+
+
+# ---- O5b: the absolute-error acceptance rule ("limit absolute errors ...") ---------------------------------
+@pytest.mark.parametrize("p", [2, 4, 6, 8])
+def test_mac_bound_holds_for_every_cell(orc, p):
+    """E_c(d) = (p+2) Q b^(p-1) / (d^(p+1) (d-b)^2) is an UPPER BOUND: for random cells and random field points at distance
+    d > s + delta from the expansion centre, the error of the order-p expansion against the direct sum over the cell's particles
+    stays below it (and is not absurdly below: the bound is within a few orders of magnitude for compact cells)."""
+    rng = np.random.default_rng(p)
+    pos, mass, t = _lists_case(orc, False)
+    cm, com, dl, mom = t.moments(p)
+    cells = t.cells()
+    _, order = t.sorted()
+    spos = t.wrapped_pos().astype(np.float64)[order]
+    smass = mass.astype(np.float64)[order]
+    side = 2.0 ** (-cells["level"].astype(np.float64))
+    eps2 = 1e-16
+    worst, n = 0.0, 0
+    for c in rng.choice(t.ncell, 400, replace=False):
+        if cells["count"][c] < 2:
+            continue
+        f, k = cells["first"][c], cells["count"][c]
+        for _ in range(5):
+            d = (side[c] + dl[c]) * (1.0 + 3.0 * rng.random() ** 2)
+            u = rng.standard_normal(3); u /= np.linalg.norm(u)
+            x = com[c] + d * u
+            r = x - spos[f:f + k]
+            exact = -(smass[f:f + k, None] * r / ((r * r).sum(1) + eps2)[:, None] ** 1.5).sum(0)
+            approx, _ = orc.m2p(p, mom[c], x - com[c], eps2)
+            err = np.linalg.norm(approx - exact)
+            bound = t.mac_bound(int(c), d)
+            assert err <= bound * (1 + 1e-9) + 1e-13 * np.linalg.norm(exact), (c, d, err, bound)
+            worst = max(worst, err / bound); n += 1
+    assert n > 500 and worst > 1e-4                        # the bound is not vacuous
+
+
+def test_mac_bound_holds_for_subtracted_cells(orc):
+    """the same for the background-subtracted copies (O4b): sources = particles - rho_bar over the cube, exact field = direct sum
+    minus rho_bar times the closed-form cuboid field; Q' = Q + rho_bar tr C in the bound"""
+    rng = np.random.default_rng(9)
+    pos, mass = workloads.clustered_box(20, 10, cfg=4)
+    t = orc.OracleTree(pos, mass, 1.0, True)
+    p = 4
+    cm, com, dl, mom = t.moments(p)
+    lb, rho, mb = t.moments_bg(p)
+    cells = t.cells()
+    _, order = t.sorted()
+    spos = t.wrapped_pos().astype(np.float64)[order]
+    smass = mass.astype(np.float64)[order]
+    n = 0
+    for c in rng.choice(len(mb), min(len(mb), 150), replace=False):
+        lev = int(cells["level"][c]); s = 2.0 ** -lev
+        hot = int(cells["hotkey"][c]) & ~(1 << (3 * lev))
+        q = [sum(((hot >> (3 * b + sh)) & 1) << b for b in range(lev)) for sh in (2, 1, 0)]
+        lo = np.array(q, float) * s; hi = lo + s
+        f, k = cells["first"][c], cells["count"][c]
+        for _ in range(4):
+            d = (s + dl[c]) * (1.0 + 2.0 * rng.random())
+            u = rng.standard_normal(3); u /= np.linalg.norm(u)
+            x = com[c] + d * u
+            r = x - spos[f:f + k]
+            exact = -(smass[f:f + k, None] * r / ((r * r).sum(1) + 1e-16)[:, None] ** 1.5).sum(0) - rho * orc.cuboid_field(lo, hi, x)[1]
+            approx, _ = orc.m2p(p, mb[c], x - com[c], 1e-16)
+            err = np.linalg.norm(approx - exact)
+            assert err <= t.mac_bound(int(c), d, sub=True) * (1 + 1e-9) + 1e-13, (c, d, err)
+            n += 1
+    assert n > 200
+
+
+@pytest.mark.parametrize("periodic", [False, True])
+def test_abs_mac_lists_and_error(orc, periodic):
+    """Lists under the absolute-error rule: the particle partition holds; every accepted entry has d > s + delta and
+    E_c(d_AABB) <= tol, every listed leaf fails one of the two (recomputed from mac_bound and the group's box); and the
+    force error against the direct sum falls with tol."""
+    ws = 1
+    pos, mass, t = _lists_case(orc, periodic)
+    n = len(pos)
+    cm, com, dl, _ = t.moments(4)
+    cells, grp = t.cells(), t.groups()
+    side = 2.0 ** (-cells["level"].astype(np.float64))
+    tol = 5.0
+
+    def d_aabb(bb, z):
+        lo = bb[:3].astype(np.float64) - z; hi = z - bb[3:].astype(np.float64)
+        d = np.maximum(np.maximum(lo, hi), 0.0)
+        return math.sqrt(float(d @ d))
+
+    t.set_mac("abs", tol)
+    nimg = (2 * ws + 1) ** 3 if periodic else 1
+    for g in np.random.default_rng(6).choice(t.ngroup, 25, replace=False):
+        mc, mi, pc, pi = t.lists(0.5, int(g), ws)
+        per_img = np.zeros(nimg, np.int64)
+        np.add.at(per_img, mi, cells["count"][mc]); np.add.at(per_img, pi, cells["count"][pc])
+        assert np.all(per_img == n)
+        bb = grp["bbox"][g]
+        for c, im in zip(mc, mi):
+            d = d_aabb(bb, com[c] + orc.image_shift(int(im), 1.0, periodic, ws))
+            assert d > side[c] + dl[c] and t.mac_bound(int(c), d) <= tol
+        for c, im in zip(pc, pi):
+            d = d_aabb(bb, com[c] + orc.image_shift(int(im), 1.0, periodic, ws))
+            assert not (d > side[c] + dl[c] and t.mac_bound(int(c), d) <= tol)
+    if not periodic:
+        sink = np.arange(0, n, 10)
+        ref = orc.direct_iso(pos, mass, 1e-3, sink)[0]
+        errs, work = [], []
+        for tl in (50.0, 5.0, 0.5):
+            t.set_mac("abs", tl)
+            a, _, n_p2p, n_m2p = t.accel(1e-3, 0.5, 4, sink)
+            errs.append(_erms(a, ref)); work.append(n_p2p + n_m2p)
+        assert errs[0] > errs[1] > errs[2] and work[0] < work[1] < work[2], (errs, work)
+    t.set_mac("theta")
