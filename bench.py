@@ -370,6 +370,43 @@ def measure_config(cfgid, steps, warmup, dev, world, rank, dist, want_e2e, want_
     return out
 
 
+def at_fixed_error(dev):
+    """The metric as the paper states it (a particle rate AT an RMS force accuracy of ~1e-4), on configs[1]:
+    the fastest settings `bench.py --sweep` found for E_rms <= 1e-4 under each acceptance rule (profiles/r02_sweep_c2.md),
+    re-timed here (5 evaluations, CUDA events, L2 flushed between) with E_rms re-measured against the oracle's fp64 direct sum on a 1024-sink sample."""
+    import torch
+    import oracle
+    from paper_1407_2600_b200 import dsk, workloads
+    cfg = dict(workloads.CONFIGS[2])
+    pos, mass = workloads.make(2)
+    n = len(pos)
+    sink = workloads.subsample(2, n, 1024)
+    ref = oracle.direct_iso(pos, mass, cfg["eps"], sink)[0]
+    arms = float(np.sqrt((ref ** 2).sum(1).mean()))
+    d = dsk.Dsk(n, 1.0, False, cfg["eps"], 0.5, 4, device=dev)
+    tp, tm = torch.from_numpy(pos).to(dev), torch.from_numpy(mass).to(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+    out = {"workload": WORKLOADS[2], "target_E_rms": 1e-4, "reference": "oracle fp64 direct sum, 1024 sinks", "a_rms": arms}
+    for name, kind, theta, p, tol in (("opening_angle", "theta", 0.7, 4, 0.0), ("absolute_error", "abs", 0.5, 2, 3e-3 * arms),
+                                      ("config_default", "theta", cfg["theta"], cfg["p"], 0.0)):
+        d.set_params(theta=theta, p=p); d.set_mac(kind, tol)
+        ms = []
+        for it in range(8):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); d.build_tree(tp, tm); acc = d.accel(tp, tm, want_pot=False)[0]; e1.record(stream); e1.synchronize()
+            if it >= 3:
+                ms.append(e0.elapsed_time(e1))
+        a = acc.cpu().numpy().astype(np.float64)[sink]
+        E = float(np.sqrt(((a - ref) ** 2).sum() / (ref ** 2).sum()))
+        t = float(np.mean(ms))
+        out[name] = {"rule": kind, "theta": theta, "p": p, "tol_over_a_rms": tol / arms if kind == "abs" else None,
+                     "ms_per_step": t, "value": n / (t * 1e-3), "unit": UNIT, "E_rms": E}
+    d.close()
+    return out
+
+
 def probe_peak():
     """dsk_probe_fp32_peak, all three operand forms (include/dsk.h): the measured FP32 denominator."""
     from paper_1407_2600_b200 import dsk
@@ -424,10 +461,76 @@ def run_ours(args):
             except Exception as ex:          # e.g. not enough device memory for 512^3 on a shared box: say so, keep the headline
                 others[f"configs[{cid - 1}]"] = {"error": repr(ex)[:300]}
         out["other_configs"] = others
+        try:
+            out["at_fixed_error"] = at_fixed_error(dev)
+        except Exception as ex:
+            out["at_fixed_error"] = {"error": repr(ex)[:300]}
     if use_dist:
         dist.destroy_process_group()
     if rank == 0:
         print(json.dumps(out))
+
+
+def run_sweep(args):
+    """bench.py --sweep: the metric the paper states (particle rate AT an RMS force accuracy) for the two
+    acceptance rules.  For configs[1] (and configs[3] with --config 4): ms per force evaluation (tree + forces, no potential) and
+    E_rms for a grid of (theta, p) and of (absolute tolerance, p); prints one JSON object with the table and, per rule, the
+    fastest setting that reaches E_rms <= 1e-4.  Error reference: the fp64 direct sum of the oracle on a 4096-sink sample
+    (isolated), or the library itself at theta 0.3, p 8, WS 2 on all particles (periodic)."""
+    import torch
+    from paper_1407_2600_b200 import dsk, workloads
+    cid = args.config
+    cfg = dict(workloads.CONFIGS[cid])
+    pos, mass = workloads.make(cid)
+    n = len(pos)
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    d = dsk.Dsk(n, cfg["box"], cfg["periodic"], cfg["eps"], cfg["theta"], cfg["p"], device=dev, p_max=8)
+    tp, tm = torch.from_numpy(pos).to(dev), torch.from_numpy(mass).to(dev)
+    d.build_tree(tp, tm)
+    if cfg["periodic"]:
+        d.set_image_block(2); d.set_params(theta=0.3, p=8)
+        ref = d.accel(tp, tm, want_pot=False)[0].double()
+        d.set_image_block(1)
+        sink = None
+        refname = "library at theta 0.3, p 8, WS 2, all particles"
+    else:
+        import oracle
+        sink_np = workloads.subsample(cid, n, 4096)
+        ref = torch.from_numpy(oracle.direct_iso(pos, mass, cfg["eps"], sink_np)[0]).to(dev)
+        sink = torch.from_numpy(sink_np).to(dev)
+        refname = "oracle fp64 direct sum, 4096 sinks"
+    arms = float(torch.sqrt((ref ** 2).sum(1).mean()))
+
+    def measure():
+        ms = []
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); d.build_tree(tp, tm); acc = d.accel(tp, tm, want_pot=False)[0]; e1.record(); e1.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        a = acc.double() if sink is None else acc.double()[sink]
+        st = d.get_stats()
+        return min(ms), float(torch.sqrt(((a - ref) ** 2).sum() / (ref ** 2).sum())), st["n_m2p"] / n, st["n_p2p"] / n
+
+    rows = []
+    for p in (2, 4, 6):
+        for theta in (0.4, 0.5, 0.6, 0.7, 0.8, 1.0):
+            d.set_mac("theta"); d.set_params(theta=theta, p=p)
+            ms, E, m2p, p2p = measure()
+            rows.append({"rule": "theta", "theta": theta, "p": p, "ms": round(ms, 3), "E_rms": E, "m2p_per_sink": round(m2p, 1), "p2p_per_sink": round(p2p, 1)})
+        for rel in (1e-1, 3e-2, 1e-2, 3e-3, 1e-3, 3e-4):
+            d.set_params(theta=0.5, p=p); d.set_mac("abs", rel * arms)
+            ms, E, m2p, p2p = measure()
+            rows.append({"rule": "abs", "tol_over_arms": rel, "p": p, "ms": round(ms, 3), "E_rms": E, "m2p_per_sink": round(m2p, 1), "p2p_per_sink": round(p2p, 1)})
+    best = {}
+    for target in (1e-3, 1e-4, 1e-5):
+        for rule in ("theta", "abs"):
+            ok = [r for r in rows if r["rule"] == rule and r["E_rms"] <= target]
+            if ok:
+                b = min(ok, key=lambda r: r["ms"])
+                best[f"{rule}@{target:g}"] = dict(b, particles_per_s=n / (b["ms"] * 1e-3))
+    d.close()
+    print(json.dumps({"sweep": WORKLOADS[cid], "N": n, "a_rms": arms, "reference": refname, "rows": rows, "fastest_at_or_below_target": best}))
 
 
 def main():
@@ -438,13 +541,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the C1/C3/C4/C5 lines appended to the default run")
+    ap.add_argument("--sweep", action="store_true", help="(theta, p) and (absolute tolerance, p) sweep of --config 2 or 4: ms and E_rms, see run_sweep")
     ap.add_argument("--peak", action="store_true", help="only run the FP32 issue-rate probe (dsk_probe_fp32_peak) and print it")
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5],
                     help="BASELINE.json config number (1-based); the default 2 is the workload the metric is quoted on")
     args = ap.parse_args()
     global CFG
     CFG = args.config
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
