@@ -185,7 +185,7 @@ def run_reference(args):
 
 
 # ---- our arm ------------------------------------------------------------------------------------------------
-def measure_config(cfgid, steps, warmup, dev, world, rank, dist, want_e2e, want_cpu, peak_meas):
+def measure_config(cfgid, steps, warmup, dev, world, rank, dist, want_e2e, want_cpu, peak_meas, shard=False):
     """Time `steps` steps of BASELINE.json config `cfgid` on this rank's device (after max(warmup, 3) untimed ones) and
     return the dict of everything the JSON line reports about it (rank 0; None on the other ranks)."""
     import torch
@@ -225,6 +225,25 @@ def measure_config(cfgid, steps, warmup, dev, world, rank, dist, want_e2e, want_
             d.kdk_reset()
             d.kdk_step(tp2, vel2, tm2, 0.5, DA)
             hacc.copy_(tp2, non_blocking=True); hv.copy_(vel2, non_blocking=True)
+    elif shard:
+        # strong scaling: every rank builds the whole tree, evaluates its work-weighted run of sink groups
+        # (dsk_accel_shard) and a sum-reduction over NVLink assembles acc and pot on all ranks: the path's one exchange step
+        from paper_1407_2600_b200 import sharding
+
+        def step():
+            d.build_tree(tp, tm)
+            acc.zero_(); pot.zero_()
+            d.accel_shard(rank, world, acc, pot)
+            sharding.assemble(dist if use_dist else None, acc)
+            sharding.assemble(dist if use_dist else None, pot)
+
+        def step_e2e():
+            tp2.copy_(hp, non_blocking=True); tm2.copy_(hm, non_blocking=True)
+            d.build_tree(tp2, tm2)
+            acc.zero_(); pot.zero_()
+            d.accel_shard(rank, world, acc, pot)
+            sharding.assemble(dist if use_dist else None, acc); sharding.assemble(dist if use_dist else None, pot)
+            hacc.copy_(acc, non_blocking=True); hpot.copy_(pot, non_blocking=True)
     else:
         def step():
             d.build_tree(tp, tm)
@@ -272,6 +291,8 @@ def measure_config(cfgid, steps, warmup, dev, world, rank, dist, want_e2e, want_
     barrier()
     clk = clocks.stop() if rank == 0 else None
     ms_max, units = aggregate(dist if use_dist else None, ms_total, n * steps, dev)
+    if shard:
+        units = float(n * steps)           # strong scaling: the job evaluates N particles per step, whatever the number of ranks
     value = units / (ms_max * 1e-3)
 
     e2e = None
@@ -335,8 +356,9 @@ def measure_config(cfgid, steps, warmup, dev, world, rank, dist, want_e2e, want_
         variant = "nopot" if kdk else "pot"
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
                "warmup": nwarm, "ms_per_step": ms_max / steps, "higher_is_better": True,
-               "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-               "config": config_dict(cfg, world, (dsk.get_param("NLEAF"), dsk.get_param("NCRIT"))),
+               "scaling": "strong" if shard else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+               "config": dict(config_dict(cfg, world, (dsk.get_param("NLEAF"), dsk.get_param("NCRIT"))),
+                              **({"parallelism": f"sink groups sharded over {world} rank(s), work-weighted; all-reduce of acc and pot"} if shard else {})),
                "roofline": {"bound": "alu", "kernel": f"k_m2p<{cfg['p']},{variant},{'periodic' if cfg['periodic'] else 'isolated'}>",
                             "achieved": ach_m2p / 1e12, "peak": peak_fp32 / 1e12, "unit": "TFLOP/s", "frac": ach_m2p / peak_fp32,
                             "peak_measured": pm / 1e12 if pm else None, "frac_measured": ach_m2p / pm if pm else None,
@@ -444,7 +466,7 @@ def run_ours(args):
     peak_meas = probe_peak() if rank == 0 else None
     head_cfg = args.config
     out = measure_config(head_cfg, args.steps, args.warmup, dev, world, rank, dist, True,
-                         world == 1 and not args.no_cpu_baseline, peak_meas)
+                         world == 1 and not args.no_cpu_baseline, peak_meas, shard=args.shard and head_cfg != 5)
     if rank == 0:
         out["fp32_peak_probe"] = peak_meas
     # The other BASELINE.json configs, AFTER the headline's timed region (so that it does not move): fewer steps, no
@@ -541,6 +563,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the C1/C3/C4/C5 lines appended to the default run")
+    ap.add_argument("--shard", action="store_true", help="N > 1: shard the sink groups over the ranks (strong scaling, dsk_accel_shard + all-reduce) "
+                    "instead of running N replicas; not for --config 5")
     ap.add_argument("--sweep", action="store_true", help="(theta, p) and (absolute tolerance, p) sweep of --config 2 or 4: ms and E_rms, see run_sweep")
     ap.add_argument("--peak", action="store_true", help="only run the FP32 issue-rate probe (dsk_probe_fp32_peak) and print it")
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5],

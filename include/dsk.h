@@ -103,6 +103,15 @@ int dsk_accel(dsk_ctx *ctx, const float *pos, const float *mass, float *acc, flo
  * hold an active particle are walked and evaluated; acc/pot entries of inactive particles are left untouched. */
 int dsk_accel_active(dsk_ctx *ctx, const float *pos, const float *mass, const uint8_t *active, float *acc, float *pot);
 
+/* The same for ONE SHARD of the sink groups (the sorted list is cut into pieces weighted
+ * by work).  Every rank of a multi-GPU job holds all particles and builds the same tree; rank `rank` of `nranks` (<= 1023)
+ * evaluates the contiguous run of sink groups (Morton order) whose work, n_sinks x (M2P list length x flop per M2P + P2P sources
+ * x flop per pair) from a counting walk of ALL groups, falls into its 1/nranks of the total; every particle stays a source.
+ * The cut is a function of the tree, theta and the acceptance rule alone, so the ranks agree on it without communicating.
+ * acc/pot entries of particles in other shards are left untouched: with acc zero-filled beforehand, a sum-reduction over the
+ * ranks (ncclAllReduce) assembles the full result.  first_group / end_group (host, may be NULL) receive the run [first, end). */
+int dsk_accel_shard(dsk_ctx *ctx, int rank, int nranks, float *acc, float *pot, int64_t *first_group, int64_t *end_group);
+
 /* One kick-drift-kick step of the comoving leapfrog (O9), in place:
  * vel is the canonical momentum per unit mass a^2 dx/dt; periodic: Einstein-de Sitter factors from
  * the total mass in the box, positions wrapped to [0,box); isolated: Newtonian with dt = da.

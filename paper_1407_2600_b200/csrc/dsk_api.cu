@@ -240,12 +240,15 @@ extern "C" int dsk_build_tree(dsk_ctx *c, const float *pos, const float *mass)
     return DSK_OK;
 }
 
-static int accel_impl(dsk_ctx *c, const uint8_t *active, float *acc, float *pot)
+// shard_rank >= 0: evaluate only the contiguous run of sink groups that the work-weighted cut gives this rank (dsk_accel_shard)
+static int accel_impl(dsk_ctx *c, const uint8_t *active, float *acc, float *pot, int shard_rank = -1, int shard_n = 1,
+                      int64_t *shard_lo = nullptr, int64_t *shard_hi = nullptr)
 {
     if (!c || !acc) return DSK_EINVAL;
     if (!c->ws) return DSK_ENOWORKSPACE;
     if (!c->have_tree) return DSK_ENOTREE;
     int e;
+    uint32_t r_lo = 0, r_hi = 0xffffffffu;
     if (c->moments_p != c->p) {
         e = dsk_run_upward(c);
         if (e) return e;
@@ -259,13 +262,31 @@ static int accel_impl(dsk_ctx *c, const uint8_t *active, float *acc, float *pot)
         c->gact_cur = c->gact;
         c->lists_valid = 0;
     }
+    if (shard_rank >= 0) {
+        static const uint32_t fm[4] = {78, 252, 682, 1536};         // flop per M2P interaction at p = 2, 4, 6, 8
+        uint32_t cut[1025];
+        e = dsk_run_shard(c, shard_rank, shard_n, fm[c->p / 2 - 1], 19u, cut);
+        if (e) return e;
+        const uint32_t g_lo = cut[shard_rank], g_hi = cut[shard_rank + 1], ng = c->hstate->ngroup;
+        if (shard_lo) *shard_lo = g_lo;
+        if (shard_hi) *shard_hi = g_hi;
+        // the shard's sorted ranks [first rank of g_lo, first rank of g_hi)
+        uint32_t ends[2] = {0, (uint32_t)c->N};
+        if (g_lo < ng) DSK_CUDA(cudaMemcpyAsync(&ends[0], c->gfirst + g_lo, 4, cudaMemcpyDeviceToHost, c->stream));
+        else ends[0] = (uint32_t)c->N;
+        if (g_hi < ng) DSK_CUDA(cudaMemcpyAsync(&ends[1], c->gfirst + g_hi, 4, cudaMemcpyDeviceToHost, c->stream));
+        DSK_CUDA(cudaStreamSynchronize(c->stream));
+        r_lo = ends[0]; r_hi = ends[1];
+        c->gact_cur = c->gact;
+        c->lists_valid = 0;
+    }
     if (!(c->lists_valid && c->lists_theta == c->theta)) {
         e = dsk_run_walk(c);
         if (e) { c->gact_cur = nullptr; return e; }
     }
     e = dsk_run_force(c, pot != nullptr);
     c->gact_cur = nullptr;
-    if (active) c->lists_valid = 0;
+    if (active || shard_rank >= 0) c->lists_valid = 0;
     if (e) return e;
     cudaEventRecord(c->ev[12], c->stream);
     if (c->periodic) {
@@ -277,7 +298,7 @@ static int accel_impl(dsk_ctx *c, const uint8_t *active, float *acc, float *pot)
         }
     }
     cudaEventRecord(c->ev[13], c->stream);
-    e = dsk_run_scatter(c, acc, pot, active);
+    e = dsk_run_scatter(c, acc, pot, active, r_lo, r_hi);
     if (e) return e;
     cudaEventRecord(c->ev[14], c->stream);
     e = read_state(c);
@@ -301,6 +322,12 @@ extern "C" int dsk_accel_active(dsk_ctx *c, const float *pos, const float *mass,
     (void)pos; (void)mass;
     if (!active) return DSK_EINVAL;
     return accel_impl(c, active, acc, pot);
+}
+
+extern "C" int dsk_accel_shard(dsk_ctx *c, int rank, int nranks, float *acc, float *pot, int64_t *first_group, int64_t *end_group)
+{
+    if (!c || nranks < 1 || nranks > 1023 || rank < 0 || rank >= nranks) return DSK_EINVAL;
+    return accel_impl(c, nullptr, acc, pot, rank, nranks, first_group, end_group);
 }
 
 // Leapfrog factors (O9 / O9b): H0^2 = (8 pi/3) M_tot / (box^3 Omega_m),

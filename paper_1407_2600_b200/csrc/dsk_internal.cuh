@@ -219,7 +219,7 @@ static inline bool *dsk_device_flag(bool *flags)
 
 // ---- internal entry points (one per source file) -------------------------------------------------
 int dsk_run_keysort(dsk_ctx *c, const float *pos, const float *mass);         // keysort.cu: K, S, gather
-int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot, const uint8_t *active);   // keysort.cu: X
+int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot, const uint8_t *active, uint32_t r_lo, uint32_t r_hi);   // keysort.cu: X
 int dsk_run_group_active(dsk_ctx *c, const uint8_t *active);                  // keysort.cu
 void dsk_exclusive_scan_u32(dsk_ctx *c, const uint32_t *in, uint32_t *out, const uint32_t *n_dev,
                             uint32_t n_max, uint32_t *total_dev);             // keysort.cu
@@ -227,6 +227,7 @@ int dsk_run_build(dsk_ctx *c);                                                //
 int dsk_run_upward(dsk_ctx *c);                                               // upward.cu: U
 int dsk_run_get_moments(dsk_ctx *c, float *com_mass, float *moments, int scaled);         // upward.cu
 int dsk_run_walk(dsk_ctx *c);                                                 // walk.cu: W
+int dsk_run_shard(dsk_ctx *c, int rank, int nranks, uint32_t flop_m2p, uint32_t flop_p2p, uint32_t *cut_host);   // walk.cu
 int dsk_run_force(dsk_ctx *c, int want_pot);                                  // force.cu: F1 + orchestration
 int dsk_frow_len(int p, int dip);                                             // m2p.cu
 int dsk_run_frows(dsk_ctx *c);                                                // m2p.cu: moment rows -> force rows

@@ -260,10 +260,10 @@ __global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pos, c
 __global__ void __launch_bounds__(256) k_scatter(const float4 *__restrict__ sacc, const float4 *__restrict__ sacc_lo,
                                                  const uint32_t *__restrict__ order, int64_t n,
                                                  float *__restrict__ acc, float *__restrict__ pot,
-                                                 const uint8_t *__restrict__ active)
+                                                 const uint8_t *__restrict__ active, uint32_t r_lo, uint32_t r_hi)
 {
     int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (r >= n) return;
+    if (r >= n || r < (int64_t)r_lo || r >= (int64_t)r_hi) return;     // dsk_accel_shard: only the ranks (sorted positions) of this shard
     uint32_t i = order[r];
     if (active && !active[i]) return;            // dsk_accel_active: inactive entries are left untouched
     float4 a = sacc[r];
@@ -323,10 +323,10 @@ int dsk_run_group_active(dsk_ctx *c, const uint8_t *active)
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
-int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot, const uint8_t *active)
+int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot, const uint8_t *active, uint32_t r_lo, uint32_t r_hi)
 {
     const int nb = (int)((c->N + 255) / 256);
-    k_scatter<<<nb, 256, 0, c->stream>>>(c->sacc, c->sacc_lo, c->idx_a, c->N, acc, pot, active);
+    k_scatter<<<nb, 256, 0, c->stream>>>(c->sacc, c->sacc_lo, c->idx_a, c->N, acc, pot, active, r_lo, r_hi);
     DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }

@@ -501,3 +501,58 @@ int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint6
     DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
+
+// ---- sink-group sharding over ranks ("cut the sorted list into N_p pieces weighted by work") ----------
+// Every rank holds the whole tree.  A COUNT walk of all groups gives each group's list lengths, hence its work
+//   w_g = n_sinks (len_M2P flop_M2P + src_P2P flop_P2P);
+// the groups are in Morton order, and rank r takes the contiguous run whose prefix sums fall in [r, r+1) total / nranks.  All ranks
+// compute the same cut from the same tree: no communication is needed to agree on it.
+__global__ void __launch_bounds__(256) k_shard_weight(uint32_t ng, const uint32_t *__restrict__ gcount, const uint32_t *__restrict__ m2p_len,
+                                                      const uint32_t *__restrict__ p2p_src, uint32_t fm, uint32_t fp, uint32_t *__restrict__ w)
+{
+    const uint32_t g = blockIdx.x * 256 + threadIdx.x;
+    if (g >= ng) return;
+    const unsigned long long v = (unsigned long long)gcount[g] * ((unsigned long long)m2p_len[g] * fm + (unsigned long long)p2p_src[g] * fp);
+    w[g] = (uint32_t)min(v >> 10, 0xffffffffull) + 1u;          // + 1: an empty list still costs a task
+}
+__global__ void k_shard_cut(uint32_t ng, const uint64_t *__restrict__ off, int nranks, uint32_t *__restrict__ cut)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k > nranks) return;
+    const uint64_t total = off[ng], target = (uint64_t)(((unsigned __int128)total * (unsigned)k) / (unsigned)nranks);
+    uint32_t lo = 0, hi = ng;                                    // first g with off[g] >= target
+    while (lo < hi) {
+        const uint32_t mid = lo + ((hi - lo) >> 1);
+        if (off[mid] < target) lo = mid + 1; else hi = mid;
+    }
+    cut[k] = k == nranks ? ng : lo;
+}
+__global__ void __launch_bounds__(256) k_shard_mark(uint32_t ng, uint32_t g_lo, uint32_t g_hi, uint8_t *__restrict__ gact)
+{
+    const uint32_t g = blockIdx.x * 256 + threadIdx.x;
+    if (g < ng) gact[g] = (g >= g_lo && g < g_hi) ? 1 : 0;
+}
+
+// cut[0..nranks] (host) for the current tree, theta and acceptance rule; marks the groups of `rank` in c->gact
+int dsk_run_shard(dsk_ctx *c, int rank, int nranks, uint32_t flop_m2p, uint32_t flop_p2p, uint32_t *cut_host)
+{
+    const uint32_t ng = c->hstate->ngroup, nc = c->hstate->ncell;
+    cudaStream_t s = c->stream;
+    const bool ABS = c->mac_kind == 1;
+    k_walk_mac<<<(nc + 255) / 256, 256, 0, s>>>(nc, c->box, ABS ? 1.0f : 1.0f / c->theta, ABS ? c->mac_tol : 0.0f, c->p, dsk_rowlen(c->p), c->rows,
+                                                c->periodic && c->bg ? c->ntop : 0u, c->rows_bg, c->cell, c->whdr, c->wmac, c->kbg);
+    (ABS ? k_walk<0, true> : k_walk<0, false>)<<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, c->p + 1, c->cell, c->wmac,
+                                                     c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len,
+                                                     c->g_p2p_src, nullptr, nullptr, 0, 0, nullptr, nullptr,
+                                                     nullptr, 0, 0, nullptr, nullptr, make_walk_bg(c, 0, 0), c->dstate);
+    uint32_t *w = c->gscan;                                      // [N] scratch of the group extraction, free by now
+    k_shard_weight<<<(ng + 255) / 256, 256, 0, s>>>(ng, c->gcount, c->g_m2p_len, c->g_p2p_src, flop_m2p, flop_p2p, w);
+    scan64(c, w, ng, c->g_m2p_off);                              // the offsets are rewritten by the walk that follows
+    uint32_t *cut = c->task_hist;                                // [1024] scratch
+    k_shard_cut<<<(nranks + 1 + 63) / 64, 64, 0, s>>>(ng, c->g_m2p_off, nranks, cut);
+    DSK_CUDA(cudaMemcpyAsync(cut_host, cut, sizeof(uint32_t) * (size_t)(nranks + 1), cudaMemcpyDeviceToHost, s));
+    DSK_CUDA(cudaStreamSynchronize(s));
+    k_shard_mark<<<(ng + 255) / 256, 256, 0, s>>>(ng, cut_host[rank], cut_host[rank + 1], c->gact);
+    DSK_COUNT(c, 7);
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
+}

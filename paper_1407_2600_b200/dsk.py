@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libdsk.so")
 
 SYMBOLS = [
     "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
-    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_set_background", "dsk_get_background", "dsk_set_image_block", "dsk_get_image_block", "dsk_set_mac", "dsk_get_bg_moments", "dsk_get_keys",
+    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_accel_shard", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_set_background", "dsk_get_background", "dsk_set_image_block", "dsk_get_image_block", "dsk_set_mac", "dsk_get_bg_moments", "dsk_get_keys",
     "dsk_get_tree", "dsk_get_moments", "dsk_get_moments_scaled", "dsk_get_groups", "dsk_get_stats", "dsk_get_param", "dsk_get_task_widths",
     "dsk_get_lattice_tensors", "dsk_probe_fp32_peak", "dsk_probe_fp32_peak_ex", "dsk_strerror",
 ]
@@ -59,6 +59,7 @@ def load_library(path=LIB_PATH):
     lib.dsk_build_tree.argtypes = [vp, vp, vp]
     lib.dsk_accel.argtypes = [vp, vp, vp, vp, vp]
     lib.dsk_accel_active.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.dsk_accel_shard.argtypes = [vp, i32, i32, vp, vp, C.POINTER(i64), C.POINTER(i64)]
     lib.dsk_kdk_step.argtypes = [vp, vp, vp, vp, f64, f64]
     lib.dsk_kdk_block_step.argtypes = [vp, vp, vp, vp, vp, f64, f64, i32, f32]
     lib.dsk_kdk_reset.argtypes = [vp]
@@ -207,6 +208,14 @@ class Dsk:
         _check(self.lib.dsk_accel_active(self._h, _ptr(pos), _ptr(mass), C.c_void_p(active.data_ptr()), _ptr(acc),
                                          _ptr(pot) if pot is not None else None))
         return acc, pot
+
+    def accel_shard(self, rank, nranks, acc, pot=None):
+        """forces of this rank's work-weighted run of sink groups, written into acc/pot in place; returns the run [first, end)"""
+        _dev_f32(acc, (self.N, 3))
+        lo, hi = C.c_int64(0), C.c_int64(0)
+        _check(self.lib.dsk_accel_shard(self._h, int(rank), int(nranks), _ptr(acc), _ptr(pot) if pot is not None else None,
+                                        C.byref(lo), C.byref(hi)))
+        return lo.value, hi.value
 
     def kdk_step(self, pos, vel, mass, a, da):
         _dev_f32(pos, (self.N, 3)); _dev_f32(vel, (self.N, 3)); _dev_f32(mass, (self.N,))

@@ -72,3 +72,67 @@ def test_accounting_matches_kernel_op_counts():
             # (a few more where the compiler packs scalar pairs itself, e.g. the sinks' offsets from the group centre)
             assert fadd + 24 <= fn[0].count(" FADD2 ") <= fadd + 32, (p, mode, fn[0].count(" FADD2 "), fadd)
     assert accounting.m2p_flops(4, dip=True) - accounting.m2p_flops(4) == 2 * 6 - 1
+
+
+def _shard_worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    import numpy as np
+    import torch.distributed as dist
+    from paper_1407_2600_b200 import sharding
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    rng = np.random.default_rng(5)                      # the same "tree" on every rank
+    ng = 5000
+    count = rng.integers(1, 193, ng)
+    first = np.concatenate([[0], np.cumsum(count)[:-1]])
+    n = int(count.sum())
+    w = sharding.group_work(count, rng.integers(500, 4000, ng), rng.integers(1000, 9000, ng), 252)
+    cut = sharding.cut_points(w, world)
+    full = torch.from_numpy(rng.standard_normal((n, 3)).astype(np.float32))      # what a full evaluation would give
+    order = torch.from_numpy(rng.permutation(n))                                  # sorted rank -> caller index
+    acc = torch.zeros((n, 3))
+    r_lo = int(first[cut[rank]]) if cut[rank] < ng else n
+    r_hi = int(first[cut[rank + 1]]) if cut[rank + 1] < ng else n
+    mine = order[r_lo:r_hi]
+    acc[mine] = full[mine]                              # this rank's shard, caller order; the rest stays zero
+    sharding.assemble(dist, acc)
+    ok = bool(torch.equal(acc, full))
+    dist.barrier()
+    dist.destroy_process_group()
+    q.put((rank, ok, cut, float(w[cut[rank]:cut[rank + 1]].sum()) / float(w.sum())))
+
+
+def test_shard_assembly_world2_gloo():
+    """N > 1 path of bench.py --shard on CPU: both ranks derive the same cut from the same tree, fill disjoint shards that
+    cover every particle once, and the sum-reduction leaves the full result on both."""
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 31500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_shard_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert all(ok for _, ok, _, _ in res)
+    assert res[0][2] == res[1][2] and res[0][2][0] == 0 and res[0][2][-1] == 5000
+    assert abs(res[0][3] - 0.5) < 0.01 and abs(res[1][3] - 0.5) < 0.01
+
+
+def test_shard_cut_balances_clustered_weights():
+    """the cut rule on weights shaped like configs[3]'s (a few heavy groups next to halos among many light ones): every group
+    in exactly one shard, shards balanced to 5 % for 2, 4 and 8 ranks"""
+    import numpy as np
+    from paper_1407_2600_b200 import sharding
+    rng = np.random.default_rng(1)
+    ng = 400000
+    w = sharding.group_work(rng.integers(1, 193, ng), (2000 * rng.lognormal(0.0, 0.5, ng)).astype(np.int64),
+                            (4000 * rng.lognormal(0.0, 0.8, ng)).astype(np.int64), 682)
+    for nr in (1, 2, 4, 8, 7):
+        cut = sharding.cut_points(w, nr)
+        assert cut[0] == 0 and cut[-1] == ng and all(cut[i] <= cut[i + 1] for i in range(nr))
+        share = np.array([float(w[cut[i]:cut[i + 1]].sum()) for i in range(nr)]) / float(w.sum())
+        assert np.max(np.abs(share * nr - 1.0)) < 0.05, (nr, share)
+    assert sharding.cut_points([5], 3) == [0, 0, 1, 1] or sharding.cut_points([5], 3)[-1] == 1

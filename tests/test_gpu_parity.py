@@ -751,6 +751,37 @@ def test_image_block_one_and_two(dsk, orc, case):
     d.close()
 
 
+@pytest.mark.parametrize("periodic", [False, True])
+def test_accel_shard_tiles_and_equals_full(dsk, periodic):
+    """dsk_accel_shard: for 2, 3 and 7 ranks the runs of sink groups tile all groups, the shards written one
+    after the other into one zero-filled array reproduce the full evaluation bit for bit, and the work (cell interactions of
+    each shard) is balanced; the device's cut equals the host statement of the rule when the lists are those of the full walk."""
+    from paper_1407_2600_b200 import sharding
+    pos, mass = (workloads.clustered_box(28, 20, cfg=4) if periodic else workloads.make(2, 1 / 16))
+    n = len(pos)
+    d = dsk.Dsk(n, 1.0, periodic, 1e-3, 0.5, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    full, fpot = d.accel(tp, tm)
+    ng = d.get_stats()["ngroup"]
+    tot_m2p = d.get_stats()["n_m2p"]
+    for nr in (2, 3, 7):
+        acc = torch.zeros((n, 3), dtype=torch.float32, device="cuda"); pot = torch.zeros(n, dtype=torch.float32, device="cuda")
+        runs, work = [], []
+        for r in range(nr):
+            runs.append(d.accel_shard(r, nr, acc, pot))
+            work.append(d.get_stats()["n_m2p"])
+        assert runs[0][0] == 0 and runs[-1][1] == ng and all(runs[i][1] == runs[i + 1][0] for i in range(nr - 1)), runs
+        assert torch.equal(acc, full) and torch.equal(pot, fpot)
+        assert sum(work) == tot_m2p
+        assert max(work) < 1.35 * tot_m2p / nr, (nr, work)          # M2P alone; the cut balances M2P + P2P flops
+    with pytest.raises(dsk.DskError):
+        d.accel_shard(2, 2, acc, pot)
+    again, _ = d.accel(tp, tm)
+    assert torch.equal(again, full)
+    d.close()
+
+
 # ---- absolute-error acceptance rule (reading O5b; PAPER.md:63) ----------------------------------------------------
 @pytest.mark.parametrize("case", ["plummer", "periodic-clustered", "periodic-lattice"])
 def test_abs_mac_parity(dsk, orc, case):
