@@ -308,6 +308,29 @@ def bg_halfwidth(theta, lb, ws=WS):
     return int(lib().orc_bg_halfwidth(C.c_double(theta), C.c_int(ws), C.c_int(lb)))
 
 
+# ---- softening law (O6 / O6b) -----------------------------------------------------------------------------
+class softening:
+    """`with oracle.softening("k1"):` — every pair term inside the block uses Dehnen's K1 kernel with support h = the `eps` argument
+    of the calls (direct sums, tree P2P; the tree's far cells become Newtonian and are accepted only beyond h); "plummer" is the default."""
+    def __init__(self, kind):
+        self.kind = {"plummer": 0, "k1": 1}[kind]
+
+    def __enter__(self):
+        self.old = int(lib().orc_get_softening())
+        lib().orc_set_softening(C.c_int(self.kind))
+        return self
+
+    def __exit__(self, *a):
+        lib().orc_set_softening(C.c_int(self.old))
+
+
+def soft_pair(r2, length):
+    """(f, phi) of the current softening law: acc = -m d f, pot = -m phi"""
+    f = C.c_double(0); ph = C.c_double(0)
+    lib().orc_soft_pair(C.c_double(r2), C.c_double(length), C.byref(f), C.byref(ph))
+    return f.value, ph.value
+
+
 # ---- D ---------------------------------------------------------------------------------------------
 def direct_iso(pos, mass, eps, sink=None):
     pos = _f32(pos); mass = _f32(mass); sink = _sink(sink)

@@ -9,7 +9,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["orc_tree.c", "orc_moments.c", "orc_eval.c", "orc_periodic.c", "orc_bg.c"]
+SOURCES = ["orc_tree.c", "orc_moments.c", "orc_eval.c", "orc_periodic.c", "orc_bg.c", "orc_soft.c"]
 LIB = os.path.join(HERE, "libdsk_oracle.so")
 
 

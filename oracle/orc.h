@@ -57,6 +57,7 @@ typedef struct orc_tree {
     /* O5b acceptance rule in use (orc_tree_set_mac): 0 opening angle, 1 absolute error bound   */
     int mac_kind;
     double mac_tol;
+    double soft_len;       /* softening length of the walk in progress (K1: the MAC needs h)  */
 } orc_tree;
 
 /* multi-index helpers (orc_tree.c) */
@@ -93,6 +94,11 @@ void orc_group_lists(orc_tree *t, double theta, int ws, int bg, int64_t g, int64
 void orc_cell_coords(const orc_tree *t, int64_t c, int64_t q[3]);
 void orc_tree_set_mac(orc_tree *t, int kind, double tol);
 double orc_mac_bound(const orc_tree *t, int64_t c, int sub, double d);
+
+/* softening law: 0 Plummer, 1 Dehnen K1 (orc_soft.c); a setting of the whole oracle library */
+void orc_set_softening(int kind);
+int orc_get_softening(void);
+void orc_soft_pair(double r2, double len, double *f, double *phi);
 
 /* background subtraction, reading O4b (orc_bg.c) */
 void orc_cuboid_field(const double lo[3], const double hi[3], const double x[3], double *I, double g[3]);

@@ -36,7 +36,6 @@ void orc_set_threads(int n)
 void orc_direct_iso(int64_t n, const float *pos, const float *mass, double eps, int64_t nsink,
                     const int64_t *sink, double *acc, double *pot)
 {
-    double e2 = eps * eps;
 #pragma omp parallel for schedule(dynamic, 16)
     for (int64_t s = 0; s < nsink; s++) {
         int64_t i = sink ? sink[s] : s;
@@ -46,10 +45,10 @@ void orc_direct_iso(int64_t n, const float *pos, const float *mass, double eps, 
             if (j == i) continue;
             double dx = xi - (double)pos[3 * j], dy = yi - (double)pos[3 * j + 1],
                    dz = zi - (double)pos[3 * j + 2];
-            double R2 = dx * dx + dy * dy + dz * dz + e2;
-            double rinv = 1.0 / sqrt(R2), m = (double)mass[j];
-            double mr3 = m * rinv / R2;
-            ax -= mr3 * dx; ay -= mr3 * dy; az -= mr3 * dz; ph -= m * rinv;
+            double f, phi, m = (double)mass[j];
+            orc_soft_pair(dx * dx + dy * dy + dz * dz, eps, &f, &phi);      /* Plummer: (r^2+eps^2)^(-3/2), (r^2+eps^2)^(-1/2) */
+            double mr3 = m * f;
+            ax -= mr3 * dx; ay -= mr3 * dy; az -= mr3 * dz; ph -= m * phi;
         }
         acc[3 * s] = ax; acc[3 * s + 1] = ay; acc[3 * s + 2] = az;
         if (pot) pot[s] = ph;
@@ -193,12 +192,15 @@ static void walk_rec(walk_t *w, int64_t c)
      * counted twice inside the window */
     const int straddles = top && inter && !inside;
     int ok;
+    /* O6b: with the compact K1 kernel a cell is expanded (Newtonian) only if every source lies outside the kernel's support of every
+     * sink: d - b > h, b = sqrt(3)/2 s + delta the radius of the ball about the expansion centre that holds the cell */
+    const int k1_near = orc_get_softening() == 1 && !(sqrt(d2) - (0.5 * sqrt(3.0) * s + t->delta[c]) > t->soft_len);
     if (t->mac_kind == 0) ok = d2 > rc * rc;                            /* opening angle (strict) */
     else {                                                              /* O5b: theta = 1 for validity, then the error bound */
         double r1 = s + t->delta[c];
         ok = d2 > r1 * r1 && orc_mac_bound(t, c, top && !inter, sqrt(d2)) <= t->mac_tol;
     }
-    if (!straddles && ok) {                                             /* accept             */
+    if (!straddles && !k1_near && ok) {                                 /* accept             */
         il_push(w->m2p, c, w->im, (int8_t)(top && !inter));              /* outside the window: background subtracted */
         return;
     }
@@ -331,7 +333,10 @@ int orc_tree_accel(orc_tree *t, double eps, double theta, int ws, int bg, int64_
 {
     if (t->p < 0) return -3;
     int p = t->p, np = ORC_NP(p);
-    double e2 = eps * eps;
+    /* the far cells are expanded with the softened Green's function of reading A8 (Plummer), or, for the compact K1 kernel,
+     * with the Newtonian one: the walk then accepts a cell only if all its sources are farther than h from the group (O6b) */
+    double e2 = orc_get_softening() == 0 ? eps * eps : 0.0;
+    t->soft_len = eps;
     gs_t *gs = malloc(sizeof(gs_t) * (size_t)(nsink > 0 ? nsink : 1));
     for (int64_t s = 0; s < nsink; s++) {
         int64_t i = sink ? sink[s] : s;
@@ -367,9 +372,10 @@ int orc_tree_accel(orc_tree *t, double eps, double theta, int ws, int bg, int64_
                         if (self_image && j == r) continue;
                         double dx = x[0] - (t->spos[3 * j] + sh[0]), dy = x[1] - (t->spos[3 * j + 1] + sh[1]),
                                dz = x[2] - (t->spos[3 * j + 2] + sh[2]);
-                        double R2 = dx * dx + dy * dy + dz * dz + e2, rinv = 1.0 / sqrt(R2);
-                        double mr3 = t->smass[j] * rinv / R2;
-                        a[0] -= mr3 * dx; a[1] -= mr3 * dy; a[2] -= mr3 * dz; ph -= t->smass[j] * rinv;
+                        double f, phi;
+                        orc_soft_pair(dx * dx + dy * dy + dz * dz, eps, &f, &phi);
+                        double mr3 = t->smass[j] * f;
+                        a[0] -= mr3 * dx; a[1] -= mr3 * dy; a[2] -= mr3 * dz; ph -= t->smass[j] * phi;
                         tot_p2p++;
                     }
                 }

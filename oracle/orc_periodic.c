@@ -88,11 +88,13 @@ double orc_ewald_self(double L, double alpha, int nmax, int hmax)
  * particle and itself) has no Newtonian term to remove here; the caller handles it. */
 static void plummer_minus_newton(const double d[3], double e2, double a[3], double *ph)
 {
+    /* softened minus Newtonian pair term; the softening law is orc_soft_pair's (Plummer unless the K1 kernel is selected) */
     double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
-    double R = sqrt(r2 + e2), r = sqrt(r2);
-    double fp = 1.0 / (R * R * R), fn = 1.0 / (r * r * r);
-    for (int k = 0; k < 3; k++) a[k] += -d[k] * fp + d[k] * fn;
-    *ph += -1.0 / R + 1.0 / r;
+    double r = sqrt(r2), fs, phis;
+    orc_soft_pair(r2, sqrt(e2), &fs, &phis);
+    double fn = 1.0 / (r * r * r);
+    for (int k = 0; k < 3; k++) a[k] += -d[k] * fs + d[k] * fn;
+    *ph += -phis + 1.0 / r;
 }
 
 /* D-per, pair by pair exactly as SURVEY.md §8(c) writes it:
@@ -117,7 +119,7 @@ void orc_direct_per_pairwise(int64_t n, const float *pos, const float *mass, dou
                 /* regular part of psi at 0; the force's regular part vanishes by symmetry.  For a
                  * coincident *distinct* pair the Plummer term at d = 0 is kept: -1/eps, no force */
                 ph = self;
-                if (j != i) ph += -1.0 / sqrt(e2);
+                if (j != i) { double f0, p0; orc_soft_pair(0.0, eps, &f0, &p0); ph += -p0; }
             }
             for (int ix = -ws; ix <= ws; ix++)
                 for (int iy = -ws; iy <= ws; iy++)
@@ -211,7 +213,7 @@ void orc_direct_per(int64_t n, const float *pos, const float *mass, double L, do
                         int inblock = (abs(ix) <= ws && abs(iy) <= ws && abs(iz) <= ws);
                         if (zero && !ix && !iy && !iz) {
                             ph += selfreal;
-                            if (j != i) ph += -1.0 / sqrt(e2);
+                            if (j != i) { double f0, p0; orc_soft_pair(0.0, eps, &f0, &p0); ph += -p0; }
                             continue;
                         }
                         double r2 = dn[0] * dn[0] + dn[1] * dn[1] + dn[2] * dn[2];
