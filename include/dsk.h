@@ -129,6 +129,13 @@ int dsk_kdk_reset(dsk_ctx *ctx);
  * background in the far field alone (and fp64 monopoles).
  * DSK_EINVAL for on != 0 in an isolated context.  Changing it invalidates moments, lists and the cached KDK force. */
 int dsk_set_background(dsk_ctx *ctx, int on);
+/* Pair softening law.  kind 0 (default): Plummer, phi = -m (r^2 + eps^2)^(-1/2), length = eps (the same as dsk_set_params' eps).
+ * kind 1: Dehnen's K1 compensating kernel of compact support h = length ("using a Dehnen K1 compensating smoothing kernel
+ * (Dehnen 2001)"; reading O6b of DESIGN.md): the point mass is the density 105/(64 pi h^3)(1 - u)(5 - 9u), u = r^2/h^2 < 1 (unit mass,
+ * zero second moment), the pair force is -m d/h^3 (175/16 - 147/8 u + 135/16 u^2) inside h and exactly Newtonian outside.  Cells are then
+ * expanded with the Newtonian Green's function and accepted only if all their sources lie farther than h from the sink group.
+ * dsk_set_params keeps the kind and changes the length.  DSK_EINVAL for another kind or length <= 0. */
+int dsk_set_softening(dsk_ctx *ctx, int kind, float length);
 /* Acceptance rule of the walk.  kind 0 (default): the opening angle of dsk_create / dsk_set_params, accept iff
  * d^2 > (s/theta + delta)^2.  kind 1: an ABSOLUTE ERROR BOUND per cell interaction ("We adjust the error tolerance
  * parameter to limit absolute errors ..."; reading O5b of DESIGN.md): accept iff d^2 > (s + delta)^2 and

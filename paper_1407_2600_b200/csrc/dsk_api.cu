@@ -390,6 +390,14 @@ extern "C" int dsk_set_cosmology(dsk_ctx *c, double omega_m, double omega_lambda
     return DSK_OK;
 }
 
+extern "C" int dsk_set_softening(dsk_ctx *c, int kind, float length)
+{
+    if (!c || (kind != 0 && kind != 1) || !(length > 0.0f) || !isfinite(length)) return DSK_EINVAL;
+    c->soft_kind = kind; c->eps = length;
+    c->lists_valid = 0; c->kdk_have_acc = 0;          // the K1 walk keeps cells out of the kernel's support: other lists
+    return DSK_OK;
+}
+
 extern "C" int dsk_set_mac(dsk_ctx *c, int kind, float tol)
 {
     if (!c || (kind != 0 && kind != 1)) return DSK_EINVAL;

@@ -70,7 +70,11 @@ struct leaf_batch {              // one leaf per lane
     float shx, shy, shz;
 };
 
-template <bool POT>
+// K1: Dehnen's K1 compensating kernel of support h instead of Plummer softening (reading O6b of DESIGN.md): for
+// u = r^2/h^2 < 1   acc = -m d / h^3 (175/16 - 147/8 u + 135/16 u^2),  pot = -(m/h)(105/32 - 175/32 u + 147/32 u^2 - 135/96 u^3),
+// Newtonian beyond (eps2 then carries h^2).  Both branches are evaluated packed and the halves selected: ~27 packed instructions
+// per pair instead of 13.
+template <bool POT, bool K1>
 __global__ void __launch_bounds__(FW * 32, P2P_MINB) k_p2p(uint32_t t0, uint32_t t1, const uint32_t *__restrict__ taskmap, int periodic, float box, float eps2,
                                                  const dsk_cellrec *__restrict__ cell, const float4 *__restrict__ spos,
                                                  const uint32_t *__restrict__ gfirst, const uint32_t *__restrict__ gcount,
@@ -87,6 +91,7 @@ __global__ void __launch_bounds__(FW * 32, P2P_MINB) k_p2p(uint32_t t0, uint32_t
     const float4 ma = spos[t.sa], mb = spos[t.sb];
     const f2 X = f2_make(ma.x, mb.x), Y = f2_make(ma.y, mb.y), Z = f2_make(ma.z, mb.z);
     const f2 E2 = f2_dup(eps2);
+    const float hinv = rsqrtf(eps2), hinv2 = hinv * hinv, hinv3 = hinv2 * hinv;       // K1: eps2 = h^2
     const uint32_t n = len[t.g];
     const uint32_t *lst = list + (off[t.g] - base);
     sink_acc A;                                               // two-float running sums (see k_m2p)
@@ -180,6 +185,26 @@ __global__ void __launch_bounds__(FW * 32, P2P_MINB) k_p2p(uint32_t t0, uint32_t
             f2 ax = f2_dup(0.0f), ay = f2_dup(0.0f), az = f2_dup(0.0f), pot = f2_dup(0.0f);
             auto pair = [&](const float4 s) {
                 const f2 dx = f2_sub(f2_dup(s.x), X), dy = f2_sub(f2_dup(s.y), Y), dz = f2_sub(f2_dup(s.z), Z);
+                if constexpr (K1) {
+                    f2 r2 = f2_mul(dx, dx);
+                    r2 = f2_fma(dy, dy, r2);
+                    r2 = f2_fma(dz, dz, r2);
+                    const f2 u = f2_mul(r2, f2_dup(hinv2));
+                    const f2 rs = f2_make(rsqrtf(fmaxf(f2_lo(r2), 1e-37f)), rsqrtf(fmaxf(f2_hi(r2), 1e-37f)));
+                    const f2 n3 = f2_mul(f2_mul(rs, rs), rs);
+                    const f2 pf = f2_mul(f2_fma(f2_fma(f2_dup(8.4375f), u, f2_dup(-18.375f)), u, f2_dup(10.9375f)), f2_dup(hinv3));
+                    const bool in_lo = f2_lo(u) < 1.0f, in_hi = f2_hi(u) < 1.0f;
+                    const f2 f = f2_make(in_lo ? f2_lo(pf) : f2_lo(n3), in_hi ? f2_hi(pf) : f2_hi(n3));
+                    const f2 mf = f2_mul(f2_dup(s.w), f);
+                    ax = f2_fma(dx, mf, ax); ay = f2_fma(dy, mf, ay); az = f2_fma(dz, mf, az);
+                    if (POT) {
+                        const f2 pp = f2_mul(f2_fma(f2_fma(f2_fma(f2_dup(-1.40625f), u, f2_dup(4.59375f)), u, f2_dup(-5.46875f)), u, f2_dup(3.28125f)),
+                                             f2_dup(hinv));
+                        const f2 ph = f2_make(in_lo ? f2_lo(pp) : f2_lo(rs), in_hi ? f2_hi(pp) : f2_hi(rs));
+                        pot = f2_sub(pot, f2_mul(f2_dup(s.w), ph));
+                    }
+                    return;
+                }
                 f2 r2 = f2_fma(dx, dx, E2);
                 r2 = f2_fma(dy, dy, r2);
                 r2 = f2_fma(dz, dz, r2);
@@ -211,7 +236,8 @@ __global__ void __launch_bounds__(FW * 32, P2P_MINB) k_p2p(uint32_t t0, uint32_t
     }
     // the sink's own leaf is always in the list: remove its self term -m_i/eps from the potential (once)
     if (POT && t.active && t.sub == 0) {
-        f2_fold(A.hi[3], A.lo[3], f2_make(ma.w * rsqrtf(eps2), mb.w * rsqrtf(eps2)));
+        const float self = K1 ? 3.28125f * hinv : rsqrtf(eps2);          // -m phi(0): m/eps (Plummer), (105/32) m/h (K1)
+        f2_fold(A.hi[3], A.lo[3], f2_make(ma.w * self, mb.w * self));
     }
     __syncwarp();
     task_store(t, A, reinterpret_cast<double *>(src_all[warp][0]), sacc, sacc_lo);
@@ -231,12 +257,15 @@ static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_
         int e = dsk_order_tasks(c, t0, t1, c->g_p2p_src, 6);      // longest first (m2p.cu)
         if (e) return e;
     }
-    if (want_pot)
-        k_p2p<true><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->cell, c->spos, c->gfirst,
-                                           c->gcount, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
-    else
-        k_p2p<false><<<(t1 - t0 + FW - 1) / FW, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->cell, c->spos, c->gfirst,
-                                            c->gcount, c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
+    {
+        const unsigned grid = (t1 - t0 + FW - 1) / FW;
+        auto launch = [&](auto kern) {
+            kern<<<grid, FW * 32, 0, s>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->cell, c->spos, c->gfirst, c->gcount,
+                                          c->list_p2p, c->g_p2p_off, pb, c->g_p2p_len, c->sacc, c->sacc_lo);
+        };
+        if (c->soft_kind == 1) { if (want_pot) launch(k_p2p<true, true>); else launch(k_p2p<false, true>); }
+        else { if (want_pot) launch(k_p2p<true, false>); else launch(k_p2p<false, false>); }
+    }
     cudaEventRecord(c->ev[9], s);
     {
         int e = dsk_launch_m2p(c, t0, t1, mb, want_pot);

@@ -513,7 +513,7 @@ static int launch_m2p_v(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base)
         DSK_CUDA(cudaFuncSetAttribute(k_m2p<P, POT, MODE>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         *attr_done = true;
     }
-    const float e2 = c->eps * c->eps;
+    const float e2 = c->soft_kind == 1 ? 0.0f : c->eps * c->eps;      // K1 (O6b): the accepted cells lie beyond the kernel's support, Newtonian expansion
     const unsigned grid = (t1 - t0 + FW - 1) / FW;
     k_m2p<P, POT, MODE><<<grid, FW * 32, smem, c->stream>>>(t0, t1, c->g_task_sorted, c->periodic, c->box, e2, c->frows, c->spos,
                                                             c->gfirst, c->gcount, c->gcell, c->list_m2p, c->g_m2p_off, base,

@@ -106,7 +106,7 @@ __device__ __forceinline__ uint32_t wk_exposed(bool whole, int lvl, int lb, cons
 // b = sqrt(3)/2 s + delta, kappa_c = (p + 2) Q_c / (tol b^2), i.e. E_c(d) = (p+2) Q b^(p-1) / (d^(p+1) (d-b)^2) <= tol.
 // The MAC record then holds s + delta in .w and kappa_c in the slot of `first` (which the walk does not use).
 template <int MODE, bool ABS>          // MODE 0 COUNT, 1 FILL at the scanned offsets, 2 ONE pass into a fixed capacity per group
-__global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int periodic, float box, int pow1,
+__global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int periodic, float box, int pow1, float k1_h,
                                                   const dsk_cellrec *__restrict__ cell,
                                                   const float4 *__restrict__ wmac,
                                                   const float4 *__restrict__ gbox,
@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
                     float xp = x;
                     for (int k = 1; k < pow1; k++) xp *= x;
                     const float kappa = (top && entry != e[q]) ? bg.kbg[c] : rr[q].x;      // the subtracted copy has its own bound
-                    ok = xp * (d - b) * (d - b) >= kappa;
+                    ok = xp * (d - b) * (d - b) >= kappa && d > b + k1_h;      // k1_h = 0 unless K1 softening (O6b)
                 }
                 accept[q] = !straddles && ok;
                 if (!accept[q]) {
@@ -397,7 +397,9 @@ static void scan64(dsk_ctx *c, const uint32_t *len, uint32_t n, uint64_t *off)
 // the 32 bytes the walk reads per tested cell: centre of mass and critical radius s/theta + delta | the cell record.
 // abs_tol > 0 (absolute-error MAC): critical radius s + delta, and kappa_c = (p + 2) Q_c / (tol b_c^2) in the slot of `first`;
 // kbg[c] = the same for the background-subtracted copy of a top cell, Q' = Q + rho_bar tr C = 2 Q - tr M'.
-__global__ void __launch_bounds__(256) k_walk_mac(uint32_t ncell, float box, float inv_theta, float abs_tol, int p, int rowlen,
+// k1_h > 0 (K1 softening, O6b): the critical radius is at least b + h, b = sqrt(3)/2 s + delta: a cell is expanded only if all its
+// sources lie outside the kernel's support of every sink of the group.
+__global__ void __launch_bounds__(256) k_walk_mac(uint32_t ncell, float box, float inv_theta, float abs_tol, float k1_h, int p, int rowlen,
                                                   const float *__restrict__ rows, uint32_t ntop, const float *__restrict__ rows_bg,
                                                   const dsk_cellrec *__restrict__ cell, const float4 *__restrict__ whdr,
                                                   float4 *__restrict__ wmac, float *__restrict__ kbg)
@@ -408,6 +410,7 @@ __global__ void __launch_bounds__(256) k_walk_mac(uint32_t ncell, float box, flo
     const int level = (int)(cell[c].meta >> 8);
     const float s = box * exp2f((float)-level), delta = h.w;
     h.w = s * inv_theta + delta;
+    if (k1_h > 0.0f && !(abs_tol > 0.0f)) h.w = fmaxf(h.w, 0.8660254f * s + delta + k1_h);     // (the absolute-error walk tests d > b + h itself)
     wmac[2 * (size_t)c] = h;
     // the cell record rides in the same 32-byte sector: a rejected cell needs it, and a second, dependent load would
     // double the latency of every walk iteration
@@ -455,7 +458,7 @@ int dsk_run_walk(dsk_ctx *c)
     cudaEventRecord(c->ev[7], s);
     const uint32_t nc = c->hstate->ncell;
     const bool ABS = c->mac_kind == 1;
-    k_walk_mac<<<(nc + 255) / 256, 256, 0, s>>>(nc, c->box, ABS ? 1.0f : inv_theta, ABS ? c->mac_tol : 0.0f, c->p, dsk_rowlen(c->p), c->rows,
+    k_walk_mac<<<(nc + 255) / 256, 256, 0, s>>>(nc, c->box, ABS ? 1.0f : inv_theta, ABS ? c->mac_tol : 0.0f, c->soft_kind == 1 ? c->eps : 0.0f, c->p, dsk_rowlen(c->p), c->rows,
                                                 c->periodic && c->bg ? c->ntop : 0u, c->rows_bg, c->cell, c->whdr, c->wmac, c->kbg);
     DSK_COUNT(c, 1);
     c->walk_onepass = 0;
@@ -470,7 +473,7 @@ int dsk_run_walk(dsk_ctx *c)
         const uint32_t cm = tiny ? 64u : (uint32_t)(cap_m > 0xffffff00ull ? 0xffffff00ull : cap_m),
                        cp = tiny ? 8u : (uint32_t)(cap_p > 0xffffff00ull ? 0xffffff00ull : cap_p),
                        cl = (uint32_t)(cap_l > 0xffffff00ull ? 0xffffff00ull : cap_l);
-        (ABS ? k_walk<2, true> : k_walk<2, false>)<<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, pow1, c->cell, c->wmac, c->gbox, c->gcount,
+        (ABS ? k_walk<2, true> : k_walk<2, false>)<<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, pow1, c->soft_kind == 1 ? c->eps : 0.0f, c->cell, c->wmac, c->gbox, c->gcount,
                                                          c->g_m2p_len, c->g_p2p_len, c->g_p2p_src, nullptr, nullptr, 0, 0,
                                                          c->list_m2p, c->list_p2p, c->gact_cur, cm, cp, c->g_m2p_off,
                                                          c->g_p2p_off, make_walk_bg(c, 0, cl), c->dstate);
@@ -481,7 +484,7 @@ int dsk_run_walk(dsk_ctx *c)
         if (!ovf) { c->walk_onepass = 1; return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA; }
         c->onepass_bad_theta = c->theta;
     }
-    (ABS ? k_walk<0, true> : k_walk<0, false>)<<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, pow1, c->cell, c->wmac,
+    (ABS ? k_walk<0, true> : k_walk<0, false>)<<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, pow1, c->soft_kind == 1 ? c->eps : 0.0f, c->cell, c->wmac,
                                                      c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len,
                                                      c->g_p2p_src, nullptr, nullptr, 0, 0, nullptr, nullptr,
                                                      c->gact_cur, 0, 0, nullptr, nullptr, make_walk_bg(c, 0, 0), c->dstate);
@@ -495,7 +498,7 @@ int dsk_run_walk(dsk_ctx *c)
 int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base, uint64_t left_base)
 {
     (c->mac_kind == 1 ? k_walk<1, true> : k_walk<1, false>)<<<(g1 - g0 + WW - 1) / WW, WW * 32, 0, c->stream>>>(
-        g0, g1, c->periodic ? c->img_ws : 0, c->box, c->p + 1, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len,
+        g0, g1, c->periodic ? c->img_ws : 0, c->box, c->p + 1, c->soft_kind == 1 ? c->eps : 0.0f, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len,
         c->g_p2p_len, c->g_p2p_src, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p,
         c->gact_cur, 0, 0, nullptr, nullptr, make_walk_bg(c, left_base, 0), c->dstate);
     DSK_COUNT(c, 1);
@@ -539,9 +542,9 @@ int dsk_run_shard(dsk_ctx *c, int rank, int nranks, uint32_t flop_m2p, uint32_t 
     const uint32_t ng = c->hstate->ngroup, nc = c->hstate->ncell;
     cudaStream_t s = c->stream;
     const bool ABS = c->mac_kind == 1;
-    k_walk_mac<<<(nc + 255) / 256, 256, 0, s>>>(nc, c->box, ABS ? 1.0f : 1.0f / c->theta, ABS ? c->mac_tol : 0.0f, c->p, dsk_rowlen(c->p), c->rows,
+    k_walk_mac<<<(nc + 255) / 256, 256, 0, s>>>(nc, c->box, ABS ? 1.0f : 1.0f / c->theta, ABS ? c->mac_tol : 0.0f, c->soft_kind == 1 ? c->eps : 0.0f, c->p, dsk_rowlen(c->p), c->rows,
                                                 c->periodic && c->bg ? c->ntop : 0u, c->rows_bg, c->cell, c->whdr, c->wmac, c->kbg);
-    (ABS ? k_walk<0, true> : k_walk<0, false>)<<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, c->p + 1, c->cell, c->wmac,
+    (ABS ? k_walk<0, true> : k_walk<0, false>)<<<(ng + WW - 1) / WW, WW * 32, 0, s>>>(0, ng, c->periodic ? c->img_ws : 0, c->box, c->p + 1, c->soft_kind == 1 ? c->eps : 0.0f, c->cell, c->wmac,
                                                      c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len,
                                                      c->g_p2p_src, nullptr, nullptr, 0, 0, nullptr, nullptr,
                                                      nullptr, 0, 0, nullptr, nullptr, make_walk_bg(c, 0, 0), c->dstate);

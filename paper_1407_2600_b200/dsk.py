@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libdsk.so")
 
 SYMBOLS = [
     "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
-    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_accel_shard", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_set_background", "dsk_get_background", "dsk_set_image_block", "dsk_get_image_block", "dsk_set_mac", "dsk_get_bg_moments", "dsk_get_keys",
+    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_accel_shard", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_set_background", "dsk_get_background", "dsk_set_image_block", "dsk_get_image_block", "dsk_set_mac", "dsk_set_softening", "dsk_get_bg_moments", "dsk_get_keys",
     "dsk_get_tree", "dsk_get_moments", "dsk_get_moments_scaled", "dsk_get_groups", "dsk_get_stats", "dsk_get_param", "dsk_get_task_widths",
     "dsk_get_lattice_tensors", "dsk_probe_fp32_peak", "dsk_probe_fp32_peak_ex", "dsk_strerror",
 ]
@@ -66,6 +66,7 @@ def load_library(path=LIB_PATH):
     lib.dsk_set_walk_mode.argtypes = [vp, i32]
     lib.dsk_set_background.argtypes = [vp, i32]
     lib.dsk_set_mac.argtypes = [vp, i32, f32]
+    lib.dsk_set_softening.argtypes = [vp, i32, f32]
     lib.dsk_set_image_block.argtypes = [vp, i32]
     lib.dsk_get_image_block.argtypes = [vp, C.POINTER(i32)]
     lib.dsk_get_background.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i64), C.POINTER(f64)]
@@ -227,6 +228,11 @@ class Dsk:
             raise TypeError("rung: contiguous uint8 CUDA tensor [N]")
         _check(self.lib.dsk_kdk_block_step(self._h, _ptr(pos), _ptr(vel), _ptr(mass), C.c_void_p(rung.data_ptr()),
                                            float(a), float(da), int(rmax), float(eta)))
+
+    def set_softening(self, kind="plummer", length=None):
+        """pair softening law: "plummer" (length = eps) or "k1" (Dehnen's K1 kernel, length = its support h)"""
+        self.eps = self.eps if length is None else float(length)
+        _check(self.lib.dsk_set_softening(self._h, {"plummer": 0, "k1": 1}[kind], self.eps))
 
     def set_mac(self, kind="theta", tol=0.0):
         """acceptance rule: "theta" (opening angle) or "abs" (absolute error bound tol per cell interaction)"""

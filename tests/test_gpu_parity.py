@@ -782,6 +782,48 @@ def test_accel_shard_tiles_and_equals_full(dsk, periodic):
     d.close()
 
 
+# ---- Dehnen K1 softening (reading O6b) -------------------------------------------------------------
+@pytest.mark.parametrize("case", ["plummer-sphere", "periodic-clustered", "uniform-large-h"])
+def test_k1_softening_parity(dsk, orc, case):
+    """dsk_set_softening(1, h): forces and potentials against the oracle with the same law (tree) and against its direct sum;
+    structure untouched; both acceptance rules; switching back to Plummer restores the earlier result bit for bit."""
+    if case == "plummer-sphere":
+        pos, mass = workloads.make(2, 1 / 16); periodic, h, theta = False, 4e-4, 0.5
+    elif case == "periodic-clustered":
+        pos, mass = workloads.clustered_box(24, 20, cfg=4); periodic, h, theta = True, 3.0 / 960, 0.6
+    else:                                                  # support larger than the leaves: the d - b > h condition decides many cells
+        pos, mass = workloads.uniform_box(20000); periodic, h, theta = False, 0.08, 0.7
+    n = len(pos)
+    d = dsk.Dsk(n, 1.0, periodic, h, theta, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    plummer = d.accel(tp, tm)[0].clone()
+    sink = workloads.subsample(2, n, 1200)
+    t = orc.OracleTree(pos, mass, 1.0, periodic)
+    with orc.softening("k1"):
+        direct = (orc.direct_per(pos, mass, 1.0, h, sink[:96]) if periodic else orc.direct_iso(pos, mass, h, sink))[0]
+        arms = float(np.sqrt((direct ** 2).sum(1).mean()))
+        d.set_softening("k1", h)
+        for mac in (("theta",), ("abs", 3e-3 * arms)):
+            d.set_mac(*mac)
+            acc, pot = d.accel(tp, tm)
+            a = acc.cpu().numpy().astype(np.float64); ph = pot.cpu().numpy().astype(np.float64)
+            ta, tpot, _, n_m2p, _ = orc.tree_force(pos, mass, 1.0, periodic, h, theta, 4, sink, tree=t, mac=mac)
+            rel = np.linalg.norm(a[sink] - ta, axis=1) / np.linalg.norm(ta, axis=1)
+            assert np.quantile(rel, 0.999) < 1e-4, (case, mac, np.quantile(rel, 0.999))
+            assert np.max(np.abs(ph[sink] - tpot)) < 1e-4 * np.abs(tpot).max() + 1e-6
+            m = len(direct)
+            assert _erms(a[sink[:m]], direct) <= 1.1 * _erms(ta[:m], direct) + 1e-6
+        t.set_mac("theta"); d.set_mac("theta")
+    assert _erms(acc.cpu().numpy().astype(np.float64), plummer.cpu().numpy().astype(np.float64)) > 1e-6     # a different law
+    d.set_softening("plummer", h)
+    again = d.accel(tp, tm)[0]
+    assert torch.equal(again, plummer)
+    with pytest.raises(dsk.DskError):
+        d.set_softening("k1", 0.0)
+    d.close()
+
+
 # ---- absolute-error acceptance rule (reading O5b; PAPER.md:63) ----------------------------------------------------
 @pytest.mark.parametrize("case", ["plummer", "periodic-clustered", "periodic-lattice"])
 def test_abs_mac_parity(dsk, orc, case):
