@@ -231,13 +231,26 @@ extern "C" int dsk_build_tree(dsk_ctx *c, const float *pos, const float *mass)
     c->have_tree = 1;
     e = dsk_run_upward(c);
     if (e) return e;
-    DSK_CUDA(cudaStreamSynchronize(c->stream));
-    c->stats.ms_key = ev_ms(c->ev[0], c->ev[1]);
-    c->stats.ms_sort = ev_ms(c->ev[1], c->ev[2]);
-    c->stats.ms_build = ev_ms(c->ev[2], c->ev[3]);
-    c->stats.ms_group = ev_ms(c->ev[3], c->ev[4]);
-    c->stats.ms_upward = ev_ms(c->ev[5], c->ev[6]);
+    c->pending_build_ms = 3;                 // phase times are read at the next synchronisation anyway due (end of dsk_accel, dsk_get_stats)
     return DSK_OK;
+}
+
+// the stream is synchronised: read the event times that earlier calls left pending
+static void finish_ms(dsk_ctx *c)
+{
+    if (c->pending_build_ms & 1) {
+        c->stats.ms_key = ev_ms(c->ev[0], c->ev[1]);
+        c->stats.ms_sort = ev_ms(c->ev[1], c->ev[2]);
+        c->stats.ms_build = ev_ms(c->ev[2], c->ev[3]);
+        c->stats.ms_group = ev_ms(c->ev[3], c->ev[4]);
+    }
+    if (c->pending_build_ms & 2) c->stats.ms_upward = ev_ms(c->ev[5], c->ev[6]);
+    if (c->pending_force_ms) {
+        if (c->pending_force_ms == 2) c->stats.ms_walk = ev_ms(c->ev[7], c->ev[8]);
+        c->stats.ms_p2p = ev_ms(c->ev[8], c->ev[9]);
+        c->stats.ms_m2p = ev_ms(c->ev[9], c->ev[10]);
+    }
+    c->pending_build_ms = c->pending_force_ms = 0;
 }
 
 // shard_rank >= 0: evaluate only the contiguous run of sink groups that the work-weighted cut gives this rank (dsk_accel_shard)
@@ -252,8 +265,7 @@ static int accel_impl(dsk_ctx *c, const uint8_t *active, float *acc, float *pot,
     if (c->moments_p != c->p) {
         e = dsk_run_upward(c);
         if (e) return e;
-        DSK_CUDA(cudaStreamSynchronize(c->stream));
-        c->stats.ms_upward = ev_ms(c->ev[5], c->ev[6]);
+        c->pending_build_ms |= 2;
     }
     c->gact_cur = nullptr;
     if (active) {                                   // lists of an active subset are never reused
@@ -301,7 +313,8 @@ static int accel_impl(dsk_ctx *c, const uint8_t *active, float *acc, float *pot,
     e = dsk_run_scatter(c, acc, pot, active, r_lo, r_hi);
     if (e) return e;
     cudaEventRecord(c->ev[14], c->stream);
-    e = read_state(c);
+    e = read_state(c);                   // the call's closing synchronisation: every event of this and of the build before it has completed
+    finish_ms(c);
     c->stats.ms_far = ev_ms(c->ev[12], c->ev[13]);
     c->stats.ms_scatter = ev_ms(c->ev[13], c->ev[14]);
     c->stats.n_p2p = (int64_t)c->hstate->n_p2p; c->stats.n_m2p = (int64_t)c->hstate->n_m2p;
@@ -660,6 +673,10 @@ extern "C" int dsk_get_groups(dsk_ctx *c, int64_t *ngroup, uint32_t *first, uint
 extern "C" int dsk_get_stats(dsk_ctx *c, dsk_stats *out)
 {
     if (!c || !out) return DSK_EINVAL;
+    if (c->pending_build_ms || c->pending_force_ms) {
+        DSK_CUDA(cudaStreamSynchronize(c->stream));
+        finish_ms(c);
+    }
     *out = c->stats;
     return DSK_OK;
 }

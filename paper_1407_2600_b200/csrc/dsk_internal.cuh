@@ -198,6 +198,7 @@ struct dsk_ctx {
     float onepass_bad_theta;  // theta at which a list overflowed its fixed capacity (skip the one-pass attempt)
     double far_T[DSK_NFAR];
     dsk_stats stats;
+    int pending_build_ms, pending_force_ms;   // event times not read yet: 1 = the stream has to be synchronised first (dsk_get_stats, end of dsk_accel)
     cudaEvent_t ev[20];
     int nsm;
 };

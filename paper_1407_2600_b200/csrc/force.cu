@@ -295,12 +295,11 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     const uint32_t ng = c->hstate->ngroup;
     const bool reuse = c->lists_valid && c->lists_theta == c->theta;
     c->stats.ms_p2p = c->stats.ms_m2p = 0.0f;
+    c->pending_force_ms = 0;
     if (reuse) {
         int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, 0, want_pot, false);
         if (e) return e;
-        DSK_CUDA(cudaStreamSynchronize(s));
-        add_ms(c->ev[8], c->ev[9], &c->stats.ms_p2p);
-        add_ms(c->ev[9], c->ev[10], &c->stats.ms_m2p);
+        c->pending_force_ms = 1;                      // the event times are read after the call's one closing synchronisation (dsk_api.cu)
         c->stats.ms_walk = 0.0f;
         return DSK_OK;
     }
@@ -308,10 +307,7 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     if (c->walk_onepass) {                        // the lists are already there (walk.cu): one batch, no FILL pass
         int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, 0, want_pot, false);
         if (e) return e;
-        DSK_CUDA(cudaStreamSynchronize(s));
-        add_ms(c->ev[7], c->ev[8], &c->stats.ms_walk);
-        add_ms(c->ev[8], c->ev[9], &c->stats.ms_p2p);
-        add_ms(c->ev[9], c->ev[10], &c->stats.ms_m2p);
+        c->pending_force_ms = 2;
         c->stats.nbatch = 1;
         c->lists_valid = 1; c->lists_theta = c->theta;
         return DSK_OK;
@@ -334,10 +330,7 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     if (tot[0] <= cap_m && tot[1] <= cap_p && tot[2] <= cap_l) {
         int e = eval_batch(c, 0, ng, 0, c->hstate->ntask, 0, 0, 0, want_pot, true);
         if (e) return e;
-        DSK_CUDA(cudaStreamSynchronize(s));
-        add_ms(c->ev[7], c->ev[8], &c->stats.ms_walk);
-        add_ms(c->ev[8], c->ev[9], &c->stats.ms_p2p);
-        add_ms(c->ev[9], c->ev[10], &c->stats.ms_m2p);
+        c->pending_force_ms = 2;
         c->stats.nbatch = 1;
         c->lists_valid = 1; c->lists_theta = c->theta;
         return DSK_OK;
