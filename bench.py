@@ -433,7 +433,8 @@ def probe_peak():
     """dsk_probe_fp32_peak, all three operand forms (include/dsk.h): the measured FP32 denominator."""
     from paper_1407_2600_b200 import dsk
     forms = ("ffma2_three_packed_operands", "ffma2_one_scalar_broadcast_operand", "scalar_ffma_three_registers",
-             "ffma2_sources_repeated", "scalar_ffma_sources_repeated")
+             "ffma2_sources_repeated", "scalar_ffma_sources_repeated", "ffma2_m2p_pattern_new_scalar_each",
+             "ffma2_m2p_pattern_scalar_used_twice")
     res = {}
     for v, name in enumerate(forms):
         t, c, m, tc = dsk.probe_fp32_peak_ex(v)

@@ -216,7 +216,8 @@ int dsk_get_lattice_tensors(dsk_ctx *ctx, double *T /* host [165] */);
  * sub-partition, and the SM clock in MHz the kernel ran at.  variant 0: packed fma.rn.f32x2 with three register operands;
  * 1: packed, one operand a scalar broadcast to both halves (the form the force kernels feed sources in); 2: scalar FFMA
  * with three distinct registers; 3 and 4: packed and scalar with the two source operands repeated from one instruction to
- * the next (operand-reuse cache; 0-2 are register-bandwidth bound).  DSK_EINVAL for another variant or a NULL pointer,
+ * the next (operand-reuse cache; 0-2 are register-bandwidth bound); 5 and 6: the M2P body's pattern, a new scalar coefficient
+ * every instruction / every second instruction.  DSK_EINVAL for another variant or a NULL pointer,
  * DSK_ECUDA without a device. */
 int dsk_probe_fp32_peak(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz);
 /* the same, plus TFLOP/s as implied by the SMs' own cycle counters and clock (cross-check of the event timing) */

@@ -7,6 +7,8 @@
 //   variant 2  scalar FFMA, three distinct registers                  a = fma(x, y, a)
 //   variant 3  FFMA2, the two source operands shared by all chains    a_k = fma(a_k, {s,s}, y)   (operand-reuse cache hits)
 //   variant 4  scalar FFMA, the two source operands shared            a_k = fma(a_k, s, y)
+//   variant 5  the M2P body's pattern: a_k = fma({s_i,s_i}, m_k, a_k), a new scalar s_i every instruction, m_k and a_k distinct
+//   variant 6  the same with each scalar used by TWO consecutive instructions (what four sinks per lane would give)
 // Variants 0-2 read five or six, three distinct registers per instruction and are bound by register-file bandwidth (measured:
 // one FFMA2 per 2.6 - 3.0 cycles, one FFMA per 1.5); 3 and 4 show what the pipe itself issues when operands repeat, which is
 // what a real inner loop (one coefficient against many monomials) looks like.
@@ -35,7 +37,23 @@ __global__ void __launch_bounds__(PK_THREADS, PK_BLOCKS_PER_SM) k_fp32_peak(int 
     const unsigned long long t0 = pk_globaltimer();
     const long long c0 = clock64();
     float res = 0.0f;
-    if (VARIANT == 4) {
+    if (VARIANT == 5 || VARIANT == 6) {
+        f2 a[PK_CHAINS], m[PK_CHAINS];
+        float sc[PK_CHAINS];
+#pragma unroll
+        for (int k = 0; k < PK_CHAINS; k++) {
+            a[k] = f2_make(s0 + (float)k, s1 + (float)k);
+            m[k] = f2_make(s1 * 1e-3f + 1e-4f * (float)(k + threadIdx.x), s0 * 1e-3f + 2e-4f * (float)k);
+            sc[k] = s1 * 0.5f + 1e-3f * (float)k;
+        }
+        for (int it = 0; it < iters; it++)
+#pragma unroll
+            for (int u = 0; u < PK_UNROLL; u++)
+#pragma unroll
+                for (int k = 0; k < PK_CHAINS; k++) a[k] = f2_fma(f2_dup(sc[VARIANT == 5 ? k : (k >> 1)]), m[k], a[k]);
+#pragma unroll
+        for (int k = 0; k < PK_CHAINS; k++) res += f2_lo(a[k]) + f2_hi(a[k]);
+    } else if (VARIANT == 4) {
         float a[PK_CHAINS];
         const float x = s1 + 1e-3f * (float)threadIdx.x, y = s0 * 0.5f;
 #pragma unroll
@@ -101,7 +119,7 @@ extern "C" int dsk_probe_fp32_peak_ex(int variant, double *tflops, double *cycle
 }
 static int probe_impl(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz, double *tflops_by_cycles)
 {
-    if (variant < 0 || variant > 4 || !tflops || !cycles_per_inst_smsp || !sm_mhz) return DSK_EINVAL;
+    if (variant < 0 || variant > 6 || !tflops || !cycles_per_inst_smsp || !sm_mhz) return DSK_EINVAL;
     int dev = 0, nsm = 0;
     DSK_CUDA(cudaGetDevice(&dev));
     DSK_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
@@ -123,7 +141,9 @@ static int probe_impl(int variant, double *tflops, double *cycles_per_inst_smsp,
         else if (variant == 1) k_fp32_peak<1><<<grid, PK_THREADS>>>(iters, seed, out, clk);
         else if (variant == 2) k_fp32_peak<2><<<grid, PK_THREADS>>>(iters, seed, out, clk);
         else if (variant == 3) k_fp32_peak<3><<<grid, PK_THREADS>>>(iters, seed, out, clk);
-        else k_fp32_peak<4><<<grid, PK_THREADS>>>(iters, seed, out, clk);
+        else if (variant == 4) k_fp32_peak<4><<<grid, PK_THREADS>>>(iters, seed, out, clk);
+        else if (variant == 5) k_fp32_peak<5><<<grid, PK_THREADS>>>(iters, seed, out, clk);
+        else k_fp32_peak<6><<<grid, PK_THREADS>>>(iters, seed, out, clk);
         cudaEventRecord(e1);
         if (cudaEventSynchronize(e1) != cudaSuccess) break;
         float ms = 0.0f;

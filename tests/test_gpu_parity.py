@@ -538,12 +538,12 @@ def test_error_cell_overflow_and_recovery(dsk, orc):
 
 def test_fp32_peak_probe(dsk):
     """dsk_probe_fp32_peak returns a plausible issue rate for each operand form (the roofline's measured denominator)."""
-    r = [dsk.probe_fp32_peak(v) for v in (0, 1, 2, 3, 4)]
+    r = [dsk.probe_fp32_peak(v) for v in range(7)]
     for tf, cyc, mhz in r:
         assert 500.0 < mhz < 2500.0 and 0.9 < cyc < 6.0 and 10.0 < tf < 85.0, r
     assert max(x[0] for x in r) > 0.6 * 148 * 128 * 2 * r[0][2] * 1e6 / 1e12        # some form gets within reach of 2 flop/lane/clock
     with pytest.raises(dsk.DskError):
-        dsk.probe_fp32_peak(5)
+        dsk.probe_fp32_peak(7)
 
 
 # ---- forces, periodic ---------------------------------------------------------------------------------
