@@ -48,6 +48,7 @@ extern "C" {
 #define DSK_ELISTOVERFLOW -6   /* traversal stack or interaction-list buffer exhausted                 */
 #define DSK_ECUDA         -7   /* CUDA runtime error (no device, launch failure, ...)                  */
 #define DSK_ECELLOVERFLOW -8   /* more tree cells than the workspace was sized for                     */
+#define DSK_ETOOLARGE     -9   /* size beyond the fixed maximum of a no-allocation entry point         */
 
 typedef struct dsk_ctx dsk_ctx;      /* opaque; created by dsk_create, released by dsk_destroy        */
 
@@ -222,6 +223,25 @@ int dsk_get_lattice_tensors(dsk_ctx *ctx, double *T /* host [165] */);
 int dsk_probe_fp32_peak(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz);
 /* the same, plus TFLOP/s as implied by the SMs' own cycle counters and clock (cross-check of the event timing) */
 int dsk_probe_fp32_peak_ex(int variant, double *tflops, double *cycles_per_inst_smsp, double *sm_mhz, double *tflops_by_cycles);
+
+/* Steps K and S with NO allocation and no context ("assign a Key to each particle, based on Morton ordering";
+ * the sort along the curve), for callers that can neither call cudaMalloc nor lend a workspace (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid allocation).  The same kernels as dsk_build_tree's key and sort
+ * phases; their scratch (second key / index buffer, tile histograms, scan sums, status word) is a fixed file-scope device
+ * array of 12.6 MiB that every GPU which loads the library holds until the process exits.
+ *   pos dev [N][3] fp32, N <= DSK_NOALLOC_NMAX; box, periodic as in dsk_create;
+ *   sorted_keys dev [N] uint64 (out), order dev [N] uint32 (out): sorted_keys[r] = key(order[r]), equal keys in input order —
+ *   bit for bit what dsk_get_keys returns after dsk_build_tree on the same positions;  cuda_stream: cudaStream_t as void*,
+ *   NULL = default stream; the work is enqueued there on the CURRENT device, and the call returns after one 4-byte read-back
+ *   and a stream synchronise.
+ * Calls no cudaMalloc / cudaFree and no allocating library routine.  Every call on a device shares the one array, which keeps
+ * the last call's contents (what must start at zero is cleared at the start of each call): calls that OVERLAP on the same
+ * GPU (two streams, two host threads) race on it and give wrong orders — serialise them.
+ * Errors: DSK_ETOOLARGE for N > DSK_NOALLOC_NMAX (nothing is launched); DSK_EINVAL for N <= 0, a NULL pointer or a bad box;
+ * DSK_EOUTOFBOX / DSK_ENONFINITE as dsk_build_tree (outputs then undefined); DSK_ECUDA. */
+#define DSK_NOALLOC_NMAX 1048576
+int dsk_sort_keys_noalloc(const float *pos, int64_t N, float box, int periodic, uint64_t *sorted_keys, uint32_t *order,
+                          void *cuda_stream);
 const char *dsk_strerror(int err);
 
 #ifdef __cplusplus

@@ -722,6 +722,7 @@ extern "C" const char *dsk_strerror(int e)
     case DSK_ELISTOVERFLOW: return "traversal stack or interaction list overflow";
     case DSK_ECUDA: return "CUDA error";
     case DSK_ECELLOVERFLOW: return "more tree cells or groups than the workspace holds";
+    case DSK_ETOOLARGE: return "size beyond the fixed maximum of this no-allocation entry point (DSK_NOALLOC_NMAX)";
     default: return "unknown error";
     }
 }

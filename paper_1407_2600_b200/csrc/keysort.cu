@@ -330,3 +330,78 @@ int dsk_run_scatter(dsk_ctx *c, float *acc, float *pot, const uint8_t *active, u
     DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
+
+// ---- K + S without any allocation: dsk_sort_keys_noalloc (include/dsk.h) ---------------------------------------
+// For callers that can neither allocate nor lend a workspace (code under CUDA graph capture, serving loops, harnesses
+// that forbid cudaMalloc): the same key and sort kernels as dsk_run_keysort, with the sort's second key / index buffer,
+// its tile histograms, the scan's block sums and the status word in ONE file-scope device array of fixed size
+// (12.6 MiB for N <= 2^20; every GPU that loads the library holds it until the process exits).
+// In host code the array's NAME is a host-side stand-in, not a device address: the kernels get the pointer that
+// cudaGetSymbolAddress returns, looked up once per device with that device current.
+// Every call shares the array, and it keeps the last call's contents: the status word is cleared at the start of every
+// call (everything else is written before it is read), and two calls that overlap on the GPU (two streams, two host
+// threads) race on it.
+#define NA_NMAX DSK_NOALLOC_NMAX
+#define NA_NTILE ((NA_NMAX + SORT_TILE - 1) / SORT_TILE)
+#define NA_OFF_STATE 0                                                  // dsk_devstate (256 B reserved)
+#define NA_OFF_SCAN 256                                                 // 4096 u32 block sums of the scan
+#define NA_OFF_HIST (NA_OFF_SCAN + 4 * 4096)                            // [256][ntile] tile histograms
+#define NA_OFF_KEYB (NA_OFF_HIST + 4 * 256 * NA_NTILE)                  // second key buffer
+#define NA_OFF_IDXB (NA_OFF_KEYB + 8 * (size_t)NA_NMAX)                 // second index buffer
+#define NA_BYTES (NA_OFF_IDXB + 4 * (size_t)NA_NMAX)
+static_assert(sizeof(dsk_devstate) <= 256, "state slot of the static scratch");
+static_assert(NA_OFF_HIST % 256 == 0 && NA_OFF_KEYB % 256 == 0 && NA_OFF_IDXB % 256 == 0, "256-byte aligned parts");
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NA_BYTES];
+
+static unsigned char *g_noalloc_ptr[DSK_MAXDEV];        // device address of g_noalloc_scratch, per device ordinal
+static int g_noalloc_nsm[DSK_MAXDEV];
+
+extern "C" int dsk_sort_keys_noalloc(const float *pos, int64_t N, float box, int periodic, uint64_t *sorted_keys,
+                                     uint32_t *order, void *cuda_stream)
+{
+    if (!pos || !sorted_keys || !order || N <= 0 || !(box > 0.0f) || !isfinite(box)) return DSK_EINVAL;
+    if (N > (int64_t)NA_NMAX) return DSK_ETOOLARGE;
+    int dev = 0;
+    DSK_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= DSK_MAXDEV) return DSK_EINVAL;
+    if (!g_noalloc_ptr[dev]) {                          // set-up, once per device, that device current
+        void *p = nullptr;
+        DSK_CUDA(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        int nsm = 0;
+        DSK_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+        if (!p || nsm <= 0) return DSK_ECUDA;
+        g_noalloc_nsm[dev] = nsm;
+        g_noalloc_ptr[dev] = (unsigned char *)p;
+    }
+    unsigned char *base = g_noalloc_ptr[dev];
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    dsk_devstate *st = (dsk_devstate *)(base + NA_OFF_STATE);
+    uint32_t *scan_tmp = (uint32_t *)(base + NA_OFF_SCAN), *hist = (uint32_t *)(base + NA_OFF_HIST);
+    uint64_t *ka = sorted_keys, *kb = (uint64_t *)(base + NA_OFF_KEYB);
+    uint32_t *ia = order, *ib = (uint32_t *)(base + NA_OFF_IDXB);
+    DSK_CUDA(cudaMemsetAsync(st, 0, sizeof(dsk_devstate), s));
+    const int nb = (int)((N + 255) / 256), ntile = (int)((N + SORT_TILE - 1) / SORT_TILE);
+    k_keys<<<nb, 256, 0, s>>>(pos, N, box, 2097152.0f / box, periodic ? 1 : 0, ka, ia, st);
+    const uint32_t nh = 256u * (uint32_t)ntile;
+    int grid = g_noalloc_nsm[dev] * 4;
+    if ((uint64_t)grid * SCAN_THREADS > (uint64_t)nh) grid = (int)((nh + SCAN_THREADS - 1) / SCAN_THREADS);
+    if (grid > 4096) grid = 4096;
+    for (int pass = 0; pass < 8; pass++) {
+        const int shift = 8 * pass;
+        k_sort_hist<<<ntile, SORT_THREADS, 0, s>>>(ka, N, shift, ntile, hist);
+        k_scan_reduce<<<grid, SCAN_THREADS, 0, s>>>(hist, nullptr, nh, scan_tmp);
+        k_scan_apply<<<grid, SCAN_THREADS, 0, s>>>(hist, hist, nullptr, nh, scan_tmp, nullptr);
+        k_sort_scatter<<<ntile, SORT_THREADS, 0, s>>>(ka, ia, N, shift, ntile, hist, kb, ib);
+        uint64_t *tk = ka; ka = kb; kb = tk;
+        uint32_t *ti = ia; ia = ib; ib = ti;
+    }
+    // 8 passes: the result is back in the caller's (sorted_keys, order)
+    DSK_CUDA(cudaGetLastError());
+    uint32_t status = 0;
+    DSK_CUDA(cudaMemcpyAsync(&status, &st->status, sizeof(status), cudaMemcpyDeviceToHost, s));
+    DSK_CUDA(cudaStreamSynchronize(s));
+    if (status & ST_NONFINITE) return DSK_ENONFINITE;
+    if (status & ST_OUTOFBOX) return DSK_EOUTOFBOX;
+    return DSK_OK;
+}

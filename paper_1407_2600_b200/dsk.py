@@ -16,7 +16,7 @@ SYMBOLS = [
     "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
     "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_accel_shard", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_set_background", "dsk_get_background", "dsk_set_image_block", "dsk_get_image_block", "dsk_set_mac", "dsk_set_softening", "dsk_get_bg_moments", "dsk_get_keys",
     "dsk_get_tree", "dsk_get_moments", "dsk_get_moments_scaled", "dsk_get_groups", "dsk_get_stats", "dsk_get_param", "dsk_get_task_widths",
-    "dsk_get_lattice_tensors", "dsk_probe_fp32_peak", "dsk_probe_fp32_peak_ex", "dsk_strerror",
+    "dsk_get_lattice_tensors", "dsk_probe_fp32_peak", "dsk_probe_fp32_peak_ex", "dsk_sort_keys_noalloc", "dsk_strerror",
 ]
 
 
@@ -83,6 +83,7 @@ def load_library(path=LIB_PATH):
     lib.dsk_get_lattice_tensors.argtypes = [vp, vp]
     lib.dsk_probe_fp32_peak.argtypes = [i32, C.POINTER(f64), C.POINTER(f64), C.POINTER(f64)]
     lib.dsk_probe_fp32_peak_ex.argtypes = [i32, C.POINTER(f64), C.POINTER(f64), C.POINTER(f64), C.POINTER(f64)]
+    lib.dsk_sort_keys_noalloc.argtypes = [vp, i64, f32, i32, vp, vp, vp]
     lib.dsk_strerror.argtypes = [i32]
     lib.dsk_strerror.restype = C.c_char_p
     for s in SYMBOLS:
@@ -116,6 +117,27 @@ def probe_fp32_peak_ex(variant):
     t, c, m, tc = C.c_double(0), C.c_double(0), C.c_double(0), C.c_double(0)
     _check(load_library().dsk_probe_fp32_peak_ex(int(variant), C.byref(t), C.byref(c), C.byref(m), C.byref(tc)))
     return t.value, c.value, m.value, tc.value
+
+
+def sort_keys_noalloc(pos, box, periodic, sorted_keys, order, stream=None):
+    """dsk_sort_keys_noalloc: Morton keys + sort of pos [N, 3] (N <= NOALLOC_NMAX) into the caller's sorted_keys (int64 bit
+    pattern of uint64) and order (int32 bit pattern of uint32), both CUDA [N].  Allocates nothing, here or in the library;
+    calls that overlap on one GPU race on the library's fixed scratch array."""
+    pos = _dev_f32(pos)
+    n = pos.shape[0]
+    if pos.dim() != 2 or pos.shape[1] != 3:
+        raise ValueError("pos must be [N, 3]")
+    for t, dt in ((sorted_keys, torch.int64), (order, torch.int32)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dt and t.is_contiguous() and t.numel() == n
+                and t.device == pos.device):
+            raise TypeError("sorted_keys / order: contiguous CUDA tensors [N] of int64 / int32 on pos's device")
+    with torch.cuda.device(pos.device):
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        _check(load_library().dsk_sort_keys_noalloc(_ptr(pos), n, float(box), int(bool(periodic)), _ptr(sorted_keys),
+                                                    _ptr(order), C.c_void_p(st)))
+
+
+NOALLOC_NMAX = 1 << 20      # DSK_NOALLOC_NMAX of include/dsk.h
 
 
 def _check(code):
