@@ -197,6 +197,8 @@ def measure_config(cfgid, steps, warmup, dev, world, rank, dist, want_e2e, want_
     pos, mass = workloads.make(cfgid)
     n = len(pos)
     d = dsk.Dsk(n, cfg["box"], cfg["periodic"], cfg["eps"], cfg["theta"], cfg["p"], device=dev)
+    if os.environ.get("DSK_WALK_SHARING"):          # experiments: groups per shared walk (dsk_set_walk_sharing); default = the library's choice
+        d.set_walk_sharing(int(os.environ["DSK_WALK_SHARING"]))
     stream = torch.cuda.current_stream(dev)
     tp, tm = torch.from_numpy(pos).to(dev), torch.from_numpy(mass).to(dev)
     acc = torch.empty((n, 3), dtype=torch.float32, device=dev)

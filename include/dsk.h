@@ -169,6 +169,16 @@ int dsk_get_bg_moments(dsk_ctx *ctx, float *moments);
  * lists are longer cannot be evaluated and dsk_accel returns DSK_ELISTOVERFLOW (the context stays usable). */
 int dsk_set_walk_mode(dsk_ctx *ctx, int mode);
 
+/* The walk variant (second half; "bundle a set of m source cells which have interactions in
+ * common with a set of n sink particles"): up to `groups` consecutive sink groups (neighbours along the Morton curve, and, with
+ * background subtraction, of one window) are walked by one warp.  Against the union of their boxes it lists once, for all of them,
+ * every cell the union accepts, opens once every cell all of them reject, and sets aside the cells they disagree on, which each
+ * group then walks by itself.  Every group's lists hold exactly the entries a walk of its own would give, in another order, so the
+ * forces differ by fp32 summation order only.  groups = 1: every group walks alone; 2..8: share; 0 (default): as many (<= 8) as
+ * leave every SM 16 walks.  Sharded, batched and active-subset evaluations list a group's entries in the same order as a full one
+ * (the sets are formed from the group indices, not from what is evaluated).  DSK_EINVAL outside 0..8. */
+int dsk_set_walk_sharing(dsk_ctx *ctx, int groups);
+
 /* One BLOCK step of size da with hierarchical individual time steps (reading O9c of DESIGN.md; "adaptive
  * symplectic integrator (Quinn et al. 1997)").  rung dev uint8 [N], in/out: particle i takes steps of da / 2^rung[i],
  * 0 <= rung <= rmax <= 8 (a larger entry is read as rmax and written back clamped).  The block is cut into 2^rmax substeps; per substep: opening half kicks of the particles whose

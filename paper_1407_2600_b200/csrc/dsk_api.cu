@@ -489,6 +489,14 @@ extern "C" int dsk_set_walk_mode(dsk_ctx *c, int mode)
     return DSK_OK;
 }
 
+extern "C" int dsk_set_walk_sharing(dsk_ctx *c, int groups)
+{
+    if (!c || groups < 0 || groups > 8) return DSK_EINVAL;
+    c->walk_share = groups;
+    c->lists_valid = 0;
+    return DSK_OK;
+}
+
 extern "C" int dsk_kdk_reset(dsk_ctx *c)
 {
     if (!c) return DSK_EINVAL;

@@ -404,14 +404,16 @@ def test_forces_random_small_cases(dsk, orc, seed):
     d.close()
 
 
+@pytest.mark.parametrize("share", [1, 8])
 @pytest.mark.parametrize("periodic", [False, True])
-def test_accel_active_subset(dsk, orc, periodic):
+def test_accel_active_subset(dsk, orc, periodic, share):
     """dsk_accel_active: forces of an active subset (every particle still a source) equal the full evaluation's
     for the active particles bit for bit, inactive entries stay untouched, and the work shrinks with the subset."""
     pos, mass = (workloads.clustered_box(24, 20, cfg=4) if periodic else workloads.make(2, 1 / 32))
     n = len(pos)
     eps = 1e-3
     d = dsk.Dsk(n, 1.0, periodic, eps, 0.5, 4)
+    d.set_walk_sharing(share)          # 1: every group walks alone; 8: neighbouring groups share a walk (dsk_set_walk_sharing)
     tp, tm = _dev(pos), _dev(mass)
     d.build_tree(tp, tm)
     full, fpot = d.accel(tp, tm)
@@ -441,13 +443,15 @@ def test_accel_active_subset(dsk, orc, periodic):
     d.close()
 
 
+@pytest.mark.parametrize("share", [1, 8])
 @pytest.mark.parametrize("periodic", [False, True])
-def test_walk_one_pass_equals_two_pass(dsk, periodic):
+def test_walk_one_pass_equals_two_pass(dsk, periodic, share):
     """The one-pass walk (fixed list capacity per group) and the COUNT + FILL form give the same lists: forces,
     potentials and interaction counts are bit-identical."""
     pos, mass = (workloads.clustered_box(24, 20, cfg=4) if periodic else workloads.make(2, 1 / 16))
     n = len(pos)
     d = dsk.Dsk(n, 1.0, periodic, 1e-3, 0.4, 4)
+    d.set_walk_sharing(share)          # 1: every group walks alone; 8: neighbouring groups share a walk (dsk_set_walk_sharing)
     tp, tm = _dev(pos), _dev(mass)
     d.build_tree(tp, tm)
     a1, p1 = d.accel(tp, tm)
@@ -465,13 +469,15 @@ def test_walk_one_pass_equals_two_pass(dsk, periodic):
     d.close()
 
 
+@pytest.mark.parametrize("share", [1, 8])
 @pytest.mark.parametrize("periodic", [False, True])
-def test_walk_batches_equal_one_batch(dsk, periodic):
+def test_walk_batches_equal_one_batch(dsk, periodic, share):
     """dsk_set_walk_mode(3): the list buffers are treated as holding 65536 / 8192 entries, so this small input takes the
     batched COUNT + FILL + evaluate path of a 512^3 run (several batches of groups): bit-identical results."""
     pos, mass = (workloads.clustered_box(24, 20, cfg=4) if periodic else workloads.make(2, 1 / 16))
     n = len(pos)
     d = dsk.Dsk(n, 1.0, periodic, 1e-3, 0.5, 4)
+    d.set_walk_sharing(share)          # 1: every group walks alone; 8: neighbouring groups share a walk (dsk_set_walk_sharing)
     tp, tm = _dev(pos), _dev(mass)
     d.build_tree(tp, tm)
     a1, p1 = d.accel(tp, tm)
@@ -483,6 +489,79 @@ def test_walk_batches_equal_one_batch(dsk, periodic):
     assert torch.equal(a1, a2) and torch.equal(p1, p2)
     assert s1["n_m2p"] == s2["n_m2p"] and s1["n_p2p"] == s2["n_p2p"] and s1["list_m2p"] == s2["list_m2p"]
     d.close()
+
+
+SHARED_WALK_CASES = {
+    "plummer": (lambda: workloads.make(2, 1 / 16), False, 1e-3, 0.5, 4, {}),
+    "plummer-theta0.3": (lambda: workloads.make(2, 1 / 8), False, 1e-4, 0.3, 2, {}),
+    "periodic-clustered": (lambda: workloads.clustered_box(32, 40, cfg=4), True, 1e-3, 0.5, 4, {}),
+    "periodic-lattice": (lambda: workloads.perturbed_lattice(32), True, 1e-3, 0.5, 4, {}),
+    "periodic-clustered-theta1": (lambda: workloads.clustered_box(40, 60, cfg=4), True, 5e-4, 1.0, 4, {}),
+    "periodic-clustered-abs": (lambda: workloads.clustered_box(32, 40, cfg=4), True, 1e-3, 0.5, 2, {"mac": 1e-3}),
+    "periodic-clustered-ws2": (lambda: workloads.clustered_box(32, 40, cfg=4), True, 1e-3, 0.5, 4, {"ws": 2}),
+    "periodic-clustered-nobg": (lambda: workloads.clustered_box(32, 40, cfg=4), True, 1e-3, 0.5, 4, {"bg": 0}),
+    "periodic-clustered-k1": (lambda: workloads.clustered_box(32, 40, cfg=4), True, 3e-3, 0.5, 4, {"k1": 1}),
+}
+
+
+@pytest.mark.parametrize("case", list(SHARED_WALK_CASES))
+def test_shared_walk_lists_equal_lone_walk(dsk, orc, case):
+    """dsk_set_walk_sharing (second half): 2, 3 or 8 neighbouring groups walked by one warp
+    (common cells listed once for all, the rest group by group) get exactly the lists of their own walks - every group's list
+    lengths and source counts are identical, the kept cubes too - in another order: forces agree to fp32 summation order, and
+    the shared walk meets the parity bar against the oracle tree by itself."""
+    mk, periodic, eps, theta, p, opt = SHARED_WALK_CASES[case]
+    pos, mass = mk()
+    n = len(pos)
+    d = dsk.Dsk(n, 1.0, periodic, eps, theta, p)
+    if "ws" in opt:
+        d.set_image_block(opt["ws"])
+    if "bg" in opt:
+        d.set_background(opt["bg"])
+    if "k1" in opt:
+        d.set_softening("k1", eps)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    d.set_walk_sharing(1)
+    mac = None
+    if "mac" in opt:
+        a0, _ = d.accel(tp, tm)
+        mac = opt["mac"] * float(a0.double().pow(2).sum(1).mean().sqrt())
+        d.set_mac("abs", mac)
+    a1, p1 = d.accel(tp, tm)
+    s1, g1 = d.get_stats(), d.get_groups()
+    for share in (2, 3, 8):
+        d.set_walk_sharing(share)
+        a, ph = d.accel(tp, tm)
+        st, g = d.get_stats(), d.get_groups()
+        assert torch.equal(g["m2p_len"], g1["m2p_len"]) and torch.equal(g["p2p_len"], g1["p2p_len"]), (case, share)
+        for k in ("n_m2p", "n_p2p", "list_m2p", "list_p2p", "list_bg"):
+            assert st[k] == s1[k], (case, share, k)
+        rel = ((a - a1).norm(dim=1) / a1.norm(dim=1)).cpu().numpy()
+        # summation order only: 1e-6 of the force - except on the near-lattice, whose forces are what is left of sums 100 x
+        # larger (DESIGN.md section 4), where order alone moves them by a good part of the parity bar
+        tol = (1e-4, 1e-3) if case == "periodic-lattice" else (5e-6, 1e-4)
+        assert np.quantile(rel, 0.999) < tol[0] and rel.max() < tol[1], (case, share, np.quantile(rel, 0.999), rel.max())
+        assert float((ph - p1).abs().max() / p1.abs().max()) < 2.0 * tol[0]
+    # the shared walk (8) against the oracle tree
+    sink = np.arange(0, n, max(1, n // 300))
+    kw = {}
+    if "ws" in opt:
+        kw["ws"] = opt["ws"]
+    if "bg" in opt:
+        kw["bg"] = bool(opt["bg"])
+    if mac is not None:
+        kw["mac"] = ("abs", mac)
+    if "k1" in opt:
+        with orc.softening("k1"):
+            ref = orc.tree_force(pos, mass, 1.0, periodic, eps, theta, p, sink, **kw)[0]
+    else:
+        ref = orc.tree_force(pos, mass, 1.0, periodic, eps, theta, p, sink, **kw)[0]
+    acc = a.cpu().numpy().astype(np.float64)[sink]
+    rel = np.linalg.norm(acc - ref, axis=1) / np.linalg.norm(ref, axis=1)
+    assert np.quantile(rel, 0.999) < 1e-4, (case, np.quantile(rel, 0.999))
+    d.close()
+
 
 
 def test_error_list_overflow_and_recovery(dsk):
@@ -751,8 +830,9 @@ def test_image_block_one_and_two(dsk, orc, case):
     d.close()
 
 
+@pytest.mark.parametrize("share", [1, 8])
 @pytest.mark.parametrize("periodic", [False, True])
-def test_accel_shard_tiles_and_equals_full(dsk, periodic):
+def test_accel_shard_tiles_and_equals_full(dsk, periodic, share):
     """dsk_accel_shard: for 2, 3 and 7 ranks the runs of sink groups tile all groups, the shards written one
     after the other into one zero-filled array reproduce the full evaluation bit for bit, and the work (cell interactions of
     each shard) is balanced; the device's cut equals the host statement of the rule when the lists are those of the full walk."""
@@ -760,6 +840,7 @@ def test_accel_shard_tiles_and_equals_full(dsk, periodic):
     pos, mass = (workloads.clustered_box(28, 20, cfg=4) if periodic else workloads.make(2, 1 / 16))
     n = len(pos)
     d = dsk.Dsk(n, 1.0, periodic, 1e-3, 0.5, 4)
+    d.set_walk_sharing(share)          # 1: every group walks alone; 8: neighbouring groups share a walk (dsk_set_walk_sharing)
     tp, tm = _dev(pos), _dev(mass)
     d.build_tree(tp, tm)
     full, fpot = d.accel(tp, tm)
