@@ -128,6 +128,9 @@ int dsk_kdk_reset(dsk_ctx *ctx);
  * cubes that stick out of it is summed exactly (closed-form field of a homogeneous cuboid); the far field acts on the
  * neutral box.  ON BY DEFAULT in a periodic context; on = 0 restores plain particle moments with the neutralising
  * background in the far field alone (and fp64 monopoles).
+ * The window's field is summed by the series of the cube's interior potential about its centre where the sinks sit well inside
+ * the window (within 0.36 of its half-width: every group at or below level l_b), by the closed form elsewhere; on = 2
+ * (diagnostic) uses the closed form everywhere - the results agree to the rounding of the fp32 accumulators.
  * DSK_EINVAL for on != 0 in an isolated context.  Changing it invalidates moments, lists and the cached KDK force. */
 int dsk_set_background(dsk_ctx *ctx, int on);
 /* Pair softening law.  kind 0 (default): Plummer, phi = -m (r^2 + eps^2)^(-1/2), length = eps (the same as dsk_set_params' eps).

@@ -10,7 +10,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = ["dsk_api.cu", "keysort.cu", "tree.cu", "upward.cu", "walk.cu", "force.cu", "m2p.cu", "farfield.cu", "background.cu", "kdk.cu", "peak.cu"]
-HEADERS = [os.path.join(CSRC, "dsk_internal.cuh"), os.path.join(CSRC, "force_task.cuh"), os.path.join(HERE, "..", "include", "dsk.h")]
+HEADERS = [os.path.join(CSRC, "dsk_internal.cuh"), os.path.join(CSRC, "force_task.cuh"), os.path.join(CSRC, "cube_series.inc"), os.path.join(HERE, "..", "include", "dsk.h")]
 LIB = os.path.join(HERE, "libdsk.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -446,7 +446,9 @@ extern "C" int dsk_set_background(dsk_ctx *c, int on)
     if (!c) return DSK_EINVAL;
     if (on && !c->periodic) return DSK_EINVAL;
     if ((on != 0) != (c->bg != 0)) { c->moments_p = -1; c->lists_valid = 0; c->kdk_have_acc = 0; }   // rows and lists depend on it
+    if (c->bg_closed != (on == 2)) c->kdk_have_acc = 0;
     c->bg = on ? 1 : 0;
+    c->bg_closed = on == 2;
     return DSK_OK;
 }
 

@@ -194,6 +194,7 @@ struct dsk_ctx {
     float mac_tol;
     float lists_theta;
     int walk_two_pass_only;   // dsk_set_walk_mode(1)
+    int bg_closed;            // dsk_set_background(2): the windows' background by the closed form everywhere (diagnostic)
     int walk_share;           // dsk_set_walk_sharing: groups per shared walk (0 = automatic)
     int walk_onepass;         // the lists of the current evaluation were written by the one-pass walk
     float onepass_bad_theta;  // theta at which a list overflowed its fixed capacity (skip the one-pass attempt)

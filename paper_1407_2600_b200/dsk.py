@@ -270,7 +270,8 @@ class Dsk:
         return w.value
 
     def set_background(self, on):
-        _check(self.lib.dsk_set_background(self._h, int(bool(on))))
+        """0 off, 1 on, 2 on with the windows' background by the closed form everywhere (diagnostic)"""
+        _check(self.lib.dsk_set_background(self._h, 2 if on == 2 else int(bool(on))))
 
     def get_background(self):
         on, lv, k, nt, rho = C.c_int(0), C.c_int(0), C.c_int(0), C.c_int64(0), C.c_double(0)

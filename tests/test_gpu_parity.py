@@ -758,6 +758,29 @@ def test_background_coarse_cubes_outside_the_window(dsk, orc, theta):
     d.close()
 
 
+@pytest.mark.parametrize("theta", [0.3, 0.5, 1.0])
+@pytest.mark.parametrize("case", ["lattice", "clustered", "clumpy"])
+def test_background_window_series_equals_closed_form(dsk, case, theta):
+    """The window's background by the series of the cube's interior potential (order 14 for k >= 2, order 22 for k = 1, closed form
+    for the groups above level l_b) against the closed form everywhere (dsk_set_background(2)): the same forces and potentials to
+    the rounding of the fp32 accumulators.  (The table itself is pinned on the CPU: tests/test_cube_series_cpu.py.)"""
+    pos, mass = {"lattice": lambda: workloads.perturbed_lattice(32), "clustered": lambda: workloads.clustered_box(40, 60, cfg=4),
+                 "clumpy": lambda: workloads.clustered_box(32, 3, cfg=4)}[case]()
+    n = len(pos)
+    d = dsk.Dsk(n, 1.0, True, 1e-3, theta, 4)
+    tp, tm = _dev(pos), _dev(mass)
+    d.build_tree(tp, tm)
+    d.set_background(2)
+    a0, p0 = d.accel(tp, tm)
+    a0, p0 = a0.clone(), p0.clone()
+    d.set_background(1)
+    a1, p1 = d.accel(tp, tm)
+    rel = ((a1 - a0).norm(dim=1) / a0.norm(dim=1)).cpu().numpy()
+    assert rel.max() < 1e-6, (case, theta, rel.max())
+    assert float((p1 - p0).abs().max() / p0.abs().max()) < 1e-6
+    d.close()
+
+
 @pytest.mark.parametrize("case", ["lattice", "clustered"])
 def test_background_off_is_the_round1_definition(dsk, orc, case):
     """dsk_set_background(0): plain particle moments, the neutralising background only in the far field (and fp64 monopoles):
