@@ -332,7 +332,7 @@ def measure_config(cfgid, steps, warmup, dev, world, rank, dist, want_e2e, want_
         rowb = 4 * (8 + (cfg["p"] + 1) * (cfg["p"] + 2) * (cfg["p"] + 3) // 6)
         alg_bytes = {
             "key": bpp["key"] * n,
-            "sort": (bpp["sort"] + bpp["gather"]) * n,
+            "sort": (accounting.sort_bytes(n) + bpp["gather"]) * n,
             "build": 8 * n + 60 * st["ncell"],
             "upward": 16 * n + st["ncell"] * 4 * rowb,                       # particles once; rows written, read by M2M, force rows written
             "walk": 4 * (st["list_m2p"] + st["list_p2p"]),                  # list entries written (the cell tests hit L2)

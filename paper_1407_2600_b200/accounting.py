@@ -79,8 +79,17 @@ def fp32_peak_flops(n_sm, sm_clock_mhz):
 # algorithmic HBM bytes per particle of the streaming phases
 BYTES_PER_PARTICLE = {
     "key": 12 + 8 + 4,
-    "sort": 8 * (8 + 12 + 12),          # per pass: histogram read 8 + scatter read 12 + write 12
+    "sort": 8 * (8 + 12 + 12),          # N > 2^22: per pass histogram read 8 + scatter read 12 + write 12 (see sort_bytes)
     "gather": 4 + 12 + 4 + 16,
     "scatter": 32 + 4 + 16,
     "kdk": 3 * 36,
 }
+
+
+SORT_ONESWEEP_NMAX = 1 << 22            # DSK_SORT_ONESWEEP_NMAX of csrc/dsk_internal.cuh
+
+
+def sort_bytes(n):
+    """algorithmic HBM bytes per particle of the radix sort: up to 2^22 keys one read for all eight histograms and one read +
+    one write of the 12-byte records per pass (200 B, the figure of SURVEY.md 8(d)); above, a histogram read per pass as well"""
+    return 8 + 8 * (12 + 12) if n <= SORT_ONESWEEP_NMAX else BYTES_PER_PARTICLE["sort"]

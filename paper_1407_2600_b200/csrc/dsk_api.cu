@@ -18,7 +18,7 @@ static size_t carve(dsk_ctx *c, char *base)
         o += align_up(bytes);
         return p;
     };
-    c->ntile = (int)((n + 2047) / 2048);
+    c->ntile = (int)((n + DSK_SORT_TILE - 1) / DSK_SORT_TILE);
     // measured <= 0.06 cells and <= 0.05 groups per particle (NLEAF 64-112, NCRIT 64-192) on every config; a pathological
     // input (deep chains of near-coincident clumps) that needs more ends in DSK_ECELLOVERFLOW, not in a fault
     c->ncell_cap = (int64_t)(n / 4 + 4096);
@@ -30,7 +30,7 @@ static size_t carve(dsk_ctx *c, char *base)
     c->key_b = (uint64_t *)take(8 * n);
     c->idx_a = (uint32_t *)take(4 * n);
     c->idx_b = (uint32_t *)take(4 * n);
-    c->sort_hist = (uint32_t *)take(4 * 256 * (size_t)c->ntile);
+    c->sort_hist = (uint32_t *)take(4 * (n <= (size_t)DSK_SORT_ONESWEEP_NMAX ? 8 * 256 + 64 + (size_t)8 * 256 * c->ntile : 256 * (size_t)c->ntile));
     c->scan_tmp = (uint32_t *)take(4 * 4096);
     c->spos = (float4 *)take(16 * n);
     c->sacc = (float4 *)take(16 * n);

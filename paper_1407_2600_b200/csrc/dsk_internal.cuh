@@ -12,6 +12,8 @@
 #ifndef DSK_NCRIT
 #define DSK_NCRIT 192        // sink group: first cell from the root with count <= NCRIT (at most 4 tasks of 32 lanes x 2 sinks)
 #endif
+#define DSK_SORT_TILE 2048               // keys per block and pass of the radix sort (keysort.cu)
+#define DSK_SORT_ONESWEEP_NMAX (1 << 22) // up to here the sort takes its one-kernel-per-pass form (keysort.cu): sizes its status words
 #define DSK_WS 2              // LARGEST image block half-width, and the one image ids are encoded for: id = ((ix+2) 5 + iy+2) 5 + iz+2.
                               // The block actually summed is the context's ws (1 or 2, dsk_set_image_block): ids with |i| <= ws.
 #define DSK_WS_DEFAULT 1      // with background subtraction WS = 1 costs 1e-4 of the rms force on a near-lattice box and saves 11-18 %
@@ -126,7 +128,7 @@ struct dsk_ctx {
     // carved arrays
     uint64_t *key_a, *key_b;
     uint32_t *idx_a, *idx_b;
-    uint32_t *sort_hist;      // [ntile * 256] per-pass tile histograms (digit-major)
+    uint32_t *sort_hist;      // [ntile * 256] per-pass tile histograms (digit-major); small N: histograms, tickets and look-back status words (keysort.cu)
     uint32_t *scan_tmp;       // block sums for the generic scan
     float4 *spos;             // sorted (x,y,z,m); periodic: wrapped
     float4 *sacc;             // sorted (ax,ay,az,pot), high part of the compensated sum

@@ -59,6 +59,7 @@ __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pos, int
 #define SORT_THREADS 256
 #define SORT_ITEMS 8
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
+static_assert(SORT_TILE == DSK_SORT_TILE, "dsk_api.cu sizes the sort scratch by DSK_SORT_TILE");
 
 __global__ void __launch_bounds__(SORT_THREADS) k_sort_hist(const uint64_t *__restrict__ key, int64_t n,
                                                             int shift, int ntile,
@@ -152,6 +153,171 @@ __global__ void __launch_bounds__(SORT_THREADS) k_sort_scatter(
     }
     __syncthreads();
     const int64_t tile0 = (int64_t)blockIdx.x * SORT_TILE;
+    const int ntile_items = (int)min((int64_t)SORT_TILE, n - tile0);
+    for (int e = threadIdx.x; e < ntile_items; e += SORT_THREADS) {
+        const uint64_t kk = skey[e];
+        const uint32_t d = (uint32_t)(kk >> shift) & 255u;
+        const uint32_t dst = goff[d] + ((uint32_t)e - dstart[d]);
+        key_out[dst] = kk;
+        idx_out[dst] = sidx[e];
+    }
+}
+
+// ---- S for small N: one read and one write of the records per pass (decoupled look-back) ---------------------------------
+// Below DSK_SORT_ONESWEEP_NMAX keys the three-kernel pass above is bound by its 40 launches, not by traffic or ranking (C1: 0.19 of
+// a 0.77 ms step).  Here the eight global digit histograms come from ONE read of the keys (k_sort_hist8) and a pass is a single
+// kernel (k_sort_pass): a block takes the next tile from a ticket counter, ranks its keys exactly as k_sort_scatter does,
+// publishes its per-digit counts and finds the counts of all earlier tiles by look-back over the tiles' status words (flag in the
+// two top bits: 0 not yet there, 1 this tile's count, 2 the inclusive count up to this tile).  Tickets make the look-back safe:
+// a tile with a lower number has started, so it publishes without waiting for anyone behind it.  Measured (sort ms, three-kernel
+// -> this): C1 0.186 -> 0.092, C2 0.250 -> 0.211; C4 2.16 -> 2.26 and C5 18.0 -> 19.1, which is why large N keeps the form above:
+// at scale a pass is bound by the ranking code (ncu: 0.4 keys per cycle and SM either way), and the look-back waits cost more
+// than the saved histogram read.
+#define SORT_FLAG_AGG 0x40000000u
+#define SORT_FLAG_INC 0x80000000u
+#define SORT_VAL_MASK 0x3fffffffu
+#define SORT_LB 4                 // status words in flight per thread during the look-back
+
+__global__ void __launch_bounds__(256) k_sort_hist8(const uint64_t *__restrict__ key, int64_t n, uint32_t *__restrict__ ghist)
+{
+    __shared__ uint32_t h[8 * 256];
+    for (int i = threadIdx.x; i < 8 * 256; i += 256) h[i] = 0;
+    __syncthreads();
+    for (int64_t j = (int64_t)blockIdx.x * 256 + threadIdx.x; j < n; j += (int64_t)gridDim.x * 256) {
+        const uint64_t k = key[j];
+#pragma unroll
+        for (int d = 0; d < 8; d++) atomicAdd(&h[d * 256 + ((uint32_t)(k >> (8 * d)) & 255u)], 1u);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < 8 * 256; i += 256)
+        if (h[i]) atomicAdd(&ghist[i], h[i]);
+}
+
+__device__ __forceinline__ uint32_t sort_ld_status(const uint32_t *p)
+{
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sort_st_status(uint32_t *p, uint32_t v)
+{
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+__global__ void __launch_bounds__(SORT_THREADS) k_sort_pass(
+    const uint64_t *__restrict__ key_in, const uint32_t *__restrict__ idx_in, int64_t n, int shift,
+    const uint32_t *__restrict__ ghist, uint32_t *status, uint32_t *ticket, uint64_t *__restrict__ key_out,
+    uint32_t *__restrict__ idx_out)
+{
+    __shared__ uint32_t cnt[SORT_THREADS / 32][256];
+    __shared__ uint32_t goff[256], dstart[256];
+    __shared__ uint64_t wtot[SORT_THREADS / 32];
+    __shared__ uint64_t skey[SORT_TILE];
+    __shared__ uint32_t sidx[SORT_TILE];
+    __shared__ uint32_t s_tile;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+    for (int i = threadIdx.x; i < (SORT_THREADS / 32) * 256; i += SORT_THREADS) (&cnt[0][0])[i] = 0;
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const int64_t tile0 = (int64_t)tile * SORT_TILE;
+    const int64_t base = tile0 + (int64_t)warp * (SORT_ITEMS * 32);
+    uint64_t k[SORT_ITEMS];
+    uint32_t v[SORT_ITEMS], rank[SORT_ITEMS];
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; i++) {
+        int64_t j = base + i * 32 + lane;
+        bool ok = j < n;
+        k[i] = ok ? key_in[j] : ~0ull;
+        v[i] = ok ? idx_in[j] : 0u;
+    }
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; i++) {
+        uint32_t d = (uint32_t)(k[i] >> shift) & 255u;
+        uint32_t peers = __match_any_sync(0xffffffffu, d);
+        uint32_t before = __popc(peers & ((1u << lane) - 1u));
+        uint32_t old = cnt[warp][d];
+        __syncwarp();
+        if (before == 0) cnt[warp][d] = old + __popc(peers);
+        __syncwarp();
+        rank[i] = old + before;
+    }
+    __syncthreads();
+    // thread = digit from here to the look-back.  Exclusive prefix over warps; the tile's count of this digit goes out at once.
+    // (the padding keys ~0 of a ragged last tile are counted in digit 255 of the tile, behind every real key: they are
+    // neither staged nor written, and no later tile exists to read that count)
+    uint32_t dtot;
+    {
+        uint32_t run = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_THREADS / 32; w++) {
+            uint32_t c = cnt[w][threadIdx.x];
+            cnt[w][threadIdx.x] = run;
+            run += c;
+        }
+        dtot = run;
+    }
+    uint32_t *my_status = status + (size_t)tile * 256 + threadIdx.x;
+    sort_st_status(my_status, (tile == 0 ? SORT_FLAG_INC : SORT_FLAG_AGG) | dtot);
+    // exclusive prefix over digits of (tile count, global count) in one 64-bit scan: where the digit's run starts inside
+    // the tile, and where the digit's region starts in the output
+    uint32_t gbase;
+    {
+        const uint64_t mine = ((uint64_t)dtot << 32) | (uint64_t)ghist[threadIdx.x];
+        uint64_t x = mine;
+        for (int o = 1; o < 32; o <<= 1) {
+            uint64_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) wtot[warp] = x;
+        __syncthreads();
+        uint64_t wpre = 0;
+        for (int w = 0; w < warp; w++) wpre += wtot[w];
+        const uint64_t ex = wpre + x - mine;
+        dstart[threadIdx.x] = (uint32_t)(ex >> 32);
+        gbase = (uint32_t)ex;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; i++) {
+        int64_t j = base + i * 32 + lane;
+        if (j < n) {
+            uint32_t d = (uint32_t)(k[i] >> shift) & 255u;
+            uint32_t lp = dstart[d] + cnt[warp][d] + rank[i];
+            skey[lp] = k[i];
+            sidx[lp] = v[i];
+        }
+    }
+    // look-back: the count of this digit in all earlier tiles.  SORT_LB status words are fetched at a time (independent loads);
+    // they are consumed nearest tile first up to the first one that is not there yet.
+    {
+        uint32_t excl = 0;
+        if (tile > 0) {
+            const uint32_t *sp = my_status - 256;
+            uint32_t left = tile;                       // predecessors not yet consumed
+            for (bool done = false; !done;) {
+                uint32_t s[SORT_LB];
+#pragma unroll
+                for (int b = 0; b < SORT_LB; b++) s[b] = (uint32_t)b < left ? sort_ld_status(sp - 256 * b) : SORT_FLAG_INC;
+                uint32_t used = 0;
+                bool open = true;
+#pragma unroll
+                for (int b = 0; b < SORT_LB; b++) {
+                    if (open && !(s[b] & (SORT_FLAG_AGG | SORT_FLAG_INC))) open = false;
+                    if (open) {
+                        excl += s[b] & SORT_VAL_MASK;
+                        used++;
+                        if (s[b] & SORT_FLAG_INC) { done = true; open = false; }
+                    }
+                }
+                sp -= 256 * used;
+                left -= used;
+            }
+            sort_st_status(my_status, SORT_FLAG_INC | (excl + dtot));
+        }
+        goff[threadIdx.x] = gbase + excl;
+    }
+    __syncthreads();
     const int ntile_items = (int)min((int64_t)SORT_TILE, n - tile0);
     for (int e = threadIdx.x; e < ntile_items; e += SORT_THREADS) {
         const uint64_t kk = skey[e];
@@ -285,18 +451,35 @@ int dsk_run_keysort(dsk_ctx *c, const float *pos, const float *mass)
     uint64_t *ka = c->key_a, *kb = c->key_b;
     uint32_t *ia = c->idx_a, *ib = c->idx_b;
     const int ntile = c->ntile;
-    for (int pass = 0; pass < 8; pass++) {
-        int shift = 8 * pass;
-        k_sort_hist<<<ntile, SORT_THREADS, 0, c->stream>>>(ka, n, shift, ntile, c->sort_hist);
-        dsk_exclusive_scan_u32(c, c->sort_hist, c->sort_hist, nullptr, (uint32_t)(256u * (uint32_t)ntile), nullptr);
-        k_sort_scatter<<<ntile, SORT_THREADS, 0, c->stream>>>(ka, ia, n, shift, ntile, c->sort_hist, kb, ib);
-        uint64_t *tk = ka; ka = kb; kb = tk;
-        uint32_t *ti = ia; ia = ib; ib = ti;
+    if (n <= (int64_t)DSK_SORT_ONESWEEP_NMAX) {
+        // sort_hist: [8][256] global digit histograms, 8 tickets (+ padding to 64 words), then [8][ntile][256] status words
+        uint32_t *ghist = c->sort_hist, *ticket = ghist + 8 * 256, *status = ticket + 64;
+        cudaMemsetAsync(ghist, 0, sizeof(uint32_t) * (8 * 256 + 64 + (size_t)8 * 256 * ntile), c->stream);
+        int64_t hb = (n + 256 * 16 - 1) / (256 * 16);
+        if (hb > (int64_t)c->nsm * 8) hb = (int64_t)c->nsm * 8;
+        k_sort_hist8<<<(unsigned)hb, 256, 0, c->stream>>>(ka, n, ghist);
+        for (int pass = 0; pass < 8; pass++) {
+            k_sort_pass<<<ntile, SORT_THREADS, 0, c->stream>>>(ka, ia, n, 8 * pass, ghist + 256 * pass, status + (size_t)pass * 256 * ntile,
+                                                               ticket + pass, kb, ib);
+            uint64_t *tk = ka; ka = kb; kb = tk;
+            uint32_t *ti = ia; ia = ib; ib = ti;
+        }
+        DSK_COUNT(c, 1 + 8);
+    } else {
+        for (int pass = 0; pass < 8; pass++) {
+            int shift = 8 * pass;
+            k_sort_hist<<<ntile, SORT_THREADS, 0, c->stream>>>(ka, n, shift, ntile, c->sort_hist);
+            dsk_exclusive_scan_u32(c, c->sort_hist, c->sort_hist, nullptr, (uint32_t)(256u * (uint32_t)ntile), nullptr);
+            k_sort_scatter<<<ntile, SORT_THREADS, 0, c->stream>>>(ka, ia, n, shift, ntile, c->sort_hist, kb, ib);
+            uint64_t *tk = ka; ka = kb; kb = tk;
+            uint32_t *ti = ia; ia = ib; ib = ti;
+        }
+        DSK_COUNT(c, 2 * 8);            // 8 x (hist, scatter); the scans count themselves
     }
     // 8 passes: the result is back in (key_a, idx_a)
     k_gather<<<nb, 256, 0, c->stream>>>(pos, mass, c->idx_a, n, c->box, c->periodic, c->spos);
     cudaEventRecord(c->ev[2], c->stream);
-    DSK_COUNT(c, 2 + 2 * 8);        // keys, gather, 8 x (hist, scatter); the scans count themselves
+    DSK_COUNT(c, 2);                // keys, gather
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
