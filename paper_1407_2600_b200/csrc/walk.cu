@@ -10,6 +10,7 @@
 // lengths, for the offsets) and FILL.
 #include "dsk_internal.cuh"
 #include <string.h>
+#include <stdio.h>
 
 // one warp per block: walks differ in length, and a block ends with its longest
 #define WRESERVE 160         // stack entries kept free for the depth-first tail (7 per level, 21 levels)
@@ -371,6 +372,11 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
 // listed and which cubes are exposed) - not on g0, g1 or the active flags, which only select the members whose lists are written:
 // a sharded, batched or active-subset evaluation lists every group's entries in the same order as a full one.
 #define WSG 8
+#ifdef DSK_DEBUG_BOUNDS
+#define WK_CHECK(cond) do { if (!(cond)) { printf("walk bounds: %s line %d block %d lane %d\n", #cond, __LINE__, blockIdx.x, threadIdx.x); __trap(); } } while (0)
+#else
+#define WK_CHECK(cond) do { } while (0)
+#endif
 template <int MODE, bool ABS>          // MODE 0 COUNT, 1 FILL at the scanned offsets, 2 ONE pass into a fixed capacity per group
 __global__ void __launch_bounds__(32) k_walk_sh(uint32_t g0, uint32_t g1, uint32_t ngroup, int sgn, int periodic, float box, int pow1, float k1_h,
                                              const dsk_cellrec *__restrict__ cell,
@@ -527,6 +533,7 @@ __global__ void __launch_bounds__(32) k_walk_sh(uint32_t g0, uint32_t g1, uint32
 #pragma unroll
                     for (int q = 0; q < WEPL; q++) {
                         act[q] = lane + 32 * q < take;
+                        WK_CHECK(!act[q] || (rp + lane + 32 * q >= rtop && rp + lane + 32 * q < WSTACK));
                         e[q] = act[q] ? stk[rp + lane + 32 * q] : 0u;
                     }
                     rp += take;
@@ -608,6 +615,7 @@ __global__ void __launch_bounds__(32) k_walk_sh(uint32_t g0, uint32_t g1, uint32
                         if (wm || wp)
                             for (uint32_t t = wset; t; t &= t - 1u) {
                                 const int i = __ffs(t) - 1;
+                                WK_CHECK(i < nrun && ((wantset >> i) & 1u));
                                 if (wm) list_m2p[moff[i] + im] = entry;
                                 if (wp) list_p2p[poff[i] + ip] = e[q];
                             }
@@ -617,6 +625,7 @@ __global__ void __launch_bounds__(32) k_walk_sh(uint32_t g0, uint32_t g1, uint32
                     if (common) {                                           // cells the members disagree on: to the residual list
                         const uint32_t bx = __ballot_sync(0xffffffffu, mixed);
                         rtop -= __popc(bx);
+                        WK_CHECK(rtop >= sp && rtop + __popc(bx) <= WSTACK);
                         if (mixed) stk[rtop + __popc(bx & lt)] = e[q];
                     }
                     if (BG && __any_sync(0xffffffffu, nexp != 0u)) {           // rare: cubes kept outside the window
@@ -649,6 +658,7 @@ __global__ void __launch_bounds__(32) k_walk_sh(uint32_t g0, uint32_t g1, uint32
 #pragma unroll
                 for (int q = 0; q < WEPL; q++) {
                     const uint32_t img = e[q] & ~CELL_MASK;
+                    WK_CHECK(at + push[q] <= (uint32_t)rtop);
 #pragma unroll
                     for (uint32_t k = 0; k < 8; k++)
                         if (k < push[q]) stk[at + k] = img | (child0[q] + k);
