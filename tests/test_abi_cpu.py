@@ -86,8 +86,19 @@ def test_create_validation_and_workspace(lib):
     # p may be lowered but not raised above dsk_create's p (the workspace is sized for it)
     assert lib.dsk_set_params(h, 1e-4, 0.3, 2) == 0 and lib.dsk_set_params(h, 1e-4, 0.3, 5) == -1
     assert lib.dsk_set_params(h, 1e-4, 0.3, 8) == -2
+    # switches validate their argument without touching the device
+    lib.dsk_set_walk_sharing.argtypes = [C.c_void_p, C.c_int]
+    assert lib.dsk_set_walk_sharing(h, 8) == 0 and lib.dsk_set_walk_sharing(h, 0) == 0
+    assert lib.dsk_set_walk_sharing(h, 9) == -1 and lib.dsk_set_walk_sharing(h, -1) == -1
+    assert lib.dsk_set_background(h, 1) == -1                    # isolated context
     assert lib.dsk_destroy(h) == 0
     assert lib.dsk_strerror(-4).decode().startswith("position outside")
+    assert "maximum" in lib.dsk_strerror(-9).decode()
+    # the no-allocation entry point rejects sizes beyond its fixed scratch before any device work
+    lib.dsk_sort_keys_noalloc.argtypes = [C.c_void_p, C.c_int64, C.c_float, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+    assert lib.dsk_sort_keys_noalloc(C.c_void_p(256), (1 << 20) + 1, 1.0, 0, C.c_void_p(256), C.c_void_p(256), None) == -9
+    assert lib.dsk_sort_keys_noalloc(C.c_void_p(256), 0, 1.0, 0, C.c_void_p(256), C.c_void_p(256), None) == -1
+    assert lib.dsk_sort_keys_noalloc(None, 10, 1.0, 0, C.c_void_p(256), C.c_void_p(256), None) == -1
     h2 = C.c_void_p(0)
     assert lib.dsk_create(C.byref(h2), 1 << 21, 1.0, 0, 1e-4, 0.5, 4) == 0
     assert 1.8 < lib.dsk_workspace_bytes(h2) / b1 < 2.2
@@ -108,3 +119,13 @@ def test_lattice_tensors_match_oracle(lib, orc):
     lib.dsk_create(C.byref(h), 100, 1.0, 0, 1e-3, 0.5, 4)
     assert lib.dsk_get_lattice_tensors(h, T.ctypes.data_as(C.c_void_p)) == -1     # isolated: none
     lib.dsk_destroy(h)
+
+
+def test_sort_threshold_is_the_same_on_both_sides_of_the_accounting():
+    """bench.py's algorithmic bytes of the sort (accounting.sort_bytes) switch where the library switches its sort form"""
+    import re
+    from paper_1407_2600_b200 import accounting
+    src = open(os.path.join(os.path.dirname(__file__), "..", "paper_1407_2600_b200", "csrc", "dsk_internal.cuh")).read()
+    m = re.search(r"#define DSK_SORT_ONESWEEP_NMAX \(1 << (\d+)\)", src)
+    assert m and (1 << int(m.group(1))) == accounting.SORT_ONESWEEP_NMAX
+    assert accounting.sort_bytes(1 << 20) == 200 and accounting.sort_bytes(1 << 24) == 256
