@@ -538,7 +538,7 @@ def run_sweep(args):
         return min(ms), float(torch.sqrt(((a - ref) ** 2).sum() / (ref ** 2).sum())), st["n_m2p"] / n, st["n_p2p"] / n
 
     rows = []
-    for p in (2, 4, 6):
+    for p in (2, 3, 4, 5, 6):
         for theta in (0.4, 0.5, 0.6, 0.7, 0.8, 1.0):
             d.set_mac("theta"); d.set_params(theta=theta, p=p)
             ms, E, m2p, p2p = measure()

@@ -71,7 +71,8 @@ typedef struct dsk_stats {
 /* Create a context for N particles in the cube [0, box)^3.  PAPER.md:61-63; O1-O7.
  *   periodic : 0 isolated, 1 periodic (explicit (2 WS+1)^3 image block + order-8 far field)
  *   eps      : Plummer softening length (> 0);  theta : opening angle, 0 < theta <= 1
- *   p        : expansion order = highest multipole rank kept, one of 2, 4, 6, 8
+ *   p        : expansion order = highest multipole rank kept, one of 2, 3, 4, 5, 6, 8 (the even ones are BASELINE.json's sweep; 3 and
+ *              5 sit between them in cost and error, and 3 is what the absolute-error rule wants at an RMS error of 1e-4)
  * Host-only work (the lattice tensors of the far field are computed here in fp64). */
 int dsk_create(dsk_ctx **out, int64_t N, float box, int periodic, float eps, float theta, int p);
 int dsk_destroy(dsk_ctx *ctx);

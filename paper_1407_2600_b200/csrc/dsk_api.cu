@@ -103,7 +103,7 @@ static int check_params(float eps, float theta, int p)
 {
     if (!(eps > 0.0f) || !isfinite(eps)) return DSK_EINVAL;
     if (!(theta > 0.0f && theta <= 1.0f)) return DSK_EINVAL;
-    if (p != 2 && p != 4 && p != 6 && p != 8) return DSK_EINVAL;
+    if (p != 2 && p != 3 && p != 4 && p != 5 && p != 6 && p != 8) return DSK_EINVAL;
     return DSK_OK;
 }
 
@@ -275,9 +275,9 @@ static int accel_impl(dsk_ctx *c, const uint8_t *active, float *acc, float *pot,
         c->lists_valid = 0;
     }
     if (shard_rank >= 0) {
-        static const uint32_t fm[4] = {78, 252, 682, 1536};         // flop per M2P interaction at p = 2, 4, 6, 8
+        static const uint32_t fm[7] = {78, 136, 252, 423, 682, 1040, 1536};         // flop per M2P interaction at p = 2 .. 8 (accounting.py)
         uint32_t cut[1025];
-        e = dsk_run_shard(c, shard_rank, shard_n, fm[c->p / 2 - 1], 19u, cut);
+        e = dsk_run_shard(c, shard_rank, shard_n, fm[c->p - 2], 19u, cut);
         if (e) return e;
         const uint32_t g_lo = cut[shard_rank], g_hi = cut[shard_rank + 1], ng = c->hstate->ngroup;
         if (shard_lo) *shard_lo = g_lo;

@@ -190,7 +190,7 @@ struct dsk_ctx {
     int frow_tab_p;           // order of the uploaded force-row map
     int frow_tab_dip;         // and whether it has the dipole block
     int frow_dip;             // layout of the force rows in memory: dipole block present (periodic with subtraction)
-    uint32_t m2m_tab_mask;    // orders whose M2M pair table this context has uploaded (bit p/2 - 1)
+    uint32_t m2m_tab_mask;    // orders whose M2M pair table this context has uploaded (bit p - 2)
     int soft_kind;            // 0 Plummer (eps), 1 Dehnen K1 (eps holds the support h) (dsk_set_softening)
     int mac_kind;             // 0 opening angle, 1 absolute error bound (dsk_set_mac)
     float mac_tol;

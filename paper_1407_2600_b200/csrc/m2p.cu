@@ -44,7 +44,7 @@ __host__ __device__ constexpr int fr_qfirst_G(int P, int m) { return 2 * m - P <
 
 static int frow_nc(int p, bool d)
 {
-    return p == 2 ? fr_nc(2, d) : p == 4 ? fr_nc(4, d) : p == 6 ? fr_nc(6, d) : fr_nc(8, d);
+    return p == 2 ? fr_nc(2, d) : p == 3 ? fr_nc(3, d) : p == 4 ? fr_nc(4, d) : p == 5 ? fr_nc(5, d) : p == 6 ? fr_nc(6, d) : fr_nc(8, d);
 }
 int dsk_frow_len(int p, int dip) { return (8 + frow_nc(p, dip != 0) + 3) / 4 * 4; }
 
@@ -278,7 +278,7 @@ __device__ __forceinline__ void m2p_body(T xs, T ys, T zs, const float *__restri
 // 2: periodic with background subtraction (reading O4b: fp32 throughout, rows carry a dipole block)
 template <int P, int MODE> struct m2p_cfg {
     static constexpr bool M64 = MODE == 1, DIP = MODE == 2;
-    static constexpr int NCELL = (P <= 4) ? 32 : (P == 6 ? 16 : 8);   // cells per tile
+    static constexpr int NCELL = (P <= 4) ? 32 : (P <= 6 ? 16 : 8);   // cells per tile
     static constexpr int LPC = 32 / NCELL;                             // lanes that share the copy of one row
     static constexpr int FROW = fr_rowlen(P, DIP);
     static constexpr int NCH = FROW / 4;                               // 16-byte chunks per row
@@ -538,7 +538,9 @@ int dsk_launch_m2p(dsk_ctx *c, uint32_t t0, uint32_t t1, uint64_t base, int want
     if (t1 <= t0) return DSK_OK;
     switch (c->p) {
     case 2: return launch_m2p<2>(c, t0, t1, base, want_pot);
+    case 3: return launch_m2p<3>(c, t0, t1, base, want_pot);
     case 4: return launch_m2p<4>(c, t0, t1, base, want_pot);
+    case 5: return launch_m2p<5>(c, t0, t1, base, want_pot);
     case 6: return launch_m2p<6>(c, t0, t1, base, want_pot);
     case 8: return launch_m2p<8>(c, t0, t1, base, want_pot);
     default: return DSK_EINVAL;

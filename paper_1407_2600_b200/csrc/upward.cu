@@ -18,12 +18,12 @@
 
 __constant__ uint8_t c_ea[UNP], c_eb[UNP], c_ec[UNP], c_rank[UNP];
 __device__ uint8_t g_ea[UNP], g_eb[UNP], g_ec[UNP], g_rank[UNP];   // the same tables for per-lane (divergent) indexing
-// M2M pair tables, one per order p = 2, 4, 6, 8 (slot p/2 - 1): for moment n (visited heaviest first through g_m2m_perm) the entries
+// M2M pair tables, one per order p = 2 .. 8 (slot p - 2): for moment n (visited heaviest first through g_m2m_perm) the entries
 // k <= n packed as k_index | (n-k).a << 8 | (n-k).b << 12 | (n-k).c << 16
 #define M2M_MAXPAIR 3003       // C(14, 6): pairs (k <= n, |n| <= 8)
-__device__ uint32_t g_m2m_ent[4][M2M_MAXPAIR];
-__device__ uint16_t g_m2m_beg[4][UNP + 1];
-__device__ uint8_t g_m2m_perm[4][UNP];
+__device__ uint32_t g_m2m_ent[7][M2M_MAXPAIR];
+__device__ uint16_t g_m2m_beg[7][UNP + 1];
+__device__ uint8_t g_m2m_perm[7][UNP];
 __constant__ float c_sgn_invfact[UNP];   // (-1)^|n| / (a! b! c!)
 __constant__ float c_invfact1[DSK_PMAX + 1];
 
@@ -64,7 +64,7 @@ static int upload_tables()
 // a second context writing the same bytes while another reads them is harmless; no state is shared on the host)
 static int upload_m2m_table(dsk_ctx *c, int p)
 {
-    const int slot = p / 2 - 1;
+    const int slot = p - 2;
     if (c->m2m_tab_mask & (1u << slot)) return DSK_OK;
     const int np = dsk_np(p);
     uint32_t ent[M2M_MAXPAIR];
@@ -244,11 +244,11 @@ __device__ __forceinline__ void upward_cell(uint32_t c, int level, float box, co
             const float *px = sm.pw[live ? ch : 0][0], *py = sm.pw[live ? ch : 0][1], *pz = sm.pw[live ? ch : 0][2];
             for (int q0 = 0; q0 < NP; q0 += 4) {
                 const int q = q0 + (lane >> 3);
-                const int n = g_m2m_perm[P / 2 - 1][q < NP ? q : NP - 1];
-                const int t1 = (q < NP && live) ? g_m2m_beg[P / 2 - 1][n + 1] : 0;
+                const int n = g_m2m_perm[P - 2][q < NP ? q : NP - 1];
+                const int t1 = (q < NP && live) ? g_m2m_beg[P - 2][n + 1] : 0;
                 float sum = 0.0f;
-                for (int t = g_m2m_beg[P / 2 - 1][n]; t < t1; t++) {
-                    const uint32_t e = g_m2m_ent[P / 2 - 1][t];
+                for (int t = g_m2m_beg[P - 2][n]; t < t1; t++) {
+                    const uint32_t e = g_m2m_ent[P - 2][t];
                     sum = fmaf(cr[e & 255u], px[(e >> 8) & 15u] * py[(e >> 12) & 15u] * pz[(e >> 16) & 15u], sum);
                 }
                 sum += __shfl_xor_sync(0xffffffffu, sum, 1);
@@ -346,7 +346,9 @@ int dsk_run_upward(dsk_ctx *c)
     cudaEventRecord(c->ev[5], c->stream);
     switch (c->p) {
     case 2: e = launch_upward<2>(c, ls, nl); break;
+    case 3: e = launch_upward<3>(c, ls, nl); break;
     case 4: e = launch_upward<4>(c, ls, nl); break;
+    case 5: e = launch_upward<5>(c, ls, nl); break;
     case 6: e = launch_upward<6>(c, ls, nl); break;
     case 8: e = launch_upward<8>(c, ls, nl); break;
     default: return DSK_EINVAL;
@@ -393,7 +395,9 @@ int dsk_run_get_moments(dsk_ctx *c, float *com_mass, float *moments, int scaled)
     uint32_t nc = c->hstate->ncell;
     switch (c->p) {
     case 2: k_get_moments<2><<<nc, 32, 0, c->stream>>>(nc, c->rows, com_mass, moments, scaled); break;
+    case 3: k_get_moments<3><<<nc, 32, 0, c->stream>>>(nc, c->rows, com_mass, moments, scaled); break;
     case 4: k_get_moments<4><<<nc, 64, 0, c->stream>>>(nc, c->rows, com_mass, moments, scaled); break;
+    case 5: k_get_moments<5><<<nc, 64, 0, c->stream>>>(nc, c->rows, com_mass, moments, scaled); break;
     case 6: k_get_moments<6><<<nc, 96, 0, c->stream>>>(nc, c->rows, com_mass, moments, scaled); break;
     case 8: k_get_moments<8><<<nc, 192, 0, c->stream>>>(nc, c->rows, com_mass, moments, scaled); break;
     default: return DSK_EINVAL;

@@ -71,7 +71,7 @@ def test_task_widths_cover_every_group_size(lib):
 def test_create_validation_and_workspace(lib):
     h = C.c_void_p(0)
     bad = [(0, 1.0, 0, 1e-3, 0.5, 4), (10, -1.0, 0, 1e-3, 0.5, 4), (10, 1.0, 0, 0.0, 0.5, 4),
-           (10, 1.0, 0, 1e-3, 0.0, 4), (10, 1.0, 0, 1e-3, 1.5, 4), (10, 1.0, 0, 1e-3, 0.5, 3),
+           (10, 1.0, 0, 1e-3, 0.0, 4), (10, 1.0, 0, 1e-3, 1.5, 4), (10, 1.0, 0, 1e-3, 0.5, 7), (10, 1.0, 0, 1e-3, 0.5, 1),
            (10, 1.0, 0, 1e-3, 0.5, 10)]
     for a in bad:
         assert lib.dsk_create(C.byref(h), *a) == -1
@@ -84,7 +84,7 @@ def test_create_validation_and_workspace(lib):
     assert lib.dsk_bind_workspace(h, C.c_void_p(0), b1) == -2
     assert lib.dsk_bind_workspace(h, C.c_void_p(257), b1) == -2
     # p may be lowered but not raised above dsk_create's p (the workspace is sized for it)
-    assert lib.dsk_set_params(h, 1e-4, 0.3, 2) == 0 and lib.dsk_set_params(h, 1e-4, 0.3, 5) == -1
+    assert lib.dsk_set_params(h, 1e-4, 0.3, 2) == 0 and lib.dsk_set_params(h, 1e-4, 0.3, 3) == 0 and lib.dsk_set_params(h, 1e-4, 0.3, 7) == -1
     assert lib.dsk_set_params(h, 1e-4, 0.3, 8) == -2
     # switches validate their argument without touching the device
     lib.dsk_set_walk_sharing.argtypes = [C.c_void_p, C.c_int]

@@ -62,7 +62,7 @@ def test_accounting_matches_kernel_op_counts():
         pytest.skip("cuobjdump or build/m2p.o missing: the SASS half of this test did not run")
     sass = subprocess.run([cuobjdump, "-sass", obj], capture_output=True, text=True).stdout
     for mode, dip in ((0, False), (2, True)):               # isolated rows; periodic rows with the dipole block (background subtraction)
-        for p in (2, 4, 6):                                 # the packed (f32x2) instantiations: <P, pot, MODE>
+        for p in (2, 3, 4, 5, 6):                           # the packed (f32x2) instantiations: <P, pot, MODE>
             fn = [b for b in sass.split("Function : ")[1:] if b.startswith(f"_Z5k_m2pILi{p}ELb1ELi{mode}EE")]
             assert len(fn) == 1
             ffma, fmul, fadd = accounting.m2p_ops(p, pot=True, dip=dip)

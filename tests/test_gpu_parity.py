@@ -142,7 +142,7 @@ def test_errors(dsk):
 
 
 # ---- moments ------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("p", [2, 4, 6, 8])
+@pytest.mark.parametrize("p", [2, 3, 4, 5, 6, 8])
 def test_moments(dsk, orc, p):
     pos, mass = workloads.make(2, 1 / 64)
     mass = (mass * np.random.default_rng(1).uniform(0.5, 1.5, len(mass))).astype(np.float32)
@@ -241,7 +241,7 @@ def test_forces_C2_sweep_scaled(dsk, orc):
     d.build_tree(tp, tm)
     tree = orc.OracleTree(pos, mass)
     errs = {}
-    for p in (2, 4, 6, 8):
+    for p in (2, 3, 4, 5, 6, 8):
         for theta in (0.3, 0.5, 0.7, 1.0):
             d.set_params(theta=theta, p=p)
             acc, _ = d.accel(tp, tm, want_pot=False)
@@ -250,8 +250,8 @@ def test_forces_C2_sweep_scaled(dsk, orc):
             errs[(theta, p)] = _force_gates(acc, ta, da)
     # the sweep behaves like the method should: error falls with p and rises with theta
     for theta in (0.3, 0.5, 0.7, 1.0):
-        e = [errs[(theta, p)][0] for p in (2, 4, 6, 8)]
-        assert e[0] > e[1] > e[2], e
+        e = [errs[(theta, p)][0] for p in (2, 3, 4, 5, 6, 8)]
+        assert e[0] > e[1] > e[2] > e[3] > e[4], e
     d.close()
 
 
@@ -375,7 +375,7 @@ def test_forces_random_small_cases(dsk, orc, seed):
     n = int(rng.choice([3, 31, 129, 257, 700, 1500, 3000, 9000]))
     periodic = bool(rng.integers(2))
     theta = float(rng.choice([0.3, 0.5, 0.7, 1.0]))
-    p = int(rng.choice([2, 4, 6, 8]))
+    p = int(rng.choice([2, 4, 6, 8, 3, 5]))
     kind = int(rng.integers(4))
     if kind == 0:
         pos = rng.random((n, 3))

@@ -1,6 +1,8 @@
 """dsk_sort_keys_noalloc: the key + sort steps with their scratch in a fixed device array of the library (no cudaMalloc, no
 workspace) against the existing path (dsk_build_tree + dsk_get_keys), bit for bit, on calls in a row.
 Collected last on purpose (the suite runs with pytest -x)."""
+import gc
+
 import numpy as np
 import pytest
 
@@ -46,13 +48,14 @@ def test_sort_keys_noalloc_equals_existing_path_on_calls_in_a_row(dsk):
         keys = torch.full((n,), -1, dtype=torch.int64, device="cuda")
         order = torch.full((n,), -1, dtype=torch.int32, device="cuda")
         for rep in range(2):                                                        # two calls in a row on the same input
+            gc.collect()                                                            # tensors of earlier tests die here, not inside the bracket
             torch.cuda.synchronize()
             free0 = torch.cuda.mem_get_info()[0]
             alloc0 = torch.cuda.memory_allocated()
             dsk.sort_keys_noalloc(pos_d, box, periodic, keys, order)
             torch.cuda.synchronize()
             if i > 0 or rep > 0:                                                    # the first launch loads the kernels
-                assert torch.cuda.memory_allocated() == alloc0
+                assert torch.cuda.memory_allocated() <= alloc0                     # nothing new from torch's allocator either
                 assert free0 - torch.cuda.mem_get_info()[0] < (1 << 20)
             assert torch.equal(keys, k_ref), (i, rep)
             assert torch.equal(order, o_ref), (i, rep)
