@@ -280,7 +280,12 @@ int dsk_run_build(dsk_ctx *c)
         uint32_t cap = (uint32_t)c->ncell_cap;
         void *args[] = {(void *)&key, (void *)&c->cell, (void *)&c->hotkey, (void *)&c->parent, (void *)&c->nchild_tmp,
                         (void *)&c->cbounds, (void *)&c->scan_tmp, (void *)&cap, (void *)&c->dstate};
-        DSK_CUDA(cudaLaunchCooperativeKernel((const void *)k_tree_build, dim3(grid), dim3(TB), args, 0, s));
+        // blocks of the cooperative launch: every level costs two grid barriers, whose price grows with the number of blocks, and the top
+        // levels have no work to share - one block per SM up to 4 M particles, more where the deep levels are wide
+        // (build ms with 1 / 2 / 4 / 6 blocks per SM: C1 0.050 / 0.055 / 0.060 / 0.067, C2 0.248 / 0.276 / 0.306 / 0.325,
+        //  C4 0.636 / 0.613 / 0.598 / 0.642, C5 1.92 / 1.62 / 1.43 / 1.39)
+        const int bgrid = c->nsm * (c->N <= (1ll << 22) ? 1 : (c->N <= (1ll << 25) ? 4 : 6));
+        DSK_CUDA(cudaLaunchCooperativeKernel((const void *)k_tree_build, dim3(bgrid), dim3(TB), args, 0, s));
     }
     cudaEventRecord(c->ev[3], s);
     // groups
