@@ -309,9 +309,11 @@ __global__ void __launch_bounds__(UTOP_WARPS * 32) k_upward_top(up_levels lv, in
 template <int P>
 static int launch_upward(dsk_ctx *c, const uint32_t *lvl_start, int nlevel)
 {
-    // levels [0, ltop) go to the single-block kernel: as many levels from the root as hold <= 96 cells together
+    // levels [0, ltop) go to the single-block kernel: as many levels from the root as hold <= 24 cells together (the root and its
+    // children; with a 64-cell level in it as well a warp works through eight cells in a row: upward ms with a limit of 96 / 24 / 1 / 600
+    // cells: C1 0.091 / 0.047 / 0.051 / 0.250, C2 0.195 / 0.171 / 0.178 / 0.270, C3 0.268 / 0.229 / 0.231 / 0.684, C4 4.36 / 4.24 / 4.25 / 5.36)
     int ltop = 0;
-    while (ltop < nlevel && lvl_start[ltop + 1] <= 96u) ltop++;
+    while (ltop < nlevel && lvl_start[ltop + 1] <= 24u) ltop++;
     for (int l = nlevel - 1; l >= ltop; l--) {
         uint32_t beg = lvl_start[l], n = lvl_start[l + 1] - beg;
         if (!n) continue;
