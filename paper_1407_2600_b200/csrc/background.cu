@@ -115,23 +115,33 @@ __global__ void __launch_bounds__(128) k_bg_rows(uint32_t ntop, int np, int rowl
     float *out = rows_bg + (size_t)c * rowlen;
     const double s = 1.0 / (double)row[3];
     const double mb = mass64[0] / ((double)box * box * box) * s * s * s;          // rho_bar s^3
-    double one[3][DSK_PMAX + 1];
-#pragma unroll
-    for (int d = 0; d < 3; d++) {
+    // lane 9 d + k holds the one-dimensional factor of axis d and power k (27 lanes; every lane computing all 27, each with a
+    // division, was 30 x the work of the moments themselves)
+    double val = 0.0;
+    if (lane < 3 * (DSK_PMAX + 1)) {
+        const int d = lane / (DSK_PMAX + 1), k = lane - d * (DSK_PMAX + 1);
         const double e = (double)row[4 + d] * (double)row[3];
         const double a = 0.5 - e, b = -0.5 - e;
         double pa = a, pb = b;
-        for (int k = 0; k <= DSK_PMAX; k++) { one[d][k] = (pa - pb) / (double)(k + 1); pa *= a; pb *= b; }
+        for (int j = 0; j < k; j++) { pa *= a; pb *= b; }
+        val = (pa - pb) / (double)(k + 1);
     }
     if (lane < 8) out[lane] = row[lane];
-    for (int n = lane; n < rowlen - 8; n += 32) {
-        float v = 0.0f;
-        if (n < np) {
-            const double cube = mb * b_sgn_invfact[n] * one[0][b_ea[n]] * one[1][b_eb[n]] * one[2][b_ec[n]];
-            const double part = n == 0 ? mass64[c] : (double)row[8 + n];
-            v = (float)(part - cube);
+    for (int n0 = 0; n0 < rowlen - 8; n0 += 32) {
+        const int n = n0 + lane;
+        const bool live = n < np;
+        const int ea = live ? b_ea[n] : 0, eb = live ? b_eb[n] : 0, ec = live ? b_ec[n] : 0;
+        const double o0 = __shfl_sync(0xffffffffu, val, ea), o1 = __shfl_sync(0xffffffffu, val, (DSK_PMAX + 1) + eb),
+                     o2 = __shfl_sync(0xffffffffu, val, 2 * (DSK_PMAX + 1) + ec);
+        if (n < rowlen - 8) {
+            float v = 0.0f;
+            if (live) {
+                const double cube = mb * b_sgn_invfact[n] * o0 * o1 * o2;
+                const double part = n == 0 ? mass64[c] : (double)row[8 + n];
+                v = (float)(part - cube);
+            }
+            out[8 + n] = v;
         }
-        out[8 + n] = v;
     }
 }
 
