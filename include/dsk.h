@@ -183,6 +183,14 @@ int dsk_set_walk_mode(dsk_ctx *ctx, int mode);
  * (the sets are formed from the group indices, not from what is evaluated).  DSK_EINVAL outside 0..8. */
 int dsk_set_walk_sharing(dsk_ctx *ctx, int groups);
 
+/* How the last evaluation sized its lists (introspection; host pointers, either may be NULL).  When the lists do not fit a fixed
+ * capacity per group (very large N: 512^3), an evaluation normally walks twice, COUNT then FILL.  From its second evaluation on the
+ * context instead sizes every group's list slots from the lengths the groups of the same region of the Morton curve had in the
+ * previous evaluation (plus a half) and walks once; a list that outgrows its slot makes the evaluation start over with COUNT + FILL
+ * (same results, the time of one walk lost) and the context sit out a few evaluations before predicting again.
+ * predicted: 1 if the last evaluation walked once into predicted slots and they held; retries: evaluations started over so far. */
+int dsk_get_walk_info(dsk_ctx *ctx, int *predicted, int64_t *retries);
+
 /* One BLOCK step of size da with hierarchical individual time steps (reading O9c of DESIGN.md; "adaptive
  * symplectic integrator (Quinn et al. 1997)").  rung dev uint8 [N], in/out: particle i takes steps of da / 2^rung[i],
  * 0 <= rung <= rmax <= 8 (a larger entry is read as rmax and written back clamped).  The block is cut into 2^rmax substeps; per substep: opening half kicks of the particles whose

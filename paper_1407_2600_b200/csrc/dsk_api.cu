@@ -63,6 +63,10 @@ static size_t carve(dsk_ctx *c, char *base)
     // give the one-pass walk ~20 per group (a group that needs more sends the evaluation to the two-pass form)
     c->list_left_cap = c->periodic ? n / 2 + (1u << 16) : 0;
     c->list_left = (uint4 *)take(16 * c->list_left_cap);
+    c->pg_key = (uint64_t *)take(8 * ng);
+    c->pg_m2p = (uint32_t *)take(4 * ng);
+    c->pg_p2p = (uint32_t *)take(4 * ng);
+    c->pg_left = (uint32_t *)take(4 * ng);
     c->frtab_beg = (uint32_t *)take(4 * DSK_FRTAB_BEG);
     c->frtab_ent = (void *)take(8 * DSK_FRTAB_ENT);
     c->gmark = (uint32_t *)take(4 * n);
@@ -164,7 +168,7 @@ extern "C" int dsk_bind_workspace(dsk_ctx *c, void *dev_ptr, size_t bytes)
     c->ws = (char *)dev_ptr;
     c->ws_bytes = bytes;
     carve(c, c->ws);
-    c->have_tree = 0; c->moments_p = -1; c->lists_valid = 0; c->kdk_have_acc = 0; c->frow_tab_p = -1; c->frow_tab_dip = -1;
+    c->have_tree = 0; c->moments_p = -1; c->lists_valid = 0; c->pg_valid = 0; c->kdk_have_acc = 0; c->frow_tab_p = -1; c->frow_tab_dip = -1;
     if (c->periodic)
         DSK_CUDA(cudaMemcpyAsync(c->far_T_dev, c->far_T, sizeof(double) * DSK_NFAR, cudaMemcpyHostToDevice, c->stream));
     DSK_CUDA(cudaMemsetAsync(c->dstate, 0, sizeof(dsk_devstate), c->stream));
@@ -184,6 +188,7 @@ extern "C" int dsk_set_params(dsk_ctx *c, float eps, float theta, int p)
     if (!c) return DSK_EINVAL;
     if (check_params(eps, theta, p)) return DSK_EINVAL;
     if (p > c->p_cap) return DSK_ENOWORKSPACE;        // rows were sized for dsk_create's p
+    if (eps != c->eps || theta != c->theta || p != c->p) c->pg_valid = 0;      // other lists: no prediction from the old ones (walk.cu)
     c->eps = eps; c->theta = theta; c->p = p;
     return DSK_OK;
 }
@@ -297,6 +302,15 @@ static int accel_impl(dsk_ctx *c, const uint8_t *active, float *acc, float *pot,
         if (e) { c->gact_cur = nullptr; return e; }
     }
     e = dsk_run_force(c, pot != nullptr);
+    if (e == DSK_RETRY_WALK) {                       // a list outgrew the slot predicted from the previous evaluation: COUNT + FILL after all
+        c->pg_valid = 0; c->lists_valid = 0;        // (P2P stores, M2P adds to it: starting over needs no clearing)
+        c->pg_retries++;
+        c->pg_backoff = c->pg_backoff >= 7 ? 15 : 2 * c->pg_backoff + 1;      // a tree that changes this fast: predict less often
+        c->pg_wait = c->pg_backoff;
+        e = dsk_run_walk(c);
+        if (e) { c->gact_cur = nullptr; return e; }
+        e = dsk_run_force(c, pot != nullptr);
+    }
     c->gact_cur = nullptr;
     if (active || shard_rank >= 0) c->lists_valid = 0;
     if (e) return e;
@@ -407,7 +421,7 @@ extern "C" int dsk_set_softening(dsk_ctx *c, int kind, float length)
 {
     if (!c || (kind != 0 && kind != 1) || !(length > 0.0f) || !isfinite(length)) return DSK_EINVAL;
     c->soft_kind = kind; c->eps = length;
-    c->lists_valid = 0; c->kdk_have_acc = 0;          // the K1 walk keeps cells out of the kernel's support: other lists
+    c->lists_valid = 0; c->pg_valid = 0; c->kdk_have_acc = 0;          // the K1 walk keeps cells out of the kernel's support: other lists
     return DSK_OK;
 }
 
@@ -416,7 +430,7 @@ extern "C" int dsk_set_mac(dsk_ctx *c, int kind, float tol)
     if (!c || (kind != 0 && kind != 1)) return DSK_EINVAL;
     if (kind == 1 && (!(tol > 0.0f) || !isfinite(tol))) return DSK_EINVAL;
     c->mac_kind = kind; c->mac_tol = kind == 1 ? tol : 0.0f;
-    c->lists_valid = 0; c->kdk_have_acc = 0;
+    c->lists_valid = 0; c->pg_valid = 0; c->kdk_have_acc = 0;
     return DSK_OK;
 }
 
@@ -430,7 +444,7 @@ extern "C" int dsk_set_image_block(dsk_ctx *c, int ws)
         DSK_CUDA(cudaMemcpyAsync(c->far_T_dev, c->far_T, sizeof(double) * DSK_NFAR, cudaMemcpyHostToDevice, c->stream));
         DSK_CUDA(cudaStreamSynchronize(c->stream));
     }
-    c->lists_valid = 0; c->kdk_have_acc = 0;
+    c->lists_valid = 0; c->pg_valid = 0; c->kdk_have_acc = 0;
     return DSK_OK;
 }
 
@@ -445,7 +459,7 @@ extern "C" int dsk_set_background(dsk_ctx *c, int on)
 {
     if (!c) return DSK_EINVAL;
     if (on && !c->periodic) return DSK_EINVAL;
-    if ((on != 0) != (c->bg != 0)) { c->moments_p = -1; c->lists_valid = 0; c->kdk_have_acc = 0; }   // rows and lists depend on it
+    if ((on != 0) != (c->bg != 0)) { c->moments_p = -1; c->lists_valid = 0; c->pg_valid = 0; c->kdk_have_acc = 0; }   // rows and lists depend on it
     if (c->bg_closed != (on == 2)) c->kdk_have_acc = 0;
     c->bg = on ? 1 : 0;
     c->bg_closed = on == 2;
@@ -487,7 +501,7 @@ extern "C" int dsk_set_walk_mode(dsk_ctx *c, int mode)
     if (!c || mode < 0 || mode > 4) return DSK_EINVAL;
     c->walk_two_pass_only = mode;
     c->onepass_bad_theta = -1.0f;
-    c->lists_valid = 0;
+    c->lists_valid = 0; c->pg_valid = 0;
     return DSK_OK;
 }
 
@@ -495,7 +509,15 @@ extern "C" int dsk_set_walk_sharing(dsk_ctx *c, int groups)
 {
     if (!c || groups < 0 || groups > 8) return DSK_EINVAL;
     c->walk_share = groups;
-    c->lists_valid = 0;
+    c->lists_valid = 0; c->pg_valid = 0;
+    return DSK_OK;
+}
+
+extern "C" int dsk_get_walk_info(dsk_ctx *c, int *predicted, int64_t *retries)
+{
+    if (!c) return DSK_EINVAL;
+    if (predicted) *predicted = c->walk_predicted;
+    if (retries) *retries = c->pg_retries;
     return DSK_OK;
 }
 

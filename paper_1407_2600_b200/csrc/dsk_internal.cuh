@@ -12,6 +12,7 @@
 #ifndef DSK_NCRIT
 #define DSK_NCRIT 192        // sink group: first cell from the root with count <= NCRIT (at most 4 tasks of 32 lanes x 2 sinks)
 #endif
+#define DSK_RETRY_WALK 1000            // internal: a predicted list slot overflowed (force.cu -> dsk_api.cu): evaluate again with COUNT + FILL
 #define DSK_SORT_TILE 2048               // keys per block and pass of the radix sort (keysort.cu)
 #define DSK_SORT_ONESWEEP_NMAX (1 << 22) // up to here the sort takes its one-kernel-per-pass form (keysort.cu): sizes its status words
 #define DSK_WS 2              // LARGEST image block half-width, and the one image ids are encoded for: id = ((ix+2) 5 + iy+2) 5 + iz+2.
@@ -197,6 +198,13 @@ struct dsk_ctx {
     float lists_theta;
     int walk_two_pass_only;   // dsk_set_walk_mode(1)
     int bg_closed;            // dsk_set_background(2): the windows' background by the closed form everywhere (diagnostic)
+    uint64_t *pg_key;         // [ngroup_cap] previous evaluation's groups: start of the Morton-key interval of the group's cell (walk.cu)
+    uint32_t *pg_m2p, *pg_p2p, *pg_left;      // ... and their list lengths
+    uint32_t pg_n;
+    int pg_valid;             // the remembered lengths belong to this context's current parameters
+    int64_t pg_retries;       // evaluations that started over because a predicted slot overflowed (dsk_get_walk_info)
+    int pg_backoff, pg_wait;  // after an overflow: evaluations to sit out before predicting again (1, 3, 7, 15; 0 after a success)
+    int walk_predicted;       // the offsets of the current evaluation are scanned PREDICTED capacities: fill with MODE 3, check the overflow flag
     int walk_share;           // dsk_set_walk_sharing: groups per shared walk (0 = automatic)
     int walk_onepass;         // the lists of the current evaluation were written by the one-pass walk
     float onepass_bad_theta;  // theta at which a list overflowed its fixed capacity (skip the one-pass attempt)
@@ -232,6 +240,7 @@ void dsk_exclusive_scan_u32(dsk_ctx *c, const uint32_t *in, uint32_t *out, const
 int dsk_run_build(dsk_ctx *c);                                                // tree.cu: T, G
 int dsk_run_upward(dsk_ctx *c);                                               // upward.cu: U
 int dsk_run_get_moments(dsk_ctx *c, float *com_mass, float *moments, int scaled);         // upward.cu
+int dsk_walk_remember(dsk_ctx *c);                                           // walk.cu: list lengths for the next evaluation
 int dsk_run_walk(dsk_ctx *c);                                                 // walk.cu: W
 int dsk_run_shard(dsk_ctx *c, int rank, int nranks, uint32_t flop_m2p, uint32_t flop_p2p, uint32_t *cut_host);   // walk.cu
 int dsk_run_force(dsk_ctx *c, int want_pot);                                  // force.cu: F1 + orchestration

@@ -267,6 +267,12 @@ static int eval_batch(dsk_ctx *c, uint32_t g0, uint32_t g1, uint32_t t0, uint32_
     if (fill) {
         int e = dsk_walk_fill(c, g0, g1, mb, pb, lb);
         if (e) return e;
+        if (c->walk_predicted) {             // slots sized from the previous evaluation (walk.cu): did every list fit?
+            unsigned long long ovf = 0;
+            DSK_CUDA(cudaMemcpyAsync(&ovf, &c->dstate->scratch[0], sizeof(ovf), cudaMemcpyDeviceToHost, s));
+            DSK_CUDA(cudaStreamSynchronize(s));
+            if (ovf) return DSK_RETRY_WALK;
+        }
     }
     cudaEventRecord(c->ev[8], s);
     const float e2 = c->eps * c->eps;
@@ -339,6 +345,7 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
     // reset the interaction counters (filled by the FILL pass)
     DSK_CUDA(cudaMemsetAsync(&c->dstate->tot_m2p_list, 0, sizeof(unsigned long long) * 5, s));
     DSK_CUDA(cudaMemsetAsync(&c->dstate->tot_left_list, 0, sizeof(unsigned long long), s));
+    DSK_CUDA(cudaMemsetAsync(&c->dstate->scratch[0], 0, sizeof(unsigned long long), s));          // overflow flag of a predicted fill
     // diagnostic modes 3 / 4 (dsk_set_walk_mode): pretend the list buffers are small (batches on small inputs) or tiny
     // (not even one group fits: DSK_ELISTOVERFLOW)
     const size_t cap_m = c->walk_two_pass_only == 3 ? (size_t)65536 : c->walk_two_pass_only == 4 ? (size_t)256 : c->list_m2p_cap;
@@ -349,7 +356,8 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
         if (e) return e;
         c->pending_force_ms = 2;
         c->stats.nbatch = 1;
-        c->lists_valid = 1; c->lists_theta = c->theta;
+        c->lists_valid = !c->walk_predicted; c->lists_theta = c->theta;      // (predicted slots are not tight: the cached-list path assumes nothing about that, but keep it simple)
+        if (!c->gact_cur) dsk_walk_remember(c);
         return DSK_OK;
     }
     // batches: cut the group range where a list would overflow.  The cut is found on the device (binary search over the three
@@ -375,6 +383,7 @@ int dsk_run_force(dsk_ctx *c, int want_pot)
         g0 = g1; nb++;
     }
     DSK_COUNT(c, nb);
+    if (rc == DSK_OK && !c->gact_cur) dsk_walk_remember(c);
     c->stats.nbatch = nb;
     c->lists_valid = 0;
     return rc;

@@ -140,7 +140,8 @@ __device__ __forceinline__ float wk_d2(float zx, float zy, float zz, const float
 
 // THE LONE WALK: one warp per group.
 #define WW 1                 // warps (groups) per block: walks differ in length, a block ends with its longest
-template <int MODE, bool ABS>          // MODE 0 COUNT, 1 FILL at the scanned offsets, 2 ONE pass into a fixed capacity per group
+template <int MODE, bool ABS>          // MODE 0 COUNT, 1 FILL at the scanned offsets, 2 ONE pass into a fixed capacity per group,
+                                       // 3 ONE pass into PREDICTED capacities: the offsets are scanned capacities (dsk_run_walk), lengths are written
 __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int periodic, float box, int pow1, float k1_h,
                                                   const dsk_cellrec *__restrict__ cell,
                                                   const float4 *__restrict__ wmac,
@@ -213,8 +214,13 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
     __syncwarp();
     uint32_t nm = 0, np = 0, nsrc = 0, nl = 0;
     uint64_t mo = 0, po = 0, lo_ = 0;
-    if (MODE == 1) { mo = m2p_off[g] - m2p_base; po = p2p_off[g] - p2p_base; if (BG) lo_ = bg.left_off[g] - bg.left_base; }
-    if (MODE == 2) { mo = (uint64_t)g * cap_m; po = (uint64_t)g * cap_p; if (BG) lo_ = (uint64_t)g * bg.cap_l; }
+    uint32_t lim_m = 0xffffffffu, lim_p = 0xffffffffu, lim_l = 0xffffffffu;          // what the group's list slots hold
+    if (MODE == 1 || MODE == 3) { mo = m2p_off[g] - m2p_base; po = p2p_off[g] - p2p_base; if (BG) lo_ = bg.left_off[g] - bg.left_base; }
+    if (MODE == 2) { mo = (uint64_t)g * cap_m; po = (uint64_t)g * cap_p; if (BG) lo_ = (uint64_t)g * bg.cap_l; lim_m = cap_m; lim_p = cap_p; lim_l = bg.cap_l; }
+    if (MODE == 3) {
+        lim_m = (uint32_t)(m2p_off[g + 1] - m2p_off[g]); lim_p = (uint32_t)(p2p_off[g + 1] - p2p_off[g]);
+        if (BG) lim_l = (uint32_t)(bg.left_off[g + 1] - bg.left_off[g]);
+    }
     const uint32_t lt = (1u << lane) - 1u;
     // WEPL stack entries per lane and trip: their loads are independent, so a trip exposes one L2 round trip for
     // 32 * WEPL cells
@@ -294,8 +300,8 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
             const uint32_t bl = __ballot_sync(0xffffffffu, leaf[q]);
             if (FILL) {
                 const uint32_t im = nm + __popc(bm & lt), ip = np + __popc(bl & lt);
-                if (accept[q] && (MODE == 1 || im < cap_m)) list_m2p[mo + im] = entry;
-                if (leaf[q] && (MODE == 1 || ip < cap_p)) list_p2p[po + ip] = e[q];
+                if (accept[q] && (MODE == 1 || im < lim_m)) list_m2p[mo + im] = entry;
+                if (leaf[q] && (MODE == 1 || ip < lim_p)) list_p2p[po + ip] = e[q];
             }
             nm += __popc(bm); np += __popc(bl);
             if (leaf[q]) nsrc += cnt;
@@ -306,7 +312,7 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
                     if (lane >= o) x += y;
                 }
                 const uint32_t tot = __shfl_sync(0xffffffffu, x, 31), at = nl + x - nexp;
-                if (FILL && nexp && (MODE == 1 || at + nexp <= bg.cap_l))
+                if (FILL && nexp && (MODE == 1 || at + nexp <= lim_l))
                     wk_exposed(whole, geo[q].w & 255, bg.lb, geo[q], ish, wlo, whi, bg.list_left + lo_ + at);
                 nl += tot;
             }
@@ -344,8 +350,9 @@ __global__ void __launch_bounds__(WW * 32) k_walk(uint32_t g0, uint32_t g1, int 
         if (MODE == 2) {
             m2p_off_out[g] = (uint64_t)g * cap_m; p2p_off_out[g] = (uint64_t)g * cap_p;
             if (BG) bg.left_off_out[g] = (uint64_t)g * bg.cap_l;
-            if (nm > cap_m || np > cap_p || (BG && nl > bg.cap_l)) st->scratch[0] = 1ull;      // a list did not fit: the host falls back to two passes
         }
+        if (MODE >= 2 && (nm > lim_m || np > lim_p || (BG && nl > lim_l)))      // a list did not fit: the host falls back to two passes
+            atomicOr(&st->scratch[0], (nm > lim_m ? 1ull : 0ull) | (np > lim_p ? 2ull : 0ull) | (BG && nl > lim_l ? 4ull : 0ull));
         if (FILL) {
             const unsigned long long ns = gcount[g];
             atomicAdd(&st->n_m2p, ns * nm);
@@ -843,14 +850,72 @@ static void launch_walk(dsk_ctx *c, uint32_t g0, uint32_t g1, const uint64_t *m2
     const bool ABS = c->mac_kind == 1;
     const int sgn = walk_sgn(c), per = c->periodic ? c->img_ws : 0, pow1 = c->p + 1;
     const float k1_h = c->soft_kind == 1 ? c->eps : 0.0f;
-    if (sgn > 1)
-        (ABS ? k_walk_sh<MODE, true> : k_walk_sh<MODE, false>)<<<walk_grid(g0, g1, sgn), 32, 0, c->stream>>>(
-            g0, g1, c->hstate->ngroup, sgn, per, c->box, pow1, k1_h, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len, c->g_p2p_src,
-            m2p_off, p2p_off, m2p_base, p2p_base, list_m2p, list_p2p, gact, cap_m, cap_p, m2p_off_out, p2p_off_out, bg, c->dstate);
-    else
+    if constexpr (MODE != 3) {          // (predicted capacities are a lone-walk form: dsk_run_walk does not predict when groups share)
+        if (sgn > 1) {
+            (ABS ? k_walk_sh<MODE, true> : k_walk_sh<MODE, false>)<<<walk_grid(g0, g1, sgn), 32, 0, c->stream>>>(
+                g0, g1, c->hstate->ngroup, sgn, per, c->box, pow1, k1_h, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len, c->g_p2p_src,
+                m2p_off, p2p_off, m2p_base, p2p_base, list_m2p, list_p2p, gact, cap_m, cap_p, m2p_off_out, p2p_off_out, bg, c->dstate);
+            return;
+        }
+    }
+    {
         (ABS ? k_walk<MODE, true> : k_walk<MODE, false>)<<<(g1 - g0 + WW - 1) / WW, WW * 32, 0, c->stream>>>(
             g0, g1, per, c->box, pow1, k1_h, c->cell, c->wmac, c->gbox, c->gcount, c->g_m2p_len, c->g_p2p_len, c->g_p2p_src,
             m2p_off, p2p_off, m2p_base, p2p_base, list_m2p, list_p2p, gact, cap_m, cap_p, m2p_off_out, p2p_off_out, bg, c->dstate);
+    }
+}
+
+// ---- list lengths predicted from the previous evaluation ---------------------------------------------------------------------------
+// When the lists do not fit a fixed capacity per group (512^3: 3.4 M groups, lists of 1500 cells on average and 2800 at most against a
+// 12 GiB buffer), the walk runs twice, COUNT and FILL: 2 x 28 ms of a dsk_kdk_step.  From one step to the next the tree hardly changes, so
+// the second evaluation onwards sizes every group's slots from the lengths the groups of the SAME REGION had last time: a group is a tree
+// cell, i.e. an interval of Morton keys; the old groups' interval starts are kept sorted (they are in Morton order), a new group takes the
+// largest old length among the old groups its interval meets, plus a half and 128 entries (cells; twice + 64 for the leaves).  One walk
+// (MODE 3) fills the slots and writes the true lengths; a list that outgrew its slot sets the overflow flag and the evaluation starts
+// over with COUNT + FILL, and the context then sits out 1, 3, 7, 15 evaluations before it predicts again.  Measured on C5 (a synthetic
+// box far from equilibrium: the number of groups falls 3.47 -> 3.07 -> 2.67 -> 2.60 M over the first steps): no overflow from the
+// second step on, 1351 -> 1319 ms per step; with margins of a quarter + 96 / 32 a slot overflowed in every step (then 1382 ms).
+__device__ __forceinline__ uint64_t pg_interval(uint32_t cg, const dsk_cellrec *__restrict__ cell, const uint64_t *__restrict__ hotkey, uint64_t *hi)
+{
+    const int l = (int)(cell[cg].meta >> 8), sh = 3 * (DSK_KEY_LEVELS - l);
+    const uint64_t prefix = hotkey[cg] & ~(1ull << (3 * l));
+    const uint64_t lo = prefix << sh;
+    *hi = lo + (1ull << sh);
+    return lo;
+}
+__global__ void __launch_bounds__(256) k_pg_store(uint32_t ng, const uint32_t *__restrict__ gcell, const dsk_cellrec *__restrict__ cell,
+                                                  const uint64_t *__restrict__ hotkey, const uint32_t *__restrict__ m2p_len,
+                                                  const uint32_t *__restrict__ p2p_len, const uint32_t *__restrict__ left_len,
+                                                  uint64_t *__restrict__ pg_key, uint32_t *__restrict__ pg_m2p, uint32_t *__restrict__ pg_p2p,
+                                                  uint32_t *__restrict__ pg_left)
+{
+    const uint32_t g = blockIdx.x * 256 + threadIdx.x;
+    if (g >= ng) return;
+    uint64_t hi;
+    pg_key[g] = pg_interval(gcell[g], cell, hotkey, &hi);
+    pg_m2p[g] = m2p_len[g]; pg_p2p[g] = p2p_len[g]; pg_left[g] = left_len ? left_len[g] : 0u;
+}
+__global__ void __launch_bounds__(256) k_pg_predict(uint32_t ng, const uint32_t *__restrict__ gcell, const dsk_cellrec *__restrict__ cell,
+                                                    const uint64_t *__restrict__ hotkey, uint32_t pg_n, const uint64_t *__restrict__ pg_key,
+                                                    const uint32_t *__restrict__ pg_m2p, const uint32_t *__restrict__ pg_p2p,
+                                                    const uint32_t *__restrict__ pg_left, uint32_t *__restrict__ cap_m,
+                                                    uint32_t *__restrict__ cap_p, uint32_t *__restrict__ cap_l)
+{
+    const uint32_t g = blockIdx.x * 256 + threadIdx.x;
+    if (g >= ng) return;
+    uint64_t hi;
+    const uint64_t lo = pg_interval(gcell[g], cell, hotkey, &hi);
+    uint32_t a = 0, b = pg_n;                        // last old group whose interval starts at or before lo (or the first)
+    while (b - a > 1) {
+        const uint32_t mid = a + ((b - a) >> 1);
+        if (pg_key[mid] <= lo) a = mid; else b = mid;
+    }
+    uint32_t m = 0, p = 0, l = 0;
+    for (uint32_t j = a, k = 0; j < pg_n && k < 64 && (k < 2 || pg_key[j] < hi); j++, k++) {       // it, its successor, and all that start inside
+        m = max(m, pg_m2p[j]); p = max(p, pg_p2p[j]); l = max(l, pg_left[j]);
+    }
+    cap_m[g] = m + (m >> 1) + 128u; cap_p[g] = 2u * p + 64u;
+    if (cap_l) cap_l[g] = 2u * l + 16u;
 }
 
 // W.  First choice: ONE pass into a fixed capacity per group (list buffer / number of groups), which saves the COUNT
@@ -887,7 +952,15 @@ int dsk_run_walk(dsk_ctx *c)
         if (!ovf) { c->walk_onepass = 1; return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA; }
         c->onepass_bad_theta = c->theta;
     }
-    launch_walk<0>(c, 0, ng, nullptr, nullptr, 0, 0, nullptr, nullptr, c->gact_cur, 0, 0, nullptr, nullptr, make_walk_bg(c, 0, 0));
+    c->walk_predicted = 0;
+    if (c->pg_valid && c->pg_n > 0 && !c->gact_cur && walk_sgn(c) == 1 && c->walk_two_pass_only != 1 && ng > 0) {
+        // no COUNT pass: slots sized from the previous evaluation's lengths (above); dsk_run_force fills them with MODE 3
+        k_pg_predict<<<(ng + 255) / 256, 256, 0, s>>>(ng, c->gcell, c->cell, c->hotkey, c->pg_n, c->pg_key, c->pg_m2p, c->pg_p2p, c->pg_left,
+                                                      c->g_m2p_len, c->g_p2p_len, BG ? c->g_left_len : nullptr);
+        c->walk_predicted = 1;
+    } else {
+        launch_walk<0>(c, 0, ng, nullptr, nullptr, 0, 0, nullptr, nullptr, c->gact_cur, 0, 0, nullptr, nullptr, make_walk_bg(c, 0, 0));
+    }
     scan64(c, c->g_m2p_len, ng, c->g_m2p_off);
     scan64(c, c->g_p2p_len, ng, c->g_p2p_off);
     if (BG) scan64(c, c->g_left_len, ng, c->g_left_off);
@@ -895,10 +968,31 @@ int dsk_run_walk(dsk_ctx *c)
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }
 
+// after an evaluation in the two-pass regime: remember every group's key interval and list lengths for the next one
+int dsk_walk_remember(dsk_ctx *c)
+{
+    const uint32_t ng = c->hstate->ngroup;
+    c->pg_valid = 0;
+    if (!ng || (int64_t)ng > c->ngroup_cap) return DSK_OK;
+    const bool BG = c->periodic && c->bg;
+    k_pg_store<<<(ng + 255) / 256, 256, 0, c->stream>>>(ng, c->gcell, c->cell, c->hotkey, c->g_m2p_len, c->g_p2p_len, BG ? c->g_left_len : nullptr,
+                                                        c->pg_key, c->pg_m2p, c->pg_p2p, c->pg_left);
+    DSK_COUNT(c, 1);
+    c->pg_n = ng;
+    if (c->walk_predicted) c->pg_backoff = 0;        // the prediction held
+    if (c->pg_wait > 0) c->pg_wait--;               // sitting out after an overflow (dsk_api.cu)
+    else c->pg_valid = 1;
+    return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
+}
+
 int dsk_walk_fill(dsk_ctx *c, uint32_t g0, uint32_t g1, uint64_t m2p_base, uint64_t p2p_base, uint64_t left_base)
 {
-    launch_walk<1>(c, g0, g1, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p, c->gact_cur, 0, 0, nullptr, nullptr,
-                   make_walk_bg(c, left_base, 0));
+    if (c->walk_predicted)
+        launch_walk<3>(c, g0, g1, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p, c->gact_cur, 0, 0, nullptr, nullptr,
+                       make_walk_bg(c, left_base, 0));
+    else
+        launch_walk<1>(c, g0, g1, c->g_m2p_off, c->g_p2p_off, m2p_base, p2p_base, c->list_m2p, c->list_p2p, c->gact_cur, 0, 0, nullptr, nullptr,
+                       make_walk_bg(c, left_base, 0));
     DSK_COUNT(c, 1);
     return cudaGetLastError() == cudaSuccess ? DSK_OK : DSK_ECUDA;
 }

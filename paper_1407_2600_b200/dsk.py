@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libdsk.so")
 
 SYMBOLS = [
     "dsk_create", "dsk_destroy", "dsk_workspace_bytes", "dsk_bind_workspace", "dsk_set_stream",
-    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_accel_shard", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_set_walk_sharing", "dsk_set_background", "dsk_get_background", "dsk_set_image_block", "dsk_get_image_block", "dsk_set_mac", "dsk_set_softening", "dsk_get_bg_moments", "dsk_get_keys",
+    "dsk_set_params", "dsk_build_tree", "dsk_accel", "dsk_accel_active", "dsk_accel_shard", "dsk_kdk_step", "dsk_kdk_block_step", "dsk_kdk_reset", "dsk_set_cosmology", "dsk_set_walk_mode", "dsk_set_walk_sharing", "dsk_get_walk_info", "dsk_set_background", "dsk_get_background", "dsk_set_image_block", "dsk_get_image_block", "dsk_set_mac", "dsk_set_softening", "dsk_get_bg_moments", "dsk_get_keys",
     "dsk_get_tree", "dsk_get_moments", "dsk_get_moments_scaled", "dsk_get_groups", "dsk_get_stats", "dsk_get_param", "dsk_get_task_widths",
     "dsk_get_lattice_tensors", "dsk_probe_fp32_peak", "dsk_probe_fp32_peak_ex", "dsk_sort_keys_noalloc", "dsk_strerror",
 ]
@@ -65,6 +65,7 @@ def load_library(path=LIB_PATH):
     lib.dsk_kdk_reset.argtypes = [vp]
     lib.dsk_set_walk_mode.argtypes = [vp, i32]
     lib.dsk_set_walk_sharing.argtypes = [vp, i32]
+    lib.dsk_get_walk_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64)]
     lib.dsk_set_background.argtypes = [vp, i32]
     lib.dsk_set_mac.argtypes = [vp, i32, f32]
     lib.dsk_set_softening.argtypes = [vp, i32, f32]
@@ -289,6 +290,12 @@ class Dsk:
 
     def set_walk_sharing(self, groups):
         _check(self.lib.dsk_set_walk_sharing(self._h, int(groups)))
+
+    def get_walk_info(self):
+        """(the last evaluation walked once into slots predicted from the previous one, evaluations started over so far)"""
+        pr, rt = C.c_int(0), C.c_int64(0)
+        _check(self.lib.dsk_get_walk_info(self._h, C.byref(pr), C.byref(rt)))
+        return bool(pr.value), rt.value
 
     def set_cosmology(self, omega_m, omega_lambda):
         _check(self.lib.dsk_set_cosmology(self._h, float(omega_m), float(omega_lambda)))

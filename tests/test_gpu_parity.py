@@ -491,6 +491,66 @@ def test_walk_batches_equal_one_batch(dsk, periodic, share):
     d.close()
 
 
+@pytest.mark.parametrize("periodic", [False, True])
+def test_walk_predicted_list_slots(dsk, periodic):
+    """In the two-pass regime (here forced by dsk_set_walk_mode(3): small pretended list buffers, batches) the second evaluation
+    onwards sizes every group's list slots from the lengths the groups of the same region had in the previous evaluation and walks
+    once (walk.cu, MODE 3) instead of COUNT + FILL.  Same lists: bit-identical forces on the same tree, over a chain of KDK steps
+    against the default regime, and - when the particles are replaced by others, so that the remembered lengths are wrong and a slot
+    overflows - after the fallback to COUNT + FILL."""
+    pos, mass = (workloads.clustered_box(24, 20, cfg=4) if periodic else workloads.make(2, 1 / 16))
+    n = len(pos)
+    tp, tm = _dev(pos), _dev(mass)
+    ref = dsk.Dsk(n, 1.0, periodic, 1e-3, 0.5, 4)
+    ref.build_tree(tp, tm)
+    a0, p0 = ref.accel(tp, tm)
+    s0 = ref.get_stats()
+    d = dsk.Dsk(n, 1.0, periodic, 1e-3, 0.5, 4)
+    d.set_walk_mode(3)
+    for it in range(3):                                   # COUNT + FILL, then twice with predicted slots
+        d.build_tree(tp, tm)
+        a, ph = d.accel(tp, tm)
+        st = d.get_stats()
+        assert torch.equal(a, a0) and torch.equal(ph, p0), it
+        assert st["nbatch"] > 1 and st["n_m2p"] == s0["n_m2p"] and st["n_p2p"] == s0["n_p2p"] and st["list_m2p"] == s0["list_m2p"], it
+        assert d.get_walk_info() == (it > 0, 0), (it, d.get_walk_info())          # predicted from the second evaluation on, no retry
+    # a chain of steps: the tree changes a little every step
+    vel = (np.random.default_rng(2).standard_normal((n, 3)) * 0.02).astype(np.float32)
+    x1, v1 = tp.clone(), _dev(vel)
+    x2, v2 = tp.clone(), _dev(vel)
+    ref.kdk_reset(); d.kdk_reset()
+    da = 0.01 if periodic else 1e-5                      # (the Plummer core is stiff: a small step keeps everyone in the box)
+    for k in range(5):
+        ref.kdk_step(x1, v1, tm, 0.5 + da * k, da)
+        d.kdk_step(x2, v2, tm, 0.5 + da * k, da)
+        assert torch.equal(x1, x2) and torch.equal(v1, v2), k
+    assert d.get_walk_info() == (True, 0) and ref.get_walk_info() == (False, 0)      # the slots held through the chain; the default regime never predicts
+    # other particles in the same context: two points, every particle on one of them - lists of a few entries; then the first set again,
+    # whose lists are a hundred times longer than the slots sized from those: overflow, COUNT + FILL, the same forces
+    two = np.tile(np.array([[0.25, 0.25, 0.25]], np.float32), (n, 1)); two[::2] = [0.75, 0.7, 0.8]
+    to = _dev(two)
+    ref.build_tree(to, tm); b0, q0 = ref.accel(to, tm)
+    d.build_tree(to, tm); b, q = d.accel(to, tm)
+    assert torch.equal(b, b0) and torch.equal(q, q0)
+    r0 = d.get_walk_info()[1]
+    d.build_tree(to, tm); d.accel(to, tm)                  # (remembered whatever the evaluation before did)
+    d.build_tree(tp, tm); a, ph = d.accel(tp, tm)
+    assert torch.equal(a, a0) and torch.equal(ph, p0)
+    assert d.get_walk_info() == (False, r0 + 1)           # a slot overflowed: started over with COUNT + FILL
+    sat_out = 0                                           # it sits out 1 (first overflow) or 3 (second in a row) evaluations ...
+    while True:
+        d.build_tree(tp, tm); a, ph = d.accel(tp, tm)
+        assert torch.equal(a, a0) and torch.equal(ph, p0)
+        pred, retries = d.get_walk_info()
+        assert retries == r0 + 1
+        if pred:
+            break                                         # ... and predicts again
+        sat_out += 1
+        assert sat_out <= 3
+    assert sat_out in (1, 3)
+    ref.close(); d.close()
+
+
 SHARED_WALK_CASES = {
     "plummer": (lambda: workloads.make(2, 1 / 16), False, 1e-3, 0.5, 4, {}),
     "plummer-theta0.3": (lambda: workloads.make(2, 1 / 8), False, 1e-4, 0.3, 2, {}),
